@@ -1,0 +1,773 @@
+/*
+ * lisa_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, step-by-step CPU implementation of the time-domain LISA response
+ * of arXiv 2505.09600 (Valencia & Husa): full response, low-frequency
+ * approximation (LFA) and hybrid.  Written from the paper ("P:n" = line n of
+ * /root/reference/PAPER.md) with the readings listed in DESIGN.md ("G1".."G23",
+ * SURVEY.md section 8c).  It shares no code, header, table or constant generator
+ * with the CUDA path under paper_2505_09600_b200/csrc, and neither imports the
+ * other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.
+ *
+ * The same source is compiled twice (oracle/build.py):
+ *   -DORC_REAL_LD  : real = long double (x87 80 bit) -> the parity reference
+ *   (default)      : real = double                  -> timed baseline, fp64 floor
+ * Inputs and outputs are always IEEE double arrays; only the arithmetic in
+ * between changes.  No blocking, fusion or reordering: every function follows
+ * the cited equation in the paper's order.  OpenMP only splits the outermost
+ * loop over output samples / sources, which are independent.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): Lagrange exactness on
+ * polynomials, weights sum to 1, integer delay = pure shift; stencil exactness
+ * on polynomials; orthonormal triad; rigid-triangle orbit, |R_i| = R(1 +- e),
+ * Sagnac amplitude of Eq. (B22); constant strain -> zero response;
+ * monochromatic plane-wave closed form on a frozen constellation (Eq. C3);
+ * X_2.0[n] = X_1.5[n] - X_1.5[n - 4L/(c dt)] for static equal arms; Eq. (3.7)
+ * low-frequency relation; LFA -> full as f L / c -> 0 with the x / sin x law of
+ * Eq. (B4); T^LFA = 0 for equal arms; psi invariances; Eq. (4.2)/(4.4) printed
+ * values 0.95 / 0.97 / 0.99; taper partition of unity.
+ * Parity unpinned: absolute amplitudes of the paper's figures (no printed
+ * input -> output example exists in the paper).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORC_REAL_LD
+typedef long double real;
+#define R_SIN sinl
+#define R_COS cosl
+#define R_SQRT sqrtl
+#define R_CEIL ceill
+#define R_EXP expl
+#define R_POW powl
+#define R_PI 3.14159265358979323846264338327950288L
+#else
+typedef double real;
+#define R_SIN sin
+#define R_COS cos
+#define R_SQRT sqrt
+#define R_CEIL ceil
+#define R_EXP exp
+#define R_POW pow
+#define R_PI 3.14159265358979323846
+#endif
+
+#define ORC_OK 0
+#define ORC_EINVAL (-1)
+
+#define ORC_C_LIGHT 299792458.0 /* m/s, exact (SI) */
+
+enum { ORC_GEN_15 = 15, ORC_GEN_20 = 20 };
+enum { ORC_ORBIT_STATIC_EQUALARM = 0, ORC_ORBIT_KEPLERIAN = 1, ORC_ORBIT_TABLES = 2 };
+enum { ORC_TAPER_SIGMOID = 0, ORC_TAPER_COSINE = 1 };
+
+typedef struct {
+    double t0, dt;   /* t_n = t0 + n dt [s] */
+    int64_t n;       /* samples */
+    double arm_m;    /* nominal arm length L [m] */
+    double R_m;      /* orbital radius R [m] */
+    double period_s; /* orbital period [s], Omega = 2 pi / period */
+    double alpha0;   /* orbital phase at t = 0 [rad] */
+    double rot0;     /* constellation rotation phase [rad] */
+    int32_t mode;    /* ORC_ORBIT_* */
+} orc_orbit_desc;
+
+typedef struct { double beta, lambda, psi; } orc_source;
+typedef struct { double t_hyb, window_s, sigma_s; int32_t taper; } orc_hybrid;
+
+/* Links: index 0..5 = l = +1,+2,+3,-1,-2,-3 ; y_{s l r}: sender s -> receiver r.
+ * +1: 3->2 (y_312)  +2: 1->3 (y_123)  +3: 2->1 (y_231)
+ * -1: 2->3 (y_2-13) -2: 3->1 (y_3-21) -3: 1->2 (y_1-32)      spacecraft 0-based below */
+static const int LINK_S[6] = { 2, 0, 1, 1, 2, 0 };
+static const int LINK_R[6] = { 1, 2, 0, 2, 0, 1 };
+
+static int link_index(int label) /* label in {+-1,+-2,+-3} -> 0..5 */
+{
+    return label > 0 ? label - 1 : 2 - label;
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O4  Lagrange fractional-delay interpolation (reading G10)                */
+/* ---------------------------------------------------------------------------------- */
+
+/* w_k(eps) = prod_{m != k} (eps - m) / (k - m),  k, m = -(M/2-1) .. M/2,  M = order+1 */
+static void lagrange_weights(real eps, int order, real *w)
+{
+    const int M = order + 1, kmin = -(M / 2 - 1), kmax = M / 2;
+    for (int k = kmin; k <= kmax; ++k) {
+        real num = 1, den = 1;
+        for (int m = kmin; m <= kmax; ++m) {
+            if (m == k) continue;
+            num *= (eps - (real)m);
+            den *= (real)(k - m);
+        }
+        w[k - kmin] = num / den;
+    }
+}
+
+/* split a delay d [s] into the integer shift q = ceil(d/dt) and eps = q - d/dt in [0,1).
+ * Only the small quantity d/dt enters, never the absolute time. */
+static void delay_split(real d, real dt, int64_t *q, real *eps)
+{
+    const real s = d / dt;
+    const real qc = R_CEIL(s);
+    *q = (int64_t)qc;
+    *eps = qc - s;
+}
+
+/* value of the series x (length len, first element = absolute sample x0) at t_n - d.
+ * Samples outside [x0, x0+len) read as 0 (they are only touched inside margins). */
+static real interp_series(const real *x, int64_t x0, int64_t len, int64_t n, real d, real dt,
+                          int order)
+{
+    real w[64];
+    int64_t q;
+    real eps;
+    const int M = order + 1, kmin = -(M / 2 - 1);
+    delay_split(d, dt, &q, &eps);
+    lagrange_weights(eps, order, w);
+    const int64_t j = n - q;
+    real acc = 0;
+    for (int i = 0; i < M; ++i) {
+        const int64_t idx = j + kmin + i - x0;
+        const real v = (idx >= 0 && idx < len) ? x[idx] : (real)0;
+        acc += w[i] * v;
+    }
+    return acc;
+}
+
+/* same, reading a double array (the input strain) */
+static real interp_input(const double *x, int64_t len, int64_t n, real d, real dt, int order)
+{
+    real w[64];
+    int64_t q;
+    real eps;
+    const int M = order + 1, kmin = -(M / 2 - 1);
+    delay_split(d, dt, &q, &eps);
+    lagrange_weights(eps, order, w);
+    const int64_t j = n - q;
+    real acc = 0;
+    for (int i = 0; i < M; ++i) {
+        const int64_t idx = j + kmin + i;
+        const real v = (idx >= 0 && idx < len) ? (real)x[idx] : (real)0;
+        acc += w[i] * v;
+    }
+    return acc;
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O8 stencils (reading G15): central differences of accuracy order 2 / 4             */
+/* ---------------------------------------------------------------------------------- */
+#define AT(x, i) ((real)(x)[(i)])
+
+static real fd1_in(const double *x, int64_t i, real dt, int fd_order)
+{
+    if (fd_order == 2) return (AT(x, i + 1) - AT(x, i - 1)) / (2 * dt);
+    return (8 * (AT(x, i + 1) - AT(x, i - 1)) - (AT(x, i + 2) - AT(x, i - 2))) / (12 * dt);
+}
+static real fd1_r(const real *x, int64_t i, real dt, int fd_order)
+{
+    if (fd_order == 2) return (x[i + 1] - x[i - 1]) / (2 * dt);
+    return (8 * (x[i + 1] - x[i - 1]) - (x[i + 2] - x[i - 2])) / (12 * dt);
+}
+static real fd2_r(const real *x, int64_t i, real dt, int fd_order)
+{
+    const real d1 = (x[i + 1] - x[i]) - (x[i] - x[i - 1]);
+    if (fd_order == 2) return d1 / (dt * dt);
+    const real d2 = (x[i + 2] - x[i]) - (x[i] - x[i - 2]);
+    return (16 * d1 - d2) / (12 * dt * dt);
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O1  orbits (readings G5, G6, G7): first-order Keplerian, rigid rotating triangle   */
+/* ---------------------------------------------------------------------------------- */
+typedef struct {
+    orc_orbit_desc d;
+    const double *Rtab; /* mode TABLES: [3][3][n] spacecraft, component, sample [m] */
+    const double *Ltab; /* mode TABLES: [6][n] light travel times [s], link order +1,+2,+3,-1,-2,-3 */
+} orbit_ctx;
+
+typedef struct {
+    real R[3][3];  /* spacecraft positions [m] */
+    real nh[6][3]; /* link unit vectors, sender -> receiver (G7) */
+    real L[6];     /* light travel times [s] */
+} geom_t;
+
+static void orbit_geometry(const orbit_ctx *o, int64_t n, geom_t *g)
+{
+    const real c = ORC_C_LIGHT;
+    real V[3][3] = { { 0 } };
+    if (o->d.mode == ORC_ORBIT_TABLES) {
+        for (int i = 0; i < 3; ++i)
+            for (int a = 0; a < 3; ++a) g->R[i][a] = (real)o->Rtab[(int64_t)(i * 3 + a) * o->d.n + n];
+    } else {
+        const real t = (real)o->d.t0 + (real)n * (real)o->d.dt;
+        const real R = o->d.R_m, L = o->d.arm_m;
+        const real adot = 2 * R_PI / (real)o->d.period_s;
+        const real alpha = adot * t + (real)o->d.alpha0;
+        const real e = L / (2 * R_SQRT((real)3) * R);
+        for (int i = 0; i < 3; ++i) {
+            const real b = 2 * R_PI * (real)i / 3 + (real)o->d.rot0;
+            g->R[i][0] = R * R_COS(alpha) + (real)0.5 * e * R * (R_COS(2 * alpha - b) - 3 * R_COS(b));
+            g->R[i][1] = R * R_SIN(alpha) + (real)0.5 * e * R * (R_SIN(2 * alpha - b) - 3 * R_SIN(b));
+            g->R[i][2] = -R_SQRT((real)3) * e * R * R_COS(alpha - b);
+            V[i][0] = -R * adot * R_SIN(alpha) - e * R * adot * R_SIN(2 * alpha - b);
+            V[i][1] = R * adot * R_COS(alpha) + e * R * adot * R_COS(2 * alpha - b);
+            V[i][2] = R_SQRT((real)3) * e * R * adot * R_SIN(alpha - b);
+        }
+    }
+    for (int l = 0; l < 6; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real dvec[3], len2 = 0;
+        for (int a = 0; a < 3; ++a) {
+            dvec[a] = g->R[r][a] - g->R[s][a]; /* L_l n_l ~ R_r - R_s */
+            len2 += dvec[a] * dvec[a];
+        }
+        const real len = R_SQRT(len2);
+        for (int a = 0; a < 3; ++a) g->nh[l][a] = dvec[a] / len;
+        if (o->d.mode == ORC_ORBIT_STATIC_EQUALARM) {
+            g->L[l] = (real)o->d.arm_m / c; /* "equal and constant" delays */
+        } else if (o->d.mode == ORC_ORBIT_KEPLERIAN) {
+            /* first-order light time: L_l != L_-l through the sender velocity (B22) */
+            real nv = 0;
+            for (int a = 0; a < 3; ++a) nv += g->nh[l][a] * V[s][a];
+            g->L[l] = (len / c) * (1 + nv / c);
+        } else {
+            g->L[l] = (real)o->Ltab[(int64_t)l * o->d.n + n];
+        }
+    }
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O2  source frame, Eq. (2.1) with reading G1; O3 antenna patterns (2.2)-(2.4)        */
+/* ---------------------------------------------------------------------------------- */
+typedef struct { real k[3], u[3], v[3], c2, s2; } frame_t;
+
+static void source_frame(const orc_source *s, frame_t *f)
+{
+    const real b = s->beta, l = s->lambda, p = s->psi;
+    f->k[0] = -R_COS(b) * R_COS(l); f->k[1] = -R_COS(b) * R_SIN(l); f->k[2] = -R_SIN(b); /* -e_r     */
+    f->u[0] = R_SIN(l);             f->u[1] = -R_COS(l);            f->u[2] = 0;         /* -e_phi   */
+    f->v[0] = -R_SIN(b) * R_COS(l); f->v[1] = -R_SIN(b) * R_SIN(l); f->v[2] = R_COS(b);  /* -e_theta */
+    f->c2 = R_COS(2 * p);
+    f->s2 = R_SIN(2 * p);
+}
+
+static real dot3(const real *a, const real *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+/* F^+_l, F^x_l such that H_l = F^+ h_+ + F^x h_x  ( = xi^+ h^SSB_+ + xi^x h^SSB_x, (2.2)+(2.3), G17 ) */
+static void antenna(const frame_t *f, const real *nh, real *Fp, real *Fc)
+{
+    const real un = dot3(f->u, nh), vn = dot3(f->v, nh);
+    const real xip = un * un - vn * vn; /* (2.4a) */
+    const real xic = 2 * un * vn;       /* (2.4b) */
+    *Fp = xip * f->c2 + xic * f->s2;
+    *Fc = -xip * f->s2 + xic * f->c2;
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O10 margins (reading G11)                                                          */
+/* ---------------------------------------------------------------------------------- */
+typedef struct { int64_t m1, m2, w, lo, hi; } margins_t;
+
+static int64_t iceil(double x) { return (int64_t)ceil(x); }
+
+static void margins(const orc_orbit_desc *d, int gen, int order, int fd_order, margins_t *m)
+{
+    const int M = order + 1;
+    const double c = ORC_C_LIGHT;
+    m->m1 = iceil(1.02 * (d->R_m + d->arm_m) / c / d->dt) + M / 2;
+    m->m2 = iceil((gen == ORC_GEN_20 ? 7.2 : 3.1) * (d->arm_m / c) / d->dt) + M / 2;
+    m->w = fd_order / 2;
+    m->lo = m->m1 + m->m2 + 2 * m->w;
+    m->hi = m->m1 + M / 2 + 2 * m->w;
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O5  single-link response, Eq. (2.5) with delays (2.6) (readings G3, G4)             */
+/* ---------------------------------------------------------------------------------- */
+static void links_full_at(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc,
+                          int64_t n, int order, real y[6])
+{
+    const real c = ORC_C_LIGHT, dt = o->d.dt;
+    geom_t g;
+    orbit_geometry(o, n, &g);
+    for (int l = 0; l < 6; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real Fp, Fc;
+        antenna(f, g.nh[l], &Fp, &Fc);
+        const real kn = dot3(f->k, g.nh[l]);
+        const real delta_s = g.L[l] + dot3(f->k, g.R[s]) / c; /* (2.6a) */
+        const real delta_r = dot3(f->k, g.R[r]) / c;          /* (2.6b) */
+        const real Hs = Fp * interp_input(hp, o->d.n, n, delta_s, dt, order) +
+                        Fc * interp_input(hc, o->d.n, n, delta_s, dt, order);
+        const real Hr = Fp * interp_input(hp, o->d.n, n, delta_r, dt, order) +
+                        Fc * interp_input(hc, o->d.n, n, delta_r, dt, order);
+        y[l] = (Hs - Hr) / (2 * (1 - kn)); /* (2.5) */
+    }
+}
+
+/* LFA single link, Eq. (3.1) = (B10), retarded time (B1) (readings G14, G16); only l = +1,+2,+3 */
+static void links_lfa_at(const orbit_ctx *o, const frame_t *f, const real *gp, const real *gc,
+                         int64_t g0, int64_t glen, int64_t n, int order, real y[6])
+{
+    const real c = ORC_C_LIGHT, dt = o->d.dt;
+    geom_t g;
+    orbit_geometry(o, n, &g);
+    for (int l = 0; l < 6; ++l) y[l] = 0; /* "the rest are set to zero" */
+    for (int l = 0; l < 3; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real Fp, Fc;
+        antenna(f, g.nh[l], &Fp, &Fc);
+        const real tau = g.L[l] / 2 + (dot3(f->k, g.R[s]) + dot3(f->k, g.R[r])) / (2 * c); /* (B1) */
+        const real dHp = interp_series(gp, g0, glen, n, tau, dt, order);
+        const real dHc = interp_series(gc, g0, glen, n, tau, dt, order);
+        y[l] = -(g.L[l] / 2) * (Fp * dHp + Fc * dHc); /* (B10), L_l in seconds */
+    }
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* O6  Michelson TDI, Eqs. (2.7), (2.8) with G8, G9, G12; ch = 0,1,2 -> X,Y,Z          */
+/* ---------------------------------------------------------------------------------- */
+static int cyc(int label, int times) /* 1->2->3->1 on |l|, sign kept */
+{
+    int a = label > 0 ? label : -label;
+    for (int i = 0; i < times; ++i) a = a % 3 + 1;
+    return label > 0 ? a : -a;
+}
+
+typedef struct { const real *y[6]; int64_t y0, ylen; } yseries_t;
+
+static real ydel(const yseries_t *ys, int label, int64_t n, real delay, real dt, int order)
+{
+    const int l = link_index(label);
+    if (delay == 0) { /* undelayed terms are taken from the grid */
+        const int64_t i = n - ys->y0;
+        return (i >= 0 && i < ys->ylen) ? ys->y[l][i] : (real)0;
+    }
+    return interp_series(ys->y[l], ys->y0, ys->ylen, n, delay, dt, order);
+}
+
+static real michelson_at(const yseries_t *ys, const real Lsec[6], int ch, int gen, int64_t n, real dt,
+                         int order)
+{
+    /* X uses |l| = 2, 3; Y and Z by cyclic permutation */
+    const int p2 = cyc(2, ch), p3 = cyc(3, ch);
+    const real Lp2 = Lsec[link_index(p2)], Lm2 = Lsec[link_index(-p2)];
+    const real Lp3 = Lsec[link_index(p3)], Lm3 = Lsec[link_index(-p3)];
+#define Y(label, delay) ydel(ys, (label), n, (delay), dt, order)
+    /* Eq. (2.7), term by term in the printed order (y_1-32, y_231, y_123, y_3-21 for X) */
+    real X = Y(-p3, Lm2 + Lp2 + Lp3) - Y(-p3, Lp3)
+           + Y(+p3, Lp2 + Lm2)       - Y(+p3, (real)0)
+           + Y(+p2, Lm2)             - Y(+p2, Lm2 + Lm3 + Lp3)
+           + Y(-p2, (real)0)         - Y(-p2, Lm3 + Lp3);
+    if (gen == ORC_GEN_20) {
+        /* Eq. (2.8); the 7th term with reading G9 (L_-2 + L_2 + 2 L_3 + 2 L_-3) */
+        X += Y(-p3, Lm2 + Lp2 + 2 * Lp3 + Lm3)         - Y(-p3, 2 * Lp3 + Lm3 + 2 * Lm2 + 2 * Lp2)
+           + Y(+p3, Lm2 + Lp2 + Lp3 + Lm3)             - Y(+p3, Lp3 + Lm3 + 2 * Lm2 + 2 * Lp2)
+           + Y(+p2, 2 * Lm2 + Lp2 + 2 * Lp3 + 2 * Lm3) - Y(+p2, Lp3 + Lm3 + 2 * Lm2 + Lp2)
+           + Y(-p2, Lm2 + Lp2 + 2 * Lp3 + 2 * Lm3)     - Y(-p2, Lp3 + Lm3 + Lm2 + Lp2);
+    }
+#undef Y
+    return X;
+}
+
+/* LFA Michelson, Eq. (B25) (gen 1.5) / (B33) (gen 2.0); dy[l] = FD1 or FD2 of y_l, l = +1,+2,+3 */
+static real michelson_lfa_at(const yseries_t *dys, const real Lsec[6], int ch, int gen, int64_t n,
+                             real dt, int order)
+{
+    const int p2 = cyc(2, ch), p3 = cyc(3, ch);
+    const real L2 = Lsec[link_index(p2)], L3 = Lsec[link_index(p3)]; /* positive-link values, G14 */
+    /* y_123 is link +2 (p2), y_231 is link +3 (p3) */
+    if (gen == ORC_GEN_15)
+        return 4 * (L3 * ydel(dys, +p2, n, L3 + L2 / 2, dt, order) -
+                    L2 * ydel(dys, +p3, n, L2 + L3 / 2, dt, order));
+    return 8 * (L2 + L3) * (L3 * ydel(dys, +p2, n, 2 * L3 + 3 * L2 / 2, dt, order) -
+                            L2 * ydel(dys, +p3, n, 2 * L2 + 3 * L3 / 2, dt, order));
+}
+
+/* O7  Eq. (2.9) */
+static void aet(real X, real Y, real Z, real *A, real *E, real *T)
+{
+    *A = (Z - X) / R_SQRT((real)2);
+    *E = (X - 2 * Y + Z) / R_SQRT((real)6);
+    *T = (X + Y + Z) / R_SQRT((real)3);
+}
+
+/* O9  hybrid weights, Eqs. (4.1), (4.5) (reading G18) and the raised-cosine taper (G20) */
+static void hybrid_weights(const orc_hybrid *h, real t, real *w_lfa, real *w_full)
+{
+    const real th = h->t_hyb, T = h->window_s;
+    if (h->taper == ORC_TAPER_SIGMOID) {
+        const real sg = h->sigma_s;
+        *w_lfa = (t <= th + T / 2) ? 1 / (1 + R_EXP((t - th) / sg)) : (real)0;   /* Sigma(+1) */
+        *w_full = (t >= th - T / 2) ? 1 / (1 + R_EXP(-(t - th) / sg)) : (real)0; /* Sigma(-1) */
+    } else {
+        const real x = (t - th + T / 2) / T;
+        if (x <= 0) *w_full = 0;
+        else if (x >= 1) *w_full = 1;
+        else *w_full = (real)0.5 * (1 - R_COS(R_PI * x));
+        *w_lfa = 1 - *w_full;
+    }
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* drivers: outputs for absolute samples [nb, ne) of every source, compact rows of      */
+/* length ne - nb.  Any output pointer may be NULL.                                     */
+/* ---------------------------------------------------------------------------------- */
+typedef struct {
+    real *y[6];      /* link series on [y0, y0 + ylen) */
+    real *X[3];      /* Michelson on [nb, ne) */
+    int64_t y0, ylen;
+} work_t;
+
+static int64_t imax(int64_t a, int64_t b) { return a > b ? a : b; }
+static int64_t imin(int64_t a, int64_t b) { return a < b ? a : b; }
+
+static int work_alloc(work_t *w, int64_t y0, int64_t ylen, int64_t nout)
+{
+    memset(w, 0, sizeof *w);
+    w->y0 = y0;
+    w->ylen = ylen;
+    for (int l = 0; l < 6; ++l)
+        if (!(w->y[l] = (real *)calloc((size_t)imax(ylen, 1), sizeof(real)))) return ORC_EINVAL;
+    for (int c = 0; c < 3; ++c)
+        if (!(w->X[c] = (real *)calloc((size_t)imax(nout, 1), sizeof(real)))) return ORC_EINVAL;
+    return ORC_OK;
+}
+static void work_free(work_t *w)
+{
+    for (int l = 0; l < 6; ++l) free(w->y[l]);
+    for (int c = 0; c < 3; ++c) free(w->X[c]);
+}
+
+/* full response for one source: y (6 links) on the halo range, X,Y,Z on [nb,ne) */
+static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
+                    int order, const margins_t *mg, int64_t lo, int64_t hi, int64_t nb, int64_t ne,
+                    work_t *w)
+{
+    const int64_t N = o->d.n;
+    const int64_t y0 = imax(0, nb - mg->m2), y1 = imin(N, ne + (order + 1) / 2 + 1);
+    if (work_alloc(w, y0, y1 - y0, ne - nb)) return ORC_EINVAL;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = y0; m < y1; ++m) {
+        if (m < mg->m1 || m >= N - mg->m1) continue; /* margin: y = 0 (G11) */
+        real y[6];
+        links_full_at(o, f, hp, hc, m, order, y);
+        for (int l = 0; l < 6; ++l) w->y[l][m - y0] = y[l];
+    }
+    yseries_t ys = { { w->y[0], w->y[1], w->y[2], w->y[3], w->y[4], w->y[5] }, y0, y1 - y0 };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = nb; n < ne; ++n) {
+        if (n < lo || n >= N - hi) continue; /* margin: X = 0 */
+        geom_t g;
+        orbit_geometry(o, n, &g); /* every delay evaluated at t_n */
+        for (int c = 0; c < 3; ++c)
+            w->X[c][n - nb] = michelson_at(&ys, g.L, c, gen, n, (real)o->d.dt, order);
+    }
+    return ORC_OK;
+}
+
+/* LFA response for one source */
+static int lfa_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
+                   int order, int fd_order, const margins_t *mg, int64_t nb, int64_t ne, work_t *w)
+{
+    const int64_t N = o->d.n, wd = mg->w;
+    const real dt = o->d.dt;
+    /* ranges, innermost last: X on [nb,ne) <- dy on [d0,d1) <- y on [y0,y1) <- g on [g0,g1) */
+    const int64_t d0 = imax(0, nb - mg->m2), d1 = imin(N, ne + (order + 1) / 2 + 1);
+    const int64_t y0 = imax(0, d0 - wd), y1 = imin(N, d1 + wd);
+    const int64_t g0 = imax(0, y0 - mg->m1), g1 = imin(N, y1 + mg->m1);
+    real *gp = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *gc = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *dy[3] = { 0, 0, 0 };
+    for (int l = 0; l < 3; ++l) dy[l] = (real *)calloc((size_t)imax(d1 - d0, 1), sizeof(real));
+    if (!gp || !gc || !dy[0] || !dy[1] || !dy[2] || work_alloc(w, y0, y1 - y0, ne - nb)) return ORC_EINVAL;
+    /* g = d h / dt by the central stencil on the grid */
+#pragma omp parallel for
+    for (int64_t i = g0; i < g1; ++i) {
+        if (i < wd || i >= N - wd) continue;
+        gp[i - g0] = fd1_in(hp, i, dt, fd_order);
+        gc[i - g0] = fd1_in(hc, i, dt, fd_order);
+    }
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = y0; m < y1; ++m) {
+        if (m < mg->m1 + wd || m >= N - mg->m1 - wd) continue;
+        real y[6];
+        links_lfa_at(o, f, gp, gc, g0, g1 - g0, m, order, y);
+        for (int l = 0; l < 6; ++l) w->y[l][m - y0] = y[l];
+    }
+    /* dy = first (gen 1.5) or second (gen 2.0) time derivative of y_l, l = +1,+2,+3 */
+#pragma omp parallel for
+    for (int64_t i = d0; i < d1; ++i) {
+        if (i < mg->m1 + 2 * wd || i >= N - mg->m1 - 2 * wd) continue;
+        for (int l = 0; l < 3; ++l)
+            dy[l][i - d0] = (gen == ORC_GEN_15) ? fd1_r(w->y[l], i - y0, dt, fd_order)
+                                                : fd2_r(w->y[l], i - y0, dt, fd_order);
+    }
+    yseries_t dys = { { dy[0], dy[1], dy[2], 0, 0, 0 }, d0, d1 - d0 };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = nb; n < ne; ++n) {
+        if (n < mg->lo || n >= N - mg->hi) continue;
+        geom_t g;
+        orbit_geometry(o, n, &g);
+        for (int c = 0; c < 3; ++c)
+            w->X[c][n - nb] = michelson_lfa_at(&dys, g.L, c, gen, n, dt, order);
+    }
+    free(gp); free(gc);
+    for (int l = 0; l < 3; ++l) free(dy[l]);
+    return ORC_OK;
+}
+
+static void emit(const work_t *w, int64_t nb, int64_t ne, int64_t b, int64_t batch, double *A, double *E,
+                 double *T, double *XYZ, double *y)
+{
+    const int64_t len = ne - nb;
+    for (int64_t i = 0; i < len; ++i) {
+        real a, e, t;
+        aet(w->X[0][i], w->X[1][i], w->X[2][i], &a, &e, &t);
+        if (A) A[b * len + i] = (double)a;
+        if (E) E[b * len + i] = (double)e;
+        if (T) T[b * len + i] = (double)t;
+        if (XYZ)
+            for (int c = 0; c < 3; ++c) XYZ[(c * batch + b) * len + i] = (double)w->X[c][i];
+        if (y)
+            for (int l = 0; l < 6; ++l) {
+                const int64_t m = nb + i - w->y0;
+                y[(l * batch + b) * len + i] = (m >= 0 && m < w->ylen) ? (double)w->y[l][m] : 0.0;
+            }
+    }
+}
+
+static int check_args(const orc_orbit_desc *d, int gen, int order, int fd_order, int need_fd, int64_t ld,
+                      int64_t nb, int64_t ne)
+{
+    if (!d || d->n <= 0 || d->dt <= 0) return ORC_EINVAL;
+    if (gen != ORC_GEN_15 && gen != ORC_GEN_20) return ORC_EINVAL;
+    if (order < 1 || order > 63 || order % 2 == 0) return ORC_EINVAL;
+    if (need_fd && fd_order != 2 && fd_order != 4) return ORC_EINVAL;
+    if (ld < d->n || nb < 0 || ne > d->n || nb > ne) return ORC_EINVAL;
+    return ORC_OK;
+}
+
+/* ---- exported API ---------------------------------------------------------------- */
+
+int orc_real_bits(void) { return (int)(sizeof(real) * 8); }
+int orc_real_mant_dig(void)
+{
+#ifdef ORC_REAL_LD
+    return __LDBL_MANT_DIG__;
+#else
+    return __DBL_MANT_DIG__;
+#endif
+}
+
+int orc_margins(const orc_orbit_desc *d, int gen, int order, int fd_order, int64_t *lo, int64_t *hi)
+{
+    margins_t m;
+    if (!d || !lo || !hi) return ORC_EINVAL;
+    margins(d, gen, order, fd_order, &m);
+    *lo = m.lo;
+    *hi = m.hi;
+    return ORC_OK;
+}
+
+/* margins of the link series y itself (valid on [ylo, n - yhi)) */
+int orc_link_margins(const orc_orbit_desc *d, int order, int fd_order, int64_t *ylo, int64_t *yhi)
+{
+    margins_t m;
+    if (!d || !ylo || !yhi) return ORC_EINVAL;
+    margins(d, ORC_GEN_15, order, fd_order, &m);
+    *ylo = m.m1 + m.w;
+    *yhi = m.m1 + m.w;
+    return ORC_OK;
+}
+
+/* Eq. (4.2): t_hyb = t_c - 5 (8 pi f_hyb)^(-8/3) (G Mc / c^3)^(-5/3) */
+double orc_hyb_time(double f_hyb_hz, double mchirp_s, double t_c)
+{
+    return (double)((real)t_c - 5 * R_POW(8 * R_PI * (real)f_hyb_hz, -(real)8 / 3) *
+                                    R_POW((real)mchirp_s, -(real)5 / 3));
+}
+
+/* Eq. (4.3) */
+double orc_lfa_fraction(double f_hyb, double f_min, double f_max)
+{
+    const real e = -(real)8 / 3;
+    return (double)((R_POW((real)f_min, e) - R_POW((real)f_hyb, e)) /
+                    (R_POW((real)f_min, e) - R_POW((real)f_max, e)));
+}
+
+void orc_lagrange_weights(double eps, int order, double *w)
+{
+    real wr[64];
+    lagrange_weights((real)eps, order, wr);
+    for (int i = 0; i <= order; ++i) w[i] = (double)wr[i];
+}
+
+/* I[x](n, d): value of x at t_n - d (O4) */
+double orc_interp(const double *x, int64_t len, int64_t n, double d, double dt, int order)
+{
+    return (double)interp_input(x, len, n, (real)d, (real)dt, order);
+}
+
+/* derivative stencils on a double series, which = 1 (FD1) or 2 (FD2); out[i] for i in [w, len-w) */
+void orc_stencil(const double *x, int64_t len, double dt, int fd_order, int which, double *out)
+{
+    const int64_t w = fd_order / 2;
+    real *xr = (real *)malloc(sizeof(real) * (size_t)len);
+    for (int64_t i = 0; i < len; ++i) { xr[i] = x[i]; out[i] = 0; }
+    for (int64_t i = w; i < len - w; ++i)
+        out[i] = (double)(which == 1 ? fd1_r(xr, i, (real)dt, fd_order) : fd2_r(xr, i, (real)dt, fd_order));
+    free(xr);
+}
+
+/* source frame: out = k[3], u[3], v[3], cos 2psi, sin 2psi */
+void orc_source_frame(const orc_source *s, double *out)
+{
+    frame_t f;
+    source_frame(s, &f);
+    for (int a = 0; a < 3; ++a) { out[a] = (double)f.k[a]; out[3 + a] = (double)f.u[a]; out[6 + a] = (double)f.v[a]; }
+    out[9] = (double)f.c2;
+    out[10] = (double)f.s2;
+}
+
+/* orbit tables for samples [nb, ne): R [3][3][len], nhat [6][3][len], L [6][len] */
+int orc_orbit_tables(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, int64_t nb,
+                     int64_t ne, double *R, double *nhat, double *L)
+{
+    if (!d || nb < 0 || ne > d->n || nb > ne) return ORC_EINVAL;
+    if (d->mode == ORC_ORBIT_TABLES && (!Rtab || !Ltab)) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    const int64_t len = ne - nb;
+#pragma omp parallel for
+    for (int64_t n = nb; n < ne; ++n) {
+        geom_t g;
+        orbit_geometry(&o, n, &g);
+        for (int i = 0; i < 3; ++i)
+            for (int a = 0; a < 3; ++a)
+                if (R) R[(i * 3 + a) * len + (n - nb)] = (double)g.R[i][a];
+        for (int l = 0; l < 6; ++l) {
+            for (int a = 0; a < 3; ++a)
+                if (nhat) nhat[(l * 3 + a) * len + (n - nb)] = (double)g.nh[l][a];
+            if (L) L[l * len + (n - nb)] = (double)g.L[l];
+        }
+    }
+    return ORC_OK;
+}
+
+/* antenna patterns F^+_l, F^x_l and k.n_l of one source at sample n: out[6][3] */
+int orc_antenna(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const orc_source *s,
+                int64_t n, double *out)
+{
+    orbit_ctx o = { *d, Rtab, Ltab };
+    frame_t f;
+    geom_t g;
+    source_frame(s, &f);
+    orbit_geometry(&o, n, &g);
+    for (int l = 0; l < 6; ++l) {
+        real Fp, Fc;
+        antenna(&f, g.nh[l], &Fp, &Fc);
+        out[l * 3 + 0] = (double)Fp;
+        out[l * 3 + 1] = (double)Fc;
+        out[l * 3 + 2] = (double)dot3(f.k, g.nh[l]);
+    }
+    return ORC_OK;
+}
+
+void orc_hybrid_weights(const orc_hybrid *h, const double *t, int64_t len, double *w_lfa, double *w_full)
+{
+    for (int64_t i = 0; i < len; ++i) {
+        real a, b;
+        hybrid_weights(h, (real)t[i], &a, &b);
+        w_lfa[i] = (double)a;
+        w_full[i] = (double)b;
+    }
+}
+
+/*
+ * Full response (O5-O7).  hp, hc: [batch][ld]; outputs: A,E,T [batch][ne-nb],
+ * XYZ [3][batch][ne-nb], y [6][batch][ne-nb]; any may be NULL.
+ */
+int orc_response_full(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
+                      const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
+                      int order, int64_t nb, int64_t ne, double *A, double *E, double *T, double *XYZ,
+                      double *y)
+{
+    if (check_args(d, gen, order, 0, 0, ld, nb, ne) || !hp || !hc || !src) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, 0, &mg);
+    for (int64_t b = 0; b < batch; ++b) {
+        frame_t f;
+        work_t w;
+        source_frame(&src[b], &f);
+        if (full_one(&o, &f, hp + b * ld, hc + b * ld, gen, order, &mg, mg.lo, mg.hi, nb, ne, &w)) return ORC_EINVAL;
+        emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&w);
+    }
+    return ORC_OK;
+}
+
+/* LFA response (O8) */
+int orc_response_lfa(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
+                     const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
+                     int order, int fd_order, int64_t nb, int64_t ne, double *A, double *E, double *T,
+                     double *XYZ, double *y)
+{
+    if (check_args(d, gen, order, fd_order, 1, ld, nb, ne) || !hp || !hc || !src) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, fd_order, &mg);
+    for (int64_t b = 0; b < batch; ++b) {
+        frame_t f;
+        work_t w;
+        source_frame(&src[b], &f);
+        if (lfa_one(&o, &f, hp + b * ld, hc + b * ld, gen, order, fd_order, &mg, nb, ne, &w)) return ORC_EINVAL;
+        emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&w);
+    }
+    return ORC_OK;
+}
+
+/* Hybrid response (O9): both responses on the whole requested range, blended per Eqs. (4.5), (4.6);
+ * hyb has n_hyb = 1 or batch entries. */
+int orc_response_hybrid(const orc_orbit_desc *d, const double *Rtab, const double *Ltab,
+                        const double *hp, const double *hc, int64_t ld, int64_t batch,
+                        const orc_source *src, int gen, int order, int fd_order, const orc_hybrid *hyb,
+                        int64_t n_hyb, int64_t nb, int64_t ne, double *A, double *E, double *T,
+                        double *XYZ, double *y)
+{
+    if (check_args(d, gen, order, fd_order, 1, ld, nb, ne) || !hp || !hc || !src || !hyb) return ORC_EINVAL;
+    if (n_hyb != 1 && n_hyb != batch) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg, mf;
+    margins(d, gen, order, fd_order, &mg); /* hybrid margins = the (wider) LFA ones */
+    margins(d, gen, order, 0, &mf);
+    const int64_t N = d->n;
+    for (int64_t b = 0; b < batch; ++b) {
+        const orc_hybrid *h = &hyb[n_hyb == 1 ? 0 : b];
+        frame_t f;
+        work_t wl, wf, wh;
+        source_frame(&src[b], &f);
+        if (lfa_one(&o, &f, hp + b * ld, hc + b * ld, gen, order, fd_order, &mg, nb, ne, &wl)) return ORC_EINVAL;
+        if (full_one(&o, &f, hp + b * ld, hc + b * ld, gen, order, &mf, mg.lo, mg.hi, nb, ne, &wf)) return ORC_EINVAL;
+        if (work_alloc(&wh, nb, ne - nb, ne - nb)) return ORC_EINVAL;
+        for (int64_t n = nb; n < ne; ++n) {
+            real wa, wb;
+            hybrid_weights(h, (real)d->t0 + (real)n * (real)d->dt, &wa, &wb);
+            /* (4.5): links, valid where both link series are (the LFA link margins) */
+            if (n >= mg.m1 + mg.w && n < N - mg.m1 - mg.w)
+                for (int l = 0; l < 6; ++l)
+                    wh.y[l][n - nb] = wa * wl.y[l][n - wl.y0] + wb * wf.y[l][n - wf.y0];
+            /* (4.6): Michelson observables blended separately (G19) */
+            for (int c = 0; c < 3; ++c) wh.X[c][n - nb] = wa * wl.X[c][n - nb] + wb * wf.X[c][n - nb];
+        }
+        emit(&wh, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&wl); work_free(&wf); work_free(&wh);
+    }
+    return ORC_OK;
+}
