@@ -1,0 +1,152 @@
+/*
+ * lisatdi.h -- C ABI of the B200 (sm_100a) time-domain LISA response library.
+ *
+ * The operations are those of arXiv 2505.09600 (Valencia & Husa); "P:n" is line n of
+ * PAPER.md, "G<k>" a reading listed in DESIGN.md.  Everything is fp64.
+ *
+ *   full response   P:85-161   Eqs. (2.2)-(2.9): projection of h+, hx onto the six links at
+ *                               retarded times, Michelson TDI 1.5 / 2.0, A, E, T
+ *   LFA             P:210-260, P:677-957  Eqs. (3.1), (B1), (B10), (B25), (B33)
+ *   hybrid          P:263-315  Eqs. (4.1), (4.2), (4.5), (4.6)
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE memory, h_* are HOST memory; both are owned by the
+ *     caller.  The library allocates no device memory and keeps no pointer after a call
+ *     returns, except that an ltdi_orbits handle refers to the caller's table buffer.
+ *   - Every call is asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
+ *     legacy default stream), except for the copy of the small h_* parameter arrays,
+ *     which are consumed before the call returns.
+ *   - Return value: LTDI_OK or a negative LTDI_E* code.  Nothing throws or aborts.
+ *   - Time grid: t_n = t0 + n dt, n = 0 .. n-1, shared by all sources of a batch.
+ *   - Series layout: a series of source b starts at element b * ld (ld >= n).
+ *   - Links are ordered l = +1, +2, +3, -1, -2, -3 (+1: 3->2, +2: 1->3, +3: 2->1,
+ *     -1: 2->3, -2: 3->1, -3: 1->2), spacecraft 1, 2, 3.
+ *   - Fractional delays use centred Lagrange interpolation of odd order p (p + 1 taps, G10).
+ *   - Output samples n < lo or n >= n - hi (ltdi_margins) are written as exactly 0.0 (G11).
+ */
+#ifndef LISATDI_H
+#define LISATDI_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { LTDI_OK = 0, LTDI_EINVAL = -1, LTDI_EUNSUPPORTED = -2, LTDI_ECUDA = -3, LTDI_EWORKSPACE = -4 };
+enum { LTDI_GEN_15 = 15, LTDI_GEN_20 = 20 };                 /* Eq. (2.7) / Eq. (2.8) */
+enum {
+    LTDI_ORBIT_STATIC_EQUALARM = 0, /* Keplerian positions, L_l(t) = arm_m / c constant ("equal and constant") */
+    LTDI_ORBIT_KEPLERIAN = 1,       /* Keplerian positions, first-order light times, L_l != L_-l (G6)         */
+    LTDI_ORBIT_TABLES = 2           /* caller-supplied positions and light times per sample                           */
+};
+enum { LTDI_TAPER_SIGMOID = 0,      /* Eq. (4.1), the paper's weight                                  */
+       LTDI_TAPER_COSINE = 1 };     /* raised cosine over the window (BASELINE.json configs 2, 4; G20) */
+enum { LTDI_RESPONSE_FULL = 0, LTDI_RESPONSE_LFA = 1, LTDI_RESPONSE_HYBRID = 2 };
+
+/* Time grid and orbit model (first-order Keplerian orbits, G5). */
+typedef struct {
+    double t0, dt;   /* t_n = t0 + n dt [s], dt > 0 */
+    int64_t n;       /* samples, > 0 */
+    double arm_m;    /* nominal arm length L [m] (2.5e9) */
+    double R_m;      /* orbital radius [m] (1 AU) */
+    double period_s; /* orbital period [s] (Omega = 2 pi / period) */
+    double alpha0;   /* orbital phase at t = 0 [rad] */
+    double rot0;     /* constellation rotation phase [rad] */
+    int32_t mode;    /* LTDI_ORBIT_* */
+} ltdi_orbit_desc;
+
+typedef struct { double beta, lambda, psi; } ltdi_source; /* ecliptic latitude, longitude, polarisation [rad] */
+
+/* Hybridisation window: centre t_hyb [s], width window_s (T), sigmoid scale sigma_s. */
+typedef struct { double t_hyb, window_s, sigma_s; int32_t taper; } ltdi_hybrid;
+
+typedef struct ltdi_orbits ltdi_orbits; /* opaque, immutable after init */
+
+/* Rows of the device orbit table: 9 positions R_i [m] (i*3+axis), 9 unit vectors n_l for
+ * l = +1,+2,+3 (n_-l = -n_l), 6 light travel times L_l [s]; row stride = ltdi_orbits_stride(). */
+#define LTDI_TABLE_ROWS 24
+
+/* ---- S0: orbit / delay tables (Eq. (B22)) -------------------------------- */
+
+/* Bytes of the device buffer that ltdi_orbits_init* fills for this grid. */
+int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes);
+
+/* Launch the orbit/delay kernel: spacecraft positions, link unit vectors and light travel
+ * times per sample into d_tables (>= workspace bytes, 16-byte aligned).  mode must be
+ * STATIC_EQUALARM or KEPLERIAN.  *out receives a host handle (free with ltdi_orbits_destroy). */
+int ltdi_orbits_init(const ltdi_orbit_desc *desc, void *d_tables, size_t bytes, void *stream,
+                     ltdi_orbits **out);
+
+/* Same from caller-supplied device tables: d_R [3][3][n] positions [m], d_L [6][n] light travel
+ * times [s]; the unit vectors are derived (n_l = (R_r - R_s) / |R_r - R_s|).  desc->mode
+ * must be LTDI_ORBIT_TABLES; arm_m and R_m still size the margins. */
+int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L,
+                            void *d_tables, size_t bytes, void *stream, ltdi_orbits **out);
+
+int ltdi_orbits_destroy(ltdi_orbits *orb);               /* frees the handle only */
+int64_t ltdi_orbits_stride(const ltdi_orbits *orb);      /* elements between table rows */
+const double *ltdi_orbits_tables(const ltdi_orbits *orb); /* the caller's d_tables */
+
+/* ---- helpers ------------------------------------------------------------------------------ */
+
+/* Output margins (G11): response samples n < *lo and n >= n - *hi are 0.  fd_order = 0 for the
+ * full response, 2 or 4 for LFA / hybrid. */
+int ltdi_margins(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo,
+                 int64_t *hi);
+/* Margins of the link series y_slr themselves. */
+int ltdi_link_margins(const ltdi_orbit_desc *desc, int lagrange_order, int fd_order, int64_t *lo,
+                      int64_t *hi);
+/* Eq. (4.2): t_hyb = t_c - 5 (8 pi f_hyb)^(-8/3) (G Mc / c^3)^(-5/3); mchirp_s = G Mc / c^3 [s]. */
+int ltdi_hyb_time(double f_hyb_hz, double mchirp_s, double t_c, double *t_hyb);
+
+/* Bytes of d_work needed by ltdi_response_* (which = LTDI_RESPONSE_*). */
+int ltdi_workspace_bytes(int which, int64_t n, int64_t batch, int gen, int lagrange_order, size_t *bytes);
+
+/* ---- S1-S8: the three responses ------------------------------------------------------------- */
+/*
+ * Common arguments
+ *   orb             orbit tables for the time grid (n samples)
+ *   d_hp, d_hc      h+, hx sampled on the grid, [batch][ld], source frame
+ *   h_src           [batch] sky position and polarisation
+ *   gen             LTDI_GEN_15 or LTDI_GEN_20
+ *   lagrange_order  odd, 1 .. 63
+ *   d_A, d_E, d_T   [batch][ld] outputs, Eq. (2.9); required
+ *   d_XYZ           [3][batch][ld] Michelson X, Y, Z, or NULL
+ *   d_y             [6][batch][ld] single-link responses y_slr, or NULL
+ *   d_work          scratch of ltdi_workspace_bytes() bytes, 16-byte aligned
+ * Errors: LTDI_EINVAL for NULL required pointers, bad gen / order / fd_order, ld < n, batch < 1;
+ * LTDI_EWORKSPACE if work_bytes is too small; LTDI_ECUDA if a CUDA call fails.
+ */
+
+/* Full response: Eqs. (2.2)-(2.6) projection (S2, S3), Eq. (2.7)/(2.8) TDI (S4), Eq. (2.9) (S5). */
+int ltdi_response_full(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                       int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, double *d_A,
+                       double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
+                       size_t work_bytes, void *stream);
+
+/* Low-frequency approximation: Eq. (B10) links at the retarded time (B1) from central-difference
+ * derivatives of h+, hx (S6), Eq. (B25) (gen 1.5) / (B33) (gen 2.0) Michelson (S7).  fd_order 2 | 4.
+ * Links -1, -2, -3 are zero. */
+int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                      int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                      double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
+                      size_t work_bytes, void *stream);
+
+/* Hybrid: LFA for t <= t_hyb + T/2, full for t >= t_hyb - T/2, links blended by Eq. (4.5) and
+ * X, Y, Z blended separately by Eq. (4.6) (S8).  h_hyb has n_hyb = 1 or batch entries. */
+int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                         int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order,
+                         int fd_order, const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E,
+                         double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes,
+                         void *stream);
+
+/* Number of kernel launches the library has issued in this process (for bench.py's gpu_launches). */
+int64_t ltdi_launch_count(void);
+const char *ltdi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LISATDI_H */

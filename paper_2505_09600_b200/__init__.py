@@ -1,0 +1,250 @@
+"""paper_2505_09600_b200 -- thin Python binding of liblisatdi.so (include/lisatdi.h).
+
+Argument marshalling only: every step of the response runs in the CUDA kernels of
+csrc/.  PyTorch supplies device memory and streams.  There is no CPU fallback: a
+missing library or a missing GPU raises.
+
+    import paper_2505_09600_b200 as ltdi
+    orb = ltdi.Orbits(ltdi.orbit_desc(n, dt, ltdi.ORBIT_KEPLERIAN))       # orbit/delay kernel
+    out = ltdi.response_full(orb, hp, hc, sources, gen=20, order=31)      # dict of device tensors
+    out = ltdi.response_lfa(orb, hp, hc, sources, gen=20, order=31, fd_order=2)
+    out = ltdi.response_hybrid(orb, hp, hc, sources, 20, 31, 2, hybrid=[{...}])
+
+hp, hc: float64 CUDA tensors [batch][ld]; sources: [batch][3] (beta, lambda, psi), host.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+GEN_15, GEN_20 = 15, 20
+ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES = 0, 1, 2
+TAPER_SIGMOID, TAPER_COSINE = 0, 1
+RESPONSE_FULL, RESPONSE_LFA, RESPONSE_HYBRID = 0, 1, 2
+OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, -1, -2, -3, -4
+_ERR = {EINVAL: "LTDI_EINVAL", EUNSUPPORTED: "LTDI_EUNSUPPORTED", ECUDA: "LTDI_ECUDA",
+        EWORKSPACE: "LTDI_EWORKSPACE"}
+
+C_LIGHT = 299792458.0
+ARM_M = 2.5e9
+AU_M = 149597870700.0
+YEAR_S = 31558149.7635      # sidereal year; Omega = 2 pi / yr
+
+
+class LtdiError(RuntimeError):
+    def __init__(self, fn, code):
+        super().__init__(f"{fn}: {_ERR.get(code, code)}")
+        self.code = code
+
+
+class OrbitDesc(C.Structure):
+    _fields_ = [("t0", C.c_double), ("dt", C.c_double), ("n", C.c_int64), ("arm_m", C.c_double),
+                ("R_m", C.c_double), ("period_s", C.c_double), ("alpha0", C.c_double),
+                ("rot0", C.c_double), ("mode", C.c_int32)]
+
+
+class Source(C.Structure):
+    _fields_ = [("beta", C.c_double), ("lam", C.c_double), ("psi", C.c_double)]
+
+
+class Hybrid(C.Structure):
+    _fields_ = [("t_hyb", C.c_double), ("window_s", C.c_double), ("sigma_s", C.c_double),
+                ("taper", C.c_int32)]
+
+
+_vp, _dp, _i64p, _szp = C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_size_t)
+_SIGNATURES = {
+    "ltdi_orbits_workspace_bytes": (C.c_int, [C.POINTER(OrbitDesc), _szp]),
+    "ltdi_orbits_init": (C.c_int, [C.POINTER(OrbitDesc), _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
+    "ltdi_orbits_init_tables": (C.c_int, [C.POINTER(OrbitDesc), _dp, _dp, _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
+    "ltdi_orbits_destroy": (C.c_int, [_vp]),
+    "ltdi_orbits_stride": (C.c_int64, [_vp]),
+    "ltdi_orbits_tables": (_vp, [_vp]),
+    "ltdi_margins": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, C.c_int, C.c_int, _i64p, _i64p]),
+    "ltdi_link_margins": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, C.c_int, _i64p, _i64p]),
+    "ltdi_hyb_time": (C.c_int, [C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]),
+    "ltdi_workspace_bytes": (C.c_int, [C.c_int, C.c_int64, C.c_int64, C.c_int, C.c_int, _szp]),
+    "ltdi_response_full": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                     _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_lfa": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                    C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_hybrid": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                       C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _dp, _dp, _vp,
+                                       C.c_size_t, _vp]),
+    "ltdi_launch_count": (C.c_int64, []),
+    "ltdi_version": (C.c_char_p, []),
+}
+EXPORTS = tuple(_SIGNATURES)
+
+_lib = None
+
+
+def lib():
+    """Load (building first if the sources are newer) liblisatdi.so; raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        handle = C.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(handle, name)   # AttributeError if the library does not export it
+            fn.restype, fn.argtypes = res, args
+        _lib = handle
+    return _lib
+
+
+def _check(fn, code):
+    if code != OK:
+        raise LtdiError(fn, code)
+
+
+def orbit_desc(n, dt, mode=ORBIT_KEPLERIAN, t0=0.0, arm_m=ARM_M, R_m=AU_M, period_s=YEAR_S, alpha0=0.0,
+               rot0=0.0):
+    return {"t0": float(t0), "dt": float(dt), "n": int(n), "arm_m": float(arm_m), "R_m": float(R_m),
+            "period_s": float(period_s), "alpha0": float(alpha0), "rot0": float(rot0), "mode": int(mode)}
+
+
+def _desc(d):
+    return OrbitDesc(d["t0"], d["dt"], int(d["n"]), d["arm_m"], d["R_m"], d["period_s"], d["alpha0"], d["rot0"],
+                     int(d["mode"]))
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev_f64(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous float64 CUDA tensor")
+    return t
+
+
+def margins(desc, gen, order, fd_order=0):
+    lo, hi = C.c_int64(), C.c_int64()
+    d = _desc(desc)
+    _check("ltdi_margins", lib().ltdi_margins(C.byref(d), gen, order, fd_order, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def link_margins(desc, order, fd_order=0):
+    lo, hi = C.c_int64(), C.c_int64()
+    d = _desc(desc)
+    _check("ltdi_link_margins", lib().ltdi_link_margins(C.byref(d), order, fd_order, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def hyb_time(f_hyb_hz, mchirp_s, t_c):
+    out = C.c_double()
+    _check("ltdi_hyb_time", lib().ltdi_hyb_time(f_hyb_hz, mchirp_s, t_c, C.byref(out)))
+    return out.value
+
+
+def launch_count():
+    return lib().ltdi_launch_count()
+
+
+class Orbits:
+    """Device orbit tables for one time grid (S0, the orbit/delay kernel)."""
+
+    def __init__(self, desc, R_table=None, L_table=None, device="cuda:0"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2505_09600_b200 needs a CUDA device (no CPU fallback)")
+        self.desc = dict(desc)
+        self.device = torch.device(device)
+        d = _desc(desc)
+        nbytes = C.c_size_t()
+        _check("ltdi_orbits_workspace_bytes", lib().ltdi_orbits_workspace_bytes(C.byref(d), C.byref(nbytes)))
+        self.tables = torch.empty(nbytes.value // 8, dtype=torch.float64, device=self.device)
+        handle = C.c_void_p()
+        with torch.cuda.device(self.device):
+            if int(desc["mode"]) == ORBIT_TABLES:
+                self._R = _dev_f64(R_table, "R_table")   # [3][3][n]
+                self._L = _dev_f64(L_table, "L_table")   # [6][n]
+                assert self._R.shape == (3, 3, d.n) and self._L.shape == (6, d.n)
+                rc = lib().ltdi_orbits_init_tables(C.byref(d), self._R.data_ptr(), self._L.data_ptr(),
+                                                   self.tables.data_ptr(), nbytes.value, _stream(), C.byref(handle))
+            else:
+                rc = lib().ltdi_orbits_init(C.byref(d), self.tables.data_ptr(), nbytes.value, _stream(),
+                                            C.byref(handle))
+        _check("ltdi_orbits_init", rc)
+        self.handle = handle
+        self.stride = lib().ltdi_orbits_stride(handle)
+
+    @property
+    def n(self):
+        return int(self.desc["n"])
+
+    def rows(self):
+        """[24][n] view of the table: R (9 rows), n_l for l = +1,+2,+3 (9 rows), L_l (6 rows)."""
+        return self.tables.view(24, self.stride)[:, :self.n]
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:
+            _lib.ltdi_orbits_destroy(h)
+
+
+def _sources(sources):
+    s = torch.as_tensor(sources, dtype=torch.float64, device="cpu").reshape(-1, 3).contiguous()
+    return C.cast(C.c_void_p(s.data_ptr()), C.POINTER(Source)), s   # same layout as ltdi_source[batch]
+
+
+class Workspace:
+    """Preallocated outputs and scratch so that repeated calls allocate nothing."""
+
+    def __init__(self, batch, ld, device, want_xyz=False, want_y=False):
+        kw = dict(dtype=torch.float64, device=device)
+        self.A, self.E, self.T = (torch.empty(batch, ld, **kw) for _ in range(3))
+        self.XYZ = torch.empty(3, batch, ld, **kw) if want_xyz else None
+        self.y = torch.empty(6, batch, ld, **kw) if want_y else None
+        nbytes = C.c_size_t()
+        _check("ltdi_workspace_bytes",
+               lib().ltdi_workspace_bytes(RESPONSE_HYBRID, ld, batch, GEN_20, 31, C.byref(nbytes)))
+        self.work = torch.empty(nbytes.value // 8, **kw)
+
+    def outputs(self):
+        return {"A": self.A, "E": self.E, "T": self.T, "XYZ": self.XYZ, "y": self.y}
+
+
+def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, want_y, ws):
+    hp, hc = _dev_f64(hp, "hp"), _dev_f64(hc, "hc")
+    if hp.dim() == 1:
+        hp, hc = hp[None], hc[None]
+    batch, ld = hp.shape
+    assert hc.shape == hp.shape
+    src_ptr, keep = _sources(sources)
+    assert keep.shape[0] == batch, "one (beta, lambda, psi) per source"
+    if ws is None:
+        ws = Workspace(batch, ld, hp.device, want_xyz, want_y)
+    p = lambda t: None if t is None else t.data_ptr()
+    tail = [p(ws.A), p(ws.E), p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream()]
+    head = [orb.handle, hp.data_ptr(), hc.data_ptr(), ld, batch, src_ptr, gen, order]
+    with torch.cuda.device(hp.device):
+        if which == RESPONSE_FULL:
+            rc, fn = lib().ltdi_response_full(*head, *tail), "ltdi_response_full"
+        elif which == RESPONSE_LFA:
+            rc, fn = lib().ltdi_response_lfa(*head, fd_order, *tail), "ltdi_response_lfa"
+        else:
+            hl = hybrid if isinstance(hybrid, (list, tuple)) else [hybrid]
+            harr = (Hybrid * len(hl))(*[Hybrid(h["t_hyb"], h["window_s"], h["sigma_s"], int(h["taper"])) for h in hl])
+            rc, fn = lib().ltdi_response_hybrid(*head, fd_order, harr, len(hl), *tail), "ltdi_response_hybrid"
+    _check(fn, rc)
+    return ws.outputs()
+
+
+def response_full(orb, hp, hc, sources, gen, order, want_xyz=False, want_y=False, workspace=None):
+    """Eqs. (2.2)-(2.9): projection, TDI `gen`, A, E, T.  Returns dict A, E, T (, XYZ, y)."""
+    return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_xyz, want_y, workspace)
+
+
+def response_lfa(orb, hp, hc, sources, gen, order, fd_order, want_xyz=False, want_y=False, workspace=None):
+    """Eqs. (B10), (B25)/(B33): low-frequency approximation with central stencils of order fd_order."""
+    return _run(RESPONSE_LFA, orb, hp, hc, sources, gen, order, fd_order, None, want_xyz, want_y, workspace)
+
+
+def response_hybrid(orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz=False, want_y=False,
+                    workspace=None):
+    """Eqs. (4.5), (4.6): LFA spliced to the full response; hybrid = dict or list of dicts
+    {t_hyb, window_s, sigma_s, taper}."""
+    return _run(RESPONSE_HYBRID, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, want_y, workspace)

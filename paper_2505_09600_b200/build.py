@@ -1,0 +1,38 @@
+"""Build liblisatdi.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+    python -m paper_2505_09600_b200.build [--force]
+
+The .so is git-ignored but travels to the GPU box with the gpurun snapshot.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+LIB = os.path.join(HERE, "liblisatdi.so")
+SOURCES = [os.path.join(CSRC, "lisatdi.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("common.cuh", "orbit.cuh", "response.cuh")] + [
+    os.path.join(INCLUDE, "lisatdi.h")]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+         "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-I", INCLUDE]
+
+
+def build(force=False, verbose=False):
+    if (not force and os.path.exists(LIB)
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)):
+        return LIB
+    cmd = [NVCC, *FLAGS, "-o", LIB, *SOURCES]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed building liblisatdi.so")
+    if verbose:
+        print(r.stderr)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose=True))

@@ -1,0 +1,56 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a, fp64).
+//
+// Notation follows arXiv 2505.09600: links l = +1,+2,+3,-1,-2,-3 (index 0..5), spacecraft
+// 1,2,3 (index 0..2), y_slr single-link responses, X,Y,Z Michelson, A,E,T (Eq. 2.9).
+// "P:n" = PAPER.md line n, "G<k>" = reading k in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lisatdi.h"
+
+#define LTDI_C_LIGHT 299792458.0 /* m/s */
+#define LTDI_MAX_TAPS 64
+#define LTDI_FRAME_STRIDE 16 /* doubles per source in the frame buffer */
+
+struct ltdi_orbits {
+    ltdi_orbit_desc desc;
+    const double *d_tab; /* [LTDI_TABLE_ROWS][stride] */
+    int64_t stride;
+};
+
+/* table rows */
+enum { ROW_R = 0, ROW_N = 9, ROW_L = 18 };
+
+/* sender / receiver spacecraft (0-based) of link index 0..5 */
+__host__ __device__ __forceinline__ int link_sender(int l)
+{
+    /* +1: 3->2, +2: 1->3, +3: 2->1, -1: 2->3, -2: 3->1, -3: 1->2 */
+    return l < 3 ? (l + 2) % 3 : (l - 3 + 1) % 3;
+}
+__host__ __device__ __forceinline__ int link_receiver(int l)
+{
+    return l < 3 ? (l + 1) % 3 : (l - 3 + 2) % 3;
+}
+
+struct Margins {
+    int64_t m1; /* reach of the projection (both sides) */
+    int64_t m2; /* backward reach of the TDI stage */
+    int64_t w;  /* stencil half width */
+    int64_t lo, hi;
+};
+
+/* The library is one translation unit (lisatdi.cu includes the .cuh files), so that the
+ * __constant__ tables below are visible to every kernel without relocatable device code. */
+
+/* Lagrange denominators 1 / prod_{m != k} (k - m) for every even tap count M = 2 (r + 1):
+ * row r, column k + M/2 - 1 */
+__constant__ double c_lag_inv_den[32 * LTDI_MAX_TAPS];
+
+#define LTDI_CUDA_OK(expr)                     \
+    do {                                       \
+        if ((expr) != cudaSuccess) {           \
+            (void)cudaGetLastError();          \
+            return LTDI_ECUDA;                 \
+        }                                      \
+    } while (0)

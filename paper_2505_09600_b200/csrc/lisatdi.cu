@@ -1,0 +1,329 @@
+// lisatdi.cu -- the C ABI of include/lisatdi.h: argument checks, tile plan, launches.
+// Single translation unit: the kernels live in orbit.cuh and response.cuh.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "orbit.cuh"
+#include "response.cuh"
+
+namespace {
+
+std::atomic<int64_t> g_launches{0};
+inline void count_launch(int k = 1) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+
+// 1 / prod_{m != k}(k - m), k, m = -(M/2-1) .. M/2, for every even M <= 64 (rows of c_lag_inv_den)
+int init_constants()
+{
+    static std::once_flag once;
+    static int status = LTDI_OK;
+    std::call_once(once, [] {
+        std::vector<double> tab(32 * LTDI_MAX_TAPS, 0.0);
+        for (int r = 0; r < 32; ++r) {
+            const int M = 2 * (r + 1), kmin = -(M / 2 - 1);
+            for (int i = 0; i < M; ++i) {
+                long double den = 1.0L;
+                for (int j = 0; j < M; ++j)
+                    if (j != i) den *= (long double)((kmin + i) - (kmin + j));
+                tab[r * LTDI_MAX_TAPS + i] = (double)(1.0L / den);
+            }
+        }
+        if (cudaMemcpyToSymbol(c_lag_inv_den, tab.data(), tab.size() * sizeof(double)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            status = LTDI_ECUDA;
+        }
+    });
+    return status;
+}
+
+int64_t iceil(double x) { return (int64_t)std::ceil(x); }
+
+// G11 / O10: closed-form reaches.  Projection: |k.R|/c + L <= 1.02 (R + arm)/c plus half a stencil;
+// TDI: 7 light times (gen 2.0) or 3 (gen 1.5) backwards with a 3 % allowance, plus half a stencil.
+Margins compute_margins(const ltdi_orbit_desc &d, int gen, int order, int fd_order)
+{
+    Margins m;
+    const int M = order + 1;
+    m.m1 = iceil(1.02 * (d.R_m + d.arm_m) / LTDI_C_LIGHT / d.dt) + M / 2;
+    m.m2 = iceil((gen == LTDI_GEN_20 ? 7.2 : 3.1) * (d.arm_m / LTDI_C_LIGHT) / d.dt) + M / 2;
+    m.w = fd_order / 2;
+    m.lo = m.m1 + m.m2 + 2 * m.w;
+    m.hi = m.m1 + M / 2 + 2 * m.w;
+    return m;
+}
+
+bool desc_ok(const ltdi_orbit_desc *d)
+{
+    return d && d->n > 0 && d->dt > 0.0 && d->arm_m > 0.0 && d->R_m > 0.0 && d->period_s > 0.0 &&
+           d->mode >= LTDI_ORBIT_STATIC_EQUALARM && d->mode <= LTDI_ORBIT_TABLES;
+}
+bool order_ok(int order) { return order >= 1 && order <= 63 && (order & 1); }
+bool gen_ok(int gen) { return gen == LTDI_GEN_15 || gen == LTDI_GEN_20; }
+
+int64_t table_stride(int64_t n) { return (n + 31) / 32 * 32; }
+
+int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L, void *d_tables, size_t bytes,
+                  void *stream, ltdi_orbits **out)
+{
+    if (!desc_ok(desc) || !d_tables || !out) return LTDI_EINVAL;
+    const int64_t stride = table_stride(desc->n);
+    if (bytes < (size_t)stride * LTDI_TABLE_ROWS * sizeof(double)) return LTDI_EWORKSPACE;
+    if ((uintptr_t)d_tables % 16) return LTDI_EINVAL;
+    OrbitKernelParams p;
+    p.t0 = desc->t0; p.dt = desc->dt; p.n = desc->n; p.stride = stride;
+    p.arm_m = desc->arm_m; p.R_m = desc->R_m;
+    p.omega = 2.0 * 3.14159265358979323846 / desc->period_s;
+    p.alpha0 = desc->alpha0; p.rot0 = desc->rot0; p.mode = desc->mode;
+    p.R_in = d_R; p.L_in = d_L; p.tab = (double *)d_tables;
+    const int threads = 256;
+    const int64_t blocks = (desc->n + threads - 1) / threads;
+    orbit_delay_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    ltdi_orbits *o = new (std::nothrow) ltdi_orbits;
+    if (!o) return LTDI_EINVAL;
+    o->desc = *desc;
+    o->d_tab = (const double *)d_tables;
+    o->stride = stride;
+    *out = o;
+    return LTDI_OK;
+}
+
+// workspace layout (doubles): raw sources [batch][3] | frames [batch][16] | hybrid windows [n_hyb][4]
+size_t work_doubles(int64_t batch) { return (size_t)batch * (3 + LTDI_FRAME_STRIDE + 4); }
+
+struct SmallArgs { double v[32 * 7]; }; /* batch <= 32: sources and windows travel as kernel arguments */
+
+__global__ void unpack_small_kernel(SmallArgs a, int batch, int n_hyb, double *src, HybDev *hyb)
+{
+    const int i = threadIdx.x;
+    if (i < batch * 3) src[i] = a.v[i];
+    if (i < n_hyb * 4) ((double *)hyb)[i] = a.v[96 + i];
+}
+
+template <int MT, bool STAGE>
+int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t st)
+{
+    static std::atomic<size_t> configured{0};
+    if (smem > 48 * 1024 && smem > configured.load()) {
+        LTDI_CUDA_OK(cudaFuncSetAttribute(response_kernel<MT, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)smem));
+        configured.store(smem);
+    }
+    response_kernel<MT, STAGE><<<(unsigned)(p.ntiles * p.batch), threads, smem, st>>>(p);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    return LTDI_OK;
+}
+
+int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                 int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
+                 const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
+                 double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    if (!orb || !d_hp || !d_hc || !h_src || !d_A || !d_E || !d_T || !d_work) return LTDI_EINVAL;
+    if (!gen_ok(gen) || !order_ok(order) || batch < 1 || ld < orb->desc.n) return LTDI_EINVAL;
+    if (which != LTDI_RESPONSE_FULL && fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
+    if (which == LTDI_RESPONSE_FULL) fd_order = 0;
+    if (which == LTDI_RESPONSE_HYBRID) {
+        if (!h_hyb || (n_hyb != 1 && n_hyb != batch)) return LTDI_EINVAL;
+        for (int64_t i = 0; i < n_hyb; ++i) {
+            if (h_hyb[i].taper != LTDI_TAPER_SIGMOID && h_hyb[i].taper != LTDI_TAPER_COSINE) return LTDI_EINVAL;
+            if (!(h_hyb[i].window_s > 0.0)) return LTDI_EINVAL;
+            if (h_hyb[i].taper == LTDI_TAPER_SIGMOID && !(h_hyb[i].sigma_s > 0.0)) return LTDI_EINVAL;
+        }
+    } else {
+        n_hyb = 0;
+    }
+    if ((uintptr_t)d_work % 16) return LTDI_EINVAL;
+    if (work_bytes < work_doubles(batch) * sizeof(double)) return LTDI_EWORKSPACE;
+    if (batch * ((orb->desc.n + 63) / 64) >= (int64_t)1 << 31) return LTDI_EUNSUPPORTED;
+    int rc = init_constants();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    /* S1: per-source parameters to the device, then the source-frame kernel */
+    double *w_src = (double *)d_work;
+    double *w_frames = w_src + 3 * batch;
+    HybDev *w_hyb = (HybDev *)(w_frames + LTDI_FRAME_STRIDE * batch);
+    if (batch <= 32) {
+        SmallArgs a;
+        for (int64_t b = 0; b < batch; ++b) {
+            a.v[3 * b + 0] = h_src[b].beta; a.v[3 * b + 1] = h_src[b].lambda; a.v[3 * b + 2] = h_src[b].psi;
+        }
+        for (int64_t i = 0; i < n_hyb; ++i) {
+            a.v[96 + 4 * i + 0] = h_hyb[i].t_hyb; a.v[96 + 4 * i + 1] = h_hyb[i].window_s;
+            a.v[96 + 4 * i + 2] = h_hyb[i].sigma_s; a.v[96 + 4 * i + 3] = (double)h_hyb[i].taper;
+        }
+        unpack_small_kernel<<<1, 128, 0, st>>>(a, (int)batch, (int)n_hyb, w_src, w_hyb);
+        count_launch();
+        LTDI_CUDA_OK(cudaGetLastError());
+    } else {
+        std::vector<double> pack((size_t)batch * 3 + (size_t)n_hyb * 4);
+        for (int64_t b = 0; b < batch; ++b) {
+            pack[3 * b + 0] = h_src[b].beta; pack[3 * b + 1] = h_src[b].lambda; pack[3 * b + 2] = h_src[b].psi;
+        }
+        double *hy = pack.data() + 3 * batch;
+        for (int64_t i = 0; i < n_hyb; ++i) {
+            hy[4 * i + 0] = h_hyb[i].t_hyb; hy[4 * i + 1] = h_hyb[i].window_s;
+            hy[4 * i + 2] = h_hyb[i].sigma_s; hy[4 * i + 3] = (double)h_hyb[i].taper;
+        }
+        /* pageable source: the runtime has consumed `pack` when these calls return */
+        LTDI_CUDA_OK(cudaMemcpyAsync(w_src, pack.data(), sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, st));
+        if (n_hyb)
+            LTDI_CUDA_OK(cudaMemcpyAsync(w_hyb, hy, sizeof(double) * 4 * n_hyb, cudaMemcpyHostToDevice, st));
+    }
+    source_frame_kernel<<<(unsigned)((batch + 127) / 128), 128, 0, st>>>(w_src, w_frames, batch);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+
+    /* tile plan */
+    const ltdi_orbit_desc &d = orb->desc;
+    const Margins mg = compute_margins(d, gen, order, fd_order);
+    const int M = order + 1;
+    RespParams p;
+    std::memset(&p, 0, sizeof p);
+    p.tab = orb->d_tab; p.stride = orb->stride; p.n = d.n; p.t0 = d.t0; p.dt = d.dt;
+    p.hp = d_hp; p.hc = d_hc; p.ld = ld; p.batch = batch;
+    p.frames = w_frames; p.hyb = w_hyb; p.n_hyb = n_hyb;
+    p.which = which; p.gen = gen; p.M = M; p.fd = fd_order;
+    p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi;
+    p.qmax = (int)(mg.m1 - M / 2);
+    p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
+
+    int tile = 256;
+    while (tile > 64 && ((d.n + tile - 1) / tile) * batch < 2 * 148) tile /= 2; /* fill the 148 SMs */
+    int dev = 0, smem_max = 0;
+    LTDI_CUDA_OK(cudaGetDevice(&dev));
+    LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    bool stage = true;
+    size_t smem = 0;
+    for (;;) {
+        p.tile = tile;
+        p.yr = (int)(tile + mg.m2 + M / 2 + 1);
+        p.hw = (int)(p.yr + 2 * mg.m1 + 6 * mg.w + 2);
+        const int w = (int)mg.w;
+        size_t off = 0;
+        if (which != LTDI_RESPONSE_LFA) off += 6 * (size_t)p.yr;
+        p.off_yL = (int)off;
+        if (which != LTDI_RESPONSE_FULL) off += 3 * (size_t)(p.yr + 2 * w);
+        p.off_dL = (int)off;
+        if (which != LTDI_RESPONSE_FULL) off += 3 * (size_t)p.yr;
+        p.off_hs = (int)off;
+        if (stage) off += 2 * (size_t)p.hw;
+        smem = off * sizeof(double);
+        if (smem <= (size_t)smem_max) break;
+        if (stage) { stage = false; continue; }      /* very small dt: read the strain through L1 instead */
+        if (tile > 64) { tile /= 2; continue; }
+        return LTDI_EUNSUPPORTED;
+    }
+    p.ntiles = (d.n + tile - 1) / tile;
+    const int threads = tile >= 256 ? 256 : 128;
+    if (M == 32)
+        return stage ? launch_response<32, true>(p, threads, smem, st) : launch_response<32, false>(p, threads, smem, st);
+    if (M == 10)
+        return stage ? launch_response<10, true>(p, threads, smem, st) : launch_response<10, false>(p, threads, smem, st);
+    return stage ? launch_response<0, true>(p, threads, smem, st) : launch_response<0, false>(p, threads, smem, st);
+}
+
+} // namespace
+
+extern "C" {
+
+int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes)
+{
+    if (!desc_ok(desc) || !bytes) return LTDI_EINVAL;
+    *bytes = (size_t)table_stride(desc->n) * LTDI_TABLE_ROWS * sizeof(double);
+    return LTDI_OK;
+}
+
+int ltdi_orbits_init(const ltdi_orbit_desc *desc, void *d_tables, size_t bytes, void *stream, ltdi_orbits **out)
+{
+    if (desc && desc->mode == LTDI_ORBIT_TABLES) return LTDI_EINVAL;
+    return orbits_common(desc, nullptr, nullptr, d_tables, bytes, stream, out);
+}
+
+int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L, void *d_tables,
+                            size_t bytes, void *stream, ltdi_orbits **out)
+{
+    if (!desc || desc->mode != LTDI_ORBIT_TABLES || !d_R || !d_L) return LTDI_EINVAL;
+    return orbits_common(desc, d_R, d_L, d_tables, bytes, stream, out);
+}
+
+int ltdi_orbits_destroy(ltdi_orbits *orb)
+{
+    delete orb;
+    return LTDI_OK;
+}
+
+int64_t ltdi_orbits_stride(const ltdi_orbits *orb) { return orb ? orb->stride : 0; }
+const double *ltdi_orbits_tables(const ltdi_orbits *orb) { return orb ? orb->d_tab : nullptr; }
+
+int ltdi_margins(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi)
+{
+    if (!desc_ok(desc) || !gen_ok(gen) || !order_ok(lagrange_order) || !lo || !hi) return LTDI_EINVAL;
+    if (fd_order != 0 && fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
+    const Margins m = compute_margins(*desc, gen, lagrange_order, fd_order);
+    *lo = m.lo;
+    *hi = m.hi;
+    return LTDI_OK;
+}
+
+int ltdi_link_margins(const ltdi_orbit_desc *desc, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi)
+{
+    if (!desc_ok(desc) || !order_ok(lagrange_order) || !lo || !hi) return LTDI_EINVAL;
+    if (fd_order != 0 && fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
+    const Margins m = compute_margins(*desc, LTDI_GEN_15, lagrange_order, fd_order);
+    *lo = m.m1 + m.w;
+    *hi = m.m1 + m.w;
+    return LTDI_OK;
+}
+
+int ltdi_hyb_time(double f_hyb_hz, double mchirp_s, double t_c, double *t_hyb)
+{
+    if (!t_hyb || !(f_hyb_hz > 0.0) || !(mchirp_s > 0.0)) return LTDI_EINVAL;
+    *t_hyb = t_c - 5.0 * std::pow(8.0 * 3.14159265358979323846 * f_hyb_hz, -8.0 / 3.0) * std::pow(mchirp_s, -5.0 / 3.0);
+    return LTDI_OK;
+}
+
+int ltdi_workspace_bytes(int which, int64_t n, int64_t batch, int gen, int lagrange_order, size_t *bytes)
+{
+    if (which < LTDI_RESPONSE_FULL || which > LTDI_RESPONSE_HYBRID || n < 1 || batch < 1 || !bytes) return LTDI_EINVAL;
+    if (!gen_ok(gen) || !order_ok(lagrange_order)) return LTDI_EINVAL;
+    *bytes = (work_doubles(batch) * sizeof(double) + 255) / 256 * 256;
+    return LTDI_OK;
+}
+
+int ltdi_response_full(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                       const ltdi_source *h_src, int gen, int lagrange_order, double *d_A, double *d_E, double *d_T,
+                       double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_FULL, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0,
+                        d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream);
+}
+
+int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                      const ltdi_source *h_src, int gen, int lagrange_order, int fd_order, double *d_A, double *d_E,
+                      double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
+                        0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream);
+}
+
+int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                         const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                         const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T,
+                         double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_HYBRID, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order,
+                        h_hyb, n_hyb, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream);
+}
+
+int64_t ltdi_launch_count(void) { return g_launches.load(); }
+const char *ltdi_version(void) { return "lisatdi-b200 0.1 (sm_100a, fp64)"; }
+
+} // extern "C"
