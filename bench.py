@@ -1,0 +1,290 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the time-domain LISA response hot path on B200 (one JSON line).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg4s|...]
+
+A *step* is one pass of the whole hot path over one batch of synthetic input:
+the orbit/delay kernel, then the full, LFA and hybrid responses (TDI 2.0, Lagrange order 31) of the
+workload.  The default workload is BASELINE.json configs[1] ("cfg2": one MBHB merger, 30 days at dt = 5 s,
+518 400 samples).  metric = TDI output samples/s: (samples x sources x 3 responses x ranks) / step time.
+
+--impl reference times the CPU oracle (oracle/, as it stands, double build) on a bounded sample of the
+same workload on the host cores; it is the deliberately slow baseline, not a target.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+GEN, FD = 20, 2
+# algorithmic flops per output sample (SURVEY.md 8(a)/(d), M = order + 1 taps; stated in DESIGN.md):
+#   full 2.0: 72 M + 252 M + 200,  LFA: 60 M + 150
+FLOPS_FULL = lambda M: 72 * M + 252 * M + 200
+FLOPS_LFA = lambda M: 60 * M + 150
+
+WORKLOADS = {
+    # name: (config index, n, batch)  -- None = BASELINE.json size
+    "cfg2": (2, None, None),
+    "cfg1": (1, None, None),
+    "cfg4s": (4, None, 256),     # a 256-source slice of config 4 (the full 4096 x 131072 needs 21 GB of buffers)
+    "cfg5s": (5, None, 16),
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def make_inputs(workload, rank):
+    import workloads as W
+    k, n, batch = WORKLOADS[workload]
+    cfg = W.config(k, n=n, batch=batch)
+    idx = [rank * cfg["batch"] + i for i in range(cfg["batch"])]   # every rank gets its own sources
+    hp, hc, ang, metas = W.sources(cfg, idx)
+    return cfg, hp, hc, ang, metas
+
+
+def windows(metas, hyb_time):
+    return [{"t_hyb": hyb_time(m["f_hyb_hz"], m["mchirp_s"], m["t_c"]), "window_s": m["window_s"],
+             "sigma_s": m["window_s"] / 40.0, "taper": m["taper"]} for m in metas]
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.count(",") >= 8]
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        sm = [float(r[1]) for r in rows]
+        out["sm_mhz"] = float(np.median(sm))
+        out["sm_max_mhz"] = float(rows[0][2])
+        out["power_w_max"] = max(float(r[3]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        out["reasons"] = [nm for i, nm in enumerate(names) if any(r[5 + i].strip() == "Active" for r in rows)]
+        out["samples"] = len(rows)
+        return out
+
+
+def cpu_baseline(cfg, hp, hc, ang, metas, budget_samples):
+    """The oracle as it stands (double build, OpenMP) on a bounded tail sample of source 0."""
+    import workloads as W
+    from oracle import Oracle
+    orc = Oracle("f64")
+    n = min(cfg["n"], budget_samples)
+    a = cfg["n"] - n
+    orbit = W.orbit_desc(n, cfg["dt"], cfg["mode"], t0=cfg["orbit"]["t0"] + a * cfg["dt"])
+    h0, h1 = np.ascontiguousarray(hp[:1, a:]), np.ascontiguousarray(hc[:1, a:])
+    hyb = windows(metas[:1], orc.hyb_time)
+    order = cfg["order"]
+    t0 = time.perf_counter()
+    orc.response_full(orbit, h0, h1, ang[:1], GEN, order, want=())
+    orc.response_lfa(orbit, h0, h1, ang[:1], GEN, order, FD, want=())
+    orc.response_hybrid(orbit, h0, h1, ang[:1], GEN, order, FD, hyb, want=())
+    sec = time.perf_counter() - t0
+    return {"value": 3 * n / sec, "unit": "TDI samples/s", "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"last {n} samples of source 0 of {cfg['name']}: full + LFA + hybrid, TDI 2.0, order {order}, "
+                      f"double build, {sec:.1f} s"}, sec
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    cfg, hp, hc, ang, metas = make_inputs(args.workload, 0)
+    sample = 20000
+    for _ in range(args.warmup):
+        cpu_baseline(cfg, hp, hc, ang, metas, 2000)
+    secs, base = [], None
+    for _ in range(args.steps):
+        base, s = cpu_baseline(cfg, hp, hc, ang, metas, sample)
+        secs.append(s)
+    n = min(cfg["n"], sample)
+    value = 3 * n * len(secs) / sum(secs)
+    base["value"] = value
+    line = {"impl": "reference", "metric": "TDI output samples/s (full + LFA + hybrid)", "value": value,
+            "unit": "TDI samples/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * sum(secs) / len(secs), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "sample": base["sample"]},
+            "cpu_baseline": base,
+            "e2e": {"value": value, "unit": "TDI samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2505_09600_b200 as ltdi
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, hp, hc, ang, metas = make_inputs(args.workload, rank)
+    n, batch, order = cfg["n"], cfg["batch"], cfg["order"]
+    M = order + 1
+    hyb = windows(metas, ltdi.hyb_time)
+    hp_host, hc_host = torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory()
+    d_hp, d_hc = hp_host.to(dev), hc_host.to(dev)
+    ws = ltdi.Workspace(batch, n, dev)
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # 256 MB > 126 MB L2
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    per_call = {"orbit": [], "full": [], "lfa": [], "hybrid": []}
+
+    def step(record):
+        nonlocal orb
+        marks = [ev() for _ in range(5)]
+        marks[0].record()
+        orb = ltdi.Orbits(cfg["orbit"], device=dev)                                        # S0
+        marks[1].record()
+        ltdi.response_full(orb, d_hp, d_hc, ang, GEN, order, workspace=ws)                 # S1-S5
+        marks[2].record()
+        ltdi.response_lfa(orb, d_hp, d_hc, ang, GEN, order, FD, workspace=ws)              # S6-S7
+        marks[3].record()
+        ltdi.response_hybrid(orb, d_hp, d_hc, ang, GEN, order, FD, hyb, workspace=ws)      # S8
+        marks[4].record()
+        if record:
+            return marks
+        return None
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        step(False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = ltdi.launch_count()
+    all_marks = []
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.zero_()                      # evict the 126 MB L2 between timed steps (outside the events)
+        all_marks.append(step(True))
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    launches = ltdi.launch_count() - launches0
+    if world > 1:
+        dist.barrier()
+    clk = clocks.stop() if clocks else None
+    step_ms = []
+    for m in all_marks:
+        step_ms.append(m[0].elapsed_time(m[4]))
+        for name, i in (("orbit", 0), ("full", 1), ("lfa", 2), ("hybrid", 3)):
+            per_call[name].append(m[i].elapsed_time(m[i + 1]))
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_ms = float(total_ms.item())
+    ms_per_step = total_ms / args.steps
+    samples_per_step = 3 * n * batch * world
+    value = samples_per_step / (ms_per_step * 1e-3)
+
+    # end to end: host buffers in, host A, E, T out, through ltdi_response_host (copies inside the timed region)
+    pipe = ltdi.HostPipeline(orb, batch, n)
+    for _ in range(2):
+        pipe.run(ltdi.RESPONSE_FULL, hp_host, hc_host, ang, GEN, order)
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    k_e2e = max(3, min(args.steps, 10))
+    e0.record()
+    for _ in range(k_e2e):
+        pipe.run(ltdi.RESPONSE_FULL, hp_host, hc_host, ang, GEN, order)
+        pipe.run(ltdi.RESPONSE_LFA, hp_host, hc_host, ang, GEN, order, FD)
+        pipe.run(ltdi.RESPONSE_HYBRID, hp_host, hc_host, ang, GEN, order, FD, hyb)
+    e1.record()
+    e1.synchronize()
+    e2e_ms = torch.tensor([e0.elapsed_time(e1) / k_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+    e2e_value = samples_per_step / (float(e2e_ms.item()) * 1e-3)
+
+    if rank == 0:
+        # roofline of the dominant kernel: the fused response kernel in its full-response launch
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        dfma_rate = ltdi.fp64_probe(device=dev)
+        peak_tflops = 2.0 * dfma_rate / 1e12
+        full_ms = float(np.mean(per_call["full"]))
+        flops_launch = FLOPS_FULL(M) * n * batch
+        achieved = flops_launch / (full_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "response_kernel (full response launch)",
+                    "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                    "traffic": None,
+                    "peak_source": "DFMA chain probe measured in this run (2 flop per DFMA); nominal 148 SM x 64 DFMA/clk",
+                    "hbm_gbs_measured": peaks.get("hbm_gbs"),
+                    "per_call_ms": {k: float(np.mean(v)) for k, v in per_call.items()},
+                    "lfa_tflops": FLOPS_LFA(M) * n * batch / (float(np.mean(per_call["lfa"])) * 1e-3) / 1e12,
+                    "orbit_gbs": 192.0 * n / (float(np.mean(per_call["orbit"])) * 1e-3) / 1e9}
+        line = {"metric": "TDI output samples/s (full + LFA + hybrid)", "value": value, "unit": "TDI samples/s",
+                "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic",
+                "config": {"workload": cfg["name"], "samples": n, "sources_per_gpu": batch, "dt_s": cfg["dt"],
+                           "tdi": "2.0", "lagrange_order": order, "fd_order": FD, "responses": "full+lfa+hybrid",
+                           "orbit_kernel_in_step": True, "l2": "flushed between steps (256 MB write)",
+                           "wall_s_timed_region": wall},
+                "clocks": clk, "gpu_launches": int(launches),
+                "e2e": {"value": e2e_value, "unit": "TDI samples/s", "h2d_bytes_per_step": 3 * pipe.h2d_bytes,
+                        "d2h_bytes_per_step": 3 * pipe.d2h_bytes},
+                "roofline": roofline}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"], _ = cpu_baseline(cfg, hp, hc, ang, metas, 60000)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

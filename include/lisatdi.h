@@ -142,6 +142,24 @@ int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const doubl
                          double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes,
                          void *stream);
 
+/* End-to-end variant (the call a host application makes): h_hp, h_hc [batch][ld] and h_A, h_E, h_T
+ * [batch][ld] are HOST buffers (pinned memory makes the copies asynchronous).  The call enqueues, on
+ * `stream`, the host->device copies of the strain, the response `which` (LTDI_RESPONSE_*; fd_order and
+ * h_hyb / n_hyb as in the calls above, ignored where they do not apply) and the device->host copies of
+ * A, E, T.  d_scratch: device scratch of ltdi_host_scratch_bytes() bytes, 256-byte aligned.  Results
+ * are valid after the stream is synchronised. */
+int ltdi_host_scratch_bytes(int64_t ld, int64_t batch, size_t *bytes);
+int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, const double *h_hc, int64_t ld,
+                       int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                       const ltdi_hybrid *h_hyb, int64_t n_hyb, double *h_A, double *h_E, double *h_T,
+                       void *d_scratch, size_t scratch_bytes, void *stream);
+
+/* FP64 pipe probe for the roofline denominator: launches a register-resident chain of
+ * fused multiply-adds (blocks x 256 threads, 8 independent chains per thread, iters x 64 DFMA per
+ * chain step) and writes one value per thread to d_out (blocks * 256 doubles).  *dfma_per_launch
+ * receives the number of DFMA the launch executes. */
+int ltdi_fp64_probe(double *d_out, int blocks, int iters, void *stream, double *dfma_per_launch);
+
 /* Number of kernel launches the library has issued in this process (for bench.py's gpu_launches). */
 int64_t ltdi_launch_count(void);
 const char *ltdi_version(void);

@@ -86,6 +86,9 @@ class Oracle:
             arr[i] = _Source(b, l, p)
         return arr, len(s)
 
+    def num_threads(self):
+        return self.lib.orc_num_threads()
+
     def mant_dig(self):
         return self.lib.orc_real_mant_dig()
 

@@ -556,6 +556,12 @@ static int check_args(const orc_orbit_desc *d, int gen, int order, int fd_order,
 /* ---- exported API ---------------------------------------------------------------- */
 
 int orc_real_bits(void) { return (int)(sizeof(real) * 8); }
+#ifdef _OPENMP
+#include <omp.h>
+int orc_num_threads(void) { return omp_get_max_threads(); }
+#else
+int orc_num_threads(void) { return 1; }
+#endif
 int orc_real_mant_dig(void)
 {
 #ifdef ORC_REAL_LD

@@ -73,6 +73,10 @@ _SIGNATURES = {
     "ltdi_response_hybrid": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                        C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _dp, _dp, _vp,
                                        C.c_size_t, _vp]),
+    "ltdi_host_scratch_bytes": (C.c_int, [C.c_int64, C.c_int64, _szp]),
+    "ltdi_response_host": (C.c_int, [C.c_int, _vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                     C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_fp64_probe": (C.c_int, [_dp, C.c_int, C.c_int, _vp, C.POINTER(C.c_double)]),
     "ltdi_launch_count": (C.c_int64, []),
     "ltdi_version": (C.c_char_p, []),
 }
@@ -248,3 +252,51 @@ def response_hybrid(orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz
     """Eqs. (4.5), (4.6): LFA spliced to the full response; hybrid = dict or list of dicts
     {t_hyb, window_s, sigma_s, taper}."""
     return _run(RESPONSE_HYBRID, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, want_y, workspace)
+
+
+def _hybrid_array(hybrid):
+    if hybrid is None:
+        return None, 0
+    hl = hybrid if isinstance(hybrid, (list, tuple)) else [hybrid]
+    return (Hybrid * len(hl))(*[Hybrid(h["t_hyb"], h["window_s"], h["sigma_s"], int(h["taper"])) for h in hl]), len(hl)
+
+
+class HostPipeline:
+    """End-to-end call with HOST buffers (ltdi_response_host): pinned strain in, pinned A, E, T out."""
+
+    def __init__(self, orb, batch, ld):
+        self.orb, self.batch, self.ld = orb, batch, ld
+        nbytes = C.c_size_t()
+        _check("ltdi_host_scratch_bytes", lib().ltdi_host_scratch_bytes(ld, batch, C.byref(nbytes)))
+        self.scratch = torch.empty(nbytes.value // 8, dtype=torch.float64, device=orb.device)
+        self.A, self.E, self.T = (torch.empty(batch, ld, dtype=torch.float64).pin_memory() for _ in range(3))
+        self.h2d_bytes = 2 * batch * ld * 8
+        self.d2h_bytes = 3 * batch * ld * 8
+
+    def run(self, which, hp_host, hc_host, sources, gen, order, fd_order=2, hybrid=None):
+        assert hp_host.dtype == torch.float64 and not hp_host.is_cuda and hp_host.is_contiguous()
+        src_ptr, keep = _sources(sources)
+        harr, nh = _hybrid_array(hybrid)
+        with torch.cuda.device(self.orb.device):
+            rc = lib().ltdi_response_host(which, self.orb.handle, hp_host.data_ptr(), hc_host.data_ptr(), self.ld,
+                                          self.batch, src_ptr, gen, order, fd_order, harr, nh, self.A.data_ptr(),
+                                          self.E.data_ptr(), self.T.data_ptr(), self.scratch.data_ptr(),
+                                          self.scratch.numel() * 8, _stream())
+        _check("ltdi_response_host", rc)
+        return self.A, self.E, self.T
+
+
+def fp64_probe(blocks=148 * 8, iters=2000, repeats=5, device="cuda:0"):
+    """Measured DFMA issue rate [DFMA/s] of the device (register-resident chains, CUDA events)."""
+    out = torch.empty(blocks * 256, dtype=torch.float64, device=device)
+    n = C.c_double()
+    best = 0.0
+    with torch.cuda.device(out.device):
+        for _ in range(repeats + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            _check("ltdi_fp64_probe", lib().ltdi_fp64_probe(out.data_ptr(), blocks, iters, _stream(), C.byref(n)))
+            e1.record()
+            e1.synchronize()
+            best = max(best, n.value / (e0.elapsed_time(e1) * 1e-3))
+    return best

@@ -230,9 +230,76 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     return stage ? launch_response<0, true>(p, threads, smem, st) : launch_response<0, false>(p, threads, smem, st);
 }
 
+// register-resident DFMA chains: the FP64 pipe's issue rate, used as the "alu" roofline peak
+__global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters)
+{
+    double a[8];
+    const double x = 1.0 + 1e-9 * (double)threadIdx.x, y = 1e-12 * (double)(blockIdx.x + 1);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = (double)i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = fma(a[i], x, y);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 } // namespace
 
 extern "C" {
+
+int ltdi_fp64_probe(double *d_out, int blocks, int iters, void *stream, double *dfma_per_launch)
+{
+    if (!d_out || blocks < 1 || iters < 1) return LTDI_EINVAL;
+    fp64_probe_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(d_out, iters);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    if (dfma_per_launch) *dfma_per_launch = (double)blocks * 256.0 * 64.0 * (double)iters;
+    return LTDI_OK;
+}
+
+int ltdi_host_scratch_bytes(int64_t ld, int64_t batch, size_t *bytes)
+{
+    if (ld < 1 || batch < 1 || !bytes) return LTDI_EINVAL;
+    const size_t series = ((size_t)ld * (size_t)batch * sizeof(double) + 255) / 256 * 256;
+    *bytes = 5 * series + (work_doubles(batch) * sizeof(double) + 255) / 256 * 256;
+    return LTDI_OK;
+}
+
+int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, const double *h_hc, int64_t ld,
+                       int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                       const ltdi_hybrid *h_hyb, int64_t n_hyb, double *h_A, double *h_E, double *h_T,
+                       void *d_scratch, size_t scratch_bytes, void *stream)
+{
+    if (!h_hp || !h_hc || !h_A || !h_E || !h_T || !d_scratch || ld < 1 || batch < 1) return LTDI_EINVAL;
+    if (which < LTDI_RESPONSE_FULL || which > LTDI_RESPONSE_HYBRID) return LTDI_EINVAL;
+    if ((uintptr_t)d_scratch % 256) return LTDI_EINVAL;
+    size_t need = 0;
+    ltdi_host_scratch_bytes(ld, batch, &need);
+    if (scratch_bytes < need) return LTDI_EWORKSPACE;
+    const size_t bytes = (size_t)ld * (size_t)batch * sizeof(double);
+    const size_t series = (bytes + 255) / 256 * 256;
+    char *base = (char *)d_scratch;
+    double *d_hp = (double *)base, *d_hc = (double *)(base + series);
+    double *d_A = (double *)(base + 2 * series), *d_E = (double *)(base + 3 * series), *d_T = (double *)(base + 4 * series);
+    void *d_work = base + 5 * series;
+    cudaStream_t st = (cudaStream_t)stream;
+    LTDI_CUDA_OK(cudaMemcpyAsync(d_hp, h_hp, bytes, cudaMemcpyHostToDevice, st));
+    LTDI_CUDA_OK(cudaMemcpyAsync(d_hc, h_hc, bytes, cudaMemcpyHostToDevice, st));
+    const int rc = run_response(which, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, h_hyb,
+                                n_hyb, d_A, d_E, d_T, nullptr, nullptr, d_work, need - 5 * series, stream);
+    if (rc) return rc;
+    LTDI_CUDA_OK(cudaMemcpyAsync(h_A, d_A, bytes, cudaMemcpyDeviceToHost, st));
+    LTDI_CUDA_OK(cudaMemcpyAsync(h_E, d_E, bytes, cudaMemcpyDeviceToHost, st));
+    LTDI_CUDA_OK(cudaMemcpyAsync(h_T, d_T, bytes, cudaMemcpyDeviceToHost, st));
+    return LTDI_OK;
+}
 
 int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes)
 {

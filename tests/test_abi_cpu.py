@@ -1,0 +1,75 @@
+"""CPU-side checks of the C-ABI library (no GPU): it loads, exports every symbol include/lisatdi.h
+declares, and its host-only helpers (margins, Eq. 4.2) agree with the oracle's independent versions."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def ltdi():
+    import paper_2505_09600_b200 as m
+    m.lib()
+    return m
+
+
+def test_library_exports_every_declared_symbol(ltdi):
+    header = open(os.path.join(ROOT, "include", "lisatdi.h")).read()
+    declared = set(re.findall(r"\b(ltdi_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations found"
+    handle = C.CDLL(ltdi._build.LIB)
+    for name in sorted(declared):
+        assert hasattr(handle, name), name
+    assert declared == set(ltdi.EXPORTS)
+
+
+def test_margins_match_the_oracle(ltdi, orc80):
+    for dt in (1.0, 5.0, 10.0, 15.0):
+        for order in (1, 9, 31, 63):
+            for gen in (15, 20):
+                for fd in (0, 2, 4):
+                    d = W.orbit_desc(100000, dt)
+                    assert ltdi.margins(d, gen, order, fd) == orc80.margins(d, gen, order, fd)
+                    assert ltdi.link_margins(d, order, fd) == orc80.link_margins(d, order, fd)
+
+
+def test_hyb_time_matches_the_oracle(ltdi, orc80):
+    for M, q, f in ((1e6, 1.0, 2e-3), (1e5, 9.0, 2e-3), (7e6, 3.0, 3e-4)):
+        mc = W.chirp_mass_s(M, q)
+        a, b = ltdi.hyb_time(f, mc, 2.5e6), orc80.hyb_time(f, mc, 2.5e6)
+        assert abs(a - b) <= 1e-9 * abs(2.5e6 - b)
+
+
+def test_invalid_arguments_are_reported_not_raised_across_the_abi(ltdi):
+    lib = ltdi.lib()
+    d = ltdi._desc(W.orbit_desc(1000, 5.0))
+    lo, hi = C.c_int64(), C.c_int64()
+    assert lib.ltdi_margins(C.byref(d), 17, 31, 0, C.byref(lo), C.byref(hi)) == ltdi.EINVAL      # bad generation
+    assert lib.ltdi_margins(C.byref(d), 20, 30, 0, C.byref(lo), C.byref(hi)) == ltdi.EINVAL      # even order
+    assert lib.ltdi_margins(C.byref(d), 20, 65, 0, C.byref(lo), C.byref(hi)) == ltdi.EINVAL      # order > 63
+    assert lib.ltdi_margins(C.byref(d), 20, 31, 3, C.byref(lo), C.byref(hi)) == ltdi.EINVAL      # bad stencil
+    nbytes = C.c_size_t()
+    bad = ltdi._desc(W.orbit_desc(0, 5.0))
+    assert lib.ltdi_orbits_workspace_bytes(C.byref(bad), C.byref(nbytes)) == ltdi.EINVAL
+    assert lib.ltdi_orbits_workspace_bytes(C.byref(d), C.byref(nbytes)) == ltdi.OK
+    assert nbytes.value == 24 * 1024 * 8                                                           # rows padded to 32
+    out = C.c_double()
+    assert lib.ltdi_hyb_time(-1.0, 1.0, 0.0, C.byref(out)) == ltdi.EINVAL
+    # NULL required pointers: rejected before any CUDA call
+    assert lib.ltdi_response_full(None, None, None, 10, 1, None, 20, 31, None, None, None, None, None, None, 0,
+                                  None) == ltdi.EINVAL
+    assert lib.ltdi_fp64_probe(None, 1, 1, None, None) == ltdi.EINVAL
+    assert ltdi.launch_count() == 0
+
+
+def test_no_cpu_fallback(ltdi):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(RuntimeError):
+        ltdi.Orbits(W.orbit_desc(100, 5.0))

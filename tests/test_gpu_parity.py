@@ -1,0 +1,176 @@
+"""GPU parity: the CUDA path (through the C ABI) against the long-double oracle, element by element, on
+the same seeded inputs.  Bar: per-channel relative L2 <= 1e-11 over the non-margin samples (BASELINE.json
+north_star); margins must be exactly 0.0."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from parity_util import TOL, channel_errors, hybrid_params, series_errors, to_numpy
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ltdi():
+    import paper_2505_09600_b200 as m
+    assert torch.cuda.is_available(), "GPU parity tests need a CUDA device"
+    return m
+
+
+def run_case(ltdi, orc, cfg, which, gen, fd, order=None, taper=W.TAPER_COSINE, idx=None, ld_pad=0):
+    n, batch = cfg["n"], cfg["batch"]
+    order = order or cfg["order"]
+    idx = list(range(batch)) if idx is None else idx
+    hp, hc, ang, metas = W.sources(cfg, idx)
+    orbit = cfg["orbit"]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    if ld_pad:
+        pad = np.full((len(idx), ld_pad), 7.0)   # columns beyond n must never be read or written
+        dhp = torch.from_numpy(np.concatenate([hp, pad], 1)).to(dev)
+        dhc = torch.from_numpy(np.concatenate([hc, pad], 1)).to(dev)
+    else:
+        dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    if which == "full":
+        ref = orc.response_full(orbit, hp, hc, ang, gen, order)
+        out = ltdi.response_full(orb, dhp, dhc, ang, gen, order, True, True)
+    elif which == "lfa":
+        ref = orc.response_lfa(orbit, hp, hc, ang, gen, order, fd)
+        out = ltdi.response_lfa(orb, dhp, dhc, ang, gen, order, fd, True, True)
+    else:
+        ref = orc.response_hybrid(orbit, hp, hc, ang, gen, order, fd, hybrid_params(metas, orc.hyb_time, taper, cfg["dt"]))
+        out = ltdi.response_hybrid(orb, dhp, dhc, ang, gen, order, fd,
+                                   hybrid_params(metas, ltdi.hyb_time, taper, cfg["dt"]), True, True)
+    torch.cuda.synchronize()
+    out = to_numpy(out)
+    for k in out:
+        out[k] = out[k][..., :n]
+    lo, hi = orc.margins(orbit, gen, order, fd)
+    assert (lo, hi) == ltdi.margins(orbit, gen, order, fd)
+    return out, ref, lo, hi
+
+
+def check(out, ref, lo, hi, n, tol=TOL):
+    for c in "AET":   # margins are exactly zero
+        assert np.all(out[c][:, :lo] == 0.0) and np.all(out[c][:, n - hi:] == 0.0), c
+    errs = channel_errors(out, ref, lo, n, hi)
+    for c, (e, near_null) in errs.items():
+        assert e <= tol, (c, e, "near-null" if near_null else "")
+    for name in ("XYZ", "y"):
+        for i, e in enumerate(series_errors(out[name], ref[name], lo, n, hi)):
+            assert e <= tol, (name, i, e)
+    return errs
+
+
+def test_orbit_delay_kernel(ltdi, orc80):
+    """S0: tables against the oracle's orbit (differences come from sincos rounding only)"""
+    for mode in (W.ORBIT_KEPLERIAN, W.ORBIT_STATIC_EQUALARM):
+        orbit = W.orbit_desc(70001, 5.0, mode, t0=1.0e7, alpha0=0.3, rot0=1.1)
+        R, nh, L = orc80.orbit_tables(orbit)
+        rows = ltdi.Orbits(orbit).rows().cpu().numpy()
+        assert np.abs(rows[0:9].reshape(3, 3, -1) - R).max() <= 4e-16 * np.abs(R).max()
+        assert np.abs(rows[9:18].reshape(3, 3, -1) - nh[:3]).max() <= 2e-14
+        assert np.abs(rows[18:24] - L).max() <= 1e-14 * L.max()
+        assert np.array_equal(nh[3:], -nh[:3])        # n_-l = -n_l is what the table layout assumes
+
+
+def test_config1_full_tdi15(ltdi, orc80):
+    cfg = W.config(1)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, "full", 15, 0)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("which,gen,taper", [("full", 20, 0), ("full", 15, 0), ("lfa", 20, 0), ("lfa", 15, 0),
+                                             ("hybrid", 20, W.TAPER_COSINE), ("hybrid", 20, W.TAPER_SIGMOID),
+                                             ("hybrid", 15, W.TAPER_COSINE)])
+def test_config2_merger(ltdi, orc80, which, gen, taper):
+    """config 2 shortened to its last 40 000 samples (several tiles, ragged tail, merger + ringdown)"""
+    cfg = W.config(2, n=40007)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, which, gen, 2, taper=taper)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("gen", [15, 20])
+@pytest.mark.parametrize("fd", [2, 4])
+def test_config3_long_inspiral_lfa(ltdi, orc80, gen, fd):
+    cfg = W.config(3, n=30011)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, "lfa", gen, fd)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+def test_config4_batch_hybrid(ltdi, orc80):
+    """config 4 slice: 40 sources (the > 32 sources parameter path) of 20 001 samples, per-source windows"""
+    cfg = W.config(4, n=20001, batch=40)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, "hybrid", 20, 2)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("which", ["full", "lfa"])
+def test_config5_eccentric(ltdi, orc80, which):
+    cfg = W.config(5, n=65536, batch=2)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, which, 20, 2)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("order", [1, 5, 13, 63])
+def test_generic_lagrange_orders(ltdi, orc80, order):
+    cfg = W.config(2, n=5003, batch=2)
+    for which in ("full", "lfa"):
+        out, ref, lo, hi = run_case(ltdi, orc80, cfg, which, 20, 4, order=order, ld_pad=13)
+        check(out, ref, lo, hi, cfg["n"])
+
+
+def test_series_shorter_than_the_margins_is_all_zero(ltdi, orc80):
+    cfg = W.config(2, n=200)
+    out, ref, lo, hi = run_case(ltdi, orc80, cfg, "full", 20, 0)
+    assert lo + hi > cfg["n"]
+    for c in "AET":
+        assert np.all(out[c] == 0.0) and np.all(ref[c] == 0.0)
+
+
+def test_frozen_tables_mode(ltdi, orc80):
+    """LTDI_ORBIT_TABLES with caller-supplied positions and light times"""
+    n, dt = 4000, 5.0
+    snap = W.orbit_desc(1, 1.0, W.ORBIT_KEPLERIAN, t0=0.37 * W.YEAR_S)
+    R, _, L = orc80.orbit_tables(snap)
+    orbit = W.frozen_tables(W.orbit_desc(n, dt), R[:, :, 0], L[:, 0])
+    hp, hc = W.monochromatic(n, dt, 3e-3)
+    ang = [(0.3, 1.0, 0.7)]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, torch.from_numpy(orbit["R_table"]).to(dev), torch.from_numpy(orbit["L_table"]).to(dev))
+    out = to_numpy(ltdi.response_full(orb, torch.from_numpy(hp[None]).to(dev), torch.from_numpy(hc[None]).to(dev),
+                                      ang, 20, 31, True, True))
+    ref = orc80.response_full(orbit, hp[None], hc[None], ang, 20, 31)
+    lo, hi = orc80.margins(orbit, 20, 31, 0)
+    check(out, ref, lo, hi, n)
+
+
+def test_errors_from_the_device_entry_points(ltdi):
+    dev = torch.device("cuda:0")
+    orbit = W.orbit_desc(3000, 5.0)
+    orb = ltdi.Orbits(orbit, device=dev)
+    h = torch.zeros(1, 3000, dtype=torch.float64, device=dev)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.response_full(orb, h, h, [(0, 0, 0)], 17, 31)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.response_lfa(orb, h, h, [(0, 0, 0)], 20, 31, 3)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.response_full(orb, h[:, :2000].contiguous(), h[:, :2000].contiguous(), [(0, 0, 0)], 20, 31)  # ld < n
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.response_hybrid(orb, h, h, [(0, 0, 0)], 20, 31, 2,
+                             {"t_hyb": 0.0, "window_s": -1.0, "sigma_s": 1.0, "taper": 0})
+
+
+def test_host_pipeline_matches_device_call(ltdi):
+    """ltdi_response_host (host buffers in and out) gives bit-identical A, E, T"""
+    dev = torch.device("cuda:0")
+    cfg = W.config(2, n=9000, batch=3)
+    hp, hc, ang, metas = W.sources(cfg, [0, 1, 2])
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    ref = ltdi.response_lfa(orb, torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev), ang, 20, 31, 2)
+    pipe = ltdi.HostPipeline(orb, 3, 9000)
+    A, E, T = pipe.run(ltdi.RESPONSE_LFA, torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory(), ang,
+                       20, 31, 2)
+    torch.cuda.synchronize()
+    assert torch.equal(A, ref["A"].cpu()) and torch.equal(E, ref["E"].cpu()) and torch.equal(T, ref["T"].cpu())
