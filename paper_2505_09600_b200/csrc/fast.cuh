@@ -1,0 +1,789 @@
+// fast.cuh -- the tuned sm_100a path for Lagrange orders 9 and 31 (M = 10, 32 taps).
+//
+// Three kernels per response, the link series y_slr travelling through an L2-resident scratch:
+//
+//   anchor_kernel   per time tile of the TDI stage and per distinct TDI delay: integer shift q, and the
+//                   Lagrange weights w_k(eps_c) with their first and second derivatives at the tile-centre
+//                   delay.  The TDI delays (sums of L_l(t_n)) drift by < 1e-7 samples over a tile, so
+//                   w_k(eps_n) = w_k(eps_c) + D w_k' + D^2 w_k''/2 with D = eps_n - eps_c is exact to rounding
+//                   (|D| <= 1e-6 is checked per tile; a tile that fails, or whose q changes, takes the exact
+//                   per-sample weights instead).  The weights do not depend on the source: a batch shares them.
+//   link_kernel     S2 + S3 (Eq. 2.4-2.6) resp. S6 (Eq. B10): one thread owns TWO consecutive samples, builds
+//                   the per-sample weights of each of the 9 (3) retarded times from the symmetric pair form
+//                   below, and streams the shared 33-sample window of h+ / hx out of shared memory once for
+//                   both samples (the shared-memory pipe, not the FP64 pipe, limits a one-sample-per-thread
+//                   kernel: SURVEY.md section 7, hard part 4).
+//   tdi_kernel      S4 + S5 (Eq. 2.7-2.9) resp. S7 (B25/B33) and S8 (4.5/4.6): one thread owns SEVEN
+//                   consecutive samples of one Michelson channel and slides a 7-sample register window over
+//                   the link series (stride-7 shared-memory reads are conflict free), weights broadcast from
+//                   the anchors.
+//
+// Symmetric pair form of the Lagrange weights.  Taps k = -(H-1) .. H (M = 2H), eps in [0,1).  Pair j = 0..H-1
+// holds taps k = j+1 and k = -j, nodes +-(j+1/2) about u = eps - 1/2:
+//   prod_{m != k}(eps - m) = (eps + j) G_j      (k = j+1),      ((j+1) - eps) G_j * (-1)   (k = -j)
+//   G_j = prod_{i != j} g_i,   g_i = u^2 - (i+1/2)^2 = (eps + i)(eps - i - 1)
+// and 1 / prod_{m != k}(k - m) = +-c_j.  Scaling g_i by lambda_i with prod_{i != j} lambda_i = c_j folds the
+// denominators into the products: w_{j+1} = Gt_j (eps + j), w_{-j} = Gt_j (j + 1 - eps), Gt_j = prod_{i != j}
+// lambda_i g_i  -- 3.4 M flops per weight set instead of 5 M for prefix x suffix over all taps.
+#pragma once
+#include "common.cuh"
+
+#define FAST_TC_R 7                       /* samples per thread in the TDI kernel */
+#define FAST_TC_G 64                      /* thread groups per channel */
+#define FAST_TC (FAST_TC_R * FAST_TC_G)   /* 448 output samples per TDI tile */
+#define FAST_TC_THREADS (3 * FAST_TC_G)   /* 192 */
+#define FAST_TA_THREADS 192
+#define FAST_TA (2 * FAST_TA_THREADS)     /* 384 samples per link tile */
+#define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
+#define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
+#define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
+#define FAST_DMAX 1.0e-6                  /* |eps_n - eps_c| bound for the second-order weights */
+
+/* lambda_i and kappa_i = -lambda_i (i + 1/2)^2 for H = 5 (row 0) and H = 16 (row 1) */
+__constant__ double c_sym_lam[2][16];
+__constant__ double c_sym_kap[2][16];
+
+struct FastParams {
+    const double *tab;
+    int64_t stride, n;
+    double t0, dt, inv_dt;
+    const double *hp, *hc;
+    int64_t ld, batch;       /* batch = sources of this launch (a chunk) */
+    const double *frames;    /* [batch][LTDI_FRAME_STRIDE] of this chunk */
+    const double *hyb;       /* [n_hyb][4] of this chunk (t_hyb, window, sigma, taper) */
+    int64_t n_hyb;
+    int which, gen, fd;
+    int64_t m1, m2, w, lo, hi;
+    int qmax;
+    double *yF, *yL;         /* scratch link series [6][batch][lds], [3][batch][lds] */
+    int64_t lds;
+    double *A, *E, *T, *XYZ, *Y; /* outputs of this chunk ([batch][ld] ...), XYZ / Y strides use batch_all */
+    int64_t batch_all, b0;   /* full batch and first source of the chunk (for the [3][batch][ld] outputs) */
+    const double *anc;       /* [ntilesC][FAST_NA][M][4] */
+    const double *anc_hdr;   /* [ntilesC][FAST_NA][4]: d_c [s], q, eps_c, valid */
+    int64_t ntilesA, ntilesC;
+};
+
+// ---------------------------------------------------------------------------------------------
+// helpers
+// ---------------------------------------------------------------------------------------------
+// s = d / dt to within one rounding of the correctly rounded quotient (one Newton correction)
+__device__ __forceinline__ double div_dt(double d, double dt, double inv_dt)
+{
+    const double s0 = d * inv_dt;
+    const double r = fma(-s0, dt, d);
+    return fma(r, inv_dt, s0);
+}
+
+__device__ __forceinline__ void split_delay_fast(double d, double dt, double inv_dt, int &q, double &eps)
+{
+    const double s = div_dt(d, dt, inv_dt);
+    const double qc = ceil(s);
+    q = (int)qc;
+    eps = qc - s;
+}
+
+// generic exact weights (prefix x suffix over all taps), used by the rare slow paths
+template <int M>
+__device__ __noinline__ void lagrange_exact(double eps, double *w)
+{
+    const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
+    const int kmin = -(M / 2 - 1);
+    double run = 1.0;
+    for (int i = 0; i < M; ++i) {
+        w[i] = run;
+        run *= eps - (double)(kmin + i);
+    }
+    run = 1.0;
+    for (int i = M - 1; i >= 0; --i) {
+        w[i] = (w[i] * run) * c[i];
+        run *= eps - (double)(kmin + i);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the pair interpolator of the link kernel
+// ---------------------------------------------------------------------------------------------
+// Window W[i] = x[js + i], i = 0 .. M: sample 0 uses W[0..M-1], sample 1 uses W[1..M].  The staged series are
+// split by parity (even samples / odd samples), so that lanes that own consecutive sample PAIRS read
+// consecutive addresses.  W[i] = (i odd ? p1[(i-1)/2] : p0[i/2]).
+template <int H>
+__device__ __forceinline__ void interp_pair(double e0, double e1, const double *__restrict__ P0,
+                                            const double *__restrict__ P1, const double *__restrict__ C0,
+                                            const double *__restrict__ C1, double &ap0, double &ac0, double &ap1,
+                                            double &ac1)
+{
+    constexpr int row = (H == 16) ? 1 : 0;
+    const double uu0 = (e0 - 0.5) * (e0 - 0.5), uu1 = (e1 - 0.5) * (e1 - 0.5);
+    // suffix products S[j] = prod_{i > j} lambda_i g_i
+    double S0[H], S1[H];
+    S0[H - 1] = 1.0;
+    S1[H - 1] = 1.0;
+#pragma unroll
+    for (int j = H - 2; j >= 0; --j) {
+        const double g0 = fma(c_sym_lam[row][j + 1], uu0, c_sym_kap[row][j + 1]);
+        const double g1 = fma(c_sym_lam[row][j + 1], uu1, c_sym_kap[row][j + 1]);
+        S0[j] = S0[j + 1] * g0;
+        S1[j] = S1[j + 1] * g1;
+    }
+    // centre of the window
+#define W_AT(Q0, Q1, i) (((i) & 1) ? (Q1)[((i) - 1) >> 1] : (Q0)[(i) >> 1])
+    double plo = W_AT(P0, P1, H), clo = W_AT(C0, C1, H);
+    double phi = plo, chi = clo;
+    double a_p0 = 0.0, a_c0 = 0.0, a_p1 = 0.0, a_c1 = 0.0;
+    double pre0 = 1.0, pre1 = 1.0;
+#pragma unroll
+    for (int j = 0; j < H; ++j) {
+        const double G0 = pre0 * S0[j], G1 = pre1 * S1[j];
+        const double t0 = G0 * e0, t1 = G1 * e1;
+        const double w0p = fma(G0, (double)j, t0), w0m = fma(G0, (double)(j + 1), -t0); /* taps k = j+1, k = -j */
+        const double w1p = fma(G1, (double)j, t1), w1m = fma(G1, (double)(j + 1), -t1);
+        const double pl = W_AT(P0, P1, H - 1 - j), ph = W_AT(P0, P1, H + 1 + j);
+        const double cl = W_AT(C0, C1, H - 1 - j), ch = W_AT(C0, C1, H + 1 + j);
+        a_p0 = fma(w0m, pl, a_p0);
+        a_p0 = fma(w0p, phi, a_p0);
+        a_c0 = fma(w0m, cl, a_c0);
+        a_c0 = fma(w0p, chi, a_c0);
+        a_p1 = fma(w1m, plo, a_p1);
+        a_p1 = fma(w1p, ph, a_p1);
+        a_c1 = fma(w1m, clo, a_c1);
+        a_c1 = fma(w1p, ch, a_c1);
+        plo = pl; phi = ph; clo = cl; chi = ch;
+        if (j + 1 < H) {
+            if (j == 0) {
+                pre0 = c_sym_lam[row][0] * (e0 * (e0 - 1.0)); /* g_0 = eps (eps - 1): no cancellation near 0, 1 */
+                pre1 = c_sym_lam[row][0] * (e1 * (e1 - 1.0));
+            } else {
+                pre0 *= fma(c_sym_lam[row][j], uu0, c_sym_kap[row][j]);
+                pre1 *= fma(c_sym_lam[row][j], uu1, c_sym_kap[row][j]);
+            }
+        }
+    }
+#undef W_AT
+    ap0 = a_p0; ac0 = a_c0; ap1 = a_p1; ac1 = a_c1;
+}
+
+// one sample, taps ascending, exact weights: the pair's two samples have different integer shifts
+template <int H>
+__device__ __noinline__ void interp_single(double eps, const double *he_p, const double *ho_p, const double *he_c,
+                                           const double *ho_c, int js /* window start relative to the staged origin */,
+                                           double &ap, double &ac)
+{
+    double w[2 * H];
+    lagrange_exact<2 * H>(eps, w);
+    double sp = 0.0, sc = 0.0;
+    for (int i = 0; i < 2 * H; ++i) {
+        const int g = js + i;
+        const double xp = (g & 1) ? ho_p[g >> 1] : he_p[g >> 1];
+        const double xc = (g & 1) ? ho_c[g >> 1] : he_c[g >> 1];
+        sp = fma(w[i], xp, sp);
+        sc = fma(w[i], xc, sc);
+    }
+    ap = sp;
+    ac = sc;
+}
+
+// interpolate both series at the two samples m0, m0+1 of a pair with delays d0, d1 [s]
+template <int H>
+__device__ __forceinline__ void interp_delays(const FastParams &p, double d0, double d1, int rel0 /* m0 - origin */,
+                                              const double *he_p, const double *ho_p, const double *he_c,
+                                              const double *ho_c, double &ap0, double &ac0, double &ap1, double &ac1)
+{
+    int q0, q1;
+    double e0, e1;
+    split_delay_fast(d0, p.dt, p.inv_dt, q0, e0);
+    split_delay_fast(d1, p.dt, p.inv_dt, q1, e1);
+    q0 = max(-p.qmax, min(p.qmax, q0));
+    q1 = max(-p.qmax, min(p.qmax, q1));
+    const int js = rel0 - q0 - (H - 1); /* >= 0 by the margin bound */
+    if (q0 == q1) {
+        const int c = js >> 1;
+        const double *P0, *P1, *C0, *C1;
+        if (js & 1) { P0 = ho_p + c; P1 = he_p + c + 1; C0 = ho_c + c; C1 = he_c + c + 1; }
+        else        { P0 = he_p + c; P1 = ho_p + c;     C0 = he_c + c; C1 = ho_c + c; }
+        interp_pair<H>(e0, e1, P0, P1, C0, C1, ap0, ac0, ap1, ac1);
+    } else {
+        interp_single<H>(e0, he_p, ho_p, he_c, ho_c, js, ap0, ac0);
+        interp_single<H>(e1, he_p, ho_p, he_c, ho_c, rel0 + 1 - q1 - (H - 1), ap1, ac1);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// link kernel: LFA == false: Eq. (2.5), six links;  LFA == true: Eq. (B10) at (B1), links +1, +2, +3
+// ---------------------------------------------------------------------------------------------
+template <int H, bool LFA>
+__global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
+{
+    extern __shared__ double smem[];
+    const int64_t b = (int64_t)blockIdx.x % p.batch;
+    const int64_t tile = (int64_t)blockIdx.x / p.batch;
+    const int64_t a0 = tile * FAST_TA;               /* first sample of the tile (even) */
+    const int tid = threadIdx.x;
+    const int w = LFA ? (int)p.w : 0;
+
+    __shared__ double fr[LTDI_FRAME_STRIDE];
+    if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
+
+    if (p.which == LTDI_RESPONSE_HYBRID) { /* skip tiles whose links the hybrid never uses */
+        const double *hy = p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
+        const double halo = (double)(p.m2 + 2 * p.w + H + 2) * p.dt;
+        const double t_first = p.t0 + (double)a0 * p.dt, t_last = p.t0 + (double)(a0 + FAST_TA - 1) * p.dt;
+        if (LFA) { if (t_first - halo - hy[0] > 0.5 * hy[1]) return; }
+        else     { if (t_last + halo - hy[0] < -0.5 * hy[1]) return; }
+    }
+
+    /* staged strain: samples [org, org + 2 * hw2), org even; parity split; LFA: FD1 numerators of the strain */
+    const int64_t org = a0 - p.m1 - (p.m1 & 1);
+    const int hw2 = (int)((FAST_TA + 2 * p.m1 + 4) / 2);   /* pairs */
+    double *he_p = smem, *ho_p = he_p + hw2, *he_c = ho_p + hw2, *ho_c = he_c + hw2;
+    const double *gp = p.hp + b * p.ld, *gc = p.hc + b * p.ld;
+    for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
+        const int64_t g = org + i;
+        double vp = 0.0, vc = 0.0;
+        if (!LFA) {
+            if (g >= 0 && g < p.n) { vp = gp[g]; vc = gc[g]; }
+        } else if (g >= w && g < p.n - w) {
+            if (w == 1) {
+                vp = gp[g + 1] - gp[g - 1];
+                vc = gc[g + 1] - gc[g - 1];
+            } else {
+                vp = 8.0 * (gp[g + 1] - gp[g - 1]) - (gp[g + 2] - gp[g - 2]);
+                vc = 8.0 * (gc[g + 1] - gc[g - 1]) - (gc[g + 2] - gc[g - 2]);
+            }
+        }
+        double *dp = (i & 1) ? ho_p : he_p, *dc = (i & 1) ? ho_c : he_c;
+        dp[i >> 1] = vp;
+        dc[i >> 1] = vc;
+    }
+    __syncthreads();
+
+    const int64_t m0 = a0 + 2 * tid;
+    if (m0 >= p.n) return;
+    const int rel0 = (int)(m0 - org);
+    const int64_t vlo = p.m1 + w, vhi = p.n - p.m1 - w;   /* valid link samples */
+    const bool in0 = m0 >= vlo && m0 < vhi, in1 = m0 + 1 >= vlo && m0 + 1 < vhi;
+    double *yout = (LFA ? p.yL : p.yF) + b * p.lds + m0;
+    const int64_t ystride = p.batch * p.lds;
+    constexpr int NL = LFA ? 3 : 6;
+    if (!in0 && !in1) {
+#pragma unroll
+        for (int l = 0; l < NL; ++l) *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(0.0, 0.0);
+        return;
+    }
+
+    const double *t = p.tab + m0;
+    const double inv_c = 1.0 / LTDI_C_LIGHT;
+    auto row2 = [&](int r) { return *reinterpret_cast<const double2 *>(t + (int64_t)r * p.stride); };
+    auto kdotR = [&](int i, double &k0, double &k1) {
+        const double2 x = row2(ROW_R + 3 * i), y = row2(ROW_R + 3 * i + 1), z = row2(ROW_R + 3 * i + 2);
+        k0 = (fr[0] * x.x + fr[1] * y.x + fr[2] * z.x) * inv_c;
+        k1 = (fr[0] * x.y + fr[1] * y.y + fr[2] * z.y) * inv_c;
+    };
+
+    if (!LFA) {
+        double rp0[3], rc0[3], rp1[3], rc1[3]; /* h+, hx at the receiver times t - k.R_r / c (2.6b) */
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            double k0, k1;
+            kdotR(i, k0, k1);
+            interp_delays<H>(p, k0, k1, rel0, he_p, ho_p, he_c, ho_c, rp0[i], rc0[i], rp1[i], rc1[i]);
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double2 nx = row2(ROW_N + 3 * a), ny = row2(ROW_N + 3 * a + 1), nz = row2(ROW_N + 3 * a + 2);
+            double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
+            {
+                const double un = fr[3] * nx.x + fr[4] * ny.x + fr[5] * nz.x;
+                const double vn = fr[6] * nx.x + fr[7] * ny.x + fr[8] * nz.x;
+                kn0 = fr[0] * nx.x + fr[1] * ny.x + fr[2] * nz.x;
+                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;   /* (2.4) */
+                Fp0 = xip * fr[9] + xic * fr[10];                              /* (2.2) + (2.3), G17 */
+                Fc0 = xic * fr[9] - xip * fr[10];
+            }
+            {
+                const double un = fr[3] * nx.y + fr[4] * ny.y + fr[5] * nz.y;
+                const double vn = fr[6] * nx.y + fr[7] * ny.y + fr[8] * nz.y;
+                kn1 = fr[0] * nx.y + fr[1] * ny.y + fr[2] * nz.y;
+                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
+                Fp1 = xip * fr[9] + xic * fr[10];
+                Fc1 = xic * fr[9] - xip * fr[10];
+            }
+#pragma unroll
+            for (int sg = 0; sg < 2; ++sg) {
+                const int l = a + 3 * sg;
+                const int s = link_sender(l), r = link_receiver(l);
+                double k0, k1;
+                kdotR(s, k0, k1);
+                const double2 L = row2(ROW_L + l);
+                double sp0, sc0, sp1, sc1;
+                interp_delays<H>(p, L.x + k0, L.y + k1, rel0, he_p, ho_p, he_c, ho_c, sp0, sc0, sp1, sc1); /* (2.6a) */
+                const double d0 = 2.0 * (1.0 - (sg ? -kn0 : kn0)), d1 = 2.0 * (1.0 - (sg ? -kn1 : kn1));
+                const double y0 = (Fp0 * (sp0 - rp0[r]) + Fc0 * (sc0 - rc0[r])) / d0;   /* (2.5) */
+                const double y1 = (Fp1 * (sp1 - rp1[r]) + Fc1 * (sc1 - rc1[r])) / d1;
+                *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
+            }
+        }
+    } else {
+        const double den = (w == 1 ? 2.0 : 12.0) * p.dt;
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            const int s = link_sender(l), r = link_receiver(l);
+            const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
+            double ks0, ks1, kr0, kr1;
+            kdotR(s, ks0, ks1);
+            kdotR(r, kr0, kr1);
+            const double2 L = row2(ROW_L + l);
+            double ap0, ac0, ap1, ac1;
+            interp_delays<H>(p, 0.5 * L.x + 0.5 * (ks0 + kr0), 0.5 * L.y + 0.5 * (ks1 + kr1), rel0, he_p, ho_p, he_c,
+                             ho_c, ap0, ac0, ap1, ac1);                                    /* (B1) */
+            double y0, y1;
+            {
+                const double un = fr[3] * nx.x + fr[4] * ny.x + fr[5] * nz.x;
+                const double vn = fr[6] * nx.x + fr[7] * ny.x + fr[8] * nz.x;
+                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
+                const double Fp = xip * fr[9] + xic * fr[10], Fc = xic * fr[9] - xip * fr[10];
+                y0 = -(0.5 * L.x) * (Fp * (ap0 / den) + Fc * (ac0 / den));                 /* (B10) */
+            }
+            {
+                const double un = fr[3] * nx.y + fr[4] * ny.y + fr[5] * nz.y;
+                const double vn = fr[6] * nx.y + fr[7] * ny.y + fr[8] * nz.y;
+                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
+                const double Fp = xip * fr[9] + xic * fr[10], Fc = xic * fr[9] - xip * fr[10];
+                y1 = -(0.5 * L.y) * (Fp * (ap1 / den) + Fc * (ac1 / den));
+            }
+            *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// TDI delays.  Channel ch = 0,1,2 (X,Y,Z; cyclic): i2 = (1+ch)%3, i3 = (2+ch)%3,
+// dP = L[i2+3], dU = L[i3], a = L[i2+3] + L[i2], b = L[i3] + L[i3+3].  The 13 distinct delays of a channel are
+// base + i a + j b with base in {0, dP, dU}:
+// ---------------------------------------------------------------------------------------------
+struct DelayDef { signed char base, i, j; };   /* base: 0 none, 1 dP, 2 dU */
+__constant__ DelayDef c_delay_def[13] = {
+    {1, 0, 0}, {1, 0, 1}, {0, 0, 1}, {2, 0, 0}, {2, 1, 0}, {0, 1, 0}, {1, 1, 1},
+    {1, 1, 2}, {0, 1, 1}, {0, 1, 2}, {2, 1, 1}, {2, 2, 1}, {0, 2, 1}};
+/* the 14 interpolated terms of Eq. (2.7) / (2.8): series (0 P, 1 Q, 2 U, 3 W), delay id, sign; the first 6
+ * are TDI 1.5 */
+struct TermDef { signed char series, delay, sign; };
+__constant__ TermDef c_term_def[14] = {
+    {0, 0, +1}, {0, 1, -1}, {1, 2, -1}, {2, 3, -1}, {2, 4, +1}, {3, 5, +1},
+    {0, 6, -1}, {0, 7, +1}, {1, 8, -1}, {1, 9, +1}, {2, 10, +1}, {2, 11, -1}, {3, 8, +1}, {3, 12, -1}};
+
+__device__ __forceinline__ double tdi_delay(int id, double dP, double dU, double a, double b)
+{
+    /* the same expressions, in the same order, as the slow path and the oracle use */
+    switch (id) {
+    case 0: return dP;
+    case 1: return dP + b;
+    case 2: return b;
+    case 3: return dU;
+    case 4: return dU + a;
+    case 5: return a;
+    case 6: return dP + a + b;
+    case 7: return dP + a + 2.0 * b;
+    case 8: return a + b;
+    case 9: return a + 2.0 * b;
+    case 10: return dU + a + b;
+    case 11: return dU + 2.0 * a + b;
+    default: return 2.0 * a + b;
+    }
+}
+/* LFA delays (B25) / (B33): id 0: arm i2 term (series d123-like), id 1: arm i3 term */
+__device__ __forceinline__ double lfa_delay(int gen, int id, double L2, double L3)
+{
+    if (gen == LTDI_GEN_15) return id == 0 ? L3 + 0.5 * L2 : L2 + 0.5 * L3;
+    return id == 0 ? 2.0 * L3 + 1.5 * L2 : 2.0 * L2 + 1.5 * L3;
+}
+
+// ---------------------------------------------------------------------------------------------
+// anchor kernel: one block per TDI tile; thread a < FAST_NA builds the anchor of delay a
+// ---------------------------------------------------------------------------------------------
+template <int M>
+__global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, double *hdr)
+{
+    const int64_t tile = blockIdx.x;
+    const int64_t n0 = tile * FAST_TC, n1 = min(n0 + (int64_t)FAST_TC, p.n);
+    const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
+    const int tid = threadIdx.x;
+    __shared__ double dev[6]; /* max |L_l(n) - L_l(nc)| over the tile */
+    __shared__ double Lc[6];
+    if (tid < 6) {
+        const double *row = p.tab + (int64_t)(ROW_L + tid) * p.stride;
+        const double c = row[nc];
+        double d = 0.0;
+        for (int64_t n = n0; n < n1; ++n) d = fmax(d, fabs(row[n] - c));
+        dev[tid] = d;
+        Lc[tid] = c;
+    }
+    __syncthreads();
+    if (tid >= FAST_NA) return;
+    double d, bound;
+    if (tid < FAST_NA_FULL) {
+        const int ch = tid / 13, id = tid % 13;
+        const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
+        const double dP = Lc[i2 + 3], dU = Lc[i3], a = Lc[i2 + 3] + Lc[i2], b = Lc[i3] + Lc[i3 + 3];
+        d = tdi_delay(id, dP, dU, a, b);
+        const DelayDef df = c_delay_def[id];
+        bound = (df.base == 1 ? dev[i2 + 3] : df.base == 2 ? dev[i3] : 0.0) + df.i * (dev[i2 + 3] + dev[i2]) +
+                df.j * (dev[i3] + dev[i3 + 3]);
+    } else {
+        const int ch = (tid - FAST_NA_FULL) / 2, id = (tid - FAST_NA_FULL) % 2;
+        const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
+        d = lfa_delay(p.gen, id, Lc[i2], Lc[i3]);
+        bound = 2.0 * (dev[i2] + dev[i3]);
+    }
+    bound *= p.inv_dt;
+    int q;
+    double eps;
+    split_delay_fast(d, p.dt, p.inv_dt, q, eps);
+    /* usable if the Taylor remainder is below rounding, the integer shift cannot change inside the tile and the
+     * stencil stays inside the staged halo */
+    const bool ok = bound <= FAST_DMAX && eps - bound >= 0.0 && eps + bound < 1.0 && q >= 0 &&
+                    q + M / 2 <= p.m2;
+    double *h = hdr + (tile * FAST_NA + tid) * 4;
+    h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? 1.0 : 0.0;
+
+    /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); first and second
+     * derivatives by the product rule carried along the same sweeps */
+    double *out = anc + (tile * FAST_NA + tid) * (int64_t)(M * 4);
+    const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
+    const int kmin = -(M / 2 - 1);
+    double f = 1.0, f1 = 0.0, f2 = 0.0;
+    for (int i = 0; i < M; ++i) {
+        out[4 * i + 0] = f; out[4 * i + 1] = f1; out[4 * i + 2] = f2;
+        const double e = eps - (double)(kmin + i);
+        f2 = f2 * e + 2.0 * f1;
+        f1 = f1 * e + f;
+        f = f * e;
+    }
+    double g = 1.0, g1 = 0.0, g2 = 0.0;
+    for (int i = M - 1; i >= 0; --i) {
+        const double a0 = out[4 * i + 0], a1 = out[4 * i + 1], a2 = out[4 * i + 2];
+        out[4 * i + 0] = c[i] * (a0 * g);
+        out[4 * i + 1] = c[i] * (a1 * g + a0 * g1);
+        out[4 * i + 2] = 0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2));   /* w'' / 2 */
+        out[4 * i + 3] = 0.0;
+        const double e = eps - (double)(kmin + i);
+        g2 = g2 * e + 2.0 * g1;
+        g1 = g1 * e + g;
+        g = g * e;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// TDI kernel
+// ---------------------------------------------------------------------------------------------
+// exact per-sample interpolation of a staged series (slow path): ys[0] = sample y0, length len
+template <int M>
+__device__ __noinline__ double slow_delayed(const double *ys, int len, int idx /* n - y0 */, double delay, double dt,
+                                            double inv_dt)
+{
+    int q;
+    double eps;
+    split_delay_fast(delay, dt, inv_dt, q, eps);
+    double w[M];
+    lagrange_exact<M>(eps, w);
+    const int j = idx - q - (M / 2 - 1);
+    double acc = 0.0;
+    for (int i = 0; i < M; ++i) {
+        const int jj = j + i;
+        if (jj >= 0 && jj < len) acc = fma(w[i], ys[jj], acc);
+    }
+    return acc;
+}
+
+// Eqs. (4.1), (4.5) with G18; raised cosine, G20
+__device__ __forceinline__ void hybrid_weights_fast(const double *h, double t, double &w_lfa, double &w_full)
+{
+    const double x0 = t - h[0], T = h[1];
+    if (h[3] == (double)LTDI_TAPER_SIGMOID) {
+        w_lfa = (x0 <= 0.5 * T) ? 1.0 / (1.0 + exp(x0 / h[2])) : 0.0;
+        w_full = (x0 >= -0.5 * T) ? 1.0 / (1.0 + exp(-x0 / h[2])) : 0.0;
+    } else {
+        const double x = (x0 + 0.5 * T) / T;
+        if (x <= 0.0) w_full = 0.0;
+        else if (x >= 1.0) w_full = 1.0;
+        else w_full = 0.5 * (1.0 - cospi(x));
+        w_lfa = 1.0 - w_full;
+    }
+}
+
+// 7 consecutive outputs of one interpolated term: acc[r] += sum_k w_k(eps_c + D[r]) x[base + r + k]
+template <int M>
+__device__ __forceinline__ void term7(const double *__restrict__ anc /* [M][4] shared */, const double *__restrict__ x,
+                                      const double (&D)[FAST_TC_R], double (&acc)[FAST_TC_R])
+{
+    double win[FAST_TC_R];
+#pragma unroll
+    for (int r = 0; r < FAST_TC_R - 1; ++r) win[r] = x[r];
+#pragma unroll
+    for (int k = 0; k < M; ++k) {
+        const double2 w01 = *reinterpret_cast<const double2 *>(anc + 4 * k);
+        const double w2 = anc[4 * k + 2];
+        win[(k + FAST_TC_R - 1) % FAST_TC_R] = x[k + FAST_TC_R - 1];
+#pragma unroll
+        for (int r = 0; r < FAST_TC_R; ++r) {
+            const double wk = fma(D[r], fma(D[r], w2, w01.y), w01.x);
+            acc[r] = fma(wk, win[(k + r) % FAST_TC_R], acc[r]);
+        }
+    }
+}
+
+template <int M>
+__global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
+{
+    extern __shared__ double smem[];
+    constexpr int H = M / 2;
+    const int64_t b = (int64_t)blockIdx.x % p.batch;
+    const int64_t tile = (int64_t)blockIdx.x / p.batch;
+    const int64_t n0 = tile * FAST_TC;
+    const int64_t n1 = min(n0 + (int64_t)FAST_TC, p.n);
+    const int tid = threadIdx.x;
+    const int w = (int)p.w;
+
+    bool need_full = p.which == LTDI_RESPONSE_FULL, need_lfa = p.which == LTDI_RESPONSE_LFA;
+    const double *hy = nullptr;
+    if (p.which == LTDI_RESPONSE_HYBRID) {
+        hy = p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
+        const double t_first = p.t0 + (double)n0 * p.dt, t_last = p.t0 + (double)(n1 - 1) * p.dt;
+        need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0, Eq. (4.5) */
+        need_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0 */
+    }
+
+    /* shared memory: link series [6][yr] (full) | LFA links [3][yr + 2w] and their derivative [3][yr] | anchors |
+     * X, Y, Z of the tile */
+    const int yr = FAST_TC + (int)p.m2 + H + 2;
+    const int64_t y0 = n0 - p.m2;
+    double *yF = smem;                                  /* element 0 = sample y0 */
+    double *yL = yF + (p.which != LTDI_RESPONSE_LFA ? 6 * yr : 0);              /* element 0 = sample y0 - w */
+    double *dL = yL + (p.which != LTDI_RESPONSE_FULL ? 3 * (yr + 2 * w) : 0);   /* element 0 = sample y0 */
+    double *sa = dL + (p.which != LTDI_RESPONSE_FULL ? 3 * yr : 0);             /* anchors [FAST_NA][M][4] */
+    double *Xs = sa + FAST_NA * M * 4;                  /* [3][FAST_TC] */
+    __shared__ double s_hdr[FAST_NA * 4];
+    __shared__ int s_ok;
+
+    if (tid == 0) s_ok = 1;
+    if (need_full) {
+        const double *src = p.yF + b * p.lds;
+        const int64_t ystride = p.batch * p.lds;
+        for (int i = tid; i < 6 * yr; i += FAST_TC_THREADS) {
+            const int l = i / yr, k = i - l * yr;
+            const int64_t g = y0 + k;
+            yF[i] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
+        }
+    }
+    if (need_lfa) {
+        const double *src = p.yL + b * p.lds;
+        const int64_t ystride = p.batch * p.lds;
+        const int len = yr + 2 * w;
+        for (int i = tid; i < 3 * len; i += FAST_TC_THREADS) {
+            const int l = i / len, k = i - l * len;
+            const int64_t g = y0 - w + k;
+            yL[i] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
+        }
+    }
+    {
+        const double *ga = p.anc + tile * (int64_t)(FAST_NA * M * 4);
+        const int a_lo = need_full ? 0 : FAST_NA_FULL * M * 4, a_hi = need_lfa ? FAST_NA * M * 4 : FAST_NA_FULL * M * 4;
+        for (int i = a_lo / 2 + tid; i < a_hi / 2; i += FAST_TC_THREADS)
+            reinterpret_cast<double2 *>(sa)[i] = reinterpret_cast<const double2 *>(ga)[i];
+        for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[tile * (FAST_NA * 4) + i];
+    }
+    __syncthreads();
+    if (tid < FAST_NA) {
+        const bool used = tid < FAST_NA_FULL ? (need_full && (p.gen == LTDI_GEN_20 || (tid % 13) < 6)) : need_lfa;
+        if (used && s_hdr[4 * tid + 3] == 0.0) s_ok = 0;
+    }
+    if (need_lfa) {
+        /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
+        const double dt = p.dt;
+        const int len = yr + 2 * w;
+        for (int i = tid; i < 3 * yr; i += FAST_TC_THREADS) {
+            const int l = i / yr, k = i - l * yr;
+            const int64_t m = y0 + k;
+            const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
+            const double *x = yL + l * len + k + w;
+            double d = 0.0;
+            if (in) {
+                if (p.gen == LTDI_GEN_15) {
+                    d = (w == 1) ? (x[1] - x[-1]) / (2.0 * dt) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2])) / (12.0 * dt);
+                } else {
+                    const double d1 = (x[1] - x[0]) - (x[0] - x[-1]);
+                    if (w == 1) d = d1 / (dt * dt);
+                    else {
+                        const double d2 = (x[2] - x[0]) - (x[0] - x[-2]);
+                        d = (16.0 * d1 - d2) / (12.0 * dt * dt);
+                    }
+                }
+            }
+            dL[i] = d;
+        }
+    }
+    __syncthreads();
+
+    const int ch = tid / FAST_TC_G, g = tid % FAST_TC_G;
+    const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
+    const int r0 = FAST_TC_R * g;                       /* first of my 7 samples, relative to n0 */
+    const int64_t nf = n0 + r0;
+    double Xf[FAST_TC_R], Xl[FAST_TC_R];
+#pragma unroll
+    for (int r = 0; r < FAST_TC_R; ++r) { Xf[r] = 0.0; Xl[r] = 0.0; }
+
+    if (s_ok) {
+        /* D = eps_n - eps_c = (d_c - d_n) / dt, from the light times of my samples */
+        const double *hd = s_hdr + 4 * (13 * ch);
+        const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
+        const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
+        const double cP = tabL[(i2 + 3) * p.stride + nc], cp2 = tabL[i2 * p.stride + nc];
+        const double cU = tabL[i3 * p.stride + nc], cm3 = tabL[(i3 + 3) * p.stride + nc];
+        double DP[FAST_TC_R], DU[FAST_TC_R], Da[FAST_TC_R], Db[FAST_TC_R];
+#pragma unroll
+        for (int r = 0; r < FAST_TC_R; ++r) {
+            const int64_t n = min(nf + r, p.n - 1);
+            const double eP = cP - tabL[(i2 + 3) * p.stride + n], e2 = cp2 - tabL[i2 * p.stride + n];
+            const double eU = cU - tabL[i3 * p.stride + n], e3 = cm3 - tabL[(i3 + 3) * p.stride + n];
+            DP[r] = eP * p.inv_dt;
+            DU[r] = eU * p.inv_dt;
+            Da[r] = (eP + e2) * p.inv_dt;
+            Db[r] = (eU + e3) * p.inv_dt;
+        }
+        if (need_full) {
+            const double *ser[4] = {yF + i2 * yr, yF + (i2 + 3) * yr, yF + (i3 + 3) * yr, yF + i3 * yr}; /* P Q U W */
+            const int nterm = p.gen == LTDI_GEN_20 ? 14 : 6;
+#pragma unroll 1
+            for (int tm = 0; tm < nterm; ++tm) {
+                const TermDef td = c_term_def[tm];
+                const DelayDef df = c_delay_def[td.delay];
+                double D[FAST_TC_R], acc[FAST_TC_R];
+#pragma unroll
+                for (int r = 0; r < FAST_TC_R; ++r) {
+                    const double base = df.base == 1 ? DP[r] : (df.base == 2 ? DU[r] : 0.0);
+                    D[r] = fma((double)df.j, Db[r], fma((double)df.i, Da[r], base));
+                    acc[r] = 0.0;
+                }
+                const int q = (int)hd[4 * td.delay + 1];
+                const double *x = ser[td.series] + ((int)(nf - y0) - q - (H - 1));
+                term7<M>(sa + (13 * ch + td.delay) * (M * 4), x, D, acc);
+                const double sgn = (double)td.sign;
+#pragma unroll
+                for (int r = 0; r < FAST_TC_R; ++r) Xf[r] = fma(sgn, acc[r], Xf[r]);
+            }
+            /* the two undelayed terms: + Q(t) - W(t) */
+            const int i0 = (int)(nf - y0);
+#pragma unroll
+            for (int r = 0; r < FAST_TC_R; ++r) Xf[r] += ser[1][i0 + r] - ser[3][i0 + r];
+        }
+        if (need_lfa) {
+            const double *hl = s_hdr + 4 * (FAST_NA_FULL + 2 * ch);
+            const double *a_l = sa + (FAST_NA_FULL + 2 * ch) * (M * 4);
+            const double *d123 = dL + i2 * yr, *d231 = dL + i3 * yr;
+            double L2[FAST_TC_R], L3[FAST_TC_R], D[FAST_TC_R], acc2[FAST_TC_R], acc3[FAST_TC_R];
+#pragma unroll
+            for (int r = 0; r < FAST_TC_R; ++r) {
+                const int64_t n = min(nf + r, p.n - 1);
+                L2[r] = tabL[i2 * p.stride + n];
+                L3[r] = tabL[i3 * p.stride + n];
+                /* gen 1.5: L3 + L2/2 | gen 2.0: 2 L3 + 3 L2 / 2 */
+                const double e2 = cp2 - L2[r], e3 = cU - L3[r];
+                D[r] = (p.gen == LTDI_GEN_15 ? e3 + 0.5 * e2 : 2.0 * e3 + 1.5 * e2) * p.inv_dt;
+                acc2[r] = 0.0;
+                acc3[r] = 0.0;
+            }
+            const int base = (int)(nf - y0) - (H - 1);
+            term7<M>(a_l, d123 + (base - (int)hl[1]), D, acc2);
+#pragma unroll
+            for (int r = 0; r < FAST_TC_R; ++r) {
+                const double e2 = cp2 - L2[r], e3 = cU - L3[r];
+                D[r] = (p.gen == LTDI_GEN_15 ? e2 + 0.5 * e3 : 2.0 * e2 + 1.5 * e3) * p.inv_dt;
+            }
+            term7<M>(a_l + M * 4, d231 + (base - (int)hl[5]), D, acc3);
+#pragma unroll
+            for (int r = 0; r < FAST_TC_R; ++r) {
+                if (p.gen == LTDI_GEN_15) Xl[r] = 4.0 * (L3[r] * acc2[r] - L2[r] * acc3[r]);              /* (B25) */
+                else Xl[r] = 8.0 * (L2[r] + L3[r]) * (L3[r] * acc2[r] - L2[r] * acc3[r]);                /* (B33) */
+            }
+        }
+    } else {
+        /* exact per-sample weights */
+        const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
+        for (int r = 0; r < FAST_TC_R; ++r) {
+            const int64_t n = nf + r;
+            if (n >= n1) break;
+            double L[6];
+            for (int l = 0; l < 6; ++l) L[l] = tabL[l * p.stride + n];
+            const int idx = (int)(n - y0);
+            if (need_full) {
+                const double *ser[4] = {yF + i2 * yr, yF + (i2 + 3) * yr, yF + (i3 + 3) * yr, yF + i3 * yr};
+                const double dP = L[i2 + 3], dU = L[i3], a = L[i2 + 3] + L[i2], bb = L[i3] + L[i3 + 3];
+                const int nterm = p.gen == LTDI_GEN_20 ? 14 : 6;
+                double x = ser[1][idx] - ser[3][idx];
+                for (int tm = 0; tm < nterm; ++tm) {
+                    const TermDef td = c_term_def[tm];
+                    x += (double)td.sign *
+                         slow_delayed<M>(ser[td.series], yr, idx, tdi_delay(td.delay, dP, dU, a, bb), p.dt, p.inv_dt);
+                }
+                Xf[r] = x;
+            }
+            if (need_lfa) {
+                const double L2 = L[i2], L3 = L[i3];
+                const double v2 = slow_delayed<M>(dL + i2 * yr, yr, idx, lfa_delay(p.gen, 0, L2, L3), p.dt, p.inv_dt);
+                const double v3 = slow_delayed<M>(dL + i3 * yr, yr, idx, lfa_delay(p.gen, 1, L2, L3), p.dt, p.inv_dt);
+                Xl[r] = (p.gen == LTDI_GEN_15 ? 4.0 : 8.0 * (L2 + L3)) * (L3 * v2 - L2 * v3);
+            }
+        }
+    }
+
+    /* blend (4.6), margins, exchange through shared memory */
+#pragma unroll
+    for (int r = 0; r < FAST_TC_R; ++r) {
+        const int64_t n = nf + r;
+        double x;
+        if (p.which == LTDI_RESPONSE_FULL) x = Xf[r];
+        else if (p.which == LTDI_RESPONSE_LFA) x = Xl[r];
+        else {
+            double wa, wb;
+            hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+            x = 0.0;
+            if (need_lfa && wa != 0.0) x = wa * Xl[r];
+            if (need_full && wb != 0.0) x = fma(wb, Xf[r], x);
+        }
+        if (!(n >= p.lo && n < p.n - p.hi)) x = 0.0;
+        Xs[ch * FAST_TC + r0 + r] = x;
+    }
+    __syncthreads();
+
+    const double is2 = 0.70710678118654752440, is6 = 0.40824829046386301637, is3 = 0.57735026918962576451;
+    const int64_t src_off = b * p.ld;
+    for (int i = tid; i < FAST_TC; i += FAST_TC_THREADS) {
+        const int64_t n = n0 + i;
+        if (n >= n1) break;
+        const double X = Xs[i], Y = Xs[FAST_TC + i], Z = Xs[2 * FAST_TC + i];
+        p.A[src_off + n] = (Z - X) * is2;                 /* (2.9a) */
+        p.E[src_off + n] = (X - 2.0 * Y + Z) * is6;       /* (2.9b) */
+        p.T[src_off + n] = (X + Y + Z) * is3;             /* (2.9c) */
+        if (p.XYZ) {
+            p.XYZ[((int64_t)0 * p.batch_all + p.b0 + b) * p.ld + n] = X;
+            p.XYZ[((int64_t)1 * p.batch_all + p.b0 + b) * p.ld + n] = Y;
+            p.XYZ[((int64_t)2 * p.batch_all + p.b0 + b) * p.ld + n] = Z;
+        }
+        if (p.Y) {
+            const int iy = (int)(n - y0);
+            double wa = 1.0, wb = 1.0;
+            if (p.which == LTDI_RESPONSE_HYBRID) hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+#pragma unroll
+            for (int l = 0; l < 6; ++l) {
+                double v = 0.0;
+                if (p.which == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
+                else if (p.which == LTDI_RESPONSE_LFA) v = l < 3 ? yL[l * (yr + 2 * w) + iy + w] : 0.0;
+                else if (n >= p.m1 + w && n < p.n - p.m1 - w) { /* (4.5) */
+                    if (need_lfa && l < 3 && wa != 0.0) v = wa * yL[l * (yr + 2 * w) + iy + w];
+                    if (need_full && wb != 0.0) v = fma(wb, yF[l * yr + iy], v);
+                }
+                p.Y[((int64_t)l * p.batch_all + p.b0 + b) * p.ld + n] = v;
+            }
+        }
+    }
+}

@@ -1,5 +1,6 @@
 // lisatdi.cu -- the C ABI of include/lisatdi.h: argument checks, tile plan, launches.
 // Single translation unit: the kernels live in orbit.cuh and response.cuh.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstring>
@@ -10,6 +11,7 @@
 #include "common.cuh"
 #include "orbit.cuh"
 #include "response.cuh"
+#include "fast.cuh"
 
 namespace {
 
@@ -33,6 +35,38 @@ int init_constants()
             }
         }
         if (cudaMemcpyToSymbol(c_lag_inv_den, tab.data(), tab.size() * sizeof(double)) != cudaSuccess) {
+            (void)cudaGetLastError();
+            status = LTDI_ECUDA;
+        }
+        /* symmetric pair form (fast.cuh): lambda_i with prod_{i != j} lambda_i = c_j = 1 / (2 a_j prod_{i != j}
+         * (a_j^2 - a_i^2)), a_j = j + 1/2.  With Lambda = prod lambda_i: lambda_j = Lambda / c_j and
+         * Lambda^(H-1) = prod c_i; computed through logarithms in long double (prod c_i underflows). */
+        double lam[2][16] = {}, kap[2][16] = {};
+        const int Hs[2] = {5, 16};
+        for (int r = 0; r < 2; ++r) {
+            const int H = Hs[r];
+            long double c[16], logsum = 0.0L;
+            int neg = 0;
+            for (int j = 0; j < H; ++j) {
+                const long double aj = j + 0.5L;
+                long double den = 2.0L * aj;
+                for (int i = 0; i < H; ++i)
+                    if (i != j) den *= aj * aj - (i + 0.5L) * (i + 0.5L);
+                c[j] = 1.0L / den;
+                logsum += logl(fabsl(c[j]));
+                neg += c[j] < 0;
+            }
+            /* sign: H - 1 odd -> Lambda takes the sign of prod c_i; H - 1 even -> prod c_i > 0 for H = 5 */
+            long double Lambda = expl(logsum / (H - 1));
+            if (((H - 1) & 1) && (neg & 1)) Lambda = -Lambda;
+            for (int j = 0; j < H; ++j) {
+                const long double l = Lambda / c[j];
+                lam[r][j] = (double)l;
+                kap[r][j] = (double)(-l * (j + 0.5L) * (j + 0.5L));
+            }
+        }
+        if (cudaMemcpyToSymbol(c_sym_lam, lam, sizeof lam) != cudaSuccess ||
+            cudaMemcpyToSymbol(c_sym_kap, kap, sizeof kap) != cudaSuccess) {
             (void)cudaGetLastError();
             status = LTDI_ECUDA;
         }
@@ -94,7 +128,33 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
 }
 
 // workspace layout (doubles): raw sources [batch][3] | frames [batch][16] | hybrid windows [n_hyb][4]
-size_t work_doubles(int64_t batch) { return (size_t)batch * (3 + LTDI_FRAME_STRIDE + 4); }
+size_t work_doubles(int64_t batch) { return ((size_t)batch * (3 + LTDI_FRAME_STRIDE + 4) + 31) / 32 * 32; }
+
+bool fast_order(int order) { return order == 9 || order == 31; }
+
+/* workspace of the fast path behind the per-source parameters: anchors | anchor headers | link-series scratch
+ * for one chunk of sources.  The chunk is sized so that the scratch stays L2 resident. */
+struct FastLayout {
+    int64_t ntilesA, ntilesC, lds, chunk;
+    size_t anc, hdr, y;     /* doubles */
+    size_t total;           /* doubles, including work_doubles(batch) */
+};
+FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
+{
+    FastLayout f;
+    f.ntilesA = (n + FAST_TA - 1) / FAST_TA;
+    f.ntilesC = (n + FAST_TC - 1) / FAST_TC;
+    f.lds = (n + 15) / 16 * 16;
+    const int rows = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 3 : 9;
+    const size_t cap = (size_t)96 << 20; /* bytes of scratch per chunk */
+    int64_t chunk = (int64_t)(cap / ((size_t)rows * f.lds * sizeof(double)));
+    f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
+    f.anc = (size_t)f.ntilesC * FAST_NA * M * 4;
+    f.hdr = (size_t)f.ntilesC * FAST_NA * 4;
+    f.y = (size_t)rows * f.chunk * f.lds;
+    f.total = work_doubles(batch) + f.anc + f.hdr + f.y;
+    return f;
+}
 
 struct SmallArgs { double v[32 * 7]; }; /* batch <= 32: sources and windows travel as kernel arguments */
 
@@ -120,6 +180,74 @@ int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t 
     return LTDI_OK;
 }
 
+template <typename K>
+int set_smem(K kernel, size_t smem, int smem_max)
+{
+    if (smem > (size_t)smem_max) return LTDI_EUNSUPPORTED;
+    if (smem > 48 * 1024) LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    return LTDI_OK;
+}
+
+// the tuned path: anchors once per call, then link kernel(s) and TDI kernel per chunk of sources
+template <int M>
+int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work, cudaStream_t st)
+{
+    constexpr int H = M / 2;
+    const ltdi_orbit_desc &d = orb->desc;
+    const FastLayout lay = fast_layout(which, d.n, rp.batch, M);
+    if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_EUNSUPPORTED;
+    int dev = 0, smem_max = 0;
+    LTDI_CUDA_OK(cudaGetDevice(&dev));
+    LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+
+    FastParams p;
+    std::memset(&p, 0, sizeof p);
+    p.tab = rp.tab; p.stride = rp.stride; p.n = rp.n; p.t0 = rp.t0; p.dt = rp.dt; p.inv_dt = 1.0 / rp.dt;
+    p.ld = rp.ld; p.n_hyb = rp.n_hyb; p.which = which; p.gen = rp.gen; p.fd = rp.fd;
+    p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi; p.qmax = rp.qmax;
+    p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
+    double *anc = work, *hdr = anc + lay.anc, *ys = hdr + lay.hdr;
+    p.anc = anc; p.anc_hdr = hdr;
+
+    const bool full = which != LTDI_RESPONSE_LFA, lfa = which != LTDI_RESPONSE_FULL;
+    const int yr = FAST_TC + (int)mg.m2 + H + 2, w = (int)mg.w;
+    const size_t smem_link = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
+    const size_t smem_tdi = ((size_t)(full ? 6 * yr : 0) + (lfa ? 3 * (yr + 2 * w) + 3 * yr : 0) + FAST_NA * M * 4 +
+                             3 * FAST_TC) * sizeof(double);
+    int rc;
+    if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
+    if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link, smem_max))) return rc;
+    if ((rc = set_smem(tdi_kernel<M>, smem_tdi, smem_max))) return rc;
+
+    anchor_kernel<M><<<(unsigned)lay.ntilesC, 64, 0, st>>>(p, anc, hdr);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+
+    for (int64_t b0 = 0; b0 < rp.batch; b0 += lay.chunk) {
+        const int64_t nb = std::min(lay.chunk, rp.batch - b0);
+        p.batch = nb; p.b0 = b0;
+        p.hp = rp.hp + b0 * rp.ld; p.hc = rp.hc + b0 * rp.ld;
+        p.frames = rp.frames + b0 * LTDI_FRAME_STRIDE;
+        p.hyb = (const double *)rp.hyb + (rp.n_hyb == 1 ? 0 : 4 * b0);
+        p.A = rp.A + b0 * rp.ld; p.E = rp.E + b0 * rp.ld; p.T = rp.T + b0 * rp.ld;
+        p.XYZ = rp.XYZ; p.Y = rp.Y;
+        p.yF = ys; p.yL = ys + (full ? (size_t)6 * nb * lay.lds : 0);
+        if (lay.ntilesA * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
+        if (full) {
+            link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+            count_launch();
+        }
+        if (lfa) {
+            link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+            count_launch();
+        }
+        tdi_kernel<M><<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
+        count_launch();
+        LTDI_CUDA_OK(cudaGetLastError());
+    }
+    return LTDI_OK;
+}
+
 int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
@@ -140,7 +268,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         n_hyb = 0;
     }
     if ((uintptr_t)d_work % 16) return LTDI_EINVAL;
-    if (work_bytes < work_doubles(batch) * sizeof(double)) return LTDI_EWORKSPACE;
+    {
+        const size_t need = fast_order(order) ? fast_layout(which, orb->desc.n, batch, order + 1).total : work_doubles(batch);
+        if (work_bytes < need * sizeof(double)) return LTDI_EWORKSPACE;
+    }
     if (batch * ((orb->desc.n + 63) / 64) >= (int64_t)1 << 31) return LTDI_EUNSUPPORTED;
     int rc = init_constants();
     if (rc) return rc;
@@ -194,6 +325,12 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi;
     p.qmax = (int)(mg.m1 - M / 2);
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
+
+    if (fast_order(order)) {
+        const int frc = M == 32 ? run_fast<32>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st)
+                                : run_fast<10>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st);
+        if (frc != LTDI_EUNSUPPORTED) return frc;   /* else: shapes the tuned kernels do not cover */
+    }
 
     int tile = 256;
     while (tile > 64 && ((d.n + tile - 1) / tile) * batch < 2 * 148) tile /= 2; /* fill the 148 SMs */
@@ -268,7 +405,7 @@ int ltdi_host_scratch_bytes(int64_t ld, int64_t batch, size_t *bytes)
 {
     if (ld < 1 || batch < 1 || !bytes) return LTDI_EINVAL;
     const size_t series = ((size_t)ld * (size_t)batch * sizeof(double) + 255) / 256 * 256;
-    *bytes = 5 * series + (work_doubles(batch) * sizeof(double) + 255) / 256 * 256;
+    *bytes = 5 * series + (fast_layout(LTDI_RESPONSE_HYBRID, ld, batch, 32).total * sizeof(double) + 255) / 256 * 256;
     return LTDI_OK;
 }
 
@@ -361,7 +498,8 @@ int ltdi_workspace_bytes(int which, int64_t n, int64_t batch, int gen, int lagra
 {
     if (which < LTDI_RESPONSE_FULL || which > LTDI_RESPONSE_HYBRID || n < 1 || batch < 1 || !bytes) return LTDI_EINVAL;
     if (!gen_ok(gen) || !order_ok(lagrange_order)) return LTDI_EINVAL;
-    *bytes = (work_doubles(batch) * sizeof(double) + 255) / 256 * 256;
+    const size_t dbl = fast_order(lagrange_order) ? fast_layout(which, n, batch, lagrange_order + 1).total : work_doubles(batch);
+    *bytes = (dbl * sizeof(double) + 255) / 256 * 256;
     return LTDI_OK;
 }
 

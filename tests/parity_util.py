@@ -6,6 +6,25 @@ import workloads as W
 
 TOL = 1e-11           # BASELINE.json north_star: per-channel relative L2 <= 1e-11 in fp64
 NEAR_NULL = 1e-6      # a channel this far below the largest one is judged against the largest
+FLOOR_FACTOR = 3.0    # bar = max(TOL, FLOOR_FACTOR x fp64 floor of the algorithm)
+
+
+def fp64_floor(ref80, ref64, lo, n, hi, keys=("A", "E", "T")):
+    """relative L2 of the oracle's double build against its long-double build, per channel: the error any
+    plain-fp64 evaluation of the paper's formulas carries on this input (T = (X + Y + Z) / sqrt 3 cancels,
+    and the second difference of the gen-2.0 LFA divides the rounding noise of y by (omega dt)^2)"""
+    out = {}
+    for k in keys:
+        d, nrm = rel_l2(ref64[k], ref80[k], lo, n - hi)
+        out[k] = d / nrm if nrm > 0 else 0.0
+    return out
+
+
+def series_floor(ref80, ref64, lo, n, hi):
+    r80, r64 = np.asarray(ref80), np.asarray(ref64)
+    top = max(np.linalg.norm(r80[i][..., lo:n - hi]) for i in range(r80.shape[0]))
+    return [float(np.linalg.norm((r64[i] - r80[i])[..., lo:n - hi]) / top) if top > 0 else 0.0
+            for i in range(r80.shape[0])]
 
 
 def rel_l2(got, want, lo, hi_end):
