@@ -28,6 +28,17 @@ GEN, FD = 20, 2
 #   full 2.0: 72 M + 252 M + 200,  LFA: 60 M + 150
 FLOPS_FULL = lambda M: 72 * M + 252 * M + 200
 FLOPS_LFA = lambda M: 60 * M + 150
+# the same model split per kernel: flops per output sample of one launch
+KERNEL_FLOPS = {
+    ("full", "link_full"): lambda M: 72 * M + 200,    # S2 + S3: 9 retarded times x (weights 4M + two dots 4M)
+    ("full", "tdi"): lambda M: 252 * M,               # S4 + S5: 3 channels x 14 interpolations x 6M
+    ("lfa", "link_lfa"): lambda M: 24 * M + 150,      # S6: 3 retarded times x 8M
+    ("lfa", "tdi"): lambda M: 36 * M,                 # S7: 3 channels x 2 interpolations x 6M
+}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/), cfg2 only; None where no capture exists for the kernel
+TRAFFIC = {}
 
 WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
@@ -244,6 +255,17 @@ def main():
     samples_per_step = 3 * n * batch * world
     value = samples_per_step / (ms_per_step * 1e-3)
 
+    # per-kernel device times: the same K steps again with the library's per-kernel CUDA events switched on
+    # (events recorded on the launching stream around every kernel; ltdi_profile_* in include/lisatdi.h)
+    ltdi.profile_reset()
+    ltdi.profile_enable(True)
+    for _ in range(args.steps):
+        flush.zero_()
+        step(False)
+    torch.cuda.synchronize()
+    ltdi.profile_enable(False)
+    prof = ltdi.profile_read()
+
     # end to end: host buffers in, host A, E, T out, through ltdi_response_host (copies inside the timed region)
     pipe = ltdi.HostPipeline(orb, batch, n)
     for _ in range(2):
@@ -272,17 +294,36 @@ def main():
             pass
         dfma_rate = ltdi.fp64_probe(device=dev)
         peak_tflops = 2.0 * dfma_rate / 1e12
+        # per launch: device ms (mean over the profiled steps) and achieved algorithmic TFLOP/s per kernel
+        kernels = {}
+        for resp, ks in prof.items():
+            for name, (ms, cnt) in ks.items():
+                per_step = ms / args.steps                      # all launches of this kernel in one step
+                ent = {"ms_per_step": per_step, "launches_per_step": cnt / args.steps}
+                fl = KERNEL_FLOPS.get((resp, name))
+                if fl is not None:
+                    ent["tflops"] = fl(M) * n * batch / (per_step * 1e-3) / 1e12
+                    ent["frac_of_dfma_peak"] = ent["tflops"] / peak_tflops
+                if name == "orbit":
+                    ent["gbs"] = 192.0 * n / (per_step * 1e-3) / 1e9
+                    ent["frac_of_hbm_measured"] = ent["gbs"] / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None
+                kernels[f"{resp}/{name}"] = ent
+        dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])       # the dominant kernel of the step
+        if "tflops" not in kernels[dom]:
+            dom = max((k for k in kernels if "tflops" in kernels[k]), key=lambda k: kernels[k]["ms_per_step"])
+        achieved = kernels[dom]["tflops"]
         full_ms = float(np.mean(per_call["full"]))
-        flops_launch = FLOPS_FULL(M) * n * batch
-        achieved = flops_launch / (full_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "response_kernel (full response launch)",
+        roofline = {"bound": "alu", "kernel": dom + " (response/kernel; see include/lisatdi.h LTDI_KERNEL_*)",
                     "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                    "traffic": None,
+                    "traffic": TRAFFIC.get(dom),
                     "peak_source": "DFMA chain probe measured in this run (2 flop per DFMA); nominal 148 SM x 64 DFMA/clk",
+                    "timed_with": "per-kernel CUDA events on the launching stream (ltdi_profile_*), over %d steps "
+                                  "identical to the timed ones, run right after them" % args.steps,
                     "hbm_gbs_measured": peaks.get("hbm_gbs"),
+                    "kernels": kernels,
                     "per_call_ms": {k: float(np.mean(v)) for k, v in per_call.items()},
-                    "lfa_tflops": FLOPS_LFA(M) * n * batch / (float(np.mean(per_call["lfa"])) * 1e-3) / 1e12,
-                    "orbit_gbs": 192.0 * n / (float(np.mean(per_call["orbit"])) * 1e-3) / 1e9}
+                    "full_call_tflops": FLOPS_FULL(M) * n * batch / (full_ms * 1e-3) / 1e12,
+                    "lfa_call_tflops": FLOPS_LFA(M) * n * batch / (float(np.mean(per_call["lfa"])) * 1e-3) / 1e12}
         line = {"metric": "TDI output samples/s (full + LFA + hybrid)", "value": value, "unit": "TDI samples/s",
                 "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",

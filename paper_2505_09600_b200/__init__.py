@@ -77,6 +77,9 @@ _SIGNATURES = {
     "ltdi_response_host": (C.c_int, [C.c_int, _vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                      C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_fp64_probe": (C.c_int, [_dp, C.c_int, C.c_int, _vp, C.POINTER(C.c_double)]),
+    "ltdi_profile_enable": (C.c_int, [C.c_int]),
+    "ltdi_profile_read": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), _i64p]),
+    "ltdi_profile_reset": (C.c_int, []),
     "ltdi_launch_count": (C.c_int64, []),
     "ltdi_version": (C.c_char_p, []),
 }
@@ -146,6 +149,30 @@ def hyb_time(f_hyb_hz, mchirp_s, t_c):
 
 def launch_count():
     return lib().ltdi_launch_count()
+
+
+KERNELS = ("orbit", "prep", "anchor", "link_full", "link_lfa", "tdi", "generic")   # LTDI_KERNEL_* order
+
+
+def profile_enable(on=True):
+    _check("ltdi_profile_enable", lib().ltdi_profile_enable(int(bool(on))))
+
+
+def profile_reset():
+    _check("ltdi_profile_reset", lib().ltdi_profile_reset())
+
+
+def profile_read():
+    """{response: {kernel name: (device ms accumulated, launches)}} from the library's per-kernel CUDA events."""
+    out = {}
+    for w, resp in enumerate(("full", "lfa", "hybrid")):
+        out[resp] = {}
+        for i, name in enumerate(KERNELS):
+            ms, n = C.c_double(), C.c_int64()
+            _check("ltdi_profile_read", lib().ltdi_profile_read(i, w, C.byref(ms), C.byref(n)))
+            if n.value:
+                out[resp][name] = (ms.value, n.value)
+    return out
 
 
 class Orbits:

@@ -410,13 +410,22 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
     const int tid = threadIdx.x;
     __shared__ double dev[6]; /* max |L_l(n) - L_l(nc)| over the tile */
     __shared__ double Lc[6];
-    if (tid < 6) {
-        const double *row = p.tab + (int64_t)(ROW_L + tid) * p.stride;
-        const double c = row[nc];
-        double d = 0.0;
-        for (int64_t n = n0; n < n1; ++n) d = fmax(d, fabs(row[n] - c));
-        dev[tid] = d;
-        Lc[tid] = c;
+    /* warp w < 2 reduces rows 3w .. 3w+2: coalesced sweeps over the tile, then a shuffle tree */
+    {
+        const int warp = tid >> 5, lane = tid & 31;
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const double *row = p.tab + (int64_t)(ROW_L + 3 * warp + r) * p.stride;
+            const double c = row[nc];
+            double d = 0.0;
+            for (int64_t n = n0 + lane; n < n1; n += 32) d = fmax(d, fabs(row[n] - c));
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) d = fmax(d, __shfl_xor_sync(0xffffffffu, d, o));
+            if (lane == 0) {
+                dev[3 * warp + r] = d;
+                Lc[3 * warp + r] = c;
+            }
+        }
     }
     __syncthreads();
     if (tid >= FAST_NA) return;
@@ -447,25 +456,32 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
     h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? 1.0 : 0.0;
 
     /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); first and second
-     * derivatives by the product rule carried along the same sweeps */
+     * derivatives by the product rule carried along the same sweeps (registers; one coalesced-ish store at the end) */
     double *out = anc + (tile * FAST_NA + tid) * (int64_t)(M * 4);
     const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
-    const int kmin = -(M / 2 - 1);
-    double f = 1.0, f1 = 0.0, f2 = 0.0;
-    for (int i = 0; i < M; ++i) {
-        out[4 * i + 0] = f; out[4 * i + 1] = f1; out[4 * i + 2] = f2;
-        const double e = eps - (double)(kmin + i);
-        f2 = f2 * e + 2.0 * f1;
-        f1 = f1 * e + f;
-        f = f * e;
+    constexpr int kmin = -(M / 2 - 1);
+    double pf[M], pf1[M], pf2[M];
+    {
+        double f = 1.0, f1 = 0.0, f2 = 0.0;
+#pragma unroll
+        for (int i = 0; i < M; ++i) {
+            pf[i] = f; pf1[i] = f1; pf2[i] = f2;
+            const double e = eps - (double)(kmin + i);
+            f2 = f2 * e + 2.0 * f1;
+            f1 = f1 * e + f;
+            f = f * e;
+        }
     }
     double g = 1.0, g1 = 0.0, g2 = 0.0;
+#pragma unroll
     for (int i = M - 1; i >= 0; --i) {
-        const double a0 = out[4 * i + 0], a1 = out[4 * i + 1], a2 = out[4 * i + 2];
-        out[4 * i + 0] = c[i] * (a0 * g);
-        out[4 * i + 1] = c[i] * (a1 * g + a0 * g1);
-        out[4 * i + 2] = 0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2));   /* w'' / 2 */
-        out[4 * i + 3] = 0.0;
+        const double a0 = pf[i], a1 = pf1[i], a2 = pf2[i];
+        double4 o;
+        o.x = c[i] * (a0 * g);
+        o.y = c[i] * (a1 * g + a0 * g1);
+        o.z = 0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2));   /* w'' / 2 */
+        o.w = 0.0;
+        *reinterpret_cast<double4 *>(out + 4 * i) = o;
         const double e = eps - (double)(kmin + i);
         g2 = g2 * e + 2.0 * g1;
         g1 = g1 * e + g;

@@ -18,6 +18,43 @@ namespace {
 std::atomic<int64_t> g_launches{0};
 inline void count_launch(int k = 1) { g_launches.fetch_add(k, std::memory_order_relaxed); }
 
+/* Per-kernel timing (ltdi_profile_*): while enabled, every kernel launch is bracketed by two CUDA events on
+ * the stream it is launched on; ltdi_profile_read() turns the pairs into per-kernel totals. */
+struct ProfPair { int id; cudaEvent_t e0, e1; };
+std::mutex g_prof_mu;
+bool g_prof_on = false;
+std::vector<ProfPair> g_prof_pending;
+std::vector<cudaEvent_t> g_prof_pool;
+double g_prof_ms[3 * LTDI_KERNEL_COUNT] = {};   /* [which][kernel] */
+int64_t g_prof_n[3 * LTDI_KERNEL_COUNT] = {};
+
+struct ProfScope {
+    cudaStream_t st;
+    ProfPair pr;
+    bool on;
+    static cudaEvent_t get()
+    {
+        cudaEvent_t e = nullptr;
+        if (!g_prof_pool.empty()) { e = g_prof_pool.back(); g_prof_pool.pop_back(); }
+        else if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); e = nullptr; }
+        return e;
+    }
+    ProfScope(int id, cudaStream_t s) : st(s), on(false)
+    {
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        if (!g_prof_on) return;
+        pr.id = id; pr.e0 = get(); pr.e1 = get();
+        if (pr.e0 && pr.e1) { on = true; cudaEventRecord(pr.e0, st); }
+    }
+    ~ProfScope()
+    {
+        if (!on) return;
+        cudaEventRecord(pr.e1, st);
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        g_prof_pending.push_back(pr);
+    }
+};
+
 // 1 / prod_{m != k}(k - m), k, m = -(M/2-1) .. M/2, for every even M <= 64 (rows of c_lag_inv_den)
 int init_constants()
 {
@@ -115,7 +152,10 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
     p.R_in = d_R; p.L_in = d_L; p.tab = (double *)d_tables;
     const int threads = 256;
     const int64_t blocks = (desc->n + threads - 1) / threads;
-    orbit_delay_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
+    {
+        ProfScope ps(LTDI_KERNEL_ORBIT, (cudaStream_t)stream);
+        orbit_delay_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
+    }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
     ltdi_orbits *o = new (std::nothrow) ltdi_orbits;
@@ -158,11 +198,12 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
 
 struct SmallArgs { double v[32 * 7]; }; /* batch <= 32: sources and windows travel as kernel arguments */
 
-__global__ void unpack_small_kernel(SmallArgs a, int batch, int n_hyb, double *src, HybDev *hyb)
+__global__ void unpack_small_kernel(SmallArgs a, int batch, int n_hyb, double *src, double *frames, HybDev *hyb)
 {
     const int i = threadIdx.x;
     if (i < batch * 3) src[i] = a.v[i];
     if (i < n_hyb * 4) ((double *)hyb)[i] = a.v[96 + i];
+    if (i < batch) source_frame_one(a.v[3 * i], a.v[3 * i + 1], a.v[3 * i + 2], frames + i * LTDI_FRAME_STRIDE); /* S1 */
 }
 
 template <int MT, bool STAGE>
@@ -174,7 +215,10 @@ int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t 
                                           (int)smem));
         configured.store(smem);
     }
-    response_kernel<MT, STAGE><<<(unsigned)(p.ntiles * p.batch), threads, smem, st>>>(p);
+    {
+        ProfScope ps(LTDI_KERNEL_GENERIC + LTDI_KERNEL_COUNT * p.which, st);
+        response_kernel<MT, STAGE><<<(unsigned)(p.ntiles * p.batch), threads, smem, st>>>(p);
+    }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
     return LTDI_OK;
@@ -184,7 +228,20 @@ template <typename K>
 int set_smem(K kernel, size_t smem, int smem_max)
 {
     if (smem > (size_t)smem_max) return LTDI_EUNSUPPORTED;
-    if (smem > 48 * 1024) LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem <= 48 * 1024) return LTDI_OK;
+    /* the attribute is sticky per device function: raise it only when a call needs more than any before */
+    static std::mutex mu;
+    static std::vector<std::pair<const void *, size_t>> seen;
+    std::lock_guard<std::mutex> lk(mu);
+    for (auto &e : seen)
+        if (e.first == (const void *)kernel) {
+            if (e.second >= smem) return LTDI_OK;
+            LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            e.second = smem;
+            return LTDI_OK;
+        }
+    LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    seen.emplace_back((const void *)kernel, smem);
     return LTDI_OK;
 }
 
@@ -196,9 +253,14 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     const ltdi_orbit_desc &d = orb->desc;
     const FastLayout lay = fast_layout(which, d.n, rp.batch, M);
     if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_EUNSUPPORTED;
-    int dev = 0, smem_max = 0;
-    LTDI_CUDA_OK(cudaGetDevice(&dev));
-    LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    static std::atomic<int> smem_max_cached{0};   /* one device per process (one process per GPU) */
+    int smem_max = smem_max_cached.load();
+    if (!smem_max) {
+        int dev = 0;
+        LTDI_CUDA_OK(cudaGetDevice(&dev));
+        LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        smem_max_cached.store(smem_max);
+    }
 
     FastParams p;
     std::memset(&p, 0, sizeof p);
@@ -219,7 +281,10 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link, smem_max))) return rc;
     if ((rc = set_smem(tdi_kernel<M>, smem_tdi, smem_max))) return rc;
 
-    anchor_kernel<M><<<(unsigned)lay.ntilesC, 64, 0, st>>>(p, anc, hdr);
+    {
+        ProfScope ps(LTDI_KERNEL_ANCHOR + LTDI_KERNEL_COUNT * which, st);
+        anchor_kernel<M><<<(unsigned)lay.ntilesC, 64, 0, st>>>(p, anc, hdr);
+    }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
 
@@ -234,14 +299,19 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         p.yF = ys; p.yL = ys + (full ? (size_t)6 * nb * lay.lds : 0);
         if (lay.ntilesA * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
         if (full) {
+            ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
             link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
             count_launch();
         }
         if (lfa) {
+            ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
             link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
             count_launch();
         }
-        tdi_kernel<M><<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
+        {
+            ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
+            tdi_kernel<M><<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
+        }
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
     }
@@ -290,7 +360,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
             a.v[96 + 4 * i + 0] = h_hyb[i].t_hyb; a.v[96 + 4 * i + 1] = h_hyb[i].window_s;
             a.v[96 + 4 * i + 2] = h_hyb[i].sigma_s; a.v[96 + 4 * i + 3] = (double)h_hyb[i].taper;
         }
-        unpack_small_kernel<<<1, 128, 0, st>>>(a, (int)batch, (int)n_hyb, w_src, w_hyb);
+        {
+            ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
+            unpack_small_kernel<<<1, 128, 0, st>>>(a, (int)batch, (int)n_hyb, w_src, w_frames, w_hyb);
+        }
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
     } else {
@@ -307,10 +380,13 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         LTDI_CUDA_OK(cudaMemcpyAsync(w_src, pack.data(), sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, st));
         if (n_hyb)
             LTDI_CUDA_OK(cudaMemcpyAsync(w_hyb, hy, sizeof(double) * 4 * n_hyb, cudaMemcpyHostToDevice, st));
+        {
+            ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
+            source_frame_kernel<<<(unsigned)((batch + 127) / 128), 128, 0, st>>>(w_src, w_frames, batch);
+        }
+        count_launch();
+        LTDI_CUDA_OK(cudaGetLastError());
     }
-    source_frame_kernel<<<(unsigned)((batch + 127) / 128), 128, 0, st>>>(w_src, w_frames, batch);
-    count_launch();
-    LTDI_CUDA_OK(cudaGetLastError());
 
     /* tile plan */
     const ltdi_orbit_desc &d = orb->desc;
@@ -529,6 +605,43 @@ int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const doubl
 }
 
 int64_t ltdi_launch_count(void) { return g_launches.load(); }
+
+int ltdi_profile_enable(int on)
+{
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_on = on != 0;
+    return LTDI_OK;
+}
+
+int ltdi_profile_read(int kernel, int which, double *total_ms, int64_t *launches)
+{
+    if (kernel < 0 || kernel >= LTDI_KERNEL_COUNT || which < 0 || which > 2 || !total_ms || !launches) return LTDI_EINVAL;
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (const ProfPair &pr : g_prof_pending) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(pr.e1) != cudaSuccess || cudaEventElapsedTime(&ms, pr.e0, pr.e1) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return LTDI_ECUDA;
+        }
+        g_prof_ms[pr.id] += ms;
+        g_prof_n[pr.id] += 1;
+        g_prof_pool.push_back(pr.e0);
+        g_prof_pool.push_back(pr.e1);
+    }
+    g_prof_pending.clear();
+    *total_ms = g_prof_ms[kernel + LTDI_KERNEL_COUNT * which];
+    *launches = g_prof_n[kernel + LTDI_KERNEL_COUNT * which];
+    return LTDI_OK;
+}
+
+int ltdi_profile_reset(void)
+{
+    double ms; int64_t n;
+    const int rc = ltdi_profile_read(0, 0, &ms, &n);   /* drains pending pairs */
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (int i = 0; i < 3 * LTDI_KERNEL_COUNT; ++i) { g_prof_ms[i] = 0.0; g_prof_n[i] = 0; }
+    return rc;
+}
 const char *ltdi_version(void) { return "lisatdi-b200 0.1 (sm_100a, fp64)"; }
 
 } // extern "C"

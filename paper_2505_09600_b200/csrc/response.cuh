@@ -36,20 +36,23 @@ struct RespParams {
 // ---------------------------------------------------------------------------------------------
 // S1: source frame, Eq. (2.1) with G1: k = -e_r, u = -e_phi, v = -e_theta; cos 2psi, sin 2psi (2.3)
 // ---------------------------------------------------------------------------------------------
-__global__ void source_frame_kernel(const double *__restrict__ src, double *__restrict__ frames, int64_t batch)
+__device__ __forceinline__ void source_frame_one(double beta, double lam, double psi, double *f)
 {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= batch) return;
-    const double beta = src[3 * b + 0], lam = src[3 * b + 1], psi = src[3 * b + 2];
     double sb, cb, sl, cl, s2, c2;
     sincos(beta, &sb, &cb);
     sincos(lam, &sl, &cl);
     sincos(2.0 * psi, &s2, &c2);
-    double *f = frames + b * LTDI_FRAME_STRIDE;
     f[0] = -cb * cl; f[1] = -cb * sl; f[2] = -sb;   /* k */
     f[3] = sl;       f[4] = -cl;      f[5] = 0.0;   /* u */
     f[6] = -sb * cl; f[7] = -sb * sl; f[8] = cb;    /* v */
     f[9] = c2;       f[10] = s2;
+}
+
+__global__ void source_frame_kernel(const double *__restrict__ src, double *__restrict__ frames, int64_t batch)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    source_frame_one(src[3 * b + 0], src[3 * b + 1], src[3 * b + 2], frames + b * LTDI_FRAME_STRIDE);
 }
 
 // ---------------------------------------------------------------------------------------------
