@@ -38,6 +38,8 @@
 #define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
 #define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
 #define FAST_DMAX 1.0e-6                  /* |eps_n - eps_c| bound for the second-order weights */
+/* one anchor = [M] double2 {w_k, w_k'} followed by [M] float w_k''/2 (padded to 16 bytes), in doubles */
+#define FAST_ANC_DOUBLES(M) (2 * (M) + 2 * (((M) + 3) / 4))
 
 /* lambda_i and kappa_i = -lambda_i (i + 1/2)^2 for H = 5 (row 0) and H = 16 (row 1) */
 __constant__ double c_sym_lam[2][16];
@@ -216,7 +218,9 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
 {
     extern __shared__ double smem[];
     const int64_t b = (int64_t)blockIdx.x % p.batch;
-    const int64_t tile = (int64_t)blockIdx.x / p.batch;
+    int64_t tile = (int64_t)blockIdx.x / p.batch;
+    /* hybrid: the full links live at the end of the series; schedule those tiles first (no long tail) */
+    if (!LFA && p.which == LTDI_RESPONSE_HYBRID) tile = p.ntilesA - 1 - tile;
     const int64_t a0 = tile * FAST_TA;               /* first sample of the tile (even) */
     const int tid = threadIdx.x;
     const int w = LFA ? (int)p.w : 0;
@@ -457,7 +461,8 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
 
     /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); first and second
      * derivatives by the product rule carried along the same sweeps (registers; one coalesced-ish store at the end) */
-    double *out = anc + (tile * FAST_NA + tid) * (int64_t)(M * 4);
+    double *out = anc + (tile * FAST_NA + tid) * (int64_t)FAST_ANC_DOUBLES(M);
+    float *out2 = reinterpret_cast<float *>(out + 2 * M);
     const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
     constexpr int kmin = -(M / 2 - 1);
     double pf[M], pf1[M], pf2[M];
@@ -476,17 +481,18 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
 #pragma unroll
     for (int i = M - 1; i >= 0; --i) {
         const double a0 = pf[i], a1 = pf1[i], a2 = pf2[i];
-        double4 o;
+        double2 o;
         o.x = c[i] * (a0 * g);
         o.y = c[i] * (a1 * g + a0 * g1);
-        o.z = 0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2));   /* w'' / 2 */
-        o.w = 0.0;
-        *reinterpret_cast<double4 *>(out + 4 * i) = o;
+        *reinterpret_cast<double2 *>(out + 2 * i) = o;
+        out2[i] = (float)(0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2)));   /* w'' / 2 */
         const double e = eps - (double)(kmin + i);
         g2 = g2 * e + 2.0 * g1;
         g1 = g1 * e + g;
         g = g * e;
     }
+#pragma unroll
+    for (int i = M; i < 4 * ((M + 3) / 4); ++i) out2[i] = 0.f;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -527,93 +533,166 @@ __device__ __forceinline__ void hybrid_weights_fast(const double *h, double t, d
     }
 }
 
-// 7 consecutive outputs of one interpolated term: acc[r] += sum_k w_k(eps_c + D[r]) x[base + r + k]
+
+// FAST_TC_R consecutive outputs of one interpolated term.  With D = eps_n - eps_c,
+//   sum_k w_k(eps_c + D) x_k = S0 + D (S1 + D S2),   S_m = sum_k w_k^(m)(eps_c) / m!  x_k :
+// three constant-coefficient FIR filters over the tile.  S0 and S1 are accumulated in fp64 (2 DFMA per tap and
+// sample, FAST_TC_R x 2 independent chains); S2 enters multiplied by D^2 <= 1e-12, so fp32 carries it (its
+// rounding, <= 1e-5 |x|, contributes <= 1e-17 |x|) on the FMA pipe, which issues beside the FP64 pipe.
 template <int M>
-__device__ __forceinline__ void term7(const double *__restrict__ anc /* [M][4] shared */, const double *__restrict__ x,
-                                      const double (&D)[FAST_TC_R], double (&acc)[FAST_TC_R])
+__device__ __forceinline__ void term7(const double *__restrict__ anc, const double *__restrict__ x,
+                                      const float *__restrict__ xf, double (&s0)[FAST_TC_R], double (&s1)[FAST_TC_R],
+                                      float (&s2)[FAST_TC_R])
 {
+    const double2 *w01 = reinterpret_cast<const double2 *>(anc);
+    const float4 *w2 = reinterpret_cast<const float4 *>(anc + 2 * M);
     double win[FAST_TC_R];
+    float wf[FAST_TC_R];
 #pragma unroll
-    for (int r = 0; r < FAST_TC_R - 1; ++r) win[r] = x[r];
+    for (int r = 0; r < FAST_TC_R; ++r) { s0[r] = 0.0; s1[r] = 0.0; s2[r] = 0.f; }
+#pragma unroll
+    for (int r = 0; r < FAST_TC_R - 1; ++r) { win[r] = x[r]; wf[r] = xf[r]; }
+    float4 q2 = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
     for (int k = 0; k < M; ++k) {
-        const double2 w01 = *reinterpret_cast<const double2 *>(anc + 4 * k);
-        const double w2 = anc[4 * k + 2];
+        const double2 w = w01[k];
+        if ((k & 3) == 0) q2 = w2[k >> 2];
+        const float w2k = (k & 3) == 0 ? q2.x : (k & 3) == 1 ? q2.y : (k & 3) == 2 ? q2.z : q2.w;
         win[(k + FAST_TC_R - 1) % FAST_TC_R] = x[k + FAST_TC_R - 1];
+        wf[(k + FAST_TC_R - 1) % FAST_TC_R] = xf[k + FAST_TC_R - 1];
 #pragma unroll
         for (int r = 0; r < FAST_TC_R; ++r) {
-            const double wk = fma(D[r], fma(D[r], w2, w01.y), w01.x);
-            acc[r] = fma(wk, win[(k + r) % FAST_TC_R], acc[r]);
+            const double xv = win[(k + r) % FAST_TC_R];
+            s0[r] = fma(w.x, xv, s0[r]);
+            s1[r] = fma(w.y, xv, s1[r]);
+            s2[r] = fmaf(w2k, wf[(k + r) % FAST_TC_R], s2[r]);
         }
     }
 }
 
-template <int M>
+// finite float copy of a link sample for the fp32 second-order filter
+__device__ __forceinline__ float to_f32(double v)
+{
+    const float f = (float)v;
+    return fabsf(f) <= 3.0e38f ? f : 0.f;
+}
+
+// Ampere-style asynchronous copies (LDGSTS): the staging loops issue all their loads at once and wait once
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
+template <int M, int WHICH>
 __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int H = M / 2;
+    constexpr int ANC = FAST_ANC_DOUBLES(M);
+    constexpr bool has_full = WHICH != LTDI_RESPONSE_LFA, has_lfa = WHICH != LTDI_RESPONSE_FULL;
     const int64_t b = (int64_t)blockIdx.x % p.batch;
-    const int64_t tile = (int64_t)blockIdx.x / p.batch;
+    int64_t tile = (int64_t)blockIdx.x / p.batch;
+    /* hybrid: tiles past t_hyb carry the 14-term full response; schedule them first (no long tail) */
+    if (WHICH == LTDI_RESPONSE_HYBRID) tile = p.ntilesC - 1 - tile;
     const int64_t n0 = tile * FAST_TC;
     const int64_t n1 = min(n0 + (int64_t)FAST_TC, p.n);
     const int tid = threadIdx.x;
     const int w = (int)p.w;
 
-    bool need_full = p.which == LTDI_RESPONSE_FULL, need_lfa = p.which == LTDI_RESPONSE_LFA;
+    bool need_full = WHICH == LTDI_RESPONSE_FULL, need_lfa = WHICH == LTDI_RESPONSE_LFA;
     const double *hy = nullptr;
-    if (p.which == LTDI_RESPONSE_HYBRID) {
+    if (WHICH == LTDI_RESPONSE_HYBRID) {
         hy = p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
         const double t_first = p.t0 + (double)n0 * p.dt, t_last = p.t0 + (double)(n1 - 1) * p.dt;
         need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0, Eq. (4.5) */
         need_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0 */
     }
 
-    /* shared memory: link series [6][yr] (full) | LFA links [3][yr + 2w] and their derivative [3][yr] | anchors |
-     * X, Y, Z of the tile */
+    /* shared memory (host: tdi_smem_bytes):
+     *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
+     *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0)
+     *   R    scratch region, in turn: LFA links [3][yr + 2w] (element 0 = y0 - w) -> light times of the tile, then
+     *        their drifts eL [6][FAST_TC] -> X, Y, Z of the tile [3][FAST_TC]
+     *   yFf  [6][yr], dLf [3][yr]         float copies for the second-order filter */
     const int yr = FAST_TC + (int)p.m2 + H + 2;
     const int64_t y0 = n0 - p.m2;
-    double *yF = smem;                                  /* element 0 = sample y0 */
-    double *yL = yF + (p.which != LTDI_RESPONSE_LFA ? 6 * yr : 0);              /* element 0 = sample y0 - w */
-    double *dL = yL + (p.which != LTDI_RESPONSE_FULL ? 3 * (yr + 2 * w) : 0);   /* element 0 = sample y0 */
-    double *sa = dL + (p.which != LTDI_RESPONSE_FULL ? 3 * yr : 0);             /* anchors [FAST_NA][M][4] */
-    double *Xs = sa + FAST_NA * M * 4;                  /* [3][FAST_TC] */
+    constexpr int na_full = has_full ? FAST_NA_FULL : 0;
+    double *sa = smem;
+    double *yF = sa + (size_t)(na_full + (has_lfa ? FAST_NA_LFA : 0)) * ANC;
+    double *dL = yF + (has_full ? 6 * yr : 0);
+    double *R = dL + (has_lfa ? 3 * yr : 0);
+    const int r_len = max(6 * FAST_TC, has_lfa ? 3 * (yr + 2 * w) : 0);
+    float *yFf = reinterpret_cast<float *>(R + r_len);
+    float *dLf = yFf + (has_full ? 6 * yr : 0);
+    double *yL = R, *eL = R, *Xs = R;
+    const double *sa_lfa = sa + (size_t)na_full * ANC;
+    const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
+    const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
     __shared__ double s_hdr[FAST_NA * 4];
+    __shared__ double s_Lc[6];
     __shared__ int s_ok;
 
+    /* phase 0: every global read of the tile is issued asynchronously, then one wait */
+    auto stage_light_times = [&]() {
+        for (int i = tid; i < 6 * FAST_TC; i += FAST_TC_THREADS) {
+            const int l = i / FAST_TC, k = i - l * FAST_TC;
+            cp_async8(eL + i, tabL + l * p.stride + min(n0 + k, p.n - 1));
+        }
+    };
     if (tid == 0) s_ok = 1;
-    if (need_full) {
+    if (tid < 6) s_Lc[tid] = tabL[tid * p.stride + nc];
+    if (has_full && need_full) {
         const double *src = p.yF + b * p.lds;
         const int64_t ystride = p.batch * p.lds;
         for (int i = tid; i < 6 * yr; i += FAST_TC_THREADS) {
             const int l = i / yr, k = i - l * yr;
             const int64_t g = y0 + k;
-            yF[i] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
+            if (g >= 0 && g < p.n) cp_async8(yF + i, src + l * ystride + g);
+            else yF[i] = 0.0;
         }
     }
-    if (need_lfa) {
+    if (has_lfa && need_lfa) {
         const double *src = p.yL + b * p.lds;
         const int64_t ystride = p.batch * p.lds;
         const int len = yr + 2 * w;
         for (int i = tid; i < 3 * len; i += FAST_TC_THREADS) {
             const int l = i / len, k = i - l * len;
             const int64_t g = y0 - w + k;
-            yL[i] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
+            if (g >= 0 && g < p.n) cp_async8(yL + i, src + l * ystride + g);
+            else yL[i] = 0.0;
         }
+    } else {
+        stage_light_times();
     }
     {
-        const double *ga = p.anc + tile * (int64_t)(FAST_NA * M * 4);
-        const int a_lo = need_full ? 0 : FAST_NA_FULL * M * 4, a_hi = need_lfa ? FAST_NA * M * 4 : FAST_NA_FULL * M * 4;
-        for (int i = a_lo / 2 + tid; i < a_hi / 2; i += FAST_TC_THREADS)
-            reinterpret_cast<double2 *>(sa)[i] = reinterpret_cast<const double2 *>(ga)[i];
+        const double *ga = p.anc + tile * (int64_t)(FAST_NA * ANC);
+        if (has_full && need_full)
+            for (int i = tid; i < FAST_NA_FULL * ANC / 2; i += FAST_TC_THREADS)
+                cp_async16(sa + 2 * i, ga + 2 * i);
+        if (has_lfa && need_lfa)
+            for (int i = tid; i < FAST_NA_LFA * ANC / 2; i += FAST_TC_THREADS)
+                cp_async16(sa + (size_t)na_full * ANC + 2 * i, ga + FAST_NA_FULL * ANC + 2 * i);
         for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[tile * (FAST_NA * 4) + i];
     }
+    cp_async_wait_all();
     __syncthreads();
+
+    /* phase 1: float copies, anchor validity, derivative of the LFA links */
+    if (has_full && need_full)
+        for (int i = tid; i < 6 * yr; i += FAST_TC_THREADS) yFf[i] = to_f32(yF[i]);
     if (tid < FAST_NA) {
         const bool used = tid < FAST_NA_FULL ? (need_full && (p.gen == LTDI_GEN_20 || (tid % 13) < 6)) : need_lfa;
         if (used && s_hdr[4 * tid + 3] == 0.0) s_ok = 0;
     }
-    if (need_lfa) {
+    if (has_lfa && need_lfa) {
         /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
         const double dt = p.dt;
         const int len = yr + 2 * w;
@@ -636,102 +715,97 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
                 }
             }
             dL[i] = d;
+            dLf[i] = to_f32(d);
         }
     }
-    __syncthreads();
+    __syncthreads();   /* s_ok final; the LFA links in R are dead */
+
+    /* phase 2: light-time drifts eL[l][i] = L_l(n_c) - L_l(n0 + i): D = eps_n - eps_c = (d_c - d_n) / dt */
+    if (s_ok) {
+        if (has_lfa && need_lfa) {
+            stage_light_times();
+            cp_async_wait_all();
+            __syncthreads();
+        }
+        for (int i = tid; i < 6 * FAST_TC; i += FAST_TC_THREADS) eL[i] = s_Lc[i / FAST_TC] - eL[i];
+        __syncthreads();
+    }
 
     const int ch = tid / FAST_TC_G, g = tid % FAST_TC_G;
     const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
-    const int r0 = FAST_TC_R * g;                       /* first of my 7 samples, relative to n0 */
+    const int r0 = FAST_TC_R * g;                       /* first of my samples, relative to n0 */
     const int64_t nf = n0 + r0;
     double Xf[FAST_TC_R], Xl[FAST_TC_R];
 #pragma unroll
     for (int r = 0; r < FAST_TC_R; ++r) { Xf[r] = 0.0; Xl[r] = 0.0; }
 
     if (s_ok) {
-        /* D = eps_n - eps_c = (d_c - d_n) / dt, from the light times of my samples */
-        const double *hd = s_hdr + 4 * (13 * ch);
-        const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
-        const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
-        const double cP = tabL[(i2 + 3) * p.stride + nc], cp2 = tabL[i2 * p.stride + nc];
-        const double cU = tabL[i3 * p.stride + nc], cm3 = tabL[(i3 + 3) * p.stride + nc];
-        double DP[FAST_TC_R], DU[FAST_TC_R], Da[FAST_TC_R], Db[FAST_TC_R];
-#pragma unroll
-        for (int r = 0; r < FAST_TC_R; ++r) {
-            const int64_t n = min(nf + r, p.n - 1);
-            const double eP = cP - tabL[(i2 + 3) * p.stride + n], e2 = cp2 - tabL[i2 * p.stride + n];
-            const double eU = cU - tabL[i3 * p.stride + n], e3 = cm3 - tabL[(i3 + 3) * p.stride + n];
-            DP[r] = eP * p.inv_dt;
-            DU[r] = eU * p.inv_dt;
-            Da[r] = (eP + e2) * p.inv_dt;
-            Db[r] = (eU + e3) * p.inv_dt;
-        }
-        if (need_full) {
-            const double *ser[4] = {yF + i2 * yr, yF + (i2 + 3) * yr, yF + (i3 + 3) * yr, yF + i3 * yr}; /* P Q U W */
-            const int nterm = p.gen == LTDI_GEN_20 ? 14 : 6;
+        /* one loop over the interpolated terms of this channel: 6 / 14 of Eq. (2.7) / (2.8) on the full links, then
+         * the two of (B25) / (B33) on the differentiated LFA links.  Per term: anchor, series offset, and the
+         * coefficients of D = (cP eP + c2 e2 + cU eU + c3 e3) / dt in the light-time drifts of the channel's links
+         * (a = L_-p2 + L_p2 -> eP + e2, b = L_p3 + L_-p3 -> eU + e3, dP -> eP, dU -> eU; LFA: L_p2 -> e2, L_p3 -> eU) */
+        const double *eP = eL + (i2 + 3) * FAST_TC + r0, *e2 = eL + i2 * FAST_TC + r0;
+        const double *eU = eL + i3 * FAST_TC + r0, *e3 = eL + (i3 + 3) * FAST_TC + r0;
+        const int nfull = (has_full && need_full) ? (p.gen == LTDI_GEN_20 ? 14 : 6) : 0;
+        const int i0 = (int)(nf - y0);
+        const double lfa_hi = p.gen == LTDI_GEN_15 ? 1.0 : 2.0, lfa_lo = p.gen == LTDI_GEN_15 ? 0.5 : 1.5;
 #pragma unroll 1
-            for (int tm = 0; tm < nterm; ++tm) {
+        for (int tm = nfull ? 0 : 14; tm < ((has_lfa && need_lfa) ? 16 : nfull); tm = (tm + 1 == nfull ? 14 : tm + 1)) {
+            const bool lt = has_lfa && (!has_full || tm >= 14);
+            const double *anc_t, *xs;
+            const float *xfs;
+            double cP, c2, cU, c3, sgn = 0.0;
+            if (!lt) {
                 const TermDef td = c_term_def[tm];
                 const DelayDef df = c_delay_def[td.delay];
-                double D[FAST_TC_R], acc[FAST_TC_R];
+                const int series = td.series == 0 ? i2 : td.series == 1 ? i2 + 3 : td.series == 2 ? i3 + 3 : i3; /* P Q U W */
+                const int off = series * yr + i0 - (int)s_hdr[4 * (13 * ch + td.delay) + 1] - (H - 1);
+                anc_t = sa + (13 * ch + td.delay) * ANC;
+                xs = yF + off;
+                xfs = yFf + off;
+                cP = (double)((df.base == 1) + df.i); c2 = (double)df.i;
+                cU = (double)((df.base == 2) + df.j); c3 = (double)df.j;
+                sgn = (double)td.sign;
+            } else {
+                const int id = tm - 14;   /* 0: d/dt y_{p2} at L_p3 + L_p2 / 2 (gen 1.5);  1: d/dt y_{p3} at L_p2 + L_p3 / 2 */
+                const int off = (id == 0 ? i2 : i3) * yr + i0 - (int)s_hdr[4 * (FAST_NA_FULL + 2 * ch + id) + 1] - (H - 1);
+                anc_t = sa_lfa + (2 * ch + id) * ANC;
+                xs = dL + off;
+                xfs = dLf + off;
+                cP = 0.0; c3 = 0.0;
+                c2 = id == 0 ? lfa_lo : lfa_hi;
+                cU = id == 0 ? lfa_hi : lfa_lo;
+            }
+            double s0[FAST_TC_R], s1[FAST_TC_R];
+            float s2[FAST_TC_R];
+            term7<M>(anc_t, xs, xfs, s0, s1, s2);
 #pragma unroll
-                for (int r = 0; r < FAST_TC_R; ++r) {
-                    const double base = df.base == 1 ? DP[r] : (df.base == 2 ? DU[r] : 0.0);
-                    D[r] = fma((double)df.j, Db[r], fma((double)df.i, Da[r], base));
-                    acc[r] = 0.0;
+            for (int r = 0; r < FAST_TC_R; ++r) {
+                const double D = fma(cP, eP[r], fma(c2, e2[r], fma(cU, eU[r], c3 * e3[r]))) * p.inv_dt;
+                const double v = fma(D, fma(D, (double)s2[r], s1[r]), s0[r]);
+                if (!lt) Xf[r] = fma(sgn, v, Xf[r]);
+                else {
+                    const int64_t n = min(nf + r, p.n - 1);
+                    const double L2 = tabL[i2 * p.stride + n], L3 = tabL[i3 * p.stride + n];
+                    const double pre = p.gen == LTDI_GEN_15 ? 4.0 : 8.0 * (L2 + L3);   /* (B25) / (B33) */
+                    Xl[r] = fma(tm == 14 ? pre * L3 : -(pre * L2), v, Xl[r]);
                 }
-                const int q = (int)hd[4 * td.delay + 1];
-                const double *x = ser[td.series] + ((int)(nf - y0) - q - (H - 1));
-                term7<M>(sa + (13 * ch + td.delay) * (M * 4), x, D, acc);
-                const double sgn = (double)td.sign;
-#pragma unroll
-                for (int r = 0; r < FAST_TC_R; ++r) Xf[r] = fma(sgn, acc[r], Xf[r]);
             }
-            /* the two undelayed terms: + Q(t) - W(t) */
-            const int i0 = (int)(nf - y0);
-#pragma unroll
-            for (int r = 0; r < FAST_TC_R; ++r) Xf[r] += ser[1][i0 + r] - ser[3][i0 + r];
         }
-        if (need_lfa) {
-            const double *hl = s_hdr + 4 * (FAST_NA_FULL + 2 * ch);
-            const double *a_l = sa + (FAST_NA_FULL + 2 * ch) * (M * 4);
-            const double *d123 = dL + i2 * yr, *d231 = dL + i3 * yr;
-            double L2[FAST_TC_R], L3[FAST_TC_R], D[FAST_TC_R], acc2[FAST_TC_R], acc3[FAST_TC_R];
+        if (has_full && need_full) { /* the two undelayed terms: + Q(t) - W(t) */
+            const double *Q = yF + (i2 + 3) * yr + i0, *W = yF + i3 * yr + i0;
 #pragma unroll
-            for (int r = 0; r < FAST_TC_R; ++r) {
-                const int64_t n = min(nf + r, p.n - 1);
-                L2[r] = tabL[i2 * p.stride + n];
-                L3[r] = tabL[i3 * p.stride + n];
-                /* gen 1.5: L3 + L2/2 | gen 2.0: 2 L3 + 3 L2 / 2 */
-                const double e2 = cp2 - L2[r], e3 = cU - L3[r];
-                D[r] = (p.gen == LTDI_GEN_15 ? e3 + 0.5 * e2 : 2.0 * e3 + 1.5 * e2) * p.inv_dt;
-                acc2[r] = 0.0;
-                acc3[r] = 0.0;
-            }
-            const int base = (int)(nf - y0) - (H - 1);
-            term7<M>(a_l, d123 + (base - (int)hl[1]), D, acc2);
-#pragma unroll
-            for (int r = 0; r < FAST_TC_R; ++r) {
-                const double e2 = cp2 - L2[r], e3 = cU - L3[r];
-                D[r] = (p.gen == LTDI_GEN_15 ? e2 + 0.5 * e3 : 2.0 * e2 + 1.5 * e3) * p.inv_dt;
-            }
-            term7<M>(a_l + M * 4, d231 + (base - (int)hl[5]), D, acc3);
-#pragma unroll
-            for (int r = 0; r < FAST_TC_R; ++r) {
-                if (p.gen == LTDI_GEN_15) Xl[r] = 4.0 * (L3[r] * acc2[r] - L2[r] * acc3[r]);              /* (B25) */
-                else Xl[r] = 8.0 * (L2[r] + L3[r]) * (L3[r] * acc2[r] - L2[r] * acc3[r]);                /* (B33) */
-            }
+            for (int r = 0; r < FAST_TC_R; ++r) Xf[r] += Q[r] - W[r];
         }
     } else {
         /* exact per-sample weights */
-        const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
         for (int r = 0; r < FAST_TC_R; ++r) {
             const int64_t n = nf + r;
             if (n >= n1) break;
             double L[6];
             for (int l = 0; l < 6; ++l) L[l] = tabL[l * p.stride + n];
             const int idx = (int)(n - y0);
-            if (need_full) {
+            if (has_full && need_full) {
                 const double *ser[4] = {yF + i2 * yr, yF + (i2 + 3) * yr, yF + (i3 + 3) * yr, yF + i3 * yr};
                 const double dP = L[i2 + 3], dU = L[i3], a = L[i2 + 3] + L[i2], bb = L[i3] + L[i3 + 3];
                 const int nterm = p.gen == LTDI_GEN_20 ? 14 : 6;
@@ -743,7 +817,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
                 }
                 Xf[r] = x;
             }
-            if (need_lfa) {
+            if (has_lfa && need_lfa) {
                 const double L2 = L[i2], L3 = L[i3];
                 const double v2 = slow_delayed<M>(dL + i2 * yr, yr, idx, lfa_delay(p.gen, 0, L2, L3), p.dt, p.inv_dt);
                 const double v3 = slow_delayed<M>(dL + i3 * yr, yr, idx, lfa_delay(p.gen, 1, L2, L3), p.dt, p.inv_dt);
@@ -751,20 +825,21 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
             }
         }
     }
+    __syncthreads();   /* every thread is done with eL: R becomes X, Y, Z */
 
     /* blend (4.6), margins, exchange through shared memory */
 #pragma unroll
     for (int r = 0; r < FAST_TC_R; ++r) {
         const int64_t n = nf + r;
         double x;
-        if (p.which == LTDI_RESPONSE_FULL) x = Xf[r];
-        else if (p.which == LTDI_RESPONSE_LFA) x = Xl[r];
+        if (WHICH == LTDI_RESPONSE_FULL) x = Xf[r];
+        else if (WHICH == LTDI_RESPONSE_LFA) x = Xl[r];
         else {
             double wa, wb;
             hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
             x = 0.0;
-            if (need_lfa && wa != 0.0) x = wa * Xl[r];
-            if (need_full && wb != 0.0) x = fma(wb, Xf[r], x);
+            if (has_lfa && need_lfa && wa != 0.0) x = wa * Xl[r];
+            if (has_full && need_full && wb != 0.0) x = fma(wb, Xf[r], x);
         }
         if (!(n >= p.lo && n < p.n - p.hi)) x = 0.0;
         Xs[ch * FAST_TC + r0 + r] = x;
@@ -773,6 +848,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
 
     const double is2 = 0.70710678118654752440, is6 = 0.40824829046386301637, is3 = 0.57735026918962576451;
     const int64_t src_off = b * p.ld;
+    const int64_t ystride = p.batch * p.lds;
     for (int i = tid; i < FAST_TC; i += FAST_TC_THREADS) {
         const int64_t n = n0 + i;
         if (n >= n1) break;
@@ -786,20 +862,36 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
             p.XYZ[((int64_t)2 * p.batch_all + p.b0 + b) * p.ld + n] = Z;
         }
         if (p.Y) {
+            /* optional link output: the LFA links come back from the scratch series (their shared copy is gone) */
             const int iy = (int)(n - y0);
+            const double *gl = p.yL + b * p.lds + n;
             double wa = 1.0, wb = 1.0;
-            if (p.which == LTDI_RESPONSE_HYBRID) hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+            if (WHICH == LTDI_RESPONSE_HYBRID) hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
 #pragma unroll
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
-                if (p.which == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
-                else if (p.which == LTDI_RESPONSE_LFA) v = l < 3 ? yL[l * (yr + 2 * w) + iy + w] : 0.0;
+                if (WHICH == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
+                else if (WHICH == LTDI_RESPONSE_LFA) v = l < 3 ? gl[l * ystride] : 0.0;
                 else if (n >= p.m1 + w && n < p.n - p.m1 - w) { /* (4.5) */
-                    if (need_lfa && l < 3 && wa != 0.0) v = wa * yL[l * (yr + 2 * w) + iy + w];
+                    if (need_lfa && l < 3 && wa != 0.0) v = wa * gl[l * ystride];
                     if (need_full && wb != 0.0) v = fma(wb, yF[l * yr + iy], v);
                 }
                 p.Y[((int64_t)l * p.batch_all + p.b0 + b) * p.ld + n] = v;
             }
         }
     }
+}
+
+/* dynamic shared memory of tdi_kernel<M> in bytes (mirrors the carve-up above) */
+template <int M>
+static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
+{
+    const bool has_full = which != LTDI_RESPONSE_LFA, has_lfa = which != LTDI_RESPONSE_FULL;
+    const size_t yr = FAST_TC + (size_t)m2 + M / 2 + 2;
+    size_t dbl = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0)) * FAST_ANC_DOUBLES(M);
+    dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
+    const size_t r_len = std::max((size_t)6 * FAST_TC, has_lfa ? 3 * (yr + 2 * (size_t)w) : (size_t)0);
+    dbl += r_len;
+    const size_t flt = (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
+    return dbl * sizeof(double) + (flt * sizeof(float) + 15) / 16 * 16;
 }

@@ -189,7 +189,7 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
     const size_t cap = (size_t)96 << 20; /* bytes of scratch per chunk */
     int64_t chunk = (int64_t)(cap / ((size_t)rows * f.lds * sizeof(double)));
     f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
-    f.anc = (size_t)f.ntilesC * FAST_NA * M * 4;
+    f.anc = (size_t)f.ntilesC * FAST_NA * FAST_ANC_DOUBLES(M);
     f.hdr = (size_t)f.ntilesC * FAST_NA * 4;
     f.y = (size_t)rows * f.chunk * f.lds;
     f.total = work_doubles(batch) + f.anc + f.hdr + f.y;
@@ -272,14 +272,15 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     p.anc = anc; p.anc_hdr = hdr;
 
     const bool full = which != LTDI_RESPONSE_LFA, lfa = which != LTDI_RESPONSE_FULL;
-    const int yr = FAST_TC + (int)mg.m2 + H + 2, w = (int)mg.w;
     const size_t smem_link = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
-    const size_t smem_tdi = ((size_t)(full ? 6 * yr : 0) + (lfa ? 3 * (yr + 2 * w) + 3 * yr : 0) + FAST_NA * M * 4 +
-                             3 * FAST_TC) * sizeof(double);
+    const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
     int rc;
     if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
     if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link, smem_max))) return rc;
-    if ((rc = set_smem(tdi_kernel<M>, smem_tdi, smem_max))) return rc;
+    void (*tdi)(FastParams) = which == LTDI_RESPONSE_FULL  ? tdi_kernel<M, LTDI_RESPONSE_FULL>
+                              : which == LTDI_RESPONSE_LFA ? tdi_kernel<M, LTDI_RESPONSE_LFA>
+                                                           : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
+    if ((rc = set_smem(tdi, smem_tdi, smem_max))) return rc;
 
     {
         ProfScope ps(LTDI_KERNEL_ANCHOR + LTDI_KERNEL_COUNT * which, st);
@@ -310,7 +311,7 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         }
         {
             ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
-            tdi_kernel<M><<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
+            tdi<<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
         }
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
