@@ -229,10 +229,12 @@ class Workspace:
         self.A, self.E, self.T = (torch.empty(batch, ld, **kw) for _ in range(3))
         self.XYZ = torch.empty(3, batch, ld, **kw) if want_xyz else None
         self.y = torch.empty(6, batch, ld, **kw) if want_y else None
-        nbytes = C.c_size_t()
-        _check("ltdi_workspace_bytes",
-               lib().ltdi_workspace_bytes(RESPONSE_HYBRID, ld, batch, GEN_20, 31, C.byref(nbytes)))
-        self.work = torch.empty(nbytes.value // 8, **kw)
+        need = 0   # one scratch buffer that serves every response (the chunking differs per response)
+        for which in (RESPONSE_FULL, RESPONSE_LFA, RESPONSE_HYBRID):
+            nbytes = C.c_size_t()
+            _check("ltdi_workspace_bytes", lib().ltdi_workspace_bytes(which, ld, batch, GEN_20, 31, C.byref(nbytes)))
+            need = max(need, nbytes.value)
+        self.work = torch.empty(need // 8, **kw)
 
     def outputs(self):
         return {"A": self.A, "E": self.E, "T": self.T, "XYZ": self.XYZ, "y": self.y}

@@ -482,7 +482,10 @@ int ltdi_host_scratch_bytes(int64_t ld, int64_t batch, size_t *bytes)
 {
     if (ld < 1 || batch < 1 || !bytes) return LTDI_EINVAL;
     const size_t series = ((size_t)ld * (size_t)batch * sizeof(double) + 255) / 256 * 256;
-    *bytes = 5 * series + (fast_layout(LTDI_RESPONSE_HYBRID, ld, batch, 32).total * sizeof(double) + 255) / 256 * 256;
+    size_t work = 0; /* the chunking of the link scratch differs per response: size for the largest */
+    for (int which = LTDI_RESPONSE_FULL; which <= LTDI_RESPONSE_HYBRID; ++which)
+        work = std::max(work, fast_layout(which, ld, batch, 32).total);
+    *bytes = 5 * series + (work * sizeof(double) + 255) / 256 * 256;
     return LTDI_OK;
 }
 
