@@ -69,6 +69,19 @@ struct FastParams {
 // ---------------------------------------------------------------------------------------------
 // helpers
 // ---------------------------------------------------------------------------------------------
+// Ampere-style asynchronous copies (LDGSTS): the staging loops issue all their loads at once and wait once
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // s = d / dt to within one rounding of the correctly rounded quotient (one Newton correction)
 __device__ __forceinline__ double div_dt(double d, double dt, double inv_dt)
 {
@@ -241,11 +254,23 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
     const int hw2 = (int)((FAST_TA + 2 * p.m1 + 4) / 2);   /* pairs */
     double *he_p = smem, *ho_p = he_p + hw2, *he_c = ho_p + hw2, *ho_c = he_c + hw2;
     const double *gp = p.hp + b * p.ld, *gc = p.hc + b * p.ld;
+    /* orbit-table rows of the tile: rows 0..23 (full) or 0..20 (LFA: R, n, L_+l), [row][FAST_TA] */
+    constexpr int NROWS = LFA ? ROW_L + 3 : LTDI_TABLE_ROWS;
+    double *tb = ho_c + hw2;
+    for (int i = tid; i < NROWS * (FAST_TA / 2); i += FAST_TA_THREADS) {
+        const int r = i / (FAST_TA / 2), c = 2 * (i - r * (FAST_TA / 2));
+        if (a0 + c < p.stride) cp_async16(tb + r * FAST_TA + c, p.tab + (int64_t)r * p.stride + a0 + c);
+        else *reinterpret_cast<double2 *>(tb + r * FAST_TA + c) = make_double2(0.0, 0.0);
+    }
     for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
         const int64_t g = org + i;
         double vp = 0.0, vc = 0.0;
         if (!LFA) {
-            if (g >= 0 && g < p.n) { vp = gp[g]; vc = gc[g]; }
+            if (g >= 0 && g < p.n) {
+                cp_async8(((i & 1) ? ho_p : he_p) + (i >> 1), gp + g);
+                cp_async8(((i & 1) ? ho_c : he_c) + (i >> 1), gc + g);
+                continue;
+            }
         } else if (g >= w && g < p.n - w) {
             if (w == 1) {
                 vp = gp[g + 1] - gp[g - 1];
@@ -259,6 +284,7 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
         dp[i >> 1] = vp;
         dc[i >> 1] = vc;
     }
+    cp_async_wait_all();
     __syncthreads();
 
     const int64_t m0 = a0 + 2 * tid;
@@ -275,64 +301,74 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
         return;
     }
 
-    const double *t = p.tab + m0;
+    const double *t = tb + 2 * tid;
     const double inv_c = 1.0 / LTDI_C_LIGHT;
-    auto row2 = [&](int r) { return *reinterpret_cast<const double2 *>(t + (int64_t)r * p.stride); };
+    auto row2 = [&](int r) { return *reinterpret_cast<const double2 *>(t + r * FAST_TA); };
+    /* k . R_i / c [s] of the two samples; i may be a run-time index (rows come from shared memory) */
     auto kdotR = [&](int i, double &k0, double &k1) {
         const double2 x = row2(ROW_R + 3 * i), y = row2(ROW_R + 3 * i + 1), z = row2(ROW_R + 3 * i + 2);
         k0 = (fr[0] * x.x + fr[1] * y.x + fr[2] * z.x) * inv_c;
         k1 = (fr[0] * x.y + fr[1] * y.y + fr[2] * z.y) * inv_c;
     };
-
-    if (!LFA) {
-        double rp0[3], rc0[3], rp1[3], rc1[3]; /* h+, hx at the receiver times t - k.R_r / c (2.6b) */
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            double k0, k1;
-            kdotR(i, k0, k1);
-            interp_delays<H>(p, k0, k1, rel0, he_p, ho_p, he_c, ho_c, rp0[i], rc0[i], rp1[i], rc1[i]);
+    /* F^+, F^x (2.2)-(2.4) with G17 and k . n of link |l| = a + 1 for the two samples */
+    auto patterns = [&](int a, double &Fp0, double &Fc0, double &kn0, double &Fp1, double &Fc1, double &kn1) {
+        const double2 nx = row2(ROW_N + 3 * a), ny = row2(ROW_N + 3 * a + 1), nz = row2(ROW_N + 3 * a + 2);
+        {
+            const double un = fr[3] * nx.x + fr[4] * ny.x + fr[5] * nz.x;
+            const double vn = fr[6] * nx.x + fr[7] * ny.x + fr[8] * nz.x;
+            kn0 = fr[0] * nx.x + fr[1] * ny.x + fr[2] * nz.x;
+            const double xip = un * un - vn * vn, xic = 2.0 * un * vn;   /* (2.4) */
+            Fp0 = xip * fr[9] + xic * fr[10];                              /* (2.2) + (2.3), G17 */
+            Fc0 = xic * fr[9] - xip * fr[10];
         }
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const double2 nx = row2(ROW_N + 3 * a), ny = row2(ROW_N + 3 * a + 1), nz = row2(ROW_N + 3 * a + 2);
-            double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
-            {
-                const double un = fr[3] * nx.x + fr[4] * ny.x + fr[5] * nz.x;
-                const double vn = fr[6] * nx.x + fr[7] * ny.x + fr[8] * nz.x;
-                kn0 = fr[0] * nx.x + fr[1] * ny.x + fr[2] * nz.x;
-                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;   /* (2.4) */
-                Fp0 = xip * fr[9] + xic * fr[10];                              /* (2.2) + (2.3), G17 */
-                Fc0 = xic * fr[9] - xip * fr[10];
-            }
-            {
-                const double un = fr[3] * nx.y + fr[4] * ny.y + fr[5] * nz.y;
-                const double vn = fr[6] * nx.y + fr[7] * ny.y + fr[8] * nz.y;
-                kn1 = fr[0] * nx.y + fr[1] * ny.y + fr[2] * nz.y;
-                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
-                Fp1 = xip * fr[9] + xic * fr[10];
-                Fc1 = xic * fr[9] - xip * fr[10];
-            }
-#pragma unroll
-            for (int sg = 0; sg < 2; ++sg) {
-                const int l = a + 3 * sg;
-                const int s = link_sender(l), r = link_receiver(l);
-                double k0, k1;
-                kdotR(s, k0, k1);
+        {
+            const double un = fr[3] * nx.y + fr[4] * ny.y + fr[5] * nz.y;
+            const double vn = fr[6] * nx.y + fr[7] * ny.y + fr[8] * nz.y;
+            kn1 = fr[0] * nx.y + fr[1] * ny.y + fr[2] * nz.y;
+            const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
+            Fp1 = xip * fr[9] + xic * fr[10];
+            Fc1 = xic * fr[9] - xip * fr[10];
+        }
+    };
+
+    /* ONE instance of the pair interpolator in a rolled loop: the kernel stays small enough for the instruction
+     * cache (nine inlined copies made 113 KB of code and "no instruction" the top stall reason). */
+    if (!LFA) {
+        /* step = 3 r + s: receiver spacecraft r, then the two links it receives: s = 1: link +((r+2)%3 + 1) sent by
+         * spacecraft (r+1)%3, s = 2: link -((r+1)%3 + 1) sent by spacecraft (r+2)%3 */
+        double rp0 = 0.0, rc0 = 0.0, rp1 = 0.0, rc1 = 0.0; /* h+, hx at the receiver time t - k.R_r / c (2.6b) */
+#pragma unroll 1
+        for (int step = 0; step < 9; ++step) {
+            const int r = step / 3, s = step - 3 * r;
+            const int a = s == 1 ? (r + 2) % 3 : (r + 1) % 3;   /* |l| - 1 */
+            const int l = s == 2 ? a + 3 : a;
+            const int sc = s == 0 ? r : (s == 1 ? (r + 1) % 3 : (r + 2) % 3);
+            double k0, k1;
+            kdotR(sc, k0, k1);
+            double d0 = k0, d1 = k1;
+            if (s != 0) {
                 const double2 L = row2(ROW_L + l);
-                double sp0, sc0, sp1, sc1;
-                interp_delays<H>(p, L.x + k0, L.y + k1, rel0, he_p, ho_p, he_c, ho_c, sp0, sc0, sp1, sc1); /* (2.6a) */
-                const double d0 = 2.0 * (1.0 - (sg ? -kn0 : kn0)), d1 = 2.0 * (1.0 - (sg ? -kn1 : kn1));
-                const double y0 = (Fp0 * (sp0 - rp0[r]) + Fc0 * (sc0 - rc0[r])) / d0;   /* (2.5) */
-                const double y1 = (Fp1 * (sp1 - rp1[r]) + Fc1 * (sc1 - rc1[r])) / d1;
+                d0 = L.x + k0;                                           /* (2.6a) */
+                d1 = L.y + k1;
+            }
+            double ap0, ac0, ap1, ac1;
+            interp_delays<H>(p, d0, d1, rel0, he_p, ho_p, he_c, ho_c, ap0, ac0, ap1, ac1);
+            if (s == 0) {
+                rp0 = ap0; rc0 = ac0; rp1 = ap1; rc1 = ac1;
+            } else {
+                double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
+                patterns(a, Fp0, Fc0, kn0, Fp1, Fc1, kn1);
+                const double e0 = 2.0 * (1.0 - (s == 2 ? -kn0 : kn0)), e1 = 2.0 * (1.0 - (s == 2 ? -kn1 : kn1));
+                const double y0 = (Fp0 * (ap0 - rp0) + Fc0 * (ac0 - rc0)) / e0;   /* (2.5) */
+                const double y1 = (Fp1 * (ap1 - rp1) + Fc1 * (ac1 - rc1)) / e1;
                 *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
             }
         }
     } else {
         const double den = (w == 1 ? 2.0 : 12.0) * p.dt;
-#pragma unroll
+#pragma unroll 1
         for (int l = 0; l < 3; ++l) {
             const int s = link_sender(l), r = link_receiver(l);
-            const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
             double ks0, ks1, kr0, kr1;
             kdotR(s, ks0, ks1);
             kdotR(r, kr0, kr1);
@@ -340,21 +376,10 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
             double ap0, ac0, ap1, ac1;
             interp_delays<H>(p, 0.5 * L.x + 0.5 * (ks0 + kr0), 0.5 * L.y + 0.5 * (ks1 + kr1), rel0, he_p, ho_p, he_c,
                              ho_c, ap0, ac0, ap1, ac1);                                    /* (B1) */
-            double y0, y1;
-            {
-                const double un = fr[3] * nx.x + fr[4] * ny.x + fr[5] * nz.x;
-                const double vn = fr[6] * nx.x + fr[7] * ny.x + fr[8] * nz.x;
-                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
-                const double Fp = xip * fr[9] + xic * fr[10], Fc = xic * fr[9] - xip * fr[10];
-                y0 = -(0.5 * L.x) * (Fp * (ap0 / den) + Fc * (ac0 / den));                 /* (B10) */
-            }
-            {
-                const double un = fr[3] * nx.y + fr[4] * ny.y + fr[5] * nz.y;
-                const double vn = fr[6] * nx.y + fr[7] * ny.y + fr[8] * nz.y;
-                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;
-                const double Fp = xip * fr[9] + xic * fr[10], Fc = xic * fr[9] - xip * fr[10];
-                y1 = -(0.5 * L.y) * (Fp * (ap1 / den) + Fc * (ac1 / den));
-            }
+            double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
+            patterns(l, Fp0, Fc0, kn0, Fp1, Fc1, kn1);
+            const double y0 = -(0.5 * L.x) * (Fp0 * (ap0 / den) + Fc0 * (ac0 / den));      /* (B10) */
+            const double y1 = -(0.5 * L.y) * (Fp1 * (ap1 / den) + Fc1 * (ac1 / den));
             *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
         }
     }
@@ -576,19 +601,6 @@ __device__ __forceinline__ float to_f32(double v)
     const float f = (float)v;
     return fabsf(f) <= 3.0e38f ? f : 0.f;
 }
-
-// Ampere-style asynchronous copies (LDGSTS): the staging loops issue all their loads at once and wait once
-__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>

@@ -272,11 +272,14 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     p.anc = anc; p.anc_hdr = hdr;
 
     const bool full = which != LTDI_RESPONSE_LFA, lfa = which != LTDI_RESPONSE_FULL;
-    const size_t smem_link = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
+    /* staged strain (4 parity-split series) + the orbit-table rows of the tile */
+    const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
+    const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
+    const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double);
     const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
     int rc;
     if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
-    if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link, smem_max))) return rc;
+    if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link_lfa, smem_max))) return rc;
     void (*tdi)(FastParams) = which == LTDI_RESPONSE_FULL  ? tdi_kernel<M, LTDI_RESPONSE_FULL>
                               : which == LTDI_RESPONSE_LFA ? tdi_kernel<M, LTDI_RESPONSE_LFA>
                                                            : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
@@ -306,7 +309,7 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         }
         if (lfa) {
             ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
-            link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+            link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
             count_launch();
         }
         {
