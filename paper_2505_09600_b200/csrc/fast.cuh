@@ -3,10 +3,11 @@
 // Three kernels per response, the link series y_slr travelling through an L2-resident scratch:
 //
 //   anchor_kernel   per time tile of the TDI stage and per distinct TDI delay: integer shift q, and the
-//                   Lagrange weights w_k(eps_c) with their first and second derivatives at the tile-centre
-//                   delay.  The TDI delays (sums of L_l(t_n)) drift by < 1e-7 samples over a tile, so
-//                   w_k(eps_n) = w_k(eps_c) + D w_k' + D^2 w_k''/2 with D = eps_n - eps_c is exact to rounding
-//                   (|D| <= 1e-6 is checked per tile; a tile that fails, or whose q changes, takes the exact
+//                   Lagrange weights w_k(eps_c) with their first derivative at the tile-centre delay.  The TDI
+//                   delays (sums of L_l(t_n)) drift by ~1e-7 samples over a tile, so w_k(eps_n) =
+//                   w_k(eps_c) + D w_k' with D = eps_n - eps_c: the neglected term (D^2 / 2) sum_k w_k'' x_k =
+//                   (D^2 / 2) dt^2 x''(t) is <= 1.3e-13 (omega dt)^2 |x| for the checked bound |D| <= 5e-7
+//                   (a tile that fails the check, or whose q changes, takes the exact
 //                   per-sample weights instead).  The weights do not depend on the source: a batch shares them.
 //   link_kernel     S2 + S3 (Eq. 2.4-2.6) resp. S6 (Eq. B10): one thread owns TWO consecutive samples, builds
 //                   the per-sample weights of each of the 9 (3) retarded times from the symmetric pair form
@@ -37,9 +38,9 @@
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
 #define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
 #define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
-#define FAST_DMAX 1.0e-6                  /* |eps_n - eps_c| bound for the second-order weights */
-/* one anchor = [M] double2 {w_k, w_k'} followed by [M] float w_k''/2 (padded to 16 bytes), in doubles */
-#define FAST_ANC_DOUBLES(M) (2 * (M) + 2 * (((M) + 3) / 4))
+#define FAST_DMAX 5.0e-7                  /* |eps_n - eps_c| bound for the first-order weights */
+/* one anchor = [M] double2 {w_k, w_k'}, in doubles */
+#define FAST_ANC_DOUBLES(M) (2 * (M))
 
 /* lambda_i and kappa_i = -lambda_i (i + 1/2)^2 for H = 5 (row 0) and H = 16 (row 1) */
 __constant__ double c_sym_lam[2][16];
@@ -484,45 +485,44 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
     double *h = hdr + (tile * FAST_NA + tid) * 4;
     h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? 1.0 : 0.0;
 
-    /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); first and second
-     * derivatives by the product rule carried along the same sweeps (registers; one coalesced-ish store at the end) */
-    double *out = anc + (tile * FAST_NA + tid) * (int64_t)FAST_ANC_DOUBLES(M);
-    float *out2 = reinterpret_cast<float *>(out + 2 * M);
+    /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); the first derivative
+     * by the product rule carried along the same sweeps */
+    double2 *out = reinterpret_cast<double2 *>(anc + (tile * FAST_NA + tid) * (int64_t)FAST_ANC_DOUBLES(M));
     const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
     constexpr int kmin = -(M / 2 - 1);
-    double pf[M], pf1[M], pf2[M];
+    double pf[M], pf1[M];
     {
-        double f = 1.0, f1 = 0.0, f2 = 0.0;
+        double f = 1.0, f1 = 0.0;
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            pf[i] = f; pf1[i] = f1; pf2[i] = f2;
+            pf[i] = f; pf1[i] = f1;
             const double e = eps - (double)(kmin + i);
-            f2 = f2 * e + 2.0 * f1;
             f1 = f1 * e + f;
             f = f * e;
         }
     }
-    double g = 1.0, g1 = 0.0, g2 = 0.0;
+    double g = 1.0, g1 = 0.0;
 #pragma unroll
     for (int i = M - 1; i >= 0; --i) {
-        const double a0 = pf[i], a1 = pf1[i], a2 = pf2[i];
         double2 o;
-        o.x = c[i] * (a0 * g);
-        o.y = c[i] * (a1 * g + a0 * g1);
-        *reinterpret_cast<double2 *>(out + 2 * i) = o;
-        out2[i] = (float)(0.5 * (c[i] * (a2 * g + 2.0 * a1 * g1 + a0 * g2)));   /* w'' / 2 */
+        o.x = c[i] * (pf[i] * g);
+        o.y = c[i] * (pf1[i] * g + pf[i] * g1);
+        out[i] = o;
         const double e = eps - (double)(kmin + i);
-        g2 = g2 * e + 2.0 * g1;
         g1 = g1 * e + g;
         g = g * e;
     }
-#pragma unroll
-    for (int i = M; i < 4 * ((M + 3) / 4); ++i) out2[i] = 0.f;
 }
 
 // ---------------------------------------------------------------------------------------------
 // TDI kernel
 // ---------------------------------------------------------------------------------------------
+// staged link window of a TDI tile: it starts tdi_back(m2) >= m2 samples before the tile (even, so that the
+// rows can be copied in 16-byte pieces) and holds tdi_yr<M>(m2) samples (even)
+__host__ __device__ __forceinline__ int tdi_back(int64_t m2) { return (int)((m2 + 1) & ~(int64_t)1); }
+template <int M>
+__host__ __device__ __forceinline__ int tdi_yr(int64_t m2) { return (FAST_TC + tdi_back(m2) + M / 2 + 2 + 1) & ~1; }
+
 // exact per-sample interpolation of a staged series (slow path): ys[0] = sample y0, length len
 template <int M>
 __device__ __noinline__ double slow_delayed(const double *ys, int len, int idx /* n - y0 */, double delay, double dt,
@@ -560,46 +560,30 @@ __device__ __forceinline__ void hybrid_weights_fast(const double *h, double t, d
 
 
 // FAST_TC_R consecutive outputs of one interpolated term.  With D = eps_n - eps_c,
-//   sum_k w_k(eps_c + D) x_k = S0 + D (S1 + D S2),   S_m = sum_k w_k^(m)(eps_c) / m!  x_k :
-// three constant-coefficient FIR filters over the tile.  S0 and S1 are accumulated in fp64 (2 DFMA per tap and
-// sample, FAST_TC_R x 2 independent chains); S2 enters multiplied by D^2 <= 1e-12, so fp32 carries it (its
-// rounding, <= 1e-5 |x|, contributes <= 1e-17 |x|) on the FMA pipe, which issues beside the FP64 pipe.
+//   sum_k w_k(eps_c + D) x_k = S0 + D S1,   S_m = sum_k w_k^(m)(eps_c) x_k :
+// two constant-coefficient FIR filters over the tile, 2 DFMA per tap and sample in FAST_TC_R x 2 independent
+// chains; the weights are broadcast reads, the samples slide through a register window.
 template <int M>
 __device__ __forceinline__ void term7(const double *__restrict__ anc, const double *__restrict__ x,
-                                      const float *__restrict__ xf, double (&s0)[FAST_TC_R], double (&s1)[FAST_TC_R],
-                                      float (&s2)[FAST_TC_R])
+                                      double (&s0)[FAST_TC_R], double (&s1)[FAST_TC_R])
 {
     const double2 *w01 = reinterpret_cast<const double2 *>(anc);
-    const float4 *w2 = reinterpret_cast<const float4 *>(anc + 2 * M);
     double win[FAST_TC_R];
-    float wf[FAST_TC_R];
 #pragma unroll
-    for (int r = 0; r < FAST_TC_R; ++r) { s0[r] = 0.0; s1[r] = 0.0; s2[r] = 0.f; }
+    for (int r = 0; r < FAST_TC_R; ++r) { s0[r] = 0.0; s1[r] = 0.0; }
 #pragma unroll
-    for (int r = 0; r < FAST_TC_R - 1; ++r) { win[r] = x[r]; wf[r] = xf[r]; }
-    float4 q2 = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int r = 0; r < FAST_TC_R - 1; ++r) win[r] = x[r];
 #pragma unroll
     for (int k = 0; k < M; ++k) {
         const double2 w = w01[k];
-        if ((k & 3) == 0) q2 = w2[k >> 2];
-        const float w2k = (k & 3) == 0 ? q2.x : (k & 3) == 1 ? q2.y : (k & 3) == 2 ? q2.z : q2.w;
         win[(k + FAST_TC_R - 1) % FAST_TC_R] = x[k + FAST_TC_R - 1];
-        wf[(k + FAST_TC_R - 1) % FAST_TC_R] = xf[k + FAST_TC_R - 1];
 #pragma unroll
         for (int r = 0; r < FAST_TC_R; ++r) {
             const double xv = win[(k + r) % FAST_TC_R];
             s0[r] = fma(w.x, xv, s0[r]);
             s1[r] = fma(w.y, xv, s1[r]);
-            s2[r] = fmaf(w2k, wf[(k + r) % FAST_TC_R], s2[r]);
         }
     }
-}
-
-// finite float copy of a link sample for the fp32 second-order filter
-__device__ __forceinline__ float to_f32(double v)
-{
-    const float f = (float)v;
-    return fabsf(f) <= 3.0e38f ? f : 0.f;
 }
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
@@ -610,6 +594,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
     constexpr int H = M / 2;
     constexpr int ANC = FAST_ANC_DOUBLES(M);
     constexpr bool has_full = WHICH != LTDI_RESPONSE_LFA, has_lfa = WHICH != LTDI_RESPONSE_FULL;
+    constexpr int NLR = has_full ? 6 : 3;   /* light-time rows the tile needs (LFA: the positive links) */
     const int64_t b = (int64_t)blockIdx.x % p.batch;
     int64_t tile = (int64_t)blockIdx.x / p.batch;
     /* hybrid: tiles past t_hyb carry the 14-term full response; schedule them first (no long tail) */
@@ -630,45 +615,43 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
 
     /* shared memory (host: tdi_smem_bytes):
      *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
-     *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0)
-     *   R    scratch region, in turn: LFA links [3][yr + 2w] (element 0 = y0 - w) -> light times of the tile, then
-     *        their drifts eL [6][FAST_TC] -> X, Y, Z of the tile [3][FAST_TC]
-     *   yFf  [6][yr], dLf [3][yr]         float copies for the second-order filter */
-    const int yr = FAST_TC + (int)p.m2 + H + 2;
-    const int64_t y0 = n0 - p.m2;
+     *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0, even)
+     *   Lr   [NLR][FAST_TC] light times L_l(n0 + i) of the tile; after the term loop: X, Y, Z of the tile
+     *   yL   [3][yr + 2w] LFA links       (element 0 = sample y0 - w) */
+    const int yr = tdi_yr<M>(p.m2);
+    const int64_t y0 = n0 - tdi_back(p.m2);
     constexpr int na_full = has_full ? FAST_NA_FULL : 0;
     double *sa = smem;
     double *yF = sa + (size_t)(na_full + (has_lfa ? FAST_NA_LFA : 0)) * ANC;
     double *dL = yF + (has_full ? 6 * yr : 0);
-    double *R = dL + (has_lfa ? 3 * yr : 0);
-    const int r_len = max(6 * FAST_TC, has_lfa ? 3 * (yr + 2 * w) : 0);
-    float *yFf = reinterpret_cast<float *>(R + r_len);
-    float *dLf = yFf + (has_full ? 6 * yr : 0);
-    double *yL = R, *eL = R, *Xs = R;
+    double *Lr = dL + (has_lfa ? 3 * yr : 0);
+    double *yL = Lr + NLR * FAST_TC;
+    double *Xs = Lr;
     const double *sa_lfa = sa + (size_t)na_full * ANC;
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
-    const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
     __shared__ double s_hdr[FAST_NA * 4];
-    __shared__ double s_Lc[6];
-    __shared__ int s_ok;
 
     /* phase 0: every global read of the tile is issued asynchronously, then one wait */
-    auto stage_light_times = [&]() {
-        for (int i = tid; i < 6 * FAST_TC; i += FAST_TC_THREADS) {
-            const int l = i / FAST_TC, k = i - l * FAST_TC;
-            cp_async8(eL + i, tabL + l * p.stride + min(n0 + k, p.n - 1));
+    for (int i = tid; i < NLR * (FAST_TC / 2); i += FAST_TC_THREADS) {
+        const int l = i / (FAST_TC / 2), k = 2 * (i - l * (FAST_TC / 2));
+        const double *src = tabL + l * p.stride;
+        if (n0 + k + 1 < p.n) cp_async16(Lr + l * FAST_TC + k, src + n0 + k);
+        else {
+            Lr[l * FAST_TC + k] = src[min(n0 + k, p.n - 1)];
+            Lr[l * FAST_TC + k + 1] = src[p.n - 1];
         }
-    };
-    if (tid == 0) s_ok = 1;
-    if (tid < 6) s_Lc[tid] = tabL[tid * p.stride + nc];
+    }
     if (has_full && need_full) {
         const double *src = p.yF + b * p.lds;
         const int64_t ystride = p.batch * p.lds;
-        for (int i = tid; i < 6 * yr; i += FAST_TC_THREADS) {
-            const int l = i / yr, k = i - l * yr;
+        for (int i = tid; i < 6 * (yr / 2); i += FAST_TC_THREADS) {
+            const int l = i / (yr / 2), k = 2 * (i - l * (yr / 2));
             const int64_t g = y0 + k;
-            if (g >= 0 && g < p.n) cp_async8(yF + i, src + l * ystride + g);
-            else yF[i] = 0.0;
+            if (g >= 0 && g + 1 < p.n) cp_async16(yF + l * yr + k, src + l * ystride + g);
+            else {
+                yF[l * yr + k] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
+                yF[l * yr + k + 1] = (g + 1 >= 0 && g + 1 < p.n) ? src[l * ystride + g + 1] : 0.0;
+            }
         }
     }
     if (has_lfa && need_lfa) {
@@ -681,8 +664,6 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
             if (g >= 0 && g < p.n) cp_async8(yL + i, src + l * ystride + g);
             else yL[i] = 0.0;
         }
-    } else {
-        stage_light_times();
     }
     {
         const double *ga = p.anc + tile * (int64_t)(FAST_NA * ANC);
@@ -697,49 +678,33 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
     cp_async_wait_all();
     __syncthreads();
 
-    /* phase 1: float copies, anchor validity, derivative of the LFA links */
-    if (has_full && need_full)
-        for (int i = tid; i < 6 * yr; i += FAST_TC_THREADS) yFf[i] = to_f32(yF[i]);
-    if (tid < FAST_NA) {
-        const bool used = tid < FAST_NA_FULL ? (need_full && (p.gen == LTDI_GEN_20 || (tid % 13) < 6)) : need_lfa;
-        if (used && s_hdr[4 * tid + 3] == 0.0) s_ok = 0;
-    }
-    if (has_lfa && need_lfa) {
-        /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
-        const double dt = p.dt;
-        const int len = yr + 2 * w;
-        for (int i = tid; i < 3 * yr; i += FAST_TC_THREADS) {
-            const int l = i / yr, k = i - l * yr;
-            const int64_t m = y0 + k;
-            const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
-            const double *x = yL + l * len + k + w;
-            double d = 0.0;
-            if (in) {
-                if (p.gen == LTDI_GEN_15) {
-                    d = (w == 1) ? (x[1] - x[-1]) / (2.0 * dt) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2])) / (12.0 * dt);
-                } else {
-                    const double d1 = (x[1] - x[0]) - (x[0] - x[-1]);
-                    if (w == 1) d = d1 / (dt * dt);
-                    else {
-                        const double d2 = (x[2] - x[0]) - (x[0] - x[-2]);
-                        d = (16.0 * d1 - d2) / (12.0 * dt * dt);
+    /* phase 1 (LFA, hybrid): derivative of the LFA links */
+    if (has_lfa) {
+        if (need_lfa) {
+            /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
+            const double dt = p.dt;
+            const int len = yr + 2 * w;
+            for (int i = tid; i < 3 * yr; i += FAST_TC_THREADS) {
+                const int l = i / yr, k = i - l * yr;
+                const int64_t m = y0 + k;
+                const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
+                const double *x = yL + l * len + k + w;
+                double d = 0.0;
+                if (in) {
+                    if (p.gen == LTDI_GEN_15) {
+                        d = (w == 1) ? (x[1] - x[-1]) / (2.0 * dt) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2])) / (12.0 * dt);
+                    } else {
+                        const double d1 = (x[1] - x[0]) - (x[0] - x[-1]);
+                        if (w == 1) d = d1 / (dt * dt);
+                        else {
+                            const double d2 = (x[2] - x[0]) - (x[0] - x[-2]);
+                            d = (16.0 * d1 - d2) / (12.0 * dt * dt);
+                        }
                     }
                 }
+                dL[i] = d;
             }
-            dL[i] = d;
-            dLf[i] = to_f32(d);
         }
-    }
-    __syncthreads();   /* s_ok final; the LFA links in R are dead */
-
-    /* phase 2: light-time drifts eL[l][i] = L_l(n_c) - L_l(n0 + i): D = eps_n - eps_c = (d_c - d_n) / dt */
-    if (s_ok) {
-        if (has_lfa && need_lfa) {
-            stage_light_times();
-            cp_async_wait_all();
-            __syncthreads();
-        }
-        for (int i = tid; i < 6 * FAST_TC; i += FAST_TC_THREADS) eL[i] = s_Lc[i / FAST_TC] - eL[i];
         __syncthreads();
     }
 
@@ -751,13 +716,23 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
 #pragma unroll
     for (int r = 0; r < FAST_TC_R; ++r) { Xf[r] = 0.0; Xl[r] = 0.0; }
 
-    if (s_ok) {
+    /* every anchor this channel uses must be valid for the tile (the decision is per channel: no barrier needed) */
+    bool ok = true;
+    if (has_full && need_full) {
+        const int nd = p.gen == LTDI_GEN_20 ? 13 : 6;
+        for (int id = 0; id < nd; ++id) ok = ok && s_hdr[4 * (13 * ch + id) + 3] != 0.0;
+    }
+    if (has_lfa && need_lfa)
+        ok = ok && s_hdr[4 * (FAST_NA_FULL + 2 * ch) + 3] != 0.0 && s_hdr[4 * (FAST_NA_FULL + 2 * ch + 1) + 3] != 0.0;
+
+    if (ok) {
         /* one loop over the interpolated terms of this channel: 6 / 14 of Eq. (2.7) / (2.8) on the full links, then
          * the two of (B25) / (B33) on the differentiated LFA links.  Per term: anchor, series offset, and the
-         * coefficients of D = (cP eP + c2 e2 + cU eU + c3 e3) / dt in the light-time drifts of the channel's links
-         * (a = L_-p2 + L_p2 -> eP + e2, b = L_p3 + L_-p3 -> eU + e3, dP -> eP, dU -> eU; LFA: L_p2 -> e2, L_p3 -> eU) */
-        const double *eP = eL + (i2 + 3) * FAST_TC + r0, *e2 = eL + i2 * FAST_TC + r0;
-        const double *eU = eL + i3 * FAST_TC + r0, *e3 = eL + (i3 + 3) * FAST_TC + r0;
+         * coefficients of the delay d_n = cP L_-p2 + c2 L_p2 + cU L_p3 + c3 L_-p3 in the light times of the channel's
+         * links (a = L_-p2 + L_p2, b = L_p3 + L_-p3, dP = L_-p2, dU = L_p3; LFA: L_p2 and L_p3 only);
+         * D = eps_n - eps_c = (d_c - d_n) / dt */
+        const double *LP = Lr + (has_full ? (i2 + 3) * FAST_TC : 0) + r0, *L2p = Lr + i2 * FAST_TC + r0;
+        const double *LU = Lr + i3 * FAST_TC + r0, *L3m = Lr + (has_full ? (i3 + 3) * FAST_TC : 0) + r0;
         const int nfull = (has_full && need_full) ? (p.gen == LTDI_GEN_20 ? 14 : 6) : 0;
         const int i0 = (int)(nf - y0);
         const double lfa_hi = p.gen == LTDI_GEN_15 ? 1.0 : 2.0, lfa_lo = p.gen == LTDI_GEN_15 ? 0.5 : 1.5;
@@ -765,40 +740,37 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
         for (int tm = nfull ? 0 : 14; tm < ((has_lfa && need_lfa) ? 16 : nfull); tm = (tm + 1 == nfull ? 14 : tm + 1)) {
             const bool lt = has_lfa && (!has_full || tm >= 14);
             const double *anc_t, *xs;
-            const float *xfs;
-            double cP, c2, cU, c3, sgn = 0.0;
+            double cP, c2, cU, c3, dc, sgn = 0.0;
             if (!lt) {
                 const TermDef td = c_term_def[tm];
                 const DelayDef df = c_delay_def[td.delay];
                 const int series = td.series == 0 ? i2 : td.series == 1 ? i2 + 3 : td.series == 2 ? i3 + 3 : i3; /* P Q U W */
-                const int off = series * yr + i0 - (int)s_hdr[4 * (13 * ch + td.delay) + 1] - (H - 1);
+                const double *hd = s_hdr + 4 * (13 * ch + td.delay);
+                dc = hd[0];
+                xs = yF + series * yr + i0 - (int)hd[1] - (H - 1);
                 anc_t = sa + (13 * ch + td.delay) * ANC;
-                xs = yF + off;
-                xfs = yFf + off;
                 cP = (double)((df.base == 1) + df.i); c2 = (double)df.i;
                 cU = (double)((df.base == 2) + df.j); c3 = (double)df.j;
                 sgn = (double)td.sign;
             } else {
                 const int id = tm - 14;   /* 0: d/dt y_{p2} at L_p3 + L_p2 / 2 (gen 1.5);  1: d/dt y_{p3} at L_p2 + L_p3 / 2 */
-                const int off = (id == 0 ? i2 : i3) * yr + i0 - (int)s_hdr[4 * (FAST_NA_FULL + 2 * ch + id) + 1] - (H - 1);
+                const double *hd = s_hdr + 4 * (FAST_NA_FULL + 2 * ch + id);
+                dc = hd[0];
+                xs = dL + (id == 0 ? i2 : i3) * yr + i0 - (int)hd[1] - (H - 1);
                 anc_t = sa_lfa + (2 * ch + id) * ANC;
-                xs = dL + off;
-                xfs = dLf + off;
                 cP = 0.0; c3 = 0.0;
                 c2 = id == 0 ? lfa_lo : lfa_hi;
                 cU = id == 0 ? lfa_hi : lfa_lo;
             }
             double s0[FAST_TC_R], s1[FAST_TC_R];
-            float s2[FAST_TC_R];
-            term7<M>(anc_t, xs, xfs, s0, s1, s2);
+            term7<M>(anc_t, xs, s0, s1);
 #pragma unroll
             for (int r = 0; r < FAST_TC_R; ++r) {
-                const double D = fma(cP, eP[r], fma(c2, e2[r], fma(cU, eU[r], c3 * e3[r]))) * p.inv_dt;
-                const double v = fma(D, fma(D, (double)s2[r], s1[r]), s0[r]);
+                const double D = fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
+                const double v = fma(D, s1[r], s0[r]);
                 if (!lt) Xf[r] = fma(sgn, v, Xf[r]);
                 else {
-                    const int64_t n = min(nf + r, p.n - 1);
-                    const double L2 = tabL[i2 * p.stride + n], L3 = tabL[i3 * p.stride + n];
+                    const double L2 = L2p[r], L3 = LU[r];
                     const double pre = p.gen == LTDI_GEN_15 ? 4.0 : 8.0 * (L2 + L3);   /* (B25) / (B33) */
                     Xl[r] = fma(tm == 14 ? pre * L3 : -(pre * L2), v, Xl[r]);
                 }
@@ -837,7 +809,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
             }
         }
     }
-    __syncthreads();   /* every thread is done with eL: R becomes X, Y, Z */
+    __syncthreads();   /* every thread is done with the light times: Lr becomes X, Y, Z */
 
     /* blend (4.6), margins, exchange through shared memory */
 #pragma unroll
@@ -899,11 +871,10 @@ template <int M>
 static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
 {
     const bool has_full = which != LTDI_RESPONSE_LFA, has_lfa = which != LTDI_RESPONSE_FULL;
-    const size_t yr = FAST_TC + (size_t)m2 + M / 2 + 2;
+    const size_t yr = (size_t)tdi_yr<M>(m2);
     size_t dbl = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0)) * FAST_ANC_DOUBLES(M);
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
-    const size_t r_len = std::max((size_t)6 * FAST_TC, has_lfa ? 3 * (yr + 2 * (size_t)w) : (size_t)0);
-    dbl += r_len;
-    const size_t flt = (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
-    return dbl * sizeof(double) + (flt * sizeof(float) + 15) / 16 * 16;
+    dbl += (size_t)(has_full ? 6 : 3) * FAST_TC;
+    dbl += has_lfa ? 3 * (yr + 2 * (size_t)w) : 0;
+    return dbl * sizeof(double);
 }
