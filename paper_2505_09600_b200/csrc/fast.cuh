@@ -811,32 +811,35 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
     }
     __syncthreads();   /* every thread is done with the light times: Lr becomes X, Y, Z */
 
-    /* blend (4.6), margins, exchange through shared memory */
+    /* exchange through shared memory: rows 0..2 = X, Y, Z (hybrid: of the full response, rows 3..5 = of the LFA) */
 #pragma unroll
     for (int r = 0; r < FAST_TC_R; ++r) {
-        const int64_t n = nf + r;
-        double x;
-        if (WHICH == LTDI_RESPONSE_FULL) x = Xf[r];
-        else if (WHICH == LTDI_RESPONSE_LFA) x = Xl[r];
-        else {
-            double wa, wb;
-            hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
-            x = 0.0;
-            if (has_lfa && need_lfa && wa != 0.0) x = wa * Xl[r];
-            if (has_full && need_full && wb != 0.0) x = fma(wb, Xf[r], x);
-        }
-        if (!(n >= p.lo && n < p.n - p.hi)) x = 0.0;
-        Xs[ch * FAST_TC + r0 + r] = x;
+        if (WHICH == LTDI_RESPONSE_LFA) Xs[ch * FAST_TC + r0 + r] = Xl[r];
+        else Xs[ch * FAST_TC + r0 + r] = Xf[r];
+        if (WHICH == LTDI_RESPONSE_HYBRID) Xs[(3 + ch) * FAST_TC + r0 + r] = Xl[r];
     }
     __syncthreads();
 
+    /* blend (4.6), margins, A, E, T (2.9): one sample per thread and pass, the taper evaluated once per sample */
     const double is2 = 0.70710678118654752440, is6 = 0.40824829046386301637, is3 = 0.57735026918962576451;
     const int64_t src_off = b * p.ld;
     const int64_t ystride = p.batch * p.lds;
+#pragma unroll 1
     for (int i = tid; i < FAST_TC; i += FAST_TC_THREADS) {
         const int64_t n = n0 + i;
         if (n >= n1) break;
-        const double X = Xs[i], Y = Xs[FAST_TC + i], Z = Xs[2 * FAST_TC + i];
+        double X = Xs[i], Y = Xs[FAST_TC + i], Z = Xs[2 * FAST_TC + i];
+        double wa = 1.0, wb = 1.0;
+        if (WHICH == LTDI_RESPONSE_HYBRID) {
+            hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+            const bool use_l = need_lfa && wa != 0.0, use_f = need_full && wb != 0.0;
+            const double xl = Xs[3 * FAST_TC + i], yl = Xs[4 * FAST_TC + i], zl = Xs[5 * FAST_TC + i];
+            const double x0 = use_l ? wa * xl : 0.0, y0b = use_l ? wa * yl : 0.0, z0 = use_l ? wa * zl : 0.0;
+            X = use_f ? fma(wb, X, x0) : x0;
+            Y = use_f ? fma(wb, Y, y0b) : y0b;
+            Z = use_f ? fma(wb, Z, z0) : z0;
+        }
+        if (!(n >= p.lo && n < p.n - p.hi)) { X = 0.0; Y = 0.0; Z = 0.0; }
         p.A[src_off + n] = (Z - X) * is2;                 /* (2.9a) */
         p.E[src_off + n] = (X - 2.0 * Y + Z) * is6;       /* (2.9b) */
         p.T[src_off + n] = (X + Y + Z) * is3;             /* (2.9c) */
@@ -849,9 +852,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
             /* optional link output: the LFA links come back from the scratch series (their shared copy is gone) */
             const int iy = (int)(n - y0);
             const double *gl = p.yL + b * p.lds + n;
-            double wa = 1.0, wb = 1.0;
-            if (WHICH == LTDI_RESPONSE_HYBRID) hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
-#pragma unroll
+#pragma unroll 1
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
                 if (WHICH == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
