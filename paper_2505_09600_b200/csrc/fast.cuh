@@ -33,7 +33,7 @@
 #define FAST_TC_G 64                      /* thread groups per channel */
 #define FAST_TC (FAST_TC_R * FAST_TC_G)   /* 448 output samples per TDI tile */
 #define FAST_TC_THREADS (3 * FAST_TC_G)   /* 192 */
-#define FAST_TA_THREADS 192
+#define FAST_TA_THREADS 128
 #define FAST_TA (2 * FAST_TA_THREADS)     /* 384 samples per link tile */
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
 #define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
@@ -228,7 +228,7 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
 // link kernel: LFA == false: Eq. (2.5), six links;  LFA == true: Eq. (B10) at (B1), links +1, +2, +3
 // ---------------------------------------------------------------------------------------------
 template <int H, bool LFA>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 2) link_kernel(FastParams p)
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
 {
     extern __shared__ double smem[];
     const int64_t b = (int64_t)blockIdx.x % p.batch;
@@ -447,8 +447,12 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
         for (int r = 0; r < 3; ++r) {
             const double *row = p.tab + (int64_t)(ROW_L + 3 * warp + r) * p.stride;
             const double c = row[nc];
+            double v[FAST_TC / 32];   /* all loads of the sweep in flight at once (index clamped: max is idempotent) */
+#pragma unroll
+            for (int k = 0; k < FAST_TC / 32; ++k) v[k] = row[min(n0 + lane + 32 * k, n1 - 1)];
             double d = 0.0;
-            for (int64_t n = n0 + lane; n < n1; n += 32) d = fmax(d, fabs(row[n] - c));
+#pragma unroll
+            for (int k = 0; k < FAST_TC / 32; ++k) d = fmax(d, fabs(v[k] - c));
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) d = fmax(d, __shfl_xor_sync(0xffffffffu, d, o));
             if (lane == 0) {
