@@ -30,9 +30,13 @@
 #include "common.cuh"
 
 #define FAST_TC_R 7                       /* samples per thread in the TDI kernel */
-#define FAST_TC_G 64                      /* thread groups per channel */
-#define FAST_TC (FAST_TC_R * FAST_TC_G)   /* 448 output samples per TDI tile */
-#define FAST_TC_THREADS (3 * FAST_TC_G)   /* 192 */
+#define FAST_TCA 448                      /* samples per anchor tile */
+/* TDI tile geometry per response: G thread groups per channel, 7 G samples per tile, 3 G threads.  Full and LFA:
+ * one warp per Michelson channel (224 samples, 96 threads, four CTAs per SM); the hybrid instance needs the shared
+ * memory of both and runs 448-sample tiles with 192 threads, two CTAs per SM. */
+__host__ __device__ constexpr int tdi_g(int which) { return which == LTDI_RESPONSE_HYBRID ? 64 : 32; }
+__host__ __device__ constexpr int tdi_tc(int which) { return FAST_TC_R * tdi_g(which); }
+__host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(which); }
 #define FAST_TA_THREADS 128
 #define FAST_TA (2 * FAST_TA_THREADS)     /* 384 samples per link tile */
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
@@ -62,8 +66,8 @@ struct FastParams {
     int64_t lds;
     double *A, *E, *T, *XYZ, *Y; /* outputs of this chunk ([batch][ld] ...), XYZ / Y strides use batch_all */
     int64_t batch_all, b0;   /* full batch and first source of the chunk (for the [3][batch][ld] outputs) */
-    const double *anc;       /* [ntilesC][FAST_NA][M][4] */
-    const double *anc_hdr;   /* [ntilesC][FAST_NA][4]: d_c [s], q, eps_c, valid */
+    const double *anc;       /* [anchor tiles][FAST_NA][M][2] */
+    const double *anc_hdr;   /* [anchor tiles][FAST_NA][4]: d_c [s], q, eps_c, valid */
     int64_t ntilesA, ntilesC;
 };
 
@@ -435,8 +439,8 @@ template <int M>
 __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, double *hdr)
 {
     const int64_t tile = blockIdx.x;
-    const int64_t n0 = tile * FAST_TC, n1 = min(n0 + (int64_t)FAST_TC, p.n);
-    const int64_t nc = min(n0 + FAST_TC / 2, p.n - 1);
+    const int64_t n0 = tile * FAST_TCA, n1 = min(n0 + (int64_t)FAST_TCA, p.n);
+    const int64_t nc = min(n0 + FAST_TCA / 2, p.n - 1);
     const int tid = threadIdx.x;
     __shared__ double dev[6]; /* max |L_l(n) - L_l(nc)| over the tile */
     __shared__ double Lc[6];
@@ -447,12 +451,12 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
         for (int r = 0; r < 3; ++r) {
             const double *row = p.tab + (int64_t)(ROW_L + 3 * warp + r) * p.stride;
             const double c = row[nc];
-            double v[FAST_TC / 32];   /* all loads of the sweep in flight at once (index clamped: max is idempotent) */
+            double v[FAST_TCA / 32];   /* all loads of the sweep in flight at once (index clamped: max is idempotent) */
 #pragma unroll
-            for (int k = 0; k < FAST_TC / 32; ++k) v[k] = row[min(n0 + lane + 32 * k, n1 - 1)];
+            for (int k = 0; k < FAST_TCA / 32; ++k) v[k] = row[min(n0 + lane + 32 * k, n1 - 1)];
             double d = 0.0;
 #pragma unroll
-            for (int k = 0; k < FAST_TC / 32; ++k) d = fmax(d, fabs(v[k] - c));
+            for (int k = 0; k < FAST_TCA / 32; ++k) d = fmax(d, fabs(v[k] - c));
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) d = fmax(d, __shfl_xor_sync(0xffffffffu, d, o));
             if (lane == 0) {
@@ -525,7 +529,7 @@ __global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, d
 // rows can be copied in 16-byte pieces) and holds tdi_yr<M>(m2) samples (even)
 __host__ __device__ __forceinline__ int tdi_back(int64_t m2) { return (int)((m2 + 1) & ~(int64_t)1); }
 template <int M>
-__host__ __device__ __forceinline__ int tdi_yr(int64_t m2) { return (FAST_TC + tdi_back(m2) + M / 2 + 2 + 1) & ~1; }
+__host__ __device__ __forceinline__ int tdi_yr(int tc, int64_t m2) { return (tc + tdi_back(m2) + M / 2 + 2 + 1) & ~1; }
 
 // exact per-sample interpolation of a staged series (slow path): ys[0] = sample y0, length len
 template <int M>
@@ -592,9 +596,11 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>
-__global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(FastParams p)
 {
     extern __shared__ double smem[];
+    constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);
+    constexpr int FAST_TCA_TILES = FAST_TCA / FAST_TC;
     constexpr int H = M / 2;
     constexpr int ANC = FAST_ANC_DOUBLES(M);
     constexpr bool has_full = WHICH != LTDI_RESPONSE_LFA, has_lfa = WHICH != LTDI_RESPONSE_FULL;
@@ -622,7 +628,7 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
      *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0, even)
      *   Lr   [NLR][FAST_TC] light times L_l(n0 + i) of the tile; after the term loop: X, Y, Z of the tile
      *   yL   [3][yr + 2w] LFA links       (element 0 = sample y0 - w) */
-    const int yr = tdi_yr<M>(p.m2);
+    const int yr = tdi_yr<M>(FAST_TC, p.m2);
     const int64_t y0 = n0 - tdi_back(p.m2);
     constexpr int na_full = has_full ? FAST_NA_FULL : 0;
     double *sa = smem;
@@ -670,14 +676,15 @@ __global__ void __launch_bounds__(FAST_TC_THREADS, 2) tdi_kernel(FastParams p)
         }
     }
     {
-        const double *ga = p.anc + tile * (int64_t)(FAST_NA * ANC);
+        const int64_t atile = tile / FAST_TCA_TILES;
+        const double *ga = p.anc + atile * (int64_t)(FAST_NA * ANC);
         if (has_full && need_full)
             for (int i = tid; i < FAST_NA_FULL * ANC / 2; i += FAST_TC_THREADS)
                 cp_async16(sa + 2 * i, ga + 2 * i);
         if (has_lfa && need_lfa)
             for (int i = tid; i < FAST_NA_LFA * ANC / 2; i += FAST_TC_THREADS)
                 cp_async16(sa + (size_t)na_full * ANC + 2 * i, ga + FAST_NA_FULL * ANC + 2 * i);
-        for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[tile * (FAST_NA * 4) + i];
+        for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[atile * (FAST_NA * 4) + i];
     }
     cp_async_wait_all();
     __syncthreads();
@@ -876,10 +883,10 @@ template <int M>
 static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
 {
     const bool has_full = which != LTDI_RESPONSE_LFA, has_lfa = which != LTDI_RESPONSE_FULL;
-    const size_t yr = (size_t)tdi_yr<M>(m2);
+    const size_t yr = (size_t)tdi_yr<M>(tdi_tc(which), m2);
     size_t dbl = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0)) * FAST_ANC_DOUBLES(M);
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
-    dbl += (size_t)(has_full ? 6 : 3) * FAST_TC;
+    dbl += (size_t)(has_full ? 6 : 3) * tdi_tc(which);
     dbl += has_lfa ? 3 * (yr + 2 * (size_t)w) : 0;
     return dbl * sizeof(double);
 }

@@ -175,7 +175,7 @@ bool fast_order(int order) { return order == 9 || order == 31; }
 /* workspace of the fast path behind the per-source parameters: anchors | anchor headers | link-series scratch
  * for one chunk of sources.  The chunk is sized so that the scratch stays L2 resident. */
 struct FastLayout {
-    int64_t ntilesA, ntilesC, lds, chunk;
+    int64_t ntilesA, ntilesC, ntilesN, lds, chunk;   /* link tiles, TDI tiles, anchor tiles */
     size_t anc, hdr, y;     /* doubles */
     size_t total;           /* doubles, including work_doubles(batch) */
 };
@@ -183,14 +183,15 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
 {
     FastLayout f;
     f.ntilesA = (n + FAST_TA - 1) / FAST_TA;
-    f.ntilesC = (n + FAST_TC - 1) / FAST_TC;
+    f.ntilesC = (n + tdi_tc(which) - 1) / tdi_tc(which);
+    f.ntilesN = (n + FAST_TCA - 1) / FAST_TCA;
     f.lds = (n + 15) / 16 * 16;
     const int rows = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 3 : 9;
     const size_t cap = (size_t)96 << 20; /* bytes of scratch per chunk */
     int64_t chunk = (int64_t)(cap / ((size_t)rows * f.lds * sizeof(double)));
     f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
-    f.anc = (size_t)f.ntilesC * FAST_NA * FAST_ANC_DOUBLES(M);
-    f.hdr = (size_t)f.ntilesC * FAST_NA * 4;
+    f.anc = (size_t)f.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
+    f.hdr = (size_t)f.ntilesN * FAST_NA * 4;
     f.y = (size_t)rows * f.chunk * f.lds;
     f.total = work_doubles(batch) + f.anc + f.hdr + f.y;
     return f;
@@ -287,7 +288,7 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
 
     {
         ProfScope ps(LTDI_KERNEL_ANCHOR + LTDI_KERNEL_COUNT * which, st);
-        anchor_kernel<M><<<(unsigned)lay.ntilesC, 64, 0, st>>>(p, anc, hdr);
+        anchor_kernel<M><<<(unsigned)lay.ntilesN, 64, 0, st>>>(p, anc, hdr);
     }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
@@ -314,7 +315,7 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         }
         {
             ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
-            tdi<<<(unsigned)(lay.ntilesC * nb), FAST_TC_THREADS, smem_tdi, st>>>(p);
+            tdi<<<(unsigned)(lay.ntilesC * nb), tdi_threads(which), smem_tdi, st>>>(p);
         }
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
