@@ -267,30 +267,54 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
         if (a0 + c < p.stride) cp_async16(tb + r * FAST_TA + c, p.tab + (int64_t)r * p.stride + a0 + c);
         else *reinterpret_cast<double2 *>(tb + r * FAST_TA + c) = make_double2(0.0, 0.0);
     }
-    for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
-        const int64_t g = org + i;
-        double vp = 0.0, vc = 0.0;
-        if (!LFA) {
+    if (!LFA) {
+        for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
+            const int64_t g = org + i;
+            double *dp = ((i & 1) ? ho_p : he_p) + (i >> 1), *dc = ((i & 1) ? ho_c : he_c) + (i >> 1);
             if (g >= 0 && g < p.n) {
-                cp_async8(((i & 1) ? ho_p : he_p) + (i >> 1), gp + g);
-                cp_async8(((i & 1) ? ho_c : he_c) + (i >> 1), gc + g);
-                continue;
-            }
-        } else if (g >= w && g < p.n - w) {
-            if (w == 1) {
-                vp = gp[g + 1] - gp[g - 1];
-                vc = gc[g + 1] - gc[g - 1];
+                cp_async8(dp, gp + g);
+                cp_async8(dc, gc + g);
             } else {
-                vp = 8.0 * (gp[g + 1] - gp[g - 1]) - (gp[g + 2] - gp[g - 2]);
-                vc = 8.0 * (gc[g + 1] - gc[g - 1]) - (gc[g + 2] - gc[g - 2]);
+                *dp = 0.0;
+                *dc = 0.0;
             }
         }
-        double *dp = (i & 1) ? ho_p : he_p, *dc = (i & 1) ? ho_c : he_c;
-        dp[i >> 1] = vp;
-        dc[i >> 1] = vc;
+        cp_async_wait_all();
+        __syncthreads();
+    } else {
+        /* raw strain of samples org - 2 .. org + 2 hw2 + 1 (asynchronous), then the FD1 numerators (G15) */
+        const int nraw = 2 * hw2 + 4;
+        double *raw_p = tb + NROWS * FAST_TA, *raw_c = raw_p + nraw;
+        for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
+            const int64_t g = org - 2 + j;
+            if (g >= 0 && g < p.n) {
+                cp_async8(raw_p + j, gp + g);
+                cp_async8(raw_c + j, gc + g);
+            } else {
+                raw_p[j] = 0.0;
+                raw_c[j] = 0.0;
+            }
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
+            const int64_t g = org + i;
+            double vp = 0.0, vc = 0.0;
+            if (g >= w && g < p.n - w) {
+                const double *xp = raw_p + i + 2, *xc = raw_c + i + 2;
+                if (w == 1) {
+                    vp = xp[1] - xp[-1];
+                    vc = xc[1] - xc[-1];
+                } else {
+                    vp = 8.0 * (xp[1] - xp[-1]) - (xp[2] - xp[-2]);
+                    vc = 8.0 * (xc[1] - xc[-1]) - (xc[2] - xc[-2]);
+                }
+            }
+            ((i & 1) ? ho_p : he_p)[i >> 1] = vp;
+            ((i & 1) ? ho_c : he_c)[i >> 1] = vc;
+        }
+        __syncthreads();
     }
-    cp_async_wait_all();
-    __syncthreads();
 
     const int64_t m0 = a0 + 2 * tid;
     if (m0 >= p.n) return;

@@ -149,6 +149,11 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
     p.arm_m = desc->arm_m; p.R_m = desc->R_m;
     p.omega = 2.0 * 3.14159265358979323846 / desc->period_s;
     p.alpha0 = desc->alpha0; p.rot0 = desc->rot0; p.mode = desc->mode;
+    for (int i = 0; i < 3; ++i) { /* beta_i = 2 pi (i - 1) / 3 + rot0: constants of the launch */
+        const double beta = 2.0 * 3.14159265358979323846 * (double)i / 3.0 + desc->rot0;
+        p.sb[i] = std::sin(beta);
+        p.cb[i] = std::cos(beta);
+    }
     p.R_in = d_R; p.L_in = d_L; p.tab = (double *)d_tables;
     const int threads = 256;
     const int64_t blocks = (desc->n + threads - 1) / threads;
@@ -276,7 +281,8 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     /* staged strain (4 parity-split series) + the orbit-table rows of the tile */
     const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
     const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
-    const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double);
+    const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double) +
+                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double); /* + raw strain */
     const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
     int rc;
     if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;

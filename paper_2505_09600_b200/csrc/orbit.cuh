@@ -11,6 +11,7 @@ struct OrbitKernelParams {
     double t0, dt;
     int64_t n, stride;
     double arm_m, R_m, omega, alpha0, rot0;
+    double sb[3], cb[3]; /* sin, cos of beta_i */
     int mode;
     const double *R_in; /* tables mode: [3][3][n] */
     const double *L_in; /* tables mode: [6][n] */
@@ -37,13 +38,14 @@ __global__ void __launch_bounds__(256) orbit_delay_kernel(OrbitKernelParams p)
         const double eR = ecc * p.R_m;
         double sa, ca;
         sincos(alpha, &sa, &ca);
+        /* one sincos per sample: the angles 2 alpha - beta_i and alpha - beta_i by the addition theorems
+         * (a few ulp of 1 on terms that are e R = 7e8 m: 1e-6 m, far inside the table tolerance) */
+        const double s2a = 2.0 * sa * ca, c2a = (ca - sa) * (ca + sa);
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            const double b = 2.0 * 3.14159265358979323846 * (double)i / 3.0 + p.rot0;
-            double sb, cb, s2, c2, s1, c1;
-            sincos(b, &sb, &cb);
-            sincos(2.0 * alpha - b, &s2, &c2);
-            sincos(alpha - b, &s1, &c1);
+            const double sb = p.sb[i], cb = p.cb[i];
+            const double s2 = s2a * cb - c2a * sb, c2 = c2a * cb + s2a * sb;
+            const double s1 = sa * cb - ca * sb, c1 = ca * cb + sa * sb;
             R[i][0] = p.R_m * ca + 0.5 * eR * (c2 - 3.0 * cb);
             R[i][1] = p.R_m * sa + 0.5 * eR * (s2 - 3.0 * sb);
             R[i][2] = -sqrt(3.0) * eR * c1;
