@@ -62,7 +62,7 @@ typedef struct { double beta, lambda, psi; } ltdi_source; /* ecliptic latitude, 
 /* Hybridisation window: centre t_hyb [s], width window_s (T), sigmoid scale sigma_s. */
 typedef struct { double t_hyb, window_s, sigma_s; int32_t taper; } ltdi_hybrid;
 
-typedef struct ltdi_orbits ltdi_orbits; /* opaque, immutable after init */
+typedef struct ltdi_orbits ltdi_orbits; /* opaque; changed only by ltdi_orbits_prepare() after init */
 
 /* Rows of the device orbit table: 9 positions R_i [m] (i*3+axis), 9 unit vectors n_l for
  * l = +1,+2,+3 (n_-l = -n_l), 6 light travel times L_l [s]; row stride = ltdi_orbits_stride(). */
@@ -84,6 +84,15 @@ int ltdi_orbits_init(const ltdi_orbit_desc *desc, void *d_tables, size_t bytes, 
  * must be LTDI_ORBIT_TABLES; arm_m and R_m still size the margins. */
 int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L,
                             void *d_tables, size_t bytes, void *stream, ltdi_orbits **out);
+
+/* Optional: the TDI delays of Eqs. (2.7) / (2.8) and (B25) / (B33) are sums of L_l(t_n), so the
+ * Lagrange weights of the TDI stage depend on the orbit object, the generation and the order only, not on
+ * the sources.  ltdi_orbits_prepare() computes them once into d_buf (device, 16-byte aligned, >=
+ * ltdi_orbits_prepare_bytes() bytes, owned by the caller, referenced by the handle until the next prepare or
+ * destroy); responses called with the same gen and lagrange_order then skip their own weight kernel.  The
+ * results are bitwise the same with or without it.  Orders other than 9 and 31 need 0 bytes (no-op). */
+int ltdi_orbits_prepare_bytes(const ltdi_orbit_desc *desc, int lagrange_order, size_t *bytes);
+int ltdi_orbits_prepare(ltdi_orbits *orb, int gen, int lagrange_order, void *d_buf, size_t bytes, void *stream);
 
 int ltdi_orbits_destroy(ltdi_orbits *orb);               /* frees the handle only */
 int64_t ltdi_orbits_stride(const ltdi_orbits *orb);      /* elements between table rows */

@@ -59,6 +59,8 @@ _SIGNATURES = {
     "ltdi_orbits_workspace_bytes": (C.c_int, [C.POINTER(OrbitDesc), _szp]),
     "ltdi_orbits_init": (C.c_int, [C.POINTER(OrbitDesc), _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
     "ltdi_orbits_init_tables": (C.c_int, [C.POINTER(OrbitDesc), _dp, _dp, _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
+    "ltdi_orbits_prepare_bytes": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, _szp]),
+    "ltdi_orbits_prepare": (C.c_int, [_vp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
     "ltdi_orbits_destroy": (C.c_int, [_vp]),
     "ltdi_orbits_stride": (C.c_int64, [_vp]),
     "ltdi_orbits_tables": (_vp, [_vp]),
@@ -201,6 +203,24 @@ class Orbits:
         _check("ltdi_orbits_init", rc)
         self.handle = handle
         self.stride = lib().ltdi_orbits_stride(handle)
+        self._anchors = None
+
+    def prepare(self, gen, order, buffer=None):
+        """Compute the TDI-stage interpolation weights of (gen, order) once for this time grid
+        (ltdi_orbits_prepare); later responses with the same gen and order skip their weight kernel.
+        `buffer`: an existing float64 device tensor to reuse (a new one is allocated if None or too small)."""
+        nbytes = C.c_size_t()
+        _check("ltdi_orbits_prepare_bytes",
+               lib().ltdi_orbits_prepare_bytes(C.byref(_desc(self.desc)), order, C.byref(nbytes)))
+        if nbytes.value == 0:
+            return self
+        if buffer is None or buffer.numel() * 8 < nbytes.value:
+            buffer = torch.empty(nbytes.value // 8, dtype=torch.float64, device=self.device)
+        self._anchors = buffer
+        with torch.cuda.device(self.device):
+            _check("ltdi_orbits_prepare", lib().ltdi_orbits_prepare(self.handle, gen, order, buffer.data_ptr(),
+                                                                   buffer.numel() * 8, _stream()))
+        return self
 
     @property
     def n(self):

@@ -17,6 +17,8 @@ struct ltdi_orbits {
     ltdi_orbit_desc desc;
     const double *d_tab; /* [LTDI_TABLE_ROWS][stride] */
     int64_t stride;
+    const double *d_anc; /* TDI weight anchors and their headers from ltdi_orbits_prepare(), or NULL */
+    int anc_gen, anc_M;  /* generation and tap count they were computed for */
 };
 
 /* table rows */

@@ -168,6 +168,9 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
     o->desc = *desc;
     o->d_tab = (const double *)d_tables;
     o->stride = stride;
+    o->d_anc = nullptr;
+    o->anc_gen = 0;
+    o->anc_M = 0;
     *out = o;
     return LTDI_OK;
 }
@@ -292,12 +295,16 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
                                                            : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
     if ((rc = set_smem(tdi, smem_tdi, smem_max))) return rc;
 
-    {
+    if (orb->d_anc && orb->anc_gen == rp.gen && orb->anc_M == M) {
+        /* ltdi_orbits_prepare() has computed the anchors of this (generation, order) for the time grid */
+        p.anc = orb->d_anc;
+        p.anc_hdr = orb->d_anc + (size_t)lay.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
+    } else {
         ProfScope ps(LTDI_KERNEL_ANCHOR + LTDI_KERNEL_COUNT * which, st);
         anchor_kernel<M><<<(unsigned)lay.ntilesN, 64, 0, st>>>(p, anc, hdr);
+        count_launch();
+        LTDI_CUDA_OK(cudaGetLastError());
     }
-    count_launch();
-    LTDI_CUDA_OK(cudaGetLastError());
 
     for (int64_t b0 = 0; b0 < rp.batch; b0 += lay.chunk) {
         const int64_t nb = std::min(lay.chunk, rp.batch - b0);
@@ -546,6 +553,48 @@ int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, cons
 {
     if (!desc || desc->mode != LTDI_ORBIT_TABLES || !d_R || !d_L) return LTDI_EINVAL;
     return orbits_common(desc, d_R, d_L, d_tables, bytes, stream, out);
+}
+
+int ltdi_orbits_prepare_bytes(const ltdi_orbit_desc *desc, int lagrange_order, size_t *bytes)
+{
+    if (!desc_ok(desc) || !order_ok(lagrange_order) || !bytes) return LTDI_EINVAL;
+    if (!fast_order(lagrange_order)) { *bytes = 0; return LTDI_OK; }
+    const int64_t tiles = (desc->n + FAST_TCA - 1) / FAST_TCA;
+    *bytes = ((size_t)tiles * FAST_NA * (FAST_ANC_DOUBLES(lagrange_order + 1) + 4) * sizeof(double) + 255) / 256 * 256;
+    return LTDI_OK;
+}
+
+int ltdi_orbits_prepare(ltdi_orbits *orb, int gen, int lagrange_order, void *d_buf, size_t bytes, void *stream)
+{
+    if (!orb || !gen_ok(gen) || !order_ok(lagrange_order)) return LTDI_EINVAL;
+    if (!fast_order(lagrange_order)) return LTDI_OK;   /* the other orders build their weights per sample */
+    size_t need = 0;
+    ltdi_orbits_prepare_bytes(&orb->desc, lagrange_order, &need);
+    if (!d_buf || (uintptr_t)d_buf % 16) return LTDI_EINVAL;
+    if (bytes < need) return LTDI_EWORKSPACE;
+    int rc = init_constants();
+    if (rc) return rc;
+    const ltdi_orbit_desc &d = orb->desc;
+    const int M = lagrange_order + 1;
+    const Margins mg = compute_margins(d, gen, lagrange_order, 0);
+    if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_OK; /* shapes the tuned kernels do not cover */
+    FastParams p;
+    std::memset(&p, 0, sizeof p);
+    p.tab = orb->d_tab; p.stride = orb->stride; p.n = d.n; p.t0 = d.t0; p.dt = d.dt; p.inv_dt = 1.0 / d.dt;
+    p.gen = gen; p.m1 = mg.m1; p.m2 = mg.m2;
+    const int64_t tiles = (d.n + FAST_TCA - 1) / FAST_TCA;
+    double *anc = (double *)d_buf, *hdr = anc + (size_t)tiles * FAST_NA * FAST_ANC_DOUBLES(M);
+    {
+        ProfScope ps(LTDI_KERNEL_ANCHOR, (cudaStream_t)stream);
+        if (M == 32) anchor_kernel<32><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr);
+        else anchor_kernel<10><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr);
+    }
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    orb->d_anc = anc;
+    orb->anc_gen = gen;
+    orb->anc_M = M;
+    return LTDI_OK;
 }
 
 int ltdi_orbits_destroy(ltdi_orbits *orb)

@@ -200,3 +200,29 @@ def test_host_pipeline_matches_device_call(ltdi):
                        20, 31, 2)
     torch.cuda.synchronize()
     assert torch.equal(A, ref["A"].cpu()) and torch.equal(E, ref["E"].cpu()) and torch.equal(T, ref["T"].cpu())
+
+
+def test_prepared_anchors_give_bitwise_the_same_result(ltdi):
+    """ltdi_orbits_prepare(): TDI weights computed once per time grid; the responses must not change by a bit,
+    and a prepare for another generation / order must be ignored"""
+    cfg = W.config(2, n=30011, batch=3)
+    hp, hc, ang, metas = W.sources(cfg, [0, 1, 2])
+    dev = torch.device("cuda:0")
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    hyb = hybrid_params(metas, ltdi.hyb_time, W.TAPER_COSINE, cfg["dt"])
+
+    def run(orb):
+        out = []
+        for gen in (15, 20):
+            out.append(to_numpy(ltdi.response_full(orb, dhp, dhc, ang, gen, 31, True, False)))
+            out.append(to_numpy(ltdi.response_lfa(orb, dhp, dhc, ang, gen, 31, 2, True, False)))
+            out.append(to_numpy(ltdi.response_hybrid(orb, dhp, dhc, ang, gen, 31, 2, hyb, True, False)))
+        torch.cuda.synchronize()
+        return out
+
+    plain = run(ltdi.Orbits(cfg["orbit"], device=dev))
+    for gen, order in ((20, 31), (15, 31), (20, 9), (20, 13)):
+        prepared = run(ltdi.Orbits(cfg["orbit"], device=dev).prepare(gen, order))
+        for a, b in zip(plain, prepared):
+            for k in ("A", "E", "T", "XYZ"):
+                assert np.array_equal(a[k], b[k]), (gen, order, k)
