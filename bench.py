@@ -38,7 +38,10 @@ KERNEL_FLOPS = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), cfg2 only; None where no capture exists for the kernel
-TRAFFIC = {}
+TRAFFIC = {"full/tdi": 74.612736e6 + 3.713024e6}    # profiles/r01b_cfg2.md, tdi_kernel<32,FULL>, cfg2
+# sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only)
+FP64_PIPE_PCT_NCU = {"full/orbit": 53.8, "full/anchor": 12.0, "full/link_full": 63.1, "full/tdi": 65.0,
+                     "lfa/link_lfa": 49.8, "lfa/tdi": 35.3, "hybrid/tdi": 30.1}
 
 WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
@@ -316,7 +319,8 @@ def main():
         full_ms = float(np.mean(per_call["full"]))
         roofline = {"bound": "alu", "kernel": dom + " (response/kernel; see include/lisatdi.h LTDI_KERNEL_*)",
                     "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                    "traffic": TRAFFIC.get(dom),
+                    "traffic": TRAFFIC.get(dom) if args.workload == "cfg2" else None,
+                    "fp64_pipe_pct_ncu_cfg2": FP64_PIPE_PCT_NCU,
                     "peak_source": "DFMA chain probe measured in this run (2 flop per DFMA); nominal 148 SM x 64 DFMA/clk",
                     "timed_with": "per-kernel CUDA events on the launching stream (ltdi_profile_*), over %d steps "
                                   "identical to the timed ones, run right after them" % args.steps,
