@@ -54,6 +54,7 @@ struct FastParams {
     const double *tab;
     int64_t stride, n;
     double t0, dt, inv_dt;
+    double inv_fd1, inv_fd2; /* 1 / (2 dt) | 1 / (12 dt) and 1 / dt^2 | 1 / (12 dt^2): stencil denominators (fd 2 | 4) */
     const double *hp, *hc;
     int64_t ld, batch;       /* batch = sources of this launch (a chunk) */
     const double *frames;    /* [batch][LTDI_FRAME_STRIDE] of this chunk */
@@ -394,7 +395,7 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
             }
         }
     } else {
-        const double den = (w == 1 ? 2.0 : 12.0) * p.dt;
+        const double iden = p.inv_fd1;   /* the stencil denominator as a factor (one rounding, like the division) */
 #pragma unroll 1
         for (int l = 0; l < 3; ++l) {
             const int s = link_sender(l), r = link_receiver(l);
@@ -407,8 +408,8 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
                              ho_c, ap0, ac0, ap1, ac1);                                    /* (B1) */
             double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
             patterns(l, Fp0, Fc0, kn0, Fp1, Fc1, kn1);
-            const double y0 = -(0.5 * L.x) * (Fp0 * (ap0 / den) + Fc0 * (ac0 / den));      /* (B10) */
-            const double y1 = -(0.5 * L.y) * (Fp1 * (ap1 / den) + Fc1 * (ac1 / den));
+            const double y0 = -(0.5 * L.x) * (Fp0 * (ap0 * iden) + Fc0 * (ac0 * iden));    /* (B10) */
+            const double y1 = -(0.5 * L.y) * (Fp1 * (ap1 * iden) + Fc1 * (ac1 * iden));
             *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
         }
     }
@@ -717,7 +718,6 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     if (has_lfa) {
         if (need_lfa) {
             /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
-            const double dt = p.dt;
             const int len = yr + 2 * w;
             for (int i = tid; i < 3 * yr; i += FAST_TC_THREADS) {
                 const int l = i / yr, k = i - l * yr;
@@ -727,13 +727,13 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
                 double d = 0.0;
                 if (in) {
                     if (p.gen == LTDI_GEN_15) {
-                        d = (w == 1) ? (x[1] - x[-1]) / (2.0 * dt) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2])) / (12.0 * dt);
+                        d = ((w == 1) ? (x[1] - x[-1]) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2]))) * p.inv_fd1;
                     } else {
                         const double d1 = (x[1] - x[0]) - (x[0] - x[-1]);
-                        if (w == 1) d = d1 / (dt * dt);
+                        if (w == 1) d = d1 * p.inv_fd2;
                         else {
                             const double d2 = (x[2] - x[0]) - (x[0] - x[-2]);
-                            d = (16.0 * d1 - d2) / (12.0 * dt * dt);
+                            d = (16.0 * d1 - d2) * p.inv_fd2;
                         }
                     }
                 }

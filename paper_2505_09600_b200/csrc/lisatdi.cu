@@ -276,6 +276,8 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     p.tab = rp.tab; p.stride = rp.stride; p.n = rp.n; p.t0 = rp.t0; p.dt = rp.dt; p.inv_dt = 1.0 / rp.dt;
     p.ld = rp.ld; p.n_hyb = rp.n_hyb; p.which = which; p.gen = rp.gen; p.fd = rp.fd;
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi; p.qmax = rp.qmax;
+    p.inv_fd1 = 1.0 / ((mg.w == 1 ? 2.0 : 12.0) * rp.dt);
+    p.inv_fd2 = 1.0 / ((mg.w == 1 ? 1.0 : 12.0) * rp.dt * rp.dt);
     p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
     double *anc = work, *hdr = anc + lay.anc, *ys = hdr + lay.hdr;
     p.anc = anc; p.anc_hdr = hdr;
