@@ -47,6 +47,8 @@ WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
     "cfg2": (2, None, None),
     "cfg1": (1, None, None),
+    "cfg1f": (1, None, 4096),    # config 1 with the device filled: 4096 sources with fresh angles
+    "cfg3": (3, None, None),     # 1 year at dt = 5 s, one source
     "cfg4s": (4, None, 256),     # a 256-source slice of config 4 (the full 4096 x 131072 needs 21 GB of buffers)
     "cfg5s": (5, None, 16),
 }
