@@ -311,14 +311,26 @@ def _hybrid_array(hybrid):
 
 
 class HostPipeline:
-    """End-to-end call with HOST buffers (ltdi_response_host): pinned strain in, pinned A, E, T out."""
+    """End-to-end call with HOST buffers (ltdi_response_host): pinned strain in, pinned A, E, T out.
 
-    def __init__(self, orb, batch, ld):
-        self.orb, self.batch, self.ld = orb, batch, ld
+    depth = 1: every call is enqueued on the current stream.  depth > 1: successive calls rotate over `depth`
+    slots, each with its own stream, device scratch and pinned outputs, so that the device->host copy of one call
+    overlaps the host->device copy and the kernels of the next (PCIe is full duplex).  run() returns the slot's
+    pinned A, E, T, valid after synchronize() (or once the slot is reused, after its event)."""
+
+    def __init__(self, orb, batch, ld, depth=1):
+        self.orb, self.batch, self.ld, self.depth = orb, batch, ld, int(depth)
         nbytes = C.c_size_t()
         _check("ltdi_host_scratch_bytes", lib().ltdi_host_scratch_bytes(ld, batch, C.byref(nbytes)))
-        self.scratch = torch.empty(nbytes.value // 8, dtype=torch.float64, device=orb.device)
-        self.A, self.E, self.T = (torch.empty(batch, ld, dtype=torch.float64).pin_memory() for _ in range(3))
+        self.slots = []
+        for _ in range(self.depth):
+            slot = {"scratch": torch.empty(nbytes.value // 8, dtype=torch.float64, device=orb.device),
+                    "out": tuple(torch.empty(batch, ld, dtype=torch.float64).pin_memory() for _ in range(3)),
+                    "stream": torch.cuda.Stream(device=orb.device) if self.depth > 1 else None,
+                    "event": None}
+            self.slots.append(slot)
+        self.A, self.E, self.T = self.slots[0]["out"]
+        self.calls = 0
         self.h2d_bytes = 2 * batch * ld * 8
         self.d2h_bytes = 3 * batch * ld * 8
 
@@ -326,13 +338,39 @@ class HostPipeline:
         assert hp_host.dtype == torch.float64 and not hp_host.is_cuda and hp_host.is_contiguous()
         src_ptr, keep = _sources(sources)
         harr, nh = _hybrid_array(hybrid)
+        slot = self.slots[self.calls % self.depth]
+        self.calls += 1
+        A, E, T = slot["out"]
         with torch.cuda.device(self.orb.device):
+            if slot["stream"] is None:
+                stream = _stream()
+            else:
+                if slot["event"] is not None:
+                    slot["event"].synchronize()          # the slot's previous results have reached the host
+                slot["stream"].wait_stream(torch.cuda.current_stream())   # orbit tables etc. of the caller
+                stream = slot["stream"].cuda_stream
             rc = lib().ltdi_response_host(which, self.orb.handle, hp_host.data_ptr(), hc_host.data_ptr(), self.ld,
-                                          self.batch, src_ptr, gen, order, fd_order, harr, nh, self.A.data_ptr(),
-                                          self.E.data_ptr(), self.T.data_ptr(), self.scratch.data_ptr(),
-                                          self.scratch.numel() * 8, _stream())
+                                          self.batch, src_ptr, gen, order, fd_order, harr, nh, A.data_ptr(),
+                                          E.data_ptr(), T.data_ptr(), slot["scratch"].data_ptr(),
+                                          slot["scratch"].numel() * 8, stream)
+            if slot["stream"] is not None:
+                slot["event"] = torch.cuda.Event()
+                slot["event"].record(slot["stream"])
         _check("ltdi_response_host", rc)
-        return self.A, self.E, self.T
+        return A, E, T
+
+    def join(self):
+        """Make the current stream wait for every call in flight (depth > 1)."""
+        for slot in self.slots:
+            if slot["stream"] is not None:
+                torch.cuda.current_stream().wait_stream(slot["stream"])
+
+    def synchronize(self):
+        for slot in self.slots:
+            if slot["stream"] is not None:
+                slot["stream"].synchronize()
+            else:
+                torch.cuda.current_stream().synchronize()
 
 
 def fp64_probe(blocks=148 * 8, iters=2000, repeats=5, device="cuda:0"):

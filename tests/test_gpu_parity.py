@@ -226,3 +226,34 @@ def test_prepared_anchors_give_bitwise_the_same_result(ltdi):
         for a, b in zip(plain, prepared):
             for k in ("A", "E", "T", "XYZ"):
                 assert np.array_equal(a[k], b[k]), (gen, order, k)
+
+
+def test_host_pipeline_with_two_slots_matches_single_slot(ltdi):
+    """depth = 2 rotates streams / scratch / pinned outputs: same bits as the one-stream pipeline"""
+    cfg = W.config(2, n=9000, batch=3)
+    hp, hc, ang, metas = W.sources(cfg, [0, 1, 2])
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    hp_h, hc_h = torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory()
+    hyb = hybrid_params(metas, ltdi.hyb_time, W.TAPER_COSINE, cfg["dt"])
+    calls = [(ltdi.RESPONSE_FULL, 2, None), (ltdi.RESPONSE_LFA, 2, None), (ltdi.RESPONSE_HYBRID, 2, hyb),
+             (ltdi.RESPONSE_LFA, 4, None)]
+    one = ltdi.HostPipeline(orb, 3, 9000)
+    want = []
+    for which, fd, h in calls:
+        out = one.run(which, hp_h, hc_h, ang, 20, 31, fd, h)
+        one.synchronize()
+        want.append([t.clone() for t in out])
+    two = ltdi.HostPipeline(orb, 3, 9000, depth=2)
+    for rep in range(2):          # the second pass reuses slots that still hold results
+        got = []
+        for i, (which, fd, h) in enumerate(calls):
+            out = two.run(which, hp_h, hc_h, ang, 20, 31, fd, h)
+            if i >= 1:            # the previous call's slot is complete only after its event
+                two.slots[(two.calls - 2) % 2]["event"].synchronize()
+                got.append([t.clone() for t in two.slots[(two.calls - 2) % 2]["out"]])
+        two.synchronize()
+        got.append([t.clone() for t in out])
+        for w, g in zip(want, got):
+            for a, b in zip(w, g):
+                assert torch.equal(a, b)
