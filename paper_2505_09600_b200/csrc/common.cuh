@@ -6,6 +6,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
 
 #include "../../include/lisatdi.h"
 
@@ -49,10 +51,14 @@ struct Margins {
  * row r, column k + M/2 - 1 */
 __constant__ double c_lag_inv_den[32 * LTDI_MAX_TAPS];
 
-#define LTDI_CUDA_OK(expr)                     \
-    do {                                       \
-        if ((expr) != cudaSuccess) {           \
-            (void)cudaGetLastError();          \
-            return LTDI_ECUDA;                 \
-        }                                      \
+/* a failed CUDA call becomes LTDI_ECUDA; with LTDI_DEBUG set in the environment the CUDA error is printed */
+#define LTDI_CUDA_OK(expr)                                                                              \
+    do {                                                                                                \
+        const cudaError_t ltdi_err_ = (expr);                                                           \
+        if (ltdi_err_ != cudaSuccess) {                                                                 \
+            if (getenv("LTDI_DEBUG"))                                                                   \
+                fprintf(stderr, "lisatdi %s:%d: %s\n", __FILE__, __LINE__, cudaGetErrorString(ltdi_err_)); \
+            (void)cudaGetLastError();                                                                   \
+            return LTDI_ECUDA;                                                                          \
+        }                                                                                               \
     } while (0)

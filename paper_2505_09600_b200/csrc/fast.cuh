@@ -661,7 +661,10 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     double *dL = yF + (has_full ? 6 * yr : 0);
     double *Lr = dL + (has_lfa ? 3 * yr : 0);
     double *yL = Lr + NLR * FAST_TC;
-    double *Xs = Lr;
+    /* X, Y, Z exchange: its own region (full, LFA: no barrier between the term loop and the exchange), or on top of
+     * the light times (hybrid: six rows, and the shared memory of two responses) */
+    constexpr bool xs_alias = WHICH == LTDI_RESPONSE_HYBRID;
+    double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * (yr + 2 * w) : 0);
     const double *sa_lfa = sa + (size_t)na_full * ANC;
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
     __shared__ double s_hdr[FAST_NA * 4];
@@ -844,7 +847,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             }
         }
     }
-    __syncthreads();   /* every thread is done with the light times: Lr becomes X, Y, Z */
+    if (xs_alias) __syncthreads();   /* every thread is done with the light times: Lr becomes X, Y, Z */
 
     /* exchange through shared memory: rows 0..2 = X, Y, Z (hybrid: of the full response, rows 3..5 = of the LFA) */
 #pragma unroll
@@ -912,5 +915,6 @@ static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
     dbl += (size_t)(has_full ? 6 : 3) * tdi_tc(which);
     dbl += has_lfa ? 3 * (yr + 2 * (size_t)w) : 0;
+    dbl += which == LTDI_RESPONSE_HYBRID ? 0 : (size_t)3 * tdi_tc(which);   /* X, Y, Z exchange */
     return dbl * sizeof(double);
 }

@@ -219,7 +219,7 @@ template <int MT, bool STAGE>
 int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t st)
 {
     static std::atomic<size_t> configured{0};
-    if (smem > 48 * 1024 && smem > configured.load()) {
+    if (smem + 4096 > 48 * 1024 && smem > configured.load()) {   /* static shared memory counts too */
         LTDI_CUDA_OK(cudaFuncSetAttribute(response_kernel<MT, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)smem));
         configured.store(smem);
@@ -237,7 +237,7 @@ template <typename K>
 int set_smem(K kernel, size_t smem, int smem_max)
 {
     if (smem > (size_t)smem_max) return LTDI_EUNSUPPORTED;
-    if (smem <= 48 * 1024) return LTDI_OK;
+    if (smem + 4096 <= 48 * 1024) return LTDI_OK;   /* the kernels' static shared memory (<= 2 KB) counts too */
     /* the attribute is sticky per device function: raise it only when a call needs more than any before */
     static std::mutex mu;
     static std::vector<std::pair<const void *, size_t>> seen;
