@@ -126,7 +126,10 @@ int ltdi_workspace_bytes(int which, int64_t n, int64_t batch, int gen, int lagra
  *   d_y             [6][batch][ld] single-link responses y_slr, or NULL
  *   d_work          scratch of ltdi_workspace_bytes() bytes, 16-byte aligned
  * Errors: LTDI_EINVAL for NULL required pointers, bad gen / order / fd_order, ld < n, batch < 1;
- * LTDI_EWORKSPACE if work_bytes is too small; LTDI_ECUDA if a CUDA call fails.
+ * LTDI_EWORKSPACE if work_bytes is too small; LTDI_ECUDA if a CUDA call fails (set LTDI_DEBUG in the
+ * environment to have the CUDA error printed); LTDI_EUNSUPPORTED if the link series one tile needs do not fit
+ * the 227 KB of shared memory (sampling steps far below the light travel time: dt < L / (c 250) for the hybrid,
+ * TDI 2.0) or batch x tiles exceeds 2^31.
  */
 
 /* Full response: Eqs. (2.2)-(2.6) projection (S2, S3), Eq. (2.7)/(2.8) TDI (S4), Eq. (2.9) (S5). */

@@ -257,3 +257,59 @@ def test_host_pipeline_with_two_slots_matches_single_slot(ltdi):
         for w, g in zip(want, got):
             for a, b in zip(w, g):
                 assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("dt", [0.05, 0.5, 1.0, 2.0, 3.3, 4.6, 5.0, 7.5, 12.0, 30.0, 60.0])
+def test_sampling_steps_sweep_the_shared_memory_plans(ltdi, orc80, dt):
+    """the halo widths, and with them the shared-memory carve-up of every kernel, depend on dt: sweep it through the
+    opt-in threshold (48 KB), the tuned path and, for very small dt, the fall-back to the generic kernel; Keplerian
+    orbit, two sources, all three responses, both generations, orders 31 and 9"""
+    from oracle import Oracle
+    orc64 = Oracle("f64")
+    lo_max = max(orc80.margins(W.orbit_desc(10, dt), 20, 31, 4))
+    n = int(2 * lo_max + 1500) if dt >= 0.5 else int(2 * lo_max + 300)
+    orbit = W.orbit_desc(n, dt, W.ORBIT_KEPLERIAN, t0=1.234e7)
+    f = 0.02 / dt if dt >= 0.5 else 2.0e-2        # well sampled, not so low that the TDI output is rounding noise
+    hp0, hc0 = W.monochromatic(n, dt, f, t0=orbit["t0"])
+    hp1, hc1 = W.monochromatic(n, dt, 0.6 * f, a_plus=0.4, a_cross=-1.1, phi_p=2.0, phi_c=0.1, t0=orbit["t0"])
+    hp, hc = np.stack([hp0, hp1]), np.stack([hc0, hc1])
+    ang = [(0.3, 1.0, 0.7), (-0.9, 4.0, 2.2)]
+    tmid = orbit["t0"] + 0.55 * n * dt
+    hyb = [{"t_hyb": tmid, "window_s": 40 * dt, "sigma_s": dt, "taper": W.TAPER_COSINE},
+           {"t_hyb": tmid - 100 * dt, "window_s": 64 * dt, "sigma_s": 1.6 * dt, "taper": W.TAPER_SIGMOID}]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    cases = [("full", 20, 31, 0), ("lfa", 20, 31, 2), ("hybrid", 20, 31, 4), ("full", 15, 9, 0), ("hybrid", 15, 9, 2)]
+    if dt < 0.5:
+        cases = cases[:3]          # the oracle takes a second per response here
+    for which, gen, order, fd in cases:
+        if which == "full":
+            out = ltdi.response_full(orb, dhp, dhc, ang, gen, order, True, True)
+            ref, ref64 = (o.response_full(orbit, hp, hc, ang, gen, order) for o in (orc80, orc64))
+        elif which == "lfa":
+            out = ltdi.response_lfa(orb, dhp, dhc, ang, gen, order, fd, True, True)
+            ref, ref64 = (o.response_lfa(orbit, hp, hc, ang, gen, order, fd) for o in (orc80, orc64))
+        else:
+            out = ltdi.response_hybrid(orb, dhp, dhc, ang, gen, order, fd, hyb, True, True)
+            ref, ref64 = (o.response_hybrid(orbit, hp, hc, ang, gen, order, fd, hyb) for o in (orc80, orc64))
+        torch.cuda.synchronize()
+        out = to_numpy(out)
+        lo, hi = orc80.margins(orbit, gen, order, fd)
+        assert (lo, hi) == ltdi.margins(orbit, gen, order, fd)
+        ref["floor"] = fp64_floor(ref, ref64, lo, n, hi)
+        ref["floor_XYZ"] = series_floor(ref["XYZ"], ref64["XYZ"], lo, n, hi)
+        ref["floor_y"] = series_floor(ref["y"], ref64["y"], lo, n, hi)
+        check(out, ref, lo, hi, n)
+
+
+def test_unsupported_shape_is_reported(ltdi):
+    """dt = 0.02 s: the link series a hybrid TDI 2.0 tile needs (7.2 L / c = 3000 samples back, for nine series) do
+    not fit the 227 KB of shared memory: the call must say LTDI_EUNSUPPORTED, not launch (include/lisatdi.h)"""
+    n, dt = 60000, 0.02
+    orb = ltdi.Orbits(W.orbit_desc(n, dt))
+    h = torch.zeros(1, n, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(ltdi.LtdiError) as e:
+        ltdi.response_hybrid(orb, h, h, [(0.1, 0.2, 0.3)], 20, 31, 2,
+                             {"t_hyb": 600.0, "window_s": 1.0, "sigma_s": 0.1, "taper": 0})
+    assert e.value.code == ltdi.EUNSUPPORTED
