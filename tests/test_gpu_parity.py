@@ -313,3 +313,46 @@ def test_unsupported_shape_is_reported(ltdi):
         ltdi.response_hybrid(orb, h, h, [(0.1, 0.2, 0.3)], 20, 31, 2,
                              {"t_hyb": 600.0, "window_s": 1.0, "sigma_s": 0.1, "taper": 0})
     assert e.value.code == ltdi.EUNSUPPORTED
+
+
+@pytest.mark.parametrize("order", [31, 9])
+def test_fast_varying_tables_take_the_exact_weight_paths(ltdi, orc80, order):
+    """LTDI_ORBIT_TABLES with light times that breathe by 1 % within minutes and spacecraft that wobble by a light
+    second: the TDI delays drift by far more than the first-order anchors allow and cross integer shifts inside
+    tiles (exact per-sample weights in tdi_kernel), and the two samples of a link pair get different integer shifts
+    (single-sample interpolator in link_kernel).  Same bar as everywhere else."""
+    from oracle import Oracle
+    orc64 = Oracle("f64")
+    n, dt = 6000, 5.0
+    base = W.orbit_desc(n, dt, W.ORBIT_KEPLERIAN, t0=2.0e6)
+    R, _, L = orc80.orbit_tables(base)
+    t = base["t0"] + dt * np.arange(n)
+    rng = np.random.default_rng(11)
+    R = R + 3.0e8 * np.sin(2 * np.pi * t / 487.0 + rng.uniform(0, 6, (3, 3, 1)))          # [3][3][n]
+    L = L * (1.0 + 1.0e-2 * np.sin(2 * np.pi * t / 1733.0 + rng.uniform(0, 6, (6, 1))))    # [6][n]
+    orbit = dict(base, mode=W.ORBIT_TABLES, R_table=np.ascontiguousarray(R), L_table=np.ascontiguousarray(L))
+    hp0, hc0 = W.monochromatic(n, dt, 4e-3, t0=base["t0"])
+    hp1, hc1 = W.monochromatic(n, dt, 1.1e-2, a_plus=0.3, a_cross=0.9, t0=base["t0"])
+    hp, hc = np.stack([hp0, hp1]), np.stack([hc0, hc1])
+    ang = [(0.3, 1.0, 0.7), (-0.9, 4.0, 2.2)]
+    hyb = {"t_hyb": base["t0"] + 0.5 * n * dt, "window_s": 600.0, "sigma_s": 15.0, "taper": W.TAPER_SIGMOID}
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, torch.from_numpy(orbit["R_table"]).to(dev), torch.from_numpy(orbit["L_table"]).to(dev))
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    for which, gen, fd in (("full", 20, 0), ("full", 15, 0), ("lfa", 20, 2), ("lfa", 15, 4), ("hybrid", 20, 2)):
+        if which == "full":
+            out = ltdi.response_full(orb, dhp, dhc, ang, gen, order, True, True)
+            ref, ref64 = (o.response_full(orbit, hp, hc, ang, gen, order) for o in (orc80, orc64))
+        elif which == "lfa":
+            out = ltdi.response_lfa(orb, dhp, dhc, ang, gen, order, fd, True, True)
+            ref, ref64 = (o.response_lfa(orbit, hp, hc, ang, gen, order, fd) for o in (orc80, orc64))
+        else:
+            out = ltdi.response_hybrid(orb, dhp, dhc, ang, gen, order, fd, hyb, True, True)
+            ref, ref64 = (o.response_hybrid(orbit, hp, hc, ang, gen, order, fd, hyb) for o in (orc80, orc64))
+        torch.cuda.synchronize()
+        out = to_numpy(out)
+        lo, hi = orc80.margins(orbit, gen, order, fd)
+        ref["floor"] = fp64_floor(ref, ref64, lo, n, hi)
+        ref["floor_XYZ"] = series_floor(ref["XYZ"], ref64["XYZ"], lo, n, hi)
+        ref["floor_y"] = series_floor(ref["y"], ref64["y"], lo, n, hi)
+        check(out, ref, lo, hi, n)
