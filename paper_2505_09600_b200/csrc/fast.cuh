@@ -621,7 +621,7 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>
-__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(FastParams p)
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : (WHICH == LTDI_RESPONSE_LFA ? 8 : 4)) tdi_kernel(FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);
