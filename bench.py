@@ -38,10 +38,10 @@ KERNEL_FLOPS = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), cfg2 only; None where no capture exists for the kernel
-TRAFFIC = {"full/tdi": 74.612736e6 + 3.713024e6}    # profiles/r01b_cfg2.md, tdi_kernel<32,FULL>, cfg2
+TRAFFIC = {"full/tdi": 74.6e6 + 3.4e6}    # profiles/r01c_cfg2.md, tdi_kernel<32,FULL>, cfg2
 # sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only)
-FP64_PIPE_PCT_NCU = {"full/orbit": 53.8, "full/anchor": 12.0, "full/link_full": 63.1, "full/tdi": 65.0,
-                     "lfa/link_lfa": 49.8, "lfa/tdi": 35.3, "hybrid/tdi": 30.1}
+FP64_PIPE_PCT_NCU = {"full/orbit": 53.7, "full/anchor": 11.9, "full/link_full": 63.1, "full/tdi": 64.8,
+                     "lfa/link_lfa": 51.2, "lfa/tdi": 40.6, "hybrid/tdi": 32.0}
 
 WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
@@ -349,7 +349,7 @@ def main():
         if world == 1 and not args.no_cpu_baseline:
             # ~10 s of CPU work: the oracle over the last <= 600 000 samples of source 0, repeated until 10 s have passed
             base, sec, reps = None, 0.0, 0
-            while sec < 10.0 and reps < 64:
+            while sec < 10.0 and reps < 4096:
                 base, s1 = cpu_baseline(cfg, hp, hc, ang, metas, 600000)
                 sec += s1
                 reps += 1
