@@ -31,10 +31,11 @@
 
 #define FAST_TC_R 7                       /* samples per thread in the TDI kernel */
 #define FAST_TCA 448                      /* samples per anchor tile */
-/* TDI tile geometry per response: G thread groups per channel, 7 G samples per tile, 3 G threads.  Full and LFA:
- * one warp per Michelson channel (224 samples, 96 threads, four CTAs per SM); the hybrid instance needs the shared
- * memory of both and runs 448-sample tiles with 192 threads, two CTAs per SM. */
-__host__ __device__ constexpr int tdi_g(int which) { return which == LTDI_RESPONSE_HYBRID ? 64 : 32; }
+/* TDI tile geometry per response: G thread groups per channel, 7 G samples per tile, 3 G threads.  Full: one warp
+ * per Michelson channel (224 samples, 96 threads, four CTAs per SM at 168 registers).  LFA: 448 samples, 192
+ * threads, four CTAs per SM at 80 registers (its tiles are latency-bound: two interpolations per channel).
+ * Hybrid: 448 samples, 192 threads, two CTAs per SM (it needs the shared memory of both responses). */
+__host__ __device__ constexpr int tdi_g(int which) { return which == LTDI_RESPONSE_FULL ? 32 : 64; }
 __host__ __device__ constexpr int tdi_tc(int which) { return FAST_TC_R * tdi_g(which); }
 __host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(which); }
 #define FAST_TA_THREADS 128
@@ -621,7 +622,7 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>
-__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : (WHICH == LTDI_RESPONSE_LFA ? 8 : 4)) tdi_kernel(FastParams p)
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);
