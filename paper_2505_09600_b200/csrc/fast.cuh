@@ -670,38 +670,47 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
     __shared__ double s_hdr[FAST_NA * 4];
 
-    /* phase 0: every global read of the tile is issued asynchronously, then one wait */
-    for (int i = tid; i < NLR * (FAST_TC / 2); i += FAST_TC_THREADS) {
-        const int l = i / (FAST_TC / 2), k = 2 * (i - l * (FAST_TC / 2));
+    /* phase 0: every global read of the tile is issued asynchronously, then one wait (row loops: no integer
+     * division in the index arithmetic) */
+#pragma unroll 1
+    for (int l = 0; l < NLR; ++l) {
         const double *src = tabL + l * p.stride;
-        if (n0 + k + 1 < p.n) cp_async16(Lr + l * FAST_TC + k, src + n0 + k);
-        else {
-            Lr[l * FAST_TC + k] = src[min(n0 + k, p.n - 1)];
-            Lr[l * FAST_TC + k + 1] = src[p.n - 1];
+        for (int k = 2 * tid; k < FAST_TC; k += 2 * FAST_TC_THREADS) {
+            if (n0 + k + 1 < p.n) cp_async16(Lr + l * FAST_TC + k, src + n0 + k);
+            else {
+                Lr[l * FAST_TC + k] = src[min(n0 + k, p.n - 1)];
+                Lr[l * FAST_TC + k + 1] = src[p.n - 1];
+            }
         }
     }
     if (has_full && need_full) {
-        const double *src = p.yF + b * p.lds;
         const int64_t ystride = p.batch * p.lds;
-        for (int i = tid; i < 6 * (yr / 2); i += FAST_TC_THREADS) {
-            const int l = i / (yr / 2), k = 2 * (i - l * (yr / 2));
-            const int64_t g = y0 + k;
-            if (g >= 0 && g + 1 < p.n) cp_async16(yF + l * yr + k, src + l * ystride + g);
-            else {
-                yF[l * yr + k] = (g >= 0 && g < p.n) ? src[l * ystride + g] : 0.0;
-                yF[l * yr + k + 1] = (g + 1 >= 0 && g + 1 < p.n) ? src[l * ystride + g + 1] : 0.0;
+#pragma unroll 1
+        for (int l = 0; l < 6; ++l) {
+            const double *src = p.yF + b * p.lds + l * ystride;
+            double *dst = yF + l * yr;
+            for (int k = 2 * tid; k < yr; k += 2 * FAST_TC_THREADS) {
+                const int64_t g = y0 + k;
+                if (g >= 0 && g + 1 < p.n) cp_async16(dst + k, src + g);
+                else {
+                    dst[k] = (g >= 0 && g < p.n) ? src[g] : 0.0;
+                    dst[k + 1] = (g + 1 >= 0 && g + 1 < p.n) ? src[g + 1] : 0.0;
+                }
             }
         }
     }
     if (has_lfa && need_lfa) {
-        const double *src = p.yL + b * p.lds;
         const int64_t ystride = p.batch * p.lds;
         const int len = yr + 2 * w;
-        for (int i = tid; i < 3 * len; i += FAST_TC_THREADS) {
-            const int l = i / len, k = i - l * len;
-            const int64_t g = y0 - w + k;
-            if (g >= 0 && g < p.n) cp_async8(yL + i, src + l * ystride + g);
-            else yL[i] = 0.0;
+#pragma unroll 1
+        for (int l = 0; l < 3; ++l) {
+            const double *src = p.yL + b * p.lds + l * ystride;
+            double *dst = yL + l * len;
+            for (int k = tid; k < len; k += FAST_TC_THREADS) {
+                const int64_t g = y0 - w + k;
+                if (g >= 0 && g < p.n) cp_async8(dst + k, src + g);
+                else dst[k] = 0.0;
+            }
         }
     }
     {
@@ -721,27 +730,41 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     /* phase 1 (LFA, hybrid): derivative of the LFA links */
     if (has_lfa) {
         if (need_lfa) {
-            /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range */
+            /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range.  A thread takes
+             * runs of FD_RUN consecutive samples of one link and slides a register window over them. */
+            constexpr int FD_RUN = 4;
             const int len = yr + 2 * w;
-            for (int i = tid; i < 3 * yr; i += FAST_TC_THREADS) {
-                const int l = i / yr, k = i - l * yr;
-                const int64_t m = y0 + k;
-                const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
-                const double *x = yL + l * len + k + w;
-                double d = 0.0;
-                if (in) {
-                    if (p.gen == LTDI_GEN_15) {
-                        d = ((w == 1) ? (x[1] - x[-1]) : (8.0 * (x[1] - x[-1]) - (x[2] - x[-2]))) * p.inv_fd1;
-                    } else {
-                        const double d1 = (x[1] - x[0]) - (x[0] - x[-1]);
-                        if (w == 1) d = d1 * p.inv_fd2;
-                        else {
-                            const double d2 = (x[2] - x[0]) - (x[0] - x[-2]);
-                            d = (16.0 * d1 - d2) * p.inv_fd2;
+            const int runs = (yr + FD_RUN - 1) / FD_RUN;
+            const bool g15 = p.gen == LTDI_GEN_15;
+            const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
+#pragma unroll 1
+            for (int l = 0; l < 3; ++l) {
+                for (int run = tid; run < runs; run += FAST_TC_THREADS) {
+                    const int k0 = run * FD_RUN;
+                    const double *x = yL + l * len + k0;   /* x[j] = sample y0 - w + k0 + j */
+                    double v[FD_RUN + 4];
+#pragma unroll
+                    for (int j = 0; j < FD_RUN + 4; ++j) v[j] = (j < FD_RUN + 2 * w && k0 + j < len) ? x[j] : 0.0;
+#pragma unroll
+                    for (int j = 0; j < FD_RUN; ++j) {
+                        const int k = k0 + j;
+                        if (k >= yr) break;
+                        const int64_t m = y0 + k;
+                        const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
+                        double d;
+                        if (w == 1) {   /* centre v[j + 1] */
+                            d = g15 ? (v[j + 2] - v[j]) : ((v[j + 2] - v[j + 1]) - (v[j + 1] - v[j]));
+                        } else {        /* centre v[j + 2] */
+                            if (g15) d = 8.0 * (v[j + 3] - v[j + 1]) - (v[j + 4] - v[j]);
+                            else {
+                                const double d1 = (v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]);
+                                const double d2 = (v[j + 4] - v[j + 2]) - (v[j + 2] - v[j]);
+                                d = 16.0 * d1 - d2;
+                            }
                         }
+                        dL[l * yr + k] = in ? d * scale : 0.0;
                     }
                 }
-                dL[i] = d;
             }
         }
         __syncthreads();
