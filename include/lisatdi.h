@@ -166,6 +166,40 @@ int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, co
                        const ltdi_hybrid *h_hyb, int64_t n_hyb, double *h_A, double *h_E, double *h_T,
                        void *d_scratch, size_t scratch_bytes, void *stream);
 
+/* ---- SURVEY.md 8(f)-1 (first "next" row): FFT -> noise-weighted inner product, overlap, mismatch, SNR --------- */
+/*
+ * Steps iv-v of the paper's likelihood evaluation.  Noise model: the analytic "Sangria" PSDs of Sec. II C,
+ * Eqs. (2.10)-(2.13): proof-mass and optical-path noise, galactic foreground (2.11) with T_obs in years
+ * (2.12), S_n^{A,E} and S_n^T for equal arms with Lambda = 4 sin^2(2x) (TDI 2.0) or 1 (TDI 1.5), x = 2 pi f L / c.
+ */
+typedef struct {
+    double arm_m;     /* L [m] */
+    double t_obs_yr;  /* observation time of Eq. (2.12) [yr] (1 in the paper) */
+    int32_t gen;      /* LTDI_GEN_15 | LTDI_GEN_20 */
+    int32_t galactic; /* 0: without S_gal (lower panel of Fig. 2), 1: with it */
+} ltdi_noise_desc;
+
+/* d_psd [2][nf] (device): row 0 = S_n^{A,E}(f_k), row 1 = S_n^T(f_k), f_k = k df; entry k = 0 is +inf. */
+int ltdi_noise_psd(const ltdi_noise_desc *desc, double df, int64_t nf, double *d_psd, void *stream);
+
+/* Plan for series of n samples (row stride ld, batch sources): creates the cuFFT plans (host objects; their
+ * device work area is part of the caller's d_work) and returns the bytes of d_work ltdi_overlap_products needs. */
+typedef struct ltdi_overlap ltdi_overlap;
+int ltdi_overlap_create(int64_t n, int64_t ld, int64_t batch, ltdi_overlap **out, size_t *work_bytes);
+int ltdi_overlap_destroy(ltdi_overlap *ovl);
+
+/* Two responses a and b (e.g. full and hybrid) as device series A, E, T [batch][ld] each.  Per source and channel
+ * c = A, E, T: x~_k = dt DFT(x)_k over all n samples (margins are zero, no window), f_k = k / (n dt), and
+ *   <x|y> = 4 Re sum_{fmin <= f_k <= fmax, k > 0} conj(x~_k) y~_k / S_n(f_k) / (n dt)        Eq. (5.1)
+ * with S_n = d_psd row 0 for A and E, row 1 for T (nf = n / 2 + 1 entries per row).
+ * d_out [batch][3][5]: <a|a>, <b|b>, <a|b>, overlap O = <a|b> / sqrt(<a|a> <b|b>) (5.2), mismatch 1 - |O|.
+ * d_snr [batch][2] or NULL: rho = sqrt(<A|A> + <E|E> + <T|T>) of a and of b, Eq. (6.1).
+ * d_work: 256-byte aligned device scratch of work_bytes.  Asynchronous on stream. */
+int ltdi_overlap_products(ltdi_overlap *ovl, const double *d_aA, const double *d_aE, const double *d_aT,
+                          const double *d_bA, const double *d_bE, const double *d_bT, double dt, const double *d_psd,
+                          double fmin, double fmax, double *d_out, double *d_snr, void *d_work, size_t work_bytes,
+                          void *stream);
+
 /* FP64 pipe probe for the roofline denominator: launches a register-resident chain of
  * fused multiply-adds (blocks x 256 threads, 8 independent chains per thread, iters x 64 DFMA per
  * chain step) and writes one value per thread to d_out (blocks * 256 doubles).  *dfma_per_launch

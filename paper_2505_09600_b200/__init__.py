@@ -78,6 +78,11 @@ _SIGNATURES = {
     "ltdi_host_scratch_bytes": (C.c_int, [C.c_int64, C.c_int64, _szp]),
     "ltdi_response_host": (C.c_int, [C.c_int, _vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                      C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_noise_psd": (C.c_int, [C.c_void_p, C.c_double, C.c_int64, _dp, _vp]),
+    "ltdi_overlap_create": (C.c_int, [C.c_int64, C.c_int64, C.c_int64, C.POINTER(_vp), _szp]),
+    "ltdi_overlap_destroy": (C.c_int, [_vp]),
+    "ltdi_overlap_products": (C.c_int, [_vp, _dp, _dp, _dp, _dp, _dp, _dp, C.c_double, _dp, C.c_double, C.c_double,
+                                        _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_fp64_probe": (C.c_int, [_dp, C.c_int, C.c_int, _vp, C.POINTER(C.c_double)]),
     "ltdi_profile_enable": (C.c_int, [C.c_int]),
     "ltdi_profile_read": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), _i64p]),
@@ -371,6 +376,53 @@ class HostPipeline:
                 slot["stream"].synchronize()
             else:
                 torch.cuda.current_stream().synchronize()
+
+
+class NoiseDesc(C.Structure):
+    _fields_ = [("arm_m", C.c_double), ("t_obs_yr", C.c_double), ("gen", C.c_int32), ("galactic", C.c_int32)]
+
+
+class Overlap:
+    """FFT of A, E, T -> noise-weighted inner products, overlap, mismatch, SNR (Eqs. 5.1, 5.2, 6.1)
+    of two responses of the same sources.  Owns the cuFFT plan handle and its device scratch."""
+
+    def __init__(self, n, ld, batch, device="cuda:0"):
+        self.n, self.ld, self.batch, self.device = int(n), int(ld), int(batch), torch.device(device)
+        handle, nbytes = C.c_void_p(), C.c_size_t()
+        with torch.cuda.device(self.device):
+            _check("ltdi_overlap_create", lib().ltdi_overlap_create(self.n, self.ld, self.batch, C.byref(handle),
+                                                                    C.byref(nbytes)))
+        self.handle = handle
+        self.work = torch.empty((nbytes.value + 7) // 8, dtype=torch.float64, device=self.device)
+        self.nf = self.n // 2 + 1
+        self.out = torch.empty(self.batch, 3, 5, dtype=torch.float64, device=self.device)
+        self.snr = torch.empty(self.batch, 2, dtype=torch.float64, device=self.device)
+
+    def psd(self, dt, gen, arm_m=ARM_M, t_obs_yr=1.0, galactic=True):
+        """[2][nf] device tensor: S_n^{A,E}, S_n^T on f_k = k / (n dt), Eqs. (2.10)-(2.13)."""
+        d = NoiseDesc(float(arm_m), float(t_obs_yr), int(gen), int(bool(galactic)))
+        psd = torch.empty(2, self.nf, dtype=torch.float64, device=self.device)
+        with torch.cuda.device(self.device):
+            _check("ltdi_noise_psd", lib().ltdi_noise_psd(C.byref(d), 1.0 / (self.n * float(dt)), self.nf,
+                                                          psd.data_ptr(), _stream()))
+        return psd
+
+    def products(self, a, b, dt, psd, fmin, fmax):
+        """a, b: dicts with device tensors A, E, T [batch][ld].  Returns (out [batch][3][5], snr [batch][2])."""
+        t = [_dev_f64(x[c], c) for x in (a, b) for c in "AET"]
+        for x in t:
+            assert x.shape == (self.batch, self.ld) or (self.batch == 1 and x.numel() == self.ld)
+        with torch.cuda.device(self.device):
+            rc = lib().ltdi_overlap_products(self.handle, *[x.data_ptr() for x in t], float(dt), psd.data_ptr(),
+                                             float(fmin), float(fmax), self.out.data_ptr(), self.snr.data_ptr(),
+                                             self.work.data_ptr(), self.work.numel() * 8, _stream())
+        _check("ltdi_overlap_products", rc)
+        return self.out, self.snr
+
+    def __del__(self):
+        h, self.handle = getattr(self, "handle", None), None
+        if h and _lib is not None:
+            _lib.ltdi_overlap_destroy(h)
 
 
 def fp64_probe(blocks=148 * 8, iters=2000, repeats=5, device="cuda:0"):

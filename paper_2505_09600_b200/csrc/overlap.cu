@@ -1,0 +1,248 @@
+// overlap.cu -- SURVEY.md 8(f)-1, the first "next" row: steps iv-v of the paper's likelihood evaluation:
+// Fourier transform of the TDI channels, the analytic noise PSDs of Sec. II C (Eqs. 2.10-2.13) and the
+// noise-weighted inner product, overlap, mismatch and SNR of Eqs. (5.1), (5.2), (6.1).
+//
+//   noise_psd_kernel   S_n^{A,E}(f_k), S_n^T(f_k) on f_k = k df                      (ALU, tiny)
+//   cuFFT D2Z          x~_k = sum_n x_n exp(-2 pi i k n / N): a plain library transform, batched over sources
+//   products_kernel    per (source, channel, block of bins): partial sums of |a~|^2 / S, |b~|^2 / S, Re(a~* b~) / S
+//                      over the band f_min <= f_k <= f_max                           (HBM-bound: 32 B read per bin)
+//   finalize_kernel    fixed-order sum of the partials (deterministic), 4 df dt^2 scaling, overlap, mismatch, SNR
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+
+#include <algorithm>
+#include <new>
+
+#include "../../include/lisatdi.h"
+
+#define OVL_CUDA_OK(expr)                                                                                 \
+    do {                                                                                                  \
+        const cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess) {                                                                          \
+            if (getenv("LTDI_DEBUG")) fprintf(stderr, "lisatdi %s:%d: %s\n", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+            (void)cudaGetLastError();                                                                     \
+            return LTDI_ECUDA;                                                                            \
+        }                                                                                                 \
+    } while (0)
+#define OVL_FFT_OK(expr)                                                                                  \
+    do {                                                                                                  \
+        const cufftResult r_ = (expr);                                                                    \
+        if (r_ != CUFFT_SUCCESS) {                                                                        \
+            if (getenv("LTDI_DEBUG")) fprintf(stderr, "lisatdi %s:%d: cuFFT error %d\n", __FILE__, __LINE__, (int)r_); \
+            return LTDI_ECUDA;                                                                            \
+        }                                                                                                 \
+    } while (0)
+
+#define OVL_THREADS 256
+#define OVL_BINS_PER_THREAD 8
+#define OVL_BINS_PER_BLOCK (OVL_THREADS * OVL_BINS_PER_THREAD)
+
+struct ltdi_overlap {
+    cufftHandle plan, plan_tail;
+    bool has_tail;
+    int64_t n, ld, batch, chunk, tail, nf, nblk;
+    size_t fft_work, spec_bytes, part_bytes, total;
+};
+
+namespace {
+
+constexpr double kC = 299792458.0;
+
+// Eqs. (2.10)-(2.13)
+__global__ void noise_psd_kernel(ltdi_noise_desc d, double df, int64_t nf, double *__restrict__ psd)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nf) return;
+    if (k == 0) { /* f = 0 lies outside every band: 1 / S = 0 */
+        psd[0] = INFINITY;
+        psd[nf] = INFINITY;
+        return;
+    }
+    const double pi = 3.14159265358979323846;
+    const double f = (double)k * df;
+    const double x = 2.0 * pi * f * d.arm_m / kC;
+    const double s_acc = 2.4e-15 * 2.4e-15, s_oms = 7.9e-12 * 7.9e-12;
+    const double r1 = 0.0004 / f, r2 = f / 0.008, r3 = 0.002 / f;
+    const double w1 = 2.0 * pi * f * kC, w2 = 2.0 * pi * f / kC;
+    const double s_pm = s_acc / (w1 * w1) * (1.0 + r1 * r1) * (1.0 + (r2 * r2) * (r2 * r2));     /* (2.10a) */
+    const double s_op = s_oms * (w2 * w2) * (1.0 + (r3 * r3) * (r3 * r3));                       /* (2.10b) */
+    double gal = 0.0;
+    if (d.galactic) { /* (2.11), (2.12) with T_obs in years */
+        const double lt = log10(d.t_obs_yr);
+        const double f1 = pow(10.0, -0.223499956 * lt - 2.70408439);
+        const double fk = pow(10.0, -0.360976122 * lt - 2.37822436);
+        const double sx = sin(x);
+        gal = 2.0 * x * x * sx * sx * 1.28265531e-44 * pow(f, -7.0 / 3.0) * exp(-pow(f / f1, 1.62966700)) *
+              (1.0 + tanh((fk - f) / 4.81078093e-4));
+    }
+    double sx, cx;
+    sincos(x, &sx, &cx);
+    const double s2x = sin(2.0 * x), c2x = cos(2.0 * x), shx = sin(0.5 * x);
+    const double lam = d.gen == LTDI_GEN_20 ? 4.0 * s2x * s2x : 1.0;
+    psd[k] = 8.0 * lam * sx * sx * (2.0 * (3.0 + 2.0 * cx + c2x) * s_pm + (2.0 + cx) * s_op) + 1.5 * lam * gal; /* (2.13a) */
+    psd[nf + k] = 16.0 * lam * sx * sx * ((1.0 - cx) * s_op + 8.0 * (shx * shx) * (shx * shx) * s_pm) + lam * gal; /* (2.13b) */
+}
+
+// spec: [6][chunk][nf] complex (a: A, E, T, then b: A, E, T); part: [chunk][3][nblk][3]
+__global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__restrict__ spec,
+                                                               const double *__restrict__ psd, int64_t nf, int64_t chunk,
+                                                               int64_t nsrc, double df, double fmin, double fmax,
+                                                               int64_t nblk, double *__restrict__ part)
+{
+    const int c = blockIdx.y;
+    const int64_t s = blockIdx.z;
+    const double2 *a = spec + ((int64_t)c * chunk + s) * nf;
+    const double2 *b = spec + ((int64_t)(3 + c) * chunk + s) * nf;
+    const double *sn = psd + (c == 2 ? nf : 0);
+    double aa = 0.0, bb = 0.0, ab = 0.0;
+    const int64_t k0 = (int64_t)blockIdx.x * OVL_BINS_PER_BLOCK + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < OVL_BINS_PER_THREAD; ++j) {
+        const int64_t k = k0 + (int64_t)j * OVL_THREADS;
+        if (k > 0 && k < nf) {
+            const double f = (double)k * df;
+            if (f >= fmin && f <= fmax) {                      /* (5.1): rectangle rule over the bins of the band */
+                const double2 u = a[k], v = b[k];
+                const double inv = 1.0 / sn[k];
+                aa += (u.x * u.x + u.y * u.y) * inv;
+                bb += (v.x * v.x + v.y * v.y) * inv;
+                ab += (u.x * v.x + u.y * v.y) * inv;           /* Re(conj(a~) b~) */
+            }
+        }
+    }
+    (void)nsrc;
+    __shared__ double red[3][OVL_THREADS / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        aa += __shfl_xor_sync(0xffffffffu, aa, o);
+        bb += __shfl_xor_sync(0xffffffffu, bb, o);
+        ab += __shfl_xor_sync(0xffffffffu, ab, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { red[0][warp] = aa; red[1][warp] = bb; red[2][warp] = ab; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double t = 0.0;
+#pragma unroll
+        for (int w = 0; w < OVL_THREADS / 32; ++w) t += red[threadIdx.x][w];
+        part[((s * 3 + c) * nblk + blockIdx.x) * 3 + threadIdx.x] = t;
+    }
+}
+
+// out: [batch][3][5] = <a|a>, <b|b>, <a|b>, overlap (5.2), mismatch 1 - |O|;  snr: [batch][2] = rho_a, rho_b (6.1)
+__global__ void finalize_kernel(const double *__restrict__ part, int64_t nsrc, int64_t nblk, double scale,
+                                double *__restrict__ out, double *__restrict__ snr)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsrc) return;
+    double ra = 0.0, rb = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        double aa = 0.0, bb = 0.0, ab = 0.0;
+        const double *p = part + (s * 3 + c) * nblk * 3;
+        for (int64_t i = 0; i < nblk; ++i) { aa += p[3 * i]; bb += p[3 * i + 1]; ab += p[3 * i + 2]; }
+        aa *= scale; bb *= scale; ab *= scale;
+        const double ov = ab / (sqrt(aa) * sqrt(bb));
+        double *o = out + (s * 3 + c) * 5;
+        o[0] = aa; o[1] = bb; o[2] = ab; o[3] = ov; o[4] = 1.0 - fabs(ov);
+        ra += aa; rb += bb;
+    }
+    if (snr) { snr[2 * s] = sqrt(ra); snr[2 * s + 1] = sqrt(rb); }
+}
+
+size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+int make_plan(cufftHandle *plan, int64_t n, int64_t ld, int64_t nf, int64_t batch, size_t *work)
+{
+    OVL_FFT_OK(cufftCreate(plan));
+    OVL_FFT_OK(cufftSetAutoAllocation(*plan, 0));
+    long long len = n, inembed = ld, onembed = nf;
+    OVL_FFT_OK(cufftMakePlanMany64(*plan, 1, &len, &inembed, 1, ld, &onembed, 1, nf, CUFFT_D2Z, batch, work));
+    return LTDI_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int ltdi_noise_psd(const ltdi_noise_desc *desc, double df, int64_t nf, double *d_psd, void *stream)
+{
+    if (!desc || !(df > 0.0) || nf < 1 || !d_psd || !(desc->arm_m > 0.0) || !(desc->t_obs_yr > 0.0)) return LTDI_EINVAL;
+    if (desc->gen != LTDI_GEN_15 && desc->gen != LTDI_GEN_20) return LTDI_EINVAL;
+    noise_psd_kernel<<<(unsigned)((nf + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*desc, df, nf, d_psd);
+    OVL_CUDA_OK(cudaGetLastError());
+    return LTDI_OK;
+}
+
+int ltdi_overlap_create(int64_t n, int64_t ld, int64_t batch, ltdi_overlap **out, size_t *work_bytes)
+{
+    if (n < 2 || ld < n || batch < 1 || !out || !work_bytes) return LTDI_EINVAL;
+    ltdi_overlap *o = new (std::nothrow) ltdi_overlap;
+    if (!o) return LTDI_EINVAL;
+    o->n = n; o->ld = ld; o->batch = batch; o->nf = n / 2 + 1;
+    /* sources per pass: the six spectra of a pass stay below 1 GiB */
+    const size_t per_source = (size_t)6 * o->nf * sizeof(double2);
+    o->chunk = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(batch, 32768), (int64_t)(((size_t)1 << 30) / per_source)));
+    o->tail = batch % o->chunk;
+    o->has_tail = o->tail != 0;
+    o->nblk = (o->nf + OVL_BINS_PER_BLOCK - 1) / OVL_BINS_PER_BLOCK;
+    size_t w0 = 0, w1 = 0;
+    int rc = make_plan(&o->plan, n, ld, o->nf, o->chunk, &w0);
+    if (rc == LTDI_OK && o->has_tail) rc = make_plan(&o->plan_tail, n, ld, o->nf, o->tail, &w1);
+    if (rc != LTDI_OK) { delete o; return rc; }
+    o->fft_work = align256(std::max(w0, w1));
+    o->spec_bytes = align256(per_source * o->chunk);
+    o->part_bytes = align256((size_t)o->chunk * 3 * o->nblk * 3 * sizeof(double));
+    o->total = o->fft_work + o->spec_bytes + o->part_bytes;
+    *work_bytes = o->total;
+    *out = o;
+    return LTDI_OK;
+}
+
+int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_aE, const double *d_aT,
+                          const double *d_bA, const double *d_bE, const double *d_bT, double dt, const double *d_psd,
+                          double fmin, double fmax, double *d_out, double *d_snr, void *d_work, size_t work_bytes,
+                          void *stream)
+{
+    if (!o || !d_aA || !d_aE || !d_aT || !d_bA || !d_bE || !d_bT || !d_psd || !d_out || !d_work) return LTDI_EINVAL;
+    if (!(dt > 0.0) || !(fmax >= fmin)) return LTDI_EINVAL;
+    if ((uintptr_t)d_work % 256) return LTDI_EINVAL;
+    if (work_bytes < o->total) return LTDI_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *base = (char *)d_work;
+    double2 *spec = (double2 *)(base + o->fft_work);
+    double *part = (double *)(base + o->fft_work + o->spec_bytes);
+    const double *in[6] = {d_aA, d_aE, d_aT, d_bA, d_bE, d_bT};
+    const double df = 1.0 / ((double)o->n * dt);
+    const double scale = 4.0 * df * dt * dt;          /* x~ = dt * DFT(x), (5.1) rectangle rule */
+    for (int64_t b0 = 0; b0 < o->batch; b0 += o->chunk) {
+        const int64_t nb = std::min(o->chunk, o->batch - b0);
+        cufftHandle plan = nb == o->chunk ? o->plan : o->plan_tail;
+        OVL_FFT_OK(cufftSetStream(plan, st));
+        OVL_FFT_OK(cufftSetWorkArea(plan, base));
+        for (int s = 0; s < 6; ++s) /* step iv */
+            OVL_FFT_OK(cufftExecD2Z(plan, (cufftDoubleReal *)(in[s] + b0 * o->ld),
+                                    (cufftDoubleComplex *)(spec + (int64_t)s * nb * o->nf)));
+        const dim3 grid((unsigned)o->nblk, 3, (unsigned)nb);
+        products_kernel<<<grid, OVL_THREADS, 0, st>>>(spec, d_psd, o->nf, nb, nb, df, fmin, fmax, o->nblk, part);
+        OVL_CUDA_OK(cudaGetLastError());
+        finalize_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(part, nb, o->nblk, scale, d_out + b0 * 15,
+                                                                      d_snr ? d_snr + 2 * b0 : nullptr);
+        OVL_CUDA_OK(cudaGetLastError());
+    }
+    return LTDI_OK;
+}
+
+int ltdi_overlap_destroy(ltdi_overlap *o)
+{
+    if (!o) return LTDI_OK;
+    cufftDestroy(o->plan);
+    if (o->has_tail) cufftDestroy(o->plan_tail);
+    delete o;
+    return LTDI_OK;
+}
+
+} // extern "C"
