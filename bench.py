@@ -294,6 +294,34 @@ def main():
         dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
     e2e_value = samples_per_step / (float(e2e_ms.item()) * 1e-3)
 
+    # next row: FFT -> noise-weighted inner products of the full and the hybrid response (steps
+    # iv-v of P:408); reported beside the step, not part of `value`
+    keep = lambda d: {k: v.clone() for k, v in d.items() if k in "AET"}
+    r_full = keep(ltdi.response_full(orb, d_hp, d_hc, ang, GEN, order, workspace=ws))
+    r_hyb = keep(ltdi.response_hybrid(orb, d_hp, d_hc, ang, GEN, order, FD, hyb, workspace=ws))
+    ovl = ltdi.Overlap(n, n, batch, dev)
+    psd = ovl.psd(cfg["dt"], GEN)
+    for _ in range(2):
+        ovl.products(r_full, r_hyb, cfg["dt"], psd, 1e-4, 2e-2)
+    torch.cuda.synchronize()
+    k_ovl = max(3, min(args.steps, 20))
+    o0, o1 = ev(), ev()
+    o0.record()
+    for _ in range(k_ovl):
+        o_out, o_snr = ovl.products(r_full, r_hyb, cfg["dt"], psd, 1e-4, 2e-2)
+    o1.record()
+    o1.synchronize()
+    ovl_ms = o0.elapsed_time(o1) / k_ovl
+    o_out, o_snr = o_out.cpu().numpy(), o_snr.cpu().numpy()
+    overlap_row = {"ms_per_call": ovl_ms, "samples_per_s": 2.0 * n * batch / (ovl_ms * 1e-3),
+                   "what": "6 FFTs (A, E, T of the full and of the hybrid response) + Eq. (5.1) products, overlap, "
+                           "mismatch, SNR per source; band 1e-4 .. 2e-2 Hz, Sangria PSD with galactic foreground",
+                   "spectrum_gbs": 6.0 * 16.0 * (n // 2 + 1) * batch / (ovl_ms * 1e-3) / 1e9,
+                   "mismatch_hybrid_vs_full_AET_source0": [float(x) for x in o_out[0, :, 4]],
+                   "max_mismatch_AE": float(np.nanmax(o_out[:, :2, 4])),
+                   "snr_full_source0": float(o_snr[0, 0])}
+    del r_full, r_hyb, ovl
+
     if rank == 0:
         # roofline of the dominant kernel: the fused response kernel in its full-response launch
         peaks = {}
@@ -345,7 +373,7 @@ def main():
                 "clocks": clk, "gpu_launches": int(launches),
                 "e2e": {"value": e2e_value, "unit": "TDI samples/s", "h2d_bytes_per_step": 3 * pipe.h2d_bytes,
                         "d2h_bytes_per_step": 3 * pipe.d2h_bytes},
-                "roofline": roofline}
+                "roofline": roofline, "next_rows": {"overlap": overlap_row}}
         if world == 1 and not args.no_cpu_baseline:
             # ~10 s of CPU work: the oracle over the last <= 600 000 samples of source 0, repeated until 10 s have passed
             base, sec, reps = None, 0.0, 0
