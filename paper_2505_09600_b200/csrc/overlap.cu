@@ -134,23 +134,33 @@ __global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__
 }
 
 // out: [batch][3][5] = <a|a>, <b|b>, <a|b>, overlap (5.2), mismatch 1 - |O|;  snr: [batch][2] = rho_a, rho_b (6.1)
-__global__ void finalize_kernel(const double *__restrict__ part, int64_t nsrc, int64_t nblk, double scale,
-                                double *__restrict__ out, double *__restrict__ snr)
+// One block of three warps per source, warp c sums the partials of channel c: lane i takes blocks i, i + 32, ...,
+// then a shuffle tree -- a fixed order, so the result does not depend on the launch.
+__global__ void __launch_bounds__(96) finalize_kernel(const double *__restrict__ part, int64_t nsrc, int64_t nblk,
+                                                      double scale, double *__restrict__ out, double *__restrict__ snr)
 {
-    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= nsrc) return;
-    double ra = 0.0, rb = 0.0;
-    for (int c = 0; c < 3; ++c) {
-        double aa = 0.0, bb = 0.0, ab = 0.0;
-        const double *p = part + (s * 3 + c) * nblk * 3;
-        for (int64_t i = 0; i < nblk; ++i) { aa += p[3 * i]; bb += p[3 * i + 1]; ab += p[3 * i + 2]; }
-        aa *= scale; bb *= scale; ab *= scale;
+    const int64_t s = blockIdx.x;
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double aa = 0.0, bb = 0.0, ab = 0.0;
+    const double *p = part + (s * 3 + c) * nblk * 3;
+    for (int64_t i = lane; i < nblk; i += 32) { aa += p[3 * i]; bb += p[3 * i + 1]; ab += p[3 * i + 2]; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        aa += __shfl_xor_sync(0xffffffffu, aa, o);
+        bb += __shfl_xor_sync(0xffffffffu, bb, o);
+        ab += __shfl_xor_sync(0xffffffffu, ab, o);
+    }
+    aa *= scale; bb *= scale; ab *= scale;
+    __shared__ double self[3][2];
+    if (lane == 0) {
         const double ov = ab / (sqrt(aa) * sqrt(bb));
         double *o = out + (s * 3 + c) * 5;
         o[0] = aa; o[1] = bb; o[2] = ab; o[3] = ov; o[4] = 1.0 - fabs(ov);
-        ra += aa; rb += bb;
+        self[c][0] = aa; self[c][1] = bb;
     }
-    if (snr) { snr[2 * s] = sqrt(ra); snr[2 * s + 1] = sqrt(rb); }
+    __syncthreads();
+    if (snr && threadIdx.x < 2) snr[2 * s + threadIdx.x] = sqrt((self[0][threadIdx.x] + self[1][threadIdx.x]) + self[2][threadIdx.x]);
+    (void)nsrc;
 }
 
 size_t align256(size_t x) { return (x + 255) / 256 * 256; }
@@ -229,7 +239,7 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
         const dim3 grid((unsigned)o->nblk, 3, (unsigned)nb);
         products_kernel<<<grid, OVL_THREADS, 0, st>>>(spec, d_psd, o->nf, nb, nb, df, fmin, fmax, o->nblk, part);
         OVL_CUDA_OK(cudaGetLastError());
-        finalize_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(part, nb, o->nblk, scale, d_out + b0 * 15,
+        finalize_kernel<<<(unsigned)nb, 96, 0, st>>>(part, nb, o->nblk, scale, d_out + b0 * 15,
                                                                       d_snr ? d_snr + 2 * b0 : nullptr);
         OVL_CUDA_OK(cudaGetLastError());
     }
