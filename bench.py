@@ -319,7 +319,8 @@ def main():
                    "spectrum_gbs": 6.0 * 16.0 * (n // 2 + 1) * batch / (ovl_ms * 1e-3) / 1e9,
                    "mismatch_hybrid_vs_full_AET_source0": [float(x) for x in o_out[0, :, 4]],
                    "max_mismatch_AE": float(np.nanmax(o_out[:, :2, 4])),
-                   "snr_full_source0": float(o_snr[0, 0])}
+                   "snr_full_source0": float(o_snr[0, 0]),
+                   "lnL_full_as_data_hybrid_as_template_source0": float(o_snr[0, 2])}
     del r_full, r_hyb, ovl
 
     if rank == 0:

@@ -193,7 +193,9 @@ int ltdi_overlap_destroy(ltdi_overlap *ovl);
  *   <x|y> = 4 Re sum_{fmin <= f_k <= fmax, k > 0} conj(x~_k) y~_k / S_n(f_k) / (n dt)        Eq. (5.1)
  * with S_n = d_psd row 0 for A and E, row 1 for T (nf = n / 2 + 1 entries per row).
  * d_out [batch][3][5]: <a|a>, <b|b>, <a|b>, overlap O = <a|b> / sqrt(<a|a> <b|b>) (5.2), mismatch 1 - |O|.
- * d_snr [batch][2] or NULL: rho = sqrt(<A|A> + <E|E> + <T|T>) of a and of b, Eq. (6.1).
+ * d_snr [batch][3] or NULL: rho = sqrt(<A|A> + <E|E> + <T|T>) of a and of b, Eq. (6.1), and the Gaussian
+ * log-likelihood ln L = -1/2 sum_c <a_c - b_c|a_c - b_c> = -1/2 sum_c (<a|a> + <b|b> - 2 <a|b>) of Eq. (D4)
+ * with a in the role of the data d and b of the template h.
  * d_work: 256-byte aligned device scratch of work_bytes.  Asynchronous on stream. */
 int ltdi_overlap_products(ltdi_overlap *ovl, const double *d_aA, const double *d_aE, const double *d_aT,
                           const double *d_bA, const double *d_bE, const double *d_bT, double dt, const double *d_psd,

@@ -101,3 +101,10 @@ def products(a, b, dt, gen, fmin, fmax, arm_m=2.5e9, t_obs_yr=1.0, galactic=True
 def snr(prod_self):
     """Eq. (6.1): rho = sqrt(<A|A> + <E|E> + <T|T>) from the [batch][3] self products."""
     return np.sqrt(np.sum(np.asarray(prod_self), axis=-1))
+
+
+def log_likelihood(prod):
+    """Eq. (D4): ln L = -1/2 <d - h|d - h> = -1/2 (<d|d> + <h|h> - 2 <d|h>), summed over A, E, T, from the
+    [batch][3][>=3] products with a = d and b = h."""
+    p = np.asarray(prod)
+    return -0.5 * np.sum((p[:, :, 0] + p[:, :, 1]) - 2.0 * p[:, :, 2], axis=-1)

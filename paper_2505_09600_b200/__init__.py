@@ -396,7 +396,7 @@ class Overlap:
         self.work = torch.empty((nbytes.value + 7) // 8, dtype=torch.float64, device=self.device)
         self.nf = self.n // 2 + 1
         self.out = torch.empty(self.batch, 3, 5, dtype=torch.float64, device=self.device)
-        self.snr = torch.empty(self.batch, 2, dtype=torch.float64, device=self.device)
+        self.snr = torch.empty(self.batch, 3, dtype=torch.float64, device=self.device)
 
     def psd(self, dt, gen, arm_m=ARM_M, t_obs_yr=1.0, galactic=True):
         """[2][nf] device tensor: S_n^{A,E}, S_n^T on f_k = k / (n dt), Eqs. (2.10)-(2.13)."""
@@ -408,7 +408,8 @@ class Overlap:
         return psd
 
     def products(self, a, b, dt, psd, fmin, fmax):
-        """a, b: dicts with device tensors A, E, T [batch][ld].  Returns (out [batch][3][5], snr [batch][2])."""
+        """a, b: dicts with device tensors A, E, T [batch][ld].  Returns (out [batch][3][5], snr [batch][3]):
+        snr columns = rho_a, rho_b (6.1), ln L of (D4)."""
         t = [_dev_f64(x[c], c) for x in (a, b) for c in "AET"]
         for x in t:
             assert x.shape == (self.batch, self.ld) or (self.batch == 1 and x.numel() == self.ld)

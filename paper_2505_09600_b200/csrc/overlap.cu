@@ -133,8 +133,8 @@ __global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__
     }
 }
 
-// out: [batch][3][5] = <a|a>, <b|b>, <a|b>, overlap (5.2), mismatch 1 - |O|;  snr: [batch][2] = rho_a, rho_b (6.1)
-// One block of three warps per source, warp c sums the partials of channel c: lane i takes blocks i, i + 32, ...,
+// out: [batch][3][5] = <a|a>, <b|b>, <a|b>, overlap (5.2), mismatch 1 - |O|;  snr: [batch][3] = rho_a, rho_b (6.1) and
+// ln L = -1/2 <a - b|a - b> (D4).  One block of three warps per source, warp c sums the partials of channel c: lane i takes blocks i, i + 32, ...,
 // then a shuffle tree -- a fixed order, so the result does not depend on the launch.
 __global__ void __launch_bounds__(96) finalize_kernel(const double *__restrict__ part, int64_t nsrc, int64_t nblk,
                                                       double scale, double *__restrict__ out, double *__restrict__ snr)
@@ -151,15 +151,20 @@ __global__ void __launch_bounds__(96) finalize_kernel(const double *__restrict__
         ab += __shfl_xor_sync(0xffffffffu, ab, o);
     }
     aa *= scale; bb *= scale; ab *= scale;
-    __shared__ double self[3][2];
+    __shared__ double self[3][3];
     if (lane == 0) {
         const double ov = ab / (sqrt(aa) * sqrt(bb));
         double *o = out + (s * 3 + c) * 5;
         o[0] = aa; o[1] = bb; o[2] = ab; o[3] = ov; o[4] = 1.0 - fabs(ov);
-        self[c][0] = aa; self[c][1] = bb;
+        self[c][0] = aa; self[c][1] = bb; self[c][2] = ab;
     }
     __syncthreads();
-    if (snr && threadIdx.x < 2) snr[2 * s + threadIdx.x] = sqrt((self[0][threadIdx.x] + self[1][threadIdx.x]) + self[2][threadIdx.x]);
+    if (snr && threadIdx.x < 2) snr[3 * s + threadIdx.x] = sqrt((self[0][threadIdx.x] + self[1][threadIdx.x]) + self[2][threadIdx.x]);
+    if (snr && threadIdx.x == 2) { /* (D4): ln L = -1/2 <a - b|a - b> summed over the channels */
+        double q = 0.0;
+        for (int ch = 0; ch < 3; ++ch) q += (self[ch][0] + self[ch][1]) - 2.0 * self[ch][2];
+        snr[3 * s + 2] = -0.5 * q;
+    }
     (void)nsrc;
 }
 
@@ -240,7 +245,7 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
         products_kernel<<<grid, OVL_THREADS, 0, st>>>(spec, d_psd, o->nf, nb, nb, df, fmin, fmax, o->nblk, part);
         OVL_CUDA_OK(cudaGetLastError());
         finalize_kernel<<<(unsigned)nb, 96, 0, st>>>(part, nb, o->nblk, scale, d_out + b0 * 15,
-                                                                      d_snr ? d_snr + 2 * b0 : nullptr);
+                                                                      d_snr ? d_snr + 3 * b0 : nullptr);
         OVL_CUDA_OK(cudaGetLastError());
     }
     return LTDI_OK;

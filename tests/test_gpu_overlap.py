@@ -48,6 +48,9 @@ def compare(got, snr, want):
     assert np.max(np.abs(got[:, :, 3:] - want[:, :, 3:])) < 1e-12
     assert np.max(np.abs(snr[:, 0] / oo.snr(want[:, :, 0]) - 1.0)) < 1e-11
     assert np.max(np.abs(snr[:, 1] / oo.snr(want[:, :, 1]) - 1.0)) < 1e-11
+    # ln L of (D4) is a difference of the products: judged against their size
+    scale = np.sum(want[:, :, 0] + want[:, :, 1], axis=-1)
+    assert np.max(np.abs(snr[:, 2] - oo.log_likelihood(want)) / scale) < 1e-11
 
 
 @pytest.mark.parametrize("gen", [15, 20])

@@ -156,3 +156,24 @@ def test_paper_accuracy_statements_hold_on_a_synthetic_merger(orc64):
         assert m[0] < lfa_bar and m[1] < lfa_bar and 0.1 < m[2] <= 1.0, (gen, m)
     rho = oo.snr(oo.products(full, full, dt, 20, 1e-4, 2e-2)[:, :, 0])[0]
     assert 100.0 < rho < 1e4        # an MBHB at 5 Gpc: SNR in the hundreds to thousands (P:502 quotes 1876)
+
+
+def test_log_likelihood_of_eq_D4():
+    rng = np.random.default_rng(9)
+    n, dt = 5000, 10.0
+    t = dt * np.arange(n)
+    d = {c: 1e-21 * (np.sin(2 * np.pi * 3e-3 * t + i) * np.hanning(n))[None] for i, c in enumerate("AET")}
+    same = oo.products(d, d, dt, 20, 1e-4, 2e-2)
+    assert abs(oo.log_likelihood(same)[0]) < 1e-12 * oo.snr(same[:, :, 0])[0] ** 2        # h = d: ln L = 0
+    zero = {c: np.zeros_like(v) for c, v in d.items()}
+    pz = oo.products(d, zero, dt, 20, 1e-4, 2e-2)
+    assert oo.log_likelihood(pz)[0] == pytest.approx(-0.5 * oo.snr(pz[:, :, 0])[0] ** 2, rel=1e-14)   # h = 0: -rho^2 / 2
+    eps = 1e-3
+    ps = oo.products(d, {c: (1 + eps) * v for c, v in d.items()}, dt, 20, 1e-4, 2e-2)
+    assert oo.log_likelihood(ps)[0] == pytest.approx(-0.5 * eps ** 2 * oo.snr(ps[:, :, 0])[0] ** 2, rel=1e-6)
+    # direct definition: inner product of the residual with itself
+    h = {c: v + 1e-23 * rng.standard_normal(v.shape) for c, v in d.items()}
+    pr = oo.products(d, h, dt, 20, 1e-4, 2e-2)
+    res = {c: d[c] - h[c] for c in "AET"}
+    direct = -0.5 * oo.products(res, res, dt, 20, 1e-4, 2e-2)[0, :, 0].sum()
+    assert oo.log_likelihood(pr)[0] == pytest.approx(direct, rel=1e-9)
