@@ -234,11 +234,11 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
 // link kernel: LFA == false: Eq. (2.5), six links;  LFA == true: Eq. (B10) at (B1), links +1, +2, +3
 // ---------------------------------------------------------------------------------------------
 template <int H, bool LFA>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
+__device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
 {
     extern __shared__ double smem[];
-    const int64_t b = (int64_t)blockIdx.x % p.batch;
-    int64_t tile = (int64_t)blockIdx.x / p.batch;
+    const int64_t b = bid % p.batch;
+    int64_t tile = bid / p.batch;
     /* hybrid: the full links live at the end of the series; schedule those tiles first (no long tail) */
     if (!LFA && p.which == LTDI_RESPONSE_HYBRID) tile = p.ntilesA - 1 - tile;
     const int64_t a0 = tile * FAST_TA;               /* first sample of the tile (even) */
@@ -414,6 +414,22 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
             *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
         }
     }
+}
+
+template <int H, bool LFA>
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
+{
+    link_body<H, LFA>(p, blockIdx.x);
+}
+
+// hybrid: both kinds of link tiles in ONE launch -- the few full-link tiles (first in the grid: they are the heavy
+// ones) run beside the LFA-link tiles instead of as a launch of their own that leaves most SMs idle
+template <int H>
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_hybrid_kernel(FastParams p)
+{
+    const int64_t nfull = p.ntilesA * p.batch;
+    if ((int64_t)blockIdx.x < nfull) link_body<H, false>(p, blockIdx.x);
+    else link_body<H, true>(p, (int64_t)blockIdx.x - nfull);
 }
 
 // ---------------------------------------------------------------------------------------------

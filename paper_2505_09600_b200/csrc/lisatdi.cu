@@ -290,8 +290,14 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
                                  (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double); /* + raw strain */
     const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
     int rc;
-    if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
-    if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link_lfa, smem_max))) return rc;
+    const bool hybrid = which == LTDI_RESPONSE_HYBRID;
+    const size_t smem_link_hyb = std::max(smem_link, smem_link_lfa);
+    if (hybrid) {
+        if ((rc = set_smem(link_hybrid_kernel<H>, smem_link_hyb, smem_max))) return rc;
+    } else {
+        if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
+        if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link_lfa, smem_max))) return rc;
+    }
     void (*tdi)(FastParams) = which == LTDI_RESPONSE_FULL  ? tdi_kernel<M, LTDI_RESPONSE_FULL>
                               : which == LTDI_RESPONSE_LFA ? tdi_kernel<M, LTDI_RESPONSE_LFA>
                                                            : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
@@ -318,12 +324,18 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         p.XYZ = rp.XYZ; p.Y = rp.Y;
         p.yF = ys; p.yL = ys + (full ? (size_t)6 * nb * lay.lds : 0);
         if (lay.ntilesA * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
-        if (full) {
+        if (hybrid) {
+            if (2 * lay.ntilesA * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
+            ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
+            link_hybrid_kernel<H><<<(unsigned)(2 * lay.ntilesA * nb), FAST_TA_THREADS, smem_link_hyb, st>>>(p);
+            count_launch();
+        }
+        if (full && !hybrid) {
             ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
             link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
             count_launch();
         }
-        if (lfa) {
+        if (lfa && !hybrid) {
             ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
             link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
             count_launch();
