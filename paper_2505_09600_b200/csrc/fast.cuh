@@ -58,7 +58,10 @@ struct FastParams {
     double inv_fd1, inv_fd2; /* 1 / (2 dt) | 1 / (12 dt) and 1 / dt^2 | 1 / (12 dt^2): stencil denominators (fd 2 | 4) */
     const double *hp, *hc;
     int64_t ld, batch;       /* batch = sources of this launch (a chunk) */
-    const double *frames;    /* [batch][LTDI_FRAME_STRIDE] of this chunk */
+    const double *frames;    /* [batch][LTDI_FRAME_STRIDE] of this chunk (use_small == 0) */
+    int use_small;           /* batch_all <= 32: sources and hybrid windows travel in `small` as kernel arguments and
+                              * every CTA derives its source frame itself (no parameter kernel in front of the call) */
+    double small[32 * 7];    /* [32][3] beta, lambda, psi, then [32][4] t_hyb, window, sigma, taper (by absolute source) */
     const double *hyb;       /* [n_hyb][4] of this chunk (t_hyb, window, sigma, taper) */
     int64_t n_hyb;
     int which, gen, fd;
@@ -246,10 +249,15 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     const int w = LFA ? (int)p.w : 0;
 
     __shared__ double fr[LTDI_FRAME_STRIDE];
-    if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
+    if (p.use_small) {
+        if (tid == 0) { /* S1, Eq. (2.1) with G1, (2.3): the same device function as the parameter kernel */
+            const double *sr = p.small + 3 * (p.b0 + b);
+            source_frame_one(sr[0], sr[1], sr[2], fr);
+        }
+    } else if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
 
     if (p.which == LTDI_RESPONSE_HYBRID) { /* skip tiles whose links the hybrid never uses */
-        const double *hy = p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
+        const double *hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
         const double halo = (double)(p.m2 + 2 * p.w + H + 2) * p.dt;
         const double t_first = p.t0 + (double)a0 * p.dt, t_last = p.t0 + (double)(a0 + FAST_TA - 1) * p.dt;
         if (LFA) { if (t_first - halo - hy[0] > 0.5 * hy[1]) return; }
@@ -417,7 +425,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
 }
 
 template <int H, bool LFA>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(const __grid_constant__ FastParams p)
 {
     link_body<H, LFA>(p, blockIdx.x);
 }
@@ -425,7 +433,7 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(FastParams p)
 // hybrid: both kinds of link tiles in ONE launch -- the few full-link tiles (first in the grid: they are the heavy
 // ones) run beside the LFA-link tiles instead of as a launch of their own that leaves most SMs idle
 template <int H>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_hybrid_kernel(FastParams p)
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_hybrid_kernel(const __grid_constant__ FastParams p)
 {
     const int64_t nfull = p.ntilesA * p.batch;
     if ((int64_t)blockIdx.x < nfull) link_body<H, false>(p, blockIdx.x);
@@ -478,7 +486,7 @@ __device__ __forceinline__ double lfa_delay(int gen, int id, double L2, double L
 // anchor kernel: one block per TDI tile; thread a < FAST_NA builds the anchor of delay a
 // ---------------------------------------------------------------------------------------------
 template <int M>
-__global__ void __launch_bounds__(64) anchor_kernel(FastParams p, double *anc, double *hdr)
+__global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ FastParams p, double *anc, double *hdr)
 {
     const int64_t tile = blockIdx.x;
     const int64_t n0 = tile * FAST_TCA, n1 = min(n0 + (int64_t)FAST_TCA, p.n);
@@ -638,7 +646,7 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>
-__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(FastParams p)
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(const __grid_constant__ FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);
@@ -659,7 +667,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     bool need_full = WHICH == LTDI_RESPONSE_FULL, need_lfa = WHICH == LTDI_RESPONSE_LFA;
     const double *hy = nullptr;
     if (WHICH == LTDI_RESPONSE_HYBRID) {
-        hy = p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
+        hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
         const double t_first = p.t0 + (double)n0 * p.dt, t_last = p.t0 + (double)(n1 - 1) * p.dt;
         need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0, Eq. (4.5) */
         need_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0 */

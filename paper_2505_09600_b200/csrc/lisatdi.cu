@@ -256,7 +256,8 @@ int set_smem(K kernel, size_t smem, int smem_max)
 
 // the tuned path: anchors once per call, then link kernel(s) and TDI kernel per chunk of sources
 template <int M>
-int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work, cudaStream_t st)
+int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work, cudaStream_t st,
+             const double *small /* [32 * 7] host values or nullptr */)
 {
     constexpr int H = M / 2;
     const ltdi_orbit_desc &d = orb->desc;
@@ -279,6 +280,8 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     p.inv_fd1 = 1.0 / ((mg.w == 1 ? 2.0 : 12.0) * rp.dt);
     p.inv_fd2 = 1.0 / ((mg.w == 1 ? 1.0 : 12.0) * rp.dt * rp.dt);
     p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
+    p.use_small = small != nullptr;
+    if (small) std::memcpy(p.small, small, sizeof p.small);
     double *anc = work, *hdr = anc + lay.anc, *ys = hdr + lay.hdr;
     p.anc = anc; p.anc_hdr = hdr;
 
@@ -383,8 +386,11 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     double *w_src = (double *)d_work;
     double *w_frames = w_src + 3 * batch;
     HybDev *w_hyb = (HybDev *)(w_frames + LTDI_FRAME_STRIDE * batch);
+    SmallArgs small_args;
+    bool have_small = false;   /* batch <= 32: the tuned kernels take the parameters as arguments (no launch) */
     if (batch <= 32) {
         SmallArgs a;
+        std::memset(&a, 0, sizeof a);
         for (int64_t b = 0; b < batch; ++b) {
             a.v[3 * b + 0] = h_src[b].beta; a.v[3 * b + 1] = h_src[b].lambda; a.v[3 * b + 2] = h_src[b].psi;
         }
@@ -392,12 +398,8 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
             a.v[96 + 4 * i + 0] = h_hyb[i].t_hyb; a.v[96 + 4 * i + 1] = h_hyb[i].window_s;
             a.v[96 + 4 * i + 2] = h_hyb[i].sigma_s; a.v[96 + 4 * i + 3] = (double)h_hyb[i].taper;
         }
-        {
-            ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
-            unpack_small_kernel<<<1, 128, 0, st>>>(a, (int)batch, (int)n_hyb, w_src, w_frames, w_hyb);
-        }
-        count_launch();
-        LTDI_CUDA_OK(cudaGetLastError());
+        small_args = a;
+        have_small = true;
     } else {
         std::vector<double> pack((size_t)batch * 3 + (size_t)n_hyb * 4);
         for (int64_t b = 0; b < batch; ++b) {
@@ -435,9 +437,18 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
     if (fast_order(order)) {
-        const int frc = M == 32 ? run_fast<32>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st)
-                                : run_fast<10>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st);
+        const double *sm = have_small ? small_args.v : nullptr;
+        const int frc = M == 32 ? run_fast<32>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st, sm)
+                                : run_fast<10>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st, sm);
         if (frc != LTDI_EUNSUPPORTED) return frc;   /* else: shapes the tuned kernels do not cover */
+    }
+    if (have_small) { /* the generic kernel reads frames and windows from the workspace */
+        {
+            ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
+            unpack_small_kernel<<<1, 128, 0, st>>>(small_args, (int)batch, (int)n_hyb, w_src, w_frames, w_hyb);
+        }
+        count_launch();
+        LTDI_CUDA_OK(cudaGetLastError());
     }
 
     int tile = 256;
