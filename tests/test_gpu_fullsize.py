@@ -145,9 +145,23 @@ def batched_case(ltdi, orc80, orc64, k, batch, unique, runs, check_sources):
                                (cfg["name"], which, "source", s))
 
 
+def stratified_sources(orc, k, unique):
+    """the parity subset holds the chirp-mass extremes and the source whose Eq. (2.5) is worst
+    conditioned (smallest min_l (1 - k.n_l)), plus two fixed ones"""
+    cfg = W.config(k, batch=unique)
+    mc, cond = [], []
+    for i in range(unique):
+        _, _, ang, meta = W.source(W.config(k, n=16, batch=1), i)     # parameters only: a 16-sample series is cheap
+        mc.append(meta["mchirp_s"])
+        kn = orc.antenna(cfg["orbit"], ang, cfg["n"] // 2)[:, 2]
+        cond.append(float(np.min(1.0 - kn)))
+    picks = {int(np.argmin(mc)), int(np.argmax(mc)), int(np.argmin(cond)), 0, unique - 1}
+    return sorted(picks)
+
+
 def test_config4_full_batch(ltdi, orc80, orc64):
     """B = 4096 x N = 131 072 hybrid TDI 2.0 (8.6 GB in, 12.9 GB out)"""
-    batched_case(ltdi, orc80, orc64, 4, 4096, 64, [("hybrid", 20, 2)], [0, 17, 42, 63])
+    batched_case(ltdi, orc80, orc64, 4, 4096, 64, [("hybrid", 20, 2)], stratified_sources(orc80, 4, 64))
 
 
 def test_config5_full_batch(ltdi, orc80, orc64):
