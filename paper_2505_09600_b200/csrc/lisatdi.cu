@@ -215,6 +215,26 @@ __global__ void unpack_small_kernel(SmallArgs a, int batch, int n_hyb, double *s
     if (i < batch) source_frame_one(a.v[3 * i], a.v[3 * i + 1], a.v[3 * i + 2], frames + i * LTDI_FRAME_STRIDE); /* S1 */
 }
 
+/* batch > 32: the parameters of up to 512 sources per launch travel as kernel arguments (28 KB; CUDA >= 12.1 allows
+ * 32 764 bytes on sm_70+).  A cudaMemcpyAsync from pageable host memory above 64 KB would block the host until the
+ * stream has drained, which leaves the GPU idle between the calls of a step. */
+#define LTDI_BIG_SOURCES 512
+struct BigArgs { double src[LTDI_BIG_SOURCES * 3]; double hyb[LTDI_BIG_SOURCES * 4]; };
+
+__global__ void unpack_big_kernel(const __grid_constant__ BigArgs a, int count, int n_hyb_here, double *src, double *frames,
+                                  double *hyb)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) {
+        src[3 * i] = a.src[3 * i]; src[3 * i + 1] = a.src[3 * i + 1]; src[3 * i + 2] = a.src[3 * i + 2];
+        source_frame_one(a.src[3 * i], a.src[3 * i + 1], a.src[3 * i + 2], frames + i * LTDI_FRAME_STRIDE); /* S1 */
+    }
+    if (i < n_hyb_here) {
+        hyb[4 * i] = a.hyb[4 * i]; hyb[4 * i + 1] = a.hyb[4 * i + 1];
+        hyb[4 * i + 2] = a.hyb[4 * i + 2]; hyb[4 * i + 3] = a.hyb[4 * i + 3];
+    }
+}
+
 template <int MT, bool STAGE>
 int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t st)
 {
@@ -401,25 +421,32 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         small_args = a;
         have_small = true;
     } else {
-        std::vector<double> pack((size_t)batch * 3 + (size_t)n_hyb * 4);
-        for (int64_t b = 0; b < batch; ++b) {
-            pack[3 * b + 0] = h_src[b].beta; pack[3 * b + 1] = h_src[b].lambda; pack[3 * b + 2] = h_src[b].psi;
+        BigArgs *big = new (std::nothrow) BigArgs;
+        if (!big) return LTDI_EINVAL;
+        for (int64_t b0 = 0; b0 < batch; b0 += LTDI_BIG_SOURCES) {
+            const int cnt = (int)std::min<int64_t>(LTDI_BIG_SOURCES, batch - b0);
+            for (int i = 0; i < cnt; ++i) {
+                big->src[3 * i + 0] = h_src[b0 + i].beta; big->src[3 * i + 1] = h_src[b0 + i].lambda;
+                big->src[3 * i + 2] = h_src[b0 + i].psi;
+            }
+            int nh = 0;   /* hybrid windows of this slice (n_hyb is 0, 1 or batch) */
+            if (n_hyb == batch) nh = cnt;
+            else if (n_hyb == 1 && b0 == 0) nh = 1;
+            for (int i = 0; i < nh; ++i) {
+                const ltdi_hybrid &h = h_hyb[n_hyb == 1 ? 0 : b0 + i];
+                big->hyb[4 * i + 0] = h.t_hyb; big->hyb[4 * i + 1] = h.window_s;
+                big->hyb[4 * i + 2] = h.sigma_s; big->hyb[4 * i + 3] = (double)h.taper;
+            }
+            {
+                ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
+                unpack_big_kernel<<<(LTDI_BIG_SOURCES + 127) / 128, 128, 0, st>>>(
+                    *big, cnt, nh, w_src + 3 * b0, w_frames + LTDI_FRAME_STRIDE * b0,
+                    (double *)w_hyb + (n_hyb == 1 ? 0 : 4 * b0));
+            }
+            count_launch();
+            if (cudaGetLastError() != cudaSuccess) { delete big; return LTDI_ECUDA; }
         }
-        double *hy = pack.data() + 3 * batch;
-        for (int64_t i = 0; i < n_hyb; ++i) {
-            hy[4 * i + 0] = h_hyb[i].t_hyb; hy[4 * i + 1] = h_hyb[i].window_s;
-            hy[4 * i + 2] = h_hyb[i].sigma_s; hy[4 * i + 3] = (double)h_hyb[i].taper;
-        }
-        /* pageable source: the runtime has consumed `pack` when these calls return */
-        LTDI_CUDA_OK(cudaMemcpyAsync(w_src, pack.data(), sizeof(double) * 3 * batch, cudaMemcpyHostToDevice, st));
-        if (n_hyb)
-            LTDI_CUDA_OK(cudaMemcpyAsync(w_hyb, hy, sizeof(double) * 4 * n_hyb, cudaMemcpyHostToDevice, st));
-        {
-            ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
-            source_frame_kernel<<<(unsigned)((batch + 127) / 128), 128, 0, st>>>(w_src, w_frames, batch);
-        }
-        count_launch();
-        LTDI_CUDA_OK(cudaGetLastError());
+        delete big;   /* kernel arguments are copied at launch */
     }
 
     /* tile plan */
