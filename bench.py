@@ -38,10 +38,10 @@ KERNEL_FLOPS = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), cfg2 only; None where no capture exists for the kernel
-TRAFFIC = {"full/tdi": 74.6e6 + 3.4e6}    # profiles/r01c_cfg2.md, tdi_kernel<32,FULL>, cfg2
+TRAFFIC = {"full/tdi": 74.6e6 + 3.8e6}    # profiles/r01e_cfg2.md, tdi_kernel<32,FULL>, cfg2
 # sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only)
-FP64_PIPE_PCT_NCU = {"full/orbit": 53.7, "full/anchor": 11.9, "full/link_full": 63.1, "full/tdi": 64.8,
-                     "lfa/link_lfa": 51.2, "lfa/tdi": 40.6, "hybrid/tdi": 32.0}
+FP64_PIPE_PCT_NCU = {"full/orbit": 53.6, "full/anchor": 12.1, "full/link_full": 62.4, "full/tdi": 65.7,
+                     "lfa/link_lfa": 48.7, "lfa/tdi": 43.4, "hybrid/link_full": 45.8, "hybrid/tdi": 33.3}
 
 WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
