@@ -18,14 +18,19 @@ LIBS = {
 
 
 def build(force=False):
-    for _, (out, defs) in LIBS.items():
-        if (not force and os.path.exists(out)
-                and os.path.getmtime(out) >= os.path.getmtime(SRC)):
-            continue
-        # -ffp-contract=off: no fused multiply-adds the source does not spell out
-        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-ffp-contract=off",
-               "-Wall", "-Wextra", *defs, "-o", out, SRC, "-lm"]
-        subprocess.run(cmd, check=True)
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:   # several processes may build at once
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        for _, (out, defs) in LIBS.items():
+            if (not force and os.path.exists(out)
+                    and os.path.getmtime(out) >= os.path.getmtime(SRC)):
+                continue
+            # -ffp-contract=off: no fused multiply-adds the source does not spell out
+            tmp = f"{out}.{os.getpid()}.tmp"
+            cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-ffp-contract=off",
+                   "-Wall", "-Wextra", *defs, "-o", tmp, SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, out)
     return {k: v[0] for k, v in LIBS.items()}
 
 

@@ -24,13 +24,25 @@ def build(force=False, verbose=False):
     if (not force and os.path.exists(LIB)
             and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)):
         return LIB
-    cmd = [NVCC, *FLAGS, "-o", LIB, *SOURCES]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        sys.stderr.write(r.stdout + r.stderr)
-        raise RuntimeError("nvcc failed building liblisatdi.so")
-    if verbose:
-        print(r.stderr)
+    # several ranks of one node may import the package at once: one builds (into a temporary file, renamed
+    # atomically), the others wait on the lock and find the library up to date
+    import fcntl
+    with open(LIB + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if (not force and os.path.exists(LIB)
+                and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)):
+            return LIB
+        tmp = f"{LIB}.{os.getpid()}.tmp"
+        cmd = [NVCC, *FLAGS, "-o", tmp, *SOURCES]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            if os.path.exists(tmp):
+                os.remove(tmp)
+            raise RuntimeError("nvcc failed building liblisatdi.so")
+        os.replace(tmp, LIB)
+        if verbose:
+            print(r.stderr)
     return LIB
 
 
