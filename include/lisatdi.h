@@ -14,8 +14,10 @@
  *     caller.  The library allocates no device memory and keeps no pointer after a call
  *     returns, except that an ltdi_orbits handle refers to the caller's table buffer.
  *   - Every call is asynchronous on `stream` (a cudaStream_t passed as void*, NULL = the
- *     legacy default stream), except for the copy of the small h_* parameter arrays,
- *     which are consumed before the call returns.
+ *     legacy default stream); the small h_* parameter arrays are consumed before the call
+ *     returns.  ltdi_response_hybrid forks part of its work onto one internal non-blocking
+ *     stream and joins it back with events before it returns control of `stream`'s order:
+ *     to the caller the call is ordered on `stream` like the others.
  *   - Return value: LTDI_OK or a negative LTDI_E* code.  Nothing throws or aborts.
  *   - Time grid: t_n = t0 + n dt, n = 0 .. n-1, shared by all sources of a batch.
  *   - Series layout: a series of source b starts at element b * ld (ld >= n).

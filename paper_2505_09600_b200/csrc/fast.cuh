@@ -664,13 +664,24 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     const int tid = threadIdx.x;
     const int w = (int)p.w;
 
+    /* The hybrid response runs as two concurrent launches over the same 448-sample tiles: the LFA instance (80
+     * registers, four CTAs per SM) takes the tiles that lie entirely before the window (w_Full = 0 on every sample;
+     * it applies w_LFA in its epilogue), the hybrid instance (168 registers, the shared memory of both responses) the
+     * tiles that need the full response, alone or blended.  The other kind of tile exits at once. */
     bool need_full = WHICH == LTDI_RESPONSE_FULL, need_lfa = WHICH == LTDI_RESPONSE_LFA;
+    const bool hybrid_mode = WHICH != LTDI_RESPONSE_FULL && p.which == LTDI_RESPONSE_HYBRID;
     const double *hy = nullptr;
-    if (WHICH == LTDI_RESPONSE_HYBRID) {
+    if (hybrid_mode) {
         hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
         const double t_first = p.t0 + (double)n0 * p.dt, t_last = p.t0 + (double)(n1 - 1) * p.dt;
-        need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0, Eq. (4.5) */
-        need_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0 */
+        const bool tile_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0, Eq. (4.5) */
+        if (WHICH == LTDI_RESPONSE_LFA) {
+            if (tile_full) return;
+        } else {
+            if (!tile_full) return;
+            need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0 */
+            need_full = true;
+        }
     }
 
     /* shared memory (host: tdi_smem_bytes):
@@ -924,6 +935,11 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             X = use_f ? fma(wb, X, x0) : x0;
             Y = use_f ? fma(wb, Y, y0b) : y0b;
             Z = use_f ? fma(wb, Z, z0) : z0;
+        } else if (hybrid_mode) {   /* LFA instance on a tile before the window: w_Full = 0 */
+            hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+            X = wa != 0.0 ? wa * X : 0.0;
+            Y = wa != 0.0 ? wa * Y : 0.0;
+            Z = wa != 0.0 ? wa * Z : 0.0;
         }
         if (!(n >= p.lo && n < p.n - p.hi)) { X = 0.0; Y = 0.0; Z = 0.0; }
         p.A[src_off + n] = (Z - X) * is2;                 /* (2.9a) */
@@ -942,7 +958,10 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
                 if (WHICH == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
-                else if (WHICH == LTDI_RESPONSE_LFA) v = l < 3 ? gl[l * ystride] : 0.0;
+                else if (WHICH == LTDI_RESPONSE_LFA) {
+                    if (!hybrid_mode) v = l < 3 ? gl[l * ystride] : 0.0;
+                    else if (l < 3 && wa != 0.0 && n >= p.m1 + w && n < p.n - p.m1 - w) v = wa * gl[l * ystride]; /* (4.5) */
+                }
                 else if (n >= p.m1 + w && n < p.n - p.m1 - w) { /* (4.5) */
                     if (need_lfa && l < 3 && wa != 0.0) v = wa * gl[l * ystride];
                     if (need_full && wb != 0.0) v = fma(wb, yF[l * yr + iy], v);

@@ -274,6 +274,18 @@ int set_smem(K kernel, size_t smem, int smem_max)
     return LTDI_OK;
 }
 
+/* one non-blocking side stream per process for the second TDI launch of the hybrid (ordering with the caller's
+ * stream goes through events, so calls from several host threads stay correct: they only share the queue) */
+int side_stream(cudaStream_t *out)
+{
+    static std::mutex mu;
+    static cudaStream_t s = nullptr;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!s) LTDI_CUDA_OK(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    *out = s;
+    return LTDI_OK;
+}
+
 // the tuned path: anchors once per call, then link kernel(s) and TDI kernel per chunk of sources
 template <int M>
 int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work, cudaStream_t st,
@@ -325,6 +337,26 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
                               : which == LTDI_RESPONSE_LFA ? tdi_kernel<M, LTDI_RESPONSE_LFA>
                                                            : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
     if ((rc = set_smem(tdi, smem_tdi, smem_max))) return rc;
+    /* hybrid: the tiles before the window go through the LFA instance (same 448-sample tiles) on a side stream, so
+     * that its CTAs (four per SM) run beside those of the hybrid instance (two per SM) */
+    const size_t smem_tdi_lfa = tdi_smem_bytes<M>(LTDI_RESPONSE_LFA, mg.m2, mg.w);
+    static_assert(tdi_tc(LTDI_RESPONSE_LFA) == tdi_tc(LTDI_RESPONSE_HYBRID), "the two launches share the tiling");
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    if (hybrid) {
+        if ((rc = set_smem(tdi_kernel<M, LTDI_RESPONSE_LFA>, smem_tdi_lfa, smem_max))) return rc;
+        if ((rc = side_stream(&side))) return rc;
+        LTDI_CUDA_OK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+        if (cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            cudaEventDestroy(ev_fork);
+            return LTDI_ECUDA;
+        }
+    }
+    struct EventGuard {   /* an event may be destroyed while work that refers to it is still queued */
+        cudaEvent_t a, b;
+        ~EventGuard() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+    } guard{ev_fork, ev_join};
 
     if (orb->d_anc && orb->anc_gen == rp.gen && orb->anc_M == M) {
         /* ltdi_orbits_prepare() has computed the anchors of this (generation, order) for the time grid */
@@ -365,7 +397,16 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         }
         {
             ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
+            if (hybrid) { /* fork: the LFA instance on the side stream, after the link kernels of this chunk */
+                LTDI_CUDA_OK(cudaEventRecord(ev_fork, st));
+                LTDI_CUDA_OK(cudaStreamWaitEvent(side, ev_fork, 0));
+                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)(lay.ntilesC * nb), tdi_threads(LTDI_RESPONSE_LFA),
+                                                   smem_tdi_lfa, side>>>(p);
+                count_launch();
+                LTDI_CUDA_OK(cudaEventRecord(ev_join, side));
+            }
             tdi<<<(unsigned)(lay.ntilesC * nb), tdi_threads(which), smem_tdi, st>>>(p);
+            if (hybrid) LTDI_CUDA_OK(cudaStreamWaitEvent(st, ev_join, 0));   /* join before the scratch is reused */
         }
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
