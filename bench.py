@@ -50,6 +50,7 @@ WORKLOADS = {
     "cfg1f": (1, None, 4096),    # config 1 with the device filled: 4096 sources with fresh angles
     "cfg3": (3, None, None),     # 1 year at dt = 5 s, one source
     "cfg4s": (4, None, 256),     # a 256-source slice of config 4 (the full 4096 x 131072 needs 21 GB of buffers)
+    "cfg4": (4, None, None),     # config 4 at full size: 4096 sources (about 90 GB of device and 35 GB of pinned memory)
     "cfg5s": (5, None, 16),
 }
 
