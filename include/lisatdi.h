@@ -216,11 +216,11 @@ int ltdi_fp64_probe(double *d_out, int blocks, int iters, void *stream, double *
  * (LTDI_RESPONSE_*; the orbit kernel counts under 0), the accumulated device time [ms] and the number of
  * launches since the last ltdi_profile_reset().  Process-global; off by default. */
 enum { LTDI_KERNEL_ORBIT = 0,     /* orbit_delay_kernel: S0 */
-       LTDI_KERNEL_PREP = 1,      /* per-source parameters and source frames: S1 */
+       LTDI_KERNEL_PREP = 1,      /* per-source parameters and source frames: S1 (batch > 32 or generic orders only) */
        LTDI_KERNEL_ANCHOR = 2,    /* Lagrange weight anchors of the TDI delays (orders 9, 31) */
        LTDI_KERNEL_LINK_FULL = 3, /* link_kernel<.,false>: S2 + S3, Eq. (2.5); hybrid: link_hybrid_kernel, both kinds of link tiles in one launch */
        LTDI_KERNEL_LINK_LFA = 4,  /* link_kernel<.,true>: S6, Eq. (B10) */
-       LTDI_KERNEL_TDI = 5,       /* tdi_kernel: S4 + S5, S7, S8 */
+       LTDI_KERNEL_TDI = 5,       /* tdi_kernel: S4 + S5, S7, S8 (hybrid: both concurrent launches) */
        LTDI_KERNEL_GENERIC = 6,   /* response_kernel: fused tile kernel of the other Lagrange orders */
        LTDI_KERNEL_COUNT = 7 };
 int ltdi_profile_enable(int on);
