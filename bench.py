@@ -36,12 +36,20 @@ KERNEL_FLOPS = {
     ("lfa", "tdi"): lambda M: 36 * M,                 # S7: 3 channels x 2 interpolations x 6M
 }
 
+# flops the kernels actually execute per output sample: the TDI kernel shares the weights of a
+# term over an anchor tile and spends 2 DFMA (4 flop) per tap and sample where the model above counts 6 flop of
+# per-sample weights and dot product; the link kernels execute what the model counts
+KERNEL_EXEC_FLOPS = {
+    ("full", "tdi"): lambda M: 3 * 14 * 4 * M,
+    ("lfa", "tdi"): lambda M: 3 * 2 * 4 * M,
+}
+
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), cfg2 only; None where no capture exists for the kernel
-TRAFFIC = {"full/tdi": 74.6e6 + 3.8e6}    # profiles/r01e_cfg2.md, tdi_kernel<32,FULL>, cfg2
+TRAFFIC = {"full/tdi": 74.6e6 + 3.2e6}    # profiles/r01f_cfg2.md, tdi_kernel<32,FULL>, cfg2
 # sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only)
-FP64_PIPE_PCT_NCU = {"full/orbit": 53.6, "full/anchor": 12.1, "full/link_full": 62.4, "full/tdi": 65.7,
-                     "lfa/link_lfa": 48.7, "lfa/tdi": 43.4, "hybrid/link_full": 45.8, "hybrid/tdi": 33.3}
+FP64_PIPE_PCT_NCU = {"full/orbit": 53.6, "full/anchor": 12.0, "full/link_full": 62.4, "full/tdi": 65.8,
+                     "lfa/link_lfa": 48.5, "lfa/tdi": 43.0, "hybrid/link_full": 45.8, "hybrid/tdi": 42.1}
 
 WORKLOADS = {
     # name: (config index, n, batch)  -- None = BASELINE.json size
@@ -343,6 +351,9 @@ def main():
                 if fl is not None:
                     ent["tflops"] = fl(M) * n * batch / (per_step * 1e-3) / 1e12
                     ent["frac_of_dfma_peak"] = ent["tflops"] / peak_tflops
+                    fe = KERNEL_EXEC_FLOPS.get((resp, name))
+                    if fe is not None:   # the same with the flops the kernel really executes
+                        ent["frac_executed_flops"] = fe(M) * n * batch / (per_step * 1e-3) / 1e12 / peak_tflops
                 if name == "orbit":
                     ent["gbs"] = 192.0 * n / (per_step * 1e-3) / 1e9
                     ent["frac_of_hbm_measured"] = ent["gbs"] / peaks["hbm_gbs"] if peaks.get("hbm_gbs") else None
@@ -354,6 +365,10 @@ def main():
         full_ms = float(np.mean(per_call["full"]))
         roofline = {"bound": "alu", "kernel": dom + " (response/kernel; see include/lisatdi.h LTDI_KERNEL_*)",
                     "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                    "frac_executed_flops": kernels[dom].get("frac_executed_flops"),
+                    "note": "achieved = algorithmic flops of the SURVEY 8(d) model (per-sample weights 4M + dot 2M per "
+                            "interpolation); the TDI kernel executes 4M of them (weights shared over an anchor tile), "
+                            "so frac can exceed the FP64 pipe utilisation ncu reports (fp64_pipe_pct_ncu_cfg2) and 1",
                     "traffic": TRAFFIC.get(dom) if args.workload == "cfg2" else None,
                     "fp64_pipe_pct_ncu_cfg2": FP64_PIPE_PCT_NCU,
                     "peak_source": "DFMA chain probe measured in this run (2 flop per DFMA); nominal 148 SM x 64 DFMA/clk",
