@@ -356,3 +356,33 @@ def test_fast_varying_tables_take_the_exact_weight_paths(ltdi, orc80, order):
         ref["floor_XYZ"] = series_floor(ref["XYZ"], ref64["XYZ"], lo, n, hi)
         ref["floor_y"] = series_floor(ref["y"], ref64["y"], lo, n, hi)
         check(out, ref, lo, hi, n)
+
+
+@pytest.mark.parametrize("shared_window", [True, False])
+def test_parameter_slices_of_large_batches(ltdi, orc80, shared_window):
+    """600 sources (two parameter launches of 512 + 88) of 3001 samples: 8 distinct sources tiled 75 times; one
+    hybrid window for all (n_hyb = 1) or one per source; the first copies match the oracle, the replicas the first"""
+    cfg = W.config(4, n=3001, batch=8)
+    hp, hc, ang, metas = W.sources(cfg, list(range(8)))
+    reps, n, dt = 75, cfg["n"], cfg["dt"]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev).repeat(reps, 1), torch.from_numpy(hc).to(dev).repeat(reps, 1)
+    tmid = cfg["orbit"]["t0"] + 0.6 * n * dt
+    mk = lambda i: {"t_hyb": tmid + 40.0 * dt * i, "window_s": 64 * dt, "sigma_s": 1.6 * dt, "taper": i % 2}
+    hyb8 = [mk(0)] * 8 if shared_window else [mk(i) for i in range(8)]
+    hyb_gpu = mk(0) if shared_window else hyb8 * reps
+    out = to_numpy(ltdi.response_hybrid(orb, dhp, dhc, np.tile(ang, (reps, 1)), 20, 31, 2, hyb_gpu, True, True))
+    torch.cuda.synchronize()
+    for k in ("A", "E", "T"):
+        v = out[k].reshape(reps, 8, n)
+        assert np.array_equal(v, np.broadcast_to(v[0], v.shape)), k
+    first = {k: (v[:8] if v.ndim == 2 else v[:, :8]) for k, v in out.items()}
+    from oracle import Oracle
+    ref = orc80.response_hybrid(cfg["orbit"], hp, hc, ang, 20, 31, 2, hyb8)
+    ref64 = Oracle("f64").response_hybrid(cfg["orbit"], hp, hc, ang, 20, 31, 2, hyb8)
+    lo, hi = orc80.margins(cfg["orbit"], 20, 31, 2)
+    ref["floor"] = fp64_floor(ref, ref64, lo, n, hi)
+    ref["floor_XYZ"] = series_floor(ref["XYZ"], ref64["XYZ"], lo, n, hi)
+    ref["floor_y"] = series_floor(ref["y"], ref64["y"], lo, n, hi)
+    check(first, ref, lo, hi, n)
