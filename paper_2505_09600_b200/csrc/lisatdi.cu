@@ -276,15 +276,18 @@ int set_smem(K kernel, size_t smem, int smem_max)
     return LTDI_OK;
 }
 
-/* one non-blocking side stream per process for the second TDI launch of the hybrid (ordering with the caller's
+/* one non-blocking side stream per device for the second TDI launch of the hybrid (ordering with the caller's
  * stream goes through events, so calls from several host threads stay correct: they only share the queue) */
 int side_stream(cudaStream_t *out)
 {
     static std::mutex mu;
-    static cudaStream_t s = nullptr;
+    static cudaStream_t s[64] = {};   /* per device */
+    int dev = 0;
+    LTDI_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return LTDI_EUNSUPPORTED;
     std::lock_guard<std::mutex> lk(mu);
-    if (!s) LTDI_CUDA_OK(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
-    *out = s;
+    if (!s[dev]) LTDI_CUDA_OK(cudaStreamCreateWithFlags(&s[dev], cudaStreamNonBlocking));
+    *out = s[dev];
     return LTDI_OK;
 }
 
