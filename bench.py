@@ -47,7 +47,8 @@ KERNEL_EXEC_FLOPS = {
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), cfg2 only; None where no capture exists for the kernel
 TRAFFIC = {"full/tdi": 74.6e6 + 3.2e6}    # profiles/r01f_cfg2.md, tdi_kernel<32,FULL>, cfg2
-# sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only)
+# sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active of the same capture (context, cfg2 only; with the
+# device filled, cfg4s: link_full 67.6, tdi full 70.6, link_lfa 57.7, tdi LFA 48.1)
 FP64_PIPE_PCT_NCU = {"full/orbit": 53.6, "full/anchor": 12.0, "full/link_full": 62.4, "full/tdi": 65.8,
                      "lfa/link_lfa": 48.5, "lfa/tdi": 43.0, "hybrid/link_full": 45.8, "hybrid/tdi": 42.1}
 
