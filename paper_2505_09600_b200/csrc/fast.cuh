@@ -774,8 +774,9 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             const bool g15 = p.gen == LTDI_GEN_15;
             const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
 #pragma unroll 1
-            for (int l = 0; l < 3; ++l) {
-                for (int run = tid; run < runs; run += FAST_TC_THREADS) {
+            for (int idx = tid; idx < 3 * runs; idx += FAST_TC_THREADS) {   /* (link, run) pairs, evenly over the threads */
+                {
+                    const int l = idx / runs, run = idx - l * runs;
                     const int k0 = run * FD_RUN;
                     const double *x = yL + l * len + k0;   /* x[j] = sample y0 - w + k0 + j */
                     double v[FD_RUN + 4];
