@@ -40,7 +40,7 @@ __host__ __device__ constexpr int tdi_g(int which) { return which == LTDI_RESPON
 __host__ __device__ constexpr int tdi_tc(int which) { return FAST_TC_R * tdi_g(which); }
 __host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(which); }
 #define FAST_TA_THREADS 128
-#define FAST_TA (2 * FAST_TA_THREADS)     /* 384 samples per link tile */
+#define FAST_TA (2 * FAST_TA_THREADS)     /* 256 samples per link tile, three CTAs per SM */
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
 #define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
 #define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
