@@ -375,6 +375,7 @@ def main():
                     "peak_source": "DFMA chain probe measured in this run (2 flop per DFMA); nominal 148 SM x 64 DFMA/clk",
                     "timed_with": "per-kernel CUDA events on the launching stream (ltdi_profile_*), over %d steps "
                                   "identical to the timed ones, run right after them" % args.steps,
+                    "peak_nominal": 148 * 64 * 2 * ((clk or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
                     "hbm_gbs_measured": peaks.get("hbm_gbs"),
                     "kernels": kernels,
                     "per_call_ms": {k: float(np.mean(v)) for k, v in per_call.items()},
