@@ -386,3 +386,41 @@ def test_parameter_slices_of_large_batches(ltdi, orc80, shared_window):
     ref["floor_XYZ"] = series_floor(ref["XYZ"], ref64["XYZ"], lo, n, hi)
     ref["floor_y"] = series_floor(ref["y"], ref64["y"], lo, n, hi)
     check(first, ref, lo, hi, n)
+
+
+def test_decayed_ringdown_tail_keeps_relative_accuracy(ltdi, orc80):
+    """A heavy binary that merges in the middle of the segment: the ring-down decays by hundreds of e-folds, and a
+    window in that tail (1e-100 of the peak) must still match the oracle RELATIVE to its own norm -- the case that
+    catches reduced-precision shortcuts in the interpolation (fp32 underflow) which a whole-series norm hides."""
+    from oracle import Oracle
+    orc64 = Oracle("f64")
+    n, dt = 20001, 10.0
+    orbit = W.orbit_desc(n, dt, W.ORBIT_KEPLERIAN, t0=3.0e6)
+    t = orbit["t0"] + dt * np.arange(n)
+    M_s = 8.0e6 * W.GMSUN_S
+    mc = W.chirp_mass_s(8.0e6, 2.0)
+    rd = {"M_s": M_s, "dt": dt}
+    t_m = t[0] + 0.5 * n * dt
+    hp, hc = W.newtonian_chirp(t, t_m + W._tau_cut(mc, rd), mc, 3.0 * W.GPC_M, 0.3, 1.0, ringdown=rd)
+    hp, hc = hp[None], hc[None]
+    assert 0.0 < np.abs(hp[0, -2000:]).max() < 1e-60 * np.abs(hp).max()      # decayed, but not to zero
+    ang = [(0.4, 2.0, 0.9)]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    hyb = {"t_hyb": t[0] + 0.3 * n * dt, "window_s": 3600.0, "sigma_s": 90.0, "taper": W.TAPER_COSINE}
+    for which in ("full", "hybrid"):
+        if which == "full":
+            out = to_numpy(ltdi.response_full(orb, dhp, dhc, ang, 20, 31))
+            ref, ref64 = (o.response_full(orbit, hp, hc, ang, 20, 31, want=()) for o in (orc80, orc64))
+        else:
+            out = to_numpy(ltdi.response_hybrid(orb, dhp, dhc, ang, 20, 31, 2, hyb))
+            ref, ref64 = (o.response_hybrid(orbit, hp, hc, ang, 20, 31, 2, hyb, want=()) for o in (orc80, orc64))
+        lo, hi = orc80.margins(orbit, 20, 31, 2 if which == "hybrid" else 0)
+        for a, b in ((n - hi - 1500, n - hi), (n - hi - 4000, n - hi - 2500), (int(0.55 * n), int(0.55 * n) + 1500)):
+            for c in "AE":
+                w80, w64, g = ref[c][0, a:b], ref64[c][0, a:b], out[c][0, a:b]
+                nrm = np.linalg.norm(w80)
+                assert nrm > 0
+                err, floor = np.linalg.norm(g - w80) / nrm, np.linalg.norm(w64 - w80) / nrm
+                assert err <= max(TOL, FLOOR_FACTOR * floor), (which, c, (a, b), err, floor)
