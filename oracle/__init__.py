@@ -144,6 +144,18 @@ class Oracle:
         assert rc == 0
         return R, nh, L
 
+    def orbit_tables_split(self, orbit, nb=0, ne=None):
+        """n_l and L_l as hi + lo doubles (the working precision of this build split in two)."""
+        ne = orbit["n"] if ne is None else ne
+        ln = ne - nb
+        nh, nl, Lh, Ll = np.zeros((6, 3, ln)), np.zeros((6, 3, ln)), np.zeros((6, ln)), np.zeros((6, ln))
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_orbit_tables_split(C.byref(d), _ptr(Rt), _ptr(Lt), C.c_int64(nb), C.c_int64(ne),
+                                             _ptr(nh), _ptr(nl), _ptr(Lh), _ptr(Ll))
+        assert rc == 0
+        return nh, nl, Lh, Ll
+
     def antenna(self, orbit, source, n):
         out = np.zeros((6, 3))
         d = self._desc(orbit)

@@ -665,6 +665,34 @@ int orc_orbit_tables(const orc_orbit_desc *d, const double *Rtab, const double *
     return ORC_OK;
 }
 
+/* the same link quantities split as hi + lo doubles (hi = the value rounded to double, lo = the remainder of the
+ * working precision): lets the tests see the digits of n_l and L_l beyond fp64 that the CUDA orbit kernel stores
+ * as low parts.  nhat_hi / nhat_lo [6][3][len], L_hi / L_lo [6][len]. */
+int orc_orbit_tables_split(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, int64_t nb,
+                           int64_t ne, double *nhat_hi, double *nhat_lo, double *L_hi, double *L_lo)
+{
+    if (!d || nb < 0 || ne > d->n || nb > ne || !nhat_hi || !nhat_lo || !L_hi || !L_lo) return ORC_EINVAL;
+    if (d->mode == ORC_ORBIT_TABLES && (!Rtab || !Ltab)) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    const int64_t len = ne - nb;
+#pragma omp parallel for
+    for (int64_t n = nb; n < ne; ++n) {
+        geom_t g;
+        orbit_geometry(&o, n, &g);
+        for (int l = 0; l < 6; ++l) {
+            for (int a = 0; a < 3; ++a) {
+                const double hi = (double)g.nh[l][a];
+                nhat_hi[(l * 3 + a) * len + (n - nb)] = hi;
+                nhat_lo[(l * 3 + a) * len + (n - nb)] = (double)(g.nh[l][a] - (real)hi);
+            }
+            const double hi = (double)g.L[l];
+            L_hi[l * len + (n - nb)] = hi;
+            L_lo[l * len + (n - nb)] = (double)(g.L[l] - (real)hi);
+        }
+    }
+    return ORC_OK;
+}
+
 /* antenna patterns F^+_l, F^x_l and k.n_l of one source at sample n: out[6][3] */
 int orc_antenna(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const orc_source *s,
                 int64_t n, double *out)

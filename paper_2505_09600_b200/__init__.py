@@ -233,7 +233,11 @@ class Orbits:
 
     def rows(self):
         """[24][n] view of the table: R (9 rows), n_l for l = +1,+2,+3 (9 rows), L_l (6 rows)."""
-        return self.tables.view(24, self.stride)[:, :self.n]
+        return self.tables[:24 * self.stride].view(24, self.stride)[:, :self.n]
+
+    def rows_lo(self):
+        """[15][n] float32 view: low parts of the double-double n_l (9 rows) and L_l (6 rows) of the table."""
+        return self.tables[24 * self.stride:].view(torch.float32).view(16, self.stride)[:15, :self.n]
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None

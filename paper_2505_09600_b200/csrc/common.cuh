@@ -23,8 +23,12 @@ struct ltdi_orbits {
     int anc_gen, anc_M;  /* generation and tap count they were computed for */
 };
 
-/* table rows */
+/* table rows: LTDI_TABLE_ROWS rows of doubles, then LTDI_TABLE_LO_ROWS rows of floats (same row stride in elements)
+ * with the low parts of the double-double n_l and L_l (orbit.cuh) */
 enum { ROW_R = 0, ROW_N = 9, ROW_L = 18 };
+enum { LO_N = 0, LO_L = 9 };
+#define LTDI_TABLE_LO_ROWS 16
+#define LTDI_TABLE_BYTES_PER_SAMPLE (LTDI_TABLE_ROWS * 8 + LTDI_TABLE_LO_ROWS * 4)
 
 /* sender / receiver spacecraft (0-based) of link index 0..5 */
 __host__ __device__ __forceinline__ int link_sender(int l)

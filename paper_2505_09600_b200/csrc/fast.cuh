@@ -29,6 +29,7 @@
 // lambda_i g_i  -- 3.4 M flops per weight set instead of 5 M for prefix x suffix over all taps.
 #pragma once
 #include "common.cuh"
+#include "dd.cuh"
 
 #define FAST_TC_R 7                       /* samples per thread in the TDI kernel */
 #define FAST_TCA 448                      /* samples per anchor tile */
@@ -133,11 +134,17 @@ __device__ __noinline__ void lagrange_exact(double eps, double *w)
 // Window W[i] = x[js + i], i = 0 .. M: sample 0 uses W[0..M-1], sample 1 uses W[1..M].  The staged series are
 // split by parity (even samples / odd samples), so that lanes that own consecutive sample PAIRS read
 // consecutive addresses.  W[i] = (i odd ? p1[(i-1)/2] : p0[i/2]).
-template <int H>
+//
+// DIFF: the dot products run over x_k - x_ref (x_ref = the window's centre sample, returned in pref / cref) and the
+// caller adds x_ref back: sum_k w_k x_k = x_ref + sum_k w_k (x_k - x_ref) because the weights sum to 1.  The
+// differences of neighbouring samples are exact or nearly so, and the rounding errors of the weights and of the
+// accumulation now scale with |x_k - x_ref| ~ 16 omega dt |x| instead of |x|: for the low-frequency signals whose
+// LFA response amplifies the noise of y by 1 / (omega dt)^2 (Eq. (B33)) the interpolation stops contributing to it.
+template <int H, bool DIFF>
 __device__ __forceinline__ void interp_pair(double e0, double e1, const double *__restrict__ P0,
                                             const double *__restrict__ P1, const double *__restrict__ C0,
                                             const double *__restrict__ C1, double &ap0, double &ac0, double &ap1,
-                                            double &ac1)
+                                            double &ac1, double &pref, double &cref)
 {
     constexpr int row = (H == 16) ? 1 : 0;
     const double uu0 = (e0 - 0.5) * (e0 - 0.5), uu1 = (e1 - 0.5) * (e1 - 0.5);
@@ -155,6 +162,9 @@ __device__ __forceinline__ void interp_pair(double e0, double e1, const double *
     // centre of the window
 #define W_AT(Q0, Q1, i) (((i) & 1) ? (Q1)[((i) - 1) >> 1] : (Q0)[(i) >> 1])
     double plo = W_AT(P0, P1, H), clo = W_AT(C0, C1, H);
+    pref = DIFF ? plo : 0.0;
+    cref = DIFF ? clo : 0.0;
+    if (DIFF) { plo = 0.0; clo = 0.0; }
     double phi = plo, chi = clo;
     double a_p0 = 0.0, a_c0 = 0.0, a_p1 = 0.0, a_c1 = 0.0;
     double pre0 = 1.0, pre1 = 1.0;
@@ -164,8 +174,8 @@ __device__ __forceinline__ void interp_pair(double e0, double e1, const double *
         const double t0 = G0 * e0, t1 = G1 * e1;
         const double w0p = fma(G0, (double)j, t0), w0m = fma(G0, (double)(j + 1), -t0); /* taps k = j+1, k = -j */
         const double w1p = fma(G1, (double)j, t1), w1m = fma(G1, (double)(j + 1), -t1);
-        const double pl = W_AT(P0, P1, H - 1 - j), ph = W_AT(P0, P1, H + 1 + j);
-        const double cl = W_AT(C0, C1, H - 1 - j), ch = W_AT(C0, C1, H + 1 + j);
+        const double pl = W_AT(P0, P1, H - 1 - j) - pref, ph = W_AT(P0, P1, H + 1 + j) - pref;
+        const double cl = W_AT(C0, C1, H - 1 - j) - cref, ch = W_AT(C0, C1, H + 1 + j) - cref;
         a_p0 = fma(w0m, pl, a_p0);
         a_p0 = fma(w0p, phi, a_p0);
         a_c0 = fma(w0m, cl, a_c0);
@@ -210,10 +220,11 @@ __device__ __noinline__ void interp_single(double eps, const double *he_p, const
 }
 
 // interpolate both series at the two samples m0, m0+1 of a pair with delays d0, d1 [s]
-template <int H>
+template <int H, bool DIFF>
 __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, double d1, int rel0 /* m0 - origin */,
                                               const double *he_p, const double *ho_p, const double *he_c,
-                                              const double *ho_c, double &ap0, double &ac0, double &ap1, double &ac1)
+                                              const double *ho_c, double &ap0, double &ac0, double &ap1, double &ac1,
+                                              double &pref, double &cref)
 {
     int q0, q1;
     double e0, e1;
@@ -227,11 +238,88 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
         const double *P0, *P1, *C0, *C1;
         if (js & 1) { P0 = ho_p + c; P1 = he_p + c + 1; C0 = ho_c + c; C1 = he_c + c + 1; }
         else        { P0 = he_p + c; P1 = ho_p + c;     C0 = he_c + c; C1 = ho_c + c; }
-        interp_pair<H>(e0, e1, P0, P1, C0, C1, ap0, ac0, ap1, ac1);
+        interp_pair<H, DIFF>(e0, e1, P0, P1, C0, C1, ap0, ac0, ap1, ac1, pref, cref);
     } else {
+        pref = 0.0;
+        cref = 0.0;
         interp_single<H>(e0, he_p, ho_p, he_c, ho_c, js, ap0, ac0);
         interp_single<H>(e1, he_p, ho_p, he_c, ho_c, rel0 + 1 - q1 - (H - 1), ap1, ac1);
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// accurate antenna patterns of the LFA links.  F+ = n^T P+ n and Fx = n^T Px n with the symmetric matrices
+//   P+ = (u u^T - v v^T) cos 2psi + (u v^T + v u^T) sin 2psi,   Px = (u v^T + v u^T) cos 2psi - (u u^T - v v^T) sin 2psi
+// of the source (Eqs. (2.2)-(2.4) with G17 written as quadratic forms).  A quadratic form expands EXACTLY about the
+// link vector n_c of the tile centre:  F(n_c + d) = F(n_c) + (2 P n_c) . d + d^T P d.  F(n_c) is evaluated once per
+// tile, link and source in double-double from the dd link vector of the table; d = n - n_c is ~1e-4 over a tile
+// (the constellation turns by 2e-7 rad/s), so the bracket is evaluated in plain fp64 with an absolute error of
+// 1e-20, and F(n) = hi + (lo + bracket) is a double-double value for ~40 flops per sample and link.  (Rounding
+// errors of P itself are constant in time: a smooth relative offset of 1e-16, which no stencil amplifies.)
+// anchor layout (doubles): 0-1 F+_c hi lo, 2-3 Fx_c hi lo, 4-6 g+ = 2 P+ n_c, 7-9 gx, 10-12 n_c hi, 13-15 n_c lo,
+// 16-21 P+ (xx yy zz xy xz yz), 22-27 Px
+// ---------------------------------------------------------------------------------------------
+#define LFA_ANC_DOUBLES 28
+#define LFA_LO_ROWS 12
+
+__device__ __forceinline__ dd quad_form_dd(const double *P, const dd *n, double *g)
+{
+    /* t = P n (dd), g = 2 t (fp64), result n . t */
+    const dd t0 = dd_add(dd_add(dd_mul_d(n[0], P[0]), dd_mul_d(n[1], P[3])), dd_mul_d(n[2], P[4]));
+    const dd t1 = dd_add(dd_add(dd_mul_d(n[0], P[3]), dd_mul_d(n[1], P[1])), dd_mul_d(n[2], P[5]));
+    const dd t2 = dd_add(dd_add(dd_mul_d(n[0], P[4]), dd_mul_d(n[1], P[5])), dd_mul_d(n[2], P[2]));
+    g[0] = 2.0 * t0.hi; g[1] = 2.0 * t1.hi; g[2] = 2.0 * t2.hi;
+    return dd_add(dd_add(dd_mul(n[0], t0), dd_mul(n[1], t1)), dd_mul(n[2], t2));
+}
+
+__device__ __noinline__ void lfa_anchor(const double *fr, const double *tb, const float *tl, int l, int ic, double *s_anc)
+{
+    double *an = s_anc + l * LFA_ANC_DOUBLES;
+    const double *u = fr + 3, *v = fr + 6;
+    const double c2 = fr[9], s2 = fr[10];
+    const int ia[6] = {0, 1, 2, 0, 0, 1}, ib[6] = {0, 1, 2, 1, 2, 2};
+#pragma unroll
+    for (int e = 0; e < 6; ++e) {
+        const double dp = u[ia[e]] * u[ib[e]] - v[ia[e]] * v[ib[e]];     /* (2.4a) as a matrix */
+        const double dc = u[ia[e]] * v[ib[e]] + v[ia[e]] * u[ib[e]];     /* (2.4b) */
+        an[16 + e] = dp * c2 + dc * s2;                                  /* (2.2) + (2.3), G17 */
+        an[22 + e] = dc * c2 - dp * s2;
+    }
+    dd n[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        n[a] = dd_make(tb[(ROW_N + 3 * l + a) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + a) * FAST_TA + ic]);
+        an[10 + a] = n[a].hi;
+        an[13 + a] = n[a].lo;
+    }
+    const dd Fp = quad_form_dd(an + 16, n, an + 4), Fc = quad_form_dd(an + 22, n, an + 7);
+    an[0] = Fp.hi; an[1] = Fp.lo; an[2] = Fc.hi; an[3] = Fc.lo;
+}
+
+// y^LFA of one sample: n = (nx, ny, nz) + (lx, ly, lz), L = L_hi + L_lo, dh/dt numerators (pref + ap), (cref + ac)
+__device__ __forceinline__ double lfa_link_value(const double *an, double nx, double ny, double nz, double lx, double ly,
+                                                 double lz, double L_hi, double L_lo, double kscale, double pref, double ap,
+                                                 double cref, double ac)
+{
+    const double dx = (nx - an[10]) + (lx - an[13]), dy = (ny - an[11]) + (ly - an[14]), dz = (nz - an[12]) + (lz - an[15]);
+    const double *P = an + 16, *Q = an + 22;
+    const double tp0 = fma(P[0], dx, fma(P[3], dy, P[4] * dz)), tp1 = fma(P[3], dx, fma(P[1], dy, P[5] * dz)),
+                 tp2 = fma(P[4], dx, fma(P[5], dy, P[2] * dz));
+    const double tc0 = fma(Q[0], dx, fma(Q[3], dy, Q[4] * dz)), tc1 = fma(Q[3], dx, fma(Q[1], dy, Q[5] * dz)),
+                 tc2 = fma(Q[4], dx, fma(Q[5], dy, Q[2] * dz));
+    const double Fp_lo = an[1] + fma(an[4] + tp0, dx, fma(an[5] + tp1, dy, (an[6] + tp2) * dz));
+    const double Fc_lo = an[3] + fma(an[7] + tc0, dx, fma(an[8] + tc1, dy, (an[9] + tc2) * dz));
+    const double Fp_hi = an[0], Fc_hi = an[2];
+    const dd Sp = two_sum(pref, ap), Sc = two_sum(cref, ac);
+    dd a = two_prod(Fp_hi, Sp.hi), b = two_prod(Fc_hi, Sc.hi);
+    a.lo = fma(Fp_lo, Sp.hi, fma(Fp_hi, Sp.lo, a.lo));
+    b.lo = fma(Fc_lo, Sc.hi, fma(Fc_hi, Sc.lo, b.lo));
+    dd sum = two_sum(a.hi, b.hi);
+    sum.lo += a.lo + b.lo;
+    dd c = two_prod(L_hi, kscale);
+    c.lo = fma(L_lo, kscale, c.lo);
+    const dd y = two_prod(sum.hi, c.hi);
+    return y.hi + fma(sum.lo, c.hi, fma(sum.hi, c.lo, y.lo));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -250,6 +338,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     const int w = LFA ? (int)p.w : 0;
 
     __shared__ double fr[LTDI_FRAME_STRIDE];
+    __shared__ double s_anc[LFA ? 3 * LFA_ANC_DOUBLES : 1];
     if (p.use_small) {
         if (tid == 0) { /* S1, Eq. (2.1) with G1, (2.3): the same device function as the parameter kernel */
             const double *sr = p.small + 3 * (p.b0 + b);
@@ -278,6 +367,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         if (a0 + c < p.stride) cp_async16(tb + r * FAST_TA + c, p.tab + (int64_t)r * p.stride + a0 + c);
         else *reinterpret_cast<double2 *>(tb + r * FAST_TA + c) = make_double2(0.0, 0.0);
     }
+    float *tl = nullptr;   /* LFA: low parts of the dd table entries of the tile */
     if (!LFA) {
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -306,8 +396,20 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                 raw_c[j] = 0.0;
             }
         }
+        /* low parts of n_l (9 rows) and of L_+l (3 rows): float rows LO_N .. LO_L + 2 of the table */
+        tl = reinterpret_cast<float *>(raw_c + nraw);
+        {
+            const float *glo = reinterpret_cast<const float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride);
+            for (int i = tid; i < LFA_LO_ROWS * (FAST_TA / 4); i += FAST_TA_THREADS) {
+                const int r = i / (FAST_TA / 4), c = 4 * (i - r * (FAST_TA / 4));
+                if (a0 + c < p.stride) cp_async16(tl + r * FAST_TA + c, glo + (int64_t)r * p.stride + a0 + c);
+                else *reinterpret_cast<float4 *>(tl + r * FAST_TA + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+        }
         cp_async_wait_all();
         __syncthreads();
+        /* tile anchors of the antenna patterns (threads of the last warp, beside the stencil pass below) */
+        if (tid >= FAST_TA_THREADS - 3) lfa_anchor(fr, tb, tl, FAST_TA_THREADS - 1 - tid, (int)min((int64_t)(FAST_TA / 2), p.n - 1 - a0), s_anc);
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
             double vp = 0.0, vc = 0.0;
@@ -391,8 +493,8 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                 d0 = L.x + k0;                                           /* (2.6a) */
                 d1 = L.y + k1;
             }
-            double ap0, ac0, ap1, ac1;
-            interp_delays<H>(p, d0, d1, rel0, he_p, ho_p, he_c, ho_c, ap0, ac0, ap1, ac1);
+            double ap0, ac0, ap1, ac1, pref, cref;
+            interp_delays<H, false>(p, d0, d1, rel0, he_p, ho_p, he_c, ho_c, ap0, ac0, ap1, ac1, pref, cref);
             if (s == 0) {
                 rp0 = ap0; rc0 = ac0; rp1 = ap1; rc1 = ac1;
             } else {
@@ -405,7 +507,12 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             }
         }
     } else {
-        const double iden = p.inv_fd1;   /* the stencil denominator as a factor (one rounding, like the division) */
+        /* (B10): y = -(L_l / 2) (F+ dh+/dt + Fx dhx/dt) with every factor that multiplies the result carried as a
+         * double-double pair and one rounding at the end (dd.cuh: Eq. (B33) amplifies white noise of y by
+         * 2.45 / (omega dt)^2).  The stencil denominator 1 / (2 dt) is a constant factor (its rounding is a constant
+         * relative offset of 1e-16, not noise). */
+        const double kscale = -0.5 * p.inv_fd1;
+        const float *tlo = tl + 2 * tid;
 #pragma unroll 1
         for (int l = 0; l < 3; ++l) {
             const int s = link_sender(l), r = link_receiver(l);
@@ -413,13 +520,19 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             kdotR(s, ks0, ks1);
             kdotR(r, kr0, kr1);
             const double2 L = row2(ROW_L + l);
-            double ap0, ac0, ap1, ac1;
-            interp_delays<H>(p, 0.5 * L.x + 0.5 * (ks0 + kr0), 0.5 * L.y + 0.5 * (ks1 + kr1), rel0, he_p, ho_p, he_c,
-                             ho_c, ap0, ac0, ap1, ac1);                                    /* (B1) */
-            double Fp0, Fc0, kn0, Fp1, Fc1, kn1;
-            patterns(l, Fp0, Fc0, kn0, Fp1, Fc1, kn1);
-            const double y0 = -(0.5 * L.x) * (Fp0 * (ap0 * iden) + Fc0 * (ac0 * iden));    /* (B10) */
-            const double y1 = -(0.5 * L.y) * (Fp1 * (ap1 * iden) + Fc1 * (ac1 * iden));
+            double ap0, ac0, ap1, ac1, pref, cref;
+            interp_delays<H, true>(p, 0.5 * L.x + 0.5 * (ks0 + kr0), 0.5 * L.y + 0.5 * (ks1 + kr1), rel0, he_p, ho_p,
+                                   he_c, ho_c, ap0, ac0, ap1, ac1, pref, cref);               /* (B1) */
+            const double *an = s_anc + l * LFA_ANC_DOUBLES;
+            const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
+            const float2 lx = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l) * FAST_TA);
+            const float2 ly = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 1) * FAST_TA);
+            const float2 lz = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 2) * FAST_TA);
+            const float2 lL = *reinterpret_cast<const float2 *>(tlo + (LO_L + l) * FAST_TA);
+            const double y0 = lfa_link_value(an, nx.x, ny.x, nz.x, (double)lx.x, (double)ly.x, (double)lz.x, L.x,
+                                             (double)lL.x, kscale, pref, ap0, cref, ac0);
+            const double y1 = lfa_link_value(an, nx.y, ny.y, nz.y, (double)lx.y, (double)ly.y, (double)lz.y, L.y,
+                                             (double)lL.y, kscale, pref, ap1, cref, ac1);
             *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
         }
     }

@@ -142,20 +142,44 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
 {
     if (!desc_ok(desc) || !d_tables || !out) return LTDI_EINVAL;
     const int64_t stride = table_stride(desc->n);
-    if (bytes < (size_t)stride * LTDI_TABLE_ROWS * sizeof(double)) return LTDI_EWORKSPACE;
+    if (bytes < (size_t)stride * LTDI_TABLE_BYTES_PER_SAMPLE) return LTDI_EWORKSPACE;
     if ((uintptr_t)d_tables % 16) return LTDI_EINVAL;
     OrbitKernelParams p;
+    std::memset(&p, 0, sizeof p);
     p.t0 = desc->t0; p.dt = desc->dt; p.n = desc->n; p.stride = stride;
     p.arm_m = desc->arm_m; p.R_m = desc->R_m;
-    p.omega = 2.0 * 3.14159265358979323846 / desc->period_s;
-    p.alpha0 = desc->alpha0; p.rot0 = desc->rot0; p.mode = desc->mode;
-    for (int i = 0; i < 3; ++i) { /* beta_i = 2 pi (i - 1) / 3 + rot0: constants of the launch */
-        const double beta = 2.0 * 3.14159265358979323846 * (double)i / 3.0 + desc->rot0;
-        p.sb[i] = std::sin(beta);
-        p.cb[i] = std::cos(beta);
+    /* constants of the launch in long double, handed to the kernel as double-double pairs */
+    auto split = [](long double v) { dd r; r.hi = (double)v; r.lo = (double)(v - (long double)r.hi); return r; };
+    const long double pi_l = 3.14159265358979323846264338327950288L;
+    const long double omega_l = 2.0L * pi_l / (long double)desc->period_s;
+    p.omega = (double)omega_l; p.omega_dd = split(omega_l);
+    p.alpha0 = desc->alpha0; p.mode = desc->mode;
+    long double sb_l[3], cb_l[3];
+    for (int i = 0; i < 3; ++i) { /* beta_i = 2 pi (i - 1) / 3 + rot0 */
+        const long double beta = 2.0L * pi_l * (long double)i / 3.0L + (long double)desc->rot0;
+        sb_l[i] = sinl(beta); cb_l[i] = cosl(beta);
+        p.sb[i] = split(sb_l[i]); p.cb[i] = split(cb_l[i]);
+    }
+    for (int l = 0; l < 3; ++l) {
+        const int s = link_sender(l), r = link_receiver(l);
+        p.dsb[l] = split(sb_l[r] - sb_l[s]); p.dcb[l] = split(cb_l[r] - cb_l[s]);
+    }
+    {
+        const long double L = desc->arm_m, R = desc->R_m;
+        const long double e = L / (2.0L * sqrtl(3.0L) * R);
+        p.half_eR = split(0.5L * e * R);
+        p.s3_eR = split(sqrtl(3.0L) * e * R);
+        p.inv_c = split(1.0L / (long double)LTDI_C_LIGHT);
+        p.L_static = split(L / (long double)LTDI_C_LIGHT);
+        long double f = 1.0L;   /* (-1)^m / (2m+1)! and (-1)^m / (2m)! */
+        for (int m = 0; m < 12; ++m) {
+            if (m > 0) f *= (long double)(2 * m - 1) * (long double)(2 * m);
+            p.cos_c[m] = split(((m & 1) ? -1.0L : 1.0L) / f);
+            if (m < 11) p.sin_c[m] = split(((m & 1) ? -1.0L : 1.0L) / (f * (long double)(2 * m + 1)));
+        }
     }
     p.R_in = d_R; p.L_in = d_L; p.tab = (double *)d_tables;
-    const int threads = 256;
+    const int threads = 128;
     const int64_t blocks = (desc->n + threads - 1) / threads;
     {
         ProfScope ps(LTDI_KERNEL_ORBIT, (cudaStream_t)stream);
@@ -327,7 +351,8 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
     const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
     const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
     const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double) +
-                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double); /* + raw strain */
+                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double) + /* + raw strain */
+                                 (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float);                            /* + low parts */
     const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
     int rc;
     const bool hybrid = which == LTDI_RESPONSE_HYBRID;
@@ -636,7 +661,7 @@ int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, co
 int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes)
 {
     if (!desc_ok(desc) || !bytes) return LTDI_EINVAL;
-    *bytes = (size_t)table_stride(desc->n) * LTDI_TABLE_ROWS * sizeof(double);
+    *bytes = (size_t)table_stride(desc->n) * LTDI_TABLE_BYTES_PER_SAMPLE;
     return LTDI_OK;
 }
 

@@ -1,87 +1,164 @@
 // orbit.cuh -- S0: orbit / delay kernel (first-order Keplerian orbits, G5-G7).
 //
-// One thread per time sample writes the 24 table rows: spacecraft positions R_i(t_n) [m],
-// link unit vectors n_l(t_n) for l = +1,+2,+3 (sender -> receiver; n_-l = -n_l) and the
-// six light travel times L_l(t_n) [s].  HBM-bound: 192 B written per sample, nothing read
-// (analytic modes) or 120 B read (tables mode).
+// One thread per time sample writes the table rows of its sample: spacecraft positions R_i(t_n) [m], link unit
+// vectors n_l(t_n) for l = +1,+2,+3 (sender -> receiver; n_-l = -n_l) and the six light travel times
+// L_l(t_n) [s] as doubles (24 rows), plus the LOW PARTS of n_l and L_l as floats (15 rows): n_l and L_l are
+// computed in double-double arithmetic (dd.cuh) and stored as hi + lo.
+//
+// Why double-double.  n_l = (R_r - R_s) / |R_r - R_s| from positions rounded to fp64 (1.5e11 m +- 2e-5 m, arms of
+// 2.5e9 m) carries white noise of 1e-14; the gen-2.0 LFA, Eq. (B33), differences the link series twice and
+// amplifies it to 4e-10 in X at config 3 (measured: the oracle's own double build sits there).  Here the arm
+// vectors are formed analytically -- the R cos(alpha) terms of the two spacecraft cancel in exact arithmetic, what
+// remains is O(e R) = O(L) -- from sin / cos of the orbital phase evaluated in dd (phase alpha = Omega t_n + alpha0
+// in dd: t_n = t0 + n dt rounded to fp64 alone would move n_l by 7e-16 at t = 1 yr).  The positions themselves enter
+// the response only through k.R / c (needed to 1e-13 s): they are stored as correctly rounded doubles.
+//
+// Cost: about 1.2 kflop per sample (dd sincos 0.3, rotations 0.3, three links 0.6) for 252 B written: the kernel
+// is bound by the FP64 pipe, not by HBM, and runs once per time grid.
 #pragma once
 #include "common.cuh"
+#include "dd.cuh"
 
 struct OrbitKernelParams {
     double t0, dt;
     int64_t n, stride;
-    double arm_m, R_m, omega, alpha0, rot0;
-    double sb[3], cb[3]; /* sin, cos of beta_i */
+    double arm_m, R_m, omega, alpha0;
+    dd omega_dd;           /* 2 pi / period */
+    dd sb[3], cb[3];       /* sin, cos of beta_i = 2 pi i / 3 + rot0 */
+    dd dsb[3], dcb[3];     /* link l (s -> r): sin beta_r - sin beta_s, cos beta_r - cos beta_s */
+    dd half_eR, s3_eR;     /* e R / 2 and sqrt(3) e R [m], e = L / (2 sqrt(3) R) */
+    dd inv_c;              /* 1 / c */
+    dd L_static;           /* arm / c */
+    dd sin_c[11], cos_c[12]; /* (-1)^m / (2m+1)!, (-1)^m / (2m)! */
     int mode;
     const double *R_in; /* tables mode: [3][3][n] */
     const double *L_in; /* tables mode: [6][n] */
     double *tab;
 };
 
-__global__ void __launch_bounds__(256) orbit_delay_kernel(OrbitKernelParams p)
+// sin and cos of a dd angle, absolute error < 1e-30 for |a| < 1e5: reduction by multiples of pi / 2 (three-part
+// constant), Taylor series on |r| <= pi / 4 -- the high-order tail (terms below 1e-11) in plain fp64
+__device__ __forceinline__ void sincos_dd(dd a, const OrbitKernelParams &p, dd &s, dd &c)
+{
+    const double P1 = 1.570796326794896558e+00, P2 = 6.123233995736766036e-17, P3 = -1.497384904859169833e-33;
+    const double k = rint(a.hi * 0.63661977236758134308);
+    dd r = dd_sub(a, two_prod(k, P1));
+    r = dd_sub(r, two_prod(k, P2));
+    r = dd_add_d(r, -k * P3);
+    const dd r2 = dd_mul(r, r);
+    /* sin r / r and cos r as polynomials in r^2 */
+    double ts = p.sin_c[10].hi, tc = p.cos_c[11].hi;
+#pragma unroll
+    for (int m = 9; m >= 6; --m) ts = fma(ts, r2.hi, p.sin_c[m].hi);
+#pragma unroll
+    for (int m = 10; m >= 6; --m) tc = fma(tc, r2.hi, p.cos_c[m].hi);
+    dd ps = dd_make(ts, 0.0), pc = dd_make(tc, 0.0);
+#pragma unroll
+    for (int m = 5; m >= 0; --m) {
+        ps = dd_add(dd_mul(ps, r2), p.sin_c[m]);
+        pc = dd_add(dd_mul(pc, r2), p.cos_c[m]);
+    }
+    ps = dd_mul(ps, r);
+    const int q = ((int)k) & 3;
+    switch (q) {
+    case 0: s = ps; c = pc; break;
+    case 1: s = pc; c = dd_neg(ps); break;
+    case 2: s = dd_neg(ps); c = dd_neg(pc); break;
+    default: s = dd_neg(pc); c = ps; break;
+    }
+}
+
+__global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant__ OrbitKernelParams p)
 {
     const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= p.n) return;
     double R[3][3], V[3][3];
+    dd dv[3][3];   /* arm vectors R_r - R_s of links +1, +2, +3 [m] */
     if (p.mode == LTDI_ORBIT_TABLES) {
 #pragma unroll
         for (int i = 0; i < 9; ++i) {
             R[i / 3][i % 3] = p.R_in[(int64_t)i * p.n + n];
             V[i / 3][i % 3] = 0.0;
         }
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            const int s = link_sender(l), r = link_receiver(l);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) dv[l][a] = two_sum(R[r][a], -R[s][a]);
+        }
     } else {
-        // alpha(t) = Omega t + alpha0; spacecraft i: beta_i = 2 pi (i-1)/3 + rot0.  Positions to first
-        // order in the eccentricity e = L / (2 sqrt(3) R): a rigid triangle of side L, cartwheeling at 1 AU.
-        const double t = p.t0 + (double)n * p.dt;
-        const double alpha = p.omega * t + p.alpha0;
-        const double ecc = p.arm_m / (2.0 * sqrt(3.0) * p.R_m);
-        const double eR = ecc * p.R_m;
-        double sa, ca;
-        sincos(alpha, &sa, &ca);
-        /* one sincos per sample: the angles 2 alpha - beta_i and alpha - beta_i by the addition theorems
-         * (a few ulp of 1 on terms that are e R = 7e8 m: 1e-6 m, far inside the table tolerance) */
-        const double s2a = 2.0 * sa * ca, c2a = (ca - sa) * (ca + sa);
+        // alpha(t) = Omega t + alpha0; spacecraft i: beta_i = 2 pi (i-1)/3 + rot0.  Positions to first order in the
+        // eccentricity e = L / (2 sqrt(3) R): a rigid triangle of side L, cartwheeling at 1 AU.
+        dd t = two_prod((double)n, p.dt);
+        t = dd_add_d(t, p.t0);
+        const dd alpha = dd_add_d(dd_mul(p.omega_dd, t), p.alpha0);
+        dd sa, ca;
+        sincos_dd(alpha, p, sa, ca);
+        dd s2a = dd_mul(sa, ca);
+        s2a.hi *= 2.0; s2a.lo *= 2.0;
+        const dd c2a = dd_mul(dd_sub(ca, sa), dd_add(ca, sa));
+        dd c2[3], s2[3], c1[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            const double sb = p.sb[i], cb = p.cb[i];
-            const double s2 = s2a * cb - c2a * sb, c2 = c2a * cb + s2a * sb;
-            const double s1 = sa * cb - ca * sb, c1 = ca * cb + sa * sb;
-            R[i][0] = p.R_m * ca + 0.5 * eR * (c2 - 3.0 * cb);
-            R[i][1] = p.R_m * sa + 0.5 * eR * (s2 - 3.0 * sb);
-            R[i][2] = -sqrt(3.0) * eR * c1;
-            V[i][0] = -p.R_m * p.omega * sa - eR * p.omega * s2;
-            V[i][1] = p.R_m * p.omega * ca + eR * p.omega * c2;
-            V[i][2] = sqrt(3.0) * eR * p.omega * s1;
+            /* 2 alpha - beta_i and alpha - beta_i by the addition theorems */
+            c2[i] = dd_add(dd_mul(c2a, p.cb[i]), dd_mul(s2a, p.sb[i]));
+            s2[i] = dd_sub(dd_mul(s2a, p.cb[i]), dd_mul(c2a, p.sb[i]));
+            c1[i] = dd_add(dd_mul(ca, p.cb[i]), dd_mul(sa, p.sb[i]));
+            const double s1 = sa.hi * p.cb[i].hi - ca.hi * p.sb[i].hi;
+            const double eR = 2.0 * p.half_eR.hi;
+            R[i][0] = dd_to_double(dd_add_d(dd_mul_d(ca, p.R_m), p.half_eR.hi * (c2[i].hi - 3.0 * p.cb[i].hi)));
+            R[i][1] = dd_to_double(dd_add_d(dd_mul_d(sa, p.R_m), p.half_eR.hi * (s2[i].hi - 3.0 * p.sb[i].hi)));
+            R[i][2] = -p.s3_eR.hi * c1[i].hi;
+            V[i][0] = -p.R_m * p.omega * sa.hi - eR * p.omega * s2[i].hi;
+            V[i][1] = p.R_m * p.omega * ca.hi + eR * p.omega * c2[i].hi;
+            V[i][2] = p.s3_eR.hi * p.omega * s1;
+        }
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            const int s = link_sender(l), r = link_receiver(l);
+            /* R_r - R_s: the R cos(alpha), R sin(alpha) terms cancel identically */
+            dd three_c = p.dcb[l], three_s = p.dsb[l];
+            three_c = dd_mul_d(three_c, 3.0);
+            three_s = dd_mul_d(three_s, 3.0);
+            dv[l][0] = dd_mul(p.half_eR, dd_sub(dd_sub(c2[r], c2[s]), three_c));
+            dv[l][1] = dd_mul(p.half_eR, dd_sub(dd_sub(s2[r], s2[s]), three_s));
+            dv[l][2] = dd_neg(dd_mul(p.s3_eR, dd_sub(c1[r], c1[s])));
         }
     }
     double *out = p.tab + n;
+    float *lo = reinterpret_cast<float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride) + n;
 #pragma unroll
     for (int i = 0; i < 9; ++i) out[(int64_t)(ROW_R + i) * p.stride] = R[i / 3][i % 3];
-    const double inv_c = 1.0 / LTDI_C_LIGHT;
 #pragma unroll
     for (int l = 0; l < 3; ++l) {
         const int s = link_sender(l), r = link_receiver(l);
-        const double dx = R[r][0] - R[s][0], dy = R[r][1] - R[s][1], dz = R[r][2] - R[s][2];
-        const double len = sqrt(dx * dx + dy * dy + dz * dz);
-        const double nx = dx / len, ny = dy / len, nz = dz / len;
-        out[(int64_t)(ROW_N + 3 * l + 0) * p.stride] = nx;
-        out[(int64_t)(ROW_N + 3 * l + 1) * p.stride] = ny;
-        out[(int64_t)(ROW_N + 3 * l + 2) * p.stride] = nz;
-        double Lp, Lm; /* link +l (s -> r) and -l (r -> s) */
+        const dd len2 = dd_add(dd_add(dd_mul(dv[l][0], dv[l][0]), dd_mul(dv[l][1], dv[l][1])), dd_mul(dv[l][2], dv[l][2]));
+        const dd len = dd_sqrt(len2);
+        const dd inv = dd_div(dd_make(1.0, 0.0), len);
+        dd nh[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            nh[a] = dd_mul(dv[l][a], inv);
+            out[(int64_t)(ROW_N + 3 * l + a) * p.stride] = nh[a].hi;
+            lo[(int64_t)(LO_N + 3 * l + a) * p.stride] = (float)nh[a].lo;
+        }
+        dd Lp, Lm; /* link +l (s -> r) and -l (r -> s) */
         if (p.mode == LTDI_ORBIT_STATIC_EQUALARM) {
-            Lp = Lm = p.arm_m / LTDI_C_LIGHT;
+            Lp = Lm = p.L_static;
         } else if (p.mode == LTDI_ORBIT_KEPLERIAN) {
             // first-order light time |d|/c (1 + n.V_sender / c): L_l != L_-l (Eq. B22)
-            const double nvs = nx * V[s][0] + ny * V[s][1] + nz * V[s][2];
-            const double nvr = -(nx * V[r][0] + ny * V[r][1] + nz * V[r][2]);
-            Lp = (len / LTDI_C_LIGHT) * (1.0 + nvs / LTDI_C_LIGHT);
-            Lm = (len / LTDI_C_LIGHT) * (1.0 + nvr / LTDI_C_LIGHT);
+            const double nvs = nh[0].hi * V[s][0] + nh[1].hi * V[s][1] + nh[2].hi * V[s][2];
+            const double nvr = -(nh[0].hi * V[r][0] + nh[1].hi * V[r][1] + nh[2].hi * V[r][2]);
+            const dd lc = dd_mul(len, p.inv_c);
+            Lp = dd_mul(lc, two_sum(1.0, nvs * p.inv_c.hi));
+            Lm = dd_mul(lc, two_sum(1.0, nvr * p.inv_c.hi));
         } else {
-            Lp = p.L_in[(int64_t)l * p.n + n];
-            Lm = p.L_in[(int64_t)(l + 3) * p.n + n];
+            Lp = dd_make(p.L_in[(int64_t)l * p.n + n], 0.0);
+            Lm = dd_make(p.L_in[(int64_t)(l + 3) * p.n + n], 0.0);
         }
-        out[(int64_t)(ROW_L + l) * p.stride] = Lp;
-        out[(int64_t)(ROW_L + 3 + l) * p.stride] = Lm;
+        out[(int64_t)(ROW_L + l) * p.stride] = Lp.hi;
+        out[(int64_t)(ROW_L + 3 + l) * p.stride] = Lm.hi;
+        lo[(int64_t)(LO_L + l) * p.stride] = (float)Lp.lo;
+        lo[(int64_t)(LO_L + 3 + l) * p.stride] = (float)Lm.lo;
     }
-    (void)inv_c;
 }

@@ -1,5 +1,8 @@
 """Helpers of the GPU parity tests: run the CUDA path and the long-double oracle on the same seeded
 inputs and compare channel by channel (relative L2 over the non-margin samples)."""
+import json
+import os
+
 import numpy as np
 
 import workloads as W
@@ -72,3 +75,19 @@ def hybrid_params(metas, hyb_time, taper=W.TAPER_COSINE, dt=None):
 
 def to_numpy(out):
     return {k: (None if v is None else v.detach().cpu().numpy()) for k, v in out.items()}
+
+
+REPORT = os.path.join(os.environ.get("GRAFT_REPO_ROOT", os.path.dirname(os.path.dirname(os.path.abspath(__file__)))),
+                      "gpurun_out", "parity_report.jsonl")
+
+
+def record(**row):
+    """append one parity measurement (achieved error, fp64 floor of the oracle's double build, bar) to
+    gpurun_out/parity_report.jsonl; the committed summary under profiles/ is made from this file"""
+    row = {"test": os.environ.get("PYTEST_CURRENT_TEST", "").split(" ")[0], **row}
+    try:
+        os.makedirs(os.path.dirname(REPORT), exist_ok=True)
+        with open(REPORT, "a") as f:
+            f.write(json.dumps(row, default=float) + "\n")
+    except OSError:
+        pass

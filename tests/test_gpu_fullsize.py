@@ -10,7 +10,7 @@ import pytest
 import torch
 
 import workloads as W
-from parity_util import FLOOR_FACTOR, NEAR_NULL, TOL, hybrid_params
+from parity_util import FLOOR_FACTOR, NEAR_NULL, TOL, hybrid_params, record
 
 pytestmark = pytest.mark.gpu
 
@@ -48,6 +48,9 @@ def compare_window(got, ref80, ref64, nb, ne, lo, n, hi, label):
         err = np.linalg.norm(g[:, a - nb:b - nb] - w80) / den
         floor = np.linalg.norm(w64 - w80) / den
         bar = max(TOL, FLOOR_FACTOR * floor)
+        record(label=[str(x) for x in label], series=c, window=[int(nb), int(ne)], err=float(err),
+               err_vs_top=float(np.linalg.norm(g[:, a - nb:b - nb] - w80) / top), floor=float(floor), bar=float(bar),
+               near_null=bool(near_null))
         assert err <= bar, (label, c, (nb, ne), err, bar)
 
 

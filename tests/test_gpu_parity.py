@@ -6,8 +6,8 @@ import pytest
 import torch
 
 import workloads as W
-from parity_util import (FLOOR_FACTOR, TOL, channel_errors, fp64_floor, hybrid_params, series_errors, series_floor,
-                         to_numpy)
+from parity_util import (FLOOR_FACTOR, TOL, channel_errors, fp64_floor, hybrid_params, record, series_errors,
+                         series_floor, to_numpy)
 
 pytestmark = pytest.mark.gpu
 
@@ -71,12 +71,16 @@ def check(out, ref, lo, hi, n, tol=TOL):
     # where that is larger (T = (X+Y+Z)/sqrt 3 cancels; the gen-2.0 LFA second
     # difference amplifies the rounding of y by 2.4 / (omega dt)^2)
     errs = channel_errors(out, ref, lo, n, hi)
+    top = max(np.linalg.norm(ref[c][..., lo:n - hi]) for c in "AET")
     for c, (e, near_null) in errs.items():
         bar = tol if near_null else max(tol, FLOOR_FACTOR * ref["floor"][c])
+        e_top = float(np.linalg.norm((out[c] - ref[c])[..., lo:n - hi]) / top) if top > 0 else 0.0
+        record(series=c, err=e, err_vs_top=e_top, floor=ref["floor"][c], bar=bar, near_null=bool(near_null))
         assert e <= bar, (c, e, bar, "near-null" if near_null else "")
     for name in ("XYZ", "y"):
         for i, e in enumerate(series_errors(out[name], ref[name], lo, n, hi)):
             bar = max(tol, FLOOR_FACTOR * ref["floor_" + name][i])
+            record(series="%s%d" % (name, i), err=e, floor=ref["floor_" + name][i], bar=bar)
             assert e <= bar, (name, i, e, bar)
     return errs
 
