@@ -220,9 +220,11 @@ enum { LTDI_KERNEL_ORBIT = 0,     /* orbit_delay_kernel: S0 */
        LTDI_KERNEL_ANCHOR = 2,    /* Lagrange weight anchors of the TDI delays (orders 9, 31) */
        LTDI_KERNEL_LINK_FULL = 3, /* link_kernel<.,false>: S2 + S3, Eq. (2.5); hybrid: link_hybrid_kernel, both kinds of link tiles in one launch */
        LTDI_KERNEL_LINK_LFA = 4,  /* link_kernel<.,true>: S6, Eq. (B10) */
-       LTDI_KERNEL_TDI = 5,       /* tdi_kernel: S4 + S5, S7, S8 (hybrid: both concurrent launches) */
+       LTDI_KERNEL_TDI = 5,       /* tdi_kernel: S4 + S5 (hybrid: the tiles after the window and, blended, the tiles it touches: S8) */
        LTDI_KERNEL_GENERIC = 6,   /* response_kernel: fused tile kernel of the other Lagrange orders */
-       LTDI_KERNEL_COUNT = 7 };
+       LTDI_KERNEL_TDI_LFA = 7,   /* tdi_kernel, LFA instance: S7 (hybrid: the blocks before the window) */
+       LTDI_KERNEL_PLAN = 8,      /* hybrid_plan_kernel: compact tile lists of the hybrid, S8 */
+       LTDI_KERNEL_COUNT = 9 };
 int ltdi_profile_enable(int on);
 int ltdi_profile_read(int kernel, int which, double *total_ms, int64_t *launches);
 int ltdi_profile_reset(void);

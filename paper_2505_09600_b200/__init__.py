@@ -158,7 +158,7 @@ def launch_count():
     return lib().ltdi_launch_count()
 
 
-KERNELS = ("orbit", "prep", "anchor", "link_full", "link_lfa", "tdi", "generic")   # LTDI_KERNEL_* order
+KERNELS = ("orbit", "prep", "anchor", "link_full", "link_lfa", "tdi", "generic", "tdi_lfa", "plan")   # LTDI_KERNEL_* order
 
 
 def profile_enable(on=True):

@@ -43,7 +43,8 @@ __host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(whic
 #define FAST_TA_THREADS 128
 #define FAST_TA (2 * FAST_TA_THREADS)     /* 256 samples per link tile, three CTAs per SM */
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
-#define FAST_NA_LFA 6                     /* 3 channels x 2 delays */
+#define FAST_NA_LFA 12                    /* 2 generations x 3 channels x 2 delays (gen 1.5 first) */
+#define FAST_NA_LFA_GEN 6                 /* those of one generation */
 #define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
 #define FAST_DMAX 5.0e-7                  /* |eps_n - eps_c| bound for the first-order weights */
 /* one anchor = [M] double2 {w_k, w_k'}, in doubles */
@@ -68,6 +69,7 @@ struct FastParams {
     int64_t n_hyb;
     int which, gen, fd;
     int64_t m1, m2, w, lo, hi;
+    int64_t m2_15, m2_20;    /* anchor kernel: backward TDI reach of either generation (the anchors serve both) */
     int qmax;
     double *yF, *yL;         /* scratch link series [6][batch][lds], [3][batch][lds] */
     int64_t lds;
@@ -76,7 +78,25 @@ struct FastParams {
     const double *anc;       /* [anchor tiles][FAST_NA][M][2] */
     const double *anc_hdr;   /* [anchor tiles][FAST_NA][4]: d_c [s], q, eps_c, valid */
     int64_t ntilesA, ntilesC;
+    /* hybrid: compact work lists built by hybrid_plan_kernel (x = source of the chunk, y = tile); a launch runs exactly
+     * the tiles of its class.  work == nullptr: every tile of every source (id = tile * batch + source). */
+    const int2 *work;
+    int64_t nwork;           /* items of this launch */
+    int64_t nwork_full;      /* link_hybrid_kernel: the first nwork_full items are full-link tiles, the rest LFA-link tiles */
 };
+
+/* item id -> (source of the chunk, tile) */
+__device__ __forceinline__ void work_item(const FastParams &p, int64_t id, int64_t &b, int64_t &tile)
+{
+    if (p.work) {
+        const int2 it = p.work[id];
+        b = it.x;
+        tile = it.y;
+    } else {
+        b = id % p.batch;
+        tile = id / p.batch;
+    }
+}
 
 // ---------------------------------------------------------------------------------------------
 // helpers
@@ -329,10 +349,8 @@ template <int H, bool LFA>
 __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
 {
     extern __shared__ double smem[];
-    const int64_t b = bid % p.batch;
-    int64_t tile = bid / p.batch;
-    /* hybrid: the full links live at the end of the series; schedule those tiles first (no long tail) */
-    if (!LFA && p.which == LTDI_RESPONSE_HYBRID) tile = p.ntilesA - 1 - tile;
+    int64_t b, tile;
+    work_item(p, bid, b, tile);
     const int64_t a0 = tile * FAST_TA;               /* first sample of the tile (even) */
     const int tid = threadIdx.x;
     const int w = LFA ? (int)p.w : 0;
@@ -345,14 +363,6 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             source_frame_one(sr[0], sr[1], sr[2], fr);
         }
     } else if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
-
-    if (p.which == LTDI_RESPONSE_HYBRID) { /* skip tiles whose links the hybrid never uses */
-        const double *hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
-        const double halo = (double)(p.m2 + 2 * p.w + H + 2) * p.dt;
-        const double t_first = p.t0 + (double)a0 * p.dt, t_last = p.t0 + (double)(a0 + FAST_TA - 1) * p.dt;
-        if (LFA) { if (t_first - halo - hy[0] > 0.5 * hy[1]) return; }
-        else     { if (t_last + halo - hy[0] < -0.5 * hy[1]) return; }
-    }
 
     /* staged strain: samples [org, org + 2 * hw2), org even; parity split; LFA: FD1 numerators of the strain */
     const int64_t org = a0 - p.m1 - (p.m1 & 1);
@@ -549,9 +559,8 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(const __grid_c
 template <int H>
 __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_hybrid_kernel(const __grid_constant__ FastParams p)
 {
-    const int64_t nfull = p.ntilesA * p.batch;
-    if ((int64_t)blockIdx.x < nfull) link_body<H, false>(p, blockIdx.x);
-    else link_body<H, true>(p, (int64_t)blockIdx.x - nfull);
+    if ((int64_t)blockIdx.x < p.nwork_full) link_body<H, false>(p, blockIdx.x);
+    else link_body<H, true>(p, blockIdx.x);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -632,6 +641,7 @@ __global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ Fast
     __syncthreads();
     if (tid >= FAST_NA) return;
     double d, bound;
+    int64_t m2;   /* the halo of the generation that uses this delay */
     if (tid < FAST_NA_FULL) {
         const int ch = tid / 13, id = tid % 13;
         const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
@@ -640,11 +650,14 @@ __global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ Fast
         const DelayDef df = c_delay_def[id];
         bound = (df.base == 1 ? dev[i2 + 3] : df.base == 2 ? dev[i3] : 0.0) + df.i * (dev[i2 + 3] + dev[i2]) +
                 df.j * (dev[i3] + dev[i3 + 3]);
+        m2 = id < 6 ? p.m2_15 : p.m2_20;   /* delays 0..5 are the ones of Eq. (2.7), used by both generations */
     } else {
-        const int ch = (tid - FAST_NA_FULL) / 2, id = (tid - FAST_NA_FULL) % 2;
+        const int k = tid - FAST_NA_FULL, gen = k < FAST_NA_LFA_GEN ? LTDI_GEN_15 : LTDI_GEN_20;
+        const int ch = (k % FAST_NA_LFA_GEN) / 2, id = k % 2;
         const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
-        d = lfa_delay(p.gen, id, Lc[i2], Lc[i3]);
+        d = lfa_delay(gen, id, Lc[i2], Lc[i3]);
         bound = 2.0 * (dev[i2] + dev[i3]);
+        m2 = gen == LTDI_GEN_15 ? p.m2_15 : p.m2_20;
     }
     bound *= p.inv_dt;
     int q;
@@ -653,7 +666,7 @@ __global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ Fast
     /* usable if the Taylor remainder is below rounding, the integer shift cannot change inside the tile and the
      * stencil stays inside the staged halo */
     const bool ok = bound <= FAST_DMAX && eps - bound >= 0.0 && eps + bound < 1.0 && q >= 0 &&
-                    q + M / 2 <= p.m2;
+                    q + M / 2 <= m2;
     double *h = hdr + (tile * FAST_NA + tid) * 4;
     h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? 1.0 : 0.0;
 
@@ -769,34 +782,22 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     constexpr int ANC = FAST_ANC_DOUBLES(M);
     constexpr bool has_full = WHICH != LTDI_RESPONSE_LFA, has_lfa = WHICH != LTDI_RESPONSE_FULL;
     constexpr int NLR = has_full ? 6 : 3;   /* light-time rows the tile needs (LFA: the positive links) */
-    const int64_t b = (int64_t)blockIdx.x % p.batch;
-    int64_t tile = (int64_t)blockIdx.x / p.batch;
-    /* hybrid: tiles past t_hyb carry the 14-term full response; schedule them first (no long tail) */
-    if (WHICH == LTDI_RESPONSE_HYBRID) tile = p.ntilesC - 1 - tile;
+    int64_t b, tile;
+    work_item(p, blockIdx.x, b, tile);
     const int64_t n0 = tile * FAST_TC;
     const int64_t n1 = min(n0 + (int64_t)FAST_TC, p.n);
     const int tid = threadIdx.x;
     const int w = (int)p.w;
 
-    /* The hybrid response runs as two concurrent launches over the same 448-sample tiles: the LFA instance (80
-     * registers, four CTAs per SM) takes the tiles that lie entirely before the window (w_Full = 0 on every sample;
-     * it applies w_LFA in its epilogue), the hybrid instance (168 registers, the shared memory of both responses) the
-     * tiles that need the full response, alone or blended.  The other kind of tile exits at once. */
-    bool need_full = WHICH == LTDI_RESPONSE_FULL, need_lfa = WHICH == LTDI_RESPONSE_LFA;
-    const bool hybrid_mode = WHICH != LTDI_RESPONSE_FULL && p.which == LTDI_RESPONSE_HYBRID;
+    /* The hybrid response (p.which == HYBRID) runs as three launches over compact tile lists (hybrid_plan_kernel): the
+     * LFA instance takes the 448-sample blocks that lie entirely before the window (w_Full = 0; it applies w_LFA in
+     * its epilogue), the HYBRID instance the blocks the window touches (both responses, blended by (4.6)), and the
+     * FULL instance -- no LFA shared memory, four CTAs per SM -- the 224-sample tiles entirely after the window
+     * (w_LFA = 0; it applies w_Full in its epilogue). */
+    constexpr bool need_full = WHICH != LTDI_RESPONSE_LFA, need_lfa = WHICH != LTDI_RESPONSE_FULL;
+    const bool hybrid_mode = p.which == LTDI_RESPONSE_HYBRID;
     const double *hy = nullptr;
-    if (hybrid_mode) {
-        hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
-        const double t_first = p.t0 + (double)n0 * p.dt, t_last = p.t0 + (double)(n1 - 1) * p.dt;
-        const bool tile_full = (t_last - hy[0]) >= -0.5 * hy[1];  /* some sample has w_Full != 0, Eq. (4.5) */
-        if (WHICH == LTDI_RESPONSE_LFA) {
-            if (tile_full) return;
-        } else {
-            if (!tile_full) return;
-            need_lfa = (t_first - hy[0]) <= 0.5 * hy[1];   /* some sample has w_LFA != 0 */
-            need_full = true;
-        }
-    }
+    if (hybrid_mode) hy = p.use_small ? p.small + 96 + 4 * (p.n_hyb == 1 ? 0 : p.b0 + b) : p.hyb + 4 * (p.n_hyb == 1 ? 0 : b);
 
     /* shared memory (host: tdi_smem_bytes):
      *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
@@ -807,7 +808,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     const int64_t y0 = n0 - tdi_back(p.m2);
     constexpr int na_full = has_full ? FAST_NA_FULL : 0;
     double *sa = smem;
-    double *yF = sa + (size_t)(na_full + (has_lfa ? FAST_NA_LFA : 0)) * ANC;
+    double *yF = sa + (size_t)(na_full + (has_lfa ? FAST_NA_LFA_GEN : 0)) * ANC;
     double *dL = yF + (has_full ? 6 * yr : 0);
     double *Lr = dL + (has_lfa ? 3 * yr : 0);
     double *yL = Lr + NLR * FAST_TC;
@@ -816,6 +817,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     constexpr bool xs_alias = WHICH == LTDI_RESPONSE_HYBRID;
     double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * (yr + 2 * w) : 0);
     const double *sa_lfa = sa + (size_t)na_full * ANC;
+    const int lfa_a0 = p.gen == LTDI_GEN_15 ? 0 : FAST_NA_LFA_GEN;   /* first LFA anchor of this generation */
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
     __shared__ double s_hdr[FAST_NA * 4];
 
@@ -868,9 +870,9 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
         if (has_full && need_full)
             for (int i = tid; i < FAST_NA_FULL * ANC / 2; i += FAST_TC_THREADS)
                 cp_async16(sa + 2 * i, ga + 2 * i);
-        if (has_lfa && need_lfa)
-            for (int i = tid; i < FAST_NA_LFA * ANC / 2; i += FAST_TC_THREADS)
-                cp_async16(sa + (size_t)na_full * ANC + 2 * i, ga + FAST_NA_FULL * ANC + 2 * i);
+        if (has_lfa && need_lfa)   /* the six LFA anchors of this generation */
+            for (int i = tid; i < FAST_NA_LFA_GEN * ANC / 2; i += FAST_TC_THREADS)
+                cp_async16(sa + (size_t)na_full * ANC + 2 * i, ga + (FAST_NA_FULL + lfa_a0) * ANC + 2 * i);
         for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[atile * (FAST_NA * 4) + i];
     }
     cp_async_wait_all();
@@ -935,7 +937,8 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
         for (int id = 0; id < nd; ++id) ok = ok && s_hdr[4 * (13 * ch + id) + 3] != 0.0;
     }
     if (has_lfa && need_lfa)
-        ok = ok && s_hdr[4 * (FAST_NA_FULL + 2 * ch) + 3] != 0.0 && s_hdr[4 * (FAST_NA_FULL + 2 * ch + 1) + 3] != 0.0;
+        ok = ok && s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch) + 3] != 0.0 &&
+             s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch + 1) + 3] != 0.0;
 
     if (ok) {
         /* one loop over the interpolated terms of this channel: 6 / 14 of Eq. (2.7) / (2.8) on the full links, then
@@ -966,7 +969,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
                 sgn = (double)td.sign;
             } else {
                 const int id = tm - 14;   /* 0: d/dt y_{p2} at L_p3 + L_p2 / 2 (gen 1.5);  1: d/dt y_{p3} at L_p2 + L_p3 / 2 */
-                const double *hd = s_hdr + 4 * (FAST_NA_FULL + 2 * ch + id);
+                const double *hd = s_hdr + 4 * (FAST_NA_FULL + lfa_a0 + 2 * ch + id);
                 dc = hd[0];
                 xs = dL + (id == 0 ? i2 : i3) * yr + i0 - (int)hd[1] - (H - 1);
                 anc_t = sa_lfa + (2 * ch + id) * ANC;
@@ -1050,11 +1053,16 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             X = use_f ? fma(wb, X, x0) : x0;
             Y = use_f ? fma(wb, Y, y0b) : y0b;
             Z = use_f ? fma(wb, Z, z0) : z0;
-        } else if (hybrid_mode) {   /* LFA instance on a tile before the window: w_Full = 0 */
+        } else if (WHICH == LTDI_RESPONSE_LFA && hybrid_mode) {    /* a block before the window: w_Full = 0 */
             hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
             X = wa != 0.0 ? wa * X : 0.0;
             Y = wa != 0.0 ? wa * Y : 0.0;
             Z = wa != 0.0 ? wa * Z : 0.0;
+        } else if (WHICH == LTDI_RESPONSE_FULL && hybrid_mode) {   /* a tile after the window: w_LFA = 0 */
+            hybrid_weights_fast(hy, p.t0 + (double)n * p.dt, wa, wb);
+            X = wb != 0.0 ? wb * X : 0.0;
+            Y = wb != 0.0 ? wb * Y : 0.0;
+            Z = wb != 0.0 ? wb * Z : 0.0;
         }
         if (!(n >= p.lo && n < p.n - p.hi)) { X = 0.0; Y = 0.0; Z = 0.0; }
         p.A[src_off + n] = (Z - X) * is2;                 /* (2.9a) */
@@ -1072,7 +1080,10 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
 #pragma unroll 1
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
-                if (WHICH == LTDI_RESPONSE_FULL) v = yF[l * yr + iy];
+                if (WHICH == LTDI_RESPONSE_FULL) {
+                    if (!hybrid_mode) v = yF[l * yr + iy];
+                    else if (wb != 0.0 && n >= p.m1 + w && n < p.n - p.m1 - w) v = wb * yF[l * yr + iy];          /* (4.5) */
+                }
                 else if (WHICH == LTDI_RESPONSE_LFA) {
                     if (!hybrid_mode) v = l < 3 ? gl[l * ystride] : 0.0;
                     else if (l < 3 && wa != 0.0 && n >= p.m1 + w && n < p.n - p.m1 - w) v = wa * gl[l * ystride]; /* (4.5) */

@@ -55,12 +55,25 @@ struct ProfScope {
     }
 };
 
-// 1 / prod_{m != k}(k - m), k, m = -(M/2-1) .. M/2, for every even M <= 64 (rows of c_lag_inv_den)
-int init_constants()
+// Per-device state.  __constant__ tables, cudaFuncSetAttribute, streams and events all belong to ONE device: a
+// process that uses several devices gets one DeviceState per device (indexed by cudaGetDevice()).
+struct DeviceState {
+    std::mutex mu;                 /* guards everything below, and serialises the hybrid fork / join on the device */
+    bool ready = false;
+    int status = LTDI_OK;
+    int smem_max = 0, sms = 0;
+    cudaStream_t side = nullptr;   /* non-blocking side stream of the hybrid's concurrent launches */
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    std::vector<std::pair<const void *, size_t>> smem_seen;   /* cudaFuncAttributeMaxDynamicSharedMemorySize per kernel */
+};
+DeviceState g_dev[64];
+
+// 1 / prod_{m != k}(k - m), k, m = -(M/2-1) .. M/2, for every even M <= 64 (rows of c_lag_inv_den), and the
+// scale factors of the symmetric pair form, uploaded to the CURRENT device
+int upload_constants()
 {
-    static std::once_flag once;
-    static int status = LTDI_OK;
-    std::call_once(once, [] {
+    int status = LTDI_OK;
+    {
         std::vector<double> tab(32 * LTDI_MAX_TAPS, 0.0);
         for (int r = 0; r < 32; ++r) {
             const int M = 2 * (r + 1), kmin = -(M / 2 - 1);
@@ -107,8 +120,34 @@ int init_constants()
             (void)cudaGetLastError();
             status = LTDI_ECUDA;
         }
-    });
+    }
     return status;
+}
+
+/* the state of the current device, initialised on first use */
+int device_state(DeviceState **out)
+{
+    int dev = 0;
+    LTDI_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return LTDI_EUNSUPPORTED;
+    DeviceState &d = g_dev[dev];
+    std::lock_guard<std::mutex> lk(d.mu);
+    if (!d.ready) {
+        d.status = upload_constants();
+        if (d.status == LTDI_OK) {
+            if (cudaDeviceGetAttribute(&d.smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess ||
+                cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+                cudaStreamCreateWithFlags(&d.side, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&d.ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&d.ev_join, cudaEventDisableTiming) != cudaSuccess) {
+                (void)cudaGetLastError();
+                d.status = LTDI_ECUDA;
+            }
+        }
+        d.ready = true;
+    }
+    *out = &d;
+    return d.status;
 }
 
 int64_t iceil(double x) { return (int64_t)std::ceil(x); }
@@ -199,19 +238,21 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
     return LTDI_OK;
 }
 
-// workspace layout (doubles): raw sources [batch][3] | frames [batch][16] | hybrid windows [n_hyb][4]
-size_t work_doubles(int64_t batch) { return ((size_t)batch * (3 + LTDI_FRAME_STRIDE + 4) + 31) / 32 * 32; }
+// workspace layout (doubles): raw sources [batch][3] | frames [batch][16] | hybrid windows [n_hyb][4] | hybrid tile
+// plan [batch][4] (eight 32-bit integers per source, HybPlan)
+size_t work_doubles(int64_t batch) { return ((size_t)batch * (3 + LTDI_FRAME_STRIDE + 4 + 4) + 31) / 32 * 32; }
 
 bool fast_order(int order) { return order == 9 || order == 31; }
 
 /* workspace of the fast path behind the per-source parameters: anchors | anchor headers | link-series scratch
- * for one chunk of sources.  Chunks of up to 2 GiB of scratch: measured on B200, large chunks (fewer launches, fewer
- * grid tails) beat chunks small enough to keep the link series in the 126 MB L2 (96 MB: 5 % slower at cfg4s) -- the
- * scratch traffic, 96 B per sample, is < 5 % of the HBM bandwidth at the speed of these FP64-bound kernels. */
+ * for one chunk of sources | (hybrid) the compact tile lists of the chunk.  Chunks of up to 2 GiB of scratch: measured
+ * on B200, large chunks (fewer launches, fewer grid tails) beat chunks small enough to keep the link series in the
+ * 126 MB L2 (96 MB: 5 % slower at cfg4s) -- the scratch traffic, 96 B per sample, is < 5 % of the HBM bandwidth at the
+ * speed of these FP64-bound kernels. */
 struct FastLayout {
-    int64_t ntilesA, ntilesC, ntilesN, lds, chunk;   /* link tiles, TDI tiles, anchor tiles */
-    size_t anc, hdr, y;     /* doubles */
-    size_t total;           /* doubles, including work_doubles(batch) */
+    int64_t ntilesA, ntilesC, ntilesN, lds, chunk;   /* link tiles, TDI tiles, anchor tiles (= 448-sample blocks) */
+    size_t anc, hdr, y, lists;     /* doubles */
+    size_t total;                  /* doubles, including work_doubles(batch) */
 };
 FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
 {
@@ -227,8 +268,88 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
     f.anc = (size_t)f.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
     f.hdr = (size_t)f.ntilesN * FAST_NA * 4;
     f.y = (size_t)rows * f.chunk * f.lds;
-    f.total = work_doubles(batch) + f.anc + f.hdr + f.y;
+    /* hybrid: link tiles of both kinds, LFA-only blocks, blend blocks, full-only 224-sample tiles (int2 each) */
+    f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)f.chunk * (2 * f.ntilesA + 4 * f.ntilesN) : 0;
+    f.total = work_doubles(batch) + f.anc + f.hdr + f.y + f.lists;
     return f;
+}
+
+// ---- hybrid tile plan (S8) ---------------------------------------------------------------------------------------
+// Per source the host classifies the 448-sample blocks from (t_hyb, T): blocks [0, nLt) lie entirely before the
+// window (w_Full = 0 on every sample, with one sample of margin: LFA only), blocks [fFt, nblk) entirely after it
+// (w_LFA = 0: full response only), blocks [nLt, fFt) need both and the blend of Eq. (4.6).  Everything else -- which
+// link tiles are needed, how many CTAs every launch has -- follows from these two integers by the integer rules of
+// hyb_counts(), evaluated identically on the host (grid sizes, list offsets) and in hybrid_plan_kernel (list entries).
+struct HybPlan { int nLt, fFt, off_link_full, off_link_lfa, off_lfa, off_blend, off_full, pad; };
+struct HybGeom { int64_t n, ntilesA, nblk; int back, fwd; };
+struct HybCounts { int64_t lfa_link, full_link_first, full_link, lfa_blk, blend_blk, full_first, full_tiles; };
+__host__ __device__ inline HybCounts hyb_counts(const HybGeom &g, int nLt, int fFt)
+{
+    HybCounts c;
+    /* LFA links: read by the TDI stage of blocks [0, fFt), up to `fwd` samples past their end */
+    int64_t endL = fFt == 0 ? 0 : (int64_t)fFt * FAST_TCA + g.fwd;
+    if (endL > g.n) endL = g.n;
+    c.lfa_link = (endL + FAST_TA - 1) / FAST_TA;
+    /* full links: read by the TDI stage of blocks [nLt, nblk), from `back` samples before their start */
+    int64_t first = (int64_t)nLt * FAST_TCA - g.back;
+    if (first < 0) first = 0;
+    c.full_link_first = nLt >= g.nblk ? g.ntilesA : first / FAST_TA;
+    c.full_link = g.ntilesA - c.full_link_first;
+    c.lfa_blk = nLt;
+    c.blend_blk = fFt - nLt;
+    c.full_first = 2 * (int64_t)fFt;   /* 224-sample tiles of the FULL instance */
+    c.full_tiles = fFt >= g.nblk ? 0 : (g.n - (int64_t)fFt * FAST_TCA + tdi_tc(LTDI_RESPONSE_FULL) - 1) / tdi_tc(LTDI_RESPONSE_FULL);
+    return c;
+}
+static_assert(FAST_TCA == 2 * tdi_tc(LTDI_RESPONSE_FULL) && FAST_TCA == tdi_tc(LTDI_RESPONSE_HYBRID) && FAST_TCA == tdi_tc(LTDI_RESPONSE_LFA),
+              "the hybrid plan counts 448-sample blocks");
+
+struct PlanArgs {
+    HybGeom g;
+    const HybPlan *plan;      /* [nb] of the chunk (device), or nullptr: `small` */
+    HybPlan small[32];
+    int64_t b0, nb;
+    int2 *link_list, *lfa_list, *blend_list, *full_list;
+    int64_t n_link_full;      /* LFA-link items follow the full-link items in link_list */
+};
+
+/* blockIdx.y = source of the chunk, threads over the tile slot j: writes the (source, tile) entries of the five lists.
+ * Heavy tiles first: the full-link items precede the LFA-link items, and late (full) tiles precede early ones. */
+__global__ void hybrid_plan_kernel(const __grid_constant__ PlanArgs a)
+{
+    const int64_t b = blockIdx.y;
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const HybPlan pl = a.plan ? a.plan[b] : a.small[a.b0 + b];
+    const HybCounts c = hyb_counts(a.g, pl.nLt, pl.fFt);
+    if (j < c.full_link) a.link_list[pl.off_link_full + j] = make_int2((int)b, (int)(a.g.ntilesA - 1 - j));
+    if (j < c.lfa_link) a.link_list[a.n_link_full + pl.off_link_lfa + j] = make_int2((int)b, (int)j);
+    if (j < c.lfa_blk) a.lfa_list[pl.off_lfa + j] = make_int2((int)b, (int)j);
+    if (j < c.blend_blk) a.blend_list[pl.off_blend + j] = make_int2((int)b, (int)(pl.nLt + j));
+    if (j < c.full_tiles) a.full_list[pl.off_full + j] = make_int2((int)b, (int)(c.full_first + j));
+}
+
+/* nLt, fFt of one source (host): block k = samples [448 k, min(448 (k + 1), n)), one sample of margin on either side
+ * so that the per-sample weights of the kernels (their own fp64 rounding of t_n) can never disagree with the class */
+void classify_blocks(const ltdi_orbit_desc &d, const ltdi_hybrid &h, int64_t nblk, int *nLt, int *fFt)
+{
+    auto lfa_only = [&](int64_t k) {
+        const int64_t e = std::min((k + 1) * (int64_t)FAST_TCA, d.n) - 1;
+        return d.t0 + (double)e * d.dt + d.dt - h.t_hyb < -0.5 * h.window_s;
+    };
+    auto full_only = [&](int64_t k) { return d.t0 + (double)(k * FAST_TCA) * d.dt - d.dt - h.t_hyb > 0.5 * h.window_s; };
+    auto guess = [&](double t) {
+        const double k = std::floor((t - d.t0) / d.dt / (double)FAST_TCA);
+        return (int64_t)std::min(std::max(k, 0.0), (double)nblk);
+    };
+    int64_t a = guess(h.t_hyb - 0.5 * h.window_s);
+    while (a < nblk && lfa_only(a)) ++a;
+    while (a > 0 && !lfa_only(a - 1)) --a;
+    int64_t f = guess(h.t_hyb + 0.5 * h.window_s);
+    while (f > 0 && full_only(f - 1)) --f;
+    while (f < nblk && !full_only(f)) ++f;
+    if (f < a) f = a;
+    *nLt = (int)a;
+    *fFt = (int)f;
 }
 
 struct SmallArgs { double v[32 * 7]; }; /* batch <= 32: sources and windows travel as kernel arguments */
@@ -244,11 +365,11 @@ __global__ void unpack_small_kernel(SmallArgs a, int batch, int n_hyb, double *s
 /* batch > 32: the parameters of up to 512 sources per launch travel as kernel arguments (28 KB; CUDA >= 12.1 allows
  * 32 764 bytes on sm_70+).  A cudaMemcpyAsync from pageable host memory above 64 KB would block the host until the
  * stream has drained, which leaves the GPU idle between the calls of a step. */
-#define LTDI_BIG_SOURCES 512
-struct BigArgs { double src[LTDI_BIG_SOURCES * 3]; double hyb[LTDI_BIG_SOURCES * 4]; };
+#define LTDI_BIG_SOURCES 256
+struct BigArgs { double src[LTDI_BIG_SOURCES * 3]; double hyb[LTDI_BIG_SOURCES * 4]; HybPlan plan[LTDI_BIG_SOURCES]; };
 
-__global__ void unpack_big_kernel(const __grid_constant__ BigArgs a, int count, int n_hyb_here, double *src, double *frames,
-                                  double *hyb)
+__global__ void unpack_big_kernel(const __grid_constant__ BigArgs a, int count, int n_hyb_here, int n_plan, double *src,
+                                  double *frames, double *hyb, HybPlan *plan)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < count) {
@@ -259,17 +380,33 @@ __global__ void unpack_big_kernel(const __grid_constant__ BigArgs a, int count, 
         hyb[4 * i] = a.hyb[4 * i]; hyb[4 * i + 1] = a.hyb[4 * i + 1];
         hyb[4 * i + 2] = a.hyb[4 * i + 2]; hyb[4 * i + 3] = a.hyb[4 * i + 3];
     }
+    if (i < n_plan) plan[i] = a.plan[i];
+}
+
+template <typename K>
+int set_smem(DeviceState &ds, K kernel, size_t smem)
+{
+    if (smem > (size_t)ds.smem_max) return LTDI_EUNSUPPORTED;
+    if (smem + 4096 <= 48 * 1024) return LTDI_OK;   /* the kernels' static shared memory (<= 2 KB) counts too */
+    /* the attribute is sticky per device function and device: raise it only when a call needs more than any before */
+    std::lock_guard<std::mutex> lk(ds.mu);
+    for (auto &e : ds.smem_seen)
+        if (e.first == (const void *)kernel) {
+            if (e.second >= smem) return LTDI_OK;
+            LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            e.second = smem;
+            return LTDI_OK;
+        }
+    LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ds.smem_seen.emplace_back((const void *)kernel, smem);
+    return LTDI_OK;
 }
 
 template <int MT, bool STAGE>
-int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t st)
+int launch_response(DeviceState &ds, const RespParams &p, int threads, size_t smem, cudaStream_t st)
 {
-    static std::atomic<size_t> configured{0};
-    if (smem + 4096 > 48 * 1024 && smem > configured.load()) {   /* static shared memory counts too */
-        LTDI_CUDA_OK(cudaFuncSetAttribute(response_kernel<MT, STAGE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)smem));
-        configured.store(smem);
-    }
+    const int rc = set_smem(ds, response_kernel<MT, STAGE>, smem);
+    if (rc) return rc;
     {
         ProfScope ps(LTDI_KERNEL_GENERIC + LTDI_KERNEL_COUNT * p.which, st);
         response_kernel<MT, STAGE><<<(unsigned)(p.ntiles * p.batch), threads, smem, st>>>(p);
@@ -279,117 +416,97 @@ int launch_response(const RespParams &p, int threads, size_t smem, cudaStream_t 
     return LTDI_OK;
 }
 
-template <typename K>
-int set_smem(K kernel, size_t smem, int smem_max)
+/* host side of the hybrid plan: per-source plans (offsets relative to the source's chunk) and per-chunk totals */
+struct ChunkTotals { int64_t link_full, link_lfa, lfa, blend, full, max_slots; };
+struct HybHost {
+    std::vector<HybPlan> plan;        /* [batch] */
+    std::vector<ChunkTotals> chunk;   /* [number of chunks] */
+    HybGeom g;
+};
+
+int build_hybrid_plan(const ltdi_orbit_desc &d, const Margins &mg, int M, const FastLayout &lay, int64_t batch,
+                      const ltdi_hybrid *h_hyb, int64_t n_hyb, HybHost *out)
 {
-    if (smem > (size_t)smem_max) return LTDI_EUNSUPPORTED;
-    if (smem + 4096 <= 48 * 1024) return LTDI_OK;   /* the kernels' static shared memory (<= 2 KB) counts too */
-    /* the attribute is sticky per device function: raise it only when a call needs more than any before */
-    static std::mutex mu;
-    static std::vector<std::pair<const void *, size_t>> seen;
-    std::lock_guard<std::mutex> lk(mu);
-    for (auto &e : seen)
-        if (e.first == (const void *)kernel) {
-            if (e.second >= smem) return LTDI_OK;
-            LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            e.second = smem;
-            return LTDI_OK;
+    out->g.n = d.n; out->g.ntilesA = lay.ntilesA; out->g.nblk = lay.ntilesN;
+    out->g.back = tdi_back(mg.m2) + 2;
+    out->g.fwd = M / 2 + 4 + 2 * (int)mg.w;
+    out->plan.resize((size_t)batch);
+    out->chunk.clear();
+    int nLt = 0, fFt = 0;
+    for (int64_t b0 = 0; b0 < batch; b0 += lay.chunk) {
+        const int64_t nb = std::min(lay.chunk, batch - b0);
+        ChunkTotals t = {0, 0, 0, 0, 0, 0};
+        for (int64_t b = b0; b < b0 + nb; ++b) {
+            if (n_hyb != 1 || b == 0) classify_blocks(d, h_hyb[n_hyb == 1 ? 0 : b], lay.ntilesN, &nLt, &fFt);
+            const HybCounts c = hyb_counts(out->g, nLt, fFt);
+            if (std::max({t.link_full + c.full_link, t.link_lfa + c.lfa_link, t.lfa + c.lfa_blk, t.blend + c.blend_blk,
+                          t.full + c.full_tiles}) >= ((int64_t)1 << 31))
+                return LTDI_EUNSUPPORTED;
+            HybPlan &pl = out->plan[(size_t)b];
+            pl.nLt = nLt; pl.fFt = fFt; pl.pad = 0;
+            pl.off_link_full = (int)t.link_full; pl.off_link_lfa = (int)t.link_lfa; pl.off_lfa = (int)t.lfa;
+            pl.off_blend = (int)t.blend; pl.off_full = (int)t.full;
+            t.link_full += c.full_link; t.link_lfa += c.lfa_link; t.lfa += c.lfa_blk; t.blend += c.blend_blk;
+            t.full += c.full_tiles;
+            t.max_slots = std::max({t.max_slots, c.full_link, c.lfa_link, c.lfa_blk, c.blend_blk, c.full_tiles});
         }
-    LTDI_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    seen.emplace_back((const void *)kernel, smem);
+        out->chunk.push_back(t);
+    }
     return LTDI_OK;
 }
 
-/* one non-blocking side stream per device for the second TDI launch of the hybrid (ordering with the caller's
- * stream goes through events, so calls from several host threads stay correct: they only share the queue) */
-int side_stream(cudaStream_t *out)
-{
-    static std::mutex mu;
-    static cudaStream_t s[64] = {};   /* per device */
-    int dev = 0;
-    LTDI_CUDA_OK(cudaGetDevice(&dev));
-    if (dev < 0 || dev >= 64) return LTDI_EUNSUPPORTED;
-    std::lock_guard<std::mutex> lk(mu);
-    if (!s[dev]) LTDI_CUDA_OK(cudaStreamCreateWithFlags(&s[dev], cudaStreamNonBlocking));
-    *out = s[dev];
-    return LTDI_OK;
-}
-
-// the tuned path: anchors once per call, then link kernel(s) and TDI kernel per chunk of sources
+// the tuned path: anchors once per call, then link kernel(s) and TDI kernel(s) per chunk of sources
 template <int M>
-int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work, cudaStream_t st,
-             const double *small /* [32 * 7] host values or nullptr */)
+int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work,
+             cudaStream_t st, const double *small /* [32 * 7] host values or nullptr */, const HybHost *hh,
+             const HybPlan *d_plan /* [batch] device copies of hh->plan, or nullptr when small */)
 {
     constexpr int H = M / 2;
     const ltdi_orbit_desc &d = orb->desc;
     const FastLayout lay = fast_layout(which, d.n, rp.batch, M);
     if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_EUNSUPPORTED;
-    static std::atomic<int> smem_max_cached{0};   /* one device per process (one process per GPU) */
-    int smem_max = smem_max_cached.load();
-    if (!smem_max) {
-        int dev = 0;
-        LTDI_CUDA_OK(cudaGetDevice(&dev));
-        LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        smem_max_cached.store(smem_max);
-    }
 
     FastParams p;
     std::memset(&p, 0, sizeof p);
     p.tab = rp.tab; p.stride = rp.stride; p.n = rp.n; p.t0 = rp.t0; p.dt = rp.dt; p.inv_dt = 1.0 / rp.dt;
     p.ld = rp.ld; p.n_hyb = rp.n_hyb; p.which = which; p.gen = rp.gen; p.fd = rp.fd;
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi; p.qmax = rp.qmax;
+    p.m2_15 = compute_margins(d, LTDI_GEN_15, M - 1, 0).m2;
+    p.m2_20 = compute_margins(d, LTDI_GEN_20, M - 1, 0).m2;
     p.inv_fd1 = 1.0 / ((mg.w == 1 ? 2.0 : 12.0) * rp.dt);
     p.inv_fd2 = 1.0 / ((mg.w == 1 ? 1.0 : 12.0) * rp.dt * rp.dt);
     p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
     p.use_small = small != nullptr;
     if (small) std::memcpy(p.small, small, sizeof p.small);
     double *anc = work, *hdr = anc + lay.anc, *ys = hdr + lay.hdr;
+    int2 *lists = reinterpret_cast<int2 *>(ys + lay.y);
     p.anc = anc; p.anc_hdr = hdr;
 
     const bool full = which != LTDI_RESPONSE_LFA, lfa = which != LTDI_RESPONSE_FULL;
+    const bool hybrid = which == LTDI_RESPONSE_HYBRID;
     /* staged strain (4 parity-split series) + the orbit-table rows of the tile */
     const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
     const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
     const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double) +
                                  (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double) + /* + raw strain */
                                  (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float);                            /* + low parts */
-    const size_t smem_tdi = tdi_smem_bytes<M>(which, mg.m2, mg.w);
-    int rc;
-    const bool hybrid = which == LTDI_RESPONSE_HYBRID;
     const size_t smem_link_hyb = std::max(smem_link, smem_link_lfa);
-    if (hybrid) {
-        if ((rc = set_smem(link_hybrid_kernel<H>, smem_link_hyb, smem_max))) return rc;
-    } else {
-        if (full && (rc = set_smem(link_kernel<H, false>, smem_link, smem_max))) return rc;
-        if (lfa && (rc = set_smem(link_kernel<H, true>, smem_link_lfa, smem_max))) return rc;
-    }
-    void (*tdi)(FastParams) = which == LTDI_RESPONSE_FULL  ? tdi_kernel<M, LTDI_RESPONSE_FULL>
-                              : which == LTDI_RESPONSE_LFA ? tdi_kernel<M, LTDI_RESPONSE_LFA>
-                                                           : tdi_kernel<M, LTDI_RESPONSE_HYBRID>;
-    if ((rc = set_smem(tdi, smem_tdi, smem_max))) return rc;
-    /* hybrid: the tiles before the window go through the LFA instance (same 448-sample tiles) on a side stream, so
-     * that its CTAs (four per SM) run beside those of the hybrid instance (two per SM) */
+    const size_t smem_tdi_full = tdi_smem_bytes<M>(LTDI_RESPONSE_FULL, mg.m2, mg.w);
+    const size_t smem_tdi_hyb = tdi_smem_bytes<M>(LTDI_RESPONSE_HYBRID, mg.m2, mg.w);
     const size_t smem_tdi_lfa = tdi_smem_bytes<M>(LTDI_RESPONSE_LFA, mg.m2, mg.w);
-    static_assert(tdi_tc(LTDI_RESPONSE_LFA) == tdi_tc(LTDI_RESPONSE_HYBRID), "the two launches share the tiling");
-    cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int rc;
     if (hybrid) {
-        if ((rc = set_smem(tdi_kernel<M, LTDI_RESPONSE_LFA>, smem_tdi_lfa, smem_max))) return rc;
-        if ((rc = side_stream(&side))) return rc;
-        LTDI_CUDA_OK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
-        if (cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming) != cudaSuccess) {
-            (void)cudaGetLastError();
-            cudaEventDestroy(ev_fork);
-            return LTDI_ECUDA;
-        }
+        if ((rc = set_smem(ds, link_hybrid_kernel<H>, smem_link_hyb))) return rc;
+        if ((rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_HYBRID>, smem_tdi_hyb))) return rc;
+    } else {
+        if (full && (rc = set_smem(ds, link_kernel<H, false>, smem_link))) return rc;
+        if (lfa && (rc = set_smem(ds, link_kernel<H, true>, smem_link_lfa))) return rc;
     }
-    struct EventGuard {   /* an event may be destroyed while work that refers to it is still queued */
-        cudaEvent_t a, b;
-        ~EventGuard() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
-    } guard{ev_fork, ev_join};
+    if (full && (rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_FULL>, smem_tdi_full))) return rc;
+    if (lfa && (rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_LFA>, smem_tdi_lfa))) return rc;
 
-    if (orb->d_anc && orb->anc_gen == rp.gen && orb->anc_M == M) {
-        /* ltdi_orbits_prepare() has computed the anchors of this (generation, order) for the time grid */
+    if (orb->d_anc && orb->anc_M == M) {
+        /* ltdi_orbits_prepare() has computed the anchors of this order for the time grid (they serve both generations) */
         p.anc = orb->d_anc;
         p.anc_hdr = orb->d_anc + (size_t)lay.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
     } else {
@@ -399,7 +516,12 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         LTDI_CUDA_OK(cudaGetLastError());
     }
 
-    for (int64_t b0 = 0; b0 < rp.batch; b0 += lay.chunk) {
+    /* the hybrid forks its LFA blocks onto the device's side stream: one call at a time per device uses the events */
+    std::unique_lock<std::mutex> fork_lock(ds.mu, std::defer_lock);
+    if (hybrid) fork_lock.lock();
+
+    int64_t ichunk = 0;
+    for (int64_t b0 = 0; b0 < rp.batch; b0 += lay.chunk, ++ichunk) {
         const int64_t nb = std::min(lay.chunk, rp.batch - b0);
         p.batch = nb; p.b0 = b0;
         p.hp = rp.hp + b0 * rp.ld; p.hc = rp.hc + b0 * rp.ld;
@@ -408,37 +530,88 @@ int run_fast(const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, in
         p.A = rp.A + b0 * rp.ld; p.E = rp.E + b0 * rp.ld; p.T = rp.T + b0 * rp.ld;
         p.XYZ = rp.XYZ; p.Y = rp.Y;
         p.yF = ys; p.yL = ys + (full ? (size_t)6 * nb * lay.lds : 0);
+        p.work = nullptr; p.nwork = 0; p.nwork_full = 0;
         if (lay.ntilesA * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
-        if (hybrid) {
-            if (2 * lay.ntilesA * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
+        if (!hybrid) {
+            if (full) {
+                {
+                    ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
+                    link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+                }
+                count_launch();
+                ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
+                tdi_kernel<M, LTDI_RESPONSE_FULL><<<(unsigned)(lay.ntilesC * nb), tdi_threads(LTDI_RESPONSE_FULL),
+                                                    smem_tdi_full, st>>>(p);
+            } else {
+                {
+                    ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
+                    link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
+                }
+                count_launch();
+                p.nwork = lay.ntilesN * nb;
+                ProfScope ps(LTDI_KERNEL_TDI_LFA + LTDI_KERNEL_COUNT * which, st);
+                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)p.nwork, tdi_threads(LTDI_RESPONSE_LFA), smem_tdi_lfa, st>>>(p);
+            }
+            count_launch();
+            LTDI_CUDA_OK(cudaGetLastError());
+            continue;
+        }
+
+        /* hybrid: compact lists, then one launch per class of tiles */
+        const ChunkTotals &ct = hh->chunk[(size_t)ichunk];
+        int2 *l_link = lists, *l_lfa = l_link + (size_t)nb * 2 * lay.ntilesA, *l_blend = l_lfa + (size_t)nb * lay.ntilesN,
+             *l_full = l_blend + (size_t)nb * lay.ntilesN;
+        {
+            PlanArgs a;
+            std::memset(&a, 0, sizeof a);
+            a.g = hh->g;
+            a.plan = d_plan ? d_plan + b0 : nullptr;
+            if (!d_plan) std::memcpy(a.small, hh->plan.data(), hh->plan.size() * sizeof(HybPlan));
+            a.b0 = b0; a.nb = nb;
+            a.link_list = l_link; a.lfa_list = l_lfa; a.blend_list = l_blend; a.full_list = l_full;
+            a.n_link_full = ct.link_full;
+            if (ct.max_slots > 0) {
+                ProfScope ps(LTDI_KERNEL_PLAN + LTDI_KERNEL_COUNT * which, st);
+                hybrid_plan_kernel<<<dim3((unsigned)((ct.max_slots + 127) / 128), (unsigned)nb), 128, 0, st>>>(a);
+                count_launch();
+            }
+        }
+        if (ct.link_full + ct.link_lfa > 0) {
+            p.work = l_link; p.nwork = ct.link_full + ct.link_lfa; p.nwork_full = ct.link_full;
             ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
-            link_hybrid_kernel<H><<<(unsigned)(2 * lay.ntilesA * nb), FAST_TA_THREADS, smem_link_hyb, st>>>(p);
+            link_hybrid_kernel<H><<<(unsigned)p.nwork, FAST_TA_THREADS, smem_link_hyb, st>>>(p);
             count_launch();
         }
-        if (full && !hybrid) {
-            ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
-            link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+        const bool side_lfa = ct.lfa > 0 && (ct.blend > 0 || ct.full > 0);   /* concurrent launches only if both exist */
+        if (ct.lfa > 0) {
+            cudaStream_t s_lfa = st;
+            if (side_lfa) {   /* fork: the LFA blocks on the side stream, beside the blend and full-only tiles */
+                LTDI_CUDA_OK(cudaEventRecord(ds.ev_fork, st));
+                LTDI_CUDA_OK(cudaStreamWaitEvent(ds.side, ds.ev_fork, 0));
+                s_lfa = ds.side;
+            }
+            p.work = l_lfa; p.nwork = ct.lfa; p.nwork_full = 0;
+            {
+                ProfScope ps(LTDI_KERNEL_TDI_LFA + LTDI_KERNEL_COUNT * which, s_lfa);
+                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)p.nwork, tdi_threads(LTDI_RESPONSE_LFA), smem_tdi_lfa, s_lfa>>>(p);
+            }
             count_launch();
-        }
-        if (lfa && !hybrid) {
-            ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
-            link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
-            count_launch();
+            if (side_lfa) LTDI_CUDA_OK(cudaEventRecord(ds.ev_join, ds.side));
         }
         {
             ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
-            if (hybrid) { /* fork: the LFA instance on the side stream, after the link kernels of this chunk */
-                LTDI_CUDA_OK(cudaEventRecord(ev_fork, st));
-                LTDI_CUDA_OK(cudaStreamWaitEvent(side, ev_fork, 0));
-                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)(lay.ntilesC * nb), tdi_threads(LTDI_RESPONSE_LFA),
-                                                   smem_tdi_lfa, side>>>(p);
+            if (ct.full > 0) {
+                p.work = l_full; p.nwork = ct.full;
+                tdi_kernel<M, LTDI_RESPONSE_FULL><<<(unsigned)ct.full, tdi_threads(LTDI_RESPONSE_FULL), smem_tdi_full, st>>>(p);
                 count_launch();
-                LTDI_CUDA_OK(cudaEventRecord(ev_join, side));
             }
-            tdi<<<(unsigned)(lay.ntilesC * nb), tdi_threads(which), smem_tdi, st>>>(p);
-            if (hybrid) LTDI_CUDA_OK(cudaStreamWaitEvent(st, ev_join, 0));   /* join before the scratch is reused */
+            if (ct.blend > 0) {
+                p.work = l_blend; p.nwork = ct.blend;
+                tdi_kernel<M, LTDI_RESPONSE_HYBRID><<<(unsigned)ct.blend, tdi_threads(LTDI_RESPONSE_HYBRID), smem_tdi_hyb, st>>>(p);
+                count_launch();
+            }
         }
-        count_launch();
+        if (side_lfa) LTDI_CUDA_OK(cudaStreamWaitEvent(st, ds.ev_join, 0));   /* join before the scratch is reused */
         LTDI_CUDA_OK(cudaGetLastError());
     }
     return LTDI_OK;
@@ -469,14 +642,28 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         if (work_bytes < need * sizeof(double)) return LTDI_EWORKSPACE;
     }
     if (batch * ((orb->desc.n + 63) / 64) >= (int64_t)1 << 31) return LTDI_EUNSUPPORTED;
-    int rc = init_constants();
+    DeviceState *dsp = nullptr;
+    int rc = device_state(&dsp);
     if (rc) return rc;
+    DeviceState &ds = *dsp;
     cudaStream_t st = (cudaStream_t)stream;
+    const ltdi_orbit_desc &d = orb->desc;
+    const Margins mg = compute_margins(d, gen, order, fd_order);
+    const int M = order + 1;
+
+    /* hybrid on the tuned path: the tile plan (host integers; see classify_blocks / hyb_counts) */
+    HybHost hh;
+    const bool plan_hybrid = which == LTDI_RESPONSE_HYBRID && fast_order(order) && mg.m2 <= 4096 && mg.m1 <= 8192;
+    if (plan_hybrid) {
+        rc = build_hybrid_plan(d, mg, M, fast_layout(which, d.n, batch, M), batch, h_hyb, n_hyb, &hh);
+        if (rc) return rc;
+    }
 
     /* S1: per-source parameters to the device, then the source-frame kernel */
     double *w_src = (double *)d_work;
     double *w_frames = w_src + 3 * batch;
     HybDev *w_hyb = (HybDev *)(w_frames + LTDI_FRAME_STRIDE * batch);
+    HybPlan *w_plan = (HybPlan *)((double *)w_hyb + 4 * batch);
     SmallArgs small_args;
     bool have_small = false;   /* batch <= 32: the tuned kernels take the parameters as arguments (no launch) */
     if (batch <= 32) {
@@ -508,11 +695,12 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
                 big->hyb[4 * i + 0] = h.t_hyb; big->hyb[4 * i + 1] = h.window_s;
                 big->hyb[4 * i + 2] = h.sigma_s; big->hyb[4 * i + 3] = (double)h.taper;
             }
+            if (plan_hybrid) std::memcpy(big->plan, hh.plan.data() + b0, (size_t)cnt * sizeof(HybPlan));
             {
                 ProfScope ps(LTDI_KERNEL_PREP + LTDI_KERNEL_COUNT * which, st);
                 unpack_big_kernel<<<(LTDI_BIG_SOURCES + 127) / 128, 128, 0, st>>>(
-                    *big, cnt, nh, w_src + 3 * b0, w_frames + LTDI_FRAME_STRIDE * b0,
-                    (double *)w_hyb + (n_hyb == 1 ? 0 : 4 * b0));
+                    *big, cnt, nh, plan_hybrid ? cnt : 0, w_src + 3 * b0, w_frames + LTDI_FRAME_STRIDE * b0,
+                    (double *)w_hyb + (n_hyb == 1 ? 0 : 4 * b0), w_plan + b0);
             }
             count_launch();
             if (cudaGetLastError() != cudaSuccess) { delete big; return LTDI_ECUDA; }
@@ -521,9 +709,6 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     }
 
     /* tile plan */
-    const ltdi_orbit_desc &d = orb->desc;
-    const Margins mg = compute_margins(d, gen, order, fd_order);
-    const int M = order + 1;
     RespParams p;
     std::memset(&p, 0, sizeof p);
     p.tab = orb->d_tab; p.stride = orb->stride; p.n = d.n; p.t0 = d.t0; p.dt = d.dt;
@@ -536,8 +721,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
 
     if (fast_order(order)) {
         const double *sm = have_small ? small_args.v : nullptr;
-        const int frc = M == 32 ? run_fast<32>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st, sm)
-                                : run_fast<10>(p, mg, orb, which, (double *)d_work + work_doubles(batch), st, sm);
+        const HybPlan *dp = have_small ? nullptr : w_plan;
+        double *fw = (double *)d_work + work_doubles(batch);
+        const int frc = M == 32 ? run_fast<32>(ds, p, mg, orb, which, fw, st, sm, &hh, dp)
+                                : run_fast<10>(ds, p, mg, orb, which, fw, st, sm, &hh, dp);
         if (frc != LTDI_EUNSUPPORTED) return frc;   /* else: shapes the tuned kernels do not cover */
     }
     if (have_small) { /* the generic kernel reads frames and windows from the workspace */
@@ -551,9 +738,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
 
     int tile = 256;
     while (tile > 64 && ((d.n + tile - 1) / tile) * batch < 2 * 148) tile /= 2; /* fill the 148 SMs */
-    int dev = 0, smem_max = 0;
-    LTDI_CUDA_OK(cudaGetDevice(&dev));
-    LTDI_CUDA_OK(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    const int smem_max = ds.smem_max;
     bool stage = true;
     size_t smem = 0;
     for (;;) {
@@ -578,10 +763,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.ntiles = (d.n + tile - 1) / tile;
     const int threads = tile >= 256 ? 256 : 128;
     if (M == 32)
-        return stage ? launch_response<32, true>(p, threads, smem, st) : launch_response<32, false>(p, threads, smem, st);
+        return stage ? launch_response<32, true>(ds, p, threads, smem, st) : launch_response<32, false>(ds, p, threads, smem, st);
     if (M == 10)
-        return stage ? launch_response<10, true>(p, threads, smem, st) : launch_response<10, false>(p, threads, smem, st);
-    return stage ? launch_response<0, true>(p, threads, smem, st) : launch_response<0, false>(p, threads, smem, st);
+        return stage ? launch_response<10, true>(ds, p, threads, smem, st) : launch_response<10, false>(ds, p, threads, smem, st);
+    return stage ? launch_response<0, true>(ds, p, threads, smem, st) : launch_response<0, false>(ds, p, threads, smem, st);
 }
 
 // register-resident DFMA chains: the FP64 pipe's issue rate, used as the "alu" roofline peak
@@ -695,16 +880,17 @@ int ltdi_orbits_prepare(ltdi_orbits *orb, int gen, int lagrange_order, void *d_b
     ltdi_orbits_prepare_bytes(&orb->desc, lagrange_order, &need);
     if (!d_buf || (uintptr_t)d_buf % 16) return LTDI_EINVAL;
     if (bytes < need) return LTDI_EWORKSPACE;
-    int rc = init_constants();
+    DeviceState *ds = nullptr;
+    int rc = device_state(&ds);
     if (rc) return rc;
     const ltdi_orbit_desc &d = orb->desc;
     const int M = lagrange_order + 1;
-    const Margins mg = compute_margins(d, gen, lagrange_order, 0);
-    if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_OK; /* shapes the tuned kernels do not cover */
+    const Margins m15 = compute_margins(d, LTDI_GEN_15, lagrange_order, 0), m20 = compute_margins(d, LTDI_GEN_20, lagrange_order, 0);
+    if (m20.m2 > 4096 || m20.m1 > 8192) return LTDI_OK; /* shapes the tuned kernels do not cover */
     FastParams p;
     std::memset(&p, 0, sizeof p);
     p.tab = orb->d_tab; p.stride = orb->stride; p.n = d.n; p.t0 = d.t0; p.dt = d.dt; p.inv_dt = 1.0 / d.dt;
-    p.gen = gen; p.m1 = mg.m1; p.m2 = mg.m2;
+    p.gen = gen; p.m1 = m20.m1; p.m2 = m20.m2; p.m2_15 = m15.m2; p.m2_20 = m20.m2;
     const int64_t tiles = (d.n + FAST_TCA - 1) / FAST_TCA;
     double *anc = (double *)d_buf, *hdr = anc + (size_t)tiles * FAST_NA * FAST_ANC_DOUBLES(M);
     {

@@ -9,7 +9,27 @@ import workloads as W
 
 TOL = 1e-11           # BASELINE.json north_star: per-channel relative L2 <= 1e-11 in fp64
 NEAR_NULL = 1e-6      # a channel this far below the largest one is judged against the largest
-FLOOR_FACTOR = 3.0    # bar = max(TOL, FLOOR_FACTOR x fp64 floor of the algorithm)
+GROSS = 1e-8          # full-size tests: bar on a single sampled window against its OWN norm (see pooled_check)
+
+# Cases that cannot meet TOL, with the reason; (substring of the pytest id, series) -> (floor the oracle's own
+# double build must show on that input -- asserted, so that the entry cannot outlive its reason --, bar).
+# One entry; every other parity case of tests/ meets 1e-11 (A, E, X, Y, Z, links) / 1e-11 of the largest channel (T).
+ALLOW = {
+    # dt = 0.05 s (a hundredth of LISA's sampling step, there to sweep the shared-memory plans down to the generic
+    # kernel): the projection delays are 1e4 SAMPLES, so the fractional delay eps = ceil(d / dt) - d / dt that O4
+    # defines carries 2e-12 samples of fp64 rounding whatever the implementation does; at the test signal (0.4 Hz,
+    # omega dt = 0.126) that is 2e-13 of h, and the second difference of the gen-2.0 LFA inside the hybrid amplifies it
+    # by 2.45 / (omega dt)^2 = 154.  The oracle's own double build shows 7e-11 there.
+    ("test_sampling_steps_sweep_the_shared_memory_plans[0.05]", "*"): (2e-11, 2e-10),   # A, E and X, Y, Z of the hybrid case
+}
+
+
+def allowance(series):
+    test = os.environ.get("PYTEST_CURRENT_TEST", "")
+    for (frag, ser), (floor_min, bar) in ALLOW.items():
+        if frag in test and ser in (series, "*"):
+            return floor_min, bar
+    return None
 
 
 def fp64_floor(ref80, ref64, lo, n, hi, keys=("A", "E", "T")):
@@ -91,3 +111,86 @@ def record(**row):
             f.write(json.dumps(row, default=float) + "\n")
     except OSError:
         pass
+
+
+def strict_check(out, ref, lo, hi, n, tol=TOL):
+    """The north-star bar, channel by channel over the non-margin samples, against the long-double oracle:
+    A, E: relative L2 <= 1e-11 (own norm); T = (X + Y + Z) / sqrt 3, which cancels at low frequency and is identically
+    0 for equal arms: L2 error <= 1e-11 of the largest channel's norm; X, Y, Z and the six links: L2 error <= 1e-11
+    of the largest series' norm.  ref may carry "floor" dicts (the oracle's double build against its long-double
+    build) -- they are recorded beside the achieved error, never used as a bar, except for entries of ALLOW."""
+    for c in "AET":   # margins are exactly zero
+        assert np.all(out[c][..., :lo] == 0.0) and np.all(out[c][..., n - hi:] == 0.0), c
+    norms = {c: float(np.linalg.norm(ref[c][..., lo:n - hi])) for c in "AET"}
+    top = max(norms.values())
+    errs = {}
+    for c in "AET":
+        d = float(np.linalg.norm((out[c] - ref[c])[..., lo:n - hi]))
+        vs_top = c == "T" or norms[c] < NEAR_NULL * top
+        den = top if vs_top else norms[c]
+        e = d / den if den > 0 else d
+        floor = ref.get("floor", {}).get(c)
+        bar, allow = tol, allowance(c)
+        if allow is not None and e > tol:   # the entry only counts where its reason shows
+            assert floor is not None and floor >= allow[0], (c, "allow-list entry without its floor", floor, allow)
+            bar = allow[1]
+        record(series=c, err=e, err_own_norm=(d / norms[c] if norms[c] > 0 else None), floor_own_norm=floor, bar=bar,
+               vs_largest_channel=bool(vs_top))
+        assert e <= bar, (c, e, bar)
+        errs[c] = e
+    for name in ("XYZ", "y"):
+        if out.get(name) is None or ref.get(name) is None:
+            continue
+        fl = ref.get("floor_" + name)
+        for i, e in enumerate(series_errors(out[name], ref[name], lo, n, hi)):
+            bar, allow = tol, allowance("%s%d" % (name, i))
+            if allow is not None and e > tol:
+                assert fl is not None and fl[i] >= allow[0], (name, i, fl, allow)
+                bar = allow[1]
+            record(series="%s%d" % (name, i), err=e, floor=None if fl is None else fl[i], bar=bar)
+            assert e <= bar, (name, i, e, bar)
+    return errs
+
+
+class Pooled:
+    """Full-size parity on sampled windows: the north-star metric restricted to the sampled outputs.  Per channel,
+    sqrt(sum over windows ||gpu - oracle||^2) / sqrt(sum over windows ||oracle||^2) <= 1e-11 (T against the largest
+    channel).  A whole-series norm would need the oracle on 1e6 .. 5e8 samples; the pooled norm over the windows is
+    smaller, so the test is the stricter one.  Each window is also held to GROSS against its own norm, so that a
+    wrong tile in a quiet part of the series (the early inspiral is 1e-4 of the merger) cannot hide in the pooled
+    norm; the per-window numbers and the fp64 floors are recorded."""
+
+    def __init__(self, label):
+        self.label = [str(x) for x in label]
+        self.err2 = {c: 0.0 for c in "AET"}
+        self.ref2 = {c: 0.0 for c in "AET"}
+
+    def add(self, got, ref80, ref64, nb, ne, lo, n, hi):
+        a, b = max(nb, lo), min(ne, n - hi)     # valid part of the window
+        norms = {c: float(np.linalg.norm(ref80[c][:, a - nb:b - nb])) for c in "AET"}
+        top = max(norms.values())
+        for c in "AET":
+            g = got[c][:, nb:ne]
+            assert np.all(g[:, :max(0, lo - nb)] == 0.0) and np.all(g[:, max(0, n - hi - nb):] == 0.0), (self.label, c, "margin")
+            if b <= a or top == 0.0:
+                continue
+            w80 = ref80[c][:, a - nb:b - nb]
+            d = float(np.linalg.norm(g[:, a - nb:b - nb] - w80))
+            self.err2[c] += d * d
+            self.ref2[c] += norms[c] ** 2
+            vs_top = c == "T" or norms[c] < NEAR_NULL * top
+            den = top if vs_top else norms[c]
+            floor = float(np.linalg.norm(ref64[c][:, a - nb:b - nb] - w80) / den) if ref64 is not None else None
+            record(label=self.label, series=c, window=[int(nb), int(ne)], err=d / den, floor=floor, bar=GROSS,
+                   vs_largest_channel=bool(vs_top))
+            assert d / den <= GROSS, (self.label, c, (nb, ne), d / den)
+
+    def check(self, tol=TOL):
+        top2 = max(self.ref2.values())
+        for c in "AET":
+            if top2 == 0.0:
+                continue
+            vs_top = c == "T" or self.ref2[c] < NEAR_NULL ** 2 * top2
+            e = (self.err2[c] / (top2 if vs_top else self.ref2[c])) ** 0.5
+            record(label=self.label, series=c, window="pooled", err=e, bar=tol, vs_largest_channel=bool(vs_top))
+            assert e <= tol, (self.label, c, "pooled over the sampled windows", e)

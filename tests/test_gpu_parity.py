@@ -6,8 +6,7 @@ import pytest
 import torch
 
 import workloads as W
-from parity_util import (FLOOR_FACTOR, TOL, channel_errors, fp64_floor, hybrid_params, record, series_errors,
-                         series_floor, to_numpy)
+from parity_util import TOL, fp64_floor, hybrid_params, record, series_floor, strict_check, to_numpy
 
 pytestmark = pytest.mark.gpu
 
@@ -65,24 +64,8 @@ def run_case(ltdi, orc, cfg, which, gen, fd, order=None, taper=W.TAPER_COSINE, i
 
 
 def check(out, ref, lo, hi, n, tol=TOL):
-    for c in "AET":   # margins are exactly zero
-        assert np.all(out[c][:, :lo] == 0.0) and np.all(out[c][:, n - hi:] == 0.0), c
-    # bar: 1e-11 per channel, or FLOOR_FACTOR x the error the oracle's own double build makes on this input
-    # where that is larger (T = (X+Y+Z)/sqrt 3 cancels; the gen-2.0 LFA second
-    # difference amplifies the rounding of y by 2.4 / (omega dt)^2)
-    errs = channel_errors(out, ref, lo, n, hi)
-    top = max(np.linalg.norm(ref[c][..., lo:n - hi]) for c in "AET")
-    for c, (e, near_null) in errs.items():
-        bar = tol if near_null else max(tol, FLOOR_FACTOR * ref["floor"][c])
-        e_top = float(np.linalg.norm((out[c] - ref[c])[..., lo:n - hi]) / top) if top > 0 else 0.0
-        record(series=c, err=e, err_vs_top=e_top, floor=ref["floor"][c], bar=bar, near_null=bool(near_null))
-        assert e <= bar, (c, e, bar, "near-null" if near_null else "")
-    for name in ("XYZ", "y"):
-        for i, e in enumerate(series_errors(out[name], ref[name], lo, n, hi)):
-            bar = max(tol, FLOOR_FACTOR * ref["floor_" + name][i])
-            record(series="%s%d" % (name, i), err=e, floor=ref["floor_" + name][i], bar=bar)
-            assert e <= bar, (name, i, e, bar)
-    return errs
+    """1e-11 per channel (T against the largest channel) and per link / Michelson series: parity_util.strict_check"""
+    return strict_check(out, ref, lo, hi, n, tol)
 
 
 def test_orbit_delay_kernel(ltdi, orc80):
@@ -273,7 +256,10 @@ def test_sampling_steps_sweep_the_shared_memory_plans(ltdi, orc80, dt):
     lo_max = max(orc80.margins(W.orbit_desc(10, dt), 20, 31, 4))
     n = int(2 * lo_max + 1500) if dt >= 0.5 else int(2 * lo_max + 300)
     orbit = W.orbit_desc(n, dt, W.ORBIT_KEPLERIAN, t0=1.234e7)
-    f = 0.02 / dt if dt >= 0.5 else 2.0e-2        # well sampled, not so low that the TDI output is rounding noise
+    # well sampled (50 samples per cycle), but never below 2 mHz: the full TDI 2.0 response cancels as (omega L / c)^3
+    # at low frequency and NO fp64 evaluation meets 1e-11 there (the oracle's own double build: 1e-11 at 0.7 mHz,
+    # 1e-9 at 0.1 mHz, hard part 1) -- which is the regime the paper gives to the LFA
+    f = max(0.02 / dt, 2.0e-3)
     hp0, hc0 = W.monochromatic(n, dt, f, t0=orbit["t0"])
     hp1, hc1 = W.monochromatic(n, dt, 0.6 * f, a_plus=0.4, a_cross=-1.1, phi_p=2.0, phi_c=0.1, t0=orbit["t0"])
     hp, hc = np.stack([hp0, hp1]), np.stack([hc0, hc1])
@@ -427,4 +413,5 @@ def test_decayed_ringdown_tail_keeps_relative_accuracy(ltdi, orc80):
                 nrm = np.linalg.norm(w80)
                 assert nrm > 0
                 err, floor = np.linalg.norm(g - w80) / nrm, np.linalg.norm(w64 - w80) / nrm
-                assert err <= max(TOL, FLOOR_FACTOR * floor), (which, c, (a, b), err, floor)
+                record(label=[which], series=c, window=[int(a), int(b)], err=float(err), floor=float(floor), bar=TOL)
+                assert err <= TOL, (which, c, (a, b), err, floor)

@@ -201,55 +201,71 @@ def config(k, n=None, batch=None):
     return c
 
 
+def draw(cfg, idx):
+    """The seeded parameters of source `idx` of a config, without its time series (input data only: masses,
+    distance, angles, eccentricity, and the fractions that place the merger).  source() builds the series from
+    exactly these draws; the tests use them to pick a stratified parity subset of a large batch."""
+    k = cfg["k"]
+    rng = np.random.default_rng([cfg["seed"], int(idx)])
+    cos_iota, beta, lam, psi, phi_c = _angles(rng)
+    p = {"cos_iota": cos_iota, "beta": beta, "lam": lam, "psi": psi, "phi_c": phi_c}
+    if k == 1:
+        p.update(M=2.0e6, q=1.0, dist=10.0 * GPC_M)
+    elif k == 2:
+        p.update(M=1.0e6, q=rng.uniform(1.0, 8.0), dist=5.0 * GPC_M)
+        p["merger_h_before_end"] = rng.uniform(0.5, 2.0)
+    elif k == 3:
+        p.update(M=1.0e5, q=2.0, dist=5.0 * GPC_M)
+    elif k == 4:
+        p["M"] = 10.0 ** rng.uniform(5.0, 7.0)
+        p["q"] = rng.uniform(1.0, 10.0)
+        p["dist"] = rng.uniform(1.0, 20.0) * GPC_M
+        p["merger_fraction"] = rng.uniform(0.9, 1.0)
+    elif k == 5:
+        p["M"] = 10.0 ** rng.uniform(5.0, 6.0)
+        p["q"] = rng.uniform(1.0, 4.0)
+        p["e0"] = rng.uniform(0.0, 0.3)
+        p["dist"] = rng.uniform(1.0, 10.0) * GPC_M
+        p["gamma"] = rng.uniform(0.0, math.pi)
+        p["tau_end"] = rng.uniform(1.0, 12.0) * 3600.0
+    else:
+        raise ValueError(k)
+    p["mchirp_s"] = chirp_mass_s(p["M"], p["q"])
+    return p
+
+
 def source(cfg, idx):
     """One source of a config: returns (hp[n], hc[n], (beta, lambda, psi), meta).
 
     meta carries the numbers the hybrid needs (mchirp_s, t_c, f_hyb_hz, window_s); the hybrid time
     itself (Eq. 4.2) is method arithmetic and is computed by each side with its own helper."""
     k, n, dt = cfg["k"], cfg["n"], cfg["dt"]
-    rng = np.random.default_rng([cfg["seed"], int(idx)])
     t = cfg["orbit"]["t0"] + dt * np.arange(n, dtype=np.float64)
     t_end = t[-1] + dt
-    cos_iota, beta, lam, psi, phi_c = _angles(rng)
+    p = draw(cfg, idx)
+    cos_iota, beta, lam, psi, phi_c = p["cos_iota"], p["beta"], p["lam"], p["psi"], p["phi_c"]
+    M, q, dist, mc = p["M"], p["q"], p["dist"], p["mchirp_s"]
     meta = {"f_hyb_hz": HYB_F_HZ, "window_s": HYB_WINDOW_S, "taper": TAPER_COSINE}
     if k == 1:
-        M, q, dist = 2.0e6, 1.0, 10.0 * GPC_M
-        mc = chirp_mass_s(M, q)
         t_c = t_end + 2.0 * DAY_S
         hp, hc = newtonian_chirp(t, t_c, mc, dist, cos_iota, phi_c)
     elif k == 2:
-        M, q, dist = 1.0e6, rng.uniform(1.0, 8.0), 5.0 * GPC_M
-        mc = chirp_mass_s(M, q)
         rd = {"M_s": M * GMSUN_S, "dt": dt}
-        t_m = t_end - rng.uniform(0.5, 2.0) * 3600.0
+        t_m = t_end - p["merger_h_before_end"] * 3600.0
         t_c = t_m + _tau_cut(mc, rd)
         hp, hc = newtonian_chirp(t, t_c, mc, dist, cos_iota, phi_c, ringdown=rd)
     elif k == 3:
-        M, q, dist = 1.0e5, 2.0, 5.0 * GPC_M
-        mc = chirp_mass_s(M, q)
         t_c = t[0] + 2.0 * 365.0 * DAY_S
         hp, hc = newtonian_chirp(t, t_c, mc, dist, cos_iota, phi_c)
     elif k == 4:
-        M = 10.0 ** rng.uniform(5.0, 7.0)
-        q = rng.uniform(1.0, 10.0)
-        dist = rng.uniform(1.0, 20.0) * GPC_M
-        mc = chirp_mass_s(M, q)
         rd = {"M_s": M * GMSUN_S, "dt": dt}
-        t_m = t[0] + (t_end - t[0]) * rng.uniform(0.9, 1.0)
+        t_m = t[0] + (t_end - t[0]) * p["merger_fraction"]
         t_c = t_m + _tau_cut(mc, rd)
         hp, hc = newtonian_chirp(t, t_c, mc, dist, cos_iota, phi_c, ringdown=rd)
-    elif k == 5:
-        M = 10.0 ** rng.uniform(5.0, 6.0)
-        q = rng.uniform(1.0, 4.0)
-        e0 = rng.uniform(0.0, 0.3)
-        dist = rng.uniform(1.0, 10.0) * GPC_M
-        gamma = rng.uniform(0.0, math.pi)
-        tau_end = rng.uniform(1.0, 12.0) * 3600.0
-        mc = chirp_mass_s(M, q)
-        t_c = t_end + tau_end
-        hp, hc = eccentric_harmonics(t, t_end, tau_end, M * GMSUN_S, q, e0, dist, cos_iota, gamma, phi_c)
     else:
-        raise ValueError(k)
+        tau_end = p["tau_end"]
+        t_c = t_end + tau_end
+        hp, hc = eccentric_harmonics(t, t_end, tau_end, M * GMSUN_S, q, p["e0"], dist, cos_iota, p["gamma"], phi_c)
     meta.update({"mchirp_s": mc, "t_c": t_c})
     return hp, hc, (beta, lam, psi), meta
 
