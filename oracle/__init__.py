@@ -156,6 +156,18 @@ class Oracle:
         assert rc == 0
         return nh, nl, Lh, Ll
 
+    def michelson_from_links(self, orbit, y, gen, order):
+        """X, Y, Z [3][n] of Eq. (2.7) / (2.8) from caller-supplied link series y [6][n]."""
+        y = _f64(y)
+        assert y.shape == (6, orbit["n"])
+        out = np.zeros((3, orbit["n"]))
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_michelson_from_links(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(y), C.c_int(gen), C.c_int(order),
+                                               _ptr(out))
+        assert rc == 0
+        return out
+
     def antenna(self, orbit, source, n):
         out = np.zeros((6, 3))
         d = self._desc(orbit)

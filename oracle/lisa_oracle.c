@@ -722,6 +722,36 @@ void orc_hybrid_weights(const orc_hybrid *h, const double *t, int64_t len, doubl
     }
 }
 
+/* Michelson X, Y, Z of Eq. (2.7) / (2.8) from CALLER-SUPPLIED link series y [6][n] (link order +1,+2,+3,-1,-2,-3):
+ * michelson_at() on every sample of the valid range [lo, n - hi) of margins(); XYZ [3][n], zero in the margins.
+ * Lets a test plant sentinels in the margin samples of y and see that no valid output reads them (O10, G11). */
+int orc_michelson_from_links(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *y,
+                             int gen, int order, double *XYZ)
+{
+    if (check_args(d, gen, order, 0, 0, d ? d->n : 0, 0, d ? d->n : 0) || !y || !XYZ) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, 0, &mg);
+    const int64_t N = d->n;
+    real *yr[6];
+    for (int l = 0; l < 6; ++l) {
+        if (!(yr[l] = (real *)malloc(sizeof(real) * (size_t)N))) return ORC_EINVAL;
+        for (int64_t i = 0; i < N; ++i) yr[l][i] = y[(int64_t)l * N + i];
+    }
+    yseries_t ys = { { yr[0], yr[1], yr[2], yr[3], yr[4], yr[5] }, 0, N };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int c = 0; c < 3; ++c) XYZ[(int64_t)c * N + n] = 0.0;
+        if (n < mg.lo || n >= N - mg.hi) continue;
+        geom_t g;
+        orbit_geometry(&o, n, &g);
+        for (int c = 0; c < 3; ++c)
+            XYZ[(int64_t)c * N + n] = (double)michelson_at(&ys, g.L, c, gen, n, (real)d->dt, order);
+    }
+    for (int l = 0; l < 6; ++l) free(yr[l]);
+    return ORC_OK;
+}
+
 /*
  * Full response (O5-O7).  hp, hc: [batch][ld]; outputs: A,E,T [batch][ne-nb],
  * XYZ [3][batch][ne-nb], y [6][batch][ne-nb]; any may be NULL.

@@ -10,6 +10,7 @@
 #include <stdlib.h>
 
 #include "../../include/lisatdi.h"
+#include "../../include/lisatdi_bench.h"
 
 #define LTDI_C_LIGHT 299792458.0 /* m/s */
 #define LTDI_MAX_TAPS 64

@@ -114,6 +114,35 @@ __device__ __forceinline__ void cp_async16(void *dst_smem, const void *src)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// TMA 1-D bulk copies (cp.async.bulk) completing on an mbarrier: ONE thread moves a whole row, the other threads
+// spend no instruction on staging (the per-element cp.async loops of the TDI kernel were a third of its executed
+// instructions, ncu r02a).  Addresses and sizes are multiples of 16 bytes.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+
 // s = d / dt to within one rounding of the correctly rounded quotient (one Newton correction)
 __device__ __forceinline__ double div_dt(double d, double dt, double inv_dt)
 {
@@ -803,7 +832,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
      *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
      *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0, even)
      *   Lr   [NLR][FAST_TC] light times L_l(n0 + i) of the tile; after the term loop: X, Y, Z of the tile
-     *   yL   [3][yr + 2w] LFA links       (element 0 = sample y0 - w) */
+     *   yL   [3][yr + 4] LFA links        (element 0 = sample y0 - 2) */
     const int yr = tdi_yr<M>(FAST_TC, p.m2);
     const int64_t y0 = n0 - tdi_back(p.m2);
     constexpr int na_full = has_full ? FAST_NA_FULL : 0;
@@ -812,110 +841,108 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     double *dL = yF + (has_full ? 6 * yr : 0);
     double *Lr = dL + (has_lfa ? 3 * yr : 0);
     double *yL = Lr + NLR * FAST_TC;
+    const int slen = yr + 4;   /* staged LFA links: samples [y0 - 2, y0 + yr + 2), an even start for 16-byte rows */
     /* X, Y, Z exchange: its own region (full, LFA: no barrier between the term loop and the exchange), or on top of
      * the light times (hybrid: six rows, and the shared memory of two responses) */
     constexpr bool xs_alias = WHICH == LTDI_RESPONSE_HYBRID;
-    double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * (yr + 2 * w) : 0);
+    double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * slen : 0);
     const double *sa_lfa = sa + (size_t)na_full * ANC;
     const int lfa_a0 = p.gen == LTDI_GEN_15 ? 0 : FAST_NA_LFA_GEN;   /* first LFA anchor of this generation */
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
-    __shared__ double s_hdr[FAST_NA * 4];
+    __shared__ __align__(16) double s_hdr[FAST_NA * 4];
+    __shared__ uint64_t s_bar;
 
-    /* phase 0: every global read of the tile is issued asynchronously, then one wait (row loops: no integer
-     * division in the index arithmetic) */
-#pragma unroll 1
-    for (int l = 0; l < NLR; ++l) {
-        const double *src = tabL + l * p.stride;
-        for (int k = 2 * tid; k < FAST_TC; k += 2 * FAST_TC_THREADS) {
-            if (n0 + k + 1 < p.n) cp_async16(Lr + l * FAST_TC + k, src + n0 + k);
-            else {
-                Lr[l * FAST_TC + k] = src[min(n0 + k, p.n - 1)];
-                Lr[l * FAST_TC + k + 1] = src[p.n - 1];
-            }
-        }
+    /* phase 0: thread 0 issues one TMA bulk copy per staged row (clipped to the rows' allocations), everybody waits
+     * on the mbarrier.  What lies before the series is zero-filled; what lies behind it (scratch never written) only
+     * reaches margin outputs, which are overwritten with 0. */
+    if (tid == 0) {
+        mbar_init(&s_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (has_full && need_full) {
+    const int64_t g0 = max(y0, (int64_t)0), g1 = min(y0 + yr, p.lds);                  /* full links, even bounds */
+    const int64_t h0 = max(y0 - 2, (int64_t)0), h1 = min(y0 - 2 + slen, p.lds);         /* LFA links */
+    const int nyF = (int)max(g1 - g0, (int64_t)0), nyL = (int)max(h1 - h0, (int64_t)0);
+    const int nl = (int)max(min((int64_t)FAST_TC, p.stride - n0), (int64_t)0);
+    if (has_full && (y0 < 0 || nyF < yr))
+        for (int k = tid; k < 6 * yr; k += FAST_TC_THREADS) {
+            const int c = k % yr;
+            if (c < g0 - y0 || c >= g0 - y0 + nyF) yF[k] = 0.0;
+        }
+    if (has_lfa && (y0 - 2 < 0 || nyL < slen))
+        for (int k = tid; k < 3 * slen; k += FAST_TC_THREADS) {
+            const int c = k % slen;
+            if (c < h0 - (y0 - 2) || c >= h0 - (y0 - 2) + nyL) yL[k] = 0.0;
+        }
+    __syncthreads();   /* the barrier is initialised, the zero fill is visible */
+    if (tid == 0) {
         const int64_t ystride = p.batch * p.lds;
-#pragma unroll 1
-        for (int l = 0; l < 6; ++l) {
-            const double *src = p.yF + b * p.lds + l * ystride;
-            double *dst = yF + l * yr;
-            for (int k = 2 * tid; k < yr; k += 2 * FAST_TC_THREADS) {
-                const int64_t g = y0 + k;
-                if (g >= 0 && g + 1 < p.n) cp_async16(dst + k, src + g);
-                else {
-                    dst[k] = (g >= 0 && g < p.n) ? src[g] : 0.0;
-                    dst[k + 1] = (g + 1 >= 0 && g + 1 < p.n) ? src[g + 1] : 0.0;
-                }
-            }
-        }
-    }
-    if (has_lfa && need_lfa) {
-        const int64_t ystride = p.batch * p.lds;
-        const int len = yr + 2 * w;
-#pragma unroll 1
-        for (int l = 0; l < 3; ++l) {
-            const double *src = p.yL + b * p.lds + l * ystride;
-            double *dst = yL + l * len;
-            for (int k = tid; k < len; k += FAST_TC_THREADS) {
-                const int64_t g = y0 - w + k;
-                if (g >= 0 && g < p.n) cp_async8(dst + k, src + g);
-                else dst[k] = 0.0;
-            }
-        }
-    }
-    {
         const int64_t atile = tile / FAST_TCA_TILES;
         const double *ga = p.anc + atile * (int64_t)(FAST_NA * ANC);
-        if (has_full && need_full)
-            for (int i = tid; i < FAST_NA_FULL * ANC / 2; i += FAST_TC_THREADS)
-                cp_async16(sa + 2 * i, ga + 2 * i);
-        if (has_lfa && need_lfa)   /* the six LFA anchors of this generation */
-            for (int i = tid; i < FAST_NA_LFA_GEN * ANC / 2; i += FAST_TC_THREADS)
-                cp_async16(sa + (size_t)na_full * ANC + 2 * i, ga + (FAST_NA_FULL + lfa_a0) * ANC + 2 * i);
-        for (int i = tid; i < FAST_NA * 4; i += FAST_TC_THREADS) s_hdr[i] = p.anc_hdr[atile * (FAST_NA * 4) + i];
+        mbar_expect_tx(&s_bar, (unsigned)(((has_full ? 6 * nyF + FAST_NA_FULL * ANC : 0) + (has_lfa ? 3 * nyL + FAST_NA_LFA_GEN * ANC : 0) +
+                                           NLR * nl + FAST_NA * 4) * sizeof(double)));
+#pragma unroll 1
+        for (int l = 0; l < NLR; ++l)
+            if (nl > 0) bulk_g2s(Lr + l * FAST_TC, tabL + l * p.stride + n0, nl * 8u, &s_bar);
+        if (has_full) {
+#pragma unroll 1
+            for (int l = 0; l < 6; ++l)
+                if (nyF > 0) bulk_g2s(yF + l * yr + (g0 - y0), p.yF + b * p.lds + l * ystride + g0, nyF * 8u, &s_bar);
+            bulk_g2s(sa, ga, FAST_NA_FULL * ANC * 8u, &s_bar);
+        }
+        if (has_lfa) {
+#pragma unroll 1
+            for (int l = 0; l < 3; ++l)
+                if (nyL > 0) bulk_g2s(yL + l * slen + (h0 - (y0 - 2)), p.yL + b * p.lds + l * ystride + h0, nyL * 8u, &s_bar);
+            bulk_g2s(sa + (size_t)na_full * ANC, ga + (FAST_NA_FULL + lfa_a0) * ANC, FAST_NA_LFA_GEN * ANC * 8u, &s_bar);   /* this generation's six */
+        }
+        bulk_g2s(s_hdr, p.anc_hdr + atile * (FAST_NA * 4), FAST_NA * 4 * 8u, &s_bar);
     }
-    cp_async_wait_all();
-    __syncthreads();
+    mbar_wait(&s_bar, 0);
 
     /* phase 1 (LFA, hybrid): derivative of the LFA links */
     if (has_lfa) {
-        if (need_lfa) {
-            /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range.  A thread takes
-             * runs of FD_RUN consecutive samples of one link and slides a register window over them. */
-            constexpr int FD_RUN = 4;
-            const int len = yr + 2 * w;
-            const int runs = (yr + FD_RUN - 1) / FD_RUN;
-            const bool g15 = p.gen == LTDI_GEN_15;
-            const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
+        /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range.  A thread takes runs of
+         * eight consecutive samples of one link and slides a register window over them; tiles away from the ends of
+         * the series (all but two per source) take the branch without per-sample range checks. */
+        constexpr int FD_RUN = 8;
+        const int runs = (yr + FD_RUN - 1) / FD_RUN;
+        const bool g15 = p.gen == LTDI_GEN_15;
+        const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
+        const bool interior = y0 >= p.m1 + 2 * w && y0 + yr <= p.n - p.m1 - 2 * w;
 #pragma unroll 1
-            for (int idx = tid; idx < 3 * runs; idx += FAST_TC_THREADS) {   /* (link, run) pairs, evenly over the threads */
-                {
-                    const int l = idx / runs, run = idx - l * runs;
-                    const int k0 = run * FD_RUN;
-                    const double *x = yL + l * len + k0;   /* x[j] = sample y0 - w + k0 + j */
-                    double v[FD_RUN + 4];
+        for (int idx = tid; idx < 3 * runs; idx += FAST_TC_THREADS) {   /* (link, run) pairs, evenly over the threads */
+            const int l = idx / runs, k0 = (idx - l * runs) * FD_RUN;
+            const double *x = yL + l * slen + k0;   /* x[j] = sample y0 - 2 + k0 + j */
+            double *o = dL + l * yr + k0;
+            double v[FD_RUN + 4];
+            const bool whole = interior && k0 + FD_RUN <= yr;
+            if (whole) {
 #pragma unroll
-                    for (int j = 0; j < FD_RUN + 4; ++j) v[j] = (j < FD_RUN + 2 * w && k0 + j < len) ? x[j] : 0.0;
+                for (int j = 0; j < FD_RUN + 4; ++j) v[j] = x[j];
+            } else {
 #pragma unroll
-                    for (int j = 0; j < FD_RUN; ++j) {
-                        const int k = k0 + j;
-                        if (k >= yr) break;
-                        const int64_t m = y0 + k;
-                        const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
-                        double d;
-                        if (w == 1) {   /* centre v[j + 1] */
-                            d = g15 ? (v[j + 2] - v[j]) : ((v[j + 2] - v[j + 1]) - (v[j + 1] - v[j]));
-                        } else {        /* centre v[j + 2] */
-                            if (g15) d = 8.0 * (v[j + 3] - v[j + 1]) - (v[j + 4] - v[j]);
-                            else {
-                                const double d1 = (v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]);
-                                const double d2 = (v[j + 4] - v[j + 2]) - (v[j + 2] - v[j]);
-                                d = 16.0 * d1 - d2;
-                            }
-                        }
-                        dL[l * yr + k] = in ? d * scale : 0.0;
-                    }
+                for (int j = 0; j < FD_RUN + 4; ++j) v[j] = (k0 + j < slen) ? x[j] : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < FD_RUN; ++j) {
+                double d;   /* centre v[j + 2] */
+                if (w == 1) d = g15 ? (v[j + 3] - v[j + 1]) : ((v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]));
+                else if (g15) d = 8.0 * (v[j + 3] - v[j + 1]) - (v[j + 4] - v[j]);
+                else {
+                    const double d1 = (v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]);
+                    const double d2 = (v[j + 4] - v[j + 2]) - (v[j + 2] - v[j]);
+                    d = 16.0 * d1 - d2;
+                }
+                v[j] = d * scale;   /* v[j] is not read again */
+            }
+            if (whole) {
+#pragma unroll
+                for (int j = 0; j < FD_RUN; ++j) o[j] = v[j];
+            } else {
+#pragma unroll
+                for (int j = 0; j < FD_RUN; ++j) {
+                    const int64_t m = y0 + k0 + j;
+                    if (k0 + j < yr) o[j] = (m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w) ? v[j] : 0.0;
                 }
             }
         }
@@ -1107,7 +1134,7 @@ static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
     size_t dbl = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0)) * FAST_ANC_DOUBLES(M);
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
     dbl += (size_t)(has_full ? 6 : 3) * tdi_tc(which);
-    dbl += has_lfa ? 3 * (yr + 2 * (size_t)w) : 0;
+    dbl += has_lfa ? 3 * (yr + 4) : 0;
     dbl += which == LTDI_RESPONSE_HYBRID ? 0 : (size_t)3 * tdi_tc(which);   /* X, Y, Z exchange */
     return dbl * sizeof(double);
 }

@@ -69,18 +69,38 @@ def check(out, ref, lo, hi, n, tol=TOL):
 
 
 def test_orbit_delay_kernel(ltdi, orc80):
-    """S0: tables against the oracle's orbit (differences come from sincos rounding only)"""
-    for mode in (W.ORBIT_KEPLERIAN, W.ORBIT_STATIC_EQUALARM):
-        orbit = W.orbit_desc(70001, 5.0, mode, t0=1.0e7, alpha0=0.3, rot0=1.1)
+    """S0: positions to one fp64 rounding; link vectors and light times as hi + lo pairs to 2e-17 (the oracle's own
+    long-double rounding of R_r - R_s is 4e-18): the double-double orbit kernel.  Late in the mission (t = 1 yr) the
+    fp64 rounding of t_n alone would be 7e-16 in n_l."""
+    for mode, t0 in ((W.ORBIT_KEPLERIAN, 1.0e7), (W.ORBIT_KEPLERIAN, 3.1e7), (W.ORBIT_STATIC_EQUALARM, 1.0e7)):
+        orbit = W.orbit_desc(70001, 5.0, mode, t0=t0, alpha0=0.3, rot0=1.1)
         R, nh, L = orc80.orbit_tables(orbit)
-        rows = ltdi.Orbits(orbit).rows().cpu().numpy()
-        # alpha = Omega t + alpha0 is rounded to fp64 on the GPU (the oracle carries it in long double):
-        # |d alpha| <= 2 eps |alpha|, hence |dR| <= 2 eps (1 + |alpha|) R (DESIGN.md, tolerances)
-        alpha_max = 2.0 * np.pi * (orbit["t0"] + orbit["n"] * orbit["dt"]) / orbit["period_s"] + orbit["alpha0"]
-        assert np.abs(rows[0:9].reshape(3, 3, -1) - R).max() <= 2 * 2.3e-16 * (1 + alpha_max) * np.abs(R).max()
-        assert np.abs(rows[9:18].reshape(3, 3, -1) - nh[:3]).max() <= 2e-14
-        assert np.abs(rows[18:24] - L).max() <= 1e-14 * L.max()
+        nh_hi, nh_lo, L_hi, L_lo = orc80.orbit_tables_split(orbit)
+        orb = ltdi.Orbits(orbit)
+        rows, lo = orb.rows().cpu().numpy(), orb.rows_lo().double().cpu().numpy()
+        assert np.abs(rows[0:9].reshape(3, 3, -1) - R).max() <= np.spacing(np.abs(R).max())     # 3e-5 m at 1 AU
+        dn = (rows[9:18].reshape(3, 3, -1) - nh_hi[:3]) + (lo[0:9].reshape(3, 3, -1) - nh_lo[:3])
+        dL = (rows[18:24] - L_hi) + (lo[9:15] - L_lo)
+        assert np.abs(dn).max() <= 2e-17, np.abs(dn).max()
+        assert np.abs(dL).max() <= 2e-17 * L.max(), np.abs(dL).max() / L.max()
+        assert np.abs(rows[9:18].reshape(3, 3, -1) - nh[:3]).max() <= 1.2e-16       # the hi parts alone: one rounding
         assert np.array_equal(nh[3:], -nh[:3])        # n_-l = -n_l is what the table layout assumes
+
+
+def test_orbit_tables_mode_link_vectors(ltdi, orc80):
+    """LTDI_ORBIT_TABLES: n_l = (R_r - R_s) / |R_r - R_s| from the caller's fp64 positions, formed without rounding the
+    difference; light times passed through (low parts zero)"""
+    n = 5000
+    base = W.orbit_desc(n, 5.0, W.ORBIT_KEPLERIAN, t0=2.0e6)
+    R, _, L = orc80.orbit_tables(base)
+    orbit = dict(base, mode=W.ORBIT_TABLES, R_table=np.ascontiguousarray(R), L_table=np.ascontiguousarray(L))
+    nh_hi, nh_lo, L_hi, L_lo = orc80.orbit_tables_split(orbit)
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, torch.from_numpy(orbit["R_table"]).to(dev), torch.from_numpy(orbit["L_table"]).to(dev))
+    rows, lo = orb.rows().cpu().numpy(), orb.rows_lo().double().cpu().numpy()
+    dn = (rows[9:18].reshape(3, 3, -1) - nh_hi[:3]) + (lo[0:9].reshape(3, 3, -1) - nh_lo[:3])
+    assert np.abs(dn).max() <= 2e-17
+    assert np.array_equal(rows[18:24], L) and np.all(lo[9:15] == 0.0) and np.array_equal(rows[0:9].reshape(3, 3, -1), R)
 
 
 def test_config1_full_tdi15(ltdi, orc80):

@@ -480,3 +480,49 @@ def test_range_evaluation_equals_full_evaluation(orc80):
         for key in ("A", "E", "T"):
             assert np.array_equal(whole[k][key][:, 700:760], part[k][key])
         assert np.array_equal(whole[k]["y"][:, :, 700:760], part[k]["y"])
+
+
+# ---------------------------------------------------------------------------------------------
+# O10 margins (G11): no valid output reads a margin sample
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("gen", [15, 20])
+@pytest.mark.parametrize("order,dt", [(31, 5.0), (9, 10.0), (31, 1.7)])
+def test_valid_michelson_samples_never_read_the_link_margins(orc80, gen, order, dt):
+    """Plant a sentinel in every margin sample of the link series (n < m1 or n >= N - m1, orc_link_margins): X, Y, Z
+    on the valid range [lo, N - hi) of orc_margins must not change by a bit.  Fails if the TDI reach of O10 is too
+    short for the largest delay of Eq. (2.7) / (2.8) (3 resp. 7 light times plus half a stencil) or if the forward
+    stencil half overruns hi."""
+    lo, hi = orc80.margins(W.orbit_desc(10, dt), gen, order, 0)
+    n = lo + hi + 700
+    orbit = W.orbit_desc(n, dt, W.ORBIT_KEPLERIAN, t0=4.0e6)
+    ylo, yhi = orc80.link_margins(orbit, order, 0)
+    rng = np.random.default_rng(5)
+    y = rng.standard_normal((6, n))
+    ref = orc80.michelson_from_links(orbit, y, gen, order)
+    y2 = y.copy()
+    y2[:, :ylo] = 1.0e30
+    y2[:, n - yhi:] = -1.0e30
+    got = orc80.michelson_from_links(orbit, y2, gen, order)
+    assert np.array_equal(got[:, lo:n - hi], ref[:, lo:n - hi])
+    assert np.all(got[:, :lo] == 0.0) and np.all(got[:, n - hi:] == 0.0)
+    # and the bound is not vacuous: one more valid sample at the front would read the sentinel for gen 2.0 ...
+    # (the reach 7.2 L / c + M / 2 exceeds the largest delay by < 0.3 L / c + stencil slack), checked loosely:
+    assert lo - ylo < (7.2 if gen == 20 else 3.1) * (orbit["arm_m"] / W.C_LIGHT) / dt + order + 3
+
+
+def test_link_quantities_split_as_hi_plus_lo(orc80):
+    """orc_orbit_tables_split: hi is the fp64 rounding of the long-double n_l, L_l; |lo| <= ulp(hi) / 2; the plain
+    tables are the hi parts"""
+    orbit = W.orbit_desc(2001, 5.0, W.ORBIT_KEPLERIAN, t0=1.0e7)
+    nh, nl, Lh, Ll = orc80.orbit_tables_split(orbit)
+    _, n_plain, L_plain = orc80.orbit_tables(orbit)
+    assert np.array_equal(nh, n_plain) and np.array_equal(Lh, L_plain)
+    assert np.all(np.abs(nl) <= 0.5 * np.spacing(np.abs(nh)) + 1e-300) and np.all(np.abs(Ll) <= 0.5 * np.spacing(Lh))
+    assert np.abs(nl).max() > 1e-18          # the long double build really carries more digits
+    # unit vectors to beyond fp64: |n|^2 - 1 from the split pieces (exact products via math.fsum)
+    import math
+    for l in range(3):
+        for i in (0, 1000, 2000):
+            h, lw = nh[l, :, i], nl[l, :, i]
+            s = math.fsum([h[0] * h[0], h[1] * h[1], h[2] * h[2], 2 * h[0] * lw[0], 2 * h[1] * lw[1], 2 * h[2] * lw[2], -1.0])
+            assert abs(s) < 2e-16            # products rounded to fp64 in this check; the split itself is at 1e-19
