@@ -222,6 +222,40 @@ class Oracle:
                      want=("XYZ", "y")):
         return self._run("lfa", orbit, hp, hc, sources, gen, order, fd_order, None, nb, ne, want)
 
+    def stencil3(self, x, dt, fd_order):
+        x = _f64(x)
+        out = np.zeros_like(x)
+        self.lib.orc_stencil3(_ptr(x), C.c_int64(len(x)), C.c_double(dt), fd_order, _ptr(out))
+        return out
+
+    def margins_lfa_ext(self, orbit, gen, order, fd_order, terms=1):
+        lo, hi = C.c_int64(), C.c_int64()
+        d = self._desc(orbit)
+        assert self.lib.orc_margins_lfa_ext(C.byref(d), gen, order, fd_order, terms, C.byref(lo), C.byref(hi)) == 0
+        return lo.value, hi.value
+
+    def response_lfa_ext(self, orbit, hp, hc, sources, gen, order, fd_order, terms=1, point=0, nb=0, ne=None,
+                         want=("XYZ", "y")):
+        """`terms` terms of Eq. (B4) about the expansion point (0 central, 1 backward, 2 forward)."""
+        hp, hc = np.atleast_2d(_f64(hp)), np.atleast_2d(_f64(hc))
+        batch, ld = hp.shape
+        src, ns = self._sources(sources)
+        assert ns == batch and ld >= orbit["n"]
+        ne = orbit["n"] if ne is None else ne
+        ln = ne - nb
+        out = {"A": np.zeros((batch, ln)), "E": np.zeros((batch, ln)), "T": np.zeros((batch, ln))}
+        out["XYZ"] = np.zeros((3, batch, ln)) if "XYZ" in want else None
+        out["y"] = np.zeros((6, batch, ln)) if "y" in want else None
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_response_lfa_ext(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(hp), _ptr(hc), C.c_int64(ld),
+                                           C.c_int64(batch), src, C.c_int(gen), C.c_int(order), C.c_int(fd_order),
+                                           C.c_int(terms), C.c_int(point), C.c_int64(nb), C.c_int64(ne), _ptr(out["A"]),
+                                           _ptr(out["E"]), _ptr(out["T"]), _ptr(out["XYZ"]), _ptr(out["y"]))
+        if rc != 0:
+            raise ValueError(f"oracle lfa_ext: status {rc}")
+        return out
+
     def response_hybrid(self, orbit, hp, hc, sources, gen, order, fd_order, hyb, nb=0, ne=None,
                         want=("XYZ", "y")):
         return self._run("hybrid", orbit, hp, hc, sources, gen, order, fd_order, hyb, nb, ne, want)

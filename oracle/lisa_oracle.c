@@ -181,6 +181,18 @@ static real fd2_r(const real *x, int64_t i, real dt, int fd_order)
     return (16 * d1 - d2) / (12 * dt * dt);
 }
 
+/* third derivative (the m = 1 term of Eq. (B4) needs d^3 H / dt^3): central stencils of accuracy
+ * order 2, (x[+2] - 2 x[+1] + 2 x[-1] - x[-2]) / (2 dt^3), and 4,
+ * (-x[+3] + 8 x[+2] - 13 x[+1] + 13 x[-1] - 8 x[-2] + x[-3]) / (8 dt^3), written as differences of symmetric pairs
+ * (reading G15 extended: same evaluation order idea as the first-derivative stencils) */
+static real fd3_in(const double *x, int64_t i, real dt, int fd_order)
+{
+    const real p1 = AT(x, i + 1) - AT(x, i - 1), p2 = AT(x, i + 2) - AT(x, i - 2);
+    if (fd_order == 2) return (p2 - 2 * p1) / (2 * dt * dt * dt);
+    const real p3 = AT(x, i + 3) - AT(x, i - 3);
+    return (8 * p2 - 13 * p1 - p3) / (8 * dt * dt * dt);
+}
+
 /* ---------------------------------------------------------------------------------- */
 /* O1  orbits (readings G5, G6, G7): first-order Keplerian, rigid rotating triangle   */
 /* ---------------------------------------------------------------------------------- */
@@ -329,6 +341,42 @@ static void links_lfa_at(const orbit_ctx *o, const frame_t *f, const real *gp, c
     }
 }
 
+/* Extended LFA single link, l = +1,+2,+3:
+ *   point = 0: central, tau of (B1), series (B4) truncated after `terms` terms (terms = 1 is (B10)):
+ *       y = -(L_l / 2) { dH/dt + (1/6) [ (L_l / 2)(1 - k.n_l) ]^2 d^3H/dt^3 } (tau),   tau-derivatives = t-derivatives (B7)
+ *   point = 1: backward (epsilon = 0), Eq. (B13):  y = -(L_l / 2) dH/dt (t - L_l - k.R_s / c)      leading order
+ *   point = 2: forward  (epsilon = 1), Eq. (B14):  y = -(L_l / 2) dH/dt (t - k.R_r / c)            leading order
+ * with H = F+ h+ + Fx hx and the antenna patterns at reception time (B9), (G3, G17).  g1 = dh/dt, g3 = d^3h/dt^3 on
+ * the grid. */
+enum { ORC_LFA_CENTRAL = 0, ORC_LFA_BACKWARD = 1, ORC_LFA_FORWARD = 2 };
+static void links_lfa_ext_at(const orbit_ctx *o, const frame_t *f, const real *gp, const real *gc, const real *g3p,
+                             const real *g3c, int64_t g0, int64_t glen, int64_t n, int order, int terms, int point,
+                             real y[6])
+{
+    const real c = ORC_C_LIGHT, dt = o->d.dt;
+    geom_t g;
+    orbit_geometry(o, n, &g);
+    for (int l = 0; l < 6; ++l) y[l] = 0;
+    for (int l = 0; l < 3; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real Fp, Fc;
+        antenna(f, g.nh[l], &Fp, &Fc);
+        const real ds = g.L[l] + dot3(f->k, g.R[s]) / c, dr = dot3(f->k, g.R[r]) / c; /* (2.6) */
+        real tau;
+        if (point == ORC_LFA_CENTRAL) tau = g.L[l] / 2 + (dot3(f->k, g.R[s]) + dot3(f->k, g.R[r])) / (2 * c); /* (B1) */
+        else if (point == ORC_LFA_BACKWARD) tau = ds;                                                          /* tau_0 */
+        else tau = dr;                                                                                         /* tau_1 */
+        real dH = Fp * interp_series(gp, g0, glen, n, tau, dt, order) + Fc * interp_series(gc, g0, glen, n, tau, dt, order);
+        if (point == ORC_LFA_CENTRAL && terms >= 2) {
+            const real half = (g.L[l] / 2) * (1 - dot3(f->k, g.nh[l]));   /* (delta_s - delta_r) / 2 with L n = R_r - R_s */
+            const real d3H = Fp * interp_series(g3p, g0, glen, n, tau, dt, order) +
+                             Fc * interp_series(g3c, g0, glen, n, tau, dt, order);
+            dH += half * half / 6 * d3H;                                  /* m = 1 term of (B4) */
+        }
+        y[l] = -(g.L[l] / 2) * dH;
+    }
+}
+
 /* ---------------------------------------------------------------------------------- */
 /* O6  Michelson TDI, Eqs. (2.7), (2.8) with G8, G9, G12; ch = 0,1,2 -> X,Y,Z          */
 /* ---------------------------------------------------------------------------------- */
@@ -472,6 +520,65 @@ static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, cons
 }
 
 /* LFA response for one source */
+/* half width of the widest stencil applied to the strain: the first derivative (w), or with the m = 1 term of (B4)
+ * the third derivative (w + 1) */
+static int64_t lfa_strain_width(int fd_order, int terms) { return fd_order / 2 + (terms >= 2 ? 1 : 0); }
+
+static int lfa_one_ext(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
+                       int order, int fd_order, int terms, int point, const margins_t *mg, int64_t nb, int64_t ne,
+                       work_t *w)
+{
+    const int64_t N = o->d.n, wd = mg->w, ws = lfa_strain_width(fd_order, terms), extra = ws - wd;
+    const real dt = o->d.dt;
+    /* the same ranges as lfa_one; the link series is valid where the widest strain stencil fits: m1 + ws */
+    const int64_t d0 = imax(0, nb - mg->m2), d1 = imin(N, ne + (order + 1) / 2 + 1);
+    const int64_t y0 = imax(0, d0 - wd), y1 = imin(N, d1 + wd);
+    const int64_t g0 = imax(0, y0 - mg->m1), g1 = imin(N, y1 + mg->m1);
+    real *gp = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *gc = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *g3p = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *g3c = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *dy[3] = { 0, 0, 0 };
+    for (int l = 0; l < 3; ++l) dy[l] = (real *)calloc((size_t)imax(d1 - d0, 1), sizeof(real));
+    if (!gp || !gc || !g3p || !g3c || !dy[0] || !dy[1] || !dy[2] || work_alloc(w, y0, y1 - y0, ne - nb)) return ORC_EINVAL;
+#pragma omp parallel for
+    for (int64_t i = g0; i < g1; ++i) {
+        if (i < ws || i >= N - ws) continue;
+        gp[i - g0] = fd1_in(hp, i, dt, fd_order);
+        gc[i - g0] = fd1_in(hc, i, dt, fd_order);
+        if (terms >= 2) {
+            g3p[i - g0] = fd3_in(hp, i, dt, fd_order);
+            g3c[i - g0] = fd3_in(hc, i, dt, fd_order);
+        }
+    }
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = y0; m < y1; ++m) {
+        if (m < mg->m1 + ws || m >= N - mg->m1 - ws) continue;
+        real y[6];
+        links_lfa_ext_at(o, f, gp, gc, g3p, g3c, g0, g1 - g0, m, order, terms, point, y);
+        for (int l = 0; l < 6; ++l) w->y[l][m - y0] = y[l];
+    }
+#pragma omp parallel for
+    for (int64_t i = d0; i < d1; ++i) {
+        if (i < mg->m1 + ws + wd || i >= N - mg->m1 - ws - wd) continue;
+        for (int l = 0; l < 3; ++l)
+            dy[l][i - d0] = (gen == ORC_GEN_15) ? fd1_r(w->y[l], i - y0, dt, fd_order)
+                                                : fd2_r(w->y[l], i - y0, dt, fd_order);
+    }
+    yseries_t dys = { { dy[0], dy[1], dy[2], 0, 0, 0 }, d0, d1 - d0 };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = nb; n < ne; ++n) {
+        if (n < mg->lo + extra || n >= N - mg->hi - extra) continue;
+        geom_t g;
+        orbit_geometry(o, n, &g);
+        for (int c = 0; c < 3; ++c)
+            w->X[c][n - nb] = michelson_lfa_at(&dys, g.L, c, gen, n, dt, order);
+    }
+    free(gp); free(gc); free(g3p); free(g3c);
+    for (int l = 0; l < 3; ++l) free(dy[l]);
+    return ORC_OK;
+}
+
 static int lfa_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
                    int order, int fd_order, const margins_t *mg, int64_t nb, int64_t ne, work_t *w)
 {
@@ -795,6 +902,49 @@ int orc_response_lfa(const orc_orbit_desc *d, const double *Rtab, const double *
         work_free(&w);
     }
     return ORC_OK;
+}
+
+/* Extended LFA response: `terms` terms of the single-link series (B4) (1 | 2) about the expansion
+ * point `point` (0 central (B1), 1 backward (B13), 2 forward (B14); terms = 2 only with the central point), then the
+ * Michelson combination (B25) / (B33) as in orc_response_lfa.  The output margins grow by one sample per side when
+ * terms = 2 (the third-derivative stencil is one sample wider): orc_margins_lfa_ext. */
+int orc_margins_lfa_ext(const orc_orbit_desc *d, int gen, int order, int fd_order, int terms, int64_t *lo, int64_t *hi)
+{
+    margins_t m;
+    if (!d || !lo || !hi) return ORC_EINVAL;
+    margins(d, gen, order, fd_order, &m);
+    *lo = m.lo + (terms >= 2 ? 1 : 0);
+    *hi = m.hi + (terms >= 2 ? 1 : 0);
+    return ORC_OK;
+}
+
+int orc_response_lfa_ext(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
+                         const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
+                         int order, int fd_order, int terms, int point, int64_t nb, int64_t ne, double *A, double *E,
+                         double *T, double *XYZ, double *y)
+{
+    if (check_args(d, gen, order, fd_order, 1, ld, nb, ne) || !hp || !hc || !src) return ORC_EINVAL;
+    if (terms < 1 || terms > 2 || point < 0 || point > 2 || (terms == 2 && point != ORC_LFA_CENTRAL)) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, fd_order, &mg);
+    for (int64_t b = 0; b < batch; ++b) {
+        frame_t f;
+        work_t w;
+        source_frame(&src[b], &f);
+        if (lfa_one_ext(&o, &f, hp + b * ld, hc + b * ld, gen, order, fd_order, terms, point, &mg, nb, ne, &w)) return ORC_EINVAL;
+        emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&w);
+    }
+    return ORC_OK;
+}
+
+/* third-derivative stencil on a double series (for the pins): out[i] for i in [w, len - w), w = fd_order / 2 + 1 */
+void orc_stencil3(const double *x, int64_t len, double dt, int fd_order, double *out)
+{
+    const int64_t w = fd_order / 2 + 1;
+    for (int64_t i = 0; i < len; ++i) out[i] = 0;
+    for (int64_t i = w; i < len - w; ++i) out[i] = (double)fd3_in(x, i, (real)dt, fd_order);
 }
 
 /* Hybrid response (O9): both responses on the whole requested range, blended per Eqs. (4.5), (4.6);

@@ -267,3 +267,120 @@ def test_hybrid_is_separate_blend_of_links_and_michelson(orc80, taper):
         # NOT the same as recomputing X from the blended links: check (4.6) differs from that inside the window
         mid = np.abs(t - hyb["t_hyb"]) < T / 4
         assert np.abs(rh["XYZ"][0, 0, mid] - rf["XYZ"][0, 0, mid]).max() > 1e-6 * scale
+
+
+# ---------------------------------------------------------------------------------------------
+# higher-order single-link series (B4) and the other expansion points (B12)-(B14)
+# ---------------------------------------------------------------------------------------------
+def stencil3_transfer(fd_order, w, dt):
+    """Fourier symbol of the central third-derivative stencils (textbook): FD3 -> (i w)^3 S3"""
+    x = w * dt
+    if fd_order == 2:
+        return 1j * (math.sin(2 * x) - 2 * math.sin(x)) / dt ** 3
+    return 1j * (-math.sin(3 * x) + 8 * math.sin(2 * x) - 13 * math.sin(x)) / (4 * dt ** 3)
+
+
+@pytest.mark.parametrize("fd_order,exact_deg", [(2, 4), (4, 6)])
+def test_third_derivative_stencil_is_exact_on_polynomials(orc80, fd_order, exact_deg):
+    dt = 0.7
+    x = np.arange(-12, 13) * dt
+    for deg in range(exact_deg + 2):
+        c = np.random.default_rng(deg).standard_normal(deg + 1)
+        p = np.polynomial.Polynomial(c)
+        got = orc80.stencil3(p(x), dt, fd_order)
+        want = p.deriv(3)(x)
+        w = fd_order // 2 + 1
+        err = np.abs(got[w:-w] - want[w:-w]).max() / max(1.0, np.abs(want).max())
+        if deg <= exact_deg:
+            assert err < 1e-10, (deg, err)
+        else:
+            assert err > 1e-6, (deg, err)          # one degree higher: the truncation error shows
+    assert np.all(orc80.stencil3(p(x), dt, fd_order)[:w] == 0)
+    # and the symbol on a complex exponential
+    wv = 0.31
+    zs = orc80.stencil3(np.sin(wv * x), dt, fd_order)[12]       # d^3/dt^3 sin(w t) at t = 0 is -w^3: symbol / i
+    assert abs(zs - (stencil3_transfer(fd_order, wv, dt) / 1j).real) < 1e-12
+
+
+def test_lfa_ext_with_one_central_term_is_the_lfa(orc80):
+    cfg = W.config(2, n=3000)
+    hp, hc, ang, _ = W.sources(cfg, [0])
+    a = orc80.response_lfa(cfg["orbit"], hp, hc, ang, 20, 31, 4)
+    b = orc80.response_lfa_ext(cfg["orbit"], hp, hc, ang, 20, 31, 4, terms=1, point=0)
+    for k in ("A", "E", "T", "XYZ", "y"):
+        assert np.array_equal(a[k], b[k]), k
+    assert orc80.margins_lfa_ext(cfg["orbit"], 20, 31, 4, 1) == orc80.margins(cfg["orbit"], 20, 31, 4)
+    lo, hi = orc80.margins(cfg["orbit"], 20, 31, 4)
+    assert orc80.margins_lfa_ext(cfg["orbit"], 20, 31, 4, 2) == (lo + 1, hi + 1)
+    with pytest.raises(ValueError):
+        orc80.response_lfa_ext(cfg["orbit"], hp, hc, ang, 20, 31, 4, terms=2, point=1)   # (B13), (B14): leading order only
+
+
+def test_second_term_of_B4_turns_the_f2_law_into_f4(orc80):
+    """Eq. (B4) on a frozen triangle: with m = 0, 1 the ratio to the full link is (x - x^3 / 6) / sin x up to the
+    stencil symbols, x = (w L / 2)(1 - k.n): the residual falls as f^4 (factor 16 per octave) instead of f^2, and
+    matches the closed form with the textbook symbols of the two stencils"""
+    n, dt, order = 2600, 2.0, 31
+    orbit, R0, L0 = triangle_tables(orc80, n, dt)
+    src = (0.3, 5.0, 0.4)
+    beta, lam, _ = src
+    k = -np.array([math.cos(beta) * math.cos(lam), math.cos(beta) * math.sin(lam), math.sin(beta)])
+    t = dt * np.arange(n)
+    prev = None
+    for f_hz in (8e-3, 4e-3, 2e-3):
+        w = 2 * math.pi * f_hz
+        hp, hc = W.monochromatic(n, dt, f_hz)
+        rf = orc80.response_full(orbit, hp[None], hc[None], [src], 15, order)
+        r2 = orc80.response_lfa_ext(orbit, hp[None], hc[None], [src], 15, order, 4, terms=2, point=0)
+        lo, hi = orc80.margins_lfa_ext(orbit, 15, order, 4, 2)
+        errs = []
+        for l in range(3):
+            s, rr = LINKS[l]
+            nv = (R0[rr] - R0[s]) / np.linalg.norm(R0[rr] - R0[s])
+            x = 0.5 * w * L0[l] * (1 - k @ nv)
+            zf, _ = fit_complex_amplitude(rf["y"][l, 0], t, w, lo, n - hi)
+            z2, _ = fit_complex_amplitude(r2["y"][l, 0], t, w, lo, n - hi)
+            S1 = (stencil_transfer(1, 4, w, dt) / (1j * w)).real
+            S3 = (stencil3_transfer(4, w, dt) / (1j * w) ** 3).real
+            # (i w)^3 = -i w w^2: the series is i w (1 - x^2 / 6) against i w sin(x) / x of the full link
+            want = (x * S1 - x ** 3 / 6 * S3) / math.sin(x)
+            assert abs(z2 / zf - want) < 2e-8, (f_hz, l)
+            errs.append(abs(z2 / zf - 1))
+        if prev is not None:
+            for a, b in zip(prev, errs):
+                assert 12.0 < a / b < 20.0, (a, b)        # f^4 (the one-term series gives 4: test above)
+        prev = errs
+
+
+def test_forward_and_backward_points_are_first_order(orc80):
+    """(B13), (B14) on a frozen triangle: y = -(L/2) dH/dt at t - delta_s resp. t - delta_r, so
+    y_bwd / y_full = x e^{-i x} / sin x and y_fwd / y_full = x e^{+i x} / sin x: the error is O(x) -- the first-order
+    error the paper attributes to the forward form of Ref. [46] -- against O(x^2) for the central point"""
+    n, dt, order = 2600, 2.0, 31
+    orbit, R0, L0 = triangle_tables(orc80, n, dt)
+    src = (0.3, 5.0, 0.4)
+    beta, lam, _ = src
+    k = -np.array([math.cos(beta) * math.cos(lam), math.cos(beta) * math.sin(lam), math.sin(beta)])
+    t = dt * np.arange(n)
+    lo, hi = orc80.margins(orbit, 15, order, 4)
+    prev = None
+    for f_hz in (4e-3, 2e-3, 1e-3):
+        w = 2 * math.pi * f_hz
+        hp, hc = W.monochromatic(n, dt, f_hz)
+        rf = orc80.response_full(orbit, hp[None], hc[None], [src], 15, order)
+        errs = []
+        for point, sign in ((1, -1.0), (2, +1.0)):
+            r = orc80.response_lfa_ext(orbit, hp[None], hc[None], [src], 15, order, 4, terms=1, point=point)
+            for l in range(3):
+                s, rr = LINKS[l]
+                nv = (R0[rr] - R0[s]) / np.linalg.norm(R0[rr] - R0[s])
+                x = 0.5 * w * L0[l] * (1 - k @ nv)
+                zf, _ = fit_complex_amplitude(rf["y"][l, 0], t, w, lo, n - hi)
+                z, _ = fit_complex_amplitude(r["y"][l, 0], t, w, lo, n - hi)
+                S1 = (stencil_transfer(1, 4, w, dt) / (1j * w)).real
+                assert abs(z / zf - S1 * x * np.exp(sign * 1j * x) / math.sin(x)) < 2e-8, (f_hz, point, l)
+                errs.append(abs(z / zf - 1))
+        if prev is not None:
+            for a, b in zip(prev, errs):
+                assert 1.9 < a / b < 2.1, (a, b)          # first order in f
+        prev = errs
