@@ -46,6 +46,9 @@ enum {
 enum { LTDI_TAPER_SIGMOID = 0,      /* Eq. (4.1), the paper's weight                                  */
        LTDI_TAPER_COSINE = 1 };     /* raised cosine over the window (BASELINE.json configs 2, 4; G20) */
 enum { LTDI_RESPONSE_FULL = 0, LTDI_RESPONSE_LFA = 1, LTDI_RESPONSE_HYBRID = 2 };
+enum { LTDI_LFA_CENTRAL = 0,        /* expansion about tau of Eq. (B1), P:685 (the paper's choice)                 */
+       LTDI_LFA_BACKWARD = 1,       /* epsilon = 0: about t - L_l - k.R_s / c, Eq. (B13)                    */
+       LTDI_LFA_FORWARD = 2 };      /* epsilon = 1: about t - k.R_r / c, Eq. (B14), P:778 (the choice of Ref. [46]) */
 
 /* Time grid and orbit model (first-order Keplerian orbits, G5). */
 typedef struct {
@@ -147,6 +150,23 @@ int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *
                       int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
                       double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
                       size_t work_bytes, void *stream);
+
+/* higher-order and alternative LFA of the single link.
+ *   terms = 1, point = LTDI_LFA_CENTRAL: identical to ltdi_response_lfa (bitwise).
+ *   terms = 2 (central point only): the m = 1 term of the odd-derivative series Eq. (B4), P:704,
+ *       y = -(L_l / 2) { dH/dt + (1/6) [(L_l / 2)(1 - k.n_l)]^2 d^3H/dt^3 }(tau),
+ *     d^3h/dt^3 from the central stencil of accuracy order fd_order (2: (x[2] - 2 x[1] + 2 x[-1] - x[-2]) / (2 dt^3),
+ *     4: (-x[3] + 8 x[2] - 13 x[1] + 13 x[-1] - 8 x[-2] + x[-3]) / (8 dt^3)); its stencil is one sample wider than the
+ *     first derivative's, so the output margins grow by one sample per side (ltdi_margins_lfa_ext).
+ *   point = LTDI_LFA_BACKWARD / LTDI_LFA_FORWARD (terms = 1): the leading-order expressions (B13) / (B14) about the
+ *     emission / reception ends of the link, whose residual is first order in the expansion parameter.
+ * The Michelson stage is (B25) / (B33) as in ltdi_response_lfa.  Errors as there; LTDI_EINVAL for other terms / point. */
+int ltdi_response_lfa_ext(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                          int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                          int terms, int point, double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y,
+                          void *d_work, size_t work_bytes, void *stream);
+int ltdi_margins_lfa_ext(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int terms,
+                         int64_t *lo, int64_t *hi);
 
 /* Hybrid: LFA for t <= t_hyb + T/2, full for t >= t_hyb - T/2, links blended by Eq. (4.5) and
  * X, Y, Z blended separately by Eq. (4.6) (S8).  h_hyb has n_hyb = 1 or batch entries. */

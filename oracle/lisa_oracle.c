@@ -61,7 +61,7 @@ typedef double real;
 #define ORC_C_LIGHT 299792458.0 /* m/s, exact (SI) */
 
 enum { ORC_GEN_15 = 15, ORC_GEN_20 = 20 };
-enum { ORC_ORBIT_STATIC_EQUALARM = 0, ORC_ORBIT_KEPLERIAN = 1, ORC_ORBIT_TABLES = 2 };
+enum { ORC_ORBIT_STATIC_EQUALARM = 0, ORC_ORBIT_KEPLERIAN = 1, ORC_ORBIT_TABLES = 2, ORC_ORBIT_KNOTS = 3 };
 enum { ORC_TAPER_SIGMOID = 0, ORC_TAPER_COSINE = 1 };
 
 typedef struct {
@@ -198,9 +198,60 @@ static real fd3_in(const double *x, int64_t i, real dt, int fd_order)
 /* ---------------------------------------------------------------------------------- */
 typedef struct {
     orc_orbit_desc d;
-    const double *Rtab; /* mode TABLES: [3][3][n] spacecraft, component, sample [m] */
-    const double *Ltab; /* mode TABLES: [6][n] light travel times [s], link order +1,+2,+3,-1,-2,-3 */
+    const double *Rtab; /* mode TABLES: [3][3][n] spacecraft, component, sample [m];
+                         * mode KNOTS: [3][3][nk] spacecraft, component, knot [m] (a numerical orbit file) */
+    const double *Ltab; /* mode TABLES: [6][n] light travel times [s], link order +1,+2,+3,-1,-2,-3;
+                         * mode KNOTS: {tk0, dtk, nk, p_orb}: knot j at time tk0 + j dtk, Lagrange order p_orb */
 } orbit_ctx;
+
+/* O11 numerical orbits ("realistic ESA orbits"; reading G28): the spacecraft positions are
+ * tabulated at nk equidistant knots and brought to the sample time t by centred Lagrange interpolation of odd order
+ * p_orb on the knot grid -- the same weights as O4 with u = (t - tk0) / dtk - floor(.) in [0, 1) and taps
+ * k = -(M/2 - 1) .. M/2 around the knot at or before t; the velocities are the time derivative of that interpolant
+ * (derivative of the weights by the product rule, divided by dtk).  The light travel times then follow G6. */
+static void knot_weights(real u, int order, real *w, real *dw)
+{
+    const int M = order + 1, kmin = -(M / 2 - 1), kmax = M / 2;
+    for (int k = kmin; k <= kmax; ++k) {
+        real den = 1, num = 1, dnum = 0;
+        for (int m = kmin; m <= kmax; ++m)
+            if (m != k) den *= (real)(k - m);
+        for (int m = kmin; m <= kmax; ++m) {       /* product rule: sum over the factor that is differentiated */
+            if (m == k) continue;
+            real part = 1;
+            for (int j = kmin; j <= kmax; ++j)
+                if (j != k && j != m) part *= (u - (real)j);
+            dnum += part;
+            num *= (u - (real)m);
+        }
+        w[k - kmin] = num / den;
+        dw[k - kmin] = dnum / den;
+    }
+}
+
+static void knot_positions(const orbit_ctx *o, real t, real R[3][3], real V[3][3])
+{
+    const real tk0 = (real)o->Ltab[0], dtk = (real)o->Ltab[1];
+    const int64_t nk = (int64_t)o->Ltab[2];
+    const int order = (int)o->Ltab[3], M = order + 1, kmin = -(M / 2 - 1);
+    real w[64], dw[64];
+    const real s = (t - tk0) / dtk;
+    int64_t j = (int64_t)s;
+    if ((real)j > s) --j;                      /* floor */
+    knot_weights(s - (real)j, order, w, dw);
+    for (int i = 0; i < 3; ++i)
+        for (int a = 0; a < 3; ++a) {
+            real acc = 0, dacc = 0;
+            for (int m = 0; m < M; ++m) {
+                const int64_t idx = j + kmin + m;
+                const real v = (idx >= 0 && idx < nk) ? (real)o->Rtab[(int64_t)(i * 3 + a) * nk + idx] : (real)0;
+                acc += w[m] * v;
+                dacc += dw[m] * v;
+            }
+            R[i][a] = acc;
+            V[i][a] = dacc / dtk;
+        }
+}
 
 typedef struct {
     real R[3][3];  /* spacecraft positions [m] */
@@ -215,6 +266,8 @@ static void orbit_geometry(const orbit_ctx *o, int64_t n, geom_t *g)
     if (o->d.mode == ORC_ORBIT_TABLES) {
         for (int i = 0; i < 3; ++i)
             for (int a = 0; a < 3; ++a) g->R[i][a] = (real)o->Rtab[(int64_t)(i * 3 + a) * o->d.n + n];
+    } else if (o->d.mode == ORC_ORBIT_KNOTS) {
+        knot_positions(o, (real)o->d.t0 + (real)n * (real)o->d.dt, g->R, V);
     } else {
         const real t = (real)o->d.t0 + (real)n * (real)o->d.dt;
         const real R = o->d.R_m, L = o->d.arm_m;
@@ -242,7 +295,7 @@ static void orbit_geometry(const orbit_ctx *o, int64_t n, geom_t *g)
         for (int a = 0; a < 3; ++a) g->nh[l][a] = dvec[a] / len;
         if (o->d.mode == ORC_ORBIT_STATIC_EQUALARM) {
             g->L[l] = (real)o->d.arm_m / c; /* "equal and constant" delays */
-        } else if (o->d.mode == ORC_ORBIT_KEPLERIAN) {
+        } else if (o->d.mode == ORC_ORBIT_KEPLERIAN || o->d.mode == ORC_ORBIT_KNOTS) {
             /* first-order light time: L_l != L_-l through the sender velocity (B22) */
             real nv = 0;
             for (int a = 0; a < 3; ++a) nv += g->nh[l][a] * V[s][a];
@@ -423,6 +476,70 @@ static real michelson_at(const yseries_t *ys, const real Lsec[6], int ch, int ge
     return X;
 }
 
+/* O12 properly nested delays (the comparison case of P:151 -- the paper itself evaluates every L_l at t).
+ * Delay operators act as (D_l f)(t) = f(t - L_l(t)), so D_a D_b f (t) = f(t - L_a(t) - L_b(t - L_a(t))): walking a
+ * chain of links c_1 c_2 .. c_m backwards from the reception time,
+ *     d_0 = 0,   d_j = d_{j-1} + L_{c_j}(t - d_{j-1}),
+ * and the term is y(t - d_m).  With a = D_{-2} D_2, b = D_3 D_{-3} (for X; cyclic for Y, Z) and P = y_123, Q = y_3-21,
+ * U = y_1-32, W = y_231:
+ *     X_1.5 = (1 - b)(Q + D_{-2} P) - (1 - a)(W + D_3 U)
+ *     X_2.0 = (1 - b - b a + a b b)(Q + D_{-2} P) - (1 - a - a b + b a a)(W + D_3 U)
+ * which for commuting (un-nested) delays are Eqs. (2.7) and (2.8) term by term (with G9).  The light travel time at
+ * an off-grid time is the centred Lagrange interpolation of order p_L of the sampled series L_l(t_n) (reading G29);
+ * the link series are interpolated once per term at the accumulated delay, as in O6. */
+typedef struct { const real *L[6]; int64_t l0, llen; } lseries_t;
+
+static real chain_delay(const lseries_t *Ls, int64_t n, real dt, int order_L, int len, const int *labels)
+{
+    real d = 0;
+    for (int j = 0; j < len; ++j) {
+        const int l = link_index(labels[j]);
+        if (d == 0) d += Ls->L[l][n - Ls->l0];                                           /* on the grid */
+        else d += interp_series(Ls->L[l], Ls->l0, Ls->llen, n, d, dt, order_L);
+    }
+    return d;
+}
+
+static real michelson_nested_at(const yseries_t *ys, const lseries_t *Ls, int ch, int gen, int64_t n, real dt,
+                                int order, int order_L)
+{
+    const int p2 = cyc(2, ch), p3 = cyc(3, ch);
+#define CH(...) chain_delay(Ls, n, dt, order_L, (int)(sizeof((int[]){ __VA_ARGS__ }) / sizeof(int)), (int[]){ __VA_ARGS__ })
+#define Y(label, delay) ydel(ys, (label), n, (delay), dt, order)
+    /* (1 - b)(Q + D_-2 P) - (1 - a)(W + D_3 U) */
+    real X = Y(-p2, (real)0) + Y(+p2, CH(-p2))
+           - Y(-p2, CH(+p3, -p3)) - Y(+p2, CH(+p3, -p3, -p2))
+           - Y(+p3, (real)0) - Y(-p3, CH(+p3))
+           + Y(+p3, CH(-p2, +p2)) + Y(-p3, CH(-p2, +p2, +p3));
+    if (gen == ORC_GEN_20) {
+        /* (- b a + a b b)(Q + D_-2 P) - (- a b + b a a)(W + D_3 U) */
+        X += -Y(-p2, CH(+p3, -p3, -p2, +p2)) - Y(+p2, CH(+p3, -p3, -p2, +p2, -p2))
+           + Y(-p2, CH(-p2, +p2, +p3, -p3, +p3, -p3)) + Y(+p2, CH(-p2, +p2, +p3, -p3, +p3, -p3, -p2))
+           + Y(+p3, CH(-p2, +p2, +p3, -p3)) + Y(-p3, CH(-p2, +p2, +p3, -p3, +p3))
+           - Y(+p3, CH(+p3, -p3, -p2, +p2, -p2, +p2)) - Y(-p3, CH(+p3, -p3, -p2, +p2, -p2, +p2, +p3));
+    }
+#undef Y
+#undef CH
+    return X;
+}
+
+/* the sampled light travel times on [l0, l0 + len) in working precision */
+static int lseries_alloc(const orbit_ctx *o, int64_t l0, int64_t len, real *buf[6], lseries_t *Ls)
+{
+    for (int l = 0; l < 6; ++l)
+        if (!(buf[l] = (real *)calloc((size_t)(len > 0 ? len : 1), sizeof(real)))) return ORC_EINVAL;
+#pragma omp parallel for
+    for (int64_t i = 0; i < len; ++i) {
+        geom_t g;
+        orbit_geometry(o, l0 + i, &g);
+        for (int l = 0; l < 6; ++l) buf[l][i] = g.L[l];
+    }
+    for (int l = 0; l < 6; ++l) Ls->L[l] = buf[l];
+    Ls->l0 = l0;
+    Ls->llen = len;
+    return ORC_OK;
+}
+
 /* LFA Michelson, Eq. (B25) (gen 1.5) / (B33) (gen 2.0); dy[l] = FD1 or FD2 of y_l, l = +1,+2,+3 */
 static real michelson_lfa_at(const yseries_t *dys, const real Lsec[6], int ch, int gen, int64_t n,
                              real dt, int order)
@@ -493,6 +610,8 @@ static void work_free(work_t *w)
 }
 
 /* full response for one source: y (6 links) on the halo range, X,Y,Z on [nb,ne) */
+static int g_nested_order = 0; /* 0: every L_l at t (the paper); p_L > 0: nested delays (O12), set per call */
+
 static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
                     int order, const margins_t *mg, int64_t lo, int64_t hi, int64_t nb, int64_t ne,
                     work_t *w)
@@ -508,6 +627,19 @@ static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, cons
         for (int l = 0; l < 6; ++l) w->y[l][m - y0] = y[l];
     }
     yseries_t ys = { { w->y[0], w->y[1], w->y[2], w->y[3], w->y[4], w->y[5] }, y0, y1 - y0 };
+    if (g_nested_order > 0) { /* O12 */
+        real *buf[6];
+        lseries_t Ls;
+        if (lseries_alloc(o, y0, y1 - y0, buf, &Ls)) return ORC_EINVAL;
+#pragma omp parallel for schedule(dynamic, 64)
+        for (int64_t n = nb; n < ne; ++n) {
+            if (n < lo || n >= N - hi) continue;
+            for (int c = 0; c < 3; ++c)
+                w->X[c][n - nb] = michelson_nested_at(&ys, &Ls, c, gen, n, (real)o->d.dt, order, g_nested_order);
+        }
+        for (int l = 0; l < 6; ++l) free(buf[l]);
+        return ORC_OK;
+    }
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t n = nb; n < ne; ++n) {
         if (n < lo || n >= N - hi) continue; /* margin: X = 0 */
@@ -884,6 +1016,48 @@ int orc_response_full(const orc_orbit_desc *d, const double *Rtab, const double 
 }
 
 /* LFA response (O8) */
+/* Full response with properly nested TDI delays (O12); nested_order = p_L, the Lagrange order of the light-time lookups */
+int orc_response_full_nested(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
+                             const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
+                             int order, int nested_order, int64_t nb, int64_t ne, double *A, double *E, double *T,
+                             double *XYZ, double *y)
+{
+    if (nested_order < 1 || nested_order > 63 || nested_order % 2 == 0) return ORC_EINVAL;
+    g_nested_order = nested_order;
+    const int rc = orc_response_full(d, Rtab, Ltab, hp, hc, ld, batch, src, gen, order, nb, ne, A, E, T, XYZ, y);
+    g_nested_order = 0;
+    return rc;
+}
+
+/* X, Y, Z with nested delays from caller-supplied link series y [6][n] (for the pins: laser-noise cancellation) */
+int orc_michelson_nested_from_links(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *y,
+                                    int gen, int order, int nested_order, double *XYZ)
+{
+    if (check_args(d, gen, order, 0, 0, d ? d->n : 0, 0, d ? d->n : 0) || !y || !XYZ) return ORC_EINVAL;
+    if (nested_order < 1 || nested_order > 63 || nested_order % 2 == 0) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, 0, &mg);
+    const int64_t N = d->n;
+    real *yr[6], *buf[6];
+    lseries_t Ls;
+    for (int l = 0; l < 6; ++l) {
+        if (!(yr[l] = (real *)malloc(sizeof(real) * (size_t)N))) return ORC_EINVAL;
+        for (int64_t i = 0; i < N; ++i) yr[l][i] = y[(int64_t)l * N + i];
+    }
+    if (lseries_alloc(&o, 0, N, buf, &Ls)) return ORC_EINVAL;
+    yseries_t ys = { { yr[0], yr[1], yr[2], yr[3], yr[4], yr[5] }, 0, N };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int c = 0; c < 3; ++c) XYZ[(int64_t)c * N + n] = 0.0;
+        if (n < mg.lo || n >= N - mg.hi) continue;
+        for (int c = 0; c < 3; ++c)
+            XYZ[(int64_t)c * N + n] = (double)michelson_nested_at(&ys, &Ls, c, gen, n, (real)d->dt, order, nested_order);
+    }
+    for (int l = 0; l < 6; ++l) { free(yr[l]); free(buf[l]); }
+    return ORC_OK;
+}
+
 int orc_response_lfa(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
                      const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
                      int order, int fd_order, int64_t nb, int64_t ne, double *A, double *E, double *T,

@@ -23,6 +23,7 @@ GEN_15, GEN_20 = 15, 20
 ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES = 0, 1, 2
 TAPER_SIGMOID, TAPER_COSINE = 0, 1
 RESPONSE_FULL, RESPONSE_LFA, RESPONSE_HYBRID = 0, 1, 2
+LFA_CENTRAL, LFA_BACKWARD, LFA_FORWARD = 0, 1, 2
 OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, -1, -2, -3, -4
 _ERR = {EINVAL: "LTDI_EINVAL", EUNSUPPORTED: "LTDI_EUNSUPPORTED", ECUDA: "LTDI_ECUDA",
         EWORKSPACE: "LTDI_EWORKSPACE"}
@@ -72,6 +73,9 @@ _SIGNATURES = {
                                      _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                     C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_lfa_ext": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                        C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_margins_lfa_ext": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, C.c_int, C.c_int, C.c_int, _i64p, _i64p]),
     "ltdi_response_hybrid": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                        C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _dp, _dp, _vp,
                                        C.c_size_t, _vp]),
@@ -138,6 +142,13 @@ def margins(desc, gen, order, fd_order=0):
     lo, hi = C.c_int64(), C.c_int64()
     d = _desc(desc)
     _check("ltdi_margins", lib().ltdi_margins(C.byref(d), gen, order, fd_order, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def margins_lfa_ext(desc, gen, order, fd_order, terms=1):
+    lo, hi = C.c_int64(), C.c_int64()
+    d = _desc(desc)
+    _check("ltdi_margins_lfa_ext", lib().ltdi_margins_lfa_ext(C.byref(d), gen, order, fd_order, terms, C.byref(lo), C.byref(hi)))
     return lo.value, hi.value
 
 
@@ -269,7 +280,7 @@ class Workspace:
         return {"A": self.A, "E": self.E, "T": self.T, "XYZ": self.XYZ, "y": self.y}
 
 
-def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, want_y, ws):
+def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, want_y, ws, ext=None):
     hp, hc = _dev_f64(hp, "hp"), _dev_f64(hc, "hc")
     if hp.dim() == 1:
         hp, hc = hp[None], hc[None]
@@ -285,6 +296,8 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
     with torch.cuda.device(hp.device):
         if which == RESPONSE_FULL:
             rc, fn = lib().ltdi_response_full(*head, *tail), "ltdi_response_full"
+        elif which == RESPONSE_LFA and ext is not None:
+            rc, fn = lib().ltdi_response_lfa_ext(*head, fd_order, int(ext[0]), int(ext[1]), *tail), "ltdi_response_lfa_ext"
         elif which == RESPONSE_LFA:
             rc, fn = lib().ltdi_response_lfa(*head, fd_order, *tail), "ltdi_response_lfa"
         else:
@@ -303,6 +316,14 @@ def response_full(orb, hp, hc, sources, gen, order, want_xyz=False, want_y=False
 def response_lfa(orb, hp, hc, sources, gen, order, fd_order, want_xyz=False, want_y=False, workspace=None):
     """Eqs. (B10), (B25)/(B33): low-frequency approximation with central stencils of order fd_order."""
     return _run(RESPONSE_LFA, orb, hp, hc, sources, gen, order, fd_order, None, want_xyz, want_y, workspace)
+
+
+def response_lfa_ext(orb, hp, hc, sources, gen, order, fd_order, terms=1, point=LFA_CENTRAL, want_xyz=False,
+                     want_y=False, workspace=None):
+    """`terms` terms of the single-link series Eq. (B4) about the expansion point `point`
+    (LFA_CENTRAL (B1), LFA_BACKWARD (B13), LFA_FORWARD (B14)), then (B25) / (B33)."""
+    return _run(RESPONSE_LFA, orb, hp, hc, sources, gen, order, fd_order, None, want_xyz, want_y, workspace,
+                ext=(terms, point))
 
 
 def response_hybrid(orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz=False, want_y=False,

@@ -68,6 +68,8 @@ struct FastParams {
     const double *hyb;       /* [n_hyb][4] of this chunk (t_hyb, window, sigma, taper) */
     int64_t n_hyb;
     int which, gen, fd;
+    int lfa_terms, lfa_point, xw;   /* terms of Eq. (B4), expansion point LTDI_LFA_*, xw = terms - 1 */
+    double inv_fd3;                 /* 1 / (2 dt^3) | 1 / (8 dt^3): third-derivative stencil denominator (fd 2 | 4) */
     int64_t m1, m2, w, lo, hi;
     int64_t m2_15, m2_20;    /* anchor kernel: backward TDI reach of either generation (the anchors serve both) */
     int qmax;
@@ -310,6 +312,7 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
 // ---------------------------------------------------------------------------------------------
 #define LFA_ANC_DOUBLES 28
 #define LFA_LO_ROWS 12
+#define LFA_RAW_HALO 3   /* raw strain staged beyond the FD series on either side: the widest stencil (d^3/dt^3, order 4) */
 
 __device__ __forceinline__ dd quad_form_dd(const double *P, const dd *n, double *g)
 {
@@ -407,6 +410,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         else *reinterpret_cast<double2 *>(tb + r * FAST_TA + c) = make_double2(0.0, 0.0);
     }
     float *tl = nullptr;   /* LFA: low parts of the dd table entries of the tile */
+    double *he3_p = nullptr; /* LFA, terms = 2: [4][hw2] third-derivative numerators (even +, odd +, even x, odd x) */
     if (!LFA) {
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -422,11 +426,11 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         cp_async_wait_all();
         __syncthreads();
     } else {
-        /* raw strain of samples org - 2 .. org + 2 hw2 + 1 (asynchronous), then the FD1 numerators (G15) */
-        const int nraw = 2 * hw2 + 4;
+        /* raw strain of samples org - 3 .. org + 2 hw2 + 2 (asynchronous), then the FD1 numerators (G15) */
+        const int nraw = 2 * hw2 + 2 * LFA_RAW_HALO;
         double *raw_p = tb + NROWS * FAST_TA, *raw_c = raw_p + nraw;
         for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
-            const int64_t g = org - 2 + j;
+            const int64_t g = org - LFA_RAW_HALO + j;
             if (g >= 0 && g < p.n) {
                 cp_async8(raw_p + j, gp + g);
                 cp_async8(raw_c + j, gc + g);
@@ -445,15 +449,18 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                 else *reinterpret_cast<float4 *>(tl + r * FAST_TA + c) = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
+        /* SURVEY 8(f)-2, terms = 2: the d^3h/dt^3 numerators, parity-split like the first-derivative series */
+        he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * FAST_TA);
         cp_async_wait_all();
         __syncthreads();
         /* tile anchors of the antenna patterns (threads of the last warp, beside the stencil pass below) */
         if (tid >= FAST_TA_THREADS - 3) lfa_anchor(fr, tb, tl, FAST_TA_THREADS - 1 - tid, (int)min((int64_t)(FAST_TA / 2), p.n - 1 - a0), s_anc);
+        const int ws = w + p.xw;   /* the widest stencil applied to the strain */
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
             double vp = 0.0, vc = 0.0;
-            if (g >= w && g < p.n - w) {
-                const double *xp = raw_p + i + 2, *xc = raw_c + i + 2;
+            if (g >= ws && g < p.n - ws) {
+                const double *xp = raw_p + i + LFA_RAW_HALO, *xc = raw_c + i + LFA_RAW_HALO;
                 if (w == 1) {
                     vp = xp[1] - xp[-1];
                     vc = xc[1] - xc[-1];
@@ -461,6 +468,17 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                     vp = 8.0 * (xp[1] - xp[-1]) - (xp[2] - xp[-2]);
                     vc = 8.0 * (xc[1] - xc[-1]) - (xc[2] - xc[-2]);
                 }
+                if (p.lfa_terms >= 2) {
+                    const double p1 = xp[1] - xp[-1], p2 = xp[2] - xp[-2], c1 = xc[1] - xc[-1], c2 = xc[2] - xc[-2];
+                    double tp, tc;
+                    if (w == 1) { tp = p2 - 2.0 * p1; tc = c2 - 2.0 * c1; }
+                    else { tp = 8.0 * p2 - 13.0 * p1 - (xp[3] - xp[-3]); tc = 8.0 * c2 - 13.0 * c1 - (xc[3] - xc[-3]); }
+                    he3_p[((i & 1) ? hw2 : 0) + (i >> 1)] = tp;
+                    he3_p[((i & 1) ? 3 * hw2 : 2 * hw2) + (i >> 1)] = tc;
+                }
+            } else if (p.lfa_terms >= 2) {
+                he3_p[((i & 1) ? hw2 : 0) + (i >> 1)] = 0.0;
+                he3_p[((i & 1) ? 3 * hw2 : 2 * hw2) + (i >> 1)] = 0.0;
             }
             ((i & 1) ? ho_p : he_p)[i >> 1] = vp;
             ((i & 1) ? ho_c : he_c)[i >> 1] = vc;
@@ -471,7 +489,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     const int64_t m0 = a0 + 2 * tid;
     if (m0 >= p.n) return;
     const int rel0 = (int)(m0 - org);
-    const int64_t vlo = p.m1 + w, vhi = p.n - p.m1 - w;   /* valid link samples */
+    const int64_t vlo = p.m1 + w + (LFA ? p.xw : 0), vhi = p.n - vlo;   /* valid link samples */
     const bool in0 = m0 >= vlo && m0 < vhi, in1 = m0 + 1 >= vlo && m0 + 1 < vhi;
     double *yout = (LFA ? p.yL : p.yF) + b * p.lds + m0;
     const int64_t ystride = p.batch * p.lds;
@@ -560,8 +578,25 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             kdotR(r, kr0, kr1);
             const double2 L = row2(ROW_L + l);
             double ap0, ac0, ap1, ac1, pref, cref;
-            interp_delays<H, true>(p, 0.5 * L.x + 0.5 * (ks0 + kr0), 0.5 * L.y + 0.5 * (ks1 + kr1), rel0, he_p, ho_p,
-                                   he_c, ho_c, ap0, ac0, ap1, ac1, pref, cref);               /* (B1) */
+            double d0, d1;
+            if (p.lfa_point == LTDI_LFA_CENTRAL) { d0 = 0.5 * L.x + 0.5 * (ks0 + kr0); d1 = 0.5 * L.y + 0.5 * (ks1 + kr1); }   /* (B1) */
+            else if (p.lfa_point == LTDI_LFA_BACKWARD) { d0 = L.x + ks0; d1 = L.y + ks1; }                                    /* (B13) */
+            else { d0 = kr0; d1 = kr1; }                                                                                       /* (B14) */
+            interp_delays<H, true>(p, d0, d1, rel0, he_p, ho_p, he_c, ho_c, ap0, ac0, ap1, ac1, pref, cref);
+            if (p.lfa_terms >= 2) {
+                /* m = 1 term of Eq. (B4): + (1/6) [(L_l / 2)(1 - k.n_l)]^2 d^3H/dt^3 at the same retarded time;
+                 * relative to dH/dt it is (omega Delta / 2)^2 / 6, so plain fp64 serves: it joins the small part of the
+                 * (reference + difference) pair of the first-derivative numerators */
+                double bp0, bc0, bp1, bc1, p3, c3;
+                interp_delays<H, true>(p, d0, d1, rel0, he3_p, he3_p + hw2, he3_p + 2 * hw2, he3_p + 3 * hw2, bp0, bc0, bp1, bc1, p3, c3);
+                const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
+                const double h0 = (0.5 * L.x) * (1.0 - (fr[0] * nx.x + fr[1] * ny.x + fr[2] * nz.x));
+                const double h1 = (0.5 * L.y) * (1.0 - (fr[0] * nx.y + fr[1] * ny.y + fr[2] * nz.y));
+                const double r31 = p.inv_fd3 / p.inv_fd1 / 6.0;
+                const double f0 = h0 * h0 * r31, f1 = h1 * h1 * r31;
+                ap0 = fma(f0, p3 + bp0, ap0); ac0 = fma(f0, c3 + bc0, ac0);
+                ap1 = fma(f1, p3 + bp1, ap1); ac1 = fma(f1, c3 + bc1, ac1);
+            }
             const double *an = s_anc + l * LFA_ANC_DOUBLES;
             const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
             const float2 lx = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l) * FAST_TA);
@@ -908,7 +943,8 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
         const int runs = (yr + FD_RUN - 1) / FD_RUN;
         const bool g15 = p.gen == LTDI_GEN_15;
         const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
-        const bool interior = y0 >= p.m1 + 2 * w && y0 + yr <= p.n - p.m1 - 2 * w;
+        const int64_t dlo = p.m1 + 2 * w + p.xw;   /* first sample with a valid derivative of the LFA links */
+        const bool interior = y0 >= dlo && y0 + yr <= p.n - dlo;
 #pragma unroll 1
         for (int idx = tid; idx < 3 * runs; idx += FAST_TC_THREADS) {   /* (link, run) pairs, evenly over the threads */
             const int l = idx / runs, k0 = (idx - l * runs) * FD_RUN;
@@ -942,7 +978,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
 #pragma unroll
                 for (int j = 0; j < FD_RUN; ++j) {
                     const int64_t m = y0 + k0 + j;
-                    if (k0 + j < yr) o[j] = (m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w) ? v[j] : 0.0;
+                    if (k0 + j < yr) o[j] = (m >= dlo && m < p.n - dlo) ? v[j] : 0.0;
                 }
             }
         }

@@ -471,6 +471,8 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     p.tab = rp.tab; p.stride = rp.stride; p.n = rp.n; p.t0 = rp.t0; p.dt = rp.dt; p.inv_dt = 1.0 / rp.dt;
     p.ld = rp.ld; p.n_hyb = rp.n_hyb; p.which = which; p.gen = rp.gen; p.fd = rp.fd;
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi; p.qmax = rp.qmax;
+    p.lfa_terms = rp.lfa_terms; p.lfa_point = rp.lfa_point; p.xw = rp.xw;
+    p.inv_fd3 = 1.0 / ((mg.w == 1 ? 2.0 : 8.0) * rp.dt * rp.dt * rp.dt);
     p.m2_15 = compute_margins(d, LTDI_GEN_15, M - 1, 0).m2;
     p.m2_20 = compute_margins(d, LTDI_GEN_20, M - 1, 0).m2;
     p.inv_fd1 = 1.0 / ((mg.w == 1 ? 2.0 : 12.0) * rp.dt);
@@ -488,8 +490,9 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
     const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
     const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double) +
-                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 4) * sizeof(double) + /* + raw strain */
-                                 (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float);                            /* + low parts */
+                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 2 * LFA_RAW_HALO) * sizeof(double) + /* + raw strain */
+                                 (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float) +                           /* + low parts */
+                                 (rp.lfa_terms >= 2 ? smem_strain : 0);                                     /* + d^3h/dt^3 numerators */
     const size_t smem_link_hyb = std::max(smem_link, smem_link_lfa);
     const size_t smem_tdi_full = tdi_smem_bytes<M>(LTDI_RESPONSE_FULL, mg.m2, mg.w);
     const size_t smem_tdi_hyb = tdi_smem_bytes<M>(LTDI_RESPONSE_HYBRID, mg.m2, mg.w);
@@ -620,8 +623,12 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
 int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
-                 double *d_y, void *d_work, size_t work_bytes, void *stream)
+                 double *d_y, void *d_work, size_t work_bytes, void *stream, int lfa_terms = 1,
+                 int lfa_point = LTDI_LFA_CENTRAL)
 {
+    if (lfa_terms < 1 || lfa_terms > 2 || lfa_point < LTDI_LFA_CENTRAL || lfa_point > LTDI_LFA_FORWARD) return LTDI_EINVAL;
+    if (lfa_terms == 2 && lfa_point != LTDI_LFA_CENTRAL) return LTDI_EINVAL;
+    if ((lfa_terms != 1 || lfa_point != LTDI_LFA_CENTRAL) && which != LTDI_RESPONSE_LFA) return LTDI_EINVAL;
     if (!orb || !d_hp || !d_hc || !h_src || !d_A || !d_E || !d_T || !d_work) return LTDI_EINVAL;
     if (!gen_ok(gen) || !order_ok(order) || batch < 1 || ld < orb->desc.n) return LTDI_EINVAL;
     if (which != LTDI_RESPONSE_FULL && fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
@@ -648,7 +655,9 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     DeviceState &ds = *dsp;
     cudaStream_t st = (cudaStream_t)stream;
     const ltdi_orbit_desc &d = orb->desc;
-    const Margins mg = compute_margins(d, gen, order, fd_order);
+    Margins mg = compute_margins(d, gen, order, fd_order);
+    const int xw = lfa_terms >= 2 ? 1 : 0;   /* the third-derivative stencil is one sample wider than the first */
+    mg.lo += xw; mg.hi += xw;
     const int M = order + 1;
 
     /* hybrid on the tuned path: the tile plan (host integers; see classify_blocks / hyb_counts) */
@@ -717,6 +726,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.which = which; p.gen = gen; p.M = M; p.fd = fd_order;
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi;
     p.qmax = (int)(mg.m1 - M / 2);
+    p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw;
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
     if (fast_order(order)) {
@@ -744,7 +754,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     for (;;) {
         p.tile = tile;
         p.yr = (int)(tile + mg.m2 + M / 2 + 1);
-        p.hw = (int)(p.yr + 2 * mg.m1 + 6 * mg.w + 2);
+        p.hw = (int)(p.yr + 2 * mg.m1 + 6 * mg.w + 2 + 2 * xw);
         const int w = (int)mg.w;
         size_t off = 0;
         if (which != LTDI_RESPONSE_LFA) off += 6 * (size_t)p.yr;
@@ -965,6 +975,26 @@ int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *
 {
     return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
                         0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream);
+}
+
+int ltdi_response_lfa_ext(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                          const ltdi_source *h_src, int gen, int lagrange_order, int fd_order, int terms, int point,
+                          double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
+                          size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
+                        0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, terms, point);
+}
+
+int ltdi_margins_lfa_ext(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int terms, int64_t *lo,
+                         int64_t *hi)
+{
+    if (terms < 1 || terms > 2 || (fd_order != 2 && fd_order != 4)) return LTDI_EINVAL;
+    const int rc = ltdi_margins(desc, gen, lagrange_order, fd_order, lo, hi);
+    if (rc) return rc;
+    *lo += terms - 1;
+    *hi += terms - 1;
+    return LTDI_OK;
 }
 
 int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,

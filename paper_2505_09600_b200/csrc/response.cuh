@@ -30,6 +30,7 @@ struct RespParams {
     int hw;               /* samples of staged strain per tile */
     int off_yL, off_dL, off_hs; /* shared-memory offsets (doubles) of the LFA links, their derivative, the strain */
     int qmax;             /* bound on |integer shift| of a projection delay (m1 - M/2) */
+    int lfa_terms, lfa_point, xw; /* terms of Eq. (B4), expansion point LTDI_LFA_*, xw = terms - 1 */
     int64_t ntiles;
 };
 
@@ -201,7 +202,18 @@ __device__ __forceinline__ double fd1_num(const double *x)
     return 8.0 * (x[1] - x[-1]) - (x[2] - x[-2]);
 }
 
-// Eq. (B10) at the retarded time (B1): the three links l = +1, +2, +3 at sample m
+// third central difference of the strain times (2 dt^3) resp. (8 dt^3): numerators only, written as
+// differences of symmetric pairs
+template <int FD>
+__device__ __forceinline__ double fd3_num(const double *x)
+{
+    const double p1 = x[1] - x[-1], p2 = x[2] - x[-2];
+    if (FD == 2) return p2 - 2.0 * p1;
+    return 8.0 * p2 - 13.0 * p1 - (x[3] - x[-3]);
+}
+
+// Eq. (B10) at the retarded time (B1): the three links l = +1, +2, +3 at sample m.  SURVEY 8(f)-2: with
+// p.lfa_terms = 2 the m = 1 term of Eq. (B4) is added; p.lfa_point moves the expansion point to (B13) / (B14).
 template <int MT, bool STAGE>
 __device__ __forceinline__ void links_lfa(const RespParams &p, const Strain<STAGE> &h, const double *fr, int64_t m,
                                           double y[3])
@@ -212,12 +224,15 @@ __device__ __forceinline__ void links_lfa(const RespParams &p, const Strain<STAG
     const int Mx = MT ? MT : p.M;
     const int half = Mx / 2 - 1;
     const double den = (p.fd == 2 ? 2.0 : 12.0) * p.dt;
+    const double den3 = (p.fd == 2 ? 2.0 : 8.0) * p.dt * p.dt * p.dt;
 #pragma unroll
     for (int l = 0; l < 3; ++l) {
         const int s = link_sender(l), r = link_receiver(l);
         int q;
         double eps;
-        split_delay(0.5 * g.L[l] + 0.5 * (g.kR[s] + g.kR[r]), p.dt, q, eps);
+        const double tau = p.lfa_point == LTDI_LFA_CENTRAL ? 0.5 * g.L[l] + 0.5 * (g.kR[s] + g.kR[r])      /* (B1) */
+                           : p.lfa_point == LTDI_LFA_BACKWARD ? g.L[l] + g.kR[s] : g.kR[r];                 /* (B13), (B14) */
+        split_delay(tau, p.dt, q, eps);
         q = clamp_shift(q, p.qmax);
         lag.weights(eps, p.M);
         const double *xp = h.plus(m - q - half), *xc = h.cross(m - q - half);
@@ -235,7 +250,17 @@ __device__ __forceinline__ void links_lfa(const RespParams &p, const Strain<STAG
                 ac = fma(lag.w[i], fd1_num<4>(xc + i), ac);
             }
         }
-        y[l] = -(0.5 * g.L[l]) * (g.Fp[l] * (ap / den) + g.Fc[l] * (ac / den));
+        double dH = g.Fp[l] * (ap / den) + g.Fc[l] * (ac / den);
+        if (p.lfa_terms >= 2) {   /* m = 1 term of (B4): (1/6) [(L_l / 2)(1 - k.n_l)]^2 d^3H/dt^3 */
+            double bp = 0.0, bc = 0.0;
+            for (int i = 0; i < Mx; ++i) {
+                bp = fma(lag.w[i], p.fd == 2 ? fd3_num<2>(xp + i) : fd3_num<4>(xp + i), bp);
+                bc = fma(lag.w[i], p.fd == 2 ? fd3_num<2>(xc + i) : fd3_num<4>(xc + i), bc);
+            }
+            const double hf = (0.5 * g.L[l]) * (1.0 - g.kn[l]);
+            dH += hf * hf / 6.0 * (g.Fp[l] * (bp / den3) + g.Fc[l] * (bc / den3));
+        }
+        y[l] = -(0.5 * g.L[l]) * dH;
     }
 }
 
@@ -357,7 +382,7 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
     const int64_t src_off = b * p.ld;
     if (STAGE) {
         /* phase H: every sample any stencil of this tile can touch, clipped to the grid */
-        const int64_t h0 = y0 - p.m1 - 3 * w;
+        const int64_t h0 = y0 - p.m1 - 3 * w - p.xw;
         for (int i = tid; i < p.hw; i += nthr) {
             const int64_t g = h0 + i;
             const bool in = g >= 0 && g < p.n;
@@ -388,7 +413,7 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
         for (int i = tid; i < len; i += nthr) {
             const int64_t m = y0 - w + i;
             double y[3] = {0.0, 0.0, 0.0};
-            if (m >= p.m1 + w && m < p.n - p.m1 - w) links_lfa<MT, STAGE>(p, h, fr, m, y);
+            if (m >= p.m1 + w + p.xw && m < p.n - p.m1 - w - p.xw) links_lfa<MT, STAGE>(p, h, fr, m, y);
 #pragma unroll
             for (int l = 0; l < 3; ++l) yL[(size_t)l * len + i] = y[l];
         }
@@ -397,7 +422,7 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
         const double dt = p.dt;
         for (int i = tid; i < p.yr; i += nthr) {
             const int64_t m = y0 + i;
-            const bool in = m >= p.m1 + 2 * w && m < p.n - p.m1 - 2 * w;
+            const bool in = m >= p.m1 + 2 * w + p.xw && m < p.n - p.m1 - 2 * w - p.xw;
 #pragma unroll
             for (int l = 0; l < 3; ++l) {
                 const double *x = yL + (size_t)l * len + i + w; /* x[0] = y_l[m] */

@@ -435,3 +435,72 @@ def test_decayed_ringdown_tail_keeps_relative_accuracy(ltdi, orc80):
                 err, floor = np.linalg.norm(g - w80) / nrm, np.linalg.norm(w64 - w80) / nrm
                 record(label=[which], series=c, window=[int(a), int(b)], err=float(err), floor=float(floor), bar=TOL)
                 assert err <= TOL, (which, c, (a, b), err, floor)
+
+
+# ---- higher-order and alternative LFA (Eqs. (B4), (B13), (B14)) ------------------------------------
+
+def run_lfa_ext(ltdi, orc, cfg, gen, fd, terms, point, order=None, idx=None):
+    n = cfg["n"]
+    order = order or cfg["order"]
+    idx = list(range(cfg["batch"])) if idx is None else idx
+    hp, hc, ang, _ = W.sources(cfg, idx)
+    orbit = cfg["orbit"]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    ref = orc.response_lfa_ext(orbit, hp, hc, ang, gen, order, fd, terms, point)
+    out = ltdi.response_lfa_ext(orb, torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev), ang, gen, order, fd,
+                                terms, point, True, True)
+    torch.cuda.synchronize()
+    out = to_numpy(out)
+    lo, hi = orc.margins_lfa_ext(orbit, gen, order, fd, terms)
+    assert (lo, hi) == ltdi.margins_lfa_ext(orbit, gen, order, fd, terms)
+    return out, ref, lo, hi
+
+
+@pytest.mark.parametrize("gen,fd,terms,point", [(20, 2, 2, 0), (20, 4, 2, 0), (15, 2, 2, 0), (15, 4, 2, 0),
+                                                (20, 2, 1, 1), (20, 2, 1, 2), (15, 4, 1, 1), (15, 4, 1, 2)])
+def test_lfa_ext_config2(ltdi, orc80, gen, fd, terms, point):
+    """m = 1 term of Eq. (B4) and the backward / forward expansion points on config 2's merger (tuned path, p = 31)"""
+    cfg = W.config(2, n=40007)
+    out, ref, lo, hi = run_lfa_ext(ltdi, orc80, cfg, gen, fd, terms, point)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("terms,point", [(2, 0), (1, 1), (1, 2)])
+def test_lfa_ext_config3_gen20(ltdi, orc80, terms, point):
+    """the worst-conditioned case (config 3, TDI 2.0: Eq. (B33) amplifies the noise of y by 2.45 / (omega dt)^2)"""
+    cfg = W.config(3, n=30011)
+    out, ref, lo, hi = run_lfa_ext(ltdi, orc80, cfg, 20, 2, terms, point)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+def test_lfa_ext_terms1_is_the_lfa_bitwise(ltdi):
+    cfg = W.config(2, n=20011)
+    hp, hc, ang, _ = W.sources(cfg, [0])
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    for order in (31, 5):
+        a = to_numpy(ltdi.response_lfa(orb, dhp, dhc, ang, 20, order, 2, True, True))
+        b = to_numpy(ltdi.response_lfa_ext(orb, dhp, dhc, ang, 20, order, 2, 1, ltdi.LFA_CENTRAL, True, True))
+        for k in a:
+            assert np.array_equal(a[k], b[k]), (order, k)
+
+
+@pytest.mark.parametrize("order,terms,point", [(5, 2, 0), (5, 1, 1), (9, 2, 0), (9, 1, 2)])
+def test_lfa_ext_other_orders_and_batch(ltdi, orc80, order, terms, point):
+    """generic kernel (p = 5) and the tuned p = 9 path, a batch of sources with a ragged length"""
+    cfg = W.config(4, n=9001, batch=3)
+    out, ref, lo, hi = run_lfa_ext(ltdi, orc80, cfg, 20, 4 if order == 9 else 2, terms, point, order=order)
+    check(out, ref, lo, hi, cfg["n"])
+
+
+def test_lfa_ext_argument_errors(ltdi):
+    cfg = W.config(2, n=5003)
+    hp, hc, ang, _ = W.sources(cfg, [0])
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    for terms, point in ((0, 0), (3, 0), (2, 1), (2, 2), (1, 3), (1, -1)):
+        with pytest.raises(ltdi.LtdiError):
+            ltdi.response_lfa_ext(orb, dhp, dhc, ang, 20, 31, 2, terms, point)
