@@ -19,7 +19,7 @@ import numpy as np
 from . import build as _build
 
 GEN_15, GEN_20 = 15, 20
-ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES = 0, 1, 2
+ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES, ORBIT_KNOTS = 0, 1, 2, 3
 TAPER_SIGMOID, TAPER_COSINE = 0, 1
 
 
@@ -71,6 +71,10 @@ class Oracle:
 
     @staticmethod
     def _tables(orbit):
+        if int(orbit["mode"]) == ORBIT_KNOTS:   # a numerical orbit file: knots [3][3][nk] and {t0, dt, nk, order} of the knot grid
+            K = _f64(orbit["knots"])
+            assert K.ndim == 3 and K.shape[:2] == (3, 3)
+            return K, _f64([orbit["knot_t0"], orbit["knot_dt"], K.shape[2], orbit["knot_order"]])
         if int(orbit["mode"]) != ORBIT_TABLES:
             return None, None
         R = _f64(orbit["R_table"])   # [3][3][n]
@@ -217,6 +221,40 @@ class Oracle:
 
     def response_full(self, orbit, hp, hc, sources, gen, order, nb=0, ne=None, want=("XYZ", "y")):
         return self._run("full", orbit, hp, hc, sources, gen, order, 0, None, nb, ne, want)
+
+    def response_full_nested(self, orbit, hp, hc, sources, gen, order, nested_order=3, nb=0, ne=None, want=("XYZ", "y")):
+        """the full response with properly nested TDI delays (O12); nested_order = Lagrange order of the
+        light-time lookups at off-grid times."""
+        hp, hc = np.atleast_2d(_f64(hp)), np.atleast_2d(_f64(hc))
+        batch, ld = hp.shape
+        src, ns = self._sources(sources)
+        assert ns == batch and ld >= orbit["n"]
+        ne = orbit["n"] if ne is None else ne
+        ln = ne - nb
+        out = {"A": np.zeros((batch, ln)), "E": np.zeros((batch, ln)), "T": np.zeros((batch, ln))}
+        out["XYZ"] = np.zeros((3, batch, ln)) if "XYZ" in want else None
+        out["y"] = np.zeros((6, batch, ln)) if "y" in want else None
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_response_full_nested(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(hp), _ptr(hc), C.c_int64(ld),
+                                               C.c_int64(batch), src, C.c_int(gen), C.c_int(order), C.c_int(nested_order),
+                                               C.c_int64(nb), C.c_int64(ne), _ptr(out["A"]), _ptr(out["E"]), _ptr(out["T"]),
+                                               _ptr(out["XYZ"]), _ptr(out["y"]))
+        if rc != 0:
+            raise ValueError(f"oracle full_nested: status {rc}")
+        return out
+
+    def michelson_nested_from_links(self, orbit, y, gen, order, nested_order=3):
+        """X, Y, Z [3][n] with nested delays (O12) from caller-supplied link series y [6][n]."""
+        y = _f64(y)
+        assert y.shape == (6, orbit["n"])
+        out = np.zeros((3, orbit["n"]))
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_michelson_nested_from_links(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(y), C.c_int(gen), C.c_int(order),
+                                                      C.c_int(nested_order), _ptr(out))
+        assert rc == 0
+        return out
 
     def response_lfa(self, orbit, hp, hc, sources, gen, order, fd_order, nb=0, ne=None,
                      want=("XYZ", "y")):

@@ -103,7 +103,7 @@ def lib():
     """Load (building first if the sources are newer) liblisatdi.so; raises if that fails."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = os.environ.get("LTDI_LIBRARY") or _build.build()   # LTDI_LIBRARY: an already built liblisatdi.so to load instead
         handle = C.CDLL(path)
         for name, (res, args) in _SIGNATURES.items():
             fn = getattr(handle, name)   # AttributeError if the library does not export it

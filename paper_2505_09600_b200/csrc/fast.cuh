@@ -312,40 +312,54 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
 // ---------------------------------------------------------------------------------------------
 #define LFA_ANC_DOUBLES 28
 #define LFA_LO_ROWS 12
-#define LFA_RAW_HALO 3   /* raw strain staged beyond the FD series on either side: the widest stencil (d^3/dt^3, order 4) */
+#define LFA_RAW_HALO 4   /* raw strain staged beyond the FD series on either side: the widest stencil (d^3/dt^3, order 4) needs 3;
+                          * even, so that the staged run starts on a 16-byte boundary for the bulk copy */
 
-__device__ __forceinline__ dd quad_form_dd(const double *P, const dd *n, double *g)
-{
-    /* t = P n (dd), g = 2 t (fp64), result n . t */
-    const dd t0 = dd_add(dd_add(dd_mul_d(n[0], P[0]), dd_mul_d(n[1], P[3])), dd_mul_d(n[2], P[4]));
-    const dd t1 = dd_add(dd_add(dd_mul_d(n[0], P[3]), dd_mul_d(n[1], P[1])), dd_mul_d(n[2], P[5]));
-    const dd t2 = dd_add(dd_add(dd_mul_d(n[0], P[4]), dd_mul_d(n[1], P[5])), dd_mul_d(n[2], P[2]));
-    g[0] = 2.0 * t0.hi; g[1] = 2.0 * t1.hi; g[2] = 2.0 * t2.hi;
-    return dd_add(dd_add(dd_mul(n[0], t0), dd_mul(n[1], t1)), dd_mul(n[2], t2));
-}
-
-__device__ __noinline__ void lfa_anchor(const double *fr, const double *tb, const float *tl, int l, int ic, double *s_anc)
+// One warp per link: lanes 0..15 = (polarisation = lane >> 3, element e = lane & 7); e < 6 holds one element P_e of the
+// symmetric matrix and its term (1 | 2) P_e n_a n_b of the quadratic form in double-double, summed over the eight lanes
+// of the polarisation by a shuffle tree; lanes 16..21 form g = 2 P n_c, lanes 22..24 store n_c.  (As three serial
+// threads this was a fifth of the kernel's time: everybody else waited at the barrier behind ~600 dependent flops.)
+__device__ __forceinline__ void lfa_anchor_warp(const double *fr, const double *tb, const float *tl, int l, int ic,
+                                                double *s_anc, int lane)
 {
     double *an = s_anc + l * LFA_ANC_DOUBLES;
     const double *u = fr + 3, *v = fr + 6;
     const double c2 = fr[9], s2 = fr[10];
-    const int ia[6] = {0, 1, 2, 0, 0, 1}, ib[6] = {0, 1, 2, 1, 2, 2};
+    const int pol = (lane >> 3) & 1, e = lane & 7;
+    const int ia = e < 3 ? e : (e == 5 ? 1 : 0), ib = e < 3 ? e : (e == 3 ? 1 : 2);   /* xx yy zz xy xz yz */
+    const bool term = lane < 16 && e < 6;
+    const int ja = term ? ia : 0, jb = term ? ib : 0;
+    const double dp = u[ja] * u[jb] - v[ja] * v[jb];     /* (2.4a) as a matrix */
+    const double dc = u[ja] * v[jb] + v[ja] * u[jb];     /* (2.4b) */
+    const double P = pol == 0 ? dp * c2 + dc * s2 : dc * c2 - dp * s2;   /* (2.2) + (2.3), G17 */
+    const dd na = dd_make(tb[(ROW_N + 3 * l + ja) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + ja) * FAST_TA + ic]);
+    const dd nb = dd_make(tb[(ROW_N + 3 * l + jb) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + jb) * FAST_TA + ic]);
+    dd t = dd_mul_d(dd_mul(na, nb), e < 3 ? P : 2.0 * P);
+    if (!term) t = dd_make(0.0, 0.0);
 #pragma unroll
-    for (int e = 0; e < 6; ++e) {
-        const double dp = u[ia[e]] * u[ib[e]] - v[ia[e]] * v[ib[e]];     /* (2.4a) as a matrix */
-        const double dc = u[ia[e]] * v[ib[e]] + v[ia[e]] * u[ib[e]];     /* (2.4b) */
-        an[16 + e] = dp * c2 + dc * s2;                                  /* (2.2) + (2.3), G17 */
-        an[22 + e] = dc * c2 - dp * s2;
+    for (int o = 4; o > 0; o >>= 1) {
+        const dd q = dd_make(__shfl_xor_sync(0xffffffffu, t.hi, o), __shfl_xor_sync(0xffffffffu, t.lo, o));
+        t = dd_add(t, q);
     }
-    dd n[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        n[a] = dd_make(tb[(ROW_N + 3 * l + a) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + a) * FAST_TA + ic]);
-        an[10 + a] = n[a].hi;
-        an[13 + a] = n[a].lo;
+    if (lane < 16 && e == 0) { an[2 * pol] = t.hi; an[2 * pol + 1] = t.lo; }
+    if (term) an[16 + 6 * pol + e] = P;
+    /* g[a] = 2 sum_b P_ab n_b: lanes 16..21 = (polarisation, a) */
+    const int gl = lane - 16, gpol = gl >= 3 ? 1 : 0, ga = gl - 3 * gpol;
+    const int a_ = (gl >= 0 && gl < 6) ? ga : 0;
+    const int e0 = a_ == 0 ? 0 : (a_ == 1 ? 3 : 4), e1 = a_ == 0 ? 3 : (a_ == 1 ? 1 : 5), e2 = a_ == 0 ? 4 : (a_ == 1 ? 5 : 2);
+    const int base = 8 * ((gl >= 0 && gl < 6) ? gpol : 0);
+    const double P0 = __shfl_sync(0xffffffffu, P, base + e0), P1 = __shfl_sync(0xffffffffu, P, base + e1),
+                 P2 = __shfl_sync(0xffffffffu, P, base + e2);
+    if (gl >= 0 && gl < 6) {
+        const double n0 = tb[(ROW_N + 3 * l) * FAST_TA + ic], n1 = tb[(ROW_N + 3 * l + 1) * FAST_TA + ic],
+                     n2 = tb[(ROW_N + 3 * l + 2) * FAST_TA + ic];
+        an[4 + 3 * gpol + ga] = 2.0 * (P0 * n0 + P1 * n1 + P2 * n2);
     }
-    const dd Fp = quad_form_dd(an + 16, n, an + 4), Fc = quad_form_dd(an + 22, n, an + 7);
-    an[0] = Fp.hi; an[1] = Fp.lo; an[2] = Fc.hi; an[3] = Fc.lo;
+    if (lane >= 22 && lane < 25) {
+        const int a = lane - 22;
+        an[10 + a] = tb[(ROW_N + 3 * l + a) * FAST_TA + ic];
+        an[13 + a] = (double)tl[(LO_N + 3 * l + a) * FAST_TA + ic];
+    }
 }
 
 // y^LFA of one sample: n = (nx, ny, nz) + (lx, ly, lz), L = L_hi + L_lo, dh/dt numerators (pref + ap), (cref + ac)
@@ -401,17 +415,26 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     const int hw2 = (int)((FAST_TA + 2 * p.m1 + 4) / 2);   /* pairs */
     double *he_p = smem, *ho_p = he_p + hw2, *he_c = ho_p + hw2, *ho_c = he_c + hw2;
     const double *gp = p.hp + b * p.ld, *gc = p.hc + b * p.ld;
-    /* orbit-table rows of the tile: rows 0..23 (full) or 0..20 (LFA: R, n, L_+l), [row][FAST_TA] */
+    /* orbit-table rows of the tile: rows 0..23 (full) or 0..20 (LFA: R, n, L_+l), [row][FAST_TA].  Contiguous runs go
+     * through TMA bulk copies on an mbarrier, issued by the lanes of warp 0 (one row each): as per-element cp.async
+     * loops the staging was a fifth of the LFA kernel's executed instructions (ncu r02a).  A row is copied up to the
+     * table stride; what lies beyond (a tail tile) is only read by samples >= n, whose outputs are never stored. */
     constexpr int NROWS = LFA ? ROW_L + 3 : LTDI_TABLE_ROWS;
     double *tb = ho_c + hw2;
-    for (int i = tid; i < NROWS * (FAST_TA / 2); i += FAST_TA_THREADS) {
-        const int r = i / (FAST_TA / 2), c = 2 * (i - r * (FAST_TA / 2));
-        if (a0 + c < p.stride) cp_async16(tb + r * FAST_TA + c, p.tab + (int64_t)r * p.stride + a0 + c);
-        else *reinterpret_cast<double2 *>(tb + r * FAST_TA + c) = make_double2(0.0, 0.0);
-    }
+    __shared__ uint64_t s_bar;
+    const unsigned nl = (unsigned)min((int64_t)FAST_TA, p.stride - a0);   /* a multiple of 32 elements */
     float *tl = nullptr;   /* LFA: low parts of the dd table entries of the tile */
     double *he3_p = nullptr; /* LFA, terms = 2: [4][hw2] third-derivative numerators (even +, odd +, even x, odd x) */
     if (!LFA) {
+        if (tid < 32) {
+            if (tid == 0) {
+                mbar_init(&s_bar, 1);
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+                mbar_expect_tx(&s_bar, NROWS * nl * 8u);
+            }
+            __syncwarp();
+            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA, p.tab + (int64_t)tid * p.stride + a0, nl * 8u, &s_bar);
+        }
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
             double *dp = ((i & 1) ? ho_p : he_p) + (i >> 1), *dc = ((i & 1) ? ho_c : he_c) + (i >> 1);
@@ -425,36 +448,53 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         }
         cp_async_wait_all();
         __syncthreads();
+        mbar_wait(&s_bar, 0);
     } else {
-        /* raw strain of samples org - 3 .. org + 2 hw2 + 2 (asynchronous), then the FD1 numerators (G15) */
+        /* raw strain of samples org - 4 .. org + 2 hw2 + 3, then the FD1 numerators (G15); low parts of n_l (9 rows)
+         * and of L_+l (3 rows): float rows LO_N .. LO_L + 2 of the table */
         const int nraw = 2 * hw2 + 2 * LFA_RAW_HALO;
         double *raw_p = tb + NROWS * FAST_TA, *raw_c = raw_p + nraw;
-        for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
-            const int64_t g = org - LFA_RAW_HALO + j;
-            if (g >= 0 && g < p.n) {
-                cp_async8(raw_p + j, gp + g);
-                cp_async8(raw_c + j, gc + g);
-            } else {
-                raw_p[j] = 0.0;
-                raw_c[j] = 0.0;
+        tl = reinterpret_cast<float *>(raw_c + nraw);
+        const int64_t rs = org - LFA_RAW_HALO;                                   /* even */
+        const int64_t g_lo = max(rs, (int64_t)0), g_hi = min(rs + nraw, p.n);
+        const int ncopy = (int)max(g_hi - g_lo, (int64_t)0);
+        /* one bulk copy per series needs 16-byte aligned ends (an odd ld or n falls back to element copies) */
+        const bool bulk = ncopy > 0 && !(ncopy & 1) &&
+                          !((reinterpret_cast<uintptr_t>(gp + g_lo) | reinterpret_cast<uintptr_t>(gc + g_lo)) & 15);
+        if (tid < 32) {
+            if (tid == 0) {
+                mbar_init(&s_bar, 1);
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+                mbar_expect_tx(&s_bar, NROWS * nl * 8u + LFA_LO_ROWS * nl * 4u + (bulk ? 2u * ncopy * 8u : 0u));
+            }
+            __syncwarp();
+            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA, p.tab + (int64_t)tid * p.stride + a0, nl * 8u, &s_bar);
+            if (tid < LFA_LO_ROWS) {
+                const float *glo = reinterpret_cast<const float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride);
+                bulk_g2s(tl + tid * FAST_TA, glo + (int64_t)tid * p.stride + a0, nl * 4u, &s_bar);
+            }
+            if (bulk && tid >= 30) {
+                const double *src = tid == 30 ? gp : gc;
+                bulk_g2s((tid == 30 ? raw_p : raw_c) + (g_lo - rs), src + g_lo, ncopy * 8u, &s_bar);
             }
         }
-        /* low parts of n_l (9 rows) and of L_+l (3 rows): float rows LO_N .. LO_L + 2 of the table */
-        tl = reinterpret_cast<float *>(raw_c + nraw);
-        {
-            const float *glo = reinterpret_cast<const float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride);
-            for (int i = tid; i < LFA_LO_ROWS * (FAST_TA / 4); i += FAST_TA_THREADS) {
-                const int r = i / (FAST_TA / 4), c = 4 * (i - r * (FAST_TA / 4));
-                if (a0 + c < p.stride) cp_async16(tl + r * FAST_TA + c, glo + (int64_t)r * p.stride + a0 + c);
-                else *reinterpret_cast<float4 *>(tl + r * FAST_TA + c) = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
+            const int64_t g = rs + j;
+            if (g < g_lo || g >= g_hi) {
+                raw_p[j] = 0.0;
+                raw_c[j] = 0.0;
+            } else if (!bulk) {
+                cp_async8(raw_p + j, gp + g);
+                cp_async8(raw_c + j, gc + g);
             }
         }
         /* SURVEY 8(f)-2, terms = 2: the d^3h/dt^3 numerators, parity-split like the first-derivative series */
         he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * FAST_TA);
         cp_async_wait_all();
         __syncthreads();
-        /* tile anchors of the antenna patterns (threads of the last warp, beside the stencil pass below) */
-        if (tid >= FAST_TA_THREADS - 3) lfa_anchor(fr, tb, tl, FAST_TA_THREADS - 1 - tid, (int)min((int64_t)(FAST_TA / 2), p.n - 1 - a0), s_anc);
+        mbar_wait(&s_bar, 0);
+        /* tile anchors of the antenna patterns: warp l builds the anchor of link l, then joins the stencil pass */
+        if (tid < 96) lfa_anchor_warp(fr, tb, tl, tid >> 5, (int)min((int64_t)(FAST_TA / 2), p.n - 1 - a0), s_anc, tid & 31);
         const int ws = w + p.xw;   /* the widest stencil applied to the strain */
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -837,7 +877,10 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
 
 // WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
 template <int M, int WHICH>
-__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : 4) tdi_kernel(const __grid_constant__ FastParams p)
+#ifndef TDI_LFA_MINB
+#define TDI_LFA_MINB 4
+#endif
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : (WHICH == LTDI_RESPONSE_LFA ? TDI_LFA_MINB : 4)) tdi_kernel(const __grid_constant__ FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);

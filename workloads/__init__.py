@@ -307,3 +307,50 @@ def frozen_tables(orbit, R_snapshot, L_snapshot):
     o["R_table"] = np.repeat(np.asarray(R_snapshot, dtype=np.float64).reshape(3, 3, 1), n, axis=2)
     o["L_table"] = np.repeat(np.asarray(L_snapshot, dtype=np.float64).reshape(6, 1), n, axis=1)
     return o
+
+
+# ---------------------------------------------------------------------------------------
+# numerical orbit files (input data for SURVEY 8(f)-4; "realistic ESA orbits")
+# ---------------------------------------------------------------------------------------
+ORBIT_KNOTS = 3
+
+
+def numerical_orbit(n, dt, t0=0.0, knot_dt=DAY_S, knot_order=7, seed=11, arm_m=ARM_M, R_m=AU_M, period_s=YEAR_S,
+                    alpha0=0.0, rot0=0.0, scatter=5e-3):
+    """An orbit FILE as a mission would deliver it: spacecraft positions [3][3][nk] tabulated every knot_dt seconds.
+
+    The spacecraft move on exact Keplerian ellipses (Kepler's equation solved by Newton iteration) of the usual
+    cartwheel construction -- semi-major axis R, eccentricity and inclination from alpha = L / (2 R), phases 120
+    degrees apart -- with the eccentricity, inclination and phase of every spacecraft scattered by `scatter`
+    (relative; seeded), so that the three arms differ at the per-cent level and breathe by metres per second, as the
+    arms of ESA's numerically optimised orbits do.  The ellipses stand in for such a file: they are input data only
+    (neither the oracle nor the library knows how the knots were made)."""
+    rng = np.random.default_rng([seed, 4])
+    margin = (knot_order + 1) // 2 + 1
+    k0 = math.floor(t0 / knot_dt) - margin
+    nk = math.ceil((t0 + n * dt) / knot_dt) + margin - k0 + 1
+    tk0 = k0 * knot_dt
+    tk = tk0 + knot_dt * np.arange(nk)
+    a = arm_m / (2.0 * R_m)
+    nu = math.pi / 3.0 + 5.0 / 8.0 * a
+    e_nom = math.sqrt(1.0 + 4.0 * a * math.cos(nu) / math.sqrt(3.0) + 4.0 * a * a / 3.0) - 1.0
+    inc_nom = math.atan(a * math.sin(nu) / (math.sqrt(3.0) / 2.0 + a * math.cos(nu)))
+    om = 2.0 * math.pi / period_s
+    knots = np.zeros((3, 3, nk))
+    for i in range(3):
+        e = e_nom * (1.0 + scatter * rng.standard_normal())
+        inc = inc_nom * (1.0 + scatter * rng.standard_normal())
+        sig = 2.0 * math.pi * i / 3.0 + rot0 + scatter * 1e-1 * rng.standard_normal()
+        Mean = om * tk + alpha0 - sig
+        psi = Mean.copy()
+        for _ in range(12):                                   # psi + e sin psi = Mean
+            psi -= (psi + e * np.sin(psi) - Mean) / (1.0 + e * np.cos(psi))
+        xr = R_m * (np.cos(psi) + e) * math.cos(inc)
+        yr = R_m * math.sqrt(1.0 - e * e) * np.sin(psi)
+        zr = R_m * (np.cos(psi) + e) * math.sin(inc)
+        knots[i, 0] = math.cos(sig) * xr - math.sin(sig) * yr
+        knots[i, 1] = math.sin(sig) * xr + math.cos(sig) * yr
+        knots[i, 2] = zr
+    d = orbit_desc(n, dt, ORBIT_KNOTS, t0=t0, arm_m=arm_m, R_m=R_m, period_s=period_s, alpha0=alpha0, rot0=rot0)
+    d.update(knots=np.ascontiguousarray(knots), knot_t0=float(tk0), knot_dt=float(knot_dt), knot_order=int(knot_order))
+    return d
