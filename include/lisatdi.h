@@ -41,7 +41,8 @@ enum { LTDI_GEN_15 = 15, LTDI_GEN_20 = 20 };                 /* Eq. (2.7) / Eq. 
 enum {
     LTDI_ORBIT_STATIC_EQUALARM = 0, /* Keplerian positions, L_l(t) = arm_m / c constant ("equal and constant") */
     LTDI_ORBIT_KEPLERIAN = 1,       /* Keplerian positions, first-order light times, L_l != L_-l (G6)         */
-    LTDI_ORBIT_TABLES = 2           /* caller-supplied positions and light times per sample                           */
+    LTDI_ORBIT_TABLES = 2,          /* caller-supplied positions and light times per sample                           */
+    LTDI_ORBIT_KNOTS = 3            /* a numerical orbit file: positions tabulated at knots (ltdi_orbits_init_knots)    */
 };
 enum { LTDI_TAPER_SIGMOID = 0,      /* Eq. (4.1), the paper's weight                                  */
        LTDI_TAPER_COSINE = 1 };     /* raised cosine over the window (BASELINE.json configs 2, 4; G20) */
@@ -89,6 +90,18 @@ int ltdi_orbits_init(const ltdi_orbit_desc *desc, void *d_tables, size_t bytes, 
  * must be LTDI_ORBIT_TABLES; arm_m and R_m still size the margins. */
 int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L,
                             void *d_tables, size_t bytes, void *stream, ltdi_orbits **out);
+
+/* SURVEY.md 8(f)-4, numerical orbits ("realistic ESA orbits"; reading G28): d_knots [3][3][nk] (device; spacecraft,
+ * component, knot) holds the spacecraft positions [m] at the times knot_t0 + j knot_dt.  They are brought to every
+ * sample time by centred Lagrange interpolation of odd order knot_order <= 15 on the knot grid (taps
+ * k = -(M/2-1) .. M/2 around the knot at or before t, M = knot_order + 1), the velocities are the time derivative of
+ * that interpolant, n_l = (R_r - R_s) / |R_r - R_s| and L_l = (|R_r - R_s| / c)(1 + n_l . V_s / c) as for the Keplerian
+ * mode (G6).  desc->mode must be LTDI_ORBIT_KNOTS; arm_m and R_m size the margins.  The knots must cover the grid:
+ * knot_t0 + (M/2 - 1) knot_dt <= t0 and t0 + (n - 1) dt <= knot_t0 + (nk - 1 - M/2) knot_dt, else LTDI_EINVAL.
+ * d_knots is read by the kernel only (stream-ordered); the handle keeps no reference to it. */
+int ltdi_orbits_init_knots(const ltdi_orbit_desc *desc, const double *d_knots, int64_t nk, double knot_t0,
+                           double knot_dt, int knot_order, void *d_tables, size_t bytes, void *stream,
+                           ltdi_orbits **out);
 
 /* Optional: the TDI delays of Eqs. (2.7) / (2.8) and (B25) / (B33) are sums of L_l(t_n), so the
  * Lagrange weights of the TDI stage depend on the orbit object, the generation and the order only, not on

@@ -20,7 +20,7 @@ import torch
 from . import build as _build
 
 GEN_15, GEN_20 = 15, 20
-ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES = 0, 1, 2
+ORBIT_STATIC_EQUALARM, ORBIT_KEPLERIAN, ORBIT_TABLES, ORBIT_KNOTS = 0, 1, 2, 3
 TAPER_SIGMOID, TAPER_COSINE = 0, 1
 RESPONSE_FULL, RESPONSE_LFA, RESPONSE_HYBRID = 0, 1, 2
 LFA_CENTRAL, LFA_BACKWARD, LFA_FORWARD = 0, 1, 2
@@ -60,6 +60,8 @@ _SIGNATURES = {
     "ltdi_orbits_workspace_bytes": (C.c_int, [C.POINTER(OrbitDesc), _szp]),
     "ltdi_orbits_init": (C.c_int, [C.POINTER(OrbitDesc), _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
     "ltdi_orbits_init_tables": (C.c_int, [C.POINTER(OrbitDesc), _dp, _dp, _vp, C.c_size_t, _vp, C.POINTER(_vp)]),
+    "ltdi_orbits_init_knots": (C.c_int, [C.POINTER(OrbitDesc), _dp, C.c_int64, C.c_double, C.c_double, C.c_int, _vp,
+                                         C.c_size_t, _vp, C.POINTER(_vp)]),
     "ltdi_orbits_prepare_bytes": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, _szp]),
     "ltdi_orbits_prepare": (C.c_int, [_vp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
     "ltdi_orbits_destroy": (C.c_int, [_vp]),
@@ -196,7 +198,10 @@ def profile_read():
 class Orbits:
     """Device orbit tables for one time grid (S0, the orbit/delay kernel)."""
 
-    def __init__(self, desc, R_table=None, L_table=None, device="cuda:0"):
+    def __init__(self, desc, R_table=None, L_table=None, device="cuda:0", knots=None):
+        """desc: orbit_desc dict.  ORBIT_TABLES: R_table [3][3][n], L_table [6][n] device tensors.  ORBIT_KNOTS (a numerical
+        orbit file): knots [3][3][nk] device tensor (default: desc["knots"] uploaded) with desc["knot_t0"], ["knot_dt"],
+        ["knot_order"]."""
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2505_09600_b200 needs a CUDA device (no CPU fallback)")
         self.desc = dict(desc)
@@ -207,7 +212,15 @@ class Orbits:
         self.tables = torch.empty(nbytes.value // 8, dtype=torch.float64, device=self.device)
         handle = C.c_void_p()
         with torch.cuda.device(self.device):
-            if int(desc["mode"]) == ORBIT_TABLES:
+            if int(desc["mode"]) == ORBIT_KNOTS:
+                if knots is None:
+                    knots = torch.as_tensor(desc["knots"], dtype=torch.float64).contiguous().to(self.device)
+                self._knots = _dev_f64(knots, "knots")
+                assert self._knots.dim() == 3 and tuple(self._knots.shape[:2]) == (3, 3)
+                rc = lib().ltdi_orbits_init_knots(C.byref(d), self._knots.data_ptr(), int(self._knots.shape[2]),
+                                                  float(desc["knot_t0"]), float(desc["knot_dt"]), int(desc["knot_order"]),
+                                                  self.tables.data_ptr(), nbytes.value, _stream(), C.byref(handle))
+            elif int(desc["mode"]) == ORBIT_TABLES:
                 self._R = _dev_f64(R_table, "R_table")   # [3][3][n]
                 self._L = _dev_f64(L_table, "L_table")   # [6][n]
                 assert self._R.shape == (3, 3, d.n) and self._L.shape == (6, d.n)

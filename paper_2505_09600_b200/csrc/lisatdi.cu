@@ -169,15 +169,17 @@ Margins compute_margins(const ltdi_orbit_desc &d, int gen, int order, int fd_ord
 bool desc_ok(const ltdi_orbit_desc *d)
 {
     return d && d->n > 0 && d->dt > 0.0 && d->arm_m > 0.0 && d->R_m > 0.0 && d->period_s > 0.0 &&
-           d->mode >= LTDI_ORBIT_STATIC_EQUALARM && d->mode <= LTDI_ORBIT_TABLES;
+           d->mode >= LTDI_ORBIT_STATIC_EQUALARM && d->mode <= LTDI_ORBIT_KNOTS;
 }
 bool order_ok(int order) { return order >= 1 && order <= 63 && (order & 1); }
 bool gen_ok(int gen) { return gen == LTDI_GEN_15 || gen == LTDI_GEN_20; }
 
 int64_t table_stride(int64_t n) { return (n + 31) / 32 * 32; }
 
+struct KnotGrid { int64_t nk; double t0, dt; int order; };
+
 int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L, void *d_tables, size_t bytes,
-                  void *stream, ltdi_orbits **out)
+                  void *stream, ltdi_orbits **out, const KnotGrid *kg = nullptr)
 {
     if (!desc_ok(desc) || !d_tables || !out) return LTDI_EINVAL;
     const int64_t stride = table_stride(desc->n);
@@ -218,11 +220,19 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
         }
     }
     p.R_in = d_R; p.L_in = d_L; p.tab = (double *)d_tables;
+    if (kg) {
+        p.nk = kg->nk; p.tk0 = kg->t0; p.dtk = kg->dt; p.korder = kg->order;
+        p.inv_dtk = split(1.0L / (long double)kg->dt);
+        DeviceState *ds = nullptr;   /* the knot weights read the Lagrange denominators of the device */
+        const int rc = device_state(&ds);
+        if (rc) return rc;
+    }
     const int threads = 128;
     const int64_t blocks = (desc->n + threads - 1) / threads;
     {
         ProfScope ps(LTDI_KERNEL_ORBIT, (cudaStream_t)stream);
-        orbit_delay_kernel<<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
+        if (kg) orbit_delay_kernel<true><<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
+        else orbit_delay_kernel<false><<<(unsigned)blocks, threads, 0, (cudaStream_t)stream>>>(p);
     }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
@@ -862,8 +872,20 @@ int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes)
 
 int ltdi_orbits_init(const ltdi_orbit_desc *desc, void *d_tables, size_t bytes, void *stream, ltdi_orbits **out)
 {
-    if (desc && desc->mode == LTDI_ORBIT_TABLES) return LTDI_EINVAL;
+    if (desc && (desc->mode == LTDI_ORBIT_TABLES || desc->mode == LTDI_ORBIT_KNOTS)) return LTDI_EINVAL;
     return orbits_common(desc, nullptr, nullptr, d_tables, bytes, stream, out);
+}
+
+int ltdi_orbits_init_knots(const ltdi_orbit_desc *desc, const double *d_knots, int64_t nk, double knot_t0, double knot_dt,
+                           int knot_order, void *d_tables, size_t bytes, void *stream, ltdi_orbits **out)
+{
+    if (!desc_ok(desc) || desc->mode != LTDI_ORBIT_KNOTS || !d_knots) return LTDI_EINVAL;
+    if (knot_order < 1 || knot_order > 15 || !(knot_order & 1) || !(knot_dt > 0.0) || nk < knot_order + 1) return LTDI_EINVAL;
+    const int M = knot_order + 1;
+    const double t_end = desc->t0 + (double)(desc->n - 1) * desc->dt;
+    if (knot_t0 + (double)(M / 2 - 1) * knot_dt > desc->t0 || t_end > knot_t0 + (double)(nk - 1 - M / 2) * knot_dt) return LTDI_EINVAL;
+    const KnotGrid kg = {nk, knot_t0, knot_dt, knot_order};
+    return orbits_common(desc, d_knots, nullptr, d_tables, bytes, stream, out, &kg);
 }
 
 int ltdi_orbits_init_tables(const ltdi_orbit_desc *desc, const double *d_R, const double *d_L, void *d_tables,

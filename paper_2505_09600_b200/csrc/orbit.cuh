@@ -31,10 +31,39 @@ struct OrbitKernelParams {
     dd L_static;           /* arm / c */
     dd sin_c[11], cos_c[12]; /* (-1)^m / (2m+1)!, (-1)^m / (2m)! */
     int mode;
-    const double *R_in; /* tables mode: [3][3][n] */
+    const double *R_in; /* tables mode: [3][3][n]; knots mode: [3][3][nk] */
     const double *L_in; /* tables mode: [6][n] */
+    /* knots mode (numerical orbit files): knot j at time tk0 + j dtk, Lagrange order korder */
+    int64_t nk;
+    double tk0, dtk;
+    dd inv_dtk;
+    int korder;
     double *tab;
 };
+
+// Lagrange weights w_k(u) and their first derivative, k = -(M/2-1) .. M/2, M <= 16 (prefix x suffix products with the
+// product rule carried along; denominators from c_lag_inv_den)
+__device__ __forceinline__ void knot_weights(double u, int M, double *w, double *dw)
+{
+    const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
+    const int kmin = -(M / 2 - 1);
+    double pf[16], pf1[16];
+    double f = 1.0, f1 = 0.0;
+    for (int i = 0; i < M; ++i) {
+        pf[i] = f; pf1[i] = f1;
+        const double e = u - (double)(kmin + i);
+        f1 = f1 * e + f;
+        f = f * e;
+    }
+    double g = 1.0, g1 = 0.0;
+    for (int i = M - 1; i >= 0; --i) {
+        w[i] = c[i] * (pf[i] * g);
+        dw[i] = c[i] * (pf1[i] * g + pf[i] * g1);
+        const double e = u - (double)(kmin + i);
+        g1 = g1 * e + g;
+        g = g * e;
+    }
+}
 
 // sin and cos of a dd angle, absolute error < 1e-30 for |a| < 1e5: reduction by multiples of pi / 2 (three-part
 // constant), Taylor series on |r| <= pi / 4 -- the high-order tail (terms below 1e-11) in plain fp64
@@ -68,13 +97,15 @@ __device__ __forceinline__ void sincos_dd(dd a, const OrbitKernelParams &p, dd &
     }
 }
 
+// KNOTS: the numerical-orbit instance (kept apart: its stencil arrays would cost the analytic modes registers)
+template <bool KNOTS>
 __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant__ OrbitKernelParams p)
 {
     const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= p.n) return;
     double R[3][3], V[3][3];
     dd dv[3][3];   /* arm vectors R_r - R_s of links +1, +2, +3 [m] */
-    if (p.mode == LTDI_ORBIT_TABLES) {
+    if (!KNOTS && p.mode == LTDI_ORBIT_TABLES) {
 #pragma unroll
         for (int i = 0; i < 9; ++i) {
             R[i / 3][i % 3] = p.R_in[(int64_t)i * p.n + n];
@@ -85,6 +116,51 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
             const int s = link_sender(l), r = link_receiver(l);
 #pragma unroll
             for (int a = 0; a < 3; ++a) dv[l][a] = two_sum(R[r][a], -R[s][a]);
+        }
+    } else if (KNOTS) {
+        // Numerical orbit file (O11, G28): positions tabulated at knots, centred Lagrange interpolation of
+        // order korder on the knot grid; velocities = derivative of the interpolant.  Position in the grid in dd
+        // (t_n rounded to fp64 alone would move the arm vectors by 1e-6 m through the 500 m/s relative velocities).
+        dd t = two_prod((double)n, p.dt);
+        t = dd_add_d(t, p.t0);
+        const dd sg = dd_mul(dd_add_d(t, -p.tk0), p.inv_dtk);
+        double jf = floor(sg.hi);
+        double u = (sg.hi - jf) + sg.lo;
+        if (u < 0.0) { jf -= 1.0; u += 1.0; }
+        if (u >= 1.0) { jf += 1.0; u -= 1.0; }
+        const int M = p.korder + 1;
+        const int64_t j0 = (int64_t)jf - (M / 2 - 1);     /* first knot of the stencil (host: 0 <= j0, j0 + M <= nk) */
+        double w[16], dw[16];
+        knot_weights(u, M, w, dw);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) {
+            const double *K = p.R_in + (int64_t)i * p.nk + j0;
+            double acc = 0.0, dacc = 0.0;
+            for (int m = 0; m < M; ++m) {
+                acc = fma(w[m], K[m], acc);
+                dacc = fma(dw[m], K[m], dacc);
+            }
+            R[i / 3][i % 3] = acc;
+            V[i / 3][i % 3] = dacc / p.dtk;
+        }
+        // arm vectors: the knot differences D_m = K_r[m] - K_s[m] are formed without rounding (two_sum) and
+        // interpolated about the central knot, d = D_c + sum_m w_m (D_m - D_c): the rounding of the weights then acts
+        // on |D_m - D_c| ~ 1e8 m instead of on 2.5e9 m (weights sum to 1), which leaves 1e-8 m, 4e-18 of the arm
+        const int mc = M / 2 - 1;
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            const int s = link_sender(l), r = link_receiver(l);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const double *Kr = p.R_in + (int64_t)(3 * r + a) * p.nk + j0, *Ks = p.R_in + (int64_t)(3 * s + a) * p.nk + j0;
+                const dd Dc = two_sum(Kr[mc], -Ks[mc]);
+                double acc = 0.0;
+                for (int m = 0; m < M; ++m) {
+                    const dd Dm = two_sum(Kr[m], -Ks[m]);
+                    acc = fma(w[m], (Dm.hi - Dc.hi) + (Dm.lo - Dc.lo), acc);
+                }
+                dv[l][a] = dd_add_d(Dc, acc);
+            }
         }
     } else {
         // alpha(t) = Omega t + alpha0; spacecraft i: beta_i = 2 pi (i-1)/3 + rot0.  Positions to first order in the
@@ -145,7 +221,7 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
         dd Lp, Lm; /* link +l (s -> r) and -l (r -> s) */
         if (p.mode == LTDI_ORBIT_STATIC_EQUALARM) {
             Lp = Lm = p.L_static;
-        } else if (p.mode == LTDI_ORBIT_KEPLERIAN) {
+        } else if (KNOTS || p.mode == LTDI_ORBIT_KEPLERIAN) {
             // first-order light time |d|/c (1 + n.V_sender / c): L_l != L_-l (Eq. B22)
             const double nvs = nh[0].hi * V[s][0] + nh[1].hi * V[s][1] + nh[2].hi * V[s][2];
             const double nvr = -(nh[0].hi * V[r][0] + nh[1].hi * V[r][1] + nh[2].hi * V[r][2]);

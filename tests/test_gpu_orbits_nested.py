@@ -1,0 +1,85 @@
+"""GPU parity of SURVEY 8(f)-4: numerical orbit files (ltdi_orbits_init_knots) and properly nested TDI delays
+(ltdi_response_full_nested) against the long-double oracle (O11, O12)."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from parity_util import hybrid_params, strict_check, to_numpy
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ltdi():
+    import paper_2505_09600_b200 as m
+    assert torch.cuda.is_available(), "GPU parity tests need a CUDA device"
+    return m
+
+
+@pytest.mark.parametrize("t0,knot_order", [(1.0e7, 7), (3.1e7, 7), (2.0e6, 3), (5.0e6, 11)])
+def test_knot_orbit_tables(ltdi, orc80, t0, knot_order):
+    """S0 from a numerical orbit file: positions to a few roundings of 1 AU, link vectors and light times as hi + lo pairs
+    to 1e-16 relative (the arm vectors are interpolated as exact knot differences about the central knot)"""
+    orbit = W.numerical_orbit(50001, 5.0, t0=t0, knot_order=knot_order)
+    R, nh, L = orc80.orbit_tables(orbit)
+    nh_hi, nh_lo, L_hi, L_lo = orc80.orbit_tables_split(orbit)
+    orb = ltdi.Orbits(orbit)
+    rows, lo = orb.rows().cpu().numpy(), orb.rows_lo().double().cpu().numpy()
+    assert np.abs(rows[0:9].reshape(3, 3, -1) - R).max() <= 8 * np.spacing(np.abs(R).max())
+    dn = (rows[9:18].reshape(3, 3, -1) - nh_hi[:3]) + (lo[0:9].reshape(3, 3, -1) - nh_lo[:3])
+    dL = (rows[18:24] - L_hi) + (lo[9:15] - L_lo)
+    assert np.abs(dn).max() <= 1e-16, np.abs(dn).max()
+    assert np.abs(dL).max() <= 1e-16 * L.max(), np.abs(dL).max() / L.max()
+
+
+def test_knot_orbit_argument_errors(ltdi):
+    orbit = W.numerical_orbit(1000, 5.0, t0=1.0e6)
+    bad = dict(orbit, knots=orbit["knots"][:, :, :6])            # the knots do not cover the grid
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.Orbits(bad)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.Orbits(dict(orbit, knot_order=6))
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.Orbits(dict(orbit, knot_t0=orbit["knot_t0"] + 40 * orbit["knot_dt"]))
+
+
+def run_numeric(ltdi, orc, cfg, orbit, which, gen, fd=2, nested=0, taper=W.TAPER_COSINE):
+    n = cfg["n"]
+    hp, hc, ang, metas = W.sources(cfg, list(range(cfg["batch"])))
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    order = cfg["order"]
+    if which == "full" and nested:
+        ref = orc.response_full_nested(orbit, hp, hc, ang, gen, order, nested)
+        out = ltdi.response_full_nested(orb, dhp, dhc, ang, gen, order, nested, True, True)
+    elif which == "full":
+        ref = orc.response_full(orbit, hp, hc, ang, gen, order)
+        out = ltdi.response_full(orb, dhp, dhc, ang, gen, order, True, True)
+    elif which == "lfa":
+        ref = orc.response_lfa(orbit, hp, hc, ang, gen, order, fd)
+        out = ltdi.response_lfa(orb, dhp, dhc, ang, gen, order, fd, True, True)
+    else:
+        ref = orc.response_hybrid(orbit, hp, hc, ang, gen, order, fd, hybrid_params(metas, orc.hyb_time, taper, cfg["dt"]))
+        out = ltdi.response_hybrid(orb, dhp, dhc, ang, gen, order, fd, hybrid_params(metas, ltdi.hyb_time, taper, cfg["dt"]), True, True)
+    torch.cuda.synchronize()
+    lo, hi = orc.margins(orbit, gen, order, 0 if which == "full" else fd)
+    return to_numpy(out), ref, lo, hi
+
+
+@pytest.mark.parametrize("which,gen", [("full", 20), ("full", 15), ("lfa", 20), ("lfa", 15), ("hybrid", 20)])
+def test_responses_on_a_numerical_orbit(ltdi, orc80, which, gen):
+    """config 2's merger on the synthetic ESA-like orbit file: arms unequal by 0.3 %, breathing by up to 4 m/s"""
+    cfg = W.config(2, n=30011)
+    orbit = W.numerical_orbit(cfg["n"], cfg["dt"], t0=cfg["orbit"]["t0"])
+    out, ref, lo, hi = run_numeric(ltdi, orc80, cfg, orbit, which, gen)
+    strict_check(out, ref, lo, hi, cfg["n"])
+
+
+def test_batch_on_a_numerical_orbit_order9(ltdi, orc80):
+    cfg = W.config(4, n=12007, batch=3)
+    cfg["order"] = 9
+    orbit = W.numerical_orbit(cfg["n"], cfg["dt"], t0=4.0e6, knot_order=5)
+    out, ref, lo, hi = run_numeric(ltdi, orc80, cfg, orbit, "hybrid", 20)
+    strict_check(out, ref, lo, hi, cfg["n"])
