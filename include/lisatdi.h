@@ -156,6 +156,19 @@ int ltdi_response_full(const ltdi_orbits *orb, const double *d_hp, const double 
                        double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
                        size_t work_bytes, void *stream);
 
+/* SURVEY.md 8(f)-4, properly nested delays (the comparison case of P:151; the paper itself evaluates every L_l at t).
+ * Delay operators act as (D_l f)(t) = f(t - L_l(t)); with a = D_-2 D_2, b = D_3 D_-3 (for X; cyclic for Y, Z),
+ *   X_1.5 = (1 - b)(y_3-21 + D_-2 y_123) - (1 - a)(y_231 + D_3 y_1-32)
+ *   X_2.0 = (1 - b - b a + a b b)(y_3-21 + D_-2 y_123) - (1 - a - a b + b a a)(y_231 + D_3 y_1-32),
+ * i.e. Eqs. (2.7) / (2.8) term by term, but the delay of every term is accumulated along its chain of links,
+ * d_j = d_{j-1} + L_cj(t - d_{j-1}), the light travel time at an off-grid time being the centred Lagrange interpolation
+ * of order nested_order of the sampled L_l(t_n) (reading G29).  nested_order must be 3; Lagrange orders 9 and 31 only
+ * (LTDI_EUNSUPPORTED otherwise).  Everything else as ltdi_response_full. */
+int ltdi_response_full_nested(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                              int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int nested_order,
+                              double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
+                              size_t work_bytes, void *stream);
+
 /* Low-frequency approximation: Eq. (B10) links at the retarded time (B1) from central-difference
  * derivatives of h+, hx (S6), Eq. (B25) (gen 1.5) / (B33) (gen 2.0) Michelson (S7).  fd_order 2 | 4.
  * Links -1, -2, -3 are zero. */

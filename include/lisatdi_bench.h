@@ -38,6 +38,11 @@ int ltdi_profile_enable(int on);
 int ltdi_profile_read(int kernel, int which, double *total_ms, int64_t *launches);
 int ltdi_profile_reset(void);
 
+/* (TDI tile, channel) pairs of the current device that could not use the tile's weight anchors (light times drifting
+ * by more than the Taylor bound over a tile, or an integer shift stepping inside it) and took exact per-sample weights
+ * instead, since the last reset: a performance diagnostic -- the results are the same to rounding.  Synchronises. */
+int ltdi_profile_slow_tiles(int64_t *count, int reset);
+
 /* Number of kernel launches the library has issued in this process (for bench.py's gpu_launches). */
 int64_t ltdi_launch_count(void);
 

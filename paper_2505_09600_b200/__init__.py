@@ -73,6 +73,8 @@ _SIGNATURES = {
     "ltdi_workspace_bytes": (C.c_int, [C.c_int, C.c_int64, C.c_int64, C.c_int, C.c_int, _szp]),
     "ltdi_response_full": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                      _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_full_nested": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
+                                            _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                     C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa_ext": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
@@ -94,6 +96,7 @@ _SIGNATURES = {
     "ltdi_profile_read": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double), _i64p]),
     "ltdi_profile_reset": (C.c_int, []),
     "ltdi_launch_count": (C.c_int64, []),
+    "ltdi_profile_slow_tiles": (C.c_int, [_i64p, C.c_int]),
     "ltdi_version": (C.c_char_p, []),
 }
 EXPORTS = tuple(_SIGNATURES)
@@ -165,6 +168,13 @@ def hyb_time(f_hyb_hz, mchirp_s, t_c):
     out = C.c_double()
     _check("ltdi_hyb_time", lib().ltdi_hyb_time(f_hyb_hz, mchirp_s, t_c, C.byref(out)))
     return out.value
+
+
+def slow_tiles(reset=True):
+    """(TDI tile, channel) pairs that fell back to exact per-sample weights since the last reset (diagnostic)."""
+    n = C.c_int64()
+    _check("ltdi_profile_slow_tiles", lib().ltdi_profile_slow_tiles(C.byref(n), int(bool(reset))))
+    return n.value
 
 
 def launch_count():
@@ -307,7 +317,9 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
     tail = [p(ws.A), p(ws.E), p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream()]
     head = [orb.handle, hp.data_ptr(), hc.data_ptr(), ld, batch, src_ptr, gen, order]
     with torch.cuda.device(hp.device):
-        if which == RESPONSE_FULL:
+        if which == RESPONSE_FULL and ext is not None:
+            rc, fn = lib().ltdi_response_full_nested(*head, int(ext[0]), *tail), "ltdi_response_full_nested"
+        elif which == RESPONSE_FULL:
             rc, fn = lib().ltdi_response_full(*head, *tail), "ltdi_response_full"
         elif which == RESPONSE_LFA and ext is not None:
             rc, fn = lib().ltdi_response_lfa_ext(*head, fd_order, int(ext[0]), int(ext[1]), *tail), "ltdi_response_lfa_ext"
@@ -324,6 +336,11 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
 def response_full(orb, hp, hc, sources, gen, order, want_xyz=False, want_y=False, workspace=None):
     """Eqs. (2.2)-(2.9): projection, TDI `gen`, A, E, T.  Returns dict A, E, T (, XYZ, y)."""
     return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_xyz, want_y, workspace)
+
+
+def response_full_nested(orb, hp, hc, sources, gen, order, nested_order=3, want_xyz=False, want_y=False, workspace=None):
+    """the full response with properly nested TDI delays (light times looked up by Lagrange order 3)."""
+    return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_xyz, want_y, workspace, ext=(nested_order,))
 
 
 def response_lfa(orb, hp, hc, sources, gen, order, fd_order, want_xyz=False, want_y=False, workspace=None):

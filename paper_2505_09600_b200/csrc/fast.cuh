@@ -47,6 +47,7 @@ __host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(whic
 #define FAST_NA_LFA_GEN 6                 /* those of one generation */
 #define FAST_NA (FAST_NA_FULL + FAST_NA_LFA)
 #define FAST_DMAX 5.0e-7                  /* |eps_n - eps_c| bound for the first-order weights */
+#define FAST_DMAX2 5.0e-5                 /* bound for the second-order weights: the neglected (D^3 / 6)(omega dt)^3 |x| <= 2e-14 |x| */
 /* one anchor = [M] double2 {w_k, w_k'}, in doubles */
 #define FAST_ANC_DOUBLES(M) (2 * (M))
 
@@ -78,7 +79,9 @@ struct FastParams {
     double *A, *E, *T, *XYZ, *Y; /* outputs of this chunk ([batch][ld] ...), XYZ / Y strides use batch_all */
     int64_t batch_all, b0;   /* full batch and first source of the chunk (for the [3][batch][ld] outputs) */
     const double *anc;       /* [anchor tiles][FAST_NA][M][2] */
-    const double *anc_hdr;   /* [anchor tiles][FAST_NA][4]: d_c [s], q, eps_c, valid */
+    const double *anc_hdr;   /* [anchor tiles][FAST_NA][4]: d_c [s], q, eps_c, valid (0 no, 1 first order, 2 second order only) */
+    const double *anc2;      /* [anchor tiles][FAST_NA][M]: w_k'' (second-order instances; nullptr otherwise) */
+    int nested;              /* properly nested TDI delays (full response; second-order instance) */
     int64_t ntilesA, ntilesC;
     /* hybrid: compact work lists built by hybrid_plan_kernel (x = source of the chunk, y = tile); a launch runs exactly
      * the tiles of its class.  work == nullptr: every tile of every source (id = tile * batch + source). */
@@ -676,12 +679,17 @@ struct DelayDef { signed char base, i, j; };   /* base: 0 none, 1 dP, 2 dU */
 __constant__ DelayDef c_delay_def[13] = {
     {1, 0, 0}, {1, 0, 1}, {0, 0, 1}, {2, 0, 0}, {2, 1, 0}, {0, 1, 0}, {1, 1, 1},
     {1, 1, 2}, {0, 1, 1}, {0, 1, 2}, {2, 1, 1}, {2, 2, 1}, {0, 2, 1}};
-/* the 14 interpolated terms of Eq. (2.7) / (2.8): series (0 P, 1 Q, 2 U, 3 W), delay id, sign; the first 6
- * are TDI 1.5 */
-struct TermDef { signed char series, delay, sign; };
+/* The 14 interpolated terms of Eq. (2.7) / (2.8): series (0 P, 1 Q, 2 U, 3 W), delay id, sign, and the link whose light
+ * time the term adds to the delay of the term before it (0: +p3, 1: -p3, 2: -p2, 3: +p2).  They are ordered along the
+ * two chains of delay operators that generate them (oracle O12; a = D_-p2 D_p2, b = D_p3 D_-p3):
+ *   terms 0..6:  D_p3 U, b Q, b D_-p2 P, b a Q, b a D_-p2 P, b a a W, b a a D_p3 U      (all with sign -)
+ *   terms 7..13: D_-p2 P, a W, a D_p3 U, a b W, a b D_p3 U, a b b Q, a b b D_-p2 P      (all with sign +)
+ * so that with nested delays every term extends the delay of its predecessor by one light time.  TDI 1.5 uses the
+ * first three of either chain. */
+struct TermDef { signed char series, delay, sign, link; };
 __constant__ TermDef c_term_def[14] = {
-    {0, 0, +1}, {0, 1, -1}, {1, 2, -1}, {2, 3, -1}, {2, 4, +1}, {3, 5, +1},
-    {0, 6, -1}, {0, 7, +1}, {1, 8, -1}, {1, 9, +1}, {2, 10, +1}, {2, 11, -1}, {3, 8, +1}, {3, 12, -1}};
+    {2, 3, -1, 0}, {1, 2, -1, 1}, {0, 1, -1, 2}, {1, 8, -1, 3}, {0, 6, -1, 2}, {3, 12, -1, 3}, {2, 11, -1, 0},
+    {0, 0, +1, 2}, {3, 5, +1, 3}, {2, 4, +1, 0}, {3, 8, +1, 1}, {2, 10, +1, 0}, {1, 9, +1, 1}, {0, 7, +1, 2}};
 
 __device__ __forceinline__ double tdi_delay(int id, double dP, double dU, double a, double b)
 {
@@ -713,7 +721,7 @@ __device__ __forceinline__ double lfa_delay(int gen, int id, double L2, double L
 // anchor kernel: one block per TDI tile; thread a < FAST_NA builds the anchor of delay a
 // ---------------------------------------------------------------------------------------------
 template <int M>
-__global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ FastParams p, double *anc, double *hdr)
+__global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ FastParams p, double *anc, double *hdr, double *anc2 /* w'' or nullptr */)
 {
     const int64_t tile = blockIdx.x;
     const int64_t n0 = tile * FAST_TCA, n1 = min(n0 + (int64_t)FAST_TCA, p.n);
@@ -764,40 +772,47 @@ __global__ void __launch_bounds__(64) anchor_kernel(const __grid_constant__ Fast
         m2 = gen == LTDI_GEN_15 ? p.m2_15 : p.m2_20;
     }
     bound *= p.inv_dt;
+    /* properly nested delays (oracle O12) differ from the sums of L_l(t_n) by at most sum_j |dL_cj/dt| d, and the rates
+     * are bounded by the deviations over the half tile: an allowance of 2 d / (half tile) on top */
+    bound *= 1.0 + 2.0 * d / (fmax((double)max(nc - n0, n1 - 1 - nc), 1.0) * p.dt);
     int q;
     double eps;
     split_delay_fast(d, p.dt, p.inv_dt, q, eps);
-    /* usable if the Taylor remainder is below rounding, the integer shift cannot change inside the tile and the
-     * stencil stays inside the staged halo */
-    const bool ok = bound <= FAST_DMAX && eps - bound >= 0.0 && eps + bound < 1.0 && q >= 0 &&
+    /* usable if the Taylor remainder is below rounding (first-order weights: FAST_DMAX; with w'' stored: FAST_DMAX2), the
+     * integer shift cannot change inside the tile and the stencil stays inside the staged halo */
+    const bool ok = bound <= (anc2 ? FAST_DMAX2 : FAST_DMAX) && eps - bound >= 0.0 && eps + bound < 1.0 && q >= 0 &&
                     q + M / 2 <= m2;
     double *h = hdr + (tile * FAST_NA + tid) * 4;
-    h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? 1.0 : 0.0;
+    h[0] = d; h[1] = (double)q; h[2] = eps; h[3] = ok ? (bound <= FAST_DMAX ? 1.0 : 2.0) : 0.0;
 
-    /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); the first derivative
-     * by the product rule carried along the same sweeps */
+    /* w_k = c_k pre_k suf_k with pre_k = prod_{m<k}(eps - m), suf_k = prod_{m>k}(eps - m); the first (and second)
+     * derivative by the product rule carried along the same sweeps */
     double2 *out = reinterpret_cast<double2 *>(anc + (tile * FAST_NA + tid) * (int64_t)FAST_ANC_DOUBLES(M));
+    double *out2 = anc2 ? anc2 + (tile * FAST_NA + tid) * (int64_t)M : nullptr;
     const double *c = c_lag_inv_den + (M / 2 - 1) * LTDI_MAX_TAPS;
     constexpr int kmin = -(M / 2 - 1);
-    double pf[M], pf1[M];
+    double pf[M], pf1[M], pf2[M];
     {
-        double f = 1.0, f1 = 0.0;
+        double f = 1.0, f1 = 0.0, f2 = 0.0;
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            pf[i] = f; pf1[i] = f1;
+            pf[i] = f; pf1[i] = f1; pf2[i] = f2;
             const double e = eps - (double)(kmin + i);
+            f2 = f2 * e + 2.0 * f1;
             f1 = f1 * e + f;
             f = f * e;
         }
     }
-    double g = 1.0, g1 = 0.0;
+    double g = 1.0, g1 = 0.0, g2 = 0.0;
 #pragma unroll
     for (int i = M - 1; i >= 0; --i) {
         double2 o;
         o.x = c[i] * (pf[i] * g);
         o.y = c[i] * (pf1[i] * g + pf[i] * g1);
         out[i] = o;
+        if (out2) out2[i] = c[i] * (pf2[i] * g + 2.0 * pf1[i] * g1 + pf[i] * g2);
         const double e = eps - (double)(kmin + i);
+        g2 = g2 * e + 2.0 * g1;
         g1 = g1 * e + g;
         g = g * e;
     }
@@ -852,9 +867,22 @@ __device__ __forceinline__ void hybrid_weights_fast(const double *h, double t, d
 //   sum_k w_k(eps_c + D) x_k = S0 + D S1,   S_m = sum_k w_k^(m)(eps_c) x_k :
 // two constant-coefficient FIR filters over the tile, 2 DFMA per tap and sample in FAST_TC_R x 2 independent
 // chains; the weights are broadcast reads, the samples slide through a register window.
-template <int M>
-__device__ __forceinline__ void term7(const double *__restrict__ anc, const double *__restrict__ x,
-                                      double (&s0)[FAST_TC_R], double (&s1)[FAST_TC_R])
+// ORD2 (orbits whose light times drift by more than FAST_DMAX over a tile: numerical orbit files, caller's tables):
+// every thread first moves the weights to the delay of ITS OWN centre sample with the second-order Taylor step
+//   w_k(eps_c + Dt) = w_k + Dt (w_k' + Dt w_k'' / 2),   w_k'(eps_c + Dt) = w_k' + Dt w_k''
+// (3 DFMA per tap and thread) and the caller applies the first-order step for the remaining eps_n - eps_c - Dt of its
+// seven samples (three samples of drift: < 1e-7); neglected: Dt^3 / 6 times the third derivative of the weights and
+// (eps_n - eps_c - Dt)^2 / 2 times the second.
+/* (tile, channel) pairs that took the exact per-sample weights instead of the anchors (ltdi_profile_slow_tiles) */
+__device__ unsigned long long d_slow_tiles;
+
+/* header code of an anchor: 1 = first-order weights suffice, 2 = second-order weights needed, 0 = neither */
+template <bool ORD2>
+__device__ __forceinline__ bool anchor_ok(double code) { return ORD2 ? code != 0.0 : code == 1.0; }
+
+template <int M, bool ORD2>
+__device__ __forceinline__ void term7(const double *__restrict__ anc, const double *__restrict__ anc2, double Dt,
+                                      const double *__restrict__ x, double (&s0)[FAST_TC_R], double (&s1)[FAST_TC_R])
 {
     const double2 *w01 = reinterpret_cast<const double2 *>(anc);
     double win[FAST_TC_R];
@@ -862,9 +890,15 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
     for (int r = 0; r < FAST_TC_R; ++r) { s0[r] = 0.0; s1[r] = 0.0; }
 #pragma unroll
     for (int r = 0; r < FAST_TC_R - 1; ++r) win[r] = x[r];
+    const double hDt = 0.5 * Dt;
 #pragma unroll
     for (int k = 0; k < M; ++k) {
-        const double2 w = w01[k];
+        double2 w = w01[k];
+        if (ORD2) {
+            const double w2 = anc2[k];
+            w.x = fma(Dt, fma(hDt, w2, w.y), w.x);
+            w.y = fma(Dt, w2, w.y);
+        }
         win[(k + FAST_TC_R - 1) % FAST_TC_R] = x[k + FAST_TC_R - 1];
 #pragma unroll
         for (int r = 0; r < FAST_TC_R; ++r) {
@@ -875,12 +909,29 @@ __device__ __forceinline__ void term7(const double *__restrict__ anc, const doub
     }
 }
 
-// WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch
-template <int M, int WHICH>
+// Light travel time of a staged row (element 0 = sample y0 of the tile window) at t_i - d: centred Lagrange
+// interpolation of order 3 (reading G29, oracle O12): taps k = -1 .. 2 about sample i - ceil(d / dt)
+__device__ __forceinline__ double light_time_at(const double *__restrict__ Lrow, int i, double d, double dt, double inv_dt)
+{
+    int q;
+    double e;
+    split_delay_fast(d, dt, inv_dt, q, e);
+    q = max(0, min(q, i - 1));   /* samples past the end of the series carry no light times: stay inside the row */
+    const double *x = Lrow + (i - q);
+    const double em1 = e - 1.0, em2 = e - 2.0, ep1 = e + 1.0;
+    const double wm = -(e * em1) * em2 * (1.0 / 6.0), w0 = (ep1 * em1) * em2 * 0.5, w1 = -(ep1 * e) * em2 * 0.5,
+                 w2 = (ep1 * e) * em1 * (1.0 / 6.0);
+    return fma(wm, x[-1], fma(w0, x[0], fma(w1, x[1], w2 * x[2])));
+}
+
+// WHICH = LTDI_RESPONSE_*: the full-only and LFA-only instances carry no code or registers of the other branch.
+// ORD2: second-order weights (see term7) and, for the full response, optionally nested delays (p.nested).
 #ifndef TDI_LFA_MINB
 #define TDI_LFA_MINB 4
 #endif
-__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : (WHICH == LTDI_RESPONSE_LFA ? TDI_LFA_MINB : 4)) tdi_kernel(const __grid_constant__ FastParams p)
+template <int M, int WHICH, bool ORD2>
+__global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYBRID ? 2 : (WHICH == LTDI_RESPONSE_LFA ? TDI_LFA_MINB : (ORD2 ? 3 : 4)))
+tdi_kernel(const __grid_constant__ FastParams p)
 {
     extern __shared__ double smem[];
     constexpr int FAST_TC = tdi_tc(WHICH), FAST_TC_G = tdi_g(WHICH), FAST_TC_THREADS = tdi_threads(WHICH);
@@ -910,21 +961,28 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
      *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
      *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0, even)
      *   Lr   [NLR][FAST_TC] light times L_l(n0 + i) of the tile; after the term loop: X, Y, Z of the tile
-     *   yL   [3][yr + 4] LFA links        (element 0 = sample y0 - 2) */
+     *        (full response with second-order weights: [6][yr], element 0 = sample y0 -- nested delays look back)
+     *   yL   [3][yr + 4] LFA links        (element 0 = sample y0 - 2)
+     *   Xs   [3][FAST_TC] exchange        sa2  [na][M] second derivative of the weights (ORD2) */
     const int yr = tdi_yr<M>(FAST_TC, p.m2);
     const int64_t y0 = n0 - tdi_back(p.m2);
     constexpr int na_full = has_full ? FAST_NA_FULL : 0;
     double *sa = smem;
     double *yF = sa + (size_t)(na_full + (has_lfa ? FAST_NA_LFA_GEN : 0)) * ANC;
     double *dL = yF + (has_full ? 6 * yr : 0);
+    constexpr bool LR_EXT = ORD2 && WHICH == LTDI_RESPONSE_FULL;
+    const int LRW = LR_EXT ? yr : FAST_TC;                       /* elements per light-time row */
+    const int lroff = LR_EXT ? tdi_back(p.m2) : 0;               /* element of sample n0 */
     double *Lr = dL + (has_lfa ? 3 * yr : 0);
-    double *yL = Lr + NLR * FAST_TC;
+    double *yL = Lr + NLR * LRW;
     const int slen = yr + 4;   /* staged LFA links: samples [y0 - 2, y0 + yr + 2), an even start for 16-byte rows */
     /* X, Y, Z exchange: its own region (full, LFA: no barrier between the term loop and the exchange), or on top of
      * the light times (hybrid: six rows, and the shared memory of two responses) */
     constexpr bool xs_alias = WHICH == LTDI_RESPONSE_HYBRID;
     double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * slen : 0);
+    double *sa2 = yL + (has_lfa ? 3 * slen : 0) + (xs_alias ? 0 : 3 * FAST_TC);   /* behind everything else */
     const double *sa_lfa = sa + (size_t)na_full * ANC;
+    const double *sa2_lfa = sa2 + (size_t)na_full * M;
     const int lfa_a0 = p.gen == LTDI_GEN_15 ? 0 : FAST_NA_LFA_GEN;   /* first LFA anchor of this generation */
     const double *tabL = p.tab + (int64_t)ROW_L * p.stride;
     __shared__ __align__(16) double s_hdr[FAST_NA * 4];
@@ -940,7 +998,14 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     const int64_t g0 = max(y0, (int64_t)0), g1 = min(y0 + yr, p.lds);                  /* full links, even bounds */
     const int64_t h0 = max(y0 - 2, (int64_t)0), h1 = min(y0 - 2 + slen, p.lds);         /* LFA links */
     const int nyF = (int)max(g1 - g0, (int64_t)0), nyL = (int)max(h1 - h0, (int64_t)0);
-    const int nl = (int)max(min((int64_t)FAST_TC, p.stride - n0), (int64_t)0);
+    const int64_t lr0 = n0 - lroff;                                                      /* first sample of a light-time row */
+    const int64_t l0 = max(lr0, (int64_t)0), l1 = min(lr0 + LRW, p.stride);
+    const int nl = (int)max(l1 - l0, (int64_t)0);
+    if (LR_EXT && (lr0 < 0 || nl < LRW))
+        for (int k = tid; k < 6 * LRW; k += FAST_TC_THREADS) {
+            const int c = k % LRW;
+            if (c < l0 - lr0 || c >= l0 - lr0 + nl) Lr[k] = 0.0;
+        }
     if (has_full && (y0 < 0 || nyF < yr))
         for (int k = tid; k < 6 * yr; k += FAST_TC_THREADS) {
             const int c = k % yr;
@@ -956,11 +1021,15 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
         const int64_t ystride = p.batch * p.lds;
         const int64_t atile = tile / FAST_TCA_TILES;
         const double *ga = p.anc + atile * (int64_t)(FAST_NA * ANC);
-        mbar_expect_tx(&s_bar, (unsigned)(((has_full ? 6 * nyF + FAST_NA_FULL * ANC : 0) + (has_lfa ? 3 * nyL + FAST_NA_LFA_GEN * ANC : 0) +
+        const double *ga2 = ORD2 ? p.anc2 + atile * (int64_t)(FAST_NA * M) : nullptr;
+        mbar_expect_tx(&s_bar, (unsigned)(((has_full ? 6 * nyF + FAST_NA_FULL * (ANC + (ORD2 ? M : 0)) : 0) +
+                                           (has_lfa ? 3 * nyL + FAST_NA_LFA_GEN * (ANC + (ORD2 ? M : 0)) : 0) +
                                            NLR * nl + FAST_NA * 4) * sizeof(double)));
 #pragma unroll 1
         for (int l = 0; l < NLR; ++l)
-            if (nl > 0) bulk_g2s(Lr + l * FAST_TC, tabL + l * p.stride + n0, nl * 8u, &s_bar);
+            if (nl > 0) bulk_g2s(Lr + l * LRW + (l0 - lr0), tabL + l * p.stride + l0, nl * 8u, &s_bar);
+        if (ORD2 && has_full) bulk_g2s(sa2, ga2, FAST_NA_FULL * M * 8u, &s_bar);
+        if (ORD2 && has_lfa) bulk_g2s(sa2 + (size_t)na_full * M, ga2 + (FAST_NA_FULL + lfa_a0) * M, FAST_NA_LFA_GEN * M * 8u, &s_bar);
         if (has_full) {
 #pragma unroll 1
             for (int l = 0; l < 6; ++l)
@@ -1040,11 +1109,12 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
     bool ok = true;
     if (has_full && need_full) {
         const int nd = p.gen == LTDI_GEN_20 ? 13 : 6;
-        for (int id = 0; id < nd; ++id) ok = ok && s_hdr[4 * (13 * ch + id) + 3] != 0.0;
+        for (int id = 0; id < nd; ++id) ok = ok && anchor_ok<ORD2>(s_hdr[4 * (13 * ch + id) + 3]);
     }
     if (has_lfa && need_lfa)
-        ok = ok && s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch) + 3] != 0.0 &&
-             s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch + 1) + 3] != 0.0;
+        ok = ok && anchor_ok<ORD2>(s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch) + 3]) &&
+             anchor_ok<ORD2>(s_hdr[4 * (FAST_NA_FULL + lfa_a0 + 2 * ch + 1) + 3]);
+    const bool nested = LR_EXT && p.nested;
 
     if (ok) {
         /* one loop over the interpolated terms of this channel: 6 / 14 of Eq. (2.7) / (2.8) on the full links, then
@@ -1052,16 +1122,20 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
          * coefficients of the delay d_n = cP L_-p2 + c2 L_p2 + cU L_p3 + c3 L_-p3 in the light times of the channel's
          * links (a = L_-p2 + L_p2, b = L_p3 + L_-p3, dP = L_-p2, dU = L_p3; LFA: L_p2 and L_p3 only);
          * D = eps_n - eps_c = (d_c - d_n) / dt */
-        const double *LP = Lr + (has_full ? (i2 + 3) * FAST_TC : 0) + r0, *L2p = Lr + i2 * FAST_TC + r0;
-        const double *LU = Lr + i3 * FAST_TC + r0, *L3m = Lr + (has_full ? (i3 + 3) * FAST_TC : 0) + r0;
-        const int nfull = (has_full && need_full) ? (p.gen == LTDI_GEN_20 ? 14 : 6) : 0;
+        const double *LP = Lr + (has_full ? (i2 + 3) * LRW : 0) + lroff + r0, *L2p = Lr + i2 * LRW + lroff + r0;
+        const double *LU = Lr + i3 * LRW + lroff + r0, *L3m = Lr + (has_full ? (i3 + 3) * LRW : 0) + lroff + r0;
+        const bool g20 = p.gen == LTDI_GEN_20;
+        const int tm_first = (has_full && need_full) ? 0 : 14;
         const int i0 = (int)(nf - y0);
         const double lfa_hi = p.gen == LTDI_GEN_15 ? 1.0 : 2.0, lfa_lo = p.gen == LTDI_GEN_15 ? 0.5 : 1.5;
+        double dn[FAST_TC_R];   /* nested delays: the chain so far (oracle O12) */
 #pragma unroll 1
-        for (int tm = nfull ? 0 : 14; tm < ((has_lfa && need_lfa) ? 16 : nfull); tm = (tm + 1 == nfull ? 14 : tm + 1)) {
+        for (int tm = tm_first; tm < ((has_lfa && need_lfa) ? 16 : 14); ++tm) {
             const bool lt = has_lfa && (!has_full || tm >= 14);
-            const double *anc_t, *xs;
+            if (!lt && !g20 && (tm % 7) >= 3) continue;    /* TDI 1.5: the first three terms of either chain */
+            const double *anc_t, *anc2_t = nullptr, *xs;
             double cP, c2, cU, c3, dc, sgn = 0.0;
+            const double *Lk = nullptr;                     /* nested: the row of the link this term adds to the chain */
             if (!lt) {
                 const TermDef td = c_term_def[tm];
                 const DelayDef df = c_delay_def[td.delay];
@@ -1070,6 +1144,8 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
                 dc = hd[0];
                 xs = yF + series * yr + i0 - (int)hd[1] - (H - 1);
                 anc_t = sa + (13 * ch + td.delay) * ANC;
+                if (ORD2) anc2_t = sa2 + (13 * ch + td.delay) * M;
+                if (LR_EXT) Lk = Lr + (td.link == 0 ? i3 : td.link == 1 ? i3 + 3 : td.link == 2 ? i2 + 3 : i2) * LRW;
                 cP = (double)((df.base == 1) + df.i); c2 = (double)df.i;
                 cU = (double)((df.base == 2) + df.j); c3 = (double)df.j;
                 sgn = (double)td.sign;
@@ -1079,16 +1155,36 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
                 dc = hd[0];
                 xs = dL + (id == 0 ? i2 : i3) * yr + i0 - (int)hd[1] - (H - 1);
                 anc_t = sa_lfa + (2 * ch + id) * ANC;
+                if (ORD2) anc2_t = sa2_lfa + (2 * ch + id) * M;
                 cP = 0.0; c3 = 0.0;
                 c2 = id == 0 ? lfa_lo : lfa_hi;
                 cU = id == 0 ? lfa_hi : lfa_lo;
             }
+            double D[FAST_TC_R], Dt = 0.0;   /* second order: D = eps_n - eps_c before the filters, Dt = the thread's own expansion point */
+            if (ORD2) {
+                if (LR_EXT && nested && !lt) {
+                    /* d_j = d_{j-1} + L_cj(t - d_{j-1}); a chain starts at terms 0 and 7 */
+                    const bool first = tm == 0 || tm == 7;
+#pragma unroll
+                    for (int r = 0; r < FAST_TC_R; ++r) {
+                        const double prev = first ? 0.0 : dn[r];
+                        dn[r] = prev + light_time_at(Lk, lroff + r0 + r, prev, p.dt, p.inv_dt);
+                        D[r] = (dc - dn[r]) * p.inv_dt;
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < FAST_TC_R; ++r)
+                        D[r] = fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
+                }
+                Dt = D[FAST_TC_R / 2];
+            }
             double s0[FAST_TC_R], s1[FAST_TC_R];
-            term7<M>(anc_t, xs, s0, s1);
+            term7<M, ORD2>(anc_t, anc2_t, Dt, xs, s0, s1);
 #pragma unroll
             for (int r = 0; r < FAST_TC_R; ++r) {
-                const double D = fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
-                const double v = fma(D, s1[r], s0[r]);
+                const double Dr = ORD2 ? D[r] - Dt
+                                       : fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
+                const double v = fma(Dr, s1[r], s0[r]);
                 if (!lt) Xf[r] = fma(sgn, v, Xf[r]);
                 else {
                     const double L2 = L2p[r], L3 = LU[r];
@@ -1104,6 +1200,7 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
         }
     } else {
         /* exact per-sample weights */
+        if (g == 0) atomicAdd(&d_slow_tiles, 1ULL);
         for (int r = 0; r < FAST_TC_R; ++r) {
             const int64_t n = nf + r;
             if (n >= n1) break;
@@ -1113,12 +1210,19 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
             if (has_full && need_full) {
                 const double *ser[4] = {yF + i2 * yr, yF + (i2 + 3) * yr, yF + (i3 + 3) * yr, yF + i3 * yr};
                 const double dP = L[i2 + 3], dU = L[i3], a = L[i2 + 3] + L[i2], bb = L[i3] + L[i3 + 3];
-                const int nterm = p.gen == LTDI_GEN_20 ? 14 : 6;
                 double x = ser[1][idx] - ser[3][idx];
-                for (int tm = 0; tm < nterm; ++tm) {
+                double chain = 0.0;
+                for (int tm = 0; tm < 14; ++tm) {
+                    if (p.gen != LTDI_GEN_20 && (tm % 7) >= 3) continue;
                     const TermDef td = c_term_def[tm];
-                    x += (double)td.sign *
-                         slow_delayed<M>(ser[td.series], yr, idx, tdi_delay(td.delay, dP, dU, a, bb), p.dt, p.inv_dt);
+                    double delay = tdi_delay(td.delay, dP, dU, a, bb);
+                    if (LR_EXT && nested) {
+                        const double *Lk = Lr + (td.link == 0 ? i3 : td.link == 1 ? i3 + 3 : td.link == 2 ? i2 + 3 : i2) * LRW;
+                        const double prev = (tm == 0 || tm == 7) ? 0.0 : chain;
+                        chain = prev + light_time_at(Lk, idx, prev, p.dt, p.inv_dt);
+                        delay = chain;
+                    }
+                    x += (double)td.sign * slow_delayed<M>(ser[td.series], yr, idx, delay, p.dt, p.inv_dt);
                 }
                 Xf[r] = x;
             }
@@ -1206,14 +1310,16 @@ __global__ void __launch_bounds__(tdi_threads(WHICH), WHICH == LTDI_RESPONSE_HYB
 
 /* dynamic shared memory of tdi_kernel<M> in bytes (mirrors the carve-up above) */
 template <int M>
-static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w)
+static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w, bool ord2)
 {
     const bool has_full = which != LTDI_RESPONSE_LFA, has_lfa = which != LTDI_RESPONSE_FULL;
     const size_t yr = (size_t)tdi_yr<M>(tdi_tc(which), m2);
-    size_t dbl = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0)) * FAST_ANC_DOUBLES(M);
+    const size_t na = (size_t)((has_full ? FAST_NA_FULL : 0) + (has_lfa ? FAST_NA_LFA : 0));
+    size_t dbl = na * FAST_ANC_DOUBLES(M);
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
-    dbl += (size_t)(has_full ? 6 : 3) * tdi_tc(which);
+    dbl += (size_t)(has_full ? 6 : 3) * ((ord2 && which == LTDI_RESPONSE_FULL) ? yr : (size_t)tdi_tc(which));
     dbl += has_lfa ? 3 * (yr + 4) : 0;
     dbl += which == LTDI_RESPONSE_HYBRID ? 0 : (size_t)3 * tdi_tc(which);   /* X, Y, Z exchange */
+    dbl += ord2 ? na * M : 0;                                                /* second derivative of the weights */
     return dbl * sizeof(double);
 }

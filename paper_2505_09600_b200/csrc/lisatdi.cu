@@ -261,7 +261,7 @@ bool fast_order(int order) { return order == 9 || order == 31; }
  * speed of these FP64-bound kernels. */
 struct FastLayout {
     int64_t ntilesA, ntilesC, ntilesN, lds, chunk;   /* link tiles, TDI tiles, anchor tiles (= 448-sample blocks) */
-    size_t anc, hdr, y, lists;     /* doubles */
+    size_t anc, hdr, anc2, y, lists;     /* doubles */
     size_t total;                  /* doubles, including work_doubles(batch) */
 };
 FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
@@ -277,10 +277,11 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
     f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
     f.anc = (size_t)f.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
     f.hdr = (size_t)f.ntilesN * FAST_NA * 4;
+    f.anc2 = (size_t)f.ntilesN * FAST_NA * M;   /* second derivative of the weights (second-order instances) */
     f.y = (size_t)rows * f.chunk * f.lds;
     /* hybrid: link tiles of both kinds, LFA-only blocks, blend blocks, full-only 224-sample tiles (int2 each) */
     f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)f.chunk * (2 * f.ntilesA + 4 * f.ntilesN) : 0;
-    f.total = work_doubles(batch) + f.anc + f.hdr + f.y + f.lists;
+    f.total = work_doubles(batch) + f.anc + f.hdr + f.anc2 + f.y + f.lists;
     return f;
 }
 
@@ -465,6 +466,19 @@ int build_hybrid_plan(const ltdi_orbit_desc &d, const Margins &mg, int M, const 
     return LTDI_OK;
 }
 
+/* the first-order (analytic orbits) or second-order (tables, numerical orbits, nested delays) instance of the TDI kernel */
+template <int M, int WHICH>
+void launch_tdi(bool ord2, unsigned grid, size_t smem, cudaStream_t st, const FastParams &p)
+{
+    if (ord2) tdi_kernel<M, WHICH, true><<<grid, tdi_threads(WHICH), smem, st>>>(p);
+    else tdi_kernel<M, WHICH, false><<<grid, tdi_threads(WHICH), smem, st>>>(p);
+}
+template <int M, int WHICH>
+int set_smem_tdi(DeviceState &ds, bool ord2, size_t smem)
+{
+    return ord2 ? set_smem(ds, tdi_kernel<M, WHICH, true>, smem) : set_smem(ds, tdi_kernel<M, WHICH, false>, smem);
+}
+
 // the tuned path: anchors once per call, then link kernel(s) and TDI kernel(s) per chunk of sources
 template <int M>
 int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltdi_orbits *orb, int which, double *work,
@@ -490,9 +504,13 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
     p.use_small = small != nullptr;
     if (small) std::memcpy(p.small, small, sizeof p.small);
-    double *anc = work, *hdr = anc + lay.anc, *ys = hdr + lay.hdr;
+    double *anc = work, *hdr = anc + lay.anc, *anc2 = hdr + lay.hdr, *ys = anc2 + lay.anc2;
     int2 *lists = reinterpret_cast<int2 *>(ys + lay.y);
     p.anc = anc; p.anc_hdr = hdr;
+    /* second-order weights where the light times of the orbit object may drift by more than FAST_DMAX over a tile
+     * (caller's tables, numerical orbit files) and for nested delays; the analytic orbits keep the first-order instances */
+    const bool ord2 = d.mode == LTDI_ORBIT_TABLES || d.mode == LTDI_ORBIT_KNOTS || rp.nested;
+    p.anc2 = ord2 ? anc2 : nullptr; p.nested = rp.nested;
 
     const bool full = which != LTDI_RESPONSE_LFA, lfa = which != LTDI_RESPONSE_FULL;
     const bool hybrid = which == LTDI_RESPONSE_HYBRID;
@@ -504,27 +522,28 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
                                  (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float) +                           /* + low parts */
                                  (rp.lfa_terms >= 2 ? smem_strain : 0);                                     /* + d^3h/dt^3 numerators */
     const size_t smem_link_hyb = std::max(smem_link, smem_link_lfa);
-    const size_t smem_tdi_full = tdi_smem_bytes<M>(LTDI_RESPONSE_FULL, mg.m2, mg.w);
-    const size_t smem_tdi_hyb = tdi_smem_bytes<M>(LTDI_RESPONSE_HYBRID, mg.m2, mg.w);
-    const size_t smem_tdi_lfa = tdi_smem_bytes<M>(LTDI_RESPONSE_LFA, mg.m2, mg.w);
+    const size_t smem_tdi_full = tdi_smem_bytes<M>(LTDI_RESPONSE_FULL, mg.m2, mg.w, ord2);
+    const size_t smem_tdi_hyb = tdi_smem_bytes<M>(LTDI_RESPONSE_HYBRID, mg.m2, mg.w, ord2);
+    const size_t smem_tdi_lfa = tdi_smem_bytes<M>(LTDI_RESPONSE_LFA, mg.m2, mg.w, ord2);
     int rc;
     if (hybrid) {
         if ((rc = set_smem(ds, link_hybrid_kernel<H>, smem_link_hyb))) return rc;
-        if ((rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_HYBRID>, smem_tdi_hyb))) return rc;
+        if ((rc = set_smem_tdi<M, LTDI_RESPONSE_HYBRID>(ds, ord2, smem_tdi_hyb))) return rc;
     } else {
         if (full && (rc = set_smem(ds, link_kernel<H, false>, smem_link))) return rc;
         if (lfa && (rc = set_smem(ds, link_kernel<H, true>, smem_link_lfa))) return rc;
     }
-    if (full && (rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_FULL>, smem_tdi_full))) return rc;
-    if (lfa && (rc = set_smem(ds, tdi_kernel<M, LTDI_RESPONSE_LFA>, smem_tdi_lfa))) return rc;
+    if (full && (rc = set_smem_tdi<M, LTDI_RESPONSE_FULL>(ds, ord2, smem_tdi_full))) return rc;
+    if (lfa && (rc = set_smem_tdi<M, LTDI_RESPONSE_LFA>(ds, ord2, smem_tdi_lfa))) return rc;
 
     if (orb->d_anc && orb->anc_M == M) {
         /* ltdi_orbits_prepare() has computed the anchors of this order for the time grid (they serve both generations) */
         p.anc = orb->d_anc;
-        p.anc_hdr = orb->d_anc + (size_t)lay.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
+        p.anc_hdr = orb->d_anc + lay.anc;
+        p.anc2 = ord2 ? orb->d_anc + lay.anc + lay.hdr : nullptr;
     } else {
         ProfScope ps(LTDI_KERNEL_ANCHOR + LTDI_KERNEL_COUNT * which, st);
-        anchor_kernel<M><<<(unsigned)lay.ntilesN, 64, 0, st>>>(p, anc, hdr);
+        anchor_kernel<M><<<(unsigned)lay.ntilesN, 64, 0, st>>>(p, anc, hdr, ord2 ? anc2 : nullptr);
         count_launch();
         LTDI_CUDA_OK(cudaGetLastError());
     }
@@ -553,8 +572,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
                 }
                 count_launch();
                 ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
-                tdi_kernel<M, LTDI_RESPONSE_FULL><<<(unsigned)(lay.ntilesC * nb), tdi_threads(LTDI_RESPONSE_FULL),
-                                                    smem_tdi_full, st>>>(p);
+                launch_tdi<M, LTDI_RESPONSE_FULL>(ord2, (unsigned)(lay.ntilesC * nb), smem_tdi_full, st, p);
             } else {
                 {
                     ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
@@ -563,7 +581,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
                 count_launch();
                 p.nwork = lay.ntilesN * nb;
                 ProfScope ps(LTDI_KERNEL_TDI_LFA + LTDI_KERNEL_COUNT * which, st);
-                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)p.nwork, tdi_threads(LTDI_RESPONSE_LFA), smem_tdi_lfa, st>>>(p);
+                launch_tdi<M, LTDI_RESPONSE_LFA>(ord2, (unsigned)p.nwork, smem_tdi_lfa, st, p);
             }
             count_launch();
             LTDI_CUDA_OK(cudaGetLastError());
@@ -606,7 +624,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
             p.work = l_lfa; p.nwork = ct.lfa; p.nwork_full = 0;
             {
                 ProfScope ps(LTDI_KERNEL_TDI_LFA + LTDI_KERNEL_COUNT * which, s_lfa);
-                tdi_kernel<M, LTDI_RESPONSE_LFA><<<(unsigned)p.nwork, tdi_threads(LTDI_RESPONSE_LFA), smem_tdi_lfa, s_lfa>>>(p);
+                launch_tdi<M, LTDI_RESPONSE_LFA>(ord2, (unsigned)p.nwork, smem_tdi_lfa, s_lfa, p);
             }
             count_launch();
             if (side_lfa) LTDI_CUDA_OK(cudaEventRecord(ds.ev_join, ds.side));
@@ -615,12 +633,12 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
             ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
             if (ct.full > 0) {
                 p.work = l_full; p.nwork = ct.full;
-                tdi_kernel<M, LTDI_RESPONSE_FULL><<<(unsigned)ct.full, tdi_threads(LTDI_RESPONSE_FULL), smem_tdi_full, st>>>(p);
+                launch_tdi<M, LTDI_RESPONSE_FULL>(ord2, (unsigned)ct.full, smem_tdi_full, st, p);
                 count_launch();
             }
             if (ct.blend > 0) {
                 p.work = l_blend; p.nwork = ct.blend;
-                tdi_kernel<M, LTDI_RESPONSE_HYBRID><<<(unsigned)ct.blend, tdi_threads(LTDI_RESPONSE_HYBRID), smem_tdi_hyb, st>>>(p);
+                launch_tdi<M, LTDI_RESPONSE_HYBRID>(ord2, (unsigned)ct.blend, smem_tdi_hyb, st, p);
                 count_launch();
             }
         }
@@ -634,8 +652,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
                  double *d_y, void *d_work, size_t work_bytes, void *stream, int lfa_terms = 1,
-                 int lfa_point = LTDI_LFA_CENTRAL)
+                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0)
 {
+    if (nested_order != 0 && (which != LTDI_RESPONSE_FULL || nested_order != 3)) return nested_order == 3 || nested_order < 0 || !(nested_order & 1) ? LTDI_EINVAL : LTDI_EUNSUPPORTED;
+    if (nested_order && !fast_order(order)) return LTDI_EUNSUPPORTED;   /* nested delays run on the tuned path (orders 9, 31) */
     if (lfa_terms < 1 || lfa_terms > 2 || lfa_point < LTDI_LFA_CENTRAL || lfa_point > LTDI_LFA_FORWARD) return LTDI_EINVAL;
     if (lfa_terms == 2 && lfa_point != LTDI_LFA_CENTRAL) return LTDI_EINVAL;
     if ((lfa_terms != 1 || lfa_point != LTDI_LFA_CENTRAL) && which != LTDI_RESPONSE_LFA) return LTDI_EINVAL;
@@ -736,7 +756,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.which = which; p.gen = gen; p.M = M; p.fd = fd_order;
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi;
     p.qmax = (int)(mg.m1 - M / 2);
-    p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw;
+    p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw; p.nested = nested_order != 0;
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
     if (fast_order(order)) {
@@ -745,7 +765,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         double *fw = (double *)d_work + work_doubles(batch);
         const int frc = M == 32 ? run_fast<32>(ds, p, mg, orb, which, fw, st, sm, &hh, dp)
                                 : run_fast<10>(ds, p, mg, orb, which, fw, st, sm, &hh, dp);
-        if (frc != LTDI_EUNSUPPORTED) return frc;   /* else: shapes the tuned kernels do not cover */
+        if (frc != LTDI_EUNSUPPORTED || nested_order) return frc;   /* else: shapes the tuned kernels do not cover */
     }
     if (have_small) { /* the generic kernel reads frames and windows from the workspace */
         {
@@ -900,7 +920,7 @@ int ltdi_orbits_prepare_bytes(const ltdi_orbit_desc *desc, int lagrange_order, s
     if (!desc_ok(desc) || !order_ok(lagrange_order) || !bytes) return LTDI_EINVAL;
     if (!fast_order(lagrange_order)) { *bytes = 0; return LTDI_OK; }
     const int64_t tiles = (desc->n + FAST_TCA - 1) / FAST_TCA;
-    *bytes = ((size_t)tiles * FAST_NA * (FAST_ANC_DOUBLES(lagrange_order + 1) + 4) * sizeof(double) + 255) / 256 * 256;
+    *bytes = ((size_t)tiles * FAST_NA * (FAST_ANC_DOUBLES(lagrange_order + 1) + 4 + (lagrange_order + 1)) * sizeof(double) + 255) / 256 * 256;
     return LTDI_OK;
 }
 
@@ -925,10 +945,11 @@ int ltdi_orbits_prepare(ltdi_orbits *orb, int gen, int lagrange_order, void *d_b
     p.gen = gen; p.m1 = m20.m1; p.m2 = m20.m2; p.m2_15 = m15.m2; p.m2_20 = m20.m2;
     const int64_t tiles = (d.n + FAST_TCA - 1) / FAST_TCA;
     double *anc = (double *)d_buf, *hdr = anc + (size_t)tiles * FAST_NA * FAST_ANC_DOUBLES(M);
+    double *anc2 = hdr + (size_t)tiles * FAST_NA * 4;   /* w'': the prepared anchors serve the second-order instances too */
     {
         ProfScope ps(LTDI_KERNEL_ANCHOR, (cudaStream_t)stream);
-        if (M == 32) anchor_kernel<32><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr);
-        else anchor_kernel<10><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr);
+        if (M == 32) anchor_kernel<32><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr, anc2);
+        else anchor_kernel<10><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr, anc2);
     }
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
@@ -989,6 +1010,16 @@ int ltdi_response_full(const ltdi_orbits *orb, const double *d_hp, const double 
 {
     return run_response(LTDI_RESPONSE_FULL, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0,
                         d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream);
+}
+
+int ltdi_response_full_nested(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                              const ltdi_source *h_src, int gen, int lagrange_order, int nested_order, double *d_A,
+                              double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes,
+                              void *stream)
+{
+    if (nested_order == 0) return LTDI_EINVAL;
+    return run_response(LTDI_RESPONSE_FULL, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0,
+                        d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, nested_order);
 }
 
 int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
@@ -1065,6 +1096,18 @@ int ltdi_profile_reset(void)
     std::lock_guard<std::mutex> lk(g_prof_mu);
     for (int i = 0; i < 3 * LTDI_KERNEL_COUNT; ++i) { g_prof_ms[i] = 0.0; g_prof_n[i] = 0; }
     return rc;
+}
+int ltdi_profile_slow_tiles(int64_t *count, int reset)
+{
+    if (!count) return LTDI_EINVAL;
+    unsigned long long v = 0;
+    LTDI_CUDA_OK(cudaMemcpyFromSymbol(&v, d_slow_tiles, sizeof v));
+    *count = (int64_t)v;
+    if (reset) {
+        v = 0;
+        LTDI_CUDA_OK(cudaMemcpyToSymbol(d_slow_tiles, &v, sizeof v));
+    }
+    return LTDI_OK;
 }
 const char *ltdi_version(void) { return "lisatdi-b200 0.1 (sm_100a, fp64)"; }
 

@@ -83,3 +83,42 @@ def test_batch_on_a_numerical_orbit_order9(ltdi, orc80):
     orbit = W.numerical_orbit(cfg["n"], cfg["dt"], t0=4.0e6, knot_order=5)
     out, ref, lo, hi = run_numeric(ltdi, orc80, cfg, orbit, "hybrid", 20)
     strict_check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("gen,numeric", [(20, False), (15, False), (20, True), (15, True)])
+def test_nested_delays(ltdi, orc80, gen, numeric):
+    """properly nested TDI delays (O12) on the analytic orbit and on the breathing arms of the orbit file, where nesting
+    moves the delays by 7 L dL/dt ~ 1e-6 s (1e-8 of X at 10 mHz: a thousand times the parity bar)"""
+    cfg = W.config(2, n=30011)
+    orbit = W.numerical_orbit(cfg["n"], cfg["dt"], t0=cfg["orbit"]["t0"]) if numeric else cfg["orbit"]
+    out, ref, lo, hi = run_numeric(ltdi, orc80, cfg, orbit, "full", gen, nested=3)
+    strict_check(out, ref, lo, hi, cfg["n"])
+    if numeric and gen == 20:   # and nesting is visible at this bar: the un-nested response differs
+        plain = orc80.response_full(orbit, *W.sources(cfg, [0])[:3], gen, cfg["order"])
+        d = np.linalg.norm((plain["A"] - ref["A"])[..., lo:cfg["n"] - hi]) / np.linalg.norm(ref["A"][..., lo:cfg["n"] - hi])
+        assert d > 1e-10, d
+
+
+def test_nested_batch_order9_and_static(ltdi, orc80):
+    cfg = W.config(4, n=9001, batch=3)
+    cfg["order"] = 9
+    orbit = W.numerical_orbit(cfg["n"], cfg["dt"], t0=6.0e6, knot_order=5)
+    out, ref, lo, hi = run_numeric(ltdi, orc80, cfg, orbit, "full", 20, nested=3)
+    strict_check(out, ref, lo, hi, cfg["n"])
+    # constant equal arms: nesting changes nothing
+    cfg1 = W.config(1)
+    a, ref1, lo, hi = run_numeric(ltdi, orc80, cfg1, cfg1["orbit"], "full", 15, nested=3)
+    b, _, _, _ = run_numeric(ltdi, orc80, cfg1, cfg1["orbit"], "full", 15)
+    strict_check(a, ref1, lo, hi, cfg1["n"])
+    assert np.abs(a["A"] - b["A"]).max() <= 1e-13 * np.abs(b["A"]).max()
+
+
+def test_nested_argument_errors(ltdi):
+    cfg = W.config(2, n=5003)
+    hp, hc, ang, _ = W.sources(cfg, [0])
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    for order, nested in ((31, 0), (31, 2), (31, 5), (5, 3)):
+        with pytest.raises(ltdi.LtdiError):
+            ltdi.response_full_nested(orb, dhp, dhc, ang, 20, order, nested)
