@@ -33,6 +33,14 @@ class _Source(C.Structure):
     _fields_ = [("beta", C.c_double), ("lam", C.c_double), ("psi", C.c_double)]
 
 
+class _Chirp(C.Structure):
+    _fields_ = [("t_c", C.c_double), ("mc_s", C.c_double), ("dist_m", C.c_double), ("cos_iota", C.c_double),
+                ("phi_c", C.c_double), ("tau_cut", C.c_double), ("f_rd", C.c_double), ("tau_rd", C.c_double)]
+
+
+CHIRP_KEYS = ("t_c", "mc_s", "dist_m", "cos_iota", "phi_c", "tau_cut", "f_rd", "tau_rd")
+
+
 class _Hybrid(C.Structure):
     _fields_ = [("t_hyb", C.c_double), ("window_s", C.c_double), ("sigma_s", C.c_double),
                 ("taper", C.c_int32)]
@@ -254,6 +262,41 @@ class Oracle:
         rc = self.lib.orc_michelson_nested_from_links(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(y), C.c_int(gen), C.c_int(order),
                                                       C.c_int(nested_order), _ptr(out))
         assert rc == 0
+        return out
+
+    @staticmethod
+    def _chirps(params):
+        arr = (_Chirp * len(params))()
+        for i, p in enumerate(params):
+            arr[i] = _Chirp(*[float(p[k]) for k in CHIRP_KEYS])
+        return arr
+
+    def waveform_chirp(self, params, t0, dt, n):
+        """O13: the chirp + ringdown model sampled on t0 + i dt: hp, hc [batch][n] (rounded to double)."""
+        hp, hc = np.zeros((len(params), n)), np.zeros((len(params), n))
+        rc = self.lib.orc_waveform_chirp(self._chirps(params), C.c_int64(len(params)), C.c_double(t0), C.c_double(dt),
+                                         C.c_int64(n), C.c_int64(n), _ptr(hp), _ptr(hc))
+        if rc != 0:
+            raise ValueError(f"oracle waveform_chirp: status {rc}")
+        return hp, hc
+
+    def response_full_chirp(self, orbit, params, sources, gen, order, nb=0, ne=None, want=("XYZ", "y")):
+        """O13: Eq. (2.5) with the model evaluated at the retarded times, then O6 / O7."""
+        batch = len(params)
+        src, ns = self._sources(sources)
+        assert ns == batch
+        ne = orbit["n"] if ne is None else ne
+        ln = ne - nb
+        out = {"A": np.zeros((batch, ln)), "E": np.zeros((batch, ln)), "T": np.zeros((batch, ln))}
+        out["XYZ"] = np.zeros((3, batch, ln)) if "XYZ" in want else None
+        out["y"] = np.zeros((6, batch, ln)) if "y" in want else None
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_response_full_chirp(C.byref(d), _ptr(Rt), _ptr(Lt), self._chirps(params), C.c_int64(batch), src,
+                                              C.c_int(gen), C.c_int(order), C.c_int64(nb), C.c_int64(ne), _ptr(out["A"]),
+                                              _ptr(out["E"]), _ptr(out["T"]), _ptr(out["XYZ"]), _ptr(out["y"]))
+        if rc != 0:
+            raise ValueError(f"oracle full_chirp: status {rc}")
         return out
 
     def response_lfa(self, orbit, hp, hc, sources, gen, order, fd_order, nb=0, ne=None,

@@ -1121,6 +1121,119 @@ void orc_stencil3(const double *x, int64_t len, double dt, int fd_order, double 
     for (int64_t i = w; i < len - w; ++i) out[i] = (double)fd3_in(x, i, (real)dt, fd_order);
 }
 
+/* ---------------------------------------------------------------------------------- */
+/* O13  on-device waveform generation fused with the projection (SURVEY 8(f)-3,        */
+/*      step i of P:408): the leading-order chirp of Eq. (4.2)'s order joined to a      */
+/*      damped-sinusoid ringdown -- the input recipe of configs 1-4 (DESIGN.md          */
+/*      section 4) taken as a waveform MODEL with parameters, so that the strain can    */
+/*      be evaluated at any time instead of being read from a sampled series.           */
+/* ---------------------------------------------------------------------------------- */
+/* tau = t_c - t, tau_in = max(tau, tau_cut), u = tau_in / (5 Mc):
+ *   f     = (1 / pi) (5 / (256 tau_in))^(3/8) Mc^(-5/8)          (inverse of Eq. (4.2))
+ *   amp   = 4 (Mc c / d_L) (pi f Mc)^(2/3) = 4 (Mc c / d_L) (5 Mc / (256 tau_in))^(1/4)
+ *   Phi   = phi_c - 2 u^(5/8)
+ * after the join (x = tau_cut - tau > 0): amp *= exp(-x / tau_rd),
+ *   Phi  += 2 pi [ f_rd x - (f_rd - f_cut) tau_rd (1 - exp(-x / tau_rd)) ],   f_cut = f(tau_cut)
+ * h+ = amp (1 + cos^2 iota) / 2 cos Phi,   hx = amp cos iota sin Phi.   Mc = G M_c / c^3 in seconds. */
+typedef struct { double t_c, mc_s, dist_m, cos_iota, phi_c, tau_cut, f_rd, tau_rd; } orc_chirp;
+
+static void chirp_at(const orc_chirp *w, real t, real *hp, real *hc)
+{
+    const real mc = w->mc_s, tau_cut = w->tau_cut;
+    const real tau = (real)w->t_c - t;
+    const real tau_in = tau > tau_cut ? tau : tau_cut;
+    const real f_cut = (1 / R_PI) * R_POW(5 / (256 * tau_cut), (real)0.375) * R_POW(mc, (real)-0.625);
+    const real f = (1 / R_PI) * R_POW(5 / (256 * tau_in), (real)0.375) * R_POW(mc, (real)-0.625);
+    real amp = 4 * (mc * (real)ORC_C_LIGHT / (real)w->dist_m) * R_POW(R_PI * f * mc, (real)2 / 3);
+    real phase = (real)w->phi_c - 2 * R_POW(tau_in / (5 * mc), (real)0.625);
+    const real x = tau_cut - tau;
+    if (x > 0) {
+        const real decay = R_EXP(-x / (real)w->tau_rd);
+        amp *= decay;
+        phase += 2 * R_PI * ((real)w->f_rd * x - ((real)w->f_rd - f_cut) * (real)w->tau_rd * (1 - decay));
+    }
+    const real ci = w->cos_iota;
+    *hp = amp * (real)0.5 * (1 + ci * ci) * R_COS(phase);
+    *hc = amp * ci * R_SIN(phase);
+}
+
+/* the model sampled on the grid t_n = t0 + n dt, rounded to double: hp, hc [batch][ld] */
+int orc_waveform_chirp(const orc_chirp *w, int64_t batch, double t0, double dt, int64_t n, int64_t ld, double *hp,
+                       double *hc)
+{
+    if (!w || !hp || !hc || batch < 1 || n < 1 || ld < n || !(dt > 0)) return ORC_EINVAL;
+    for (int64_t b = 0; b < batch; ++b) {
+        if (!(w[b].mc_s > 0) || !(w[b].dist_m > 0) || !(w[b].tau_cut > 0) || !(w[b].tau_rd > 0)) return ORC_EINVAL;
+#pragma omp parallel for
+        for (int64_t i = 0; i < n; ++i) {
+            real a, c;
+            chirp_at(&w[b], (real)t0 + (real)i * (real)dt, &a, &c);
+            hp[b * ld + i] = (double)a;
+            hc[b * ld + i] = (double)c;
+        }
+    }
+    return ORC_OK;
+}
+
+/* Eq. (2.5) with the strain of the model evaluated AT the retarded times (no sampled series, no interpolation) */
+static void links_full_chirp_at(const orbit_ctx *o, const frame_t *f, const orc_chirp *w, int64_t n, real y[6])
+{
+    const real c = ORC_C_LIGHT;
+    const real t = (real)o->d.t0 + (real)n * (real)o->d.dt;
+    geom_t g;
+    orbit_geometry(o, n, &g);
+    for (int l = 0; l < 6; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real Fp, Fc, hps, hcs, hpr, hcr;
+        antenna(f, g.nh[l], &Fp, &Fc);
+        const real kn = dot3(f->k, g.nh[l]);
+        const real delta_s = g.L[l] + dot3(f->k, g.R[s]) / c; /* (2.6a) */
+        const real delta_r = dot3(f->k, g.R[r]) / c;          /* (2.6b) */
+        chirp_at(w, t - delta_s, &hps, &hcs);
+        chirp_at(w, t - delta_r, &hpr, &hcr);
+        y[l] = ((Fp * hps + Fc * hcs) - (Fp * hpr + Fc * hcr)) / (2 * (1 - kn)); /* (2.5) */
+    }
+}
+
+/* Full response from waveform parameters: links by links_full_chirp_at on the same ranges as full_one (the link series
+ * is still zero inside its margins, G11, so that it is the series the sampled path produces up to the interpolation
+ * error), then O6 / O7 unchanged. */
+int orc_response_full_chirp(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const orc_chirp *wav,
+                            int64_t batch, const orc_source *src, int gen, int order, int64_t nb, int64_t ne, double *A,
+                            double *E, double *T, double *XYZ, double *y)
+{
+    if (check_args(d, gen, order, 0, 0, d ? d->n : 0, nb, ne) || !wav || !src) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, 0, &mg);
+    const int64_t N = d->n;
+    for (int64_t b = 0; b < batch; ++b) {
+        frame_t f;
+        work_t w;
+        source_frame(&src[b], &f);
+        const int64_t y0 = imax(0, nb - mg.m2), y1 = imin(N, ne + (order + 1) / 2 + 1);
+        if (work_alloc(&w, y0, y1 - y0, ne - nb)) return ORC_EINVAL;
+#pragma omp parallel for schedule(dynamic, 64)
+        for (int64_t m = y0; m < y1; ++m) {
+            if (m < mg.m1 || m >= N - mg.m1) continue;
+            real yy[6];
+            links_full_chirp_at(&o, &f, &wav[b], m, yy);
+            for (int l = 0; l < 6; ++l) w.y[l][m - y0] = yy[l];
+        }
+        yseries_t ys = { { w.y[0], w.y[1], w.y[2], w.y[3], w.y[4], w.y[5] }, y0, y1 - y0 };
+#pragma omp parallel for schedule(dynamic, 64)
+        for (int64_t n = nb; n < ne; ++n) {
+            if (n < mg.lo || n >= N - mg.hi) continue;
+            geom_t g;
+            orbit_geometry(&o, n, &g);
+            for (int c = 0; c < 3; ++c) w.X[c][n - nb] = michelson_at(&ys, g.L, c, gen, n, (real)d->dt, order);
+        }
+        emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&w);
+    }
+    return ORC_OK;
+}
+
 /* Hybrid response (O9): both responses on the whole requested range, blended per Eqs. (4.5), (4.6);
  * hyb has n_hyb = 1 or batch entries. */
 int orc_response_hybrid(const orc_orbit_desc *d, const double *Rtab, const double *Ltab,

@@ -270,6 +270,30 @@ def source(cfg, idx):
     return hp, hc, (beta, lam, psi), meta
 
 
+def chirp_params(cfg, idx):
+    """Parameters of the chirp + ringdown model of source `idx` of configs 1-4 (the numbers source() feeds to
+    newtonian_chirp): dict t_c, mc_s, dist_m, cos_iota, phi_c, tau_cut, f_rd, tau_rd -- for the rows that generate the
+    strain themselves.  Without a ringdown (configs 1, 3) the join sits 1 ms before coalescence."""
+    k, n, dt = cfg["k"], cfg["n"], cfg["dt"]
+    assert k in (1, 2, 3, 4)
+    t_first = cfg["orbit"]["t0"]
+    t_end = t_first + dt * n
+    p = draw(cfg, idx)
+    mc = p["mchirp_s"]
+    out = {"mc_s": mc, "dist_m": p["dist"], "cos_iota": p["cos_iota"], "phi_c": p["phi_c"]}
+    if k in (2, 4):
+        rd = {"M_s": p["M"] * GMSUN_S, "dt": dt}
+        Mf = 0.95 * rd["M_s"]
+        t_m = t_end - p["merger_h_before_end"] * 3600.0 if k == 2 else t_first + (t_end - t_first) * p["merger_fraction"]
+        tau_cut = _tau_cut(mc, rd)
+        out.update(t_c=t_m + tau_cut, tau_cut=tau_cut, f_rd=min(0.37367 / (2.0 * math.pi * Mf), 0.2 / dt), tau_rd=Mf / 0.08896)
+    else:
+        tau_cut = 1e-3
+        t_c = t_end + 2.0 * DAY_S if k == 1 else t_first + 2.0 * 365.0 * DAY_S
+        out.update(t_c=t_c, tau_cut=tau_cut, f_rd=f_of_tau(tau_cut, mc), tau_rd=1.0)
+    return out
+
+
 def _tau_cut(mc_s, rd):
     M_s, dt = rd["M_s"], rd["dt"]
     f_grid = 0.2 / dt
