@@ -169,6 +169,38 @@ int ltdi_response_full_nested(const ltdi_orbits *orb, const double *d_hp, const 
                               double *d_A, double *d_E, double *d_T, double *d_XYZ, double *d_y, void *d_work,
                               size_t work_bytes, void *stream);
 
+/* waveform generation on the device, fused with the projection (step i of P:408).
+ * The chirp + ringdown MODEL (the recipe of BASELINE.json configs 1-4; leading-order chirp of the order of Eq. (4.2),
+ * P:283): with tau = t_c - t, Mc = G M_c / c^3 [s],
+ *   tau > tau_cut:  Phi = phi_c - 2 (tau / 5 Mc)^(5/8),  amp = 4 (Mc c / d_L)(5 Mc / (256 tau))^(1/4)
+ *   x = tau_cut - tau >= 0:  Phi = Phi(tau_cut) + 2 pi [f_rd x - (f_rd - f_cut) tau_rd (1 - exp(-x / tau_rd))],
+ *                            amp = amp(tau_cut) exp(-x / tau_rd),   f_cut = (1 / pi)(5 / (256 tau_cut))^(3/8) Mc^(-5/8)
+ *   h+ = amp (1 + cos^2 iota) / 2 cos Phi,   hx = amp cos iota sin Phi.
+ * A source without ringdown takes a tiny tau_cut (the join then lies outside the segment). */
+typedef struct {
+    double t_c;      /* coalescence time [s] (same clock as the time grid) */
+    double mc_s;     /* chirp mass G M_c / c^3 [s] */
+    double dist_m;   /* luminosity distance [m] */
+    double cos_iota; /* cosine of the inclination */
+    double phi_c;    /* phase at coalescence [rad] */
+    double tau_cut;  /* the ringdown joins tau_cut seconds before t_c, > 0 */
+    double f_rd;     /* ringdown frequency [Hz] */
+    double tau_rd;   /* ringdown damping time [s], > 0 */
+} ltdi_chirp;
+
+/* The model sampled on t0 + i dt, i < n: d_hp, d_hc [batch][ld] (device).  d_work: >= 160 bytes per source, 16-byte aligned. */
+int ltdi_waveform_chirp(const ltdi_chirp *h_wav, int64_t batch, double t0, double dt, int64_t n, int64_t ld,
+                        double *d_hp, double *d_hc, void *d_work, size_t work_bytes, void *stream);
+
+/* Full response straight from the model parameters: Eq. (2.5) with h+, hx EVALUATED at the retarded times t - delta_s,
+ * t - delta_r (no sampled strain is read and the first interpolation level is gone), then Eq. (2.7) / (2.8) and (2.9) as
+ * ltdi_response_full.  h_wav [batch]; ld = row stride of the outputs (>= n); Lagrange orders 9 and 31 (the order only
+ * acts in the TDI stage).  The result differs from ltdi_response_full on the sampled model by the interpolation error of
+ * the latter (largest where the model's envelope has its kink at the join). */
+int ltdi_response_full_chirp(const ltdi_orbits *orb, const ltdi_chirp *h_wav, int64_t ld, int64_t batch,
+                             const ltdi_source *h_src, int gen, int lagrange_order, double *d_A, double *d_E,
+                             double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream);
+
 /* Low-frequency approximation: Eq. (B10) links at the retarded time (B1) from central-difference
  * derivatives of h+, hx (S6), Eq. (B25) (gen 1.5) / (B33) (gen 2.0) Michelson (S7).  fd_order 2 | 4.
  * Links -1, -2, -3 are zero. */

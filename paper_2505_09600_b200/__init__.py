@@ -50,6 +50,21 @@ class Source(C.Structure):
     _fields_ = [("beta", C.c_double), ("lam", C.c_double), ("psi", C.c_double)]
 
 
+class Chirp(C.Structure):
+    _fields_ = [("t_c", C.c_double), ("mc_s", C.c_double), ("dist_m", C.c_double), ("cos_iota", C.c_double),
+                ("phi_c", C.c_double), ("tau_cut", C.c_double), ("f_rd", C.c_double), ("tau_rd", C.c_double)]
+
+
+CHIRP_KEYS = ("t_c", "mc_s", "dist_m", "cos_iota", "phi_c", "tau_cut", "f_rd", "tau_rd")
+
+
+def _chirps(params):
+    arr = (Chirp * len(params))()
+    for i, p in enumerate(params):
+        arr[i] = Chirp(*[float(p[k]) for k in CHIRP_KEYS])
+    return arr
+
+
 class Hybrid(C.Structure):
     _fields_ = [("t_hyb", C.c_double), ("window_s", C.c_double), ("sigma_s", C.c_double),
                 ("taper", C.c_int32)]
@@ -75,6 +90,10 @@ _SIGNATURES = {
                                      _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_full_nested": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
                                             _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_waveform_chirp": (C.c_int, [C.POINTER(Chirp), C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64, _dp, _dp, _vp,
+                                      C.c_size_t, _vp]),
+    "ltdi_response_full_chirp": (C.c_int, [_vp, C.POINTER(Chirp), C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                           _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                     C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa_ext": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
@@ -341,6 +360,33 @@ def response_full(orb, hp, hc, sources, gen, order, want_xyz=False, want_y=False
 def response_full_nested(orb, hp, hc, sources, gen, order, nested_order=3, want_xyz=False, want_y=False, workspace=None):
     """the full response with properly nested TDI delays (light times looked up by Lagrange order 3)."""
     return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_xyz, want_y, workspace, ext=(nested_order,))
+
+
+def waveform_chirp(params, t0, dt, n, device="cuda:0", out=None):
+    """the chirp + ringdown model of `params` (list of dicts, CHIRP_KEYS) sampled on t0 + i dt on the device:
+    returns hp, hc [batch][n] float64 device tensors (ltdi_waveform_chirp)."""
+    batch = len(params)
+    dev = torch.device(device)
+    hp, hc = out if out is not None else (torch.empty(batch, n, dtype=torch.float64, device=dev) for _ in range(2))
+    work = torch.empty(batch * 20, dtype=torch.float64, device=dev)
+    with torch.cuda.device(dev):
+        _check("ltdi_waveform_chirp", lib().ltdi_waveform_chirp(_chirps(params), batch, float(t0), float(dt), int(n), int(hp.shape[1]),
+                                                                hp.data_ptr(), hc.data_ptr(), work.data_ptr(), work.numel() * 8, _stream()))
+    return hp, hc
+
+
+def response_full_chirp(orb, params, sources, gen, order, want_xyz=False, want_y=False, workspace=None):
+    """full response from waveform parameters, the model evaluated at the retarded times of Eq. (2.5)."""
+    batch, ld = len(params), orb.n
+    src_ptr, keep = _sources(sources)
+    assert keep.shape[0] == batch
+    ws = workspace or Workspace(batch, ld, orb.device, want_xyz, want_y)
+    p = lambda t: None if t is None else t.data_ptr()
+    with torch.cuda.device(orb.device):
+        rc = lib().ltdi_response_full_chirp(orb.handle, _chirps(params), ws.A.shape[1], batch, src_ptr, gen, order, p(ws.A), p(ws.E),
+                                            p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream())
+    _check("ltdi_response_full_chirp", rc)
+    return ws.outputs()
 
 
 def response_lfa(orb, hp, hc, sources, gen, order, fd_order, want_xyz=False, want_y=False, workspace=None):

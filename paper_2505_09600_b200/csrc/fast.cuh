@@ -30,6 +30,7 @@
 #pragma once
 #include "common.cuh"
 #include "dd.cuh"
+#include "chirp.cuh"
 
 #define FAST_TC_R 7                       /* samples per thread in the TDI kernel */
 #define FAST_TCA 448                      /* samples per anchor tile */
@@ -659,6 +660,79 @@ template <int H, bool LFA>
 __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(const __grid_constant__ FastParams p)
 {
     link_body<H, LFA>(p, blockIdx.x);
+}
+
+// Eq. (2.5) with the strain of the chirp + ringdown model evaluated AT the nine retarded times of a sample
+// (chirp.cuh) instead of interpolated from a sampled series: no strain is read, nothing is staged but the source frame;
+// a thread owns two consecutive samples and reads its table entries straight from global memory (coalesced double2).
+// The link series go to the same scratch as link_kernel's: the TDI stage is unchanged.
+__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_chirp_kernel(const __grid_constant__ FastParams p,
+                                                                       const ChirpDev *__restrict__ wav /* of the chunk */)
+{
+    const int64_t b = (int64_t)blockIdx.x % p.batch, tile = (int64_t)blockIdx.x / p.batch;
+    const int64_t a0 = tile * FAST_TA;
+    const int tid = threadIdx.x;
+    __shared__ double fr[LTDI_FRAME_STRIDE];
+    __shared__ ChirpDev sw;
+    if (p.use_small) {
+        if (tid == 0) {
+            const double *sr = p.small + 3 * (p.b0 + b);
+            source_frame_one(sr[0], sr[1], sr[2], fr);
+        }
+    } else if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
+    if (tid >= 32 && tid < 32 + LTDI_CHIRP_STRIDE) reinterpret_cast<double *>(&sw)[tid - 32] = reinterpret_cast<const double *>(wav + b)[tid - 32];
+    __syncthreads();
+    const int64_t m0 = a0 + 2 * tid;
+    if (m0 >= p.n) return;
+    const int64_t vlo = p.m1, vhi = p.n - p.m1;
+    const bool in0 = m0 >= vlo && m0 < vhi, in1 = m0 + 1 >= vlo && m0 + 1 < vhi;
+    double *yout = p.yF + b * p.lds + m0;
+    const int64_t ystride = p.batch * p.lds;
+    if (!in0 && !in1) {
+#pragma unroll
+        for (int l = 0; l < 6; ++l) *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(0.0, 0.0);
+        return;
+    }
+    const double *t = p.tab + m0;
+    const double inv_c = 1.0 / LTDI_C_LIGHT;
+    auto row2 = [&](int r) { return *reinterpret_cast<const double2 *>(t + (int64_t)r * p.stride); };
+    const dd s0 = two_prod((double)m0, p.dt), s1 = two_prod((double)(m0 + 1), p.dt);   /* t_n - t0 */
+    double rp0 = 0.0, rc0 = 0.0, rp1 = 0.0, rc1 = 0.0;
+#pragma unroll 1
+    for (int step = 0; step < 9; ++step) {   /* receiver r, then the two links it receives (as link_body) */
+        const int r = step / 3, s = step - 3 * r;
+        const int a = s == 1 ? (r + 2) % 3 : (r + 1) % 3;
+        const int l = s == 2 ? a + 3 : a;
+        const int sc = s == 0 ? r : (s == 1 ? (r + 1) % 3 : (r + 2) % 3);
+        const double2 x = row2(ROW_R + 3 * sc), y = row2(ROW_R + 3 * sc + 1), z = row2(ROW_R + 3 * sc + 2);
+        double d0 = (fr[0] * x.x + fr[1] * y.x + fr[2] * z.x) * inv_c;
+        double d1 = (fr[0] * x.y + fr[1] * y.y + fr[2] * z.y) * inv_c;
+        if (s != 0) {
+            const double2 L = row2(ROW_L + l);
+            d0 = L.x + d0;                                           /* (2.6a) */
+            d1 = L.y + d1;
+        }
+        double ap0, ac0, ap1, ac1;
+        chirp_eval(sw, dd_add_d(s0, -d0), ap0, ac0);
+        chirp_eval(sw, dd_add_d(s1, -d1), ap1, ac1);
+        if (s == 0) {
+            rp0 = ap0; rc0 = ac0; rp1 = ap1; rc1 = ac1;
+        } else {
+            const double2 nx = row2(ROW_N + 3 * a), ny = row2(ROW_N + 3 * a + 1), nz = row2(ROW_N + 3 * a + 2);
+            double y01[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const double n0 = h ? nx.y : nx.x, n1 = h ? ny.y : ny.x, n2 = h ? nz.y : nz.x;
+                const double un = fr[3] * n0 + fr[4] * n1 + fr[5] * n2, vn = fr[6] * n0 + fr[7] * n1 + fr[8] * n2;
+                const double kn = fr[0] * n0 + fr[1] * n1 + fr[2] * n2;
+                const double xip = un * un - vn * vn, xic = 2.0 * un * vn;   /* (2.4) */
+                const double Fp = xip * fr[9] + xic * fr[10], Fc = xic * fr[9] - xip * fr[10];   /* (2.2) + (2.3), G17 */
+                const double e = 2.0 * (1.0 - (s == 2 ? -kn : kn));
+                y01[h] = (Fp * ((h ? ap1 : ap0) - (h ? rp1 : rp0)) + Fc * ((h ? ac1 : ac0) - (h ? rc1 : rc0))) / e;   /* (2.5) */
+            }
+            *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y01[0] : 0.0, in1 ? y01[1] : 0.0);
+        }
+    }
 }
 
 // hybrid: both kinds of link tiles in ONE launch -- the few full-link tiles (first in the grid: they are the heavy

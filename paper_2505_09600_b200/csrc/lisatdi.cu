@@ -249,8 +249,8 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
 }
 
 // workspace layout (doubles): raw sources [batch][3] | frames [batch][16] | hybrid windows [n_hyb][4] | hybrid tile
-// plan [batch][4] (eight 32-bit integers per source, HybPlan)
-size_t work_doubles(int64_t batch) { return ((size_t)batch * (3 + LTDI_FRAME_STRIDE + 4 + 4) + 31) / 32 * 32; }
+// plan [batch][4] (eight 32-bit integers per source, HybPlan) | waveform model constants [batch][20] (ChirpDev, 8(f)-3)
+size_t work_doubles(int64_t batch) { return ((size_t)batch * (3 + LTDI_FRAME_STRIDE + 4 + 4 + LTDI_CHIRP_STRIDE) + 31) / 32 * 32; }
 
 bool fast_order(int order) { return order == 9 || order == 31; }
 
@@ -427,6 +427,30 @@ int launch_response(DeviceState &ds, const RespParams &p, int threads, size_t sm
     return LTDI_OK;
 }
 
+/* waveform model constants of `batch` sources to the device: kernel arguments in slices of 96 sources (as BigArgs) */
+#define LTDI_CHIRP_SLICE 96
+struct ChirpArgs { ChirpDev v[LTDI_CHIRP_SLICE]; };
+__global__ void unpack_chirp_kernel(const __grid_constant__ ChirpArgs a, int count, ChirpDev *out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count * LTDI_CHIRP_STRIDE) reinterpret_cast<double *>(out)[i] = reinterpret_cast<const double *>(a.v)[i];
+}
+int upload_chirps(const ltdi_chirp *h_wav, int64_t batch, double t0, ChirpDev *d_out, cudaStream_t st)
+{
+    ChirpArgs *a = new (std::nothrow) ChirpArgs;
+    if (!a) return LTDI_EINVAL;
+    for (int64_t b0 = 0; b0 < batch; b0 += LTDI_CHIRP_SLICE) {
+        const int cnt = (int)std::min<int64_t>(LTDI_CHIRP_SLICE, batch - b0);
+        for (int i = 0; i < cnt; ++i)
+            if (chirp_fill(h_wav[b0 + i], t0, &a->v[i])) { delete a; return LTDI_EINVAL; }
+        unpack_chirp_kernel<<<(cnt * LTDI_CHIRP_STRIDE + 127) / 128, 128, 0, st>>>(*a, cnt, d_out + b0);
+        count_launch();
+        if (cudaGetLastError() != cudaSuccess) { delete a; return LTDI_ECUDA; }
+    }
+    delete a;
+    return LTDI_OK;
+}
+
 /* host side of the hybrid plan: per-source plans (offsets relative to the source's chunk) and per-chunk totals */
 struct ChunkTotals { int64_t link_full, link_lfa, lfa, blend, full, max_slots; };
 struct HybHost {
@@ -568,7 +592,8 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
             if (full) {
                 {
                     ProfScope ps(LTDI_KERNEL_LINK_FULL + LTDI_KERNEL_COUNT * which, st);
-                    link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
+                    if (rp.chirp) link_chirp_kernel<<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, 0, st>>>(p, rp.chirp + b0);
+                    else link_kernel<H, false><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link, st>>>(p);
                 }
                 count_launch();
                 ProfScope ps(LTDI_KERNEL_TDI + LTDI_KERNEL_COUNT * which, st);
@@ -652,14 +677,15 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
                  double *d_y, void *d_work, size_t work_bytes, void *stream, int lfa_terms = 1,
-                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0)
+                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0, const ltdi_chirp *h_wav = nullptr)
 {
     if (nested_order != 0 && (which != LTDI_RESPONSE_FULL || nested_order != 3)) return nested_order == 3 || nested_order < 0 || !(nested_order & 1) ? LTDI_EINVAL : LTDI_EUNSUPPORTED;
     if (nested_order && !fast_order(order)) return LTDI_EUNSUPPORTED;   /* nested delays run on the tuned path (orders 9, 31) */
     if (lfa_terms < 1 || lfa_terms > 2 || lfa_point < LTDI_LFA_CENTRAL || lfa_point > LTDI_LFA_FORWARD) return LTDI_EINVAL;
     if (lfa_terms == 2 && lfa_point != LTDI_LFA_CENTRAL) return LTDI_EINVAL;
     if ((lfa_terms != 1 || lfa_point != LTDI_LFA_CENTRAL) && which != LTDI_RESPONSE_LFA) return LTDI_EINVAL;
-    if (!orb || !d_hp || !d_hc || !h_src || !d_A || !d_E || !d_T || !d_work) return LTDI_EINVAL;
+    if (!orb || ((!d_hp || !d_hc) && !h_wav) || !h_src || !d_A || !d_E || !d_T || !d_work) return LTDI_EINVAL;
+    if (h_wav && (which != LTDI_RESPONSE_FULL || !fast_order(order))) return which != LTDI_RESPONSE_FULL ? LTDI_EINVAL : LTDI_EUNSUPPORTED;
     if (!gen_ok(gen) || !order_ok(order) || batch < 1 || ld < orb->desc.n) return LTDI_EINVAL;
     if (which != LTDI_RESPONSE_FULL && fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
     if (which == LTDI_RESPONSE_FULL) fd_order = 0;
@@ -703,6 +729,11 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     double *w_frames = w_src + 3 * batch;
     HybDev *w_hyb = (HybDev *)(w_frames + LTDI_FRAME_STRIDE * batch);
     HybPlan *w_plan = (HybPlan *)((double *)w_hyb + 4 * batch);
+    ChirpDev *w_chirp = (ChirpDev *)((double *)w_plan + 4 * batch);
+    if (h_wav) {   /* the model constants of every source (host, long double) to the workspace */
+        const int rcw = upload_chirps(h_wav, batch, orb->desc.t0, w_chirp, st);
+        if (rcw) return rcw;
+    }
     SmallArgs small_args;
     bool have_small = false;   /* batch <= 32: the tuned kernels take the parameters as arguments (no launch) */
     if (batch <= 32) {
@@ -757,6 +788,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.m1 = mg.m1; p.m2 = mg.m2; p.w = mg.w; p.lo = mg.lo; p.hi = mg.hi;
     p.qmax = (int)(mg.m1 - M / 2);
     p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw; p.nested = nested_order != 0;
+    p.chirp = h_wav ? w_chirp : nullptr;
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
     if (fast_order(order)) {
@@ -1020,6 +1052,30 @@ int ltdi_response_full_nested(const ltdi_orbits *orb, const double *d_hp, const 
     if (nested_order == 0) return LTDI_EINVAL;
     return run_response(LTDI_RESPONSE_FULL, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0,
                         d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, nested_order);
+}
+
+int ltdi_response_full_chirp(const ltdi_orbits *orb, const ltdi_chirp *h_wav, int64_t ld, int64_t batch,
+                             const ltdi_source *h_src, int gen, int lagrange_order, double *d_A, double *d_E, double *d_T,
+                             double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    if (!h_wav) return LTDI_EINVAL;
+    return run_response(LTDI_RESPONSE_FULL, orb, nullptr, nullptr, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0,
+                        d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, 0, h_wav);
+}
+
+int ltdi_waveform_chirp(const ltdi_chirp *h_wav, int64_t batch, double t0, double dt, int64_t n, int64_t ld, double *d_hp,
+                        double *d_hc, void *d_work, size_t work_bytes, void *stream)
+{
+    if (!h_wav || !d_hp || !d_hc || !d_work || batch < 1 || batch > 65535 || n < 1 || ld < n || !(dt > 0.0)) return LTDI_EINVAL;
+    if (work_bytes < (size_t)batch * sizeof(ChirpDev)) return LTDI_EWORKSPACE;
+    if ((uintptr_t)d_work % 16) return LTDI_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int rc = upload_chirps(h_wav, batch, t0, (ChirpDev *)d_work, st);
+    if (rc) return rc;
+    chirp_grid_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)batch), 256, 0, st>>>((const ChirpDev *)d_work, dt, n, ld, d_hp, d_hc);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    return LTDI_OK;
 }
 
 int ltdi_response_lfa(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,

@@ -31,6 +31,7 @@ struct RespParams {
     int off_yL, off_dL, off_hs; /* shared-memory offsets (doubles) of the LFA links, their derivative, the strain */
     int qmax;             /* bound on |integer shift| of a projection delay (m1 - M/2) */
     int nested;           /* nested TDI delays (tuned path only) */
+    const struct ChirpDev *chirp; /* waveform model constants [batch], or nullptr (sampled strain) */
     int lfa_terms, lfa_point, xw; /* terms of Eq. (B4), expansion point LTDI_LFA_*, xw = terms - 1 */
     int64_t ntiles;
 };
