@@ -333,9 +333,10 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
     if ws is None:
         ws = Workspace(batch, ld, hp.device, want_xyz, want_y)
     p = lambda t: None if t is None else t.data_ptr()
-    tail = [p(ws.A), p(ws.E), p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream()]
     head = [orb.handle, hp.data_ptr(), hc.data_ptr(), ld, batch, src_ptr, gen, order]
     with torch.cuda.device(hp.device):
+        # the stream handle must be the current stream of the tensors' device: evaluated inside the device context
+        tail = [p(ws.A), p(ws.E), p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream()]
         if which == RESPONSE_FULL and ext is not None:
             rc, fn = lib().ltdi_response_full_nested(*head, int(ext[0]), *tail), "ltdi_response_full_nested"
         elif which == RESPONSE_FULL:
@@ -455,6 +456,12 @@ class HostPipeline:
                     slot["event"].synchronize()          # the slot's previous results have reached the host
                 slot["stream"].wait_stream(torch.cuda.current_stream())   # orbit tables etc. of the caller
                 stream = slot["stream"].cuda_stream
+                # tensors allocated on another stream and read by the slot's stream: tell the caching allocator, so that
+                # dropping the Orbits object while a call is in flight cannot hand their memory out again
+                self.orb.tables.record_stream(slot["stream"])
+                if self.orb._anchors is not None:
+                    self.orb._anchors.record_stream(slot["stream"])
+                slot["scratch"].record_stream(slot["stream"])
             rc = lib().ltdi_response_host(which, self.orb.handle, hp_host.data_ptr(), hc_host.data_ptr(), self.ld,
                                           self.batch, src_ptr, gen, order, fd_order, harr, nh, A.data_ptr(),
                                           E.data_ptr(), T.data_ptr(), slot["scratch"].data_ptr(),

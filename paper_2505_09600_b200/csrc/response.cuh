@@ -51,13 +51,6 @@ __device__ __forceinline__ void source_frame_one(double beta, double lam, double
     f[9] = c2;       f[10] = s2;
 }
 
-__global__ void source_frame_kernel(const double *__restrict__ src, double *__restrict__ frames, int64_t batch)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= batch) return;
-    source_frame_one(src[3 * b + 0], src[3 * b + 1], src[3 * b + 2], frames + b * LTDI_FRAME_STRIDE);
-}
-
 // ---------------------------------------------------------------------------------------------
 // Lagrange fractional delay (G10): taps k = -(M/2-1) .. M/2 around sample j = n - ceil(d/dt)
 // ---------------------------------------------------------------------------------------------
