@@ -22,6 +22,7 @@ struct ltdi_orbits {
     int64_t stride;
     const double *d_anc; /* TDI weight anchors and their headers from ltdi_orbits_prepare(), or NULL */
     int anc_gen, anc_M;  /* generation and tap count they were computed for */
+    bool anc_has2;       /* they carry the second derivative of the weights too */
 };
 
 /* table rows: LTDI_TABLE_ROWS rows of doubles, then LTDI_TABLE_LO_ROWS rows of floats (same row stride in elements)

@@ -43,6 +43,8 @@ __host__ __device__ constexpr int tdi_tc(int which) { return FAST_TC_R * tdi_g(w
 __host__ __device__ constexpr int tdi_threads(int which) { return 3 * tdi_g(which); }
 #define FAST_TA_THREADS 128
 #define FAST_TA (2 * FAST_TA_THREADS)     /* 256 samples per link tile, three CTAs per SM */
+#define FAST_TAL (FAST_TA - 4)            /* LFA link tiles: 256 link samples give the time derivative of 252 (two samples of rim
+                                           * on either side serve the widest stencil and keep the tile start even) */
 #define FAST_NA_FULL 39                   /* anchors per tile: 3 channels x 13 delays */
 #define FAST_NA_LFA 12                    /* 2 generations x 3 channels x 2 delays (gen 1.5 first) */
 #define FAST_NA_LFA_GEN 6                 /* those of one generation */
@@ -67,6 +69,8 @@ struct FastParams {
     int use_small;           /* batch_all <= 32: sources and hybrid windows travel in `small` as kernel arguments and
                               * every CTA derives its source frame itself (no parameter kernel in front of the call) */
     double small[32 * 7];    /* [32][3] beta, lambda, psi, then [32][4] t_hyb, window, sigma, taper (by absolute source) */
+    double small_fr[32 * 11]; /* [32][11] source frames k, u, v, cos 2psi, sin 2psi (S1, formed on the host in long double: as
+                              * one thread's three sincos in front of every CTA it cost the single-source configs ~1 us per tile) */
     const double *hyb;       /* [n_hyb][4] of this chunk (t_hyb, window, sigma, taper) */
     int64_t n_hyb;
     int which, gen, fd;
@@ -75,7 +79,9 @@ struct FastParams {
     int64_t m1, m2, w, lo, hi;
     int64_t m2_15, m2_20;    /* anchor kernel: backward TDI reach of either generation (the anchors serve both) */
     int qmax;
-    double *yF, *yL;         /* scratch link series [6][batch][lds], [3][batch][lds] */
+    double *yF, *yL;         /* scratch [6][batch][lds]: full links; [3][batch][lds]: TIME DERIVATIVE (gen 1.5: first, gen 2.0:
+                              * second) of the LFA links, formed by the link kernel itself */
+    double *yLraw;           /* [3][batch][lds] the LFA links themselves, written only when the caller asks for d_y */
     int64_t lds;
     double *A, *E, *T, *XYZ, *Y; /* outputs of this chunk ([batch][ld] ...), XYZ / Y strides use batch_all */
     int64_t batch_all, b0;   /* full batch and first source of the chunk (for the [3][batch][ld] outputs) */
@@ -316,6 +322,12 @@ __device__ __forceinline__ void interp_delays(const FastParams &p, double d0, do
 // ---------------------------------------------------------------------------------------------
 #define LFA_ANC_DOUBLES 28
 #define LFA_LO_ROWS 12
+/* a staged low-part row: floats of samples a0 - 2 .. a0 + FAST_TA + 1 (+ padding), so that the copy starts on a 16-byte
+ * boundary although an LFA tile starts at a0 = 2 (mod 4); sample a0 + i sits at element 2 + i */
+#define LFA_TLW (FAST_TA + 8)
+/* doubles of the raw-strain region of the LFA link kernel: two series of 2 hw2 + 2 LFA_RAW_HALO samples, and at least the
+ * three link rows of the tile that take its place after the stencil pass */
+__host__ __device__ constexpr int lfa_raw_doubles(int hw2) { return 2 * (2 * hw2 + 8) > 3 * FAST_TA ? 2 * (2 * hw2 + 8) : 3 * FAST_TA; }
 #define LFA_RAW_HALO 4   /* raw strain staged beyond the FD series on either side: the widest stencil (d^3/dt^3, order 4) needs 3;
                           * even, so that the staged run starts on a 16-byte boundary for the bulk copy */
 
@@ -336,8 +348,8 @@ __device__ __forceinline__ void lfa_anchor_warp(const double *fr, const double *
     const double dp = u[ja] * u[jb] - v[ja] * v[jb];     /* (2.4a) as a matrix */
     const double dc = u[ja] * v[jb] + v[ja] * u[jb];     /* (2.4b) */
     const double P = pol == 0 ? dp * c2 + dc * s2 : dc * c2 - dp * s2;   /* (2.2) + (2.3), G17 */
-    const dd na = dd_make(tb[(ROW_N + 3 * l + ja) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + ja) * FAST_TA + ic]);
-    const dd nb = dd_make(tb[(ROW_N + 3 * l + jb) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + jb) * FAST_TA + ic]);
+    const dd na = dd_make(tb[(ROW_N + 3 * l + ja) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + ja) * LFA_TLW + 2 + ic]);
+    const dd nb = dd_make(tb[(ROW_N + 3 * l + jb) * FAST_TA + ic], (double)tl[(LO_N + 3 * l + jb) * LFA_TLW + 2 + ic]);
     dd t = dd_mul_d(dd_mul(na, nb), e < 3 ? P : 2.0 * P);
     if (!term) t = dd_make(0.0, 0.0);
 #pragma unroll
@@ -362,7 +374,7 @@ __device__ __forceinline__ void lfa_anchor_warp(const double *fr, const double *
     if (lane >= 22 && lane < 25) {
         const int a = lane - 22;
         an[10 + a] = tb[(ROW_N + 3 * l + a) * FAST_TA + ic];
-        an[13 + a] = (double)tl[(LO_N + 3 * l + a) * FAST_TA + ic];
+        an[13 + a] = (double)tl[(LO_N + 3 * l + a) * LFA_TLW + 2 + ic];
     }
 }
 
@@ -401,17 +413,16 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     extern __shared__ double smem[];
     int64_t b, tile;
     work_item(p, bid, b, tile);
-    const int64_t a0 = tile * FAST_TA;               /* first sample of the tile (even) */
+    /* first link sample of the tile (even).  LFA: the tile also differentiates its links in time (G15) and stores the
+     * derivative of its inner FAST_TAL samples, so consecutive tiles overlap by the rim of the stencil */
+    const int64_t a0 = LFA ? tile * FAST_TAL - 2 : tile * FAST_TA;
     const int tid = threadIdx.x;
     const int w = LFA ? (int)p.w : 0;
 
     __shared__ double fr[LTDI_FRAME_STRIDE];
     __shared__ double s_anc[LFA ? 3 * LFA_ANC_DOUBLES : 1];
     if (p.use_small) {
-        if (tid == 0) { /* S1, Eq. (2.1) with G1, (2.3): the same device function as the parameter kernel */
-            const double *sr = p.small + 3 * (p.b0 + b);
-            source_frame_one(sr[0], sr[1], sr[2], fr);
-        }
+        if (tid < 11) fr[tid] = p.small_fr[11 * (p.b0 + b) + tid];   /* S1, Eq. (2.1) with G1, (2.3) */
     } else if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
 
     /* staged strain: samples [org, org + 2 * hw2), org even; parity split; LFA: FD1 numerators of the strain */
@@ -426,7 +437,9 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     constexpr int NROWS = LFA ? ROW_L + 3 : LTDI_TABLE_ROWS;
     double *tb = ho_c + hw2;
     __shared__ uint64_t s_bar;
-    const unsigned nl = (unsigned)min((int64_t)FAST_TA, p.stride - a0);   /* a multiple of 32 elements */
+    const int64_t tl0 = max(a0, (int64_t)0), tl1 = min(a0 + FAST_TA, p.stride);       /* table samples of the tile */
+    const unsigned nl = (unsigned)max(tl1 - tl0, (int64_t)0);                          /* even */
+    const int toff = (int)(tl0 - a0);                                                  /* 0, or 2 in the first LFA tile */
     float *tl = nullptr;   /* LFA: low parts of the dd table entries of the tile */
     double *he3_p = nullptr; /* LFA, terms = 2: [4][hw2] third-derivative numerators (even +, odd +, even x, odd x) */
     if (!LFA) {
@@ -437,7 +450,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                 mbar_expect_tx(&s_bar, NROWS * nl * 8u);
             }
             __syncwarp();
-            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA, p.tab + (int64_t)tid * p.stride + a0, nl * 8u, &s_bar);
+            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA + toff, p.tab + (int64_t)tid * p.stride + tl0, nl * 8u, &s_bar);
         }
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -458,24 +471,26 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
          * and of L_+l (3 rows): float rows LO_N .. LO_L + 2 of the table */
         const int nraw = 2 * hw2 + 2 * LFA_RAW_HALO;
         double *raw_p = tb + NROWS * FAST_TA, *raw_c = raw_p + nraw;
-        tl = reinterpret_cast<float *>(raw_c + nraw);
+        tl = reinterpret_cast<float *>(raw_p + lfa_raw_doubles(hw2));   /* the raw region later holds the tile's links */
         const int64_t rs = org - LFA_RAW_HALO;                                   /* even */
         const int64_t g_lo = max(rs, (int64_t)0), g_hi = min(rs + nraw, p.n);
         const int ncopy = (int)max(g_hi - g_lo, (int64_t)0);
         /* one bulk copy per series needs 16-byte aligned ends (an odd ld or n falls back to element copies) */
+        const int64_t f0 = max(a0 - 2, (int64_t)0), f1 = min(a0 + FAST_TA + 2, p.stride);   /* low-part samples, multiples of 4 */
+        const unsigned nf = (unsigned)max(f1 - f0, (int64_t)0);
         const bool bulk = ncopy > 0 && !(ncopy & 1) &&
                           !((reinterpret_cast<uintptr_t>(gp + g_lo) | reinterpret_cast<uintptr_t>(gc + g_lo)) & 15);
         if (tid < 32) {
             if (tid == 0) {
                 mbar_init(&s_bar, 1);
                 asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-                mbar_expect_tx(&s_bar, NROWS * nl * 8u + LFA_LO_ROWS * nl * 4u + (bulk ? 2u * ncopy * 8u : 0u));
+                mbar_expect_tx(&s_bar, NROWS * nl * 8u + LFA_LO_ROWS * nf * 4u + (bulk ? 2u * ncopy * 8u : 0u));
             }
             __syncwarp();
-            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA, p.tab + (int64_t)tid * p.stride + a0, nl * 8u, &s_bar);
-            if (tid < LFA_LO_ROWS) {
+            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA + toff, p.tab + (int64_t)tid * p.stride + tl0, nl * 8u, &s_bar);
+            if (tid < LFA_LO_ROWS) {   /* float rows from sample a0 - 2 (a multiple of 4) on: see LFA_TLW */
                 const float *glo = reinterpret_cast<const float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride);
-                bulk_g2s(tl + tid * FAST_TA, glo + (int64_t)tid * p.stride + a0, nl * 4u, &s_bar);
+                bulk_g2s(tl + tid * LFA_TLW + (f0 - (a0 - 2)), glo + (int64_t)tid * p.stride + f0, nf * 4u, &s_bar);
             }
             if (bulk && tid >= 30) {
                 const double *src = tid == 30 ? gp : gc;
@@ -493,12 +508,12 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             }
         }
         /* SURVEY 8(f)-2, terms = 2: the d^3h/dt^3 numerators, parity-split like the first-derivative series */
-        he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * FAST_TA);
+        he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * LFA_TLW);
         cp_async_wait_all();
         __syncthreads();
         mbar_wait(&s_bar, 0);
         /* tile anchors of the antenna patterns: warp l builds the anchor of link l, then joins the stencil pass */
-        if (tid < 96) lfa_anchor_warp(fr, tb, tl, tid >> 5, (int)min((int64_t)(FAST_TA / 2), p.n - 1 - a0), s_anc, tid & 31);
+        if (tid < 96) lfa_anchor_warp(fr, tb, tl, tid >> 5, (int)max(min((int64_t)(FAST_TA / 2), p.n - 1 - a0), (int64_t)toff), s_anc, tid & 31);
         const int ws = w + p.xw;   /* the widest stencil applied to the strain */
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -531,18 +546,22 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     }
 
     const int64_t m0 = a0 + 2 * tid;
-    if (m0 >= p.n) return;
+    if (!LFA && m0 >= p.n) return;
     const int rel0 = (int)(m0 - org);
     const int64_t vlo = p.m1 + w + (LFA ? p.xw : 0), vhi = p.n - vlo;   /* valid link samples */
     const bool in0 = m0 >= vlo && m0 < vhi, in1 = m0 + 1 >= vlo && m0 + 1 < vhi;
-    double *yout = (LFA ? p.yL : p.yF) + b * p.lds + m0;
+    double *yout = p.yF + b * p.lds + m0;                /* full links: straight to the scratch */
+    double *ysm = LFA ? tb + NROWS * FAST_TA : nullptr;  /* LFA links of the tile [3][FAST_TA], on top of the raw strain (done with) */
     const int64_t ystride = p.batch * p.lds;
-    constexpr int NL = LFA ? 3 : 6;
     if (!in0 && !in1) {
+        if (!LFA) {
 #pragma unroll
-        for (int l = 0; l < NL; ++l) *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(0.0, 0.0);
-        return;
-    }
+            for (int l = 0; l < 6; ++l) *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(0.0, 0.0);
+            return;
+        }
+#pragma unroll
+        for (int l = 0; l < 3; ++l) *reinterpret_cast<double2 *>(ysm + l * FAST_TA + 2 * tid) = make_double2(0.0, 0.0);
+    } else {
 
     const double *t = tb + 2 * tid;
     const double inv_c = 1.0 / LTDI_C_LIGHT;
@@ -613,7 +632,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
          * 2.45 / (omega dt)^2).  The stencil denominator 1 / (2 dt) is a constant factor (its rounding is a constant
          * relative offset of 1e-16, not noise). */
         const double kscale = -0.5 * p.inv_fd1;
-        const float *tlo = tl + 2 * tid;
+        const float *tlo = tl + 2 + 2 * tid;
 #pragma unroll 1
         for (int l = 0; l < 3; ++l) {
             const int s = link_sender(l), r = link_receiver(l);
@@ -643,15 +662,45 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             }
             const double *an = s_anc + l * LFA_ANC_DOUBLES;
             const double2 nx = row2(ROW_N + 3 * l), ny = row2(ROW_N + 3 * l + 1), nz = row2(ROW_N + 3 * l + 2);
-            const float2 lx = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l) * FAST_TA);
-            const float2 ly = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 1) * FAST_TA);
-            const float2 lz = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 2) * FAST_TA);
-            const float2 lL = *reinterpret_cast<const float2 *>(tlo + (LO_L + l) * FAST_TA);
+            const float2 lx = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l) * LFA_TLW);
+            const float2 ly = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 1) * LFA_TLW);
+            const float2 lz = *reinterpret_cast<const float2 *>(tlo + (LO_N + 3 * l + 2) * LFA_TLW);
+            const float2 lL = *reinterpret_cast<const float2 *>(tlo + (LO_L + l) * LFA_TLW);
             const double y0 = lfa_link_value(an, nx.x, ny.x, nz.x, (double)lx.x, (double)ly.x, (double)lz.x, L.x,
                                              (double)lL.x, kscale, pref, ap0, cref, ac0);
             const double y1 = lfa_link_value(an, nx.y, ny.y, nz.y, (double)lx.y, (double)ly.y, (double)lz.y, L.y,
                                              (double)lL.y, kscale, pref, ap1, cref, ac1);
-            *reinterpret_cast<double2 *>(yout + l * ystride) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
+            *reinterpret_cast<double2 *>(ysm + l * FAST_TA + 2 * tid) = make_double2(in0 ? y0 : 0.0, in1 ? y1 : 0.0);
+        }
+    }
+    }   /* in0 || in1 */
+    if (LFA) {
+        /* time derivative of the tile's links (G15; gen 1.5: first, gen 2.0: second; zero outside its valid range), which is
+         * what the Michelson stage interpolates, Eq. (B25) / (B33): the TDI kernel stages it directly and has no stencil pass */
+        __syncthreads();
+        if (tid == 0 || tid == FAST_TA_THREADS - 1 || m0 >= p.n) return;   /* the rim pairs belong to the neighbouring tiles */
+        const bool g15 = p.gen == LTDI_GEN_15;
+        const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
+        const int64_t dlo = p.m1 + 2 * w + p.xw;
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            const double *v = ysm + l * FAST_TA + 2 * tid;   /* v[j] = link sample m0 + j */
+            double d[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                double x;
+                if (w == 1) x = g15 ? (v[j + 1] - v[j - 1]) : ((v[j + 1] - v[j]) - (v[j] - v[j - 1]));
+                else if (g15) x = 8.0 * (v[j + 1] - v[j - 1]) - (v[j + 2] - v[j - 2]);
+                else {
+                    const double d1 = (v[j + 1] - v[j]) - (v[j] - v[j - 1]);
+                    const double d2 = (v[j + 2] - v[j]) - (v[j] - v[j - 2]);
+                    x = 16.0 * d1 - d2;
+                }
+                const int64_t m = m0 + j;
+                d[j] = (m >= dlo && m < p.n - dlo) ? x * scale : 0.0;
+            }
+            *reinterpret_cast<double2 *>(p.yL + b * p.lds + l * ystride + m0) = make_double2(d[0], d[1]);
+            if (p.yLraw) *reinterpret_cast<double2 *>(p.yLraw + b * p.lds + l * ystride + m0) = make_double2(v[0], v[1]);
         }
     }
 }
@@ -675,10 +724,7 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_chirp_kernel(const __
     __shared__ double fr[LTDI_FRAME_STRIDE];
     __shared__ ChirpDev sw;
     if (p.use_small) {
-        if (tid == 0) {
-            const double *sr = p.small + 3 * (p.b0 + b);
-            source_frame_one(sr[0], sr[1], sr[2], fr);
-        }
+        if (tid < 11) fr[tid] = p.small_fr[11 * (p.b0 + b) + tid];
     } else if (tid < LTDI_FRAME_STRIDE) fr[tid] = p.frames[b * LTDI_FRAME_STRIDE + tid];
     if (tid >= 32 && tid < 32 + LTDI_CHIRP_STRIDE) reinterpret_cast<double *>(&sw)[tid - 32] = reinterpret_cast<const double *>(wav + b)[tid - 32];
     __syncthreads();
@@ -1033,10 +1079,10 @@ tdi_kernel(const __grid_constant__ FastParams p)
 
     /* shared memory (host: tdi_smem_bytes):
      *   sa   anchors [na][ANC]            (39 full, then 6 LFA; only the kinds this response has)
-     *   yF   [6][yr] full links           dL  [3][yr] derivative of the LFA links      (element 0 = sample y0, even)
+     *   yF   [6][yr] full links           dL  [3][yr] time derivative of the LFA links, as the link kernel stored it
+     *                                          (element 0 = sample y0, even)
      *   Lr   [NLR][FAST_TC] light times L_l(n0 + i) of the tile; after the term loop: X, Y, Z of the tile
      *        (full response with second-order weights: [6][yr], element 0 = sample y0 -- nested delays look back)
-     *   yL   [3][yr + 4] LFA links        (element 0 = sample y0 - 2)
      *   Xs   [3][FAST_TC] exchange        sa2  [na][M] second derivative of the weights (ORD2) */
     const int yr = tdi_yr<M>(FAST_TC, p.m2);
     const int64_t y0 = n0 - tdi_back(p.m2);
@@ -1048,13 +1094,12 @@ tdi_kernel(const __grid_constant__ FastParams p)
     const int LRW = LR_EXT ? yr : FAST_TC;                       /* elements per light-time row */
     const int lroff = LR_EXT ? tdi_back(p.m2) : 0;               /* element of sample n0 */
     double *Lr = dL + (has_lfa ? 3 * yr : 0);
-    double *yL = Lr + NLR * LRW;
-    const int slen = yr + 4;   /* staged LFA links: samples [y0 - 2, y0 + yr + 2), an even start for 16-byte rows */
+    double *Xs0 = Lr + NLR * LRW;
     /* X, Y, Z exchange: its own region (full, LFA: no barrier between the term loop and the exchange), or on top of
      * the light times (hybrid: six rows, and the shared memory of two responses) */
     constexpr bool xs_alias = WHICH == LTDI_RESPONSE_HYBRID;
-    double *Xs = xs_alias ? Lr : yL + (has_lfa ? 3 * slen : 0);
-    double *sa2 = yL + (has_lfa ? 3 * slen : 0) + (xs_alias ? 0 : 3 * FAST_TC);   /* behind everything else */
+    double *Xs = xs_alias ? Lr : Xs0;
+    double *sa2 = Xs0 + (xs_alias ? 0 : 3 * FAST_TC);   /* behind everything else */
     const double *sa_lfa = sa + (size_t)na_full * ANC;
     const double *sa2_lfa = sa2 + (size_t)na_full * M;
     const int lfa_a0 = p.gen == LTDI_GEN_15 ? 0 : FAST_NA_LFA_GEN;   /* first LFA anchor of this generation */
@@ -1070,8 +1115,7 @@ tdi_kernel(const __grid_constant__ FastParams p)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     const int64_t g0 = max(y0, (int64_t)0), g1 = min(y0 + yr, p.lds);                  /* full links, even bounds */
-    const int64_t h0 = max(y0 - 2, (int64_t)0), h1 = min(y0 - 2 + slen, p.lds);         /* LFA links */
-    const int nyF = (int)max(g1 - g0, (int64_t)0), nyL = (int)max(h1 - h0, (int64_t)0);
+    const int nyF = (int)max(g1 - g0, (int64_t)0), nyL = nyF;                             /* the LFA rows cover the same samples */
     const int64_t lr0 = n0 - lroff;                                                      /* first sample of a light-time row */
     const int64_t l0 = max(lr0, (int64_t)0), l1 = min(lr0 + LRW, p.stride);
     const int nl = (int)max(l1 - l0, (int64_t)0);
@@ -1085,10 +1129,10 @@ tdi_kernel(const __grid_constant__ FastParams p)
             const int c = k % yr;
             if (c < g0 - y0 || c >= g0 - y0 + nyF) yF[k] = 0.0;
         }
-    if (has_lfa && (y0 - 2 < 0 || nyL < slen))
-        for (int k = tid; k < 3 * slen; k += FAST_TC_THREADS) {
-            const int c = k % slen;
-            if (c < h0 - (y0 - 2) || c >= h0 - (y0 - 2) + nyL) yL[k] = 0.0;
+    if (has_lfa && (y0 < 0 || nyL < yr))
+        for (int k = tid; k < 3 * yr; k += FAST_TC_THREADS) {
+            const int c = k % yr;
+            if (c < g0 - y0 || c >= g0 - y0 + nyL) dL[k] = 0.0;
         }
     __syncthreads();   /* the barrier is initialised, the zero fill is visible */
     if (tid == 0) {
@@ -1113,63 +1157,12 @@ tdi_kernel(const __grid_constant__ FastParams p)
         if (has_lfa) {
 #pragma unroll 1
             for (int l = 0; l < 3; ++l)
-                if (nyL > 0) bulk_g2s(yL + l * slen + (h0 - (y0 - 2)), p.yL + b * p.lds + l * ystride + h0, nyL * 8u, &s_bar);
+                if (nyL > 0) bulk_g2s(dL + l * yr + (g0 - y0), p.yL + b * p.lds + l * ystride + g0, nyL * 8u, &s_bar);
             bulk_g2s(sa + (size_t)na_full * ANC, ga + (FAST_NA_FULL + lfa_a0) * ANC, FAST_NA_LFA_GEN * ANC * 8u, &s_bar);   /* this generation's six */
         }
         bulk_g2s(s_hdr, p.anc_hdr + atile * (FAST_NA * 4), FAST_NA * 4 * 8u, &s_bar);
     }
     mbar_wait(&s_bar, 0);
-
-    /* phase 1 (LFA, hybrid): derivative of the LFA links */
-    if (has_lfa) {
-        /* FD1 (gen 1.5) or FD2 (gen 2.0) of the LFA links, G15; zero outside the valid range.  A thread takes runs of
-         * eight consecutive samples of one link and slides a register window over them; tiles away from the ends of
-         * the series (all but two per source) take the branch without per-sample range checks. */
-        constexpr int FD_RUN = 8;
-        const int runs = (yr + FD_RUN - 1) / FD_RUN;
-        const bool g15 = p.gen == LTDI_GEN_15;
-        const double scale = g15 ? p.inv_fd1 : p.inv_fd2;
-        const int64_t dlo = p.m1 + 2 * w + p.xw;   /* first sample with a valid derivative of the LFA links */
-        const bool interior = y0 >= dlo && y0 + yr <= p.n - dlo;
-#pragma unroll 1
-        for (int idx = tid; idx < 3 * runs; idx += FAST_TC_THREADS) {   /* (link, run) pairs, evenly over the threads */
-            const int l = idx / runs, k0 = (idx - l * runs) * FD_RUN;
-            const double *x = yL + l * slen + k0;   /* x[j] = sample y0 - 2 + k0 + j */
-            double *o = dL + l * yr + k0;
-            double v[FD_RUN + 4];
-            const bool whole = interior && k0 + FD_RUN <= yr;
-            if (whole) {
-#pragma unroll
-                for (int j = 0; j < FD_RUN + 4; ++j) v[j] = x[j];
-            } else {
-#pragma unroll
-                for (int j = 0; j < FD_RUN + 4; ++j) v[j] = (k0 + j < slen) ? x[j] : 0.0;
-            }
-#pragma unroll
-            for (int j = 0; j < FD_RUN; ++j) {
-                double d;   /* centre v[j + 2] */
-                if (w == 1) d = g15 ? (v[j + 3] - v[j + 1]) : ((v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]));
-                else if (g15) d = 8.0 * (v[j + 3] - v[j + 1]) - (v[j + 4] - v[j]);
-                else {
-                    const double d1 = (v[j + 3] - v[j + 2]) - (v[j + 2] - v[j + 1]);
-                    const double d2 = (v[j + 4] - v[j + 2]) - (v[j + 2] - v[j]);
-                    d = 16.0 * d1 - d2;
-                }
-                v[j] = d * scale;   /* v[j] is not read again */
-            }
-            if (whole) {
-#pragma unroll
-                for (int j = 0; j < FD_RUN; ++j) o[j] = v[j];
-            } else {
-#pragma unroll
-                for (int j = 0; j < FD_RUN; ++j) {
-                    const int64_t m = y0 + k0 + j;
-                    if (k0 + j < yr) o[j] = (m >= dlo && m < p.n - dlo) ? v[j] : 0.0;
-                }
-            }
-        }
-        __syncthreads();
-    }
 
     const int ch = tid / FAST_TC_G, g = tid % FAST_TC_G;
     const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
@@ -1360,7 +1353,7 @@ tdi_kernel(const __grid_constant__ FastParams p)
         if (p.Y) {
             /* optional link output: the LFA links come back from the scratch series (their shared copy is gone) */
             const int iy = (int)(n - y0);
-            const double *gl = p.yL + b * p.lds + n;
+            const double *gl = p.yLraw + b * p.lds + n;   /* the LFA links themselves (written because d_y was asked for) */
 #pragma unroll 1
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
@@ -1392,7 +1385,6 @@ static inline size_t tdi_smem_bytes(int which, int64_t m2, int64_t w, bool ord2)
     size_t dbl = na * FAST_ANC_DOUBLES(M);
     dbl += (has_full ? 6 * yr : 0) + (has_lfa ? 3 * yr : 0);
     dbl += (size_t)(has_full ? 6 : 3) * ((ord2 && which == LTDI_RESPONSE_FULL) ? yr : (size_t)tdi_tc(which));
-    dbl += has_lfa ? 3 * (yr + 4) : 0;
     dbl += which == LTDI_RESPONSE_HYBRID ? 0 : (size_t)3 * tdi_tc(which);   /* X, Y, Z exchange */
     dbl += ord2 ? na * M : 0;                                                /* second derivative of the weights */
     return dbl * sizeof(double);

@@ -244,6 +244,7 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
     o->d_anc = nullptr;
     o->anc_gen = 0;
     o->anc_M = 0;
+    o->anc_has2 = false;
     *out = o;
     return LTDI_OK;
 }
@@ -260,7 +261,7 @@ bool fast_order(int order) { return order == 9 || order == 31; }
  * 126 MB L2 (96 MB: 5 % slower at cfg4s) -- the scratch traffic, 96 B per sample, is < 5 % of the HBM bandwidth at the
  * speed of these FP64-bound kernels. */
 struct FastLayout {
-    int64_t ntilesA, ntilesC, ntilesN, lds, chunk;   /* link tiles, TDI tiles, anchor tiles (= 448-sample blocks) */
+    int64_t ntilesA, ntilesAL, ntilesC, ntilesN, lds, chunk;   /* link tiles (full, LFA), TDI tiles, anchor tiles (= 448-sample blocks) */
     size_t anc, hdr, anc2, y, lists;     /* doubles */
     size_t total;                  /* doubles, including work_doubles(batch) */
 };
@@ -268,10 +269,13 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
 {
     FastLayout f;
     f.ntilesA = (n + FAST_TA - 1) / FAST_TA;
+    f.ntilesAL = (n + FAST_TAL - 1) / FAST_TAL;
     f.ntilesC = (n + tdi_tc(which) - 1) / tdi_tc(which);
     f.ntilesN = (n + FAST_TCA - 1) / FAST_TCA;
     f.lds = (n + 15) / 16 * 16;
-    const int rows = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 3 : 9;
+    /* rows of link scratch per source: six full links, three derivatives of the LFA links + the three LFA links themselves
+     * (written only when the caller asks for d_y) */
+    const int rows = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 6 : 12;
     const size_t cap = (size_t)2048 << 20; /* bytes of scratch per chunk */
     int64_t chunk = (int64_t)(cap / ((size_t)rows * f.lds * sizeof(double)));
     f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
@@ -280,7 +284,7 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
     f.anc2 = (size_t)f.ntilesN * FAST_NA * M;   /* second derivative of the weights (second-order instances) */
     f.y = (size_t)rows * f.chunk * f.lds;
     /* hybrid: link tiles of both kinds, LFA-only blocks, blend blocks, full-only 224-sample tiles (int2 each) */
-    f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)f.chunk * (2 * f.ntilesA + 4 * f.ntilesN) : 0;
+    f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)f.chunk * (f.ntilesA + f.ntilesAL + 4 * f.ntilesN) : 0;
     f.total = work_doubles(batch) + f.anc + f.hdr + f.anc2 + f.y + f.lists;
     return f;
 }
@@ -300,7 +304,7 @@ __host__ __device__ inline HybCounts hyb_counts(const HybGeom &g, int nLt, int f
     /* LFA links: read by the TDI stage of blocks [0, fFt), up to `fwd` samples past their end */
     int64_t endL = fFt == 0 ? 0 : (int64_t)fFt * FAST_TCA + g.fwd;
     if (endL > g.n) endL = g.n;
-    c.lfa_link = (endL + FAST_TA - 1) / FAST_TA;
+    c.lfa_link = (endL + FAST_TAL - 1) / FAST_TAL;   /* LFA link tiles store the derivative of FAST_TAL samples */
     /* full links: read by the TDI stage of blocks [nLt, nblk), from `back` samples before their start */
     int64_t first = (int64_t)nLt * FAST_TCA - g.back;
     if (first < 0) first = 0;
@@ -527,7 +531,18 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     p.inv_fd2 = 1.0 / ((mg.w == 1 ? 1.0 : 12.0) * rp.dt * rp.dt);
     p.lds = lay.lds; p.batch_all = rp.batch; p.ntilesA = lay.ntilesA; p.ntilesC = lay.ntilesC;
     p.use_small = small != nullptr;
-    if (small) std::memcpy(p.small, small, sizeof p.small);
+    if (small) {
+        std::memcpy(p.small, small, sizeof p.small);
+        for (int64_t b = 0; b < rp.batch && b < 32; ++b) {   /* S1 on the host, Eq. (2.1) with G1 and (2.3), in long double */
+            const long double be = small[3 * b], la = small[3 * b + 1], ps = small[3 * b + 2];
+            const long double sb = sinl(be), cb = cosl(be), sl = sinl(la), cl = cosl(la);
+            double *f = p.small_fr + 11 * b;
+            f[0] = (double)(-cb * cl); f[1] = (double)(-cb * sl); f[2] = (double)(-sb);   /* k = -e_r */
+            f[3] = (double)sl;         f[4] = (double)(-cl);      f[5] = 0.0;             /* u = -e_phi */
+            f[6] = (double)(-sb * cl); f[7] = (double)(-sb * sl); f[8] = (double)cb;      /* v = -e_theta */
+            f[9] = (double)cosl(2.0L * ps); f[10] = (double)sinl(2.0L * ps);
+        }
+    }
     double *anc = work, *hdr = anc + lay.anc, *anc2 = hdr + lay.hdr, *ys = anc2 + lay.anc2;
     int2 *lists = reinterpret_cast<int2 *>(ys + lay.y);
     p.anc = anc; p.anc_hdr = hdr;
@@ -542,8 +557,8 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     const size_t smem_strain = (size_t)4 * ((FAST_TA + 2 * mg.m1 + 4) / 2) * sizeof(double);
     const size_t smem_link = smem_strain + (size_t)LTDI_TABLE_ROWS * FAST_TA * sizeof(double);
     const size_t smem_link_lfa = smem_strain + (size_t)(ROW_L + 3) * FAST_TA * sizeof(double) +
-                                 (size_t)2 * (2 * ((FAST_TA + 2 * mg.m1 + 4) / 2) + 2 * LFA_RAW_HALO) * sizeof(double) + /* + raw strain */
-                                 (size_t)LFA_LO_ROWS * FAST_TA * sizeof(float) +                           /* + low parts */
+                                 (size_t)lfa_raw_doubles((int)((FAST_TA + 2 * mg.m1 + 4) / 2)) * sizeof(double) +          /* + raw strain */
+                                 (size_t)LFA_LO_ROWS * LFA_TLW * sizeof(float) +                          /* + low parts */
                                  (rp.lfa_terms >= 2 ? smem_strain : 0);                                     /* + d^3h/dt^3 numerators */
     const size_t smem_link_hyb = std::max(smem_link, smem_link_lfa);
     const size_t smem_tdi_full = tdi_smem_bytes<M>(LTDI_RESPONSE_FULL, mg.m2, mg.w, ord2);
@@ -560,7 +575,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
     if (full && (rc = set_smem_tdi<M, LTDI_RESPONSE_FULL>(ds, ord2, smem_tdi_full))) return rc;
     if (lfa && (rc = set_smem_tdi<M, LTDI_RESPONSE_LFA>(ds, ord2, smem_tdi_lfa))) return rc;
 
-    if (orb->d_anc && orb->anc_M == M) {
+    if (orb->d_anc && orb->anc_M == M && (!ord2 || orb->anc_has2)) {
         /* ltdi_orbits_prepare() has computed the anchors of this order for the time grid (they serve both generations) */
         p.anc = orb->d_anc;
         p.anc_hdr = orb->d_anc + lay.anc;
@@ -586,8 +601,9 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
         p.A = rp.A + b0 * rp.ld; p.E = rp.E + b0 * rp.ld; p.T = rp.T + b0 * rp.ld;
         p.XYZ = rp.XYZ; p.Y = rp.Y;
         p.yF = ys; p.yL = ys + (full ? (size_t)6 * nb * lay.lds : 0);
+        p.yLraw = (lfa && rp.Y) ? p.yL + (size_t)3 * nb * lay.lds : nullptr;
         p.work = nullptr; p.nwork = 0; p.nwork_full = 0;
-        if (lay.ntilesA * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
+        if (lay.ntilesAL * nb >= ((int64_t)1 << 31) || lay.ntilesC * nb >= ((int64_t)1 << 31)) return LTDI_EUNSUPPORTED;
         if (!hybrid) {
             if (full) {
                 {
@@ -601,7 +617,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
             } else {
                 {
                     ProfScope ps(LTDI_KERNEL_LINK_LFA + LTDI_KERNEL_COUNT * which, st);
-                    link_kernel<H, true><<<(unsigned)(lay.ntilesA * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
+                    link_kernel<H, true><<<(unsigned)(lay.ntilesAL * nb), FAST_TA_THREADS, smem_link_lfa, st>>>(p);
                 }
                 count_launch();
                 p.nwork = lay.ntilesN * nb;
@@ -615,7 +631,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
 
         /* hybrid: compact lists, then one launch per class of tiles */
         const ChunkTotals &ct = hh->chunk[(size_t)ichunk];
-        int2 *l_link = lists, *l_lfa = l_link + (size_t)nb * 2 * lay.ntilesA, *l_blend = l_lfa + (size_t)nb * lay.ntilesN,
+        int2 *l_link = lists, *l_lfa = l_link + (size_t)nb * (lay.ntilesA + lay.ntilesAL), *l_blend = l_lfa + (size_t)nb * lay.ntilesN,
              *l_full = l_blend + (size_t)nb * lay.ntilesN;
         {
             PlanArgs a;
@@ -977,12 +993,16 @@ int ltdi_orbits_prepare(ltdi_orbits *orb, int gen, int lagrange_order, void *d_b
     p.gen = gen; p.m1 = m20.m1; p.m2 = m20.m2; p.m2_15 = m15.m2; p.m2_20 = m20.m2;
     const int64_t tiles = (d.n + FAST_TCA - 1) / FAST_TCA;
     double *anc = (double *)d_buf, *hdr = anc + (size_t)tiles * FAST_NA * FAST_ANC_DOUBLES(M);
-    double *anc2 = hdr + (size_t)tiles * FAST_NA * 4;   /* w'': the prepared anchors serve the second-order instances too */
+    /* w'' for the orbit objects whose responses run on the second-order instances (caller's tables, numerical orbit files);
+     * a nested call on an analytic orbit builds its own anchors */
+    const bool has2 = d.mode == LTDI_ORBIT_TABLES || d.mode == LTDI_ORBIT_KNOTS;
+    double *anc2 = has2 ? hdr + (size_t)tiles * FAST_NA * 4 : nullptr;
     {
         ProfScope ps(LTDI_KERNEL_ANCHOR, (cudaStream_t)stream);
         if (M == 32) anchor_kernel<32><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr, anc2);
         else anchor_kernel<10><<<(unsigned)tiles, 64, 0, (cudaStream_t)stream>>>(p, anc, hdr, anc2);
     }
+    orb->anc_has2 = has2;
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
     orb->d_anc = anc;
