@@ -262,8 +262,10 @@ typedef struct {
 /* d_psd [2][nf] (device): row 0 = S_n^{A,E}(f_k), row 1 = S_n^T(f_k), f_k = k df; entry k = 0 is +inf. */
 int ltdi_noise_psd(const ltdi_noise_desc *desc, double df, int64_t nf, double *d_psd, void *stream);
 
-/* Plan for series of n samples (row stride ld, batch sources): creates the cuFFT plans (host objects; their
- * device work area is part of the caller's d_work) and returns the bytes of d_work ltdi_overlap_products needs. */
+/* Plan for series of n samples (2 <= n <= 2^27, row stride ld, batch sources): a host object with the lengths and the
+ * chunking of the library's own Fourier transform (csrc/fft.cuh: Stockham passes for powers of two, Bluestein's chirp-z
+ * for every other n); its device work area is part of the caller's d_work.  Returns the bytes of d_work that
+ * ltdi_overlap_products needs. */
 typedef struct ltdi_overlap ltdi_overlap;
 int ltdi_overlap_create(int64_t n, int64_t ld, int64_t batch, ltdi_overlap **out, size_t *work_bytes);
 int ltdi_overlap_destroy(ltdi_overlap *ovl);

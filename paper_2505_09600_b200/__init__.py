@@ -492,7 +492,7 @@ class NoiseDesc(C.Structure):
 
 class Overlap:
     """FFT of A, E, T -> noise-weighted inner products, overlap, mismatch, SNR (Eqs. 5.1, 5.2, 6.1)
-    of two responses of the same sources.  Owns the cuFFT plan handle and its device scratch."""
+    of two responses of the same sources.  Owns the transform plan (lengths, chunking) and its device scratch; the Fourier transform is the library's own (csrc/fft.cuh)."""
 
     def __init__(self, n, ld, batch, device="cuda:0"):
         self.n, self.ld, self.batch, self.device = int(n), int(ld), int(batch), torch.device(device)

@@ -13,11 +13,11 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "liblisatdi.so")
 SOURCES = [os.path.join(CSRC, "lisatdi.cu"), os.path.join(CSRC, "overlap.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("common.cuh", "dd.cuh", "orbit.cuh", "response.cuh", "fast.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("common.cuh", "dd.cuh", "orbit.cuh", "response.cuh", "fast.cuh", "chirp.cuh", "fft.cuh")] + [
     os.path.join(INCLUDE, "lisatdi.h"), os.path.join(INCLUDE, "lisatdi_bench.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-I", INCLUDE, "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+         "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-I", INCLUDE]
 
 
 def build(force=False, verbose=False):

@@ -3,12 +3,13 @@
 // noise-weighted inner product, overlap, mismatch and SNR of Eqs. (5.1), (5.2), (6.1).
 //
 //   noise_psd_kernel   S_n^{A,E}(f_k), S_n^T(f_k) on f_k = k df                      (ALU, tiny)
-//   cuFFT D2Z          x~_k = sum_n x_n exp(-2 pi i k n / N): a plain library transform, batched over sources
-//   products_kernel    per (source, channel, block of bins): partial sums of |a~|^2 / S, |b~|^2 / S, Re(a~* b~) / S
-//                      over the band f_min <= f_k <= f_max                           (HBM-bound: 32 B read per bin)
+//   fft.cuh            x~_k = sum_n x_n exp(-2 pi i k n / N), hand-written: Stockham radix-16 passes for powers of two,
+//                      Bluestein's chirp-z on top of them for every other length; the A (E, T) series of the two
+//                      responses ride in ONE complex transform, z = a + i b                  (HBM-bound passes)
+//   products_kernel    per (source, channel, block of bins): a~_k, b~_k from Z_k and Z_{n-k}, partial sums of
+//                      |a~|^2 / S, |b~|^2 / S, Re(a~* b~) / S over the band f_min <= f_k <= f_max   (HBM-bound: 32 B per bin)
 //   finalize_kernel    fixed-order sum of the partials (deterministic), 4 df dt^2 scaling, overlap, mismatch, SNR
 #include <cuda_runtime.h>
-#include <cufft.h>
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -18,6 +19,7 @@
 #include <new>
 
 #include "../../include/lisatdi.h"
+#include "fft.cuh"
 
 #define OVL_CUDA_OK(expr)                                                                                 \
     do {                                                                                                  \
@@ -28,24 +30,15 @@
             return LTDI_ECUDA;                                                                            \
         }                                                                                                 \
     } while (0)
-#define OVL_FFT_OK(expr)                                                                                  \
-    do {                                                                                                  \
-        const cufftResult r_ = (expr);                                                                    \
-        if (r_ != CUFFT_SUCCESS) {                                                                        \
-            if (getenv("LTDI_DEBUG")) fprintf(stderr, "lisatdi %s:%d: cuFFT error %d\n", __FILE__, __LINE__, (int)r_); \
-            return LTDI_ECUDA;                                                                            \
-        }                                                                                                 \
-    } while (0)
-
 #define OVL_THREADS 256
 #define OVL_BINS_PER_THREAD 8
 #define OVL_BINS_PER_BLOCK (OVL_THREADS * OVL_BINS_PER_THREAD)
 
 struct ltdi_overlap {
-    cufftHandle plan, plan_tail;
-    bool has_tail;
-    int64_t n, ld, batch, chunk, tail, nf, nblk;
-    size_t fft_work, spec_bytes, part_bytes, total;
+    int64_t n, ld, batch, chunk, nf, nblk;
+    int64_t m;            /* transform length: n if it is a power of two, else the Bluestein length 2^p >= 2 n - 1 */
+    bool pow2;
+    size_t table_bytes, buf_bytes, part_bytes, total;   /* chirp tables | two ping-pong buffers [3 chunk][m] | partials */
 };
 
 namespace {
@@ -87,16 +80,15 @@ __global__ void noise_psd_kernel(ltdi_noise_desc d, double df, int64_t nf, doubl
     psd[nf + k] = 16.0 * lam * sx * sx * ((1.0 - cx) * s_op + 8.0 * (shx * shx) * (shx * shx) * s_pm) + lam * gal; /* (2.13b) */
 }
 
-// spec: [6][chunk][nf] complex (a: A, E, T, then b: A, E, T); part: [chunk][3][nblk][3]
-__global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__restrict__ spec,
-                                                               const double *__restrict__ psd, int64_t nf, int64_t chunk,
+// zb: [chunk][3][m] complex: the transform (Bluestein: before the final chirp C_k) of z = a_c + i b_c; part: [chunk][3][nblk][3]
+__global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__restrict__ zb, const double2 *__restrict__ C,
+                                                               const double *__restrict__ psd, int64_t n, int64_t m, int64_t nf,
                                                                int64_t nsrc, double df, double fmin, double fmax,
                                                                int64_t nblk, double *__restrict__ part)
 {
     const int c = blockIdx.y;
     const int64_t s = blockIdx.z;
-    const double2 *a = spec + ((int64_t)c * chunk + s) * nf;
-    const double2 *b = spec + ((int64_t)(3 + c) * chunk + s) * nf;
+    const double2 *z = zb + (s * 3 + c) * m;
     const double *sn = psd + (c == 2 ? nf : 0);
     double aa = 0.0, bb = 0.0, ab = 0.0;
     const int64_t k0 = (int64_t)blockIdx.x * OVL_BINS_PER_BLOCK + threadIdx.x;
@@ -106,7 +98,11 @@ __global__ void __launch_bounds__(OVL_THREADS) products_kernel(const double2 *__
         if (k > 0 && k < nf) {
             const double f = (double)k * df;
             if (f >= fmin && f <= fmax) {                      /* (5.1): rectangle rule over the bins of the band */
-                const double2 u = a[k], v = b[k];
+                double2 zk = z[k], zn = z[n - k];
+                if (C) { zk = cmul(zk, C[k]); zn = cmul(zn, C[n - k]); }
+                /* a~ = (Z_k + conj Z_{n-k}) / 2, b~ = (Z_k - conj Z_{n-k}) / (2 i) */
+                const double2 u = make_double2(0.5 * (zk.x + zn.x), 0.5 * (zk.y - zn.y));
+                const double2 v = make_double2(0.5 * (zk.y + zn.y), -0.5 * (zk.x - zn.x));
                 const double inv = 1.0 / sn[k];
                 aa += (u.x * u.x + u.y * u.y) * inv;
                 bb += (v.x * v.x + v.y * v.y) * inv;
@@ -170,15 +166,6 @@ __global__ void __launch_bounds__(96) finalize_kernel(const double *__restrict__
 
 size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 
-int make_plan(cufftHandle *plan, int64_t n, int64_t ld, int64_t nf, int64_t batch, size_t *work)
-{
-    OVL_FFT_OK(cufftCreate(plan));
-    OVL_FFT_OK(cufftSetAutoAllocation(*plan, 0));
-    long long len = n, inembed = ld, onembed = nf;
-    OVL_FFT_OK(cufftMakePlanMany64(*plan, 1, &len, &inembed, 1, ld, &onembed, 1, nf, CUFFT_D2Z, batch, work));
-    return LTDI_OK;
-}
-
 } // namespace
 
 extern "C" {
@@ -194,24 +181,21 @@ int ltdi_noise_psd(const ltdi_noise_desc *desc, double df, int64_t nf, double *d
 
 int ltdi_overlap_create(int64_t n, int64_t ld, int64_t batch, ltdi_overlap **out, size_t *work_bytes)
 {
-    if (n < 2 || ld < n || batch < 1 || !out || !work_bytes) return LTDI_EINVAL;
+    if (n < 2 || n > ((int64_t)1 << 27) || ld < n || batch < 1 || !out || !work_bytes) return LTDI_EINVAL;
     ltdi_overlap *o = new (std::nothrow) ltdi_overlap;
     if (!o) return LTDI_EINVAL;
     o->n = n; o->ld = ld; o->batch = batch; o->nf = n / 2 + 1;
-    /* sources per pass: the six spectra of a pass stay below 1 GiB */
-    const size_t per_source = (size_t)6 * o->nf * sizeof(double2);
-    o->chunk = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(batch, 32768), (int64_t)(((size_t)1 << 30) / per_source)));
-    o->tail = batch % o->chunk;
-    o->has_tail = o->tail != 0;
+    o->pow2 = (n & (n - 1)) == 0;
+    o->m = n;
+    if (!o->pow2) { o->m = 1; while (o->m < 2 * n - 1) o->m <<= 1; }
+    /* sources per pass: the two ping-pong buffers of a pass stay below 1 GiB (one source at least) */
+    const size_t per_source = (size_t)2 * 3 * o->m * sizeof(double2);
+    o->chunk = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(batch, 21845), (int64_t)(((size_t)1 << 30) / per_source)));
     o->nblk = (o->nf + OVL_BINS_PER_BLOCK - 1) / OVL_BINS_PER_BLOCK;
-    size_t w0 = 0, w1 = 0;
-    int rc = make_plan(&o->plan, n, ld, o->nf, o->chunk, &w0);
-    if (rc == LTDI_OK && o->has_tail) rc = make_plan(&o->plan_tail, n, ld, o->nf, o->tail, &w1);
-    if (rc != LTDI_OK) { delete o; return rc; }
-    o->fft_work = align256(std::max(w0, w1));
-    o->spec_bytes = align256(per_source * o->chunk);
+    o->table_bytes = o->pow2 ? 0 : align256((size_t)(n + 2 * o->m) * sizeof(double2));   /* C | two buffers for the chirp's transform */
+    o->buf_bytes = align256((size_t)3 * o->chunk * o->m * sizeof(double2));
     o->part_bytes = align256((size_t)o->chunk * 3 * o->nblk * 3 * sizeof(double));
-    o->total = o->fft_work + o->spec_bytes + o->part_bytes;
+    o->total = o->table_bytes + 2 * o->buf_bytes + o->part_bytes;
     *work_bytes = o->total;
     *out = o;
     return LTDI_OK;
@@ -228,21 +212,36 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
     if (work_bytes < o->total) return LTDI_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     char *base = (char *)d_work;
-    double2 *spec = (double2 *)(base + o->fft_work);
-    double *part = (double *)(base + o->fft_work + o->spec_bytes);
-    const double *in[6] = {d_aA, d_aE, d_aT, d_bA, d_bE, d_bT};
-    const double df = 1.0 / ((double)o->n * dt);
-    const double scale = 4.0 * df * dt * dt;          /* x~ = dt * DFT(x), (5.1) rectangle rule */
+    double2 *C = o->pow2 ? nullptr : (double2 *)base;
+    double2 *buf0 = (double2 *)(base + o->table_bytes), *buf1 = (double2 *)(base + o->table_bytes + o->buf_bytes);
+    double *part = (double *)(base + o->table_bytes + 2 * o->buf_bytes);
+    const int64_t n = o->n, m = o->m;
+    const double df = 1.0 / ((double)n * dt);
+    /* x~ = dt * DFT(x), (5.1) rectangle rule; the Bluestein convolution carries 1 / m from its unnormalised inverse */
+    const double scale = 4.0 * df * dt * dt * (o->pow2 ? 1.0 : 1.0 / ((double)m * (double)m));
+    const double2 *bhat = nullptr;
+    if (!o->pow2) { /* chirp tables of this length (rebuilt per call: the work area is the caller's between calls) */
+        double2 *t0 = C + n, *t1 = t0 + m;
+        bluestein_tables_kernel<<<(unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), FFT_THREADS, 0, st>>>(n, m, C, t0);
+        bhat = fft_pow2<-1>(t0, t1, m, m, 1, st, nullptr) ? t1 : t0;
+        OVL_CUDA_OK(cudaGetLastError());
+    }
     for (int64_t b0 = 0; b0 < o->batch; b0 += o->chunk) {
         const int64_t nb = std::min(o->chunk, o->batch - b0);
-        cufftHandle plan = nb == o->chunk ? o->plan : o->plan_tail;
-        OVL_FFT_OK(cufftSetStream(plan, st));
-        OVL_FFT_OK(cufftSetWorkArea(plan, base));
-        for (int s = 0; s < 6; ++s) /* step iv */
-            OVL_FFT_OK(cufftExecD2Z(plan, (cufftDoubleReal *)(in[s] + b0 * o->ld),
-                                    (cufftDoubleComplex *)(spec + (int64_t)s * nb * o->nf)));
+        const int64_t nser = 3 * nb;
+        const int64_t off = b0 * o->ld;
+        /* step iv: z = a_c + i b_c (times the chirp), transformed */
+        fft_pack_kernel<<<dim3((unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nser), FFT_THREADS, 0, st>>>(
+            d_aA + off, d_aE + off, d_aT + off, d_bA + off, d_bE + off, d_bT + off, o->ld, n, m, C, buf0);
+        int cur = fft_pow2<-1>(buf0, buf1, m, m, nser, st, nullptr);
+        if (!o->pow2) {
+            double2 *x = cur ? buf1 : buf0, *y = cur ? buf0 : buf1;
+            fft_pointwise_kernel<<<dim3((unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nser), FFT_THREADS, 0, st>>>(x, bhat, m);
+            cur = fft_pow2<+1>(x, y, m, m, nser, st, nullptr) ? !cur : cur;
+        }
+        const double2 *zb = cur ? buf1 : buf0;
         const dim3 grid((unsigned)o->nblk, 3, (unsigned)nb);
-        products_kernel<<<grid, OVL_THREADS, 0, st>>>(spec, d_psd, o->nf, nb, nb, df, fmin, fmax, o->nblk, part);
+        products_kernel<<<grid, OVL_THREADS, 0, st>>>(zb, C, d_psd, n, m, o->nf, nb, df, fmin, fmax, o->nblk, part);
         OVL_CUDA_OK(cudaGetLastError());
         finalize_kernel<<<(unsigned)nb, 96, 0, st>>>(part, nb, o->nblk, scale, d_out + b0 * 15,
                                                                       d_snr ? d_snr + 3 * b0 : nullptr);
@@ -254,8 +253,6 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
 int ltdi_overlap_destroy(ltdi_overlap *o)
 {
     if (!o) return LTDI_OK;
-    cufftDestroy(o->plan);
-    if (o->has_tail) cufftDestroy(o->plan_tail);
     delete o;
     return LTDI_OK;
 }

@@ -1,4 +1,4 @@
-"""GPU parity of the first "next" row: noise PSD kernel, cuFFT + inner-product kernels against
+"""GPU parity of the first "next" row: noise PSD kernel, the hand-written FFT (Stockham / Bluestein) + inner-product kernels against
 the numpy oracle (oracle/overlap_oracle.py) on the same inputs.
 
 Tolerances: PSD 1e-12 relative away from its zeros (libm differences of a few ulp, amplified by
