@@ -705,8 +705,11 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
     }
 }
 
+#ifndef LINK_MINB
+#define LINK_MINB 3
+#endif
 template <int H, bool LFA>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_kernel(const __grid_constant__ FastParams p)
+__global__ void __launch_bounds__(FAST_TA_THREADS, LINK_MINB) link_kernel(const __grid_constant__ FastParams p)
 {
     link_body<H, LFA>(p, blockIdx.x);
 }
@@ -784,7 +787,7 @@ __global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_chirp_kernel(const __
 // hybrid: both kinds of link tiles in ONE launch -- the few full-link tiles (first in the grid: they are the heavy
 // ones) run beside the LFA-link tiles instead of as a launch of their own that leaves most SMs idle
 template <int H>
-__global__ void __launch_bounds__(FAST_TA_THREADS, 3) link_hybrid_kernel(const __grid_constant__ FastParams p)
+__global__ void __launch_bounds__(FAST_TA_THREADS, LINK_MINB) link_hybrid_kernel(const __grid_constant__ FastParams p)
 {
     if ((int64_t)blockIdx.x < p.nwork_full) link_body<H, false>(p, blockIdx.x);
     else link_body<H, true>(p, blockIdx.x);
