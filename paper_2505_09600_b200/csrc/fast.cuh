@@ -436,22 +436,21 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
      * table stride; what lies beyond (a tail tile) is only read by samples >= n, whose outputs are never stored. */
     constexpr int NROWS = LFA ? ROW_L + 3 : LTDI_TABLE_ROWS;
     double *tb = ho_c + hw2;
-    __shared__ uint64_t s_bar;
+    __shared__ uint64_t s_bar, s_bar2;   /* s_bar2 (LFA): the table rows, which the stencil pass does not need */
     const int64_t tl0 = max(a0, (int64_t)0), tl1 = min(a0 + FAST_TA, p.stride);       /* table samples of the tile */
     const unsigned nl = (unsigned)max(tl1 - tl0, (int64_t)0);                          /* even */
     const int toff = (int)(tl0 - a0);                                                  /* 0, or 2 in the first LFA tile */
     float *tl = nullptr;   /* LFA: low parts of the dd table entries of the tile */
     double *he3_p = nullptr; /* LFA, terms = 2: [4][hw2] third-derivative numerators (even +, odd +, even x, odd x) */
     if (!LFA) {
-        if (tid < 32) {
-            if (tid == 0) {
-                mbar_init(&s_bar, 1);
-                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-                mbar_expect_tx(&s_bar, NROWS * nl * 8u);
-            }
-            __syncwarp();
-            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA + toff, p.tab + (int64_t)tid * p.stride + tl0, nl * 8u, &s_bar);
+        if (tid == 0) {
+            mbar_init(&s_bar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            mbar_expect_tx(&s_bar, NROWS * nl * 8u);
         }
+        __syncthreads();   /* the barrier is initialised: every fourth thread issues one row (all four warps issue) */
+        if ((tid & 3) == 0 && (tid >> 2) < NROWS)
+            bulk_g2s(tb + (tid >> 2) * FAST_TA + toff, p.tab + (int64_t)(tid >> 2) * p.stride + tl0, nl * 8u, &s_bar);
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
             double *dp = ((i & 1) ? ho_p : he_p) + (i >> 1), *dc = ((i & 1) ? ho_c : he_c) + (i >> 1);
@@ -480,21 +479,25 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         const unsigned nf = (unsigned)max(f1 - f0, (int64_t)0);
         const bool bulk = ncopy > 0 && !(ncopy & 1) &&
                           !((reinterpret_cast<uintptr_t>(gp + g_lo) | reinterpret_cast<uintptr_t>(gc + g_lo)) & 15);
-        if (tid < 32) {
-            if (tid == 0) {
-                mbar_init(&s_bar, 1);
-                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-                mbar_expect_tx(&s_bar, NROWS * nl * 8u + LFA_LO_ROWS * nf * 4u + (bulk ? 2u * ncopy * 8u : 0u));
-            }
-            __syncwarp();
-            if (tid < NROWS) bulk_g2s(tb + tid * FAST_TA + toff, p.tab + (int64_t)tid * p.stride + tl0, nl * 8u, &s_bar);
-            if (tid < LFA_LO_ROWS) {   /* float rows from sample a0 - 2 (a multiple of 4) on: see LFA_TLW */
+        if (tid == 0) {
+            mbar_init(&s_bar, 1);
+            mbar_init(&s_bar2, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            mbar_expect_tx(&s_bar, bulk ? 2u * ncopy * 8u : 0u);
+            mbar_expect_tx(&s_bar2, NROWS * nl * 8u + LFA_LO_ROWS * nf * 4u);
+        }
+        __syncthreads();   /* the barriers are initialised */
+        if (tid % 3 == 0) {   /* 35 copies, one per issuing thread, spread over the four warps; the raw strain first */
+            const int id = tid / 3;
+            if (id < 2) {
+                if (bulk) bulk_g2s((id == 0 ? raw_p : raw_c) + (g_lo - rs), (id == 0 ? gp : gc) + g_lo, ncopy * 8u, &s_bar);
+            } else if (id < 2 + NROWS) {
+                const int r = id - 2;
+                bulk_g2s(tb + r * FAST_TA + toff, p.tab + (int64_t)r * p.stride + tl0, nl * 8u, &s_bar2);
+            } else if (id < 2 + NROWS + LFA_LO_ROWS) {   /* float rows from sample a0 - 2 (a multiple of 4) on: see LFA_TLW */
+                const int r = id - 2 - NROWS;
                 const float *glo = reinterpret_cast<const float *>(p.tab + (int64_t)LTDI_TABLE_ROWS * p.stride);
-                bulk_g2s(tl + tid * LFA_TLW + (f0 - (a0 - 2)), glo + (int64_t)tid * p.stride + f0, nf * 4u, &s_bar);
-            }
-            if (bulk && tid >= 30) {
-                const double *src = tid == 30 ? gp : gc;
-                bulk_g2s((tid == 30 ? raw_p : raw_c) + (g_lo - rs), src + g_lo, ncopy * 8u, &s_bar);
+                bulk_g2s(tl + r * LFA_TLW + (f0 - (a0 - 2)), glo + (int64_t)r * p.stride + f0, nf * 4u, &s_bar2);
             }
         }
         for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
@@ -511,9 +514,7 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
         he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * LFA_TLW);
         cp_async_wait_all();
         __syncthreads();
-        mbar_wait(&s_bar, 0);
-        /* tile anchors of the antenna patterns: warp l builds the anchor of link l, then joins the stencil pass */
-        if (tid < 96) lfa_anchor_warp(fr, tb, tl, tid >> 5, (int)max(min((int64_t)(FAST_TA / 2), p.n - 1 - a0), (int64_t)toff), s_anc, tid & 31);
+        mbar_wait(&s_bar, 0);      /* the raw strain: the stencil pass runs while the table rows are still arriving */
         const int ws = w + p.xw;   /* the widest stencil applied to the strain */
         for (int i = tid; i < 2 * hw2; i += FAST_TA_THREADS) {
             const int64_t g = org + i;
@@ -542,6 +543,9 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
             ((i & 1) ? ho_p : he_p)[i >> 1] = vp;
             ((i & 1) ? ho_c : he_c)[i >> 1] = vc;
         }
+        mbar_wait(&s_bar2, 0);     /* the table rows and their low parts */
+        /* tile anchors of the antenna patterns: warp l builds the anchor of link l */
+        if (tid < 96) lfa_anchor_warp(fr, tb, tl, tid >> 5, (int)max(min((int64_t)(FAST_TA / 2), p.n - 1 - a0), (int64_t)toff), s_anc, tid & 31);
         __syncthreads();
     }
 
