@@ -337,6 +337,44 @@ class Oracle:
             raise ValueError(f"oracle lfa_ext: status {rc}")
         return out
 
+    def margins_lfa6(self, orbit, gen, order, fd_order):
+        lo, hi = C.c_int64(), C.c_int64()
+        d = self._desc(orbit)
+        assert self.lib.orc_margins_lfa6(C.byref(d), gen, order, fd_order, C.byref(lo), C.byref(hi)) == 0
+        return lo.value, hi.value
+
+    def response_lfa6(self, orbit, hp, hc, sources, gen, order, fd_order, nb=0, ne=None, want=("XYZ", "y")):
+        """O14: all six LFA links and the Michelson variables of Eq. (B20) / (B30) (no link-reversal symmetry)."""
+        hp, hc = np.atleast_2d(_f64(hp)), np.atleast_2d(_f64(hc))
+        batch, ld = hp.shape
+        src, ns = self._sources(sources)
+        assert ns == batch and ld >= orbit["n"]
+        ne = orbit["n"] if ne is None else ne
+        ln = ne - nb
+        out = {"A": np.zeros((batch, ln)), "E": np.zeros((batch, ln)), "T": np.zeros((batch, ln))}
+        out["XYZ"] = np.zeros((3, batch, ln)) if "XYZ" in want else None
+        out["y"] = np.zeros((6, batch, ln)) if "y" in want else None
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_response_lfa6(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(hp), _ptr(hc), C.c_int64(ld), C.c_int64(batch), src,
+                                        C.c_int(gen), C.c_int(order), C.c_int(fd_order), C.c_int64(nb), C.c_int64(ne),
+                                        _ptr(out["A"]), _ptr(out["E"]), _ptr(out["T"]), _ptr(out["XYZ"]), _ptr(out["y"]))
+        if rc != 0:
+            raise ValueError(f"oracle lfa6: status {rc}")
+        return out
+
+    def michelson_b20_from_links(self, orbit, y, gen, order, fd_order):
+        """X, Y, Z [3][n] of Eq. (B20) / (B30) from caller-supplied link series y [6][n]."""
+        y = _f64(y)
+        assert y.shape == (6, orbit["n"])
+        out = np.zeros((3, orbit["n"]))
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_michelson_b20_from_links(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(y), C.c_int(gen), C.c_int(order),
+                                                   C.c_int(fd_order), _ptr(out))
+        assert rc == 0
+        return out
+
     def response_hybrid(self, orbit, hp, hc, sources, gen, order, fd_order, hyb, nb=0, ne=None,
                         want=("XYZ", "y")):
         return self._run("hybrid", orbit, hp, hc, sources, gen, order, fd_order, hyb, nb, ne, want)

@@ -181,6 +181,14 @@ static real fd2_r(const real *x, int64_t i, real dt, int fd_order)
     return (16 * d1 - d2) / (12 * dt * dt);
 }
 
+static real fd3_r(const real *x, int64_t i, real dt, int fd_order)
+{
+    const real p1 = x[i + 1] - x[i - 1], p2 = x[i + 2] - x[i - 2];
+    if (fd_order == 2) return (p2 - 2 * p1) / (2 * dt * dt * dt);
+    const real p3 = x[i + 3] - x[i - 3];
+    return (8 * p2 - 13 * p1 - p3) / (8 * dt * dt * dt);
+}
+
 /* third derivative (the m = 1 term of Eq. (B4) needs d^3 H / dt^3): central stencils of accuracy
  * order 2, (x[+2] - 2 x[+1] + 2 x[-1] - x[-2]) / (2 dt^3), and 4,
  * (-x[+3] + 8 x[+2] - 13 x[+1] + 13 x[-1] - 8 x[-2] + x[-3]) / (8 dt^3), written as differences of symmetric pairs
@@ -430,6 +438,24 @@ static void links_lfa_ext_at(const orbit_ctx *o, const frame_t *f, const real *g
     }
 }
 
+/* all six LFA links (O14): Eq. (B10) at the retarded time (B1) of each link with ITS OWN light time L_l (l = -1, -2, -3
+ * differ from +1, +2, +3 by L_-l != L_l only: the antenna patterns are even in n_l and R_s + R_r is symmetric) */
+static void links_lfa6_at(const orbit_ctx *o, const frame_t *f, const real *gp, const real *gc, int64_t g0,
+                          int64_t glen, int64_t n, int order, real y[6])
+{
+    const real c = ORC_C_LIGHT, dt = o->d.dt;
+    geom_t g;
+    orbit_geometry(o, n, &g);
+    for (int l = 0; l < 6; ++l) {
+        const int s = LINK_S[l], r = LINK_R[l];
+        real Fp, Fc;
+        antenna(f, g.nh[l], &Fp, &Fc);
+        const real tau = g.L[l] / 2 + (dot3(f->k, g.R[s]) + dot3(f->k, g.R[r])) / (2 * c); /* (B1) */
+        const real dH = Fp * interp_series(gp, g0, glen, n, tau, dt, order) + Fc * interp_series(gc, g0, glen, n, tau, dt, order);
+        y[l] = -(g.L[l] / 2) * dH;                                                          /* (B10) */
+    }
+}
+
 /* ---------------------------------------------------------------------------------- */
 /* O6  Michelson TDI, Eqs. (2.7), (2.8) with G8, G9, G12; ch = 0,1,2 -> X,Y,Z          */
 /* ---------------------------------------------------------------------------------- */
@@ -552,6 +578,42 @@ static real michelson_lfa_at(const yseries_t *dys, const real Lsec[6], int ch, i
                     L2 * ydel(dys, +p3, n, L2 + L3 / 2, dt, order));
     return 8 * (L2 + L3) * (L3 * ydel(dys, +p2, n, 2 * L3 + 3 * L2 / 2, dt, order) -
                             L2 * ydel(dys, +p3, n, 2 * L2 + 3 * L3 / 2, dt, order));
+}
+
+/* O14: the Michelson variables Taylor-expanded WITHOUT the link-reversal symmetry, Eq. (B20)
+ * (gen 1.5) and Eq. (B30) P:894 (gen 2.0): all six LFA links, first and second (second and third) time derivatives of
+ * each, evaluated at the mid-points (B18) / (B31) of the two arms (reading G13: the printed (B21) / (B32) disagree with
+ * them; d/dtau = d/dt as in (B7)).  For X, with P = y_123 (+p2), Q = y_3-21 (-p2), U = y_1-32 (-p3), W = y_231 (+p3),
+ * a = L_-p2 + L_p2, b = L_-p3 + L_p3:
+ *   X_1.5 = b [P' - (L_-p2 / 2) P''](tau_2) + b [Q' + (L_-p2 / 2) Q''](tau_2) - a [U' - (L_p3 / 2) U''](tau_3) - a [W' + (L_p3 / 2) W''](tau_3)
+ *     tau_2 = t - (L_-p3 + L_-p2 + L_p3) / 2,   tau_3 = t - (L_-p2 + L_p2 + L_p3) / 2                              (B18)
+ *   X_2.0 = (a + b) { b [P'' - (L_-p2 / 2) P'''](tau_2) + b [Q'' + (L_-p2 / 2) Q'''](tau_2)
+ *                    - a [U'' - (L_p3 / 2) U'''](tau_3) - a [W'' + (L_p3 / 2) W'''](tau_3) }
+ *     tau_2 = t - L_-p3 - L_-p2 - L_p3 - L_p2 / 2,   tau_3 = t - L_-p2 - L_p2 - L_p3 - L_-p3 / 2                    (B31)
+ * dlo[l], dhi[l]: the lower and the higher of the two derivatives of link l on the grid. */
+static real michelson_b20_at(const yseries_t *dlo, const yseries_t *dhi, const real Lsec[6], int ch, int gen, int64_t n,
+                             real dt, int order)
+{
+    const int p2 = cyc(2, ch), p3 = cyc(3, ch);
+    const real Lp2 = Lsec[link_index(p2)], Lm2 = Lsec[link_index(-p2)];
+    const real Lp3 = Lsec[link_index(p3)], Lm3 = Lsec[link_index(-p3)];
+    const real a = Lm2 + Lp2, b = Lm3 + Lp3;
+    real d2, d3, pre;
+    if (gen == ORC_GEN_15) {
+        d2 = (Lm3 + Lm2 + Lp3) / 2;
+        d3 = (Lm2 + Lp2 + Lp3) / 2;
+        pre = 1;
+    } else {
+        d2 = Lm3 + Lm2 + Lp3 + Lp2 / 2;
+        d3 = Lm2 + Lp2 + Lp3 + Lm3 / 2;
+        pre = a + b;
+    }
+#define DLO(label, d) ydel(dlo, (label), n, (d), dt, order)
+#define DHI(label, d) ydel(dhi, (label), n, (d), dt, order)
+    return pre * (b * (DLO(+p2, d2) - (Lm2 / 2) * DHI(+p2, d2)) + b * (DLO(-p2, d2) + (Lm2 / 2) * DHI(-p2, d2))
+                  - a * (DLO(-p3, d3) - (Lp3 / 2) * DHI(-p3, d3)) - a * (DLO(+p3, d3) + (Lp3 / 2) * DHI(+p3, d3)));
+#undef DLO
+#undef DHI
 }
 
 /* O7  Eq. (2.9) */
@@ -708,6 +770,64 @@ static int lfa_one_ext(const orbit_ctx *o, const frame_t *f, const double *hp, c
     }
     free(gp); free(gc); free(g3p); free(g3c);
     for (int l = 0; l < 3; ++l) free(dy[l]);
+    return ORC_OK;
+}
+
+/* LFA response without the link-reversal symmetry (O14) for one source; xw = 1 for gen 2.0 (third-derivative stencil) */
+static int lfa6_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen, int order,
+                    int fd_order, const margins_t *mg, int64_t nb, int64_t ne, work_t *w)
+{
+    const int64_t N = o->d.n, wd = mg->w, xw = gen == ORC_GEN_20 ? 1 : 0, wy = wd + xw;
+    const real dt = o->d.dt;
+    const int64_t d0 = imax(0, nb - mg->m2), d1 = imin(N, ne + (order + 1) / 2 + 1);
+    const int64_t y0 = imax(0, d0 - wy), y1 = imin(N, d1 + wy);
+    const int64_t g0 = imax(0, y0 - mg->m1), g1 = imin(N, y1 + mg->m1);
+    real *gp = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *gc = (real *)calloc((size_t)imax(g1 - g0, 1), sizeof(real));
+    real *lo[6], *hi[6];
+    for (int l = 0; l < 6; ++l) {
+        lo[l] = (real *)calloc((size_t)imax(d1 - d0, 1), sizeof(real));
+        hi[l] = (real *)calloc((size_t)imax(d1 - d0, 1), sizeof(real));
+        if (!lo[l] || !hi[l]) return ORC_EINVAL;
+    }
+    if (!gp || !gc || work_alloc(w, y0, y1 - y0, ne - nb)) return ORC_EINVAL;
+#pragma omp parallel for
+    for (int64_t i = g0; i < g1; ++i) {
+        if (i < wd || i >= N - wd) continue;
+        gp[i - g0] = fd1_in(hp, i, dt, fd_order);
+        gc[i - g0] = fd1_in(hc, i, dt, fd_order);
+    }
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t m = y0; m < y1; ++m) {
+        if (m < mg->m1 + wd || m >= N - mg->m1 - wd) continue;
+        real y[6];
+        links_lfa6_at(o, f, gp, gc, g0, g1 - g0, m, order, y);
+        for (int l = 0; l < 6; ++l) w->y[l][m - y0] = y[l];
+    }
+#pragma omp parallel for
+    for (int64_t i = d0; i < d1; ++i) {
+        if (i < mg->m1 + wd + wy || i >= N - mg->m1 - wd - wy) continue;
+        for (int l = 0; l < 6; ++l) {
+            if (gen == ORC_GEN_15) {
+                lo[l][i - d0] = fd1_r(w->y[l], i - y0, dt, fd_order);
+                hi[l][i - d0] = fd2_r(w->y[l], i - y0, dt, fd_order);
+            } else {
+                lo[l][i - d0] = fd2_r(w->y[l], i - y0, dt, fd_order);
+                hi[l][i - d0] = fd3_r(w->y[l], i - y0, dt, fd_order);
+            }
+        }
+    }
+    yseries_t slo = { { lo[0], lo[1], lo[2], lo[3], lo[4], lo[5] }, d0, d1 - d0 };
+    yseries_t shi = { { hi[0], hi[1], hi[2], hi[3], hi[4], hi[5] }, d0, d1 - d0 };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = nb; n < ne; ++n) {
+        if (n < mg->lo + xw || n >= N - mg->hi - xw) continue;
+        geom_t g;
+        orbit_geometry(o, n, &g);
+        for (int c = 0; c < 3; ++c) w->X[c][n - nb] = michelson_b20_at(&slo, &shi, g.L, c, gen, n, dt, order);
+    }
+    free(gp); free(gc);
+    for (int l = 0; l < 6; ++l) { free(lo[l]); free(hi[l]); }
     return ORC_OK;
 }
 
@@ -1110,6 +1230,73 @@ int orc_response_lfa_ext(const orc_orbit_desc *d, const double *Rtab, const doub
         emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
         work_free(&w);
     }
+    return ORC_OK;
+}
+
+/* O14: six LFA links and the Michelson variables of Eq. (B20) / (B30); margins grow by one sample for gen 2.0 */
+int orc_margins_lfa6(const orc_orbit_desc *d, int gen, int order, int fd_order, int64_t *lo, int64_t *hi)
+{
+    margins_t m;
+    if (!d || !lo || !hi) return ORC_EINVAL;
+    margins(d, gen, order, fd_order, &m);
+    *lo = m.lo + (gen == ORC_GEN_20 ? 1 : 0);
+    *hi = m.hi + (gen == ORC_GEN_20 ? 1 : 0);
+    return ORC_OK;
+}
+
+int orc_response_lfa6(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp, const double *hc,
+                      int64_t ld, int64_t batch, const orc_source *src, int gen, int order, int fd_order, int64_t nb,
+                      int64_t ne, double *A, double *E, double *T, double *XYZ, double *y)
+{
+    if (check_args(d, gen, order, fd_order, 1, ld, nb, ne) || !hp || !hc || !src) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, fd_order, &mg);
+    for (int64_t b = 0; b < batch; ++b) {
+        frame_t f;
+        work_t w;
+        source_frame(&src[b], &f);
+        if (lfa6_one(&o, &f, hp + b * ld, hc + b * ld, gen, order, fd_order, &mg, nb, ne, &w)) return ORC_EINVAL;
+        emit(&w, nb, ne, b, batch, A, E, T, XYZ, y);
+        work_free(&w);
+    }
+    return ORC_OK;
+}
+
+/* X, Y, Z of Eq. (B20) / (B30) from caller-supplied link series y [6][n] (for the pins): the derivatives by the stencils
+ * of order fd_order, valid where they fit */
+int orc_michelson_b20_from_links(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *y, int gen,
+                                 int order, int fd_order, double *XYZ)
+{
+    if (check_args(d, gen, order, fd_order, 1, d ? d->n : 0, 0, d ? d->n : 0) || !y || !XYZ) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, fd_order, &mg);
+    const int64_t N = d->n, wy = fd_order / 2 + 1;
+    real *yr = (real *)malloc(sizeof(real) * (size_t)N), *lo[6], *hi[6];
+    if (!yr) return ORC_EINVAL;
+    for (int l = 0; l < 6; ++l) {
+        lo[l] = (real *)calloc((size_t)N, sizeof(real));
+        hi[l] = (real *)calloc((size_t)N, sizeof(real));
+        if (!lo[l] || !hi[l]) return ORC_EINVAL;
+        for (int64_t i = 0; i < N; ++i) yr[i] = y[(int64_t)l * N + i];
+        for (int64_t i = wy; i < N - wy; ++i) {
+            lo[l][i] = gen == ORC_GEN_15 ? fd1_r(yr, i, (real)d->dt, fd_order) : fd2_r(yr, i, (real)d->dt, fd_order);
+            hi[l][i] = gen == ORC_GEN_15 ? fd2_r(yr, i, (real)d->dt, fd_order) : fd3_r(yr, i, (real)d->dt, fd_order);
+        }
+    }
+    yseries_t slo = { { lo[0], lo[1], lo[2], lo[3], lo[4], lo[5] }, 0, N }, shi = { { hi[0], hi[1], hi[2], hi[3], hi[4], hi[5] }, 0, N };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int c = 0; c < 3; ++c) XYZ[(int64_t)c * N + n] = 0.0;
+        if (n < mg.lo + 1 || n >= N - mg.hi - 1) continue;
+        geom_t g;
+        orbit_geometry(&o, n, &g);
+        for (int c = 0; c < 3; ++c)
+            XYZ[(int64_t)c * N + n] = (double)michelson_b20_at(&slo, &shi, g.L, c, gen, n, (real)d->dt, order);
+    }
+    free(yr);
+    for (int l = 0; l < 6; ++l) { free(lo[l]); free(hi[l]); }
     return ORC_OK;
 }
 
