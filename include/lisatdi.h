@@ -226,6 +226,20 @@ int ltdi_response_lfa_ext(const ltdi_orbits *orb, const double *d_hp, const doub
 int ltdi_margins_lfa_ext(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int terms,
                          int64_t *lo, int64_t *hi);
 
+/* SURVEY.md 8(f)-2, second part: the Michelson variables Taylor-expanded WITHOUT the link-reversal symmetry
+ * (L_l = L_-l, y_slr = y_r-ls) that (B25) / (B33) assume -- Eq. (B20) P:832 (gen 1.5) and Eq. (B30) P:894 (gen 2.0): all six
+ * LFA links, each from (B10) at its own retarded time (B1), their first and second (gen 2.0: second and third) time
+ * derivatives by the central stencils of order fd_order, evaluated at the mid-points (B18) / (B31) of the two arms
+ * (reading G13; d/dtau = d/dt).  With P = y_123, Q = y_3-21, U = y_1-32, W = y_231, a = L_-2 + L_2, b = L_-3 + L_3:
+ *   X_1.5 = b [P' - (L_-2 / 2) P''] + b [Q' + (L_-2 / 2) Q''] - a [U' - (L_3 / 2) U''] - a [W' + (L_3 / 2) W'']
+ *   X_2.0 = (a + b) { the same with one more derivative on every link }.
+ * d_y returns all six LFA links.  Output margins grow by one sample for gen 2.0 (ltdi_margins_lfa6).  Runs on the
+ * library's generic tile kernel (per-sample weights, plain fp64) for every Lagrange order. */
+int ltdi_response_lfa6(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                       const ltdi_source *h_src, int gen, int lagrange_order, int fd_order, double *d_A, double *d_E,
+                       double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream);
+int ltdi_margins_lfa6(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi);
+
 /* Hybrid: LFA for t <= t_hyb + T/2, full for t >= t_hyb - T/2, links blended by Eq. (4.5) and
  * X, Y, Z blended separately by Eq. (4.6) (S8).  h_hyb has n_hyb = 1 or batch entries. */
 int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,

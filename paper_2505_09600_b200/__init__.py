@@ -98,6 +98,9 @@ _SIGNATURES = {
                                     C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa_ext": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                         C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_lfa6": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
+                                     _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_margins_lfa6": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, C.c_int, C.c_int, _i64p, _i64p]),
     "ltdi_margins_lfa_ext": (C.c_int, [C.POINTER(OrbitDesc), C.c_int, C.c_int, C.c_int, C.c_int, _i64p, _i64p]),
     "ltdi_response_hybrid": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                        C.c_int, C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _dp, _dp, _vp,
@@ -341,6 +344,8 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
             rc, fn = lib().ltdi_response_full_nested(*head, int(ext[0]), *tail), "ltdi_response_full_nested"
         elif which == RESPONSE_FULL:
             rc, fn = lib().ltdi_response_full(*head, *tail), "ltdi_response_full"
+        elif which == RESPONSE_LFA and ext == "lfa6":
+            rc, fn = lib().ltdi_response_lfa6(*head, fd_order, *tail), "ltdi_response_lfa6"
         elif which == RESPONSE_LFA and ext is not None:
             rc, fn = lib().ltdi_response_lfa_ext(*head, fd_order, int(ext[0]), int(ext[1]), *tail), "ltdi_response_lfa_ext"
         elif which == RESPONSE_LFA:
@@ -401,6 +406,18 @@ def response_lfa_ext(orb, hp, hc, sources, gen, order, fd_order, terms=1, point=
     (LFA_CENTRAL (B1), LFA_BACKWARD (B13), LFA_FORWARD (B14)), then (B25) / (B33)."""
     return _run(RESPONSE_LFA, orb, hp, hc, sources, gen, order, fd_order, None, want_xyz, want_y, workspace,
                 ext=(terms, point))
+
+
+def response_lfa6(orb, hp, hc, sources, gen, order, fd_order, want_xyz=False, want_y=False, workspace=None):
+    """six LFA links and the Michelson variables of Eq. (B20) / (B30) (no link-reversal symmetry)."""
+    return _run(RESPONSE_LFA, orb, hp, hc, sources, gen, order, fd_order, None, want_xyz, want_y, workspace, ext="lfa6")
+
+
+def margins_lfa6(desc, gen, order, fd_order):
+    lo, hi = C.c_int64(), C.c_int64()
+    d = _desc(desc)
+    _check("ltdi_margins_lfa6", lib().ltdi_margins_lfa6(C.byref(d), gen, order, fd_order, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
 
 
 def response_hybrid(orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz=False, want_y=False,

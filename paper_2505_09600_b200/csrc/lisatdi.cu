@@ -693,8 +693,9 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
                  double *d_y, void *d_work, size_t work_bytes, void *stream, int lfa_terms = 1,
-                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0, const ltdi_chirp *h_wav = nullptr)
+                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0, const ltdi_chirp *h_wav = nullptr, int lfa6 = 0)
 {
+    if (lfa6 && (which != LTDI_RESPONSE_LFA || lfa_terms != 1 || lfa_point != LTDI_LFA_CENTRAL)) return LTDI_EINVAL;
     if (nested_order != 0 && (which != LTDI_RESPONSE_FULL || nested_order != 3)) return nested_order == 3 || nested_order < 0 || !(nested_order & 1) ? LTDI_EINVAL : LTDI_EUNSUPPORTED;
     if (nested_order && !fast_order(order)) return LTDI_EUNSUPPORTED;   /* nested delays run on the tuned path (orders 9, 31) */
     if (lfa_terms < 1 || lfa_terms > 2 || lfa_point < LTDI_LFA_CENTRAL || lfa_point > LTDI_LFA_FORWARD) return LTDI_EINVAL;
@@ -728,7 +729,8 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     cudaStream_t st = (cudaStream_t)stream;
     const ltdi_orbit_desc &d = orb->desc;
     Margins mg = compute_margins(d, gen, order, fd_order);
-    const int xw = lfa_terms >= 2 ? 1 : 0;   /* the third-derivative stencil is one sample wider than the first */
+    /* the third-derivative stencil is one sample wider than the first ((B4) m = 1 term: of the strain; (B30): of the links) */
+    const int xw = (lfa_terms >= 2 || (lfa6 && gen == LTDI_GEN_20)) ? 1 : 0;
     mg.lo += xw; mg.hi += xw;
     const int M = order + 1;
 
@@ -805,9 +807,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.qmax = (int)(mg.m1 - M / 2);
     p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw; p.nested = nested_order != 0;
     p.chirp = h_wav ? w_chirp : nullptr;
+    p.lfa6 = lfa6;
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
-    if (fast_order(order)) {
+    if (fast_order(order) && !lfa6) {   /* (B20) / (B30) run on the generic kernel for every order */
         const double *sm = have_small ? small_args.v : nullptr;
         const HybPlan *dp = have_small ? nullptr : w_plan;
         double *fw = (double *)d_work + work_doubles(batch);
@@ -837,9 +840,9 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
         size_t off = 0;
         if (which != LTDI_RESPONSE_LFA) off += 6 * (size_t)p.yr;
         p.off_yL = (int)off;
-        if (which != LTDI_RESPONSE_FULL) off += 3 * (size_t)(p.yr + 2 * w);
+        if (which != LTDI_RESPONSE_FULL) off += lfa6 ? 6 * (size_t)(p.yr + 2 * (w + xw)) : 3 * (size_t)(p.yr + 2 * w);
         p.off_dL = (int)off;
-        if (which != LTDI_RESPONSE_FULL) off += 3 * (size_t)p.yr;
+        if (which != LTDI_RESPONSE_FULL) off += (lfa6 ? 12 : 3) * (size_t)p.yr;
         p.off_hs = (int)off;
         if (stage) off += 2 * (size_t)p.hw;
         smem = off * sizeof(double);
@@ -1113,6 +1116,23 @@ int ltdi_response_lfa_ext(const ltdi_orbits *orb, const double *d_hp, const doub
 {
     return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
                         0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, terms, point);
+}
+
+int ltdi_response_lfa6(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                       const ltdi_source *h_src, int gen, int lagrange_order, int fd_order, double *d_A, double *d_E,
+                       double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
+                        0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, 0, nullptr, 1);
+}
+
+int ltdi_margins_lfa6(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi)
+{
+    if (fd_order != 2 && fd_order != 4) return LTDI_EINVAL;
+    const int rc = ltdi_margins(desc, gen, lagrange_order, fd_order, lo, hi);
+    if (rc) return rc;
+    if (gen == LTDI_GEN_20) { *lo += 1; *hi += 1; }
+    return LTDI_OK;
 }
 
 int ltdi_margins_lfa_ext(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int terms, int64_t *lo,

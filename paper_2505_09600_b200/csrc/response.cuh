@@ -32,6 +32,7 @@ struct RespParams {
     int qmax;             /* bound on |integer shift| of a projection delay (m1 - M/2) */
     int nested;           /* nested TDI delays (tuned path only) */
     const struct ChirpDev *chirp; /* waveform model constants [batch], or nullptr (sampled strain) */
+    int lfa6;             /* all six LFA links and the Michelson variables of Eq. (B20) / (B30) (generic kernel) */
     int lfa_terms, lfa_point, xw; /* terms of Eq. (B4), expansion point LTDI_LFA_*, xw = terms - 1 */
     int64_t ntiles;
 };
@@ -259,6 +260,35 @@ __device__ __forceinline__ void links_lfa(const RespParams &p, const Strain<STAG
     }
 }
 
+// SURVEY 8(f)-2, Eq. (B20) / (B30): all six LFA links, each at the retarded time (B1) with ITS OWN light time
+template <int MT, bool STAGE>
+__device__ __forceinline__ void links_lfa6(const RespParams &p, const Strain<STAGE> &h, const double *fr, int64_t m,
+                                           double y[6])
+{
+    Geom g;
+    load_geometry(p, fr, m, g);
+    Lagrange<MT> lag;
+    const int Mx = MT ? MT : p.M;
+    const int half = Mx / 2 - 1;
+    const double den = (p.fd == 2 ? 2.0 : 12.0) * p.dt;
+#pragma unroll 1
+    for (int l = 0; l < 6; ++l) {
+        const int s = link_sender(l), r = link_receiver(l), a = l % 3;
+        int q;
+        double eps;
+        split_delay(0.5 * g.L[l] + 0.5 * (g.kR[s] + g.kR[r]), p.dt, q, eps);      /* (B1) */
+        q = clamp_shift(q, p.qmax);
+        lag.weights(eps, p.M);
+        const double *xp = h.plus(m - q - half), *xc = h.cross(m - q - half);
+        double ap = 0.0, ac = 0.0;
+        for (int i = 0; i < Mx; ++i) {
+            ap = fma(lag.w[i], p.fd == 2 ? fd1_num<2>(xp + i) : fd1_num<4>(xp + i), ap);
+            ac = fma(lag.w[i], p.fd == 2 ? fd1_num<2>(xc + i) : fd1_num<4>(xc + i), ac);
+        }
+        y[l] = -(0.5 * g.L[l]) * (g.Fp[a] * (ap / den) + g.Fc[a] * (ac / den));   /* (B10) */
+    }
+}
+
 // D_delay y: series ys (shared memory, element 0 = absolute sample y0, length len) at t_n - delay
 template <int MT>
 __device__ __forceinline__ double delayed(const RespParams &p, const double *ys, int64_t y0, int len, int64_t n,
@@ -322,6 +352,28 @@ __device__ __forceinline__ double michelson_lfa(const RespParams &p, const doubl
                       L2 * delayed<MT>(p, d231, y0, p.yr, n, L2 + 0.5 * L3));
     return 8.0 * (L2 + L3) * (L3 * delayed<MT>(p, d123, y0, p.yr, n, 2.0 * L3 + 1.5 * L2) -
                               L2 * delayed<MT>(p, d231, y0, p.yr, n, 2.0 * L2 + 1.5 * L3));
+}
+
+// Eq. (B20) (gen 1.5) / (B30) (gen 2.0) at the mid-points (B18) / (B31) (G13): dlo / dhi = the lower / higher of the two
+// time derivatives of the six LFA links, [6][yr] each
+template <int MT>
+__device__ __forceinline__ double michelson_b20(const RespParams &p, const double *dlo, const double *dhi, int64_t y0,
+                                                int64_t n, const double L[6], int ch)
+{
+    const int i2 = (1 + ch) % 3, i3 = (2 + ch) % 3;
+    const double Lp2 = L[i2], Lm2 = L[i2 + 3], Lp3 = L[i3], Lm3 = L[i3 + 3];
+    const double a = Lm2 + Lp2, b = Lm3 + Lp3;
+    double d2, d3, pre;
+    if (p.gen == LTDI_GEN_15) { d2 = (Lm3 + Lm2 + Lp3) / 2; d3 = (Lm2 + Lp2 + Lp3) / 2; pre = 1.0; }
+    else { d2 = Lm3 + Lm2 + Lp3 + Lp2 / 2; d3 = Lm2 + Lp2 + Lp3 + Lm3 / 2; pre = a + b; }
+#define DLO(l, d) delayed<MT>(p, dlo + (size_t)(l) * p.yr, y0, p.yr, n, (d))
+#define DHI(l, d) delayed<MT>(p, dhi + (size_t)(l) * p.yr, y0, p.yr, n, (d))
+    /* P = y_{+p2}, Q = y_{-p2}, U = y_{-p3}, W = y_{+p3} */
+    const double x = b * (DLO(i2, d2) - (Lm2 / 2) * DHI(i2, d2)) + b * (DLO(i2 + 3, d2) + (Lm2 / 2) * DHI(i2 + 3, d2)) -
+                     a * (DLO(i3 + 3, d3) - (Lp3 / 2) * DHI(i3 + 3, d3)) - a * (DLO(i3, d3) + (Lp3 / 2) * DHI(i3, d3));
+#undef DLO
+#undef DHI
+    return pre * x;
 }
 
 // Eqs. (4.1), (4.5) with G18; raised cosine, G20
@@ -403,7 +455,45 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
             for (int l = 0; l < 6; ++l) yF[(size_t)l * p.yr + i] = y[l];
         }
     }
-    if (need_lfa) { /* phase A' */
+    if (need_lfa && p.lfa6) { /* six links, two derivatives of each */
+        const int wy = w + p.xw;                     /* widest stencil applied to the links (third derivative for gen 2.0) */
+        const int len = p.yr + 2 * wy;
+        for (int i = tid; i < len; i += nthr) {
+            const int64_t m = y0 - wy + i;
+            double y[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            if (m >= p.m1 + w && m < p.n - p.m1 - w) links_lfa6<MT, STAGE>(p, h, fr, m, y);
+#pragma unroll
+            for (int l = 0; l < 6; ++l) yL[(size_t)l * len + i] = y[l];
+        }
+        __syncthreads();
+        const double dt = p.dt;
+        double *dhi = dL + (size_t)6 * p.yr;
+        for (int i = tid; i < p.yr; i += nthr) {
+            const int64_t m = y0 + i;
+            const bool in = m >= p.m1 + w + wy && m < p.n - p.m1 - w - wy;
+            for (int l = 0; l < 6; ++l) {
+                const double *x = yL + (size_t)l * len + i + wy; /* x[0] = y_l[m] */
+                double d1 = 0.0, d2v = 0.0, d3v = 0.0;
+                if (in) {
+                    const double p1 = x[1] - x[-1];
+                    const double s1 = (x[1] - x[0]) - (x[0] - x[-1]);
+                    if (p.fd == 2) {
+                        d1 = p1 / (2.0 * dt);
+                        d2v = s1 / (dt * dt);
+                        if (p.gen != LTDI_GEN_15) d3v = ((x[2] - x[-2]) - 2.0 * p1) / (2.0 * dt * dt * dt);
+                    } else {
+                        const double p2 = x[2] - x[-2];
+                        const double s2 = (x[2] - x[0]) - (x[0] - x[-2]);
+                        d1 = (8.0 * p1 - p2) / (12.0 * dt);
+                        d2v = (16.0 * s1 - s2) / (12.0 * dt * dt);
+                        if (p.gen != LTDI_GEN_15) d3v = (8.0 * p2 - 13.0 * p1 - (x[3] - x[-3])) / (8.0 * dt * dt * dt);
+                    }
+                }
+                dL[(size_t)l * p.yr + i] = p.gen == LTDI_GEN_15 ? d1 : d2v;
+                dhi[(size_t)l * p.yr + i] = p.gen == LTDI_GEN_15 ? d2v : d3v;
+            }
+        }
+    } else if (need_lfa) { /* phase A' */
         const int len = p.yr + 2 * w;
         for (int i = tid; i < len; i += nthr) {
             const int64_t m = y0 - w + i;
@@ -455,7 +545,8 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
 #pragma unroll 1
             for (int ch = 0; ch < 3; ++ch) {
                 double x = 0.0;
-                if (need_lfa && wa != 0.0) x = wa * michelson_lfa<MT>(p, dL, y0, n, L, ch);
+                if (need_lfa && p.lfa6) x = michelson_b20<MT>(p, dL, dL + (size_t)6 * p.yr, y0, n, L, ch);
+                else if (need_lfa && wa != 0.0) x = wa * michelson_lfa<MT>(p, dL, y0, n, L, ch);
                 if (need_full && wb != 0.0) x = fma(wb, michelson_full<MT>(p, yF, y0, n, L, ch), x); /* (4.6) */
                 X[ch] = x;
             }
@@ -474,6 +565,7 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
             for (int l = 0; l < 6; ++l) {
                 double v = 0.0;
                 if (p.which == LTDI_RESPONSE_FULL) v = yF[(size_t)l * p.yr + iy];
+                else if (p.which == LTDI_RESPONSE_LFA && p.lfa6) v = yL[(size_t)l * (p.yr + 2 * (w + p.xw)) + iy + w + p.xw];
                 else if (p.which == LTDI_RESPONSE_LFA) v = l < 3 ? yL[(size_t)l * (p.yr + 2 * w) + iy + w] : 0.0;
                 else if (n >= p.m1 + w && n < p.n - p.m1 - w) { /* (4.5) */
                     if (need_lfa && l < 3) v = wa * yL[(size_t)l * (p.yr + 2 * w) + iy + w];

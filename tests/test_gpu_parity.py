@@ -504,3 +504,21 @@ def test_lfa_ext_argument_errors(ltdi):
     for terms, point in ((0, 0), (3, 0), (2, 1), (2, 2), (1, 3), (1, -1)):
         with pytest.raises(ltdi.LtdiError):
             ltdi.response_lfa_ext(orb, dhp, dhc, ang, 20, 31, 2, terms, point)
+
+
+# ---- SURVEY 8(f)-2, second part: Eq. (B20) / (B30), six LFA links, no link-reversal symmetry (oracle O14) ----------
+
+@pytest.mark.parametrize("k,n,batch,order,gen,fd", [(2, 40007, 1, 31, 15, 2), (2, 40007, 1, 31, 20, 2), (2, 40007, 1, 31, 20, 4),
+                                                    (1, None, 1, 9, 15, 2), (4, 9001, 3, 9, 20, 4), (4, 9001, 3, 5, 15, 4)])
+def test_lfa6_b20_b30(ltdi, orc80, k, n, batch, order, gen, fd):
+    cfg = W.config(k, n=n, batch=batch) if n else W.config(k)
+    idx = list(range(cfg["batch"]))
+    hp, hc, ang, _ = W.sources(cfg, idx)
+    orbit = cfg["orbit"]
+    dev = torch.device("cuda:0")
+    orb = ltdi.Orbits(orbit, device=dev)
+    ref = orc80.response_lfa6(orbit, hp, hc, ang, gen, order, fd)
+    out = to_numpy(ltdi.response_lfa6(orb, torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev), ang, gen, order, fd, True, True))
+    lo, hi = orc80.margins_lfa6(orbit, gen, order, fd)
+    assert (lo, hi) == ltdi.margins_lfa6(orbit, gen, order, fd)
+    check(out, ref, lo, hi, cfg["n"])
