@@ -75,3 +75,43 @@ def test_no_cpu_fallback(ltdi):
         pytest.skip("GPU present")
     with pytest.raises(RuntimeError):
         ltdi.Orbits(W.orbit_desc(100, 5.0))
+
+
+def test_margins_of_the_next_rows_match_the_oracle(ltdi, orc80):
+    """ltdi_margins_lfa_ext (8f-2, third-derivative stencil of the strain) and ltdi_margins_lfa6 ((B30): of the links)"""
+    for dt in (5.0, 10.0):
+        d = W.orbit_desc(50000, dt)
+        for order in (9, 31):
+            for gen in (15, 20):
+                for fd in (2, 4):
+                    for terms in (1, 2):
+                        assert ltdi.margins_lfa_ext(d, gen, order, fd, terms) == orc80.margins_lfa_ext(d, gen, order, fd, terms)
+                    assert ltdi.margins_lfa6(d, gen, order, fd) == orc80.margins_lfa6(d, gen, order, fd)
+
+
+def test_next_row_arguments_are_checked_before_any_cuda_call(ltdi):
+    lib = ltdi.lib()
+    d = ltdi._desc(W.orbit_desc(1000, 5.0))
+    lo, hi = C.c_int64(), C.c_int64()
+    assert lib.ltdi_margins_lfa_ext(C.byref(d), 20, 31, 2, 3, C.byref(lo), C.byref(hi)) == ltdi.EINVAL     # terms > 2
+    assert lib.ltdi_margins_lfa6(C.byref(d), 20, 31, 3, C.byref(lo), C.byref(hi)) == ltdi.EINVAL           # bad stencil
+    # numerical orbit file: wrong mode, even knot order, knots that do not cover the grid
+    handle = C.c_void_p()
+    one = C.c_double(0.0)
+    ptr = C.cast(C.byref(one), C.c_void_p)
+    kd = ltdi._desc(dict(W.orbit_desc(1000, 5.0), mode=ltdi.ORBIT_KNOTS))
+    assert lib.ltdi_orbits_init_knots(C.byref(d), ptr, 40, 0.0, 86400.0, 7, ptr, 1 << 30, None, C.byref(handle)) == ltdi.EINVAL
+    assert lib.ltdi_orbits_init_knots(C.byref(kd), ptr, 40, -4 * 86400.0, 86400.0, 6, ptr, 1 << 30, None, C.byref(handle)) == ltdi.EINVAL
+    assert lib.ltdi_orbits_init_knots(C.byref(kd), ptr, 40, 86400.0, 86400.0, 7, ptr, 1 << 30, None, C.byref(handle)) == ltdi.EINVAL
+    assert lib.ltdi_orbits_init_knots(C.byref(kd), ptr, 6, -4 * 86400.0, 86400.0, 7, ptr, 1 << 30, None, C.byref(handle)) == ltdi.EINVAL
+    # waveform model and overlap plan
+    assert lib.ltdi_waveform_chirp(None, 1, 0.0, 5.0, 10, 10, None, None, None, 0, None) == ltdi.EINVAL
+    plan, nbytes = C.c_void_p(), C.c_size_t()
+    assert lib.ltdi_overlap_create(1, 1, 1, C.byref(plan), C.byref(nbytes)) == ltdi.EINVAL                # n < 2
+    assert lib.ltdi_overlap_create(40007, 40007, 3, C.byref(plan), C.byref(nbytes)) == ltdi.OK            # a prime: Bluestein, m = 2^17
+    assert nbytes.value >= (40007 + 2 * 131072 + 2 * 9 * 131072) * 16
+    assert lib.ltdi_overlap_destroy(plan) == ltdi.OK
+    assert lib.ltdi_overlap_create(131072, 131072, 2, C.byref(plan), C.byref(nbytes)) == ltdi.OK          # a power of two: no chirp tables
+    assert nbytes.value < (2 * 6 * 131072 + 4096) * 16 + (1 << 16)
+    assert lib.ltdi_overlap_destroy(plan) == ltdi.OK
+    assert ltdi.launch_count() == 0
