@@ -71,21 +71,38 @@ __device__ __forceinline__ void dft_small(double2 *v)
     }
 }
 
+/* Where the first pass of a transform takes its input from: a complex buffer, or -- fused packing -- two real series
+ * per complex series (z = a + i b, times the Bluestein chirp if C is given, zero beyond n) */
+struct FftSource {
+    const double2 *in;          /* complex input (series q at q * stride), or nullptr: pack from the real series below */
+    const double *xa[3], *xb[3];
+    int64_t ld, n;
+    const double2 *C;
+};
+__device__ __forceinline__ double2 fft_load(const FftSource &src, int64_t q, int64_t stride, int64_t j)
+{
+    if (src.in) return src.in[q * stride + j];
+    if (j >= src.n) return make_double2(0.0, 0.0);
+    const int64_t s = q / 3;
+    const int c = (int)(q - 3 * s);
+    const double2 z = make_double2(src.xa[c][s * src.ld + j], src.xb[c][s * src.ld + j]);
+    return src.C ? cmul(z, src.C[j]) : z;
+}
+
 /* One Stockham pass of radix R over series of N points (grid.y = series): thread j < N / R reads x[j + r N / R], applies
  * the twiddles exp(SIGN 2 pi i r (j mod Ns) / (Ns R)), transforms R points and writes them Ns apart.  After the passes
  * with Ns = 1, R1, R1 R2, ... the series is transformed in natural order (autosort: no bit reversal). */
 template <int R, int SIGN>
-__global__ void __launch_bounds__(FFT_THREADS) fft_pass_kernel(const double2 *__restrict__ in, double2 *__restrict__ out, int N,
+__global__ void __launch_bounds__(FFT_THREADS) fft_pass_kernel(const __grid_constant__ FftSource src, double2 *__restrict__ out, int N,
                                                                int Ns, int64_t stride)
 {
     const int j = blockIdx.x * FFT_THREADS + threadIdx.x;
     const int T = N / R;
     if (j >= T) return;
-    in += (int64_t)blockIdx.y * stride;
     out += (int64_t)blockIdx.y * stride;
     double2 v[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) v[r] = in[j + r * T];
+    for (int r = 0; r < R; ++r) v[r] = fft_load(src, blockIdx.y, stride, (int64_t)j + (int64_t)r * T);
     const int k = j & (Ns - 1);
     if (Ns > 1) {
         /* w_r = exp(SIGN 2 pi i r k / (Ns R)): the powers of two by sincospi of an exact argument, the others as products */
@@ -113,6 +130,80 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_kernel(const double2 *__
     for (int r = 0; r < R; ++r) out[j0 + r * Ns] = v[r];
 }
 
+/* exp(SIGN 2 pi i e / 256), e = 0 .. 255 (cos, -sin stored: SIGN = -1; the other sign by conjugation) */
+__constant__ double2 c_w256[256];
+
+/* One Stockham pass of radix 256 through shared memory: a block of 256 threads takes 16 consecutive j < N / 256 and their
+ * 256 inputs x[j + r N / 256] each.  With r = c + 16 r1 and the output index q = q1 + 16 q2,
+ *   X[q1 + 16 q2] = sum_c W16^(c q2) [ W256^(c q1) sum_r1 W16^(r1 q1) x[c + 16 r1] ] :
+ * thread (jj, c) transforms the 16 inputs of residue c and applies W256^(c q1), the block transposes through shared
+ * memory (rows padded to 17: conflict free both ways), thread (jj, q1) transforms over c and writes Ns apart.  One read
+ * and one write of the series for eight bits of the length (two radix-16 passes would move it twice). */
+template <int SIGN>
+__global__ void __launch_bounds__(256) fft_pass256_kernel(const __grid_constant__ FftSource src, double2 *__restrict__ out, int N, int Ns,
+                                                          int64_t stride)
+{
+    extern __shared__ double2 fsm[];   /* [256][17] */
+    const int T = N >> 8;
+    const int jj = threadIdx.x & 15, c = threadIdx.x >> 4;
+    const int j = blockIdx.x * 16 + jj;
+    const int64_t q = blockIdx.y;
+    const bool live = j < T;
+    const int k = j & (Ns - 1);
+    double2 v[16];
+    if (live) {
+#pragma unroll
+        for (int r1 = 0; r1 < 16; ++r1) v[r1] = fft_load(src, q, stride, (int64_t)j + (int64_t)(c + 16 * r1) * T);
+        if (Ns > 1) {
+            /* input twiddles exp(SIGN 2 pi i (c + 16 r1) k / (256 Ns)) = u^c (u^16)^r1 */
+            const double base = (double)k / (double)(Ns * 128);        /* 2 k / (256 Ns) */
+            double sn, cs;
+            sincospi(base * (double)c, &sn, &cs);
+            double2 w = make_double2(cs, SIGN < 0 ? -sn : sn);
+            sincospi(base * 16.0, &sn, &cs);
+            const double2 u16 = make_double2(cs, SIGN < 0 ? -sn : sn);
+            /* powers of u16 by sincospi of exact arguments for the power-of-two exponents, products for the others */
+            double2 up[4];
+            up[0] = u16;
+#pragma unroll
+            for (int b = 1; b < 4; ++b) {
+                sincospi(base * 16.0 * (double)(1 << b), &sn, &cs);
+                up[b] = make_double2(cs, SIGN < 0 ? -sn : sn);
+            }
+#pragma unroll
+            for (int r1 = 0; r1 < 16; ++r1) {
+                double2 t = w;
+#pragma unroll
+                for (int b = 0; b < 4; ++b)
+                    if (r1 & (1 << b)) t = cmul(t, up[b]);
+                v[r1] = cmul(v[r1], t);
+            }
+        }
+        dft_small<16, SIGN>(v);    /* over r1 -> q1 */
+#pragma unroll
+        for (int q1 = 0; q1 < 16; ++q1) {
+            double2 t = c_w256[(c * q1) & 255];
+            if (SIGN > 0) t.y = -t.y;
+            fsm[(c * 16 + q1) * 17 + jj] = cmul(v[q1], t);
+        }
+    }
+    __syncthreads();
+    /* second role of the thread: output residue q1 of series element j2.  While Ns < 16 consecutive outputs of ONE j are
+     * adjacent in memory, so a warp takes 16 residues of two j (256-byte runs); later consecutive j are adjacent */
+    const bool by_residue = Ns < 16;
+    const int q1 = by_residue ? (threadIdx.x & 15) : (threadIdx.x >> 4);
+    const int jj2 = by_residue ? (threadIdx.x >> 4) : (threadIdx.x & 15);
+    const int j2 = blockIdx.x * 16 + jj2;
+    if (j2 >= T) return;
+    const int k2 = j2 & (Ns - 1);
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) v[cc] = fsm[(cc * 16 + q1) * 17 + jj2];
+    dft_small<16, SIGN>(v);        /* over c -> q2 */
+    double2 *o = out + q * stride + (int64_t)(j2 / Ns) * Ns * 256 + k2;
+#pragma unroll
+    for (int q2 = 0; q2 < 16; ++q2) o[(int64_t)(q1 + 16 * q2) * Ns] = v[q2];
+}
+
 /* c_j = exp(-i pi j^2 / n) for j < n (table C) and the wrapped conj(c) of length m (table B, to be transformed) */
 __global__ void __launch_bounds__(FFT_THREADS) bluestein_tables_kernel(int64_t n, int64_t m, double2 *__restrict__ C, double2 *__restrict__ B)
 {
@@ -130,27 +221,6 @@ __global__ void __launch_bounds__(FFT_THREADS) bluestein_tables_kernel(int64_t n
     B[j] = b;
 }
 
-/* pack two real series (row stride ld, grid.y = complex series: a-channel c and b-channel c of source s) into m complex
- * points: (x_j + i y_j) c_j for j < n (C == nullptr: no chirp, power-of-two n), zero beyond */
-__global__ void __launch_bounds__(FFT_THREADS) fft_pack_kernel(const double *__restrict__ xa0, const double *__restrict__ xa1,
-                                                               const double *__restrict__ xa2, const double *__restrict__ xb0,
-                                                               const double *__restrict__ xb1, const double *__restrict__ xb2,
-                                                               int64_t ld, int64_t n, int64_t m, const double2 *__restrict__ C,
-                                                               double2 *__restrict__ out)
-{
-    const int64_t j = (int64_t)blockIdx.x * FFT_THREADS + threadIdx.x;
-    if (j >= m) return;
-    const int64_t q = blockIdx.y, s = q / 3;
-    const int c = (int)(q - 3 * s);
-    const double *xa = (c == 0 ? xa0 : c == 1 ? xa1 : xa2) + s * ld, *xb = (c == 0 ? xb0 : c == 1 ? xb1 : xb2) + s * ld;
-    double2 z = make_double2(0.0, 0.0);
-    if (j < n) {
-        z = make_double2(xa[j], xb[j]);
-        if (C) z = cmul(z, C[j]);
-    }
-    out[q * m + j] = z;
-}
-
 /* A_k *= Bhat_k (grid.y = series) */
 __global__ void __launch_bounds__(FFT_THREADS) fft_pointwise_kernel(double2 *__restrict__ a, const double2 *__restrict__ bhat, int64_t m)
 {
@@ -160,13 +230,15 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pointwise_kernel(double2 *__r
     *p = cmul(*p, bhat[j]);
 }
 
-/* host: the radices of a power-of-two length, and the transform itself; returns the buffer (0: buf0, 1: buf1) that holds
- * the result.  Series q starts at q * stride in both buffers. */
+/* host: the radices of a power-of-two length (256 while eight bits remain, then 16 / 4 / 2), and the transform itself;
+ * returns the buffer (0: buf0, 1: buf1) that holds the result.  Series q starts at q * stride in both buffers.  `first`
+ * (optional) replaces buf0 as the input of the first pass (fused packing). */
 static inline int fft_radices(int64_t N, int *rad)
 {
     int bits = 0;
     while (((int64_t)1 << bits) < N) ++bits;
     int np = 0;
+    while (bits >= 8) { rad[np++] = 256; bits -= 8; }
     while (bits >= 4) { rad[np++] = 16; bits -= 4; }
     if (bits == 3) { rad[np++] = 4; rad[np++] = 2; }
     else if (bits == 2) rad[np++] = 4;
@@ -174,21 +246,44 @@ static inline int fft_radices(int64_t N, int *rad)
     return np;
 }
 
+#define FFT_SMEM256 (256 * 17 * sizeof(double2))
+
+static inline int fft_setup_device()
+{
+    /* twiddles of the radix-256 butterfly, exp(-2 pi i e / 256), in long double; the large dynamic shared memory of its kernels */
+    double2 w[256];
+    for (int e = 0; e < 256; ++e) {
+        const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)e / 256.0L;
+        w[e] = make_double2((double)cosl(a), (double)-sinl(a));
+    }
+    if (cudaMemcpyToSymbol(c_w256, w, sizeof w) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(fft_pass256_kernel<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(fft_pass256_kernel<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
+    return 0;
+}
+
 template <int SIGN>
-static inline int fft_pow2(double2 *buf0, double2 *buf1, int64_t N, int64_t stride, int64_t nseries, cudaStream_t st, int *launches)
+static inline int fft_pow2(double2 *buf0, double2 *buf1, int64_t N, int64_t stride, int64_t nseries, cudaStream_t st,
+                           const FftSource *first = nullptr)
 {
     int rad[16];
     const int np = fft_radices(N, rad);
     int cur = 0;
     int Ns = 1;
     for (int p = 0; p < np; ++p) {
-        const double2 *in = cur ? buf1 : buf0;
+        FftSource src = {};
+        if (p == 0 && first) src = *first;
+        else src.in = cur ? buf1 : buf0;
         double2 *out = cur ? buf0 : buf1;
-        const dim3 grid((unsigned)((N / rad[p] + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nseries);
-        if (rad[p] == 16) fft_pass_kernel<16, SIGN><<<grid, FFT_THREADS, 0, st>>>(in, out, (int)N, Ns, stride);
-        else if (rad[p] == 4) fft_pass_kernel<4, SIGN><<<grid, FFT_THREADS, 0, st>>>(in, out, (int)N, Ns, stride);
-        else fft_pass_kernel<2, SIGN><<<grid, FFT_THREADS, 0, st>>>(in, out, (int)N, Ns, stride);
-        if (launches) ++*launches;
+        if (rad[p] == 256) {
+            const dim3 grid((unsigned)(((N >> 8) + 15) / 16), (unsigned)nseries);
+            fft_pass256_kernel<SIGN><<<grid, 256, FFT_SMEM256, st>>>(src, out, (int)N, Ns, stride);
+        } else {
+            const dim3 grid((unsigned)((N / rad[p] + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nseries);
+            if (rad[p] == 16) fft_pass_kernel<16, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            else if (rad[p] == 4) fft_pass_kernel<4, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            else fft_pass_kernel<2, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+        }
         Ns *= rad[p];
         cur ^= 1;
     }

@@ -210,6 +210,16 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
     if (!(dt > 0.0) || !(fmax >= fmin)) return LTDI_EINVAL;
     if ((uintptr_t)d_work % 256) return LTDI_EINVAL;
     if (work_bytes < o->total) return LTDI_EWORKSPACE;
+    {   /* per-device set-up of the transform (twiddle table, shared-memory attribute), once */
+        static bool ready[64] = {};
+        int dev = 0;
+        OVL_CUDA_OK(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= 64) return LTDI_EUNSUPPORTED;
+        if (!ready[dev]) {
+            if (fft_setup_device()) { (void)cudaGetLastError(); return LTDI_ECUDA; }
+            ready[dev] = true;
+        }
+    }
     cudaStream_t st = (cudaStream_t)stream;
     char *base = (char *)d_work;
     double2 *C = o->pow2 ? nullptr : (double2 *)base;
@@ -223,21 +233,23 @@ int ltdi_overlap_products(ltdi_overlap *o, const double *d_aA, const double *d_a
     if (!o->pow2) { /* chirp tables of this length (rebuilt per call: the work area is the caller's between calls) */
         double2 *t0 = C + n, *t1 = t0 + m;
         bluestein_tables_kernel<<<(unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), FFT_THREADS, 0, st>>>(n, m, C, t0);
-        bhat = fft_pow2<-1>(t0, t1, m, m, 1, st, nullptr) ? t1 : t0;
+        bhat = fft_pow2<-1>(t0, t1, m, m, 1, st) ? t1 : t0;
         OVL_CUDA_OK(cudaGetLastError());
     }
     for (int64_t b0 = 0; b0 < o->batch; b0 += o->chunk) {
         const int64_t nb = std::min(o->chunk, o->batch - b0);
         const int64_t nser = 3 * nb;
         const int64_t off = b0 * o->ld;
-        /* step iv: z = a_c + i b_c (times the chirp), transformed */
-        fft_pack_kernel<<<dim3((unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nser), FFT_THREADS, 0, st>>>(
-            d_aA + off, d_aE + off, d_aT + off, d_bA + off, d_bE + off, d_bT + off, o->ld, n, m, C, buf0);
-        int cur = fft_pow2<-1>(buf0, buf1, m, m, nser, st, nullptr);
+        /* step iv: z = a_c + i b_c (times the chirp), packed by the first pass of the transform itself */
+        FftSource pack = {};
+        pack.xa[0] = d_aA + off; pack.xa[1] = d_aE + off; pack.xa[2] = d_aT + off;
+        pack.xb[0] = d_bA + off; pack.xb[1] = d_bE + off; pack.xb[2] = d_bT + off;
+        pack.ld = o->ld; pack.n = n; pack.C = C;
+        int cur = fft_pow2<-1>(buf0, buf1, m, m, nser, st, &pack);
         if (!o->pow2) {
             double2 *x = cur ? buf1 : buf0, *y = cur ? buf0 : buf1;
             fft_pointwise_kernel<<<dim3((unsigned)((m + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nser), FFT_THREADS, 0, st>>>(x, bhat, m);
-            cur = fft_pow2<+1>(x, y, m, m, nser, st, nullptr) ? !cur : cur;
+            cur = fft_pow2<+1>(x, y, m, m, nser, st) ? !cur : cur;
         }
         const double2 *zb = cur ? buf1 : buf0;
         const dim3 grid((unsigned)o->nblk, 3, (unsigned)nb);
