@@ -79,20 +79,23 @@ struct FftSource {
     int64_t ld, n;
     const double2 *C;
 };
+template <bool PACK>
 __device__ __forceinline__ double2 fft_load(const FftSource &src, int64_t q, int64_t stride, int64_t j)
 {
-    if (src.in) return src.in[q * stride + j];
-    if (j >= src.n) return make_double2(0.0, 0.0);
+    if (!PACK) return src.in[q * stride + j];
+    /* branch-free loads (clamped index, selected afterwards): the sixteen loads of a thread stay in flight together */
     const int64_t s = q / 3;
     const int c = (int)(q - 3 * s);
-    const double2 z = make_double2(src.xa[c][s * src.ld + j], src.xb[c][s * src.ld + j]);
-    return src.C ? cmul(z, src.C[j]) : z;
+    const int64_t jc = j < src.n ? j : src.n - 1;
+    double2 z = make_double2(src.xa[c][s * src.ld + jc], src.xb[c][s * src.ld + jc]);
+    if (src.C) z = cmul(z, src.C[jc]);
+    return j < src.n ? z : make_double2(0.0, 0.0);
 }
 
 /* One Stockham pass of radix R over series of N points (grid.y = series): thread j < N / R reads x[j + r N / R], applies
  * the twiddles exp(SIGN 2 pi i r (j mod Ns) / (Ns R)), transforms R points and writes them Ns apart.  After the passes
  * with Ns = 1, R1, R1 R2, ... the series is transformed in natural order (autosort: no bit reversal). */
-template <int R, int SIGN>
+template <int R, int SIGN, bool PACK>
 __global__ void __launch_bounds__(FFT_THREADS) fft_pass_kernel(const __grid_constant__ FftSource src, double2 *__restrict__ out, int N,
                                                                int Ns, int64_t stride)
 {
@@ -102,7 +105,7 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pass_kernel(const __grid_cons
     out += (int64_t)blockIdx.y * stride;
     double2 v[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) v[r] = fft_load(src, blockIdx.y, stride, (int64_t)j + (int64_t)r * T);
+    for (int r = 0; r < R; ++r) v[r] = fft_load<PACK>(src, blockIdx.y, stride, (int64_t)j + (int64_t)r * T);
     const int k = j & (Ns - 1);
     if (Ns > 1) {
         /* w_r = exp(SIGN 2 pi i r k / (Ns R)): the powers of two by sincospi of an exact argument, the others as products */
@@ -139,7 +142,7 @@ __constant__ double2 c_w256[256];
  * thread (jj, c) transforms the 16 inputs of residue c and applies W256^(c q1), the block transposes through shared
  * memory (rows padded to 17: conflict free both ways), thread (jj, q1) transforms over c and writes Ns apart.  One read
  * and one write of the series for eight bits of the length (two radix-16 passes would move it twice). */
-template <int SIGN>
+template <int SIGN, bool PACK>
 __global__ void __launch_bounds__(256) fft_pass256_kernel(const __grid_constant__ FftSource src, double2 *__restrict__ out, int N, int Ns,
                                                           int64_t stride)
 {
@@ -153,7 +156,7 @@ __global__ void __launch_bounds__(256) fft_pass256_kernel(const __grid_constant_
     double2 v[16];
     if (live) {
 #pragma unroll
-        for (int r1 = 0; r1 < 16; ++r1) v[r1] = fft_load(src, q, stride, (int64_t)j + (int64_t)(c + 16 * r1) * T);
+        for (int r1 = 0; r1 < 16; ++r1) v[r1] = fft_load<PACK>(src, q, stride, (int64_t)j + (int64_t)(c + 16 * r1) * T);
         if (Ns > 1) {
             /* input twiddles exp(SIGN 2 pi i (c + 16 r1) k / (256 Ns)) = u^c (u^16)^r1 */
             const double base = (double)k / (double)(Ns * 128);        /* 2 k / (256 Ns) */
@@ -257,8 +260,9 @@ static inline int fft_setup_device()
         w[e] = make_double2((double)cosl(a), (double)-sinl(a));
     }
     if (cudaMemcpyToSymbol(c_w256, w, sizeof w) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(fft_pass256_kernel<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(fft_pass256_kernel<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(fft_pass256_kernel<-1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(fft_pass256_kernel<-1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(fft_pass256_kernel<+1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT_SMEM256) != cudaSuccess) return -1;
     return 0;
 }
 
@@ -272,17 +276,23 @@ static inline int fft_pow2(double2 *buf0, double2 *buf1, int64_t N, int64_t stri
     int Ns = 1;
     for (int p = 0; p < np; ++p) {
         FftSource src = {};
-        if (p == 0 && first) src = *first;
+        const bool pack = p == 0 && first;   /* only forward transforms pack (SIGN = -1) */
+        if (pack) src = *first;
         else src.in = cur ? buf1 : buf0;
         double2 *out = cur ? buf0 : buf1;
         if (rad[p] == 256) {
             const dim3 grid((unsigned)(((N >> 8) + 15) / 16), (unsigned)nseries);
-            fft_pass256_kernel<SIGN><<<grid, 256, FFT_SMEM256, st>>>(src, out, (int)N, Ns, stride);
+            if (pack) fft_pass256_kernel<-1, true><<<grid, 256, FFT_SMEM256, st>>>(src, out, (int)N, Ns, stride);
+            else fft_pass256_kernel<SIGN, false><<<grid, 256, FFT_SMEM256, st>>>(src, out, (int)N, Ns, stride);
         } else {
             const dim3 grid((unsigned)((N / rad[p] + FFT_THREADS - 1) / FFT_THREADS), (unsigned)nseries);
-            if (rad[p] == 16) fft_pass_kernel<16, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
-            else if (rad[p] == 4) fft_pass_kernel<4, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
-            else fft_pass_kernel<2, SIGN><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            if (pack) {
+                if (rad[p] == 16) fft_pass_kernel<16, -1, true><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+                else if (rad[p] == 4) fft_pass_kernel<4, -1, true><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+                else fft_pass_kernel<2, -1, true><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            } else if (rad[p] == 16) fft_pass_kernel<16, SIGN, false><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            else if (rad[p] == 4) fft_pass_kernel<4, SIGN, false><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
+            else fft_pass_kernel<2, SIGN, false><<<grid, FFT_THREADS, 0, st>>>(src, out, (int)N, Ns, stride);
         }
         Ns *= rad[p];
         cur ^= 1;
