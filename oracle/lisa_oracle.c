@@ -27,6 +27,13 @@
  * low-frequency relation; LFA -> full as f L / c -> 0 with the x / sin x law of
  * Eq. (B4); T^LFA = 0 for equal arms; psi invariances; Eq. (4.2)/(4.4) printed
  * values 0.95 / 0.97 / 0.99; taper partition of unity.
+ * Rows added after the hot path, each pinned the same way (tests/test_oracle_*.py):
+ * extended LFA (m = 1 term of (B4): (x - x^3/6)/sin x; (B13)/(B14): first-order
+ * residual); O11 numerical orbits (polynomial trajectories exact, O1 reproduced);
+ * O12 nested delays (laser-noise cancellation only with nested TDI 2.0, brute-force
+ * chains); O13 waveform model (numpy generator, Eq. (4.2), join closed forms, the
+ * interpolating response); O14 Eq. (B20)/(B30) (second-order agreement with the exact
+ * combination of six unrelated links, (B25)/(B33) for equal constant arms).
  * Parity unpinned: absolute amplitudes of the paper's figures (no printed
  * input -> output example exists in the paper).
  */
