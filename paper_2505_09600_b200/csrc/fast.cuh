@@ -500,16 +500,17 @@ __device__ __forceinline__ void link_body(const FastParams &p, int64_t bid)
                 bulk_g2s(tl + r * LFA_TLW + (f0 - (a0 - 2)), glo + (int64_t)r * p.stride + f0, nf * 4u, &s_bar2);
             }
         }
-        for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
-            const int64_t g = rs + j;
-            if (g < g_lo || g >= g_hi) {
-                raw_p[j] = 0.0;
-                raw_c[j] = 0.0;
-            } else if (!bulk) {
-                cp_async8(raw_p + j, gp + g);
-                cp_async8(raw_c + j, gc + g);
+        if (!bulk || ncopy < nraw)   /* interior tiles (all but two per source) have nothing to fill and nothing to copy by element */
+            for (int j = tid; j < nraw; j += FAST_TA_THREADS) {
+                const int64_t g = rs + j;
+                if (g < g_lo || g >= g_hi) {
+                    raw_p[j] = 0.0;
+                    raw_c[j] = 0.0;
+                } else if (!bulk) {
+                    cp_async8(raw_p + j, gp + g);
+                    cp_async8(raw_c + j, gc + g);
+                }
             }
-        }
         /* SURVEY 8(f)-2, terms = 2: the d^3h/dt^3 numerators, parity-split like the first-derivative series */
         he3_p = reinterpret_cast<double *>(tl + LFA_LO_ROWS * LFA_TLW);
         cp_async_wait_all();
