@@ -265,7 +265,7 @@ struct FastLayout {
     size_t anc, hdr, anc2, y, lists;     /* doubles */
     size_t total;                  /* doubles, including work_doubles(batch) */
 };
-FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
+FastLayout fast_layout(int which, int64_t n, int64_t batch, int M, bool want_y = true)
 {
     FastLayout f;
     f.ntilesA = (n + FAST_TA - 1) / FAST_TA;
@@ -276,15 +276,20 @@ FastLayout fast_layout(int which, int64_t n, int64_t batch, int M)
     /* rows of link scratch per source: six full links, three derivatives of the LFA links + the three LFA links themselves
      * (written only when the caller asks for d_y) */
     const int rows = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 6 : 12;
+    const int rows_noy = which == LTDI_RESPONSE_FULL ? 6 : which == LTDI_RESPONSE_LFA ? 3 : 9;   /* without d_y */
     const size_t cap = (size_t)2048 << 20; /* bytes of scratch per chunk */
     int64_t chunk = (int64_t)(cap / ((size_t)rows * f.lds * sizeof(double)));
     f.chunk = chunk < 1 ? 1 : (chunk > batch ? batch : chunk);
+    /* the memory is sized for a call that returns the links; a call that does not fits more sources into the same scratch */
+    const int64_t chunk_noy = std::min<int64_t>(batch, (int64_t)(((size_t)rows * f.chunk) / rows_noy));
+    const int64_t chunk_y = f.chunk;
     f.anc = (size_t)f.ntilesN * FAST_NA * FAST_ANC_DOUBLES(M);
     f.hdr = (size_t)f.ntilesN * FAST_NA * 4;
     f.anc2 = (size_t)f.ntilesN * FAST_NA * M;   /* second derivative of the weights (second-order instances) */
-    f.y = (size_t)rows * f.chunk * f.lds;
+    f.y = (size_t)rows * chunk_y * f.lds;
     /* hybrid: link tiles of both kinds, LFA-only blocks, blend blocks, full-only 224-sample tiles (int2 each) */
-    f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)f.chunk * (f.ntilesA + f.ntilesAL + 4 * f.ntilesN) : 0;
+    f.lists = which == LTDI_RESPONSE_HYBRID ? (size_t)chunk_noy * (f.ntilesA + f.ntilesAL + 4 * f.ntilesN) : 0;
+    if (!want_y) f.chunk = chunk_noy;
     f.total = work_doubles(batch) + f.anc + f.hdr + f.anc2 + f.y + f.lists;
     return f;
 }
@@ -515,7 +520,7 @@ int run_fast(DeviceState &ds, const RespParams &rp, const Margins &mg, const ltd
 {
     constexpr int H = M / 2;
     const ltdi_orbit_desc &d = orb->desc;
-    const FastLayout lay = fast_layout(which, d.n, rp.batch, M);
+    const FastLayout lay = fast_layout(which, d.n, rp.batch, M, rp.Y != nullptr);
     if (mg.m2 > 4096 || mg.m1 > 8192) return LTDI_EUNSUPPORTED;
 
     FastParams p;
@@ -738,7 +743,7 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     HybHost hh;
     const bool plan_hybrid = which == LTDI_RESPONSE_HYBRID && fast_order(order) && mg.m2 <= 4096 && mg.m1 <= 8192;
     if (plan_hybrid) {
-        rc = build_hybrid_plan(d, mg, M, fast_layout(which, d.n, batch, M), batch, h_hyb, n_hyb, &hh);
+        rc = build_hybrid_plan(d, mg, M, fast_layout(which, d.n, batch, M, d_y != nullptr), batch, h_hyb, n_hyb, &hh);
         if (rc) return rc;
     }
 
