@@ -280,6 +280,17 @@ class Oracle:
             raise ValueError(f"oracle waveform_chirp: status {rc}")
         return hp, hc
 
+    def waveform_ecc(self, tables, params, nharm, t0, dt, n):
+        """O13b: the eccentric harmonic-sum model (tables [batch][7][nk], params [batch][6]) sampled on t0 + i dt."""
+        tab, par = _f64(tables), _f64(params)
+        batch, _, nk = tab.shape
+        hp, hc = np.zeros((batch, n)), np.zeros((batch, n))
+        rc = self.lib.orc_waveform_ecc(_ptr(tab), C.c_int64(nk), _ptr(par), C.c_int(nharm), C.c_int64(batch), C.c_double(t0),
+                                       C.c_double(dt), C.c_int64(n), C.c_int64(n), _ptr(hp), _ptr(hc))
+        if rc != 0:
+            raise ValueError(f"oracle waveform_ecc: status {rc}")
+        return hp, hc
+
     def response_full_chirp(self, orbit, params, sources, gen, order, nb=0, ne=None, want=("XYZ", "y")):
         """O13: Eq. (2.5) with the model evaluated at the retarded times, then O6 / O7."""
         batch = len(params)

@@ -37,6 +37,7 @@
  * Parity unpinned: absolute amplitudes of the paper's figures (no printed
  * input -> output example exists in the paper).
  */
+#define _DEFAULT_SOURCE /* jn, jnl (Bessel functions of the first kind) with -std=c11 */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -51,6 +52,7 @@ typedef long double real;
 #define R_EXP expl
 #define R_POW powl
 #define R_PI 3.14159265358979323846264338327950288L
+#define R_JN jnl
 #else
 typedef double real;
 #define R_SIN sin
@@ -60,6 +62,7 @@ typedef double real;
 #define R_EXP exp
 #define R_POW pow
 #define R_PI 3.14159265358979323846
+#define R_JN jn
 #endif
 
 #define ORC_OK 0
@@ -1362,6 +1365,72 @@ int orc_waveform_chirp(const orc_chirp *w, int64_t batch, double t0, double dt, 
         for (int64_t i = 0; i < n; ++i) {
             real a, c;
             chirp_at(&w[b], (real)t0 + (real)i * (real)dt, &a, &c);
+            hp[b * ld + i] = (double)a;
+            hc[b * ld + i] = (double)c;
+        }
+    }
+    return ORC_OK;
+}
+
+/* O13b: the harmonic-sum waveform of an eccentric inspiral (the input recipe of config 5, as a MODEL):
+ * the orbital evolution table F, e, l and their time derivatives at nk knots (tab [7][nk]: t, F, e, l, dF/dt, de/dt,
+ * dl/dt) is carried to time t by cubic Hermite interpolation on the knot interval that contains t, then
+ *   h+ = sum_n [ -(1 + cos^2 iota)(a_n cos 2 gamma - b_n sin 2 gamma) + (1 - cos^2 iota) c_n ]
+ *   hx = sum_n 2 cos iota (b_n cos 2 gamma + a_n sin 2 gamma),                                  n = 1 .. nharm
+ *   a_n = -n A [J_{n-2} - 2 e J_{n-1} + (2 / n) J_n + 2 e J_{n+1} - J_{n+2}](n e) cos(n l)
+ *   b_n = -n A sqrt(1 - e^2) [J_{n-2} - 2 J_n + J_{n+2}](n e) sin(n l),     c_n = 2 A J_n(n e) cos(n l)
+ *   A = (2 pi F M)^(2/3) eta M c / d_L          (Peters & Mathews 1963 in the form of Barack & Cutler 2004, Eqs. 7-9)
+ * par [6] = M [s], eta, d_L [m], cos iota, gamma, l0. */
+static real hermite_at(const double *tk, const double *yk, const double *dyk, int64_t idx, real t)
+{
+    const real h = (real)tk[idx + 1] - (real)tk[idx];
+    const real u = (t - (real)tk[idx]) / h;
+    const real h00 = (1 + 2 * u) * (1 - u) * (1 - u), h10 = u * (1 - u) * (1 - u);
+    const real h01 = u * u * (3 - 2 * u), h11 = u * u * (u - 1);
+    return h00 * (real)yk[idx] + h10 * h * (real)dyk[idx] + h01 * (real)yk[idx + 1] + h11 * h * (real)dyk[idx + 1];
+}
+
+static void ecc_at(const double *tab, int64_t nk, const double *par, int nharm, real t, real *hp, real *hc)
+{
+    const double *tk = tab;
+    int64_t lo = 0, hi = nk;                      /* upper bound: first knot > t */
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) / 2;
+        if ((real)tk[mid] <= t) lo = mid + 1; else hi = mid;
+    }
+    int64_t idx = lo - 1;
+    if (idx < 0) idx = 0;
+    if (idx > nk - 2) idx = nk - 2;
+    const real F = hermite_at(tk, tab + nk, tab + 4 * nk, idx, t);
+    const real e = hermite_at(tk, tab + 2 * nk, tab + 5 * nk, idx, t);
+    const real ell = hermite_at(tk, tab + 3 * nk, tab + 6 * nk, idx, t) + (real)par[5];
+    const real M = par[0], eta = par[1], ci = par[3], gam = par[4];
+    const real A = R_POW(2 * R_PI * F * M, (real)2 / 3) * eta * M * (real)ORC_C_LIGHT / (real)par[2];
+    const real c2g = R_COS(2 * gam), s2g = R_SIN(2 * gam), ci2 = ci * ci, sq = R_SQRT(1 - e * e);
+    real sp = 0, sc = 0;
+    for (int n = 1; n <= nharm; ++n) {
+        const real x = n * e, cn = R_COS(n * ell), sn = R_SIN(n * ell);
+        const real jm2 = R_JN(n - 2, x), jm1 = R_JN(n - 1, x), j0 = R_JN(n, x), jp1 = R_JN(n + 1, x), jp2 = R_JN(n + 2, x);
+        const real an = -n * A * (jm2 - 2 * e * jm1 + ((real)2 / n) * j0 + 2 * e * jp1 - jp2) * cn;
+        const real bn = -n * A * sq * (jm2 - 2 * j0 + jp2) * sn;
+        const real cc = 2 * A * j0 * cn;
+        sp += -(1 + ci2) * (an * c2g - bn * s2g) + (1 - ci2) * cc;
+        sc += 2 * ci * (bn * c2g + an * s2g);
+    }
+    *hp = sp;
+    *hc = sc;
+}
+
+/* the model sampled on t0 + i dt: tab [batch][7][nk], par [batch][6]; hp, hc [batch][ld] */
+int orc_waveform_ecc(const double *tab, int64_t nk, const double *par, int nharm, int64_t batch, double t0, double dt,
+                     int64_t n, int64_t ld, double *hp, double *hc)
+{
+    if (!tab || !par || !hp || !hc || nk < 2 || nharm < 1 || batch < 1 || n < 1 || ld < n || !(dt > 0)) return ORC_EINVAL;
+    for (int64_t b = 0; b < batch; ++b) {
+#pragma omp parallel for
+        for (int64_t i = 0; i < n; ++i) {
+            real a, c;
+            ecc_at(tab + b * 7 * nk, nk, par + 6 * b, nharm, (real)t0 + (real)i * (real)dt, &a, &c);
             hp[b * ld + i] = (double)a;
             hc[b * ld + i] = (double)c;
         }

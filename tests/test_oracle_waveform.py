@@ -86,3 +86,70 @@ def test_projection_at_retarded_times_equals_the_interpolated_one(orc80, k, gen)
     if n_join < cfg["n"]:   # and near the join the two differ by the interpolation error of the kink: the reason O13 is its own oracle
         near = slice(n_join - 110, n_join + 110)   # k.R / c shifts the join by up to 100 samples either way
         assert np.abs(fused["y"] - sampled["y"])[..., near].max() > 1e-6 * np.abs(sampled["y"][..., near]).max()
+
+
+# ---- O13b: the harmonic-sum waveform of an eccentric inspiral (config 5's recipe as a model) ---------------------------
+
+def test_eccentric_model_equals_the_input_generator(orc80):
+    cfg = W.config(5, n=30000, batch=2)
+    for idx in (0, 1):
+        hp, hc, _, _ = W.source(cfg, idx)
+        tab, par = W.ecc_params(cfg, idx)
+        a, c = orc80.waveform_ecc(tab[None], par[None], 10, cfg["orbit"]["t0"], cfg["dt"], cfg["n"])
+        assert np.abs(a[0] - hp).max() <= 2e-12 * np.abs(hp).max()
+        assert np.abs(c[0] - hc).max() <= 2e-12 * np.abs(hc).max()
+
+
+def _table(tk, F, dF, e, de, ell, dell):
+    return np.array([tk, F, e, ell, dF, de, dell])
+
+
+def test_circular_limit_and_hermite_exactness(orc80):
+    """e = 0: only n = 2 survives, h+ = 2 A (1 + cos^2 iota) cos(2 l + 2 gamma), hx = -4 A cos iota sin(2 l + 2 gamma); F and l
+    cubic in time: the Hermite interpolation between the knots is exact"""
+    tk = np.linspace(0.0, 4.0e4, 9)                      # 5000 s between knots
+    s = tk / 4.0e4
+    F = 1.0e-3 * (1 + 0.3 * s + 0.2 * s ** 2 + 0.1 * s ** 3)
+    dF = 1.0e-3 * (0.3 + 0.4 * s + 0.3 * s ** 2) / 4.0e4
+    ell = 2 * math.pi * 1.0e-3 * 4.0e4 * (s + 0.15 * s ** 2 + 0.2 / 3 * s ** 3)
+    dell = 2 * math.pi * 1.0e-3 * (1 + 0.3 * s + 0.2 * s ** 2)
+    M, eta, dist, ci, gam, l0 = 5.0, 0.2, 1.0e25, 0.37, 0.9, 0.4
+    tab = _table(tk, F, dF, 0 * tk, 0 * tk, ell, dell)
+    n, dt, t0 = 3000, 11.0, 777.0
+    hp, hc = orc80.waveform_ecc(tab[None], np.array([[M, eta, dist, ci, gam, l0]]), 10, t0, dt, n)
+    t = t0 + dt * np.arange(n)
+    st = t / 4.0e4
+    Ft = 1.0e-3 * (1 + 0.3 * st + 0.2 * st ** 2 + 0.1 * st ** 3)
+    lt = 2 * math.pi * 1.0e-3 * 4.0e4 * (st + 0.15 * st ** 2 + 0.2 / 3 * st ** 3) + l0
+    A = (2 * math.pi * Ft * M) ** (2.0 / 3.0) * eta * M * 299792458.0 / dist
+    want_p = 2 * A * (1 + ci * ci) * np.cos(2 * lt + 2 * gam)
+    want_c = -4 * A * ci * np.sin(2 * lt + 2 * gam)
+    assert np.abs(hp[0] - want_p).max() <= 1e-12 * np.abs(want_p).max()
+    assert np.abs(hc[0] - want_c).max() <= 1e-12 * np.abs(want_p).max()
+
+
+@pytest.mark.parametrize("e", [0.1, 0.3, 0.5])
+def test_peters_mathews_power_sum(orc80, e):
+    """the harmonic amplitudes, read off the model's own output by a Fourier analysis over one orbit, satisfy the classic sum
+    sum_n g(n, e) = (1 + 73/24 e^2 + 37/96 e^4) / (1 - e^2)^(7/2), g = n^2 / 32 [a_n^2 + b_n^2 + c_n^2 / 3] in units of A"""
+    nh, F0, N = 40, 1.0e-3, 512
+    P = 1.0 / F0
+    tk = np.array([-P, 0.0, P, 2 * P, 3 * P])
+    one = np.ones_like(tk)
+    tab = _table(tk, F0 * one, 0 * one, e * one, 0 * one, 2 * math.pi * F0 * tk, 2 * math.pi * F0 * one)
+    M, eta, dist = 5.0, 0.2, 1.0e25
+    A = (2 * math.pi * F0 * M) ** (2.0 / 3.0) * eta * M * 299792458.0 / dist
+    dt = P / N
+
+    def harmonics(ci):
+        hp, hc = orc80.waveform_ecc(tab[None], np.array([[M, eta, dist, ci, 0.0, 0.0]]), nh, 0.0, dt, N)
+        return 2 * np.fft.rfft(hp[0]).real[1:nh + 1] / N / A, -2 * np.fft.rfft(hc[0]).imag[1:nh + 1] / N / A
+
+    p1, q1 = harmonics(1.0)          # h+ = -2 a_n cos(n l),  hx = 2 b_n sin(n l)
+    p0, _ = harmonics(0.0)           # h+ = (-a_n + c_n) cos(n l)
+    a, b = -p1 / 2, q1 / 2
+    c = p0 + a
+    n = np.arange(1, nh + 1)
+    g = n ** 2 / 32.0 * (a ** 2 + b ** 2 + c ** 2 / 3.0)
+    want = (1 + 73.0 / 24 * e ** 2 + 37.0 / 96 * e ** 4) / (1 - e ** 2) ** 3.5
+    assert abs(g.sum() / want - 1.0) < 1e-9, (e, g.sum(), want)

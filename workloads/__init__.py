@@ -92,15 +92,14 @@ def _peters_rhs(F, e, M_s, eta):
     return 96.0 / 5.0 * k * F * fe1, -304.0 / 15.0 * k * e * fe2
 
 
-def eccentric_harmonics(t, t_end, tau_end, M_s, q, e0, dist_m, cos_iota, gamma, l0, nharm=10, knots=1536):
-    """h+, hx = sum over harmonics n = 1..nharm of the orbital phase with Peters-Mathews
-    quadrupole amplitudes (Peters & Mathews 1963 harmonic decomposition in the form of Barack &
-    Cutler 2004, Eqs. 7-9); F(t), e(t) from the orbit-averaged Peters (1964) equations, integrated
-    backwards from the end of the segment (RK4 on a grid uniform in log time-to-coalescence) and
-    carried to the samples by cubic Hermite interpolation."""
+def eccentric_knots(t_first, t_end, tau_end, M_s, q, e0, knots=1536):
+    """The orbital evolution table of an eccentric inspiral: F(t), e(t), l(t) and their time derivatives at `knots` times
+    (uniform in log time-to-coalescence), from the orbit-averaged Peters (1964) equations integrated backwards from the
+    end of the segment with RK4.  Returns (tk, Fk, ek, lk, dFk, dek, dlk), tk increasing.  Input data: the table plays
+    the role of a waveform-model parameter set for the rows that generate the strain themselves."""
     eta = q / (1.0 + q) ** 2
     mc_s = M_s * eta ** 0.6
-    T_seg = t_end - t[0]
+    T_seg = t_end - t_first
     F_end = 0.5 * f_of_tau(tau_end, mc_s)
     F_start_c = 0.5 * f_of_tau(tau_end + T_seg, mc_s)
     e_end = e0 * (F_start_c / F_end) ** (19.0 / 18.0)
@@ -126,6 +125,16 @@ def eccentric_harmonics(t, t_end, tau_end, M_s, q, e0, dist_m, cos_iota, gamma, 
     tk, Fk, ek, lk = tk[::-1].copy(), Fk[::-1].copy(), ek[::-1].copy(), lk[::-1].copy()
     dFk, dek = _peters_rhs(Fk, ek, M_s, eta)
     dlk = 2.0 * math.pi * Fk
+    return tk, Fk, ek, lk, dFk, dek, dlk
+
+
+def eccentric_harmonics(t, t_end, tau_end, M_s, q, e0, dist_m, cos_iota, gamma, l0, nharm=10, knots=1536):
+    """h+, hx = sum over harmonics n = 1..nharm of the orbital phase with Peters-Mathews
+    quadrupole amplitudes (Peters & Mathews 1963 harmonic decomposition in the form of Barack &
+    Cutler 2004, Eqs. 7-9); F(t), e(t), l(t) from eccentric_knots(), carried to the samples by cubic
+    Hermite interpolation."""
+    eta = q / (1.0 + q) ** 2
+    tk, Fk, ek, lk, dFk, dek, dlk = eccentric_knots(t[0], t_end, tau_end, M_s, q, e0, knots)
 
     def hermite(yk, dyk):
         idx = np.clip(np.searchsorted(tk, t, side="right") - 1, 0, knots - 2)
@@ -292,6 +301,20 @@ def chirp_params(cfg, idx):
         t_c = t_end + 2.0 * DAY_S if k == 1 else t_first + 2.0 * 365.0 * DAY_S
         out.update(t_c=t_c, tau_cut=tau_cut, f_rd=f_of_tau(tau_cut, mc), tau_rd=1.0)
     return out
+
+
+def ecc_params(cfg, idx):
+    """Orbital evolution table [7][nk] and scalars (M_s, eta, dist_m, cos_iota, gamma, l0) of source `idx` of config 5:
+    what source() feeds to eccentric_harmonics, for the rows that generate the strain themselves."""
+    assert cfg["k"] == 5
+    n, dt = cfg["n"], cfg["dt"]
+    t_first = cfg["orbit"]["t0"]
+    t_end = t_first + dt * (n - 1) + dt
+    p = draw(cfg, idx)
+    M_s = p["M"] * GMSUN_S
+    table = np.array(eccentric_knots(t_first, t_end, p["tau_end"], M_s, p["q"], p["e0"]))
+    eta = p["q"] / (1.0 + p["q"]) ** 2
+    return table, np.array([M_s, eta, p["dist"], p["cos_iota"], p["gamma"], p["phi_c"]])
 
 
 def _tau_cut(mc_s, rd):
