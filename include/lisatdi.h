@@ -192,6 +192,22 @@ typedef struct {
 int ltdi_waveform_chirp(const ltdi_chirp *h_wav, int64_t batch, double t0, double dt, int64_t n, int64_t ld,
                         double *d_hp, double *d_hc, void *d_work, size_t work_bytes, void *stream);
 
+/* The harmonic-sum waveform of an eccentric inspiral (the recipe of BASELINE.json config 5 as a model) on t0 + i dt, i < n:
+ * d_tab [batch][7][nk] (device) is the orbital evolution table of every source -- knot times t_k (increasing), orbital
+ * frequency F, eccentricity e, mean anomaly l and dF/dt, de/dt, dl/dt at the knots --, carried to the sample time by cubic
+ * Hermite interpolation on the knot interval that contains it (the first / last interval outside the table); then
+ *   h+ = sum_n [ -(1 + cos^2 iota)(a_n cos 2 gamma - b_n sin 2 gamma) + (1 - cos^2 iota) c_n ],
+ *   hx = sum_n 2 cos iota (b_n cos 2 gamma + a_n sin 2 gamma),   n = 1 .. nharm (<= 64),
+ *   a_n = -n A [J_{n-2} - 2 e J_{n-1} + (2 / n) J_n + 2 e J_{n+1} - J_{n+2}](n e) cos(n l),
+ *   b_n = -n A sqrt(1 - e^2) [J_{n-2} - 2 J_n + J_{n+2}](n e) sin(n l),   c_n = 2 A J_n(n e) cos(n l),
+ *   A = (2 pi F M)^(2/3) eta M c / d_L   (Peters & Mathews harmonics in the form of Barack & Cutler 2004, Eqs. 7-9; App. F of
+ * the paper uses eccentric signals of this kind).  h_par [batch][6] (host): M = G M_tot / c^3 [s], eta, d_L [m], cos iota,
+ * gamma, l0.  n e must stay below 8 (power series of the Bessel functions).  d_hp, d_hc [batch][ld] (device);
+ * d_work: >= 64 bytes per source, 16-byte aligned. */
+int ltdi_waveform_ecc(const double *d_tab, int64_t nk, const double *h_par, int nharm, int64_t batch, double t0,
+                      double dt, int64_t n, int64_t ld, double *d_hp, double *d_hc, void *d_work, size_t work_bytes,
+                      void *stream);
+
 /* Full response straight from the model parameters: Eq. (2.5) with h+, hx EVALUATED at the retarded times t - delta_s,
  * t - delta_r (no sampled strain is read and the first interpolation level is gone), then Eq. (2.7) / (2.8) and (2.9) as
  * ltdi_response_full.  h_wav [batch]; ld = row stride of the outputs (>= n); Lagrange orders 9 and 31 (the order only

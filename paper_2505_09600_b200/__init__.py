@@ -92,6 +92,8 @@ _SIGNATURES = {
                                             _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_waveform_chirp": (C.c_int, [C.POINTER(Chirp), C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64, _dp, _dp, _vp,
                                       C.c_size_t, _vp]),
+    "ltdi_waveform_ecc": (C.c_int, [_dp, C.c_int64, _dp, C.c_int, C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64, _dp, _dp,
+                                    _vp, C.c_size_t, _vp]),
     "ltdi_response_full_chirp": (C.c_int, [_vp, C.POINTER(Chirp), C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                            _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_lfa": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
@@ -378,6 +380,23 @@ def waveform_chirp(params, t0, dt, n, device="cuda:0", out=None):
     with torch.cuda.device(dev):
         _check("ltdi_waveform_chirp", lib().ltdi_waveform_chirp(_chirps(params), batch, float(t0), float(dt), int(n), int(hp.shape[1]),
                                                                 hp.data_ptr(), hc.data_ptr(), work.data_ptr(), work.numel() * 8, _stream()))
+    return hp, hc
+
+
+def waveform_ecc(tables, params, nharm, t0, dt, n, out=None):
+    """the eccentric harmonic-sum model on the device.  tables: float64 CUDA tensor [batch][7][nk] (t, F, e, l and
+    their time derivatives at the knots); params: host array [batch][6] (M_s, eta, dist_m, cos_iota, gamma, l0).
+    Returns hp, hc [batch][n] device tensors (ltdi_waveform_ecc)."""
+    tab = _dev_f64(tables, "tables")
+    batch, seven, nk = tab.shape
+    assert seven == 7
+    par = torch.as_tensor(params, dtype=torch.float64, device="cpu").reshape(batch, 6).contiguous()
+    hp, hc = out if out is not None else (torch.empty(batch, n, dtype=torch.float64, device=tab.device) for _ in range(2))
+    work = torch.empty(batch * 8, dtype=torch.float64, device=tab.device)
+    with torch.cuda.device(tab.device):
+        _check("ltdi_waveform_ecc", lib().ltdi_waveform_ecc(tab.data_ptr(), int(nk), par.data_ptr(), int(nharm), batch, float(t0), float(dt),
+                                                            int(n), int(hp.shape[1]), hp.data_ptr(), hc.data_ptr(), work.data_ptr(),
+                                                            work.numel() * 8, _stream()))
     return hp, hc
 
 

@@ -460,6 +460,15 @@ int upload_chirps(const ltdi_chirp *h_wav, int64_t batch, double t0, ChirpDev *d
     return LTDI_OK;
 }
 
+/* constants of the eccentric model of `batch` sources to the device, as kernel arguments in slices */
+#define LTDI_ECC_SLICE 256
+struct EccArgs { EccDev v[LTDI_ECC_SLICE]; };
+__global__ void unpack_ecc_kernel(const __grid_constant__ EccArgs a, int count, EccDev *out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count * LTDI_ECC_STRIDE) reinterpret_cast<double *>(out)[i] = reinterpret_cast<const double *>(a.v)[i];
+}
+
 /* host side of the hybrid plan: per-source plans (offsets relative to the source's chunk) and per-chunk totals */
 struct ChunkTotals { int64_t link_full, link_lfa, lfa, blend, full, max_slots; };
 struct HybHost {
@@ -1101,6 +1110,33 @@ int ltdi_waveform_chirp(const ltdi_chirp *h_wav, int64_t batch, double t0, doubl
     const int rc = upload_chirps(h_wav, batch, t0, (ChirpDev *)d_work, st);
     if (rc) return rc;
     chirp_grid_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)batch), 256, 0, st>>>((const ChirpDev *)d_work, dt, n, ld, d_hp, d_hc);
+    count_launch();
+    LTDI_CUDA_OK(cudaGetLastError());
+    return LTDI_OK;
+}
+
+int ltdi_waveform_ecc(const double *d_tab, int64_t nk, const double *h_par, int nharm, int64_t batch, double t0, double dt,
+                      int64_t n, int64_t ld, double *d_hp, double *d_hc, void *d_work, size_t work_bytes, void *stream)
+{
+    if (!d_tab || !h_par || !d_hp || !d_hc || !d_work || nk < 2 || nharm < 1 || nharm > 64 || batch < 1 || batch > 65535 ||
+        n < 1 || ld < n || !(dt > 0.0))
+        return LTDI_EINVAL;
+    if (work_bytes < (size_t)batch * sizeof(EccDev)) return LTDI_EWORKSPACE;
+    if ((uintptr_t)d_work % 16) return LTDI_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    EccDev *d_wav = (EccDev *)d_work;
+    EccArgs *a = new (std::nothrow) EccArgs;
+    if (!a) return LTDI_EINVAL;
+    for (int64_t b0 = 0; b0 < batch; b0 += LTDI_ECC_SLICE) {
+        const int cnt = (int)std::min<int64_t>(LTDI_ECC_SLICE, batch - b0);
+        for (int i = 0; i < cnt; ++i)
+            if (ecc_fill(h_par + 6 * (b0 + i), &a->v[i])) { delete a; return LTDI_EINVAL; }
+        unpack_ecc_kernel<<<(cnt * LTDI_ECC_STRIDE + 127) / 128, 128, 0, st>>>(*a, cnt, d_wav + b0);
+        count_launch();
+        if (cudaGetLastError() != cudaSuccess) { delete a; return LTDI_ECUDA; }
+    }
+    delete a;
+    ecc_grid_kernel<<<dim3((unsigned)((n + 127) / 128), (unsigned)batch), 128, 0, st>>>(d_tab, nk, d_wav, nharm, t0, dt, n, ld, d_hp, d_hc);
     count_launch();
     LTDI_CUDA_OK(cudaGetLastError());
     return LTDI_OK;

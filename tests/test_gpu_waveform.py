@@ -80,3 +80,67 @@ def test_chirp_argument_errors(ltdi):
         ltdi.response_full_chirp(orb, par, ang, 20, 7)      # tuned orders only
     with pytest.raises(ltdi.LtdiError):
         ltdi.waveform_chirp([dict(par[0], tau_rd=-1.0)], 0.0, 5.0, 100)
+
+
+@pytest.mark.parametrize("n,nharm", [(40001, 10), (262147, 6)])
+def test_eccentric_model_on_the_grid(ltdi, orc80, n, nharm):
+    """the harmonic-sum model (orbital evolution table + cubic Hermite + Bessel coefficients, ltdi_waveform_ecc) against O13b,
+    element by element: roundings of the sum of nharm harmonics, plus the oracle's own 2^-64 rounding of the mean anomaly
+    times the harmonic number"""
+    cfg = W.config(5, n=n, batch=3)
+    idx = list(range(cfg["batch"]))
+    tabs, pars = zip(*[W.ecc_params(cfg, i) for i in idx])
+    tab, par = np.stack(tabs), np.stack(pars)
+    hp, hc = ltdi.waveform_ecc(torch.as_tensor(tab, device="cuda"), par, nharm, cfg["orbit"]["t0"], cfg["dt"], cfg["n"])
+    torch.cuda.synchronize()
+    rp, rc = orc80.waveform_ecc(tab, par, nharm, cfg["orbit"]["t0"], cfg["dt"], cfg["n"])
+    for b in idx:
+        env = np.maximum.accumulate(np.abs(rp[b]) + np.abs(rc[b]))
+        env = np.maximum(env, env[-1] * 1e-300)
+        ep = np.abs(hp[b].cpu().numpy() - rp[b]) / env
+        ec = np.abs(hc[b].cpu().numpy() - rc[b]) / env
+        l_max = np.abs(tab[b, 3]).max() + abs(par[b, 5])
+        bar = 8e-15 + nharm * 2.0 ** -62 * l_max
+        record(series="h_ecc", label=["cfg5", "nharm%d" % nharm, "source", str(b)], err=float(max(ep.max(), ec.max())), bar=bar)
+        assert max(ep.max(), ec.max()) <= bar, (b, ep.max(), ec.max(), bar, l_max)
+
+
+def test_eccentric_model_outside_the_table_and_errors(ltdi, orc80):
+    """sample times before the first and after the last knot use the end intervals, as O13b does; bad arguments are refused"""
+    cfg = W.config(5, n=20001, batch=1)
+    tab, par = W.ecc_params(cfg, 0)
+    t0 = tab[0, 0] - 12 * cfg["dt"]                # under one knot interval out: the cubic is still well conditioned
+    n = 1200
+    hp, hc = ltdi.waveform_ecc(torch.as_tensor(tab[None], device="cuda"), par[None], 8, t0, cfg["dt"], n)
+    rp, rc = orc80.waveform_ecc(tab[None], par[None], 8, t0, cfg["dt"], n)
+    scale = np.abs(rp).max() + np.abs(rc).max()
+    assert np.abs(hp.cpu().numpy() - rp).max() <= 1e-13 * scale and np.abs(hc.cpu().numpy() - rc).max() <= 1e-13 * scale
+    t_last = tab[0, -1] - 388 * cfg["dt"]
+    hp, hc = ltdi.waveform_ecc(torch.as_tensor(tab[None], device="cuda"), par[None], 8, t_last, cfg["dt"], 400)
+    rp, rc = orc80.waveform_ecc(tab[None], par[None], 8, t_last, cfg["dt"], 400)
+    assert np.abs(hp.cpu().numpy() - rp).max() <= 1e-13 * scale and np.abs(hc.cpu().numpy() - rc).max() <= 1e-13 * scale
+    dtab = torch.as_tensor(tab[None], device="cuda")
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.waveform_ecc(dtab, par[None], 0, t0, cfg["dt"], n)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.waveform_ecc(dtab, par[None], 65, t0, cfg["dt"], n)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.waveform_ecc(dtab, np.array([[0.0, 0.2, 1e25, 0.3, 0.1, 0.2]]), 8, t0, cfg["dt"], n)
+    with pytest.raises(ltdi.LtdiError):
+        ltdi.waveform_ecc(dtab[:, :, :1].contiguous(), par[None], 8, t0, cfg["dt"], n)
+
+
+def test_eccentric_model_feeds_the_response(ltdi, orc80):
+    """the strain generated on the device goes straight into the full response (no host copy): A, E, T against the oracle's
+    response of the oracle's own strain, at the bar of the hot path"""
+    cfg = W.config(5, n=30001, batch=2)
+    tabs, pars = zip(*[W.ecc_params(cfg, i) for i in range(2)])
+    tab, par = np.stack(tabs), np.stack(pars)
+    ang = np.array([W.source(dict(cfg, n=16), i)[2] for i in range(2)])
+    hp, hc = ltdi.waveform_ecc(torch.as_tensor(tab, device="cuda"), par, 10, cfg["orbit"]["t0"], cfg["dt"], cfg["n"])
+    orb = ltdi.Orbits(cfg["orbit"])
+    out = to_numpy(ltdi.response_full(orb, hp, hc, ang, 20, 31, True, True))
+    rp, rc = orc80.waveform_ecc(tab, par, 10, cfg["orbit"]["t0"], cfg["dt"], cfg["n"])
+    ref = orc80.response_full(cfg["orbit"], rp, rc, ang, 20, 31)
+    lo, hi = orc80.margins(cfg["orbit"], 20, 31, 0)
+    strict_check(out, ref, lo, hi, cfg["n"])
