@@ -180,6 +180,17 @@ class Oracle:
         assert rc == 0
         return out
 
+    def sagnac_from_links(self, orbit, y, gen, order):
+        """O15: alpha, beta, gamma [3][n] from caller-supplied link series y [6][n]."""
+        y = _f64(y)
+        assert y.shape == (6, orbit["n"])
+        out = np.zeros((3, orbit["n"]))
+        d = self._desc(orbit)
+        Rt, Lt = self._tables(orbit)
+        rc = self.lib.orc_sagnac_from_links(C.byref(d), _ptr(Rt), _ptr(Lt), _ptr(y), C.c_int(gen), C.c_int(order), _ptr(out))
+        assert rc == 0
+        return out
+
     def antenna(self, orbit, source, n):
         out = np.zeros((6, 3))
         d = self._desc(orbit)
@@ -215,6 +226,8 @@ class Oracle:
                 _ptr(out["XYZ"]), _ptr(out["y"])]
         if which == "full":
             rc = self.lib.orc_response_full(*head, *tail)
+        elif which == "sagnac":
+            rc = self.lib.orc_response_full_sagnac(*head, *tail)
         elif which == "lfa":
             rc = self.lib.orc_response_lfa(*head, C.c_int(fd_order), *tail)
         else:
@@ -229,6 +242,10 @@ class Oracle:
 
     def response_full(self, orbit, hp, hc, sources, gen, order, nb=0, ne=None, want=("XYZ", "y")):
         return self._run("full", orbit, hp, hc, sources, gen, order, 0, None, nb, ne, want)
+
+    def response_full_sagnac(self, orbit, hp, hc, sources, gen, order, nb=0, ne=None, want=("XYZ", "y")):
+        """O15: the full response in the Sagnac combinations; out["XYZ"] holds alpha, beta, gamma."""
+        return self._run("sagnac", orbit, hp, hc, sources, gen, order, 0, None, nb, ne, want)
 
     def response_full_nested(self, orbit, hp, hc, sources, gen, order, nested_order=3, nb=0, ne=None, want=("XYZ", "y")):
         """the full response with properly nested TDI delays (O12); nested_order = Lagrange order of the

@@ -33,7 +33,12 @@
  * O12 nested delays (laser-noise cancellation only with nested TDI 2.0, brute-force
  * chains); O13 waveform model (numpy generator, Eq. (4.2), join closed forms, the
  * interpolating response); O14 Eq. (B20)/(B30) (second-order agreement with the exact
- * combination of six unrelated links, (B25)/(B33) for equal constant arms).
+ * combination of six unrelated links, (B25)/(B33) for equal constant arms);
+ * O13b eccentric harmonic sums (numpy generator, circular limit, Peters-Mathews power
+ * sum g(n, e)); O15 Sagnac alpha, beta, gamma (laser noise cancels in the 6-term form
+ * iff the round trips agree and in the 12-term form for any constant L_l != L_-l, with
+ * the residual in closed form; beams walked by spacecraft number; the operator identity
+ * (1 - D^2)(1 - D) sum(alpha) = -(1 + D + D^2) sum(X) for equal arms).
  * Parity unpinned: absolute amplitudes of the paper's figures (no printed
  * input -> output example exists in the paper).
  */
@@ -512,6 +517,35 @@ static real michelson_at(const yseries_t *ys, const real Lsec[6], int ch, int ge
     return X;
 }
 
+/* O15 Sagnac-type combinations alpha, beta, gamma ("Sagnac-type observables emulate the interference
+ * pattern generated by photons propagating in clockwise and counterclockwise directions around the constellation"; the
+ * paper prints no equation for them -- reading G33 -- so the textbook definition is written out in the link labelling of
+ * P:81, where link +1 runs 3 -> 2, +2: 1 -> 3, +3: 2 -> 1 and -1: 2 -> 3, -2: 3 -> 1, -3: 1 -> 2).
+ * The beam that leaves spacecraft 1, goes round 1 -> 3 -> 2 -> 1 and is read at t, and the one going round 1 -> 2 -> 3 -> 1:
+ *     S+ = y_{+3} + D_{+3} y_{+1} + D_{+3} D_{+1} y_{+2},          S- = y_{-2} + D_{-2} y_{-1} + D_{-2} D_{-1} y_{-3}
+ * In laser-noise terms y_l(t) = p_s(t - L_l) - p_r(t) each telescopes to p_1(t - T+-) - p_1(t) with the round-trip times
+ * T+ = L_3 + L_1 + L_2, T- = L_-2 + L_-1 + L_-3.  Then
+ *     gen 1.5:  alpha = S+ - S-                                     (6 terms; free of laser noise where T+ = T-)
+ *     gen 2.0:  alpha = (S+ + D_{T+} S-) - (S- + D_{T-} S+)         (12 terms; free of laser noise for any constant L_l != L_-l)
+ * beta, gamma by the cyclic permutation 1 -> 2 -> 3 -> 1 of the link labels.  Every delay is evaluated at t, as in
+ * O6, so the operators commute and a product of delays is the sum of the light times. */
+static real sagnac_at(const yseries_t *ys, const real Lsec[6], int ch, int gen, int64_t n, real dt, int order)
+{
+    const int c3 = cyc(3, ch), c1 = cyc(1, ch), c2 = cyc(2, ch);   /* the links +3, +1, +2 of alpha, permuted */
+    const real Lp3 = Lsec[link_index(c3)], Lp1 = Lsec[link_index(c1)], Lp2 = Lsec[link_index(c2)];
+    const real Lm2 = Lsec[link_index(-c2)], Lm1 = Lsec[link_index(-c1)], Lm3 = Lsec[link_index(-c3)];
+    const real Tp = Lp3 + Lp1 + Lp2, Tm = Lm2 + Lm1 + Lm3;
+#define Y(label, delay) ydel(ys, (label), n, (delay), dt, order)
+    real a = Y(+c3, (real)0) + Y(+c1, Lp3) + Y(+c2, Lp3 + Lp1)
+           - Y(-c2, (real)0) - Y(-c1, Lm2) - Y(-c3, Lm2 + Lm1);
+    if (gen == ORC_GEN_20) {
+        a += Y(-c2, Tp) + Y(-c1, Tp + Lm2) + Y(-c3, Tp + Lm2 + Lm1)
+           - Y(+c3, Tm) - Y(+c1, Tm + Lp3) - Y(+c2, Tm + Lp3 + Lp1);
+    }
+#undef Y
+    return a;
+}
+
 /* O12 properly nested delays (the comparison case of P:151 -- the paper itself evaluates every L_l at t).
  * Delay operators act as (D_l f)(t) = f(t - L_l(t)), so D_a D_b f (t) = f(t - L_a(t) - L_b(t - L_a(t))): walking a
  * chain of links c_1 c_2 .. c_m backwards from the reception time,
@@ -683,6 +717,7 @@ static void work_free(work_t *w)
 
 /* full response for one source: y (6 links) on the halo range, X,Y,Z on [nb,ne) */
 static int g_nested_order = 0; /* 0: every L_l at t (the paper); p_L > 0: nested delays (O12), set per call */
+static int g_sagnac = 0;       /* 1: alpha, beta, gamma of O15 in place of X, Y, Z, set per call */
 
 static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, const double *hc, int gen,
                     int order, const margins_t *mg, int64_t lo, int64_t hi, int64_t nb, int64_t ne,
@@ -718,7 +753,8 @@ static int full_one(const orbit_ctx *o, const frame_t *f, const double *hp, cons
         geom_t g;
         orbit_geometry(o, n, &g); /* every delay evaluated at t_n */
         for (int c = 0; c < 3; ++c)
-            w->X[c][n - nb] = michelson_at(&ys, g.L, c, gen, n, (real)o->d.dt, order);
+            w->X[c][n - nb] = g_sagnac ? sagnac_at(&ys, g.L, c, gen, n, (real)o->d.dt, order)
+                                       : michelson_at(&ys, g.L, c, gen, n, (real)o->d.dt, order);
     }
     return ORC_OK;
 }
@@ -1121,6 +1157,35 @@ int orc_michelson_from_links(const orc_orbit_desc *d, const double *Rtab, const 
     return ORC_OK;
 }
 
+/* alpha, beta, gamma of O15 from caller-supplied link series y [6][n]: sagnac_at() on the valid range of margins() (the
+ * Michelson margins of the same generation: the Sagnac delays, 2 and 5 light times, are shorter than the Michelson ones) */
+int orc_sagnac_from_links(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *y,
+                          int gen, int order, double *abc)
+{
+    if (check_args(d, gen, order, 0, 0, d ? d->n : 0, 0, d ? d->n : 0) || !y || !abc) return ORC_EINVAL;
+    orbit_ctx o = { *d, Rtab, Ltab };
+    margins_t mg;
+    margins(d, gen, order, 0, &mg);
+    const int64_t N = d->n;
+    real *yr[6];
+    for (int l = 0; l < 6; ++l) {
+        if (!(yr[l] = (real *)malloc(sizeof(real) * (size_t)N))) return ORC_EINVAL;
+        for (int64_t i = 0; i < N; ++i) yr[l][i] = y[(int64_t)l * N + i];
+    }
+    yseries_t ys = { { yr[0], yr[1], yr[2], yr[3], yr[4], yr[5] }, 0, N };
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t n = 0; n < N; ++n) {
+        for (int c = 0; c < 3; ++c) abc[(int64_t)c * N + n] = 0.0;
+        if (n < mg.lo || n >= N - mg.hi) continue;
+        geom_t g;
+        orbit_geometry(&o, n, &g);
+        for (int c = 0; c < 3; ++c)
+            abc[(int64_t)c * N + n] = (double)sagnac_at(&ys, g.L, c, gen, n, (real)d->dt, order);
+    }
+    for (int l = 0; l < 6; ++l) free(yr[l]);
+    return ORC_OK;
+}
+
 /*
  * Full response (O5-O7).  hp, hc: [batch][ld]; outputs: A,E,T [batch][ne-nb],
  * XYZ [3][batch][ne-nb], y [6][batch][ne-nb]; any may be NULL.
@@ -1146,6 +1211,19 @@ int orc_response_full(const orc_orbit_desc *d, const double *Rtab, const double 
 }
 
 /* LFA response (O8) */
+/* Full response with the Sagnac combinations (O15): alpha, beta, gamma where orc_response_full has X, Y, Z, and Eq. (2.9)
+ * applied to them for A, E, T */
+int orc_response_full_sagnac(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
+                             const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
+                             int order, int64_t nb, int64_t ne, double *A, double *E, double *T,
+                             double *XYZ, double *y)
+{
+    g_sagnac = 1;
+    const int rc = orc_response_full(d, Rtab, Ltab, hp, hc, ld, batch, src, gen, order, nb, ne, A, E, T, XYZ, y);
+    g_sagnac = 0;
+    return rc;
+}
+
 /* Full response with properly nested TDI delays (O12); nested_order = p_L, the Lagrange order of the light-time lookups */
 int orc_response_full_nested(const orc_orbit_desc *d, const double *Rtab, const double *Ltab, const double *hp,
                              const double *hc, int64_t ld, int64_t batch, const orc_source *src, int gen,
