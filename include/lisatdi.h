@@ -256,6 +256,23 @@ int ltdi_response_lfa6(const ltdi_orbits *orb, const double *d_hp, const double 
                        double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes, void *stream);
 int ltdi_margins_lfa6(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi);
 
+/* SURVEY.md 8(f)-4, third part: the full response in the Sagnac-type combinations alpha, beta, gamma ("photons
+ * propagating in clockwise and counterclockwise directions around the constellation"; the paper prints no equation, so
+ * the textbook form is taken, reading G33).  In the link labelling of P:81 (+1: 3 -> 2, +2: 1 -> 3, +3: 2 -> 1,
+ * -1: 2 -> 3, -2: 3 -> 1, -3: 1 -> 2), with the two beams read at spacecraft 1
+ *   S+ = y_{+3} + D_{+3} y_{+1} + D_{+3} D_{+1} y_{+2},   S- = y_{-2} + D_{-2} y_{-1} + D_{-2} D_{-1} y_{-3}
+ * and the round-trip times T+ = L_3 + L_1 + L_2, T- = L_-2 + L_-1 + L_-3:
+ *   gen LTDI_GEN_15: alpha = S+ - S-                             (6 terms: free of laser noise where T+ = T-)
+ *   gen LTDI_GEN_20: alpha = (S+ + D_{T+} S-) - (S- + D_{T-} S+) (12 terms: free of laser noise for constant L_l != L_-l)
+ * beta, gamma by the cyclic permutation 1 -> 2 -> 3 -> 1; every delay evaluated at t; links from Eq. (2.5).
+ * d_abc [3][batch][ld] returns alpha, beta, gamma; d_A, d_E, d_T are Eq. (2.9) applied to them; the margins are those of
+ * ltdi_margins for the same generation (the Sagnac delays, 2 and 5 light times, are shorter than the Michelson ones).
+ * Arguments, layout and errors as ltdi_response_full.  Runs on the library's generic tile kernel (per-sample weights)
+ * for every Lagrange order. */
+int ltdi_response_full_sagnac(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                              const ltdi_source *h_src, int gen, int lagrange_order, double *d_A, double *d_E,
+                              double *d_T, double *d_abc, double *d_y, void *d_work, size_t work_bytes, void *stream);
+
 /* Hybrid: LFA for t <= t_hyb + T/2, full for t >= t_hyb - T/2, links blended by Eq. (4.5) and
  * X, Y, Z blended separately by Eq. (4.6) (S8).  h_hyb has n_hyb = 1 or batch entries. */
 int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,

@@ -88,6 +88,8 @@ _SIGNATURES = {
     "ltdi_workspace_bytes": (C.c_int, [C.c_int, C.c_int64, C.c_int64, C.c_int, C.c_int, _szp]),
     "ltdi_response_full": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                      _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_full_sagnac": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
+                                            _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_full_nested": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
                                             _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_waveform_chirp": (C.c_int, [C.POINTER(Chirp), C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64, _dp, _dp, _vp,
@@ -342,7 +344,9 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
     with torch.cuda.device(hp.device):
         # the stream handle must be the current stream of the tensors' device: evaluated inside the device context
         tail = [p(ws.A), p(ws.E), p(ws.T), p(ws.XYZ), p(ws.y), ws.work.data_ptr(), ws.work.numel() * 8, _stream()]
-        if which == RESPONSE_FULL and ext is not None:
+        if which == RESPONSE_FULL and ext == "sagnac":
+            rc, fn = lib().ltdi_response_full_sagnac(*head, *tail), "ltdi_response_full_sagnac"
+        elif which == RESPONSE_FULL and ext is not None:
             rc, fn = lib().ltdi_response_full_nested(*head, int(ext[0]), *tail), "ltdi_response_full_nested"
         elif which == RESPONSE_FULL:
             rc, fn = lib().ltdi_response_full(*head, *tail), "ltdi_response_full"
@@ -363,6 +367,12 @@ def _run(which, orb, hp, hc, sources, gen, order, fd_order, hybrid, want_xyz, wa
 def response_full(orb, hp, hc, sources, gen, order, want_xyz=False, want_y=False, workspace=None):
     """Eqs. (2.2)-(2.9): projection, TDI `gen`, A, E, T.  Returns dict A, E, T (, XYZ, y)."""
     return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_xyz, want_y, workspace)
+
+
+def response_full_sagnac(orb, hp, hc, sources, gen, order, want_abc=False, want_y=False, workspace=None):
+    """the full response in the Sagnac combinations; "XYZ" of the result holds alpha, beta, gamma, and A, E, T
+    are Eq. (2.9) applied to them (ltdi_response_full_sagnac)."""
+    return _run(RESPONSE_FULL, orb, hp, hc, sources, gen, order, 0, None, want_abc, want_y, workspace, ext="sagnac")
 
 
 def response_full_nested(orb, hp, hc, sources, gen, order, nested_order=3, want_xyz=False, want_y=False, workspace=None):

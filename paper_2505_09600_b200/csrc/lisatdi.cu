@@ -707,8 +707,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
                  int64_t batch, const ltdi_source *h_src, int gen, int order, int fd_order,
                  const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, double *d_XYZ,
                  double *d_y, void *d_work, size_t work_bytes, void *stream, int lfa_terms = 1,
-                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0, const ltdi_chirp *h_wav = nullptr, int lfa6 = 0)
+                 int lfa_point = LTDI_LFA_CENTRAL, int nested_order = 0, const ltdi_chirp *h_wav = nullptr, int lfa6 = 0,
+                 int sagnac = 0)
 {
+    if (sagnac && (which != LTDI_RESPONSE_FULL || nested_order != 0 || h_wav)) return LTDI_EINVAL;
     if (lfa6 && (which != LTDI_RESPONSE_LFA || lfa_terms != 1 || lfa_point != LTDI_LFA_CENTRAL)) return LTDI_EINVAL;
     if (nested_order != 0 && (which != LTDI_RESPONSE_FULL || nested_order != 3)) return nested_order == 3 || nested_order < 0 || !(nested_order & 1) ? LTDI_EINVAL : LTDI_EUNSUPPORTED;
     if (nested_order && !fast_order(order)) return LTDI_EUNSUPPORTED;   /* nested delays run on the tuned path (orders 9, 31) */
@@ -822,9 +824,10 @@ int run_response(int which, const ltdi_orbits *orb, const double *d_hp, const do
     p.lfa_terms = lfa_terms; p.lfa_point = lfa_point; p.xw = xw; p.nested = nested_order != 0;
     p.chirp = h_wav ? w_chirp : nullptr;
     p.lfa6 = lfa6;
+    p.sagnac = sagnac;
     p.A = d_A; p.E = d_E; p.T = d_T; p.XYZ = d_XYZ; p.Y = d_y;
 
-    if (fast_order(order) && !lfa6) {   /* (B20) / (B30) run on the generic kernel for every order */
+    if (fast_order(order) && !lfa6 && !sagnac) {   /* (B20) / (B30) and the Sagnac combinations run on the generic kernel for every order */
         const double *sm = have_small ? small_args.v : nullptr;
         const HybPlan *dp = have_small ? nullptr : w_plan;
         double *fw = (double *)d_work + work_doubles(batch);
@@ -1165,6 +1168,14 @@ int ltdi_response_lfa6(const ltdi_orbits *orb, const double *d_hp, const double 
 {
     return run_response(LTDI_RESPONSE_LFA, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, nullptr,
                         0, d_A, d_E, d_T, d_XYZ, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, 0, nullptr, 1);
+}
+
+int ltdi_response_full_sagnac(const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld, int64_t batch,
+                              const ltdi_source *h_src, int gen, int lagrange_order, double *d_A, double *d_E, double *d_T,
+                              double *d_abc, double *d_y, void *d_work, size_t work_bytes, void *stream)
+{
+    return run_response(LTDI_RESPONSE_FULL, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, 0, nullptr, 0, d_A,
+                        d_E, d_T, d_abc, d_y, d_work, work_bytes, stream, 1, LTDI_LFA_CENTRAL, 0, nullptr, 0, 1);
 }
 
 int ltdi_margins_lfa6(const ltdi_orbit_desc *desc, int gen, int lagrange_order, int fd_order, int64_t *lo, int64_t *hi)

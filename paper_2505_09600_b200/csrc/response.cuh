@@ -31,6 +31,7 @@ struct RespParams {
     int off_yL, off_dL, off_hs; /* shared-memory offsets (doubles) of the LFA links, their derivative, the strain */
     int qmax;             /* bound on |integer shift| of a projection delay (m1 - M/2) */
     int nested;           /* nested TDI delays (tuned path only) */
+    int sagnac;           /* alpha, beta, gamma in place of X, Y, Z (generic kernel only) */
     const struct ChirpDev *chirp; /* waveform model constants [batch], or nullptr (sampled strain) */
     int lfa6;             /* all six LFA links and the Michelson variables of Eq. (B20) / (B30) (generic kernel) */
     int lfa_terms, lfa_point, xw; /* terms of Eq. (B4), expansion point LTDI_LFA_*, xw = terms - 1 */
@@ -339,6 +340,29 @@ __device__ __forceinline__ double michelson_full(const RespParams &p, const doub
     return x;
 }
 
+// SURVEY 8(f)-4 (reading G33): the Sagnac combinations, channel ch = 0, 1, 2 -> alpha, beta, gamma.
+// With S+ = y_{+3} + D_{+3} y_{+1} + D_{+3} D_{+1} y_{+2} (the beam 1 -> 3 -> 2 -> 1), S- = y_{-2} + D_{-2} y_{-1} +
+// D_{-2} D_{-1} y_{-3} (1 -> 2 -> 3 -> 1) and the round-trip times T+ = L_3 + L_1 + L_2, T- = L_-2 + L_-1 + L_-3:
+// gen 1.5: alpha = S+ - S- (6 terms); gen 2.0: alpha = (S+ + D_{T+} S-) - (S- + D_{T-} S+) (12 terms); all delays at t_n
+// (P:151); beta, gamma by the cyclic permutation of the labels.
+template <int MT>
+__device__ __forceinline__ double sagnac_full(const RespParams &p, const double *yF, int64_t y0, int64_t n,
+                                              const double L[6], int ch)
+{
+    const int k3 = (2 + ch) % 3, k1 = ch % 3, k2 = (1 + ch) % 3;   /* |l| - 1 of the labels 3, 1, 2 permuted */
+    const double *P3 = yF + (size_t)k3 * p.yr, *P1 = yF + (size_t)k1 * p.yr, *P2 = yF + (size_t)k2 * p.yr;
+    const double *M2 = yF + (size_t)(k2 + 3) * p.yr, *M1 = yF + (size_t)(k1 + 3) * p.yr, *M3 = yF + (size_t)(k3 + 3) * p.yr;
+    const double Lp3 = L[k3], Lp1 = L[k1], Lp2 = L[k2], Lm2 = L[k2 + 3], Lm1 = L[k1 + 3], Lm3 = L[k3 + 3];
+    const double Tp = Lp3 + Lp1 + Lp2, Tm = Lm2 + Lm1 + Lm3;
+    const int i0 = (int)(n - y0);
+#define DEL(S, d) delayed<MT>(p, S, y0, p.yr, n, (d))
+    double a = P3[i0] + DEL(P1, Lp3) + DEL(P2, Lp3 + Lp1) - M2[i0] - DEL(M1, Lm2) - DEL(M3, Lm2 + Lm1);
+    if (p.gen == LTDI_GEN_20)
+        a += DEL(M2, Tp) + DEL(M1, Tp + Lm2) + DEL(M3, Tp + Lm2 + Lm1) - DEL(P3, Tm) - DEL(P1, Tm + Lp3) - DEL(P2, Tm + Lp3 + Lp1);
+#undef DEL
+    return a;
+}
+
 // Eq. (B25) (gen 1.5) / (B33) (gen 2.0): dL = first resp. second derivative of the LFA links
 template <int MT>
 __device__ __forceinline__ double michelson_lfa(const RespParams &p, const double *dL, int64_t y0, int64_t n,
@@ -547,7 +571,8 @@ __global__ void __launch_bounds__(256) response_kernel(RespParams p)
                 double x = 0.0;
                 if (need_lfa && p.lfa6) x = michelson_b20<MT>(p, dL, dL + (size_t)6 * p.yr, y0, n, L, ch);
                 else if (need_lfa && wa != 0.0) x = wa * michelson_lfa<MT>(p, dL, y0, n, L, ch);
-                if (need_full && wb != 0.0) x = fma(wb, michelson_full<MT>(p, yF, y0, n, L, ch), x); /* (4.6) */
+                if (need_full && p.sagnac) x = sagnac_full<MT>(p, yF, y0, n, L, ch);
+                else if (need_full && wb != 0.0) x = fma(wb, michelson_full<MT>(p, yF, y0, n, L, ch), x); /* (4.6) */
                 X[ch] = x;
             }
         }

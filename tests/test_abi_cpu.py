@@ -106,6 +106,7 @@ def test_next_row_arguments_are_checked_before_any_cuda_call(ltdi):
     assert lib.ltdi_orbits_init_knots(C.byref(kd), ptr, 6, -4 * 86400.0, 86400.0, 7, ptr, 1 << 30, None, C.byref(handle)) == ltdi.EINVAL
     # waveform model and overlap plan
     assert lib.ltdi_waveform_chirp(None, 1, 0.0, 5.0, 10, 10, None, None, None, 0, None) == ltdi.EINVAL
+    assert lib.ltdi_response_full_sagnac(None, ptr, ptr, 10, 1, None, 20, 31, ptr, ptr, ptr, None, None, ptr, 1 << 20, None) == ltdi.EINVAL
     par6 = (C.c_double * 6)(50.0, 0.2, 1e25, 0.3, 0.1, 0.2)
     p6 = C.cast(par6, C.c_void_p)
     assert lib.ltdi_waveform_ecc(ptr, 1, p6, 8, 1, 0.0, 5.0, 10, 10, ptr, ptr, ptr, 64, None) == ltdi.EINVAL      # one knot
