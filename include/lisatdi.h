@@ -286,7 +286,10 @@ int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const doubl
  * `stream`, the host->device copies of the strain, the response `which` (LTDI_RESPONSE_*; fd_order and
  * h_hyb / n_hyb as in the calls above, ignored where they do not apply) and the device->host copies of
  * A, E, T.  d_scratch: device scratch of ltdi_host_scratch_bytes() bytes, 256-byte aligned.  Results
- * are valid after the stream is synchronised. */
+ * are valid after the stream is synchronised.  A batch of more than 128 MiB per series is cut into up to 16 pieces of
+ * whole sources that pass through upload, kernels and download as a pipeline (the copies on two streams of the
+ * library's own, chained to `stream` by events), so that one call keeps both directions of PCIe and the SMs busy; the
+ * results are bitwise those of the one-piece call. */
 int ltdi_host_scratch_bytes(int64_t ld, int64_t batch, size_t *bytes);
 int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, const double *h_hc, int64_t ld,
                        int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,

@@ -57,6 +57,7 @@ struct ProfScope {
 
 // Per-device state.  __constant__ tables, cudaFuncSetAttribute, streams and events all belong to ONE device: a
 // process that uses several devices gets one DeviceState per device (indexed by cudaGetDevice()).
+#define LTDI_HOST_CHUNKS 16   /* most pieces an end-to-end call is cut into */
 struct DeviceState {
     std::mutex mu;                 /* guards everything below, and serialises the hybrid fork / join on the device */
     bool ready = false;
@@ -64,6 +65,10 @@ struct DeviceState {
     int smem_max = 0, sms = 0;
     cudaStream_t side = nullptr;   /* non-blocking side stream of the hybrid's concurrent launches */
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    /* ltdi_response_host: copy streams and the events that chain upload -> kernels -> download chunk by chunk */
+    std::mutex host_mu;
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_in[LTDI_HOST_CHUNKS] = {}, ev_comp[LTDI_HOST_CHUNKS] = {};
     std::vector<std::pair<const void *, size_t>> smem_seen;   /* cudaFuncAttributeMaxDynamicSharedMemorySize per kernel */
 };
 DeviceState g_dev[64];
@@ -139,10 +144,20 @@ int device_state(DeviceState **out)
                 cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
                 cudaStreamCreateWithFlags(&d.side, cudaStreamNonBlocking) != cudaSuccess ||
                 cudaEventCreateWithFlags(&d.ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&d.ev_join, cudaEventDisableTiming) != cudaSuccess) {
+                cudaEventCreateWithFlags(&d.ev_join, cudaEventDisableTiming) != cudaSuccess ||
+                cudaStreamCreateWithFlags(&d.copy_in, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaStreamCreateWithFlags(&d.copy_out, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&d.ev_start, cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&d.ev_done, cudaEventDisableTiming) != cudaSuccess) {
                 (void)cudaGetLastError();
                 d.status = LTDI_ECUDA;
             }
+            for (int i = 0; i < LTDI_HOST_CHUNKS && d.status == LTDI_OK; ++i)
+                if (cudaEventCreateWithFlags(&d.ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+                    cudaEventCreateWithFlags(&d.ev_comp[i], cudaEventDisableTiming) != cudaSuccess) {
+                    (void)cudaGetLastError();
+                    d.status = LTDI_ECUDA;
+                }
         }
         d.ready = true;
     }
@@ -940,15 +955,60 @@ int ltdi_response_host(int which, const ltdi_orbits *orb, const double *h_hp, co
     double *d_A = (double *)(base + 2 * series), *d_E = (double *)(base + 3 * series), *d_T = (double *)(base + 4 * series);
     void *d_work = base + 5 * series;
     cudaStream_t st = (cudaStream_t)stream;
-    LTDI_CUDA_OK(cudaMemcpyAsync(d_hp, h_hp, bytes, cudaMemcpyHostToDevice, st));
-    LTDI_CUDA_OK(cudaMemcpyAsync(d_hc, h_hc, bytes, cudaMemcpyHostToDevice, st));
-    const int rc = run_response(which, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, h_hyb,
-                                n_hyb, d_A, d_E, d_T, nullptr, nullptr, d_work, need - 5 * series, stream);
+    /* A large batch is cut into pieces of whole sources that go through upload -> kernels -> download as a pipeline: the
+     * uploads on one copy stream, the kernels on the caller's stream, the downloads on a second copy stream, chained by
+     * events, so that a single call keeps both directions of PCIe and the SMs busy at once.  The caller's stream waits
+     * for the last download: the results are valid once `stream` has been synchronised, as for a one-piece call. */
+    const int64_t piece_min = std::max<int64_t>(1, ((int64_t)64 << 20) / (ld * (int64_t)sizeof(double)));   /* >= 64 MiB per series */
+    const int npiece = (int)std::max<int64_t>(1, std::min<int64_t>(LTDI_HOST_CHUNKS, batch / piece_min));
+    if (npiece == 1) {
+        LTDI_CUDA_OK(cudaMemcpyAsync(d_hp, h_hp, bytes, cudaMemcpyHostToDevice, st));
+        LTDI_CUDA_OK(cudaMemcpyAsync(d_hc, h_hc, bytes, cudaMemcpyHostToDevice, st));
+        const int rc = run_response(which, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, h_hyb,
+                                    n_hyb, d_A, d_E, d_T, nullptr, nullptr, d_work, need - 5 * series, stream);
+        if (rc) return rc;
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_A, d_A, bytes, cudaMemcpyDeviceToHost, st));
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_E, d_E, bytes, cudaMemcpyDeviceToHost, st));
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_T, d_T, bytes, cudaMemcpyDeviceToHost, st));
+        return LTDI_OK;
+    }
+    if (!h_src || (which == LTDI_RESPONSE_HYBRID && (!h_hyb || (n_hyb != 1 && n_hyb != batch)))) return LTDI_EINVAL;
+    DeviceState *dsp = nullptr;
+    int rc = device_state(&dsp);
     if (rc) return rc;
-    LTDI_CUDA_OK(cudaMemcpyAsync(h_A, d_A, bytes, cudaMemcpyDeviceToHost, st));
-    LTDI_CUDA_OK(cudaMemcpyAsync(h_E, d_E, bytes, cudaMemcpyDeviceToHost, st));
-    LTDI_CUDA_OK(cudaMemcpyAsync(h_T, d_T, bytes, cudaMemcpyDeviceToHost, st));
-    return LTDI_OK;
+    DeviceState &ds = *dsp;
+    std::lock_guard<std::mutex> lk(ds.host_mu);   /* one call at a time issues into the copy streams and their events */
+    LTDI_CUDA_OK(cudaEventRecord(ds.ev_start, st));
+    LTDI_CUDA_OK(cudaStreamWaitEvent(ds.copy_in, ds.ev_start, 0));    /* what the caller queued before this call comes first */
+    LTDI_CUDA_OK(cudaStreamWaitEvent(ds.copy_out, ds.ev_start, 0));
+    const int64_t per = (batch + npiece - 1) / npiece;
+    int used = 0;
+    for (int c = 0; c < npiece; ++c) {
+        const int64_t b0 = c * per, cnt = std::min(per, batch - b0);
+        if (cnt <= 0) break;
+        const size_t off = (size_t)b0 * (size_t)ld, nb = (size_t)cnt * (size_t)ld * sizeof(double);
+        LTDI_CUDA_OK(cudaMemcpyAsync(d_hp + off, h_hp + off, nb, cudaMemcpyHostToDevice, ds.copy_in));
+        LTDI_CUDA_OK(cudaMemcpyAsync(d_hc + off, h_hc + off, nb, cudaMemcpyHostToDevice, ds.copy_in));
+        LTDI_CUDA_OK(cudaEventRecord(ds.ev_in[c], ds.copy_in));
+        LTDI_CUDA_OK(cudaStreamWaitEvent(st, ds.ev_in[c], 0));
+        rc = run_response(which, orb, d_hp + off, d_hc + off, ld, cnt, h_src + b0, gen, lagrange_order, fd_order,
+                          h_hyb ? h_hyb + (n_hyb == batch ? b0 : 0) : nullptr, n_hyb == batch ? cnt : n_hyb, d_A + off,
+                          d_E + off, d_T + off, nullptr, nullptr, d_work, need - 5 * series, stream);
+        if (rc) break;
+        LTDI_CUDA_OK(cudaEventRecord(ds.ev_comp[c], st));
+        LTDI_CUDA_OK(cudaStreamWaitEvent(ds.copy_out, ds.ev_comp[c], 0));
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_A + off, d_A + off, nb, cudaMemcpyDeviceToHost, ds.copy_out));
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_E + off, d_E + off, nb, cudaMemcpyDeviceToHost, ds.copy_out));
+        LTDI_CUDA_OK(cudaMemcpyAsync(h_T + off, d_T + off, nb, cudaMemcpyDeviceToHost, ds.copy_out));
+        ++used;
+    }
+    /* also after an error: the caller's stream must not run ahead of copies that were already queued */
+    (void)used;
+    LTDI_CUDA_OK(cudaEventRecord(ds.ev_done, ds.copy_out));
+    LTDI_CUDA_OK(cudaStreamWaitEvent(st, ds.ev_done, 0));
+    LTDI_CUDA_OK(cudaEventRecord(ds.ev_done, ds.copy_in));
+    LTDI_CUDA_OK(cudaStreamWaitEvent(st, ds.ev_done, 0));
+    return rc;
 }
 
 int ltdi_orbits_workspace_bytes(const ltdi_orbit_desc *desc, size_t *bytes)

@@ -209,6 +209,55 @@ def test_host_pipeline_matches_device_call(ltdi):
     assert torch.equal(A, ref["A"].cpu()) and torch.equal(E, ref["E"].cpu()) and torch.equal(T, ref["T"].cpu())
 
 
+def test_host_call_cut_into_pieces_matches_device_call(ltdi):
+    """a batch above 128 MiB per series goes through ltdi_response_host as a pipeline of pieces (upload / kernels / download
+    on three streams): bitwise the device call, for the hybrid with one window per source (the per-source arrays are
+    offset piece by piece), with a shared window, and for the LFA; two calls back to back on one stream and two slots"""
+    dev = torch.device("cuda:0")
+    n, batch = 40000, 520                     # 166 MB per series: 2 pieces of 260 sources
+    cfg = W.config(4, n=n, batch=8)
+    hp8, hc8, ang8, metas8 = W.sources(cfg, list(range(8)))
+    rep = batch // 8
+    hp, hc = np.tile(hp8, (rep, 1)), np.tile(hc8, (rep, 1))
+    scale = 1.0 + 0.01 * np.arange(batch)[:, None]          # every source different
+    hp, hc = hp * scale, hc * scale
+    ang = np.tile(ang8, (rep, 1))
+    metas = [metas8[i % 8] for i in range(batch)]
+    hyb = hybrid_params(metas, ltdi.hyb_time, W.TAPER_COSINE, cfg["dt"])
+    for i, h in enumerate(hyb):                              # and every window different
+        h["t_hyb"] += 10.0 * cfg["dt"] * (i % 7)
+    orb = ltdi.Orbits(cfg["orbit"], device=dev)
+    dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+    hp_h, hc_h = torch.from_numpy(hp).pin_memory(), torch.from_numpy(hc).pin_memory()
+    keep = lambda d: [d[c].cpu() for c in "AET"]
+    want = [keep(ltdi.response_hybrid(orb, dhp, dhc, ang, 20, 31, 2, hyb)),
+            keep(ltdi.response_hybrid(orb, dhp, dhc, ang, 20, 31, 2, hyb[3])),
+            keep(ltdi.response_lfa(orb, dhp, dhc, ang, 20, 31, 2))]
+    calls = [(ltdi.RESPONSE_HYBRID, hyb), (ltdi.RESPONSE_HYBRID, hyb[3]), (ltdi.RESPONSE_LFA, None)]
+    for depth in (1, 2):
+        pipe = ltdi.HostPipeline(orb, batch, n, depth=depth)
+        for (which, h), w in zip(calls, want):
+            out = pipe.run(which, hp_h, hc_h, ang, 20, 31, 2, h)
+            pipe.synchronize()
+            torch.cuda.synchronize()
+            for a, b in zip(out, w):
+                assert torch.equal(a, b), (depth, which)
+        # back to back without a synchronisation in between: the second call must not overtake the first one's copies
+        outs = []
+        for (which, h) in calls[:2]:
+            outs.append([t for t in pipe.run(which, hp_h, hc_h, ang, 20, 31, 2, h)])
+            if depth == 1:
+                pipe.synchronize()
+                outs[-1] = [t.clone() for t in outs[-1]]
+        pipe.synchronize()
+        torch.cuda.synchronize()
+        if depth == 2:
+            for o, w in zip(outs, want[:2]):
+                for a, b in zip(o, w):
+                    assert torch.equal(a, b), depth
+        del pipe
+
+
 def test_prepared_anchors_give_bitwise_the_same_result(ltdi):
     """ltdi_orbits_prepare(): TDI weights computed once per time grid; the responses must not change by a bit,
     and a prepare for another generation / order must be ignored"""
