@@ -176,6 +176,29 @@ def margins(desc, gen, order, fd_order=0):
     return lo.value, hi.value
 
 
+def time_shard(desc, lo, hi, world, rank):
+    """the piece of ONE long series that rank `rank` of `world` computes -- the path needs no exchange step, a
+    piece only re-reads a halo of the input.  The valid outputs [lo, n - hi) (lo, hi from margins() of the response at
+    hand) are split into `world` contiguous runs [a, b); the rank evaluates the response on the sub-grid that starts lo
+    samples before a and ends hi samples after b, whose own valid range is exactly [a, b).
+    Returns (sub_desc, src, dst, a, b): sub_desc = desc with t0 and n of the sub-grid (tabulated orbits sliced with it; a
+    numerical orbit file keeps its knots), src = slice of the input samples the rank reads, dst = slice of the sub-grid's
+    output that holds the global samples [a, b).  Pure host logic: no CUDA call."""
+    n = int(desc["n"])
+    world, rank = int(world), int(rank)
+    if world < 1 or not 0 <= rank < world or lo < 0 or hi < 0 or n - hi - lo < world:
+        raise ValueError("time_shard: needs 0 <= rank < world <= number of valid samples")
+    valid = n - hi - lo
+    a = lo + valid * rank // world
+    b = lo + valid * (rank + 1) // world
+    first, last = a - lo, b + hi                     # input samples [first, last)
+    sub = dict(desc, t0=float(desc["t0"]) + first * float(desc["dt"]), n=last - first)
+    for key in ("R_table", "L_table"):               # ORBIT_TABLES: per-sample tables travel with the grid
+        if key in sub and sub[key] is not None:
+            sub[key] = sub[key][..., first:last]
+    return sub, slice(first, last), slice(lo, lo + (b - a)), a, b
+
+
 def margins_lfa_ext(desc, gen, order, fd_order, terms=1):
     lo, hi = C.c_int64(), C.c_int64()
     d = _desc(desc)

@@ -571,3 +571,36 @@ def test_lfa6_b20_b30(ltdi, orc80, k, n, batch, order, gen, fd):
     lo, hi = orc80.margins_lfa6(orbit, gen, order, fd)
     assert (lo, hi) == ltdi.margins_lfa6(orbit, gen, order, fd)
     check(out, ref, lo, hi, cfg["n"])
+
+
+@pytest.mark.parametrize("which", ["full", "lfa", "hybrid"])
+def test_one_series_split_in_time(ltdi, which):
+    """the pieces time_shard() hands to the ranks of a multi-GPU job, run here one after the other on one
+    device, stitch to the whole-series response (the sub-grids start at a t0 rounded to fp64, so 1e-13, not bitwise);
+    on a numerical orbit file as well, whose knots every piece shares"""
+    dev = torch.device("cuda:0")
+    cfg = W.config(2, n=60013)
+    hp, hc, ang, metas = W.sources(cfg, [0])
+    gen, order, fd = 20, 31, 2
+    hyb = hybrid_params(metas, ltdi.hyb_time, W.TAPER_COSINE, cfg["dt"])
+    for orbit in (cfg["orbit"], W.numerical_orbit(cfg["n"], cfg["dt"], t0=cfg["orbit"]["t0"])):
+        def call(desc, p, c):
+            orb = ltdi.Orbits(desc, device=dev)
+            p, c = torch.from_numpy(np.ascontiguousarray(p)).to(dev), torch.from_numpy(np.ascontiguousarray(c)).to(dev)
+            if which == "full":
+                return to_numpy(ltdi.response_full(orb, p, c, ang, gen, order))
+            if which == "lfa":
+                return to_numpy(ltdi.response_lfa(orb, p, c, ang, gen, order, fd))
+            return to_numpy(ltdi.response_hybrid(orb, p, c, ang, gen, order, fd, hyb))
+        whole = call(orbit, hp, hc)
+        lo, hi = ltdi.margins(orbit, gen, order, 0 if which == "full" else fd)
+        world = 3
+        got = {c: np.zeros(cfg["n"]) for c in "AET"}
+        for rank in range(world):
+            sub, src, dst, a, b = ltdi.time_shard(orbit, lo, hi, world, rank)
+            r = call(sub, hp[:, src], hc[:, src])
+            for c in "AET":
+                got[c][a:b] = r[c][0, dst]
+        scale = max(np.linalg.norm(whole[c]) for c in "AET")
+        for c in "AET":
+            assert np.linalg.norm(got[c] - whole[c][0]) <= 1e-13 * scale, (which, c)
