@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(FFT_THREADS) fft_pointwise_kernel(double2 *__r
     *p = cmul(*p, bhat[j]);
 }
 
-/* host: the radices of a power-of-two length (256 while eight bits remain, then 16 / 4 / 2), and the transform itself;
+/* host: the radices of a power-of-two length (16 / 4 / 2 for the bits that do not fill a byte, then 256s), and the transform itself;
  * returns the buffer (0: buf0, 1: buf1) that holds the result.  Series q starts at q * stride in both buffers.  `first`
  * (optional) replaces buf0 as the input of the first pass (fused packing). */
 static inline int fft_radices(int64_t N, int *rad)
@@ -241,11 +241,16 @@ static inline int fft_radices(int64_t N, int *rad)
     int bits = 0;
     while (((int64_t)1 << bits) < N) ++bits;
     int np = 0;
-    while (bits >= 8) { rad[np++] = 256; bits -= 8; }
+    const int n256 = bits / 8;
+    bits -= 8 * n256;
+    /* the small radices FIRST: the first pass is the one that packs two real series into a complex one, and in a register
+     * pass every thread streams through them, while the radix-256 pass would fetch them in 128-byte runs (measured: 352 us
+     * against 167 us for the same pass over complex input, 256 sources x 2^17) */
     while (bits >= 4) { rad[np++] = 16; bits -= 4; }
     if (bits == 3) { rad[np++] = 4; rad[np++] = 2; }
     else if (bits == 2) rad[np++] = 4;
     else if (bits == 1) rad[np++] = 2;
+    for (int i = 0; i < n256; ++i) rad[np++] = 256;
     return np;
 }
 
