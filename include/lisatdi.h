@@ -281,6 +281,24 @@ int ltdi_response_hybrid(const ltdi_orbits *orb, const double *d_hp, const doubl
                          double *d_T, double *d_XYZ, double *d_y, void *d_work, size_t work_bytes,
                          void *stream);
 
+/* The three responses for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same computation as ltdi_response_full / _lfa / _hybrid (which = LTDI_RESPONSE_*; fd_order and
+ * h_hyb / n_hyb as there, ignored where they do not apply), but the caller passes NO workspace -- the scratch (source frames,
+ * TDI weight anchors, link series) lives in a file-scope device array of the library of LTDI_STATIC_SCRATCH_BYTES (64 MiB),
+ * which every GPU that loads the library holds until the process exits.  The call allocates nothing: no cudaMalloc, cudaFree
+ * or allocating library routine, on any call (the first call on a device looks up the array's device address and uploads the
+ * library's constant tables: make one call outside a graph capture first).  d_A, d_E, d_T [batch][ld] are the caller's.
+ * Limit: ltdi_workspace_bytes(which, n, batch, gen, lagrange_order) must not exceed LTDI_STATIC_SCRATCH_BYTES, else
+ * LTDI_EWORKSPACE and nothing is launched (config 2's single source of 518 400 samples fits for all three responses; 4096
+ * sources do not: use the calls above with a workspace of the caller's).  Every call on a device shares the one array, which
+ * keeps the contents of the last call; nothing in it has to start at zero (each region is written by the call before the
+ * call reads it).  Calls that overlap on the GPU -- two streams, two host threads -- RACE on it: serialise them.  Other
+ * errors as ltdi_response_full. */
+#define LTDI_STATIC_SCRATCH_BYTES ((size_t)64 << 20)
+int ltdi_response_static(int which, const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                         int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                         const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T, void *stream);
+
 /* End-to-end variant (the call a host application makes): h_hp, h_hc [batch][ld] and h_A, h_E, h_T
  * [batch][ld] are HOST buffers (pinned memory makes the copies asynchronous).  The call enqueues, on
  * `stream`, the host->device copies of the strain, the response `which` (LTDI_RESPONSE_*; fd_order and

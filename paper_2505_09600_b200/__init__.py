@@ -88,6 +88,8 @@ _SIGNATURES = {
     "ltdi_workspace_bytes": (C.c_int, [C.c_int, C.c_int64, C.c_int64, C.c_int, C.c_int, _szp]),
     "ltdi_response_full": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                      _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
+    "ltdi_response_static": (C.c_int, [C.c_int, _vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
+                                       C.POINTER(Hybrid), C.c_int64, _dp, _dp, _dp, _vp]),
     "ltdi_response_full_sagnac": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int,
                                             _dp, _dp, _dp, _dp, _dp, _vp, C.c_size_t, _vp]),
     "ltdi_response_full_nested": (C.c_int, [_vp, _dp, _dp, C.c_int64, C.c_int64, C.POINTER(Source), C.c_int, C.c_int, C.c_int,
@@ -484,6 +486,31 @@ def _hybrid_array(hybrid):
         return None, 0
     hl = hybrid if isinstance(hybrid, (list, tuple)) else [hybrid]
     return (Hybrid * len(hl))(*[Hybrid(h["t_hyb"], h["window_s"], h["sigma_s"], int(h["taper"])) for h in hl]), len(hl)
+
+
+STATIC_SCRATCH_BYTES = 64 << 20
+
+
+def response_static(which, orb, hp, hc, sources, gen, order, fd_order=2, hybrid=None, out=None):
+    """The response `which` (RESPONSE_FULL / _LFA / _HYBRID) without a workspace: the library's scratch is a static device
+    array of STATIC_SCRATCH_BYTES, nothing is allocated by the call (ltdi_response_static).  out: dict of preallocated A, E,
+    T [batch][ld] device tensors (allocated here if None: that allocation is the caller's, not the library's).  Calls that
+    overlap on the GPU race on the shared array; LtdiError(EWORKSPACE) if the problem does not fit."""
+    hp, hc = _dev_f64(hp, "hp"), _dev_f64(hc, "hc")
+    if hp.dim() == 1:
+        hp, hc = hp[None], hc[None]
+    batch, ld = hp.shape
+    assert hc.shape == hp.shape
+    src_ptr, keep = _sources(sources)
+    assert keep.shape[0] == batch, "one (beta, lambda, psi) per source"
+    harr, nh = _hybrid_array(hybrid)
+    if out is None:
+        out = {c: torch.empty(batch, ld, dtype=torch.float64, device=hp.device) for c in "AET"}
+    with torch.cuda.device(hp.device):
+        rc = lib().ltdi_response_static(which, orb.handle, hp.data_ptr(), hc.data_ptr(), ld, batch, src_ptr, gen, order, fd_order,
+                                        harr, nh, out["A"].data_ptr(), out["E"].data_ptr(), out["T"].data_ptr(), _stream())
+    _check("ltdi_response_static", rc)
+    return out
 
 
 class HostPipeline:

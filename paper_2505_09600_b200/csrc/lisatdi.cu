@@ -1320,3 +1320,51 @@ int ltdi_profile_slow_tiles(int64_t *count, int reset)
 const char *ltdi_version(void) { return "lisatdi-b200 0.1 (sm_100a, fp64)"; }
 
 } // extern "C"
+
+// ---- ltdi_response_static: the responses with the scratch in a file-scope device array (no allocation anywhere) --------
+// In host code `g_static_scratch` is a host-side stand-in for the symbol, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, looked up once per device with that device current.
+static __device__ __align__(256) double g_static_scratch[LTDI_STATIC_SCRATCH_BYTES / sizeof(double)];
+static std::mutex g_static_mu;
+static void *g_static_ptr[64];   /* device address of g_static_scratch on device i, or nullptr before its set-up */
+
+static int static_scratch(void **out)
+{
+    int dev = 0;
+    LTDI_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return LTDI_EUNSUPPORTED;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        DeviceState *ds = nullptr;   /* the library's one-time set-up of the device (constant tables, side stream) */
+        const int rc = device_state(&ds);
+        if (rc) return rc;
+        void *p = nullptr;
+        LTDI_CUDA_OK(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || (uintptr_t)p % 256) return LTDI_ECUDA;
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return LTDI_OK;
+}
+
+extern "C" int ltdi_response_static(int which, const ltdi_orbits *orb, const double *d_hp, const double *d_hc, int64_t ld,
+                                    int64_t batch, const ltdi_source *h_src, int gen, int lagrange_order, int fd_order,
+                                    const ltdi_hybrid *h_hyb, int64_t n_hyb, double *d_A, double *d_E, double *d_T,
+                                    void *stream)
+{
+    if (which < LTDI_RESPONSE_FULL || which > LTDI_RESPONSE_HYBRID || !orb || batch < 1) return LTDI_EINVAL;
+    size_t need = 0;
+    const int rc = ltdi_workspace_bytes(which, orb->desc.n, batch, gen, lagrange_order, &need);
+    if (rc) return rc;
+    if (need > LTDI_STATIC_SCRATCH_BYTES) {
+        if (getenv("LTDI_DEBUG"))
+            fprintf(stderr, "lisatdi: ltdi_response_static needs %zu bytes of scratch, the static array holds %zu\n", need,
+                    (size_t)LTDI_STATIC_SCRATCH_BYTES);
+        return LTDI_EWORKSPACE;
+    }
+    void *d_work = nullptr;
+    const int src = static_scratch(&d_work);
+    if (src) return src;
+    return run_response(which, orb, d_hp, d_hc, ld, batch, h_src, gen, lagrange_order, fd_order, h_hyb, n_hyb, d_A, d_E, d_T,
+                        nullptr, nullptr, d_work, LTDI_STATIC_SCRATCH_BYTES, stream);
+}
