@@ -216,10 +216,6 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
         sb_l[i] = sinl(beta); cb_l[i] = cosl(beta);
         p.sb[i] = split(sb_l[i]); p.cb[i] = split(cb_l[i]);
     }
-    for (int l = 0; l < 3; ++l) {
-        const int s = link_sender(l), r = link_receiver(l);
-        p.dsb[l] = split(sb_l[r] - sb_l[s]); p.dcb[l] = split(cb_l[r] - cb_l[s]);
-    }
     {
         const long double L = desc->arm_m, R = desc->R_m;
         const long double e = L / (2.0L * sqrtl(3.0L) * R);
@@ -227,6 +223,13 @@ int orbits_common(const ltdi_orbit_desc *desc, const double *d_R, const double *
         p.s3_eR = split(sqrtl(3.0L) * e * R);
         p.inv_c = split(1.0L / (long double)LTDI_C_LIGHT);
         p.L_static = split(L / (long double)LTDI_C_LIGHT);
+        for (int l = 0; l < 3; ++l) {   /* unit vectors of the rigid triangle: coefficients with 1 / L folded in */
+            const int s = link_sender(l), r = link_receiver(l);
+            const long double dc = cb_l[r] - cb_l[s], dsn = sb_l[r] - sb_l[s];
+            p.PA[l] = split(0.5L * e * R * dc / L); p.PB[l] = split(0.5L * e * R * dsn / L);
+            p.PA3[l] = split(1.5L * e * R * dc / L); p.PB3[l] = split(1.5L * e * R * dsn / L);
+            p.PC[l] = split(sqrtl(3.0L) * e * R * dc / L); p.PD[l] = split(sqrtl(3.0L) * e * R * dsn / L);
+        }
         long double f = 1.0L;   /* (-1)^m / (2m+1)! and (-1)^m / (2m)! */
         for (int m = 0; m < 12; ++m) {
             if (m > 0) f *= (long double)(2 * m - 1) * (long double)(2 * m);

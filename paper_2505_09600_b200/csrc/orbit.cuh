@@ -13,8 +13,8 @@
 // in dd: t_n = t0 + n dt rounded to fp64 alone would move n_l by 7e-16 at t = 1 yr).  The positions themselves enter
 // the response only through k.R / c (needed to 1e-13 s): they are stored as correctly rounded doubles.
 //
-// Cost: about 1.2 kflop per sample (dd sincos 0.3, rotations 0.3, three links 0.6) for 252 B written: the kernel
-// is bound by the FP64 pipe, not by HBM, and runs once per time grid.
+// Cost: the kernel is bound by the FP64 pipe, not by HBM (252 B written per sample), and runs once per time grid; the
+// analytic modes form the unit vectors of the rigid triangle directly (no norm, no division).
 #pragma once
 #include "common.cuh"
 #include "dd.cuh"
@@ -25,10 +25,13 @@ struct OrbitKernelParams {
     double arm_m, R_m, omega, alpha0;
     dd omega_dd;           /* 2 pi / period */
     dd sb[3], cb[3];       /* sin, cos of beta_i = 2 pi i / 3 + rot0 */
-    dd dsb[3], dcb[3];     /* link l (s -> r): sin beta_r - sin beta_s, cos beta_r - cos beta_s */
     dd half_eR, s3_eR;     /* e R / 2 and sqrt(3) e R [m], e = L / (2 sqrt(3) R) */
     dd inv_c;              /* 1 / c */
     dd L_static;           /* arm / c */
+    /* analytic orbits: coefficients of the unit vector of link l in (cos 2 alpha, sin 2 alpha, cos alpha, sin alpha):
+     * PA = (e R / 2)(cos beta_r - cos beta_s) / L, PB = the same with sin, PA3 = 3 PA, PB3 = 3 PB, PC = sqrt(3) e R (cos beta_r -
+     * cos beta_s) / L, PD with sin */
+    dd PA[3], PB[3], PA3[3], PB3[3], PC[3], PD[3];
     dd sin_c[11], cos_c[12]; /* (-1)^m / (2m+1)!, (-1)^m / (2m)! */
     int mode;
     const double *R_in; /* tables mode: [3][3][n]; knots mode: [3][3][nk] */
@@ -104,7 +107,7 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
     const int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= p.n) return;
     double R[3][3], V[3][3];
-    dd dv[3][3];   /* arm vectors R_r - R_s of links +1, +2, +3 [m] */
+    dd dv[3][3];   /* arm vectors R_r - R_s of links +1, +2, +3 [m] (tables, orbit files), or the unit vectors themselves (analytic orbits) */
     if (!KNOTS && p.mode == LTDI_ORBIT_TABLES) {
 #pragma unroll
         for (int i = 0; i < 9; ++i) {
@@ -173,32 +176,35 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
         dd s2a = dd_mul(sa, ca);
         s2a.hi *= 2.0; s2a.lo *= 2.0;
         const dd c2a = dd_mul(dd_sub(ca, sa), dd_add(ca, sa));
-        dd c2[3], s2[3], c1[3];
+        const dd Rc = dd_mul_d(ca, p.R_m), Rs = dd_mul_d(sa, p.R_m);
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            /* 2 alpha - beta_i and alpha - beta_i by the addition theorems */
-            c2[i] = dd_add(dd_mul(c2a, p.cb[i]), dd_mul(s2a, p.sb[i]));
-            s2[i] = dd_sub(dd_mul(s2a, p.cb[i]), dd_mul(c2a, p.sb[i]));
-            c1[i] = dd_add(dd_mul(ca, p.cb[i]), dd_mul(sa, p.sb[i]));
-            const double s1 = sa.hi * p.cb[i].hi - ca.hi * p.sb[i].hi;
+            /* 2 alpha - beta_i and alpha - beta_i by the addition theorems.  The positions enter the response through k.R / c
+             * only and are stored as doubles: the O(e R) terms in plain fp64 (1e-7 m), the R cos(alpha) term in dd */
+            const double c2 = fma(c2a.hi, p.cb[i].hi, s2a.hi * p.sb[i].hi), s2 = fma(s2a.hi, p.cb[i].hi, -c2a.hi * p.sb[i].hi);
+            const double c1 = fma(ca.hi, p.cb[i].hi, sa.hi * p.sb[i].hi), s1 = fma(sa.hi, p.cb[i].hi, -ca.hi * p.sb[i].hi);
             const double eR = 2.0 * p.half_eR.hi;
-            R[i][0] = dd_to_double(dd_add_d(dd_mul_d(ca, p.R_m), p.half_eR.hi * (c2[i].hi - 3.0 * p.cb[i].hi)));
-            R[i][1] = dd_to_double(dd_add_d(dd_mul_d(sa, p.R_m), p.half_eR.hi * (s2[i].hi - 3.0 * p.sb[i].hi)));
-            R[i][2] = -p.s3_eR.hi * c1[i].hi;
-            V[i][0] = -p.R_m * p.omega * sa.hi - eR * p.omega * s2[i].hi;
-            V[i][1] = p.R_m * p.omega * ca.hi + eR * p.omega * c2[i].hi;
+            R[i][0] = dd_to_double(dd_add_d(Rc, p.half_eR.hi * (c2 - 3.0 * p.cb[i].hi)));
+            R[i][1] = dd_to_double(dd_add_d(Rs, p.half_eR.hi * (s2 - 3.0 * p.sb[i].hi)));
+            R[i][2] = -p.s3_eR.hi * c1;
+            V[i][0] = -p.R_m * p.omega * sa.hi - eR * p.omega * s2;
+            V[i][1] = p.R_m * p.omega * ca.hi + eR * p.omega * c2;
             V[i][2] = p.s3_eR.hi * p.omega * s1;
         }
+        /* The unit vectors directly.  In R_r - R_s the R cos(alpha), R sin(alpha) terms cancel identically and what is left
+         * is linear in the DIFFERENCES cos beta_r - cos beta_s, sin beta_r - sin beta_s (host constants: no cancellation
+         * between the two spacecraft on the device):
+         *   d_x = (e R / 2) [cos 2a dcb + sin 2a dsb - 3 dcb],  d_y = (e R / 2) [sin 2a dcb - cos 2a dsb - 3 dsb],
+         *   d_z = -sqrt(3) e R [cos a dcb + sin a dsb].
+         * The first-order Keplerian constellation is a rigid triangle: with w = e^{-i beta_r} - e^{-i beta_s}, |w|^2 = 3,
+         *   |d|^2 = (e R)^2 / 4 [30 - 6 Re(e^{2 i a} w^2)] + 3 (e R)^2 / 2 [3 + Re(e^{2 i a} w^2)] = 12 (e R)^2 = L^2
+         * at every time, so n_l = d / L with 1 / L folded into the coefficients: neither the norm nor its reciprocal (a dd
+         * square root and a dd division per link and sample) is needed; tables and orbit files need both. */
 #pragma unroll
         for (int l = 0; l < 3; ++l) {
-            const int s = link_sender(l), r = link_receiver(l);
-            /* R_r - R_s: the R cos(alpha), R sin(alpha) terms cancel identically */
-            dd three_c = p.dcb[l], three_s = p.dsb[l];
-            three_c = dd_mul_d(three_c, 3.0);
-            three_s = dd_mul_d(three_s, 3.0);
-            dv[l][0] = dd_mul(p.half_eR, dd_sub(dd_sub(c2[r], c2[s]), three_c));
-            dv[l][1] = dd_mul(p.half_eR, dd_sub(dd_sub(s2[r], s2[s]), three_s));
-            dv[l][2] = dd_neg(dd_mul(p.s3_eR, dd_sub(c1[r], c1[s])));
+            dv[l][0] = dd_sub(dd_add(dd_mul(c2a, p.PA[l]), dd_mul(s2a, p.PB[l])), p.PA3[l]);
+            dv[l][1] = dd_sub(dd_sub(dd_mul(s2a, p.PA[l]), dd_mul(c2a, p.PB[l])), p.PB3[l]);
+            dv[l][2] = dd_neg(dd_add(dd_mul(ca, p.PC[l]), dd_mul(sa, p.PD[l])));
         }
     }
     double *out = p.tab + n;
@@ -208,13 +214,17 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
 #pragma unroll
     for (int l = 0; l < 3; ++l) {
         const int s = link_sender(l), r = link_receiver(l);
-        const dd len2 = dd_add(dd_add(dd_mul(dv[l][0], dv[l][0]), dd_mul(dv[l][1], dv[l][1])), dd_mul(dv[l][2], dv[l][2]));
-        const dd len = dd_sqrt(len2);
-        const dd inv = dd_div(dd_make(1.0, 0.0), len);
+        const bool analytic = !KNOTS && p.mode != LTDI_ORBIT_TABLES;   /* dv holds the unit vector already */
+        dd len = p.L_static, inv = dd_make(1.0, 0.0);                   /* analytic: len is not used */
+        if (!analytic) {
+            const dd len2 = dd_add(dd_add(dd_mul(dv[l][0], dv[l][0]), dd_mul(dv[l][1], dv[l][1])), dd_mul(dv[l][2], dv[l][2]));
+            len = dd_sqrt(len2);
+            inv = dd_div(dd_make(1.0, 0.0), len);
+        }
         dd nh[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            nh[a] = dd_mul(dv[l][a], inv);
+            nh[a] = analytic ? dv[l][a] : dd_mul(dv[l][a], inv);
             out[(int64_t)(ROW_N + 3 * l + a) * p.stride] = nh[a].hi;
             lo[(int64_t)(LO_N + 3 * l + a) * p.stride] = (float)nh[a].lo;
         }
@@ -225,7 +235,7 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
             // first-order light time |d|/c (1 + n.V_sender / c): L_l != L_-l (Eq. B22)
             const double nvs = nh[0].hi * V[s][0] + nh[1].hi * V[s][1] + nh[2].hi * V[s][2];
             const double nvr = -(nh[0].hi * V[r][0] + nh[1].hi * V[r][1] + nh[2].hi * V[r][2]);
-            const dd lc = dd_mul(len, p.inv_c);
+            const dd lc = (!KNOTS && p.mode == LTDI_ORBIT_KEPLERIAN) ? p.L_static : dd_mul(len, p.inv_c);
             Lp = dd_mul(lc, two_sum(1.0, nvs * p.inv_c.hi));
             Lm = dd_mul(lc, two_sum(1.0, nvr * p.inv_c.hi));
         } else {
