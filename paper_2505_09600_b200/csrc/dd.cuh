@@ -51,6 +51,15 @@ __device__ __forceinline__ dd dd_add(dd a, dd b)
     return fast_two_sum(s.hi, s.lo);
 }
 __device__ __forceinline__ dd dd_sub(dd a, dd b) { return dd_add(a, dd_neg(b)); }
+// a + b with an error of 2^-104 (|a| + |b|) instead of 2^-104 |a + b|: 11 additions instead of 20.  For sums whose terms
+// do not cancel (Horner steps, combinations of O(1) terms with an O(1) result).
+__device__ __forceinline__ dd dd_add_fast(dd a, dd b)
+{
+    dd s = two_sum(a.hi, b.hi);
+    s.lo = __dadd_rn(s.lo, __dadd_rn(a.lo, b.lo));
+    return fast_two_sum(s.hi, s.lo);
+}
+__device__ __forceinline__ dd dd_sub_fast(dd a, dd b) { return dd_add_fast(a, dd_neg(b)); }
 __device__ __forceinline__ dd dd_add_d(dd a, double b)
 {
     dd s = two_sum(a.hi, b);

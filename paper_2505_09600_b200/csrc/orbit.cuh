@@ -87,8 +87,8 @@ __device__ __forceinline__ void sincos_dd(dd a, const OrbitKernelParams &p, dd &
     dd ps = dd_make(ts, 0.0), pc = dd_make(tc, 0.0);
 #pragma unroll
     for (int m = 5; m >= 0; --m) {
-        ps = dd_add(dd_mul(ps, r2), p.sin_c[m]);
-        pc = dd_add(dd_mul(pc, r2), p.cos_c[m]);
+        ps = dd_add_fast(dd_mul(ps, r2), p.sin_c[m]);   /* Horner steps: no cancellation */
+        pc = dd_add_fast(dd_mul(pc, r2), p.cos_c[m]);
     }
     ps = dd_mul(ps, r);
     const int q = ((int)k) & 3;
@@ -202,9 +202,10 @@ __global__ void __launch_bounds__(128) orbit_delay_kernel(const __grid_constant_
          * square root and a dd division per link and sample) is needed; tables and orbit files need both. */
 #pragma unroll
         for (int l = 0; l < 3; ++l) {
-            dv[l][0] = dd_sub(dd_add(dd_mul(c2a, p.PA[l]), dd_mul(s2a, p.PB[l])), p.PA3[l]);
-            dv[l][1] = dd_sub(dd_sub(dd_mul(s2a, p.PA[l]), dd_mul(c2a, p.PB[l])), p.PB3[l]);
-            dv[l][2] = dd_neg(dd_add(dd_mul(ca, p.PC[l]), dd_mul(sa, p.PD[l])));
+            /* sums of O(1) terms with an O(1) result, stored to 2^-77 (double + float): the 11-addition sum serves */
+            dv[l][0] = dd_sub_fast(dd_add_fast(dd_mul(c2a, p.PA[l]), dd_mul(s2a, p.PB[l])), p.PA3[l]);
+            dv[l][1] = dd_sub_fast(dd_sub_fast(dd_mul(s2a, p.PA[l]), dd_mul(c2a, p.PB[l])), p.PB3[l]);
+            dv[l][2] = dd_neg(dd_add_fast(dd_mul(ca, p.PC[l]), dd_mul(sa, p.PD[l])));
         }
     }
     double *out = p.tab + n;
