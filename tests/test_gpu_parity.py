@@ -604,3 +604,30 @@ def test_one_series_split_in_time(ltdi, which):
         scale = max(np.linalg.norm(whole[c]) for c in "AET")
         for c in "AET":
             assert np.linalg.norm(got[c] - whole[c][0]) <= 1e-13 * scale, (which, c)
+
+
+def test_second_device_gives_the_same_bits(ltdi):
+    """the library's per-device state (constant tables, shared-memory attributes, side streams, the static scratch of
+    ltdi_response_static) is set up for every device it is used on: the responses on cuda:1, called after cuda:0, are bitwise
+    those of cuda:0.  Needs two visible devices (skipped on the one-GPU boxes of this pool)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    cfg = W.config(2, n=20011, batch=2)
+    hp, hc, ang, metas = W.sources(cfg, [0, 1])
+    results = []
+    for index in (0, 1):
+        dev = torch.device("cuda", index)
+        hyb = hybrid_params(metas, ltdi.hyb_time, W.TAPER_COSINE, cfg["dt"])
+        orb = ltdi.Orbits(cfg["orbit"], device=dev)
+        dhp, dhc = torch.from_numpy(hp).to(dev), torch.from_numpy(hc).to(dev)
+        out = []
+        with torch.cuda.device(dev):
+            out.append(to_numpy(ltdi.response_full(orb, dhp, dhc, ang, 20, 31)))
+            out.append(to_numpy(ltdi.response_hybrid(orb, dhp, dhc, ang, 20, 31, 2, hyb)))
+            out.append(to_numpy(ltdi.response_lfa(orb, dhp, dhc, ang, 20, 5, 2)))          # generic kernel: constant tables
+            out.append(to_numpy(ltdi.response_static(ltdi.RESPONSE_LFA, orb, dhp, dhc, ang, 20, 31, 2)))
+            torch.cuda.synchronize(dev)
+        results.append(out)
+    for a, b in zip(*results):
+        for c in "AET":
+            assert np.array_equal(a[c], b[c]), c
