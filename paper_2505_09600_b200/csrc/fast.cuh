@@ -1248,8 +1248,9 @@ tdi_kernel(const __grid_constant__ FastParams p)
                     }
                 } else {
 #pragma unroll
-                    for (int r = 0; r < FAST_TC_R; ++r)
-                        D[r] = fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
+                    for (int r = 0; r < FAST_TC_R; ++r)   /* the LFA delays have no L_-p2, L_-p3 part (cP = c3 = 0: the same bits) */
+                        D[r] = (WHICH == LTDI_RESPONSE_LFA ? fma(-cU, LU[r], fma(-c2, L2p[r], dc))
+                                                           : fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc))))) * p.inv_dt;
                 }
                 Dt = D[FAST_TC_R / 2];
             }
@@ -1258,13 +1259,20 @@ tdi_kernel(const __grid_constant__ FastParams p)
 #pragma unroll
             for (int r = 0; r < FAST_TC_R; ++r) {
                 const double Dr = ORD2 ? D[r] - Dt
-                                       : fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc)))) * p.inv_dt;
+                                  : (WHICH == LTDI_RESPONSE_LFA ? fma(-cU, LU[r], fma(-c2, L2p[r], dc))
+                                                                : fma(-c3, L3m[r], fma(-cU, LU[r], fma(-c2, L2p[r], fma(-cP, LP[r], dc))))) * p.inv_dt;
                 const double v = fma(Dr, s1[r], s0[r]);
                 if (!lt) Xf[r] = fma(sgn, v, Xf[r]);
                 else {
                     const double L2 = L2p[r], L3 = LU[r];
                     const double pre = p.gen == LTDI_GEN_15 ? 4.0 : 8.0 * (L2 + L3);   /* (B25) / (B33) */
-                    Xl[r] = fma(tm == 14 ? pre * L3 : -(pre * L2), v, Xl[r]);
+                    if (WHICH == LTDI_RESPONSE_LFA) {
+                        /* the LFA instance keeps the running sum in its slot of the exchange region (the thread's own until
+                         * the barrier): in registers it was spilled across term7 under the 80-register cap of four CTAs per SM */
+                        double *xo = Xs + ch * FAST_TC + r0 + r;
+                        *xo = tm == 14 ? (pre * L3) * v : fma(-(pre * L2), v, *xo);
+                    } else
+                        Xl[r] = fma(tm == 14 ? pre * L3 : -(pre * L2), v, Xl[r]);
                 }
             }
         }
@@ -1314,8 +1322,9 @@ tdi_kernel(const __grid_constant__ FastParams p)
     /* exchange through shared memory: rows 0..2 = X, Y, Z (hybrid: of the full response, rows 3..5 = of the LFA) */
 #pragma unroll
     for (int r = 0; r < FAST_TC_R; ++r) {
-        if (WHICH == LTDI_RESPONSE_LFA) Xs[ch * FAST_TC + r0 + r] = Xl[r];
-        else Xs[ch * FAST_TC + r0 + r] = Xf[r];
+        if (WHICH == LTDI_RESPONSE_LFA) {
+            if (!ok) Xs[ch * FAST_TC + r0 + r] = Xl[r];   /* fast path: already there */
+        } else Xs[ch * FAST_TC + r0 + r] = Xf[r];
         if (WHICH == LTDI_RESPONSE_HYBRID) Xs[(3 + ch) * FAST_TC + r0 + r] = Xl[r];
     }
     __syncthreads();
